@@ -1,0 +1,11 @@
+"""Seeded synthetic input generators shared by the oracle tests and the CUDA path.
+
+This package holds NO arithmetic of the method under test (no pair force, no
+predictor): it only draws Plummer-sphere initial conditions and the derivative
+values the predictor will later consume.  See DESIGN.md "Input recipe".
+"""
+from .plummer import (CONFIGS, Workload, make_workload, make_config, lattice_workload,
+                      splitmix64_uniform, A_PLUMMER)
+
+__all__ = ["CONFIGS", "Workload", "make_workload", "make_config", "lattice_workload",
+           "splitmix64_uniform", "A_PLUMMER"]
