@@ -1,0 +1,349 @@
+"""ctypes binding of libs2b200.so -- same names as include/s2b200.h, argument marshalling only.
+
+Host arrays are numpy (fp64 / int32, C-contiguous); device arrays are torch CUDA tensors
+(passed as raw pointers).  PyTorch supplies device memory (its caching allocator, through the
+s2_allocator callbacks) and the stream (torch.cuda.current_stream()); every step of the hot
+path runs in the library's CUDA kernels.  There is no CPU fallback: if the library cannot be
+loaded, or no CUDA device is present, the calls raise.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+import re
+
+import numpy as np
+
+_PKG = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_PKG, "libs2b200.so")
+HEADER_PATH = os.path.join(os.path.dirname(_PKG), "include", "s2b200.h")
+
+S2_FP64, S2_DS, S2_FP32 = 0, 1, 2
+S2_WANT_NN, S2_WANT_NGB = 1, 2
+S2_OK, S2_EINVAL, S2_ERANGE, S2_ENOMEM, S2_ECUDA, S2_ESTATE, S2_EOVERFLOW = 0, -1, -2, -3, -4, -5, -6
+
+_ALLOC_FN = C.CFUNCTYPE(C.c_void_p, C.c_size_t, C.c_void_p)
+_FREE_FN = C.CFUNCTYPE(None, C.c_void_p, C.c_void_p)
+
+
+class s2_allocator(C.Structure):
+    _fields_ = [("alloc", _ALLOC_FN), ("free", _FREE_FN), ("user", C.c_void_p)]
+
+
+class S2Error(RuntimeError):
+    def __init__(self, code: int, where: str, detail: str = ""):
+        self.code = code
+        super().__init__(f"{where}: {s2_strerror(code)} ({code}){' -- ' + detail if detail else ''}")
+
+
+_lib = None
+
+
+def header_symbols() -> list[str]:
+    """Every function include/s2b200.h declares."""
+    src = open(HEADER_PATH).read()
+    src = re.sub(r"/\*.*?\*/", "", src, flags=re.S)
+    return sorted(set(re.findall(r"\b(s2_[a-z0-9_]+)\s*\(", src)))
+
+
+def lib() -> C.CDLL:
+    """Loads libs2b200.so (building it in-tree with nvcc if it is absent).  Raises if it cannot."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(LIB_PATH):
+        from .build import build
+        build()
+    L = C.CDLL(LIB_PATH)
+    vp, ip, dp = C.c_void_p, C.c_void_p, C.c_void_p
+    sig = {
+        "s2_open": (C.c_int, [C.POINTER(vp), C.c_int, C.c_int, C.c_int, C.c_int, C.c_int, C.POINTER(s2_allocator), vp]),
+        "s2_close": (C.c_int, [vp]),
+        "s2_set_stream": (C.c_int, [vp, vp]),
+        "s2_synchronize": (C.c_int, [vp]),
+        "s2_set_j": (C.c_int, [vp, C.c_int, ip, ip] + [dp] * 8),
+        "s2_commit_j": (C.c_int, [vp]),
+        "s2_commit_j_device": (C.c_int, [vp, C.c_int, ip, ip] + [dp] * 8),
+        "s2_predict": (C.c_int, [vp, C.c_double, C.c_int]),
+        "s2_calc_ilist": (C.c_int, [vp, C.c_int, ip, dp, C.c_double, C.c_uint]),
+        "s2_calc_ilist_device": (C.c_int, [vp, C.c_int, ip, dp, C.c_double, C.c_uint]),
+        "s2_calc_explicit": (C.c_int, [vp, C.c_int, ip, dp, dp, dp, dp, C.c_double, C.c_uint]),
+        "s2_get_results": (C.c_int, [vp, C.c_int, dp, dp, dp, dp, ip, dp, ip]),
+        "s2_get_neighbours": (C.c_int, [vp, C.c_int, C.c_int, C.POINTER(C.c_int), ip]),
+        "s2_get_neighbours_csr": (C.c_int, [vp, C.c_int, vp, ip, C.c_longlong]),
+        "s2_get_predicted_j": (C.c_int, [vp, C.c_int, C.c_int, dp, dp, dp]),
+        "s2_get_j": (C.c_int, [vp, C.c_int, C.c_int, ip, dp, dp, dp]),
+        "s2_set_tuning": (C.c_int, [vp, C.c_int, C.c_int]),
+        "s2_last_launch_info": (C.c_int, [vp, C.POINTER(C.c_int * 8)]),
+        "s2_kernel_launches": (C.c_longlong, [vp]),
+        "s2_enable_timing": (C.c_int, [vp, C.c_int]),
+        "s2_get_timing": (C.c_int, [vp, C.POINTER(C.c_float), C.POINTER(C.c_float), C.POINTER(C.c_float)]),
+        "s2_peak_fma": (C.c_int, [vp, C.c_int, C.c_int, C.POINTER(C.c_double)]),
+        "s2_strerror": (C.c_char_p, [C.c_int]),
+        "s2_last_cuda_error": (C.c_char_p, [vp]),
+        "s2_version": (C.c_char_p, []),
+    }
+    for name, (res, args) in sig.items():
+        fn = getattr(L, name)
+        fn.restype, fn.argtypes = res, args
+    _lib = L
+    return L
+
+
+# ---- marshalling helpers ------------------------------------------------------------------
+
+def _h(a, dtype, shape_tail=None, n=None, name="array"):
+    """host numpy array -> pointer (None passes NULL)."""
+    if a is None:
+        return None, None
+    a = np.ascontiguousarray(a, dtype=dtype)
+    if n is not None:
+        want = (n,) + (shape_tail or ())
+        if a.shape != want:
+            raise ValueError(f"{name}: expected shape {want}, got {a.shape}")
+    return a.ctypes.data_as(C.c_void_p), a
+
+
+def _d(t, dtype_name, numel=None, name="tensor"):
+    """torch CUDA tensor -> raw device pointer (None passes NULL)."""
+    if t is None:
+        return None
+    import torch
+    if not (isinstance(t, torch.Tensor) and t.is_cuda and t.is_contiguous()):
+        raise ValueError(f"{name}: need a contiguous CUDA tensor")
+    if str(t.dtype) != "torch." + dtype_name:
+        raise ValueError(f"{name}: need dtype {dtype_name}, got {t.dtype}")
+    if numel is not None and t.numel() != numel:
+        raise ValueError(f"{name}: expected {numel} elements, got {t.numel()}")
+    return C.c_void_p(t.data_ptr())
+
+
+def _check(rc: int, where: str, ctx=None, ok=(S2_OK,)):
+    if rc in ok:
+        return rc
+    detail = ""
+    if rc == S2_ECUDA and ctx is not None:
+        detail = (lib().s2_last_cuda_error(ctx) or b"").decode()
+    raise S2Error(rc, where, detail)
+
+
+class _TorchAllocator:
+    """s2_allocator backed by torch's CUDA caching allocator (uint8 tensors kept alive by pointer)."""
+
+    def __init__(self, device: int):
+        import torch
+        self._torch = torch
+        self._device = torch.device("cuda", device)
+        self._live: dict[int, object] = {}
+        self._alloc_cb = _ALLOC_FN(self._alloc)
+        self._free_cb = _FREE_FN(self._free)
+        self.struct = s2_allocator(self._alloc_cb, self._free_cb, None)
+        self.bytes_live = 0
+
+    def _alloc(self, nbytes, _user):
+        try:
+            t = self._torch.empty(int(nbytes), dtype=self._torch.uint8, device=self._device)
+        except Exception:
+            return None
+        self._live[t.data_ptr()] = t
+        self.bytes_live += int(nbytes)
+        return t.data_ptr()
+
+    def _free(self, ptr, _user):
+        t = self._live.pop(ptr, None)
+        if t is not None:
+            self.bytes_live -= t.numel()
+
+
+# ---- the calls, one per header entry --------------------------------------------------------
+
+class s2_ctx:
+    """Opaque context handle plus the Python objects that must outlive it."""
+
+    def __init__(self, handle, allocator, order, precision, device):
+        self.handle, self.allocator = handle, allocator
+        self.order, self.precision, self.device = order, precision, device
+        self._keep = []          # device tensors referenced by the last ASYNC call
+
+
+def s2_version() -> str:
+    return lib().s2_version().decode()
+
+
+def s2_strerror(code: int) -> str:
+    return lib().s2_strerror(int(code)).decode()
+
+
+def s2_open(device: int = 0, order: int = 4, precision: int = S2_FP64, nj_capacity: int = 1, ngb_cap: int = 256,
+            use_torch_allocator: bool = True, stream=None) -> s2_ctx:
+    L = lib()
+    import torch
+    if not torch.cuda.is_available():
+        raise S2Error(S2_ECUDA, "s2_open", "no CUDA device visible; this library has no CPU fallback")
+    alloc = _TorchAllocator(device) if use_torch_allocator else None
+    if stream is None:
+        stream = torch.cuda.current_stream(device).cuda_stream
+    h = C.c_void_p()
+    rc = L.s2_open(C.byref(h), device, order, precision, nj_capacity, ngb_cap,
+                   C.byref(alloc.struct) if alloc else None, C.c_void_p(stream))
+    _check(rc, "s2_open")
+    return s2_ctx(h, alloc, order, precision, device)
+
+
+def s2_close(ctx: s2_ctx):
+    if ctx.handle:
+        _check(lib().s2_close(ctx.handle), "s2_close")
+        ctx.handle = None
+        ctx._keep = []
+
+
+def s2_set_stream(ctx, stream):
+    _check(lib().s2_set_stream(ctx.handle, C.c_void_p(stream)), "s2_set_stream", ctx.handle)
+
+
+def s2_synchronize(ctx):
+    _check(lib().s2_synchronize(ctx.handle), "s2_synchronize", ctx.handle)
+    ctx._keep = []
+
+
+def s2_set_j(ctx, address, ident, t, mass, pos, vel, acc, jerk, snap=None, crackle=None):
+    n = int(np.asarray(address).shape[0])
+    i32, f64 = np.int32, np.float64
+    keep = []
+    args = []
+    for a, dt, tail, nm in ((address, i32, (), "address"), (ident, i32, (), "id"), (t, f64, (), "t"), (mass, f64, (), "mass"),
+                            (pos, f64, (3,), "pos"), (vel, f64, (3,), "vel"), (acc, f64, (3,), "acc"),
+                            (jerk, f64, (3,), "jerk"), (snap, f64, (3,), "snap"), (crackle, f64, (3,), "crackle")):
+        p, arr = _h(a, dt, tail, n, nm)
+        args.append(p)
+        keep.append(arr)
+    _check(lib().s2_set_j(ctx.handle, n, *args), "s2_set_j", ctx.handle)
+
+
+def s2_commit_j(ctx):
+    _check(lib().s2_commit_j(ctx.handle), "s2_commit_j", ctx.handle)
+
+
+def s2_commit_j_device(ctx, d_address, d_id, d_t, d_mass, d_pos, d_vel, d_acc, d_jerk, d_snap=None, d_crackle=None):
+    n = d_address.numel()
+    args = [_d(d_address, "int32", n, "address"), _d(d_id, "int32", n, "id"), _d(d_t, "float64", n, "t"),
+            _d(d_mass, "float64", n, "mass")]
+    for tns, nm in ((d_pos, "pos"), (d_vel, "vel"), (d_acc, "acc"), (d_jerk, "jerk"), (d_snap, "snap"), (d_crackle, "crackle")):
+        args.append(_d(tns, "float64", 3 * n, nm))
+    ctx._keep = [d_address, d_id, d_t, d_mass, d_pos, d_vel, d_acc, d_jerk, d_snap, d_crackle]
+    _check(lib().s2_commit_j_device(ctx.handle, n, *args), "s2_commit_j_device", ctx.handle)
+
+
+def s2_predict(ctx, t: float, nj: int):
+    _check(lib().s2_predict(ctx.handle, float(t), int(nj)), "s2_predict", ctx.handle)
+
+
+def s2_calc_ilist(ctx, i_address, h2=None, eps2: float = 0.0, flags: int = 0):
+    ni = int(np.asarray(i_address).shape[0])
+    pa, ka = _h(i_address, np.int32, (), ni, "i_address")
+    ph, kh = _h(h2, np.float64, (), ni, "h2")
+    _check(lib().s2_calc_ilist(ctx.handle, ni, pa, ph, float(eps2), int(flags)), "s2_calc_ilist", ctx.handle)
+
+
+def s2_calc_ilist_device(ctx, d_i_address, d_h2=None, eps2: float = 0.0, flags: int = 0):
+    ni = d_i_address.numel()
+    ctx._keep = [d_i_address, d_h2]
+    _check(lib().s2_calc_ilist_device(ctx.handle, ni, _d(d_i_address, "int32", ni, "i_address"),
+                                      _d(d_h2, "float64", ni, "h2"), float(eps2), int(flags)),
+           "s2_calc_ilist_device", ctx.handle)
+
+
+def s2_calc_explicit(ctx, ident, pos, vel, acc=None, h2=None, eps2: float = 0.0, flags: int = 0):
+    ni = int(np.asarray(ident).shape[0])
+    f64 = np.float64
+    pi, k0 = _h(ident, np.int32, (), ni, "id")
+    pp, k1 = _h(pos, f64, (3,), ni, "pos")
+    pv, k2 = _h(vel, f64, (3,), ni, "vel")
+    pa, k3 = _h(acc, f64, (3,), ni, "acc")
+    ph, k4 = _h(h2, f64, (), ni, "h2")
+    _check(lib().s2_calc_explicit(ctx.handle, ni, pi, pp, pv, pa, ph, float(eps2), int(flags)),
+           "s2_calc_explicit", ctx.handle)
+
+
+def s2_get_results(ctx, ni: int, allow_overflow: bool = True) -> dict:
+    """Returns dict(acc, jerk, snap, pot, nn_id, nn_r2, ngb_count, overflow)."""
+    out = dict(acc=np.empty((ni, 3)), jerk=np.empty((ni, 3)), snap=np.empty((ni, 3)) if ctx.order == 6 else None,
+               pot=np.empty(ni), nn_id=np.empty(ni, np.int32), nn_r2=np.empty(ni), ngb_count=np.empty(ni, np.int32))
+    p = lambda a: None if a is None else a.ctypes.data_as(C.c_void_p)
+    rc = lib().s2_get_results(ctx.handle, ni, p(out["acc"]), p(out["jerk"]), p(out["snap"]), p(out["pot"]),
+                              p(out["nn_id"]), p(out["nn_r2"]), p(out["ngb_count"]))
+    _check(rc, "s2_get_results", ctx.handle, ok=(S2_OK, S2_EOVERFLOW) if allow_overflow else (S2_OK,))
+    out["overflow"] = rc == S2_EOVERFLOW
+    ctx._keep = []
+    return out
+
+
+def s2_get_neighbours(ctx, i: int, cap: int) -> np.ndarray:
+    lst = np.empty(max(cap, 1), np.int32)
+    n = C.c_int(0)
+    rc = lib().s2_get_neighbours(ctx.handle, int(i), int(cap), C.byref(n), lst.ctypes.data_as(C.c_void_p))
+    _check(rc, "s2_get_neighbours", ctx.handle, ok=(S2_OK, S2_EOVERFLOW))
+    return lst[:n.value].copy()
+
+
+def s2_get_neighbours_csr(ctx, ni: int, list_cap: int | None = None):
+    off = np.zeros(ni + 1, np.int64)
+    if list_cap is None:   # first call sizes the list
+        rc = lib().s2_get_neighbours_csr(ctx.handle, ni, off.ctypes.data_as(C.c_void_p), None, 0)
+        if rc not in (S2_OK, S2_ERANGE, S2_EOVERFLOW):
+            _check(rc, "s2_get_neighbours_csr", ctx.handle)
+        list_cap = int(off[ni])
+    lst = np.empty(max(list_cap, 1), np.int32)
+    rc = lib().s2_get_neighbours_csr(ctx.handle, ni, off.ctypes.data_as(C.c_void_p), lst.ctypes.data_as(C.c_void_p), list_cap)
+    _check(rc, "s2_get_neighbours_csr", ctx.handle, ok=(S2_OK, S2_EOVERFLOW))
+    return off, lst[:off[ni]].copy()
+
+
+def s2_get_predicted_j(ctx, first: int, n: int):
+    pos, vel = np.empty((n, 3)), np.empty((n, 3))
+    acc = np.empty((n, 3)) if ctx.order == 6 else None
+    p = lambda a: None if a is None else a.ctypes.data_as(C.c_void_p)
+    _check(lib().s2_get_predicted_j(ctx.handle, first, n, p(pos), p(vel), p(acc)), "s2_get_predicted_j", ctx.handle)
+    return pos, vel, acc
+
+
+def s2_get_j(ctx, first: int, n: int):
+    ident, t, mass, pos = np.empty(n, np.int32), np.empty(n), np.empty(n), np.empty((n, 3))
+    p = lambda a: a.ctypes.data_as(C.c_void_p)
+    _check(lib().s2_get_j(ctx.handle, first, n, p(ident), p(t), p(mass), p(pos)), "s2_get_j", ctx.handle)
+    return ident, t, mass, pos
+
+
+def s2_set_tuning(ctx, key: int, value: int):
+    _check(lib().s2_set_tuning(ctx.handle, key, value), "s2_set_tuning", ctx.handle)
+
+
+def s2_last_launch_info(ctx) -> dict:
+    arr = (C.c_int * 8)()
+    _check(lib().s2_last_launch_info(ctx.handle, C.byref(arr)), "s2_last_launch_info", ctx.handle)
+    keys = ("S", "lanes_per_i", "warp_columns", "grid", "threads", "smem", "reduced", "ctas_per_sm")
+    return dict(zip(keys, list(arr)))
+
+
+def s2_kernel_launches(ctx) -> int:
+    return int(lib().s2_kernel_launches(ctx.handle))
+
+
+def s2_enable_timing(ctx, on: bool = True):
+    _check(lib().s2_enable_timing(ctx.handle, int(on)), "s2_enable_timing", ctx.handle)
+
+
+def s2_get_timing(ctx) -> dict:
+    a, b, c = C.c_float(), C.c_float(), C.c_float()
+    _check(lib().s2_get_timing(ctx.handle, C.byref(a), C.byref(b), C.byref(c)), "s2_get_timing", ctx.handle)
+    return dict(predict_ms=a.value, force_ms=b.value, reduce_ms=c.value)
+
+
+def s2_peak_fma(ctx, kind: int, iters: int = 2000) -> float:
+    v = C.c_double()
+    _check(lib().s2_peak_fma(ctx.handle, kind, iters, C.byref(v)), "s2_peak_fma", ctx.handle)
+    return v.value
+
+
+def s2_last_cuda_error(ctx) -> str:
+    return (lib().s2_last_cuda_error(ctx.handle) or b"").decode()

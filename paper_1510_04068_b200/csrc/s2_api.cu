@@ -1,0 +1,961 @@
+// s2_api.cu -- the C ABI of include/s2b200.h: context, device buffers, staging, the launch
+// balancer that picks (lanes per i, warp columns, j-slices), and result read-back.
+// Every arithmetic step of the hot path runs in the kernels; this file only moves bytes and
+// chooses launch shapes.
+#include <math.h>
+#include <stdio.h>
+#include <stdlib.h>
+#include <string.h>
+
+#include <algorithm>
+#include <map>
+#include <string>
+
+#include "s2_internal.h"
+
+namespace s2 {
+cudaError_t dispatch_force_fp64(int order, unsigned flags, int L, dim3 grid, size_t smem, const ForceArgs &a,
+                                cudaStream_t st, bool query, int *ctas_per_sm);
+cudaError_t dispatch_force_fp32(int order, unsigned flags, int L, dim3 grid, size_t smem, const ForceArgs &a,
+                                cudaStream_t st, bool query, int *ctas_per_sm);
+cudaError_t dispatch_force_ds(int order, unsigned flags, int L, dim3 grid, size_t smem, const ForceArgs &a,
+                              cudaStream_t st, bool query, int *ctas_per_sm);
+int force_nplanes(int precision, int order, unsigned flags);
+}  // namespace s2
+
+using namespace s2;
+
+struct Buf {
+    void *p = nullptr;
+    size_t bytes = 0;
+};
+
+struct Batch {
+    size_t offset;   // byte offset of the batch block in the staging buffer
+    int n;
+};
+
+struct s2_ctx {
+    int device = 0, order = 4, precision = S2_FP64, nj_cap = 0, ngb_cap = 0;
+    s2_allocator alloc{};
+    bool has_alloc = false;
+    cudaStream_t stream = nullptr;
+    int sm_count = 148;
+    std::string cuda_err;
+    long long launches = 0;
+
+    // device buffers
+    Buf base, planes, qplanes, stage_dev, iplanes, iqplanes, i_addr, i_h2, part, result, seg, list, flags;
+    // pinned host buffers
+    void *h_stage = nullptr;
+    size_t h_stage_bytes = 0, h_stage_used = 0;
+    void *h_io = nullptr;
+    size_t h_io_bytes = 0;
+    int *h_flags = nullptr;           // pinned, 4 ints
+    cudaEvent_t ev_stage = nullptr;   // H2D of the staging buffer finished
+    cudaEvent_t ev_io = nullptr;      // H2D of the i-list upload finished
+    std::vector<Batch> batches;
+
+    // state
+    bool have_j = false, predicted = false, calc_done = false, results_fetched = false;
+    int nj_pred = 0, ni_last = 0;
+    unsigned flags_last = 0;
+    double t_pred = 0.0;
+
+    // tuning overrides and last launch
+    int tune[5] = {0, 0, 0, 0, 0};
+    int last_info[8] = {0, 0, 0, 0, 0, 0, 0, 0};
+    std::map<long long, int> occ_cache;
+
+    // timing
+    bool timing = false;
+    cudaEvent_t ev_t[6] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};
+    bool ran_predict = false, ran_force = false, ran_reduce = false;
+};
+
+// ---- helpers ----------------------------------------------------------------------------
+
+static int fail_cuda(s2_ctx *c, cudaError_t e)
+{
+    if (c) c->cuda_err = cudaGetErrorString(e);
+    return S2_ECUDA;
+}
+#define CU(call)                                           \
+    do {                                                   \
+        cudaError_t e__ = (call);                          \
+        if (e__ != cudaSuccess) return fail_cuda(ctx, e__); \
+    } while (0)
+
+static int dev_reserve(s2_ctx *ctx, Buf &b, size_t bytes)
+{
+    if (bytes <= b.bytes) return S2_OK;
+    // grow-only; contents are not preserved (callers refill)
+    if (b.p) {
+        // the old block may still be in use by enqueued kernels: drain the stream first
+        CU(cudaStreamSynchronize(ctx->stream));
+        if (ctx->has_alloc)
+            ctx->alloc.free(b.p, ctx->alloc.user);
+        else
+            cudaFree(b.p);
+        b.p = nullptr;
+        b.bytes = 0;
+    }
+    size_t want = bytes + bytes / 4;   // 25 % head-room against repeated growth
+    want = (want + 255) & ~(size_t)255;
+    void *p = nullptr;
+    if (ctx->has_alloc) {
+        p = ctx->alloc.alloc(want, ctx->alloc.user);
+        if (!p) return S2_ENOMEM;
+    } else {
+        cudaError_t e = cudaMalloc(&p, want);
+        if (e == cudaErrorMemoryAllocation) {
+            cudaGetLastError();
+            return S2_ENOMEM;
+        }
+        if (e != cudaSuccess) return fail_cuda(ctx, e);
+    }
+    b.p = p;
+    b.bytes = want;
+    return S2_OK;
+}
+
+static void dev_release(s2_ctx *ctx, Buf &b)
+{
+    if (!b.p) return;
+    if (ctx->has_alloc)
+        ctx->alloc.free(b.p, ctx->alloc.user);
+    else
+        cudaFree(b.p);
+    b.p = nullptr;
+    b.bytes = 0;
+}
+
+static int pinned_reserve(s2_ctx *ctx, void **p, size_t *have, size_t used, size_t bytes)
+{
+    if (bytes <= *have) return S2_OK;
+    size_t want = std::max(bytes + bytes / 2, (size_t)1 << 16);
+    void *q = nullptr;
+    cudaError_t e = cudaHostAlloc(&q, want, cudaHostAllocDefault);
+    if (e == cudaErrorMemoryAllocation) {
+        cudaGetLastError();
+        return S2_ENOMEM;
+    }
+    if (e != cudaSuccess) return fail_cuda(ctx, e);
+    if (*p) {
+        if (used) memcpy(q, *p, used);
+        cudaFreeHost(*p);
+    }
+    *p = q;
+    *have = want;
+    return S2_OK;
+}
+
+static inline size_t align16(size_t x) { return (x + 15) & ~(size_t)15; }
+
+static inline double *base_field(const s2_ctx *c, int f) { return (double *)c->base.p + (size_t)f * c->nj_cap; }
+static inline int *base_id(const s2_ctx *c) { return (int *)((double *)c->base.p + (size_t)nfields(c->order) * c->nj_cap); }
+static inline double2 *plane(const s2_ctx *c, int p) { return (double2 *)c->planes.p + (size_t)p * c->nj_cap; }
+static inline float4 *qplane(const s2_ctx *c, int p) { return (float4 *)c->qplanes.p + (size_t)p * c->nj_cap; }
+static inline int n_qplanes(int precision, int order)
+{
+    if (precision == S2_FP32) return order == 6 ? 4 : 3;
+    if (precision == S2_DS) return order == 6 ? 6 : 4;
+    return 0;
+}
+
+// ---- life cycle ---------------------------------------------------------------------------
+
+extern "C" int s2_open(s2_ctx **out, int device, int order, int precision, int nj_capacity, int ngb_cap,
+                       const s2_allocator *a, void *cuda_stream)
+{
+    if (!out) return S2_EINVAL;
+    *out = nullptr;
+    if ((order != 4 && order != 6) || precision < S2_FP64 || precision > S2_FP32 || nj_capacity <= 0 || ngb_cap < 0)
+        return S2_EINVAL;
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || device < 0 || device >= ndev) {
+        cudaGetLastError();
+        return S2_ECUDA;   // no CPU fallback
+    }
+    if (cudaSetDevice(device) != cudaSuccess) return S2_ECUDA;
+    cudaDeviceProp prop;
+    if (cudaGetDeviceProperties(&prop, device) != cudaSuccess) return S2_ECUDA;
+    if (prop.major < 10) return S2_ECUDA;   // kernels are built for sm_100a only
+
+    s2_ctx *ctx = new s2_ctx();
+    ctx->device = device;
+    ctx->order = order;
+    ctx->precision = precision;
+    ctx->nj_cap = nj_capacity;
+    ctx->ngb_cap = ngb_cap;
+    ctx->stream = (cudaStream_t)cuda_stream;
+    ctx->sm_count = prop.multiProcessorCount;
+    if (a && a->alloc && a->free) {
+        ctx->alloc = *a;
+        ctx->has_alloc = true;
+    }
+    int rc = S2_OK;
+    const size_t nf = nfields(order), np = nplanes(order), nq = n_qplanes(precision, order);
+    if (rc == S2_OK) rc = dev_reserve(ctx, ctx->base, nf * nj_capacity * sizeof(double) + (size_t)nj_capacity * sizeof(int));
+    if (rc == S2_OK) rc = dev_reserve(ctx, ctx->planes, np * nj_capacity * sizeof(double2));
+    if (rc == S2_OK && nq) rc = dev_reserve(ctx, ctx->qplanes, nq * nj_capacity * sizeof(float4));
+    if (rc == S2_OK) rc = dev_reserve(ctx, ctx->flags, 256);
+    if (rc == S2_OK) {
+        cudaError_t e = cudaMemsetAsync(ctx->flags.p, 0, 256, ctx->stream);
+        if (e == cudaSuccess) e = cudaHostAlloc((void **)&ctx->h_flags, 64, cudaHostAllocDefault);
+        if (e == cudaSuccess) e = cudaEventCreateWithFlags(&ctx->ev_stage, cudaEventDisableTiming);
+        if (e == cudaSuccess) e = cudaEventCreateWithFlags(&ctx->ev_io, cudaEventDisableTiming);
+        for (int k = 0; k < 6 && e == cudaSuccess; ++k) e = cudaEventCreate(&ctx->ev_t[k]);
+        if (e == cudaSuccess) e = cudaStreamSynchronize(ctx->stream);
+        if (e != cudaSuccess) rc = fail_cuda(ctx, e);
+    }
+    if (rc != S2_OK) {
+        s2_close(ctx);
+        return rc;
+    }
+    *out = ctx;
+    return S2_OK;
+}
+
+extern "C" int s2_close(s2_ctx *ctx)
+{
+    if (!ctx) return S2_EINVAL;
+    cudaSetDevice(ctx->device);
+    cudaStreamSynchronize(ctx->stream);
+    for (Buf *b : {&ctx->base, &ctx->planes, &ctx->qplanes, &ctx->stage_dev, &ctx->iplanes, &ctx->iqplanes,
+                   &ctx->i_addr, &ctx->i_h2, &ctx->part, &ctx->result, &ctx->seg, &ctx->list, &ctx->flags})
+        dev_release(ctx, *b);
+    if (ctx->h_stage) cudaFreeHost(ctx->h_stage);
+    if (ctx->h_io) cudaFreeHost(ctx->h_io);
+    if (ctx->h_flags) cudaFreeHost(ctx->h_flags);
+    if (ctx->ev_stage) cudaEventDestroy(ctx->ev_stage);
+    if (ctx->ev_io) cudaEventDestroy(ctx->ev_io);
+    for (auto &e : ctx->ev_t)
+        if (e) cudaEventDestroy(e);
+    cudaGetLastError();
+    delete ctx;
+    return S2_OK;
+}
+
+extern "C" int s2_set_stream(s2_ctx *ctx, void *cuda_stream)
+{
+    if (!ctx) return S2_EINVAL;
+    CU(cudaStreamSynchronize(ctx->stream));
+    ctx->stream = (cudaStream_t)cuda_stream;
+    return S2_OK;
+}
+
+extern "C" int s2_synchronize(s2_ctx *ctx)
+{
+    if (!ctx) return S2_EINVAL;
+    CU(cudaStreamSynchronize(ctx->stream));
+    CU(cudaGetLastError());
+    return S2_OK;
+}
+
+// ---- a1: set / commit -------------------------------------------------------------------
+
+extern "C" int s2_set_j(s2_ctx *ctx, int n, const int *address, const int *id, const double *t, const double *mass,
+                        const double *pos, const double *vel, const double *acc, const double *jerk,
+                        const double *snap, const double *crackle)
+{
+    if (!ctx || n < 0) return S2_EINVAL;
+    if (n == 0) return S2_OK;
+    if (!address || !id || !t || !mass || !pos || !vel || !acc || !jerk) return S2_EINVAL;
+    if (ctx->order == 6 && (!snap || !crackle)) return S2_EINVAL;
+    if (n > ctx->nj_cap) return S2_ERANGE;
+    for (int k = 0; k < n; ++k)
+        if (address[k] < 0 || address[k] >= ctx->nj_cap) return S2_ERANGE;
+    for (int k = 0; k < n; ++k)
+        if (id[k] < 0) return S2_EINVAL;
+
+    // the previous commit may still be reading the staging buffer
+    if (ctx->batches.empty()) CU(cudaEventSynchronize(ctx->ev_stage));
+
+    const int nf = nfields(ctx->order);
+    const size_t off = align16(ctx->h_stage_used);
+    const size_t ints = align16((size_t)2 * n * sizeof(int));
+    const size_t bytes = ints + (size_t)nf * n * sizeof(double);
+    int rc = pinned_reserve(ctx, &ctx->h_stage, &ctx->h_stage_bytes, ctx->h_stage_used, off + bytes);
+    if (rc != S2_OK) return rc;
+    char *blk = (char *)ctx->h_stage + off;
+    memcpy(blk, address, (size_t)n * sizeof(int));
+    memcpy(blk + (size_t)n * sizeof(int), id, (size_t)n * sizeof(int));
+    double *f = (double *)(blk + ints);
+    memcpy(f, t, (size_t)n * sizeof(double));
+    memcpy(f + n, mass, (size_t)n * sizeof(double));
+    const double *vecs[6] = {pos, vel, acc, jerk, snap, crackle};
+    const int nvec = ctx->order == 6 ? 6 : 4;
+    for (int v = 0; v < nvec; ++v) {
+        double *d0 = f + (size_t)(2 + 3 * v) * n, *d1 = d0 + n, *d2 = d1 + n;
+        const double *s = vecs[v];
+        for (int k = 0; k < n; ++k) {
+            d0[k] = s[3 * (size_t)k];
+            d1[k] = s[3 * (size_t)k + 1];
+            d2[k] = s[3 * (size_t)k + 2];
+        }
+    }
+    ctx->batches.push_back({off, n});
+    ctx->h_stage_used = off + bytes;
+    return S2_OK;
+}
+
+extern "C" int s2_commit_j(s2_ctx *ctx)
+{
+    if (!ctx) return S2_EINVAL;
+    if (ctx->batches.empty()) return S2_OK;
+    CU(cudaSetDevice(ctx->device));
+    int rc = dev_reserve(ctx, ctx->stage_dev, ctx->h_stage_used);
+    if (rc != S2_OK) return rc;
+    CU(cudaMemcpyAsync(ctx->stage_dev.p, ctx->h_stage, ctx->h_stage_used, cudaMemcpyHostToDevice, ctx->stream));
+    CU(cudaEventRecord(ctx->ev_stage, ctx->stream));
+    const int nf = nfields(ctx->order);
+    for (const Batch &b : ctx->batches) {
+        ScatterArgs a{};
+        const char *blk = (const char *)ctx->stage_dev.p + b.offset;
+        a.address = (const int *)blk;
+        a.id = a.address + b.n;
+        const double *f = (const double *)(blk + align16((size_t)2 * b.n * sizeof(int)));
+        for (int k = 0; k < nf; ++k) {
+            a.src[k] = f + (size_t)k * b.n;
+            a.dst[k] = base_field(ctx, k);
+        }
+        a.dst_id = base_id(ctx);
+        a.n = b.n;
+        a.nfields = nf;
+        a.nj_cap = ctx->nj_cap;
+        a.src_soa = 1;
+        a.erange_flag = (int *)ctx->flags.p + 1;
+        CU(launch_scatter(a, ctx->stream));
+        ctx->launches++;
+    }
+    ctx->batches.clear();
+    ctx->h_stage_used = 0;
+    ctx->have_j = true;
+    ctx->predicted = false;
+    return S2_OK;
+}
+
+extern "C" int s2_commit_j_device(s2_ctx *ctx, int n, const int *d_address, const int *d_id, const double *d_t,
+                                  const double *d_mass, const double *d_pos, const double *d_vel,
+                                  const double *d_acc, const double *d_jerk, const double *d_snap,
+                                  const double *d_crackle)
+{
+    if (!ctx || n < 0) return S2_EINVAL;
+    if (n == 0) return S2_OK;
+    if (!d_address || !d_id || !d_t || !d_mass || !d_pos || !d_vel || !d_acc || !d_jerk) return S2_EINVAL;
+    if (ctx->order == 6 && (!d_snap || !d_crackle)) return S2_EINVAL;
+    if (n > ctx->nj_cap) return S2_ERANGE;
+    CU(cudaSetDevice(ctx->device));
+    ScatterArgs a{};
+    a.address = d_address;
+    a.id = d_id;
+    a.src[0] = d_t;
+    a.src[1] = d_mass;
+    const double *vecs[6] = {d_pos, d_vel, d_acc, d_jerk, d_snap, d_crackle};
+    const int nvec = ctx->order == 6 ? 6 : 4;
+    for (int v = 0; v < nvec; ++v)
+        for (int c = 0; c < 3; ++c) a.src[2 + 3 * v + c] = vecs[v] + c;
+    const int nf = nfields(ctx->order);
+    for (int k = 0; k < nf; ++k) a.dst[k] = base_field(ctx, k);
+    a.dst_id = base_id(ctx);
+    a.n = n;
+    a.nfields = nf;
+    a.nj_cap = ctx->nj_cap;
+    a.src_soa = 0;
+    a.erange_flag = (int *)ctx->flags.p + 1;
+    CU(launch_scatter(a, ctx->stream));
+    ctx->launches++;
+    ctx->have_j = true;
+    ctx->predicted = false;
+    return S2_OK;
+}
+
+// ---- a2: predict ------------------------------------------------------------------------
+
+extern "C" int s2_predict(s2_ctx *ctx, double t, int nj)
+{
+    if (!ctx) return S2_EINVAL;
+    if (nj <= 0 || nj > ctx->nj_cap) return S2_ERANGE;
+    if (!ctx->have_j || !ctx->batches.empty()) return S2_ESTATE;   // staged but uncommitted particles
+    CU(cudaSetDevice(ctx->device));
+    PredictArgs a{};
+    const int nf = nfields(ctx->order), np = nplanes(ctx->order), nq = n_qplanes(ctx->precision, ctx->order);
+    for (int k = 0; k < nf; ++k) a.f[k] = base_field(ctx, k);
+    a.id = base_id(ctx);
+    for (int k = 0; k < np; ++k) a.p[k] = plane(ctx, k);
+    for (int k = 0; k < nq; ++k) a.q[k] = qplane(ctx, k);
+    a.t = t;
+    a.nj = nj;
+    a.order = ctx->order;
+    a.precision = ctx->precision;
+    if (ctx->timing) CU(cudaEventRecord(ctx->ev_t[0], ctx->stream));
+    CU(launch_predict(a, ctx->stream));
+    if (ctx->timing) CU(cudaEventRecord(ctx->ev_t[1], ctx->stream));
+    ctx->ran_predict = true;
+    ctx->launches++;
+    ctx->predicted = true;
+    ctx->nj_pred = nj;
+    ctx->t_pred = t;
+    ctx->calc_done = false;
+    return S2_OK;
+}
+
+// ---- launch balancer ----------------------------------------------------------------------
+
+static int pow2_ceil(int x)
+{
+    int p = 1;
+    while (p < x) p <<= 1;
+    return p;
+}
+
+static cudaError_t dispatch(int precision, int order, unsigned flags, int L, dim3 grid, size_t smem,
+                            const ForceArgs &a, cudaStream_t st, bool query, int *occ)
+{
+    switch (precision) {
+    case S2_FP64: return dispatch_force_fp64(order, flags, L, grid, smem, a, st, query, occ);
+    case S2_FP32: return dispatch_force_fp32(order, flags, L, grid, smem, a, st, query, occ);
+    case S2_DS: return dispatch_force_ds(order, flags, L, grid, smem, a, st, query, occ);
+    }
+    return cudaErrorInvalidValue;
+}
+
+// Chooses lanes per i (L), warp columns (Wj), number of j-slices (S) and the tile length so that
+// the grid fills 148 SMs x resident CTAs in an integral number of waves.
+static int choose_shape(s2_ctx *ctx, int ni, int nj, unsigned flags, ForceShape *out)
+{
+    ForceShape sh{};
+    // lanes per i: minimise (number of i-groups) / L, i.e. the idle-lane waste; ties -> fewer lanes
+    int L = 1;
+    {
+        double best = 1e300;
+        for (int l = 1; l <= 32; l <<= 1) {
+            const int icta = kThreads / l;
+            const double c = (double)((ni + icta - 1) / icta) / l;
+            if (c < best * (1 - 1e-12)) {
+                best = c;
+                L = l;
+            }
+        }
+    }
+    if (ctx->tune[1] > 0) L = ctx->tune[1];
+    if (L < 1 || L > 32 || (L & (L - 1))) return S2_EINVAL;
+    int Wj = 1;
+    if (L == 32 && ni < kWarps) Wj = kWarps / pow2_ceil(ni);
+    if (ctx->tune[2] > 0) Wj = ctx->tune[2];
+    if (Wj < 1 || Wj > kWarps || (Wj & (Wj - 1)) || (Wj > 1 && L != 32)) return S2_EINVAL;
+    const int icta = (kWarps / Wj) * (32 / L);
+    const int Gi = (ni + icta - 1) / icta;
+    const int npl = force_nplanes(ctx->precision, ctx->order, flags);
+
+    int tile = ctx->tune[4] > 0 ? ctx->tune[4] : 256;
+    if (tile % 32 || tile < 32 || tile > 2048) return S2_EINVAL;
+
+    // resident CTAs per SM of this kernel variant (cached)
+    int occ = ctx->tune[3];
+    if (occ <= 0) {
+        const long long key = ((long long)flags << 32) | ((long long)L << 16) | tile;
+        auto it = ctx->occ_cache.find(key);
+        if (it == ctx->occ_cache.end()) {
+            ForceArgs dummy{};
+            cudaError_t e = dispatch(ctx->precision, ctx->order, flags, L, dim3(1), force_smem_bytes(npl, tile, 2),
+                                     dummy, ctx->stream, true, &occ);
+            if (e != cudaSuccess) return fail_cuda(ctx, e);
+            if (occ < 1) occ = 1;
+            ctx->occ_cache[key] = occ;
+        } else {
+            occ = it->second;
+        }
+    }
+    const long long slots = (long long)ctx->sm_count * occ;
+
+    int S;
+    if (ctx->tune[0] > 0) {
+        S = ctx->tune[0];
+    } else if (Wj > 1) {
+        // one tile per CTA; enough CTAs to fill the machine, slices no longer than the tile cap
+        S = (int)std::max<long long>(1, slots / Gi);
+        S = std::min(S, std::max(1, nj / (Wj * 4)));   // at least ~4 j per warp column
+        const int tcap = 512;
+        if ((nj + S - 1) / S > tcap) S = (nj + tcap - 1) / tcap;
+    } else {
+        // cost model: waves x (thread iterations per slice + fixed per-CTA overhead)
+        const double c0 = 24.0;
+        const int min_slice = std::max(32, 2 * L);
+        const int smax = (int)std::min<long long>(std::max(1, nj / min_slice),
+                                                  std::max<long long>(1, (8 * slots + Gi - 1) / Gi));
+        double best = 1e300;
+        S = 1;
+        for (int s = 1; s <= smax; ++s) {
+            const int sl = (nj + s - 1) / s;
+            const long long ctas = (long long)Gi * ((nj + sl - 1) / sl);
+            const double waves = (double)((ctas + slots - 1) / slots);
+            double cost = waves * ((double)((sl + L - 1) / L) + c0);
+            if (s > 1) cost *= 1.0 + 2e-3;   // a reduce pass follows
+            if (cost < best * (1 - 1e-9)) {
+                best = cost;
+                S = s;
+            }
+        }
+    }
+    if (S < 1 || S > 65535) return S2_EINVAL;
+    int slice_len = (nj + S - 1) / S;
+    S = (nj + slice_len - 1) / slice_len;
+    if (Wj > 1) {
+        tile = std::max(32, (slice_len + 31) / 32 * 32);
+        if (tile > 2048) return S2_EINVAL;
+    } else if (slice_len < tile) {
+        tile = std::max(32, (slice_len + 31) / 32 * 32);
+    }
+    sh.L = L;
+    sh.Wj = Wj;
+    sh.S = S;
+    sh.slice_len = slice_len;
+    sh.tile = tile;
+    sh.stages = 2;
+    ctx->last_info[7] = occ;
+    *out = sh;
+    return S2_OK;
+}
+
+// ---- a3-a8: force calls -------------------------------------------------------------------
+
+static int run_force(s2_ctx *ctx, int ni, const int *d_i_addr, const double *d_h2, bool explicit_i, double eps2,
+                     unsigned flags)
+{
+    ForceShape sh;
+    int rc = choose_shape(ctx, ni, ctx->nj_pred, flags, &sh);
+    if (rc != S2_OK) return rc;
+    const int nst = sh.S * sh.Wj;
+    const bool want_ngb = flags & S2_WANT_NGB;
+    const bool final_direct = nst == 1;
+
+    rc = dev_reserve(ctx, ctx->result, (size_t)ni * REC * sizeof(double));
+    if (rc == S2_OK && !final_direct) rc = dev_reserve(ctx, ctx->part, (size_t)nst * ni * REC * sizeof(double));
+    int segcap = 0;
+    if (want_ngb) {
+        if (ctx->ngb_cap <= 0) return S2_EINVAL;
+        const int jper = (sh.slice_len + sh.Wj - 1) / sh.Wj;   // longest j range one record covers
+        segcap = final_direct ? ctx->ngb_cap : std::min(ctx->ngb_cap, jper);
+        if (rc == S2_OK) rc = dev_reserve(ctx, ctx->list, (size_t)ni * ctx->ngb_cap * sizeof(int));
+        if (rc == S2_OK && !final_direct) rc = dev_reserve(ctx, ctx->seg, (size_t)ni * nst * segcap * sizeof(int));
+    }
+    if (rc != S2_OK) return rc;
+
+    ForceArgs a{};
+    const int np = nplanes(ctx->order), nq = n_qplanes(ctx->precision, ctx->order);
+    if (ctx->precision == S2_FP64) {
+        for (int k = 0; k < np; ++k) {
+            a.jp[k] = plane(ctx, k);
+            a.ip[k] = explicit_i ? (const void *)((double2 *)ctx->iplanes.p + (size_t)k * ni) : a.jp[k];
+        }
+    } else {
+        for (int k = 0; k < nq; ++k) {
+            a.jp[k] = qplane(ctx, k);
+            a.ip[k] = explicit_i ? (const void *)((float4 *)ctx->iqplanes.p + (size_t)k * ni) : a.jp[k];
+        }
+    }
+    if (ctx->precision != S2_FP64 && flags) {   // decisions are taken on fp64 positions in every mode
+        for (int k = 0; k < 2; ++k) {
+            a.jp[nq + k] = plane(ctx, k);
+            a.ip[nq + k] = explicit_i ? (const void *)((double2 *)ctx->iplanes.p + (size_t)k * ni) : a.jp[nq + k];
+        }
+    }
+    a.i_addr = explicit_i ? nullptr : d_i_addr;
+    a.h2 = d_h2;
+    a.jid_plane = plane(ctx, 3);
+    a.ni = ni;
+    a.nj = ctx->nj_pred;
+    a.eps2 = eps2;
+    a.S = sh.S;
+    a.slice_len = sh.slice_len;
+    a.Wj = sh.Wj;
+    a.tile = sh.tile;
+    a.nslices_total = nst;
+    a.is_final = final_direct ? 1 : 0;
+    a.rec = final_direct ? (double *)ctx->result.p : (double *)ctx->part.p;
+    a.seg = final_direct ? (int *)ctx->list.p : (int *)ctx->seg.p;
+    a.segcap = segcap;
+    a.overflow_flag = (int *)ctx->flags.p;
+    a.ngb_cap = ctx->ngb_cap;
+
+    CU(cudaMemsetAsync(ctx->flags.p, 0, sizeof(int), ctx->stream));   // overflow flag of this call
+    const int icta = (kWarps / sh.Wj) * (32 / sh.L);
+    dim3 grid((ni + icta - 1) / icta, sh.S);
+    const size_t smem = force_smem_bytes(force_nplanes(ctx->precision, ctx->order, flags), sh.tile, sh.stages);
+    if (ctx->timing) CU(cudaEventRecord(ctx->ev_t[2], ctx->stream));
+    CU(dispatch(ctx->precision, ctx->order, flags, sh.L, grid, smem, a, ctx->stream, false, nullptr));
+    if (ctx->timing) CU(cudaEventRecord(ctx->ev_t[3], ctx->stream));
+    ctx->launches++;
+    ctx->ran_force = true;
+    ctx->ran_reduce = false;
+    if (!final_direct) {
+        ReduceArgs r{};
+        r.part = (const double *)ctx->part.p;
+        r.out = (double *)ctx->result.p;
+        r.seg = (const int *)ctx->seg.p;
+        r.list = (int *)ctx->list.p;
+        r.jid_plane = plane(ctx, 3);
+        r.ni = ni;
+        r.nslices_total = nst;
+        r.segcap = segcap;
+        r.ngb_cap = ctx->ngb_cap;
+        r.order = ctx->order;
+        r.flags = flags;
+        r.overflow_flag = (int *)ctx->flags.p;
+        if (ctx->timing) CU(cudaEventRecord(ctx->ev_t[4], ctx->stream));
+        CU(launch_reduce(r, ctx->stream));
+        if (ctx->timing) CU(cudaEventRecord(ctx->ev_t[5], ctx->stream));
+        ctx->launches++;
+        ctx->ran_reduce = true;
+    }
+    int *li = ctx->last_info;
+    li[0] = sh.S; li[1] = sh.L; li[2] = sh.Wj; li[3] = (int)(grid.x * grid.y); li[4] = kThreads;
+    li[5] = (int)smem; li[6] = final_direct ? 0 : 1;
+    ctx->calc_done = true;
+    ctx->ni_last = ni;
+    ctx->flags_last = flags;
+    return S2_OK;
+}
+
+static int check_calc(s2_ctx *ctx, int ni, unsigned flags, const void *h2)
+{
+    if (!ctx || ni <= 0) return S2_EINVAL;
+    if (flags & ~(unsigned)(S2_WANT_NN | S2_WANT_NGB)) return S2_EINVAL;
+    if ((flags & S2_WANT_NGB) && (!h2 || ctx->ngb_cap <= 0)) return S2_EINVAL;
+    if (!ctx->predicted) return S2_ESTATE;
+    return S2_OK;
+}
+
+extern "C" int s2_calc_ilist_device(s2_ctx *ctx, int ni, const int *d_i_address, const double *d_h2, double eps2,
+                                    unsigned flags)
+{
+    int rc = check_calc(ctx, ni, flags, d_h2);
+    if (rc != S2_OK) return rc;
+    if (!d_i_address) return S2_EINVAL;
+    CU(cudaSetDevice(ctx->device));
+    return run_force(ctx, ni, d_i_address, d_h2, false, eps2, flags);
+}
+
+extern "C" int s2_calc_ilist(s2_ctx *ctx, int ni, const int *i_address, const double *h2, double eps2,
+                             unsigned flags)
+{
+    int rc = check_calc(ctx, ni, flags, h2);
+    if (rc != S2_OK) return rc;
+    if (!i_address) return S2_EINVAL;
+    for (int k = 0; k < ni; ++k)
+        if (i_address[k] < 0 || i_address[k] >= ctx->nj_pred) return S2_ERANGE;
+    CU(cudaSetDevice(ctx->device));
+    const bool ngb = flags & S2_WANT_NGB;
+    const size_t b_addr = align16((size_t)ni * sizeof(int)), b_h2 = ngb ? (size_t)ni * sizeof(double) : 0;
+    CU(cudaEventSynchronize(ctx->ev_io));
+    rc = pinned_reserve(ctx, &ctx->h_io, &ctx->h_io_bytes, 0, b_addr + b_h2);
+    if (rc == S2_OK) rc = dev_reserve(ctx, ctx->i_addr, b_addr + b_h2);
+    if (rc != S2_OK) return rc;
+    memcpy(ctx->h_io, i_address, (size_t)ni * sizeof(int));
+    if (ngb) memcpy((char *)ctx->h_io + b_addr, h2, b_h2);
+    CU(cudaMemcpyAsync(ctx->i_addr.p, ctx->h_io, b_addr + b_h2, cudaMemcpyHostToDevice, ctx->stream));
+    CU(cudaEventRecord(ctx->ev_io, ctx->stream));
+    return run_force(ctx, ni, (const int *)ctx->i_addr.p,
+                     ngb ? (const double *)((char *)ctx->i_addr.p + b_addr) : nullptr, false, eps2, flags);
+}
+
+static inline void split_ds_host(double x, float *hi, float *lo)
+{
+    *hi = (float)x;
+    *lo = (float)(x - (double)*hi);
+}
+
+extern "C" int s2_calc_explicit(s2_ctx *ctx, int ni, const int *id, const double *pos, const double *vel,
+                                const double *acc, const double *h2, double eps2, unsigned flags)
+{
+    int rc = check_calc(ctx, ni, flags, h2);
+    if (rc != S2_OK) return rc;
+    if (!id || !pos || !vel || (ctx->order == 6 && !acc)) return S2_EINVAL;
+    CU(cudaSetDevice(ctx->device));
+    const bool ngb = flags & S2_WANT_NGB;
+    const int np = nplanes(ctx->order), nq = n_qplanes(ctx->precision, ctx->order);
+    const size_t b_p = (size_t)np * ni * sizeof(double2), b_q = (size_t)nq * ni * sizeof(float4);
+    const size_t b_h2 = ngb ? (size_t)ni * sizeof(double) : 0;
+    CU(cudaEventSynchronize(ctx->ev_io));
+    rc = pinned_reserve(ctx, &ctx->h_io, &ctx->h_io_bytes, 0, b_p + b_q + b_h2);
+    if (rc == S2_OK) rc = dev_reserve(ctx, ctx->iplanes, b_p);
+    if (rc == S2_OK && nq) rc = dev_reserve(ctx, ctx->iqplanes, b_q);
+    if (rc == S2_OK && ngb) rc = dev_reserve(ctx, ctx->i_h2, b_h2);
+    if (rc != S2_OK) return rc;
+    // pack the i-particles into the same plane layout the predictor writes for j (pure data movement
+    // plus the fp64 -> (hi, lo) float split of the storage format)
+    double2 *P = (double2 *)ctx->h_io;
+    float4 *Q = (float4 *)((char *)ctx->h_io + b_p);
+    for (int k = 0; k < ni; ++k) {
+        const double *x = pos + 3 * (size_t)k, *v = vel + 3 * (size_t)k;
+        int idk = id[k];
+        double idbits;
+        memset(&idbits, 0, sizeof idbits);
+        memcpy(&idbits, &idk, sizeof idk);   // little-endian: low word = id, high word = 0
+        P[k] = make_double2(x[0], x[1]);
+        P[(size_t)ni + k] = make_double2(x[2], 0.0);
+        P[(size_t)2 * ni + k] = make_double2(v[0], v[1]);
+        P[(size_t)3 * ni + k] = make_double2(v[2], idbits);
+        const double *ac = ctx->order == 6 ? acc + 3 * (size_t)k : nullptr;
+        if (ac) {
+            P[(size_t)4 * ni + k] = make_double2(ac[0], ac[1]);
+            P[(size_t)5 * ni + k] = make_double2(ac[2], 0.0);
+        }
+        float idf;
+        memcpy(&idf, &idk, sizeof idf);
+        if (ctx->precision == S2_FP32) {
+            float xh[3], xl[3];
+            for (int c = 0; c < 3; ++c) split_ds_host(x[c], &xh[c], &xl[c]);
+            Q[k] = make_float4(xh[0], xh[1], xh[2], 0.f);
+            Q[(size_t)ni + k] = make_float4(xl[0], xl[1], xl[2], idf);
+            Q[(size_t)2 * ni + k] = make_float4((float)v[0], (float)v[1], (float)v[2], 0.f);
+            if (ac) Q[(size_t)3 * ni + k] = make_float4((float)ac[0], (float)ac[1], (float)ac[2], 0.f);
+        } else if (ctx->precision == S2_DS) {
+            float h[9], l[9];
+            for (int c = 0; c < 3; ++c) {
+                split_ds_host(x[c], &h[c], &l[c]);
+                split_ds_host(v[c], &h[3 + c], &l[3 + c]);
+                if (ac) split_ds_host(ac[c], &h[6 + c], &l[6 + c]);
+            }
+            Q[k] = make_float4(h[0], l[0], h[1], l[1]);
+            Q[(size_t)ni + k] = make_float4(h[2], l[2], 0.f, 0.f);
+            Q[(size_t)2 * ni + k] = make_float4(h[3], l[3], h[4], l[4]);
+            Q[(size_t)3 * ni + k] = make_float4(h[5], l[5], idf, 0.f);
+            if (ac) {
+                Q[(size_t)4 * ni + k] = make_float4(h[6], l[6], h[7], l[7]);
+                Q[(size_t)5 * ni + k] = make_float4(h[8], l[8], 0.f, 0.f);
+            }
+        }
+    }
+    if (ngb) memcpy((char *)ctx->h_io + b_p + b_q, h2, b_h2);
+    CU(cudaMemcpyAsync(ctx->iplanes.p, ctx->h_io, b_p, cudaMemcpyHostToDevice, ctx->stream));
+    if (nq) CU(cudaMemcpyAsync(ctx->iqplanes.p, (char *)ctx->h_io + b_p, b_q, cudaMemcpyHostToDevice, ctx->stream));
+    if (ngb) CU(cudaMemcpyAsync(ctx->i_h2.p, (char *)ctx->h_io + b_p + b_q, b_h2, cudaMemcpyHostToDevice, ctx->stream));
+    CU(cudaEventRecord(ctx->ev_io, ctx->stream));
+    return run_force(ctx, ni, nullptr, ngb ? (const double *)ctx->i_h2.p : nullptr, true, eps2, flags);
+}
+
+// ---- a9: results --------------------------------------------------------------------------
+
+static int fetch_flags(s2_ctx *ctx)
+{
+    CU(cudaMemcpyAsync(ctx->h_flags, ctx->flags.p, 2 * sizeof(int), cudaMemcpyDeviceToHost, ctx->stream));
+    return S2_OK;
+}
+
+static int post_sync_status(s2_ctx *ctx)
+{
+    if (ctx->h_flags[1]) {   // a device-side commit dropped out-of-range addresses
+        cudaMemsetAsync((int *)ctx->flags.p + 1, 0, sizeof(int), ctx->stream);
+        return S2_ERANGE;
+    }
+    if ((ctx->flags_last & S2_WANT_NGB) && ctx->h_flags[0]) return S2_EOVERFLOW;
+    return S2_OK;
+}
+
+extern "C" int s2_get_results(s2_ctx *ctx, int ni, double *acc, double *jerk, double *snap, double *pot, int *nn_id,
+                              double *nn_r2, int *ngb_count)
+{
+    if (!ctx || ni < 0) return S2_EINVAL;
+    if (!ctx->calc_done) return S2_ESTATE;
+    if (ni > ctx->ni_last) return S2_ERANGE;
+    CU(cudaSetDevice(ctx->device));
+    const size_t bytes = (size_t)ni * REC * sizeof(double);
+    CU(cudaEventSynchronize(ctx->ev_io));
+    int rc = pinned_reserve(ctx, &ctx->h_io, &ctx->h_io_bytes, 0, bytes);
+    if (rc != S2_OK) return rc;
+    if (ni) CU(cudaMemcpyAsync(ctx->h_io, ctx->result.p, bytes, cudaMemcpyDeviceToHost, ctx->stream));
+    rc = fetch_flags(ctx);
+    if (rc != S2_OK) return rc;
+    CU(cudaStreamSynchronize(ctx->stream));
+    CU(cudaGetLastError());
+    const double *r = (const double *)ctx->h_io;
+    for (int k = 0; k < ni; ++k, r += REC) {
+        if (acc) { acc[3 * (size_t)k] = r[0]; acc[3 * (size_t)k + 1] = r[1]; acc[3 * (size_t)k + 2] = r[2]; }
+        if (jerk) { jerk[3 * (size_t)k] = r[3]; jerk[3 * (size_t)k + 1] = r[4]; jerk[3 * (size_t)k + 2] = r[5]; }
+        if (pot) pot[k] = r[6];
+        if (nn_r2) nn_r2[k] = r[7];
+        int packed[2];
+        memcpy(packed, &r[8], sizeof packed);   // low word = nn id, high word = neighbour count
+        if (nn_id) nn_id[k] = packed[0];
+        if (ngb_count) ngb_count[k] = packed[1];
+        if (snap && ctx->order == 6) { snap[3 * (size_t)k] = r[9]; snap[3 * (size_t)k + 1] = r[10]; snap[3 * (size_t)k + 2] = r[11]; }
+    }
+    return post_sync_status(ctx);
+}
+
+extern "C" int s2_get_neighbours(s2_ctx *ctx, int i, int cap, int *n_out, int *list)
+{
+    if (!ctx || !n_out || cap < 0 || (cap > 0 && !list)) return S2_EINVAL;
+    if (!ctx->calc_done || !(ctx->flags_last & S2_WANT_NGB)) return S2_ESTATE;
+    if (i < 0 || i >= ctx->ni_last) return S2_ERANGE;
+    CU(cudaSetDevice(ctx->device));
+    double rec8 = 0.0;
+    CU(cudaMemcpyAsync(&rec8, (double *)ctx->result.p + (size_t)i * REC + 8, sizeof(double), cudaMemcpyDeviceToHost,
+                       ctx->stream));
+    CU(cudaStreamSynchronize(ctx->stream));
+    int packed[2];
+    memcpy(packed, &rec8, sizeof packed);
+    const int have = std::min(packed[1], ctx->ngb_cap);
+    const int n = std::min(have, cap);
+    if (n > 0) {
+        CU(cudaMemcpyAsync(list, (int *)ctx->list.p + (size_t)i * ctx->ngb_cap, (size_t)n * sizeof(int),
+                           cudaMemcpyDeviceToHost, ctx->stream));
+        CU(cudaStreamSynchronize(ctx->stream));
+    }
+    *n_out = n;
+    return packed[1] > ctx->ngb_cap ? S2_EOVERFLOW : S2_OK;
+}
+
+extern "C" int s2_get_neighbours_csr(s2_ctx *ctx, int ni, long long *offsets, int *list, long long list_cap)
+{
+    if (!ctx || ni < 0 || !offsets || list_cap < 0) return S2_EINVAL;
+    if (!ctx->calc_done || !(ctx->flags_last & S2_WANT_NGB)) return S2_ESTATE;
+    if (ni > ctx->ni_last) return S2_ERANGE;
+    CU(cudaSetDevice(ctx->device));
+    // counts come from the result records, lists from the fixed-stride device buffer
+    const size_t b_rec = align16((size_t)ni * REC * sizeof(double));
+    const size_t b_list = (size_t)ni * ctx->ngb_cap * sizeof(int);
+    CU(cudaEventSynchronize(ctx->ev_io));
+    int rc = pinned_reserve(ctx, &ctx->h_io, &ctx->h_io_bytes, 0, b_rec + b_list);
+    if (rc != S2_OK) return rc;
+    if (ni) {
+        CU(cudaMemcpyAsync(ctx->h_io, ctx->result.p, (size_t)ni * REC * sizeof(double), cudaMemcpyDeviceToHost, ctx->stream));
+        CU(cudaMemcpyAsync((char *)ctx->h_io + b_rec, ctx->list.p, b_list, cudaMemcpyDeviceToHost, ctx->stream));
+    }
+    CU(cudaStreamSynchronize(ctx->stream));
+    const double *r = (const double *)ctx->h_io;
+    const int *L = (const int *)((const char *)ctx->h_io + b_rec);
+    long long tot = 0;
+    bool overflow = false;
+    for (int k = 0; k < ni; ++k) {
+        int packed[2];
+        memcpy(packed, &r[(size_t)k * REC + 8], sizeof packed);
+        offsets[k] = tot;
+        if (packed[1] > ctx->ngb_cap) overflow = true;
+        tot += std::min(packed[1], ctx->ngb_cap);
+    }
+    offsets[ni] = tot;
+    if (tot > list_cap || (tot > 0 && !list)) return S2_ERANGE;
+    for (int k = 0; k < ni; ++k)
+        memcpy(list + offsets[k], L + (size_t)k * ctx->ngb_cap, (size_t)(offsets[k + 1] - offsets[k]) * sizeof(int));
+    return overflow ? S2_EOVERFLOW : S2_OK;
+}
+
+// ---- hooks and diagnostics ----------------------------------------------------------------
+
+extern "C" int s2_get_predicted_j(s2_ctx *ctx, int first, int n, double *pos, double *vel, double *acc)
+{
+    if (!ctx || n < 0 || first < 0) return S2_EINVAL;
+    if (!ctx->predicted) return S2_ESTATE;
+    if ((long long)first + n > ctx->nj_pred) return S2_ERANGE;
+    if (n == 0) return S2_OK;
+    CU(cudaSetDevice(ctx->device));
+    const int np = nplanes(ctx->order);
+    std::vector<double2> h((size_t)np * n);
+    for (int p = 0; p < np; ++p)
+        CU(cudaMemcpyAsync(h.data() + (size_t)p * n, plane(ctx, p) + first, (size_t)n * sizeof(double2),
+                           cudaMemcpyDeviceToHost, ctx->stream));
+    CU(cudaStreamSynchronize(ctx->stream));
+    for (int k = 0; k < n; ++k) {
+        if (pos) { pos[3 * (size_t)k] = h[k].x; pos[3 * (size_t)k + 1] = h[k].y; pos[3 * (size_t)k + 2] = h[(size_t)n + k].x; }
+        if (vel) { vel[3 * (size_t)k] = h[(size_t)2 * n + k].x; vel[3 * (size_t)k + 1] = h[(size_t)2 * n + k].y; vel[3 * (size_t)k + 2] = h[(size_t)3 * n + k].x; }
+        if (acc && np == 6) { acc[3 * (size_t)k] = h[(size_t)4 * n + k].x; acc[3 * (size_t)k + 1] = h[(size_t)4 * n + k].y; acc[3 * (size_t)k + 2] = h[(size_t)5 * n + k].x; }
+    }
+    return S2_OK;
+}
+
+extern "C" int s2_get_j(s2_ctx *ctx, int first, int n, int *id, double *t, double *mass, double *pos)
+{
+    if (!ctx || n < 0 || first < 0) return S2_EINVAL;
+    if (!ctx->have_j) return S2_ESTATE;
+    if ((long long)first + n > ctx->nj_cap) return S2_ERANGE;
+    if (n == 0) return S2_OK;
+    CU(cudaSetDevice(ctx->device));
+    std::vector<double> h((size_t)5 * n);
+    for (int f = 0; f < 5; ++f)
+        CU(cudaMemcpyAsync(h.data() + (size_t)f * n, base_field(ctx, f) + first, (size_t)n * sizeof(double),
+                           cudaMemcpyDeviceToHost, ctx->stream));
+    if (id) CU(cudaMemcpyAsync(id, base_id(ctx) + first, (size_t)n * sizeof(int), cudaMemcpyDeviceToHost, ctx->stream));
+    int rc = fetch_flags(ctx);
+    if (rc != S2_OK) return rc;
+    CU(cudaStreamSynchronize(ctx->stream));
+    for (int k = 0; k < n; ++k) {
+        if (t) t[k] = h[k];
+        if (mass) mass[k] = h[(size_t)n + k];
+        if (pos) for (int c = 0; c < 3; ++c) pos[3 * (size_t)k + c] = h[(size_t)(2 + c) * n + k];
+    }
+    if (ctx->h_flags[1]) {
+        cudaMemsetAsync((int *)ctx->flags.p + 1, 0, sizeof(int), ctx->stream);
+        return S2_ERANGE;
+    }
+    return S2_OK;
+}
+
+extern "C" int s2_set_tuning(s2_ctx *ctx, int key, int value)
+{
+    if (!ctx || key < 0 || key > 4 || value < 0) return S2_EINVAL;
+    ctx->tune[key] = value;
+    return S2_OK;
+}
+
+extern "C" int s2_last_launch_info(const s2_ctx *ctx, int out[8])
+{
+    if (!ctx || !out) return S2_EINVAL;
+    memcpy(out, ctx->last_info, sizeof ctx->last_info);
+    return S2_OK;
+}
+
+extern "C" long long s2_kernel_launches(const s2_ctx *ctx) { return ctx ? ctx->launches : 0; }
+
+extern "C" int s2_enable_timing(s2_ctx *ctx, int on)
+{
+    if (!ctx) return S2_EINVAL;
+    ctx->timing = on != 0;
+    ctx->ran_predict = ctx->ran_force = ctx->ran_reduce = false;
+    return S2_OK;
+}
+
+extern "C" int s2_get_timing(s2_ctx *ctx, float *predict_ms, float *force_ms, float *reduce_ms)
+{
+    if (!ctx) return S2_EINVAL;
+    if (!ctx->timing) return S2_ESTATE;
+    CU(cudaStreamSynchronize(ctx->stream));
+    float v[3] = {0.f, 0.f, 0.f};
+    const bool ran[3] = {ctx->ran_predict, ctx->ran_force, ctx->ran_reduce};
+    for (int k = 0; k < 3; ++k)
+        if (ran[k]) CU(cudaEventElapsedTime(&v[k], ctx->ev_t[2 * k], ctx->ev_t[2 * k + 1]));
+    if (predict_ms) *predict_ms = v[0];
+    if (force_ms) *force_ms = v[1];
+    if (reduce_ms) *reduce_ms = v[2];
+    return S2_OK;
+}
+
+extern "C" int s2_peak_fma(s2_ctx *ctx, int kind, int iters, double *fma_per_s)
+{
+    if (!ctx || !fma_per_s || iters <= 0 || kind < 0 || kind > 1) return S2_EINVAL;
+    CU(cudaSetDevice(ctx->device));
+    CU(run_peak_fma(kind, iters, ctx->sm_count, ctx->stream, fma_per_s));
+    ctx->launches += 2;
+    return S2_OK;
+}
+
+extern "C" const char *s2_strerror(int code)
+{
+    switch (code) {
+    case S2_OK: return "ok";
+    case S2_EINVAL: return "invalid argument";
+    case S2_ERANGE: return "address or count out of range";
+    case S2_ENOMEM: return "out of device or pinned memory";
+    case S2_ECUDA: return "CUDA error or no CUDA device (there is no CPU fallback)";
+    case S2_ESTATE: return "call order violated (commit -> predict -> calc -> get)";
+    case S2_EOVERFLOW: return "a neighbour list exceeded ngb_cap (results valid, lists truncated)";
+    }
+    return "unknown error code";
+}
+
+extern "C" const char *s2_last_cuda_error(const s2_ctx *ctx) { return ctx ? ctx->cuda_err.c_str() : ""; }
+
+extern "C" const char *s2_version(void) { return "s2b200 0.1 (sm_100a)"; }

@@ -1,0 +1,121 @@
+// s2_internal.h -- shared declarations of the CUDA library behind include/s2b200.h.
+// Not part of the ABI.  Nothing here is shared with oracle/.
+#pragma once
+
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include <vector>
+
+#include "../../include/s2b200.h"
+
+namespace s2 {
+
+// ---- data layout in HBM ----------------------------------------
+//
+// Base j-store (fp64 SoA, one array per scalar field, capacity nj_cap each):
+//   field 0 t_j, 1 m, 2-4 x, 5-7 v, 8-10 a, 11-13 jerk, [14-16 snap, 17-19 crackle], + int id[]
+// Predicted j-store, fp64 "planes" of 16-byte elements (one element per particle per plane):
+//   P0 (x, y)   P1 (z, m)   P2 (vx, vy)   P3 (vz, id bits)   [6th order: P4 (ax, ay)  P5 (az, 0)]
+// fp32 planes (float4 per particle):
+//   F0 (x_hi, y_hi, z_hi, m)   F1 (x_lo, y_lo, z_lo, id bits)   F2 (vx, vy, vz, 0)   [F3 (ax, ay, az, 0)]
+// double-single planes (float4 per particle, value = hi + lo):
+//   D0 (x_hi, x_lo, y_hi, y_lo)  D1 (z_hi, z_lo, m_hi, m_lo)  D2 (vx_hi, vx_lo, vy_hi, vy_lo)
+//   D3 (vz_hi, vz_lo, id bits, 0)   [D4 (ax_hi, ax_lo, ay_hi, ay_lo)  D5 (az_hi, az_lo, 0, 0)]
+// Result / partial record: REC doubles per (slice, i):
+//   0-2 acc, 3-5 jerk, 6 pot, 7 nn_d2, 8 {int nn (address in partials, id in finals), int ngb_count},
+//   9-11 snap (6th order)
+
+constexpr int kMaxFields = 20;
+constexpr int kMaxPlanes = 8;      // up to 6 arithmetic planes + 2 fp64 position planes for decisions
+constexpr int REC = 12;            // doubles per result record (96 B = three 32-byte sectors)
+constexpr int kThreads = 256;      // threads per force CTA
+constexpr int kWarps = kThreads / 32;
+
+inline int nfields(int order) { return order == 6 ? 20 : 14; }
+inline int nplanes(int order) { return order == 6 ? 6 : 4; }
+
+struct PredictArgs {
+    const double *f[kMaxFields];   // base fields
+    const int *id;
+    double2 *p[kMaxPlanes];        // fp64 planes (always written)
+    float4 *q[kMaxPlanes];         // precision-specific planes or nullptr
+    double t;
+    int nj;
+    int order;
+    int precision;
+};
+
+struct ScatterArgs {
+    const int *address;
+    const int *id;
+    const double *src[kMaxFields]; // scalar fields (t, m) have stride 1; vector fields are (n,3) row-major
+    double *dst[kMaxFields];
+    int *dst_id;
+    int n;
+    int nfields;
+    int nj_cap;
+    int src_soa;                   // 1: every src field is a plain length-n array (staging layout)
+    int *erange_flag;
+};
+
+struct ForceArgs {
+    const void *jp[kMaxPlanes];    // j planes staged per tile: the pair-arithmetic planes, then (non-fp64
+                                   // modes with NN/NGB) the fp64 position planes P0, P1 for the decisions
+    const void *ip[kMaxPlanes];    // same list for the i side (== jp in address mode)
+    const int *i_addr;             // nullptr: i-th i-particle lives at index i of ip
+    const double *h2;              // per i, or nullptr
+    const double2 *jid_plane;      // fp64 plane P3 of j (id lookup for final nn)
+    int ni;
+    int nj;
+    double eps2;
+    int S;                         // CTA slices over j
+    int slice_len;                 // j per CTA slice
+    int Wj;                        // warp columns over j inside a CTA (1,2,4,8)
+    int tile;                      // j per shared-memory tile
+    int nslices_total;             // S * Wj
+    int is_final;                  // 1: write final records (nn as id), no reduce kernel follows
+    double *rec;                   // [nslices_total][ni][REC]
+    int *seg;                      // [ni][nslices_total][segcap] neighbour segments
+    int segcap;
+    int *overflow_flag;
+    int ngb_cap;
+};
+
+struct ReduceArgs {
+    const double *part;            // [nslices_total][ni][REC]
+    double *out;                   // [ni][REC]
+    const int *seg;                // [ni][nslices_total][segcap]
+    int *list;                     // [ni][ngb_cap]
+    const double2 *jid_plane;      // P3 of j
+    int ni;
+    int nslices_total;
+    int segcap;
+    int ngb_cap;
+    int order;
+    unsigned flags;
+    int *overflow_flag;
+};
+
+// kernels' host-side launchers (each returns the cudaError_t of the launch)
+cudaError_t launch_scatter(const ScatterArgs &a, cudaStream_t st);
+cudaError_t launch_predict(const PredictArgs &a, cudaStream_t st);
+cudaError_t launch_reduce(const ReduceArgs &a, cudaStream_t st);
+
+struct ForceShape {                // chosen by the balancer in s2_api.cu
+    int L;                         // lanes per i (1..32)
+    int Wj;                        // warp columns
+    int S;
+    int slice_len;
+    int tile;
+    int stages;
+};
+constexpr int kSmemHeader = 64;   // mbarriers live in the first 64 bytes of dynamic shared memory
+inline size_t force_smem_bytes(int nplanes, int tile, int stages)
+{
+    return (size_t)kSmemHeader + (size_t)stages * nplanes * tile * 16;
+}
+
+cudaError_t run_peak_fma(int kind, int iters, int sm_count, cudaStream_t st, double *fma_per_s);
+
+}  // namespace s2

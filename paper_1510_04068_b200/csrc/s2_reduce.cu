@@ -1,0 +1,105 @@
+// s2_reduce.cu -- a6: deterministic combine of the per-slice partial records, and the
+// neighbour-list compaction across slices.
+//
+// PAPER.md sec 2.2.4 (L88): Sapporo1 "contains two computational kernels ... the second sums the
+// partial results"; Sapporo2 merged them with atomics.  This build keeps the second kernel
+// because floating-point atomics make the summation order (and the last digit, L84, L164)
+// run-dependent; here the order is fixed: lane l of the warp that owns i adds slices
+// l, l+32, l+64, ... in sequence, then the 32 lanes are combined by an xor-butterfly.
+// The kernel streams S*ni records of 96 bytes once: L2/HBM-bound, tiny.
+#include <math_constants.h>
+
+#include "s2_force_common.cuh"
+
+namespace s2 {
+
+__global__ void __launch_bounds__(256) reduce_kernel(ReduceArgs a)
+{
+    const int warp = (blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+    const int lane = threadIdx.x & 31;
+    if (warp >= a.ni) return;   // whole warp exits together
+    const int i = warp;
+    const int S = a.nslices_total;
+
+    double v[10];
+#pragma unroll
+    for (int c = 0; c < 10; ++c) v[c] = 0.0;
+    double nn_d2 = CUDART_INF;
+    int nn_j = -1;
+    int cnt_total = 0;     // neighbours over my slices
+    int written = 0;       // running output position (warp-uniform)
+
+    for (int s0 = 0; s0 < S; s0 += 32) {
+        const int s = s0 + lane;
+        int c = 0;
+        if (s < S) {
+            const double2 *r = reinterpret_cast<const double2 *>(a.part + ((size_t)s * a.ni + i) * REC);
+            const double2 r0 = r[0], r1 = r[1], r2 = r[2], r3 = r[3], r4 = r[4], r5 = r[5];
+            v[0] += r0.x; v[1] += r0.y; v[2] += r1.x; v[3] += r1.y; v[4] += r2.x; v[5] += r2.y;
+            v[6] += r3.x;
+            if (a.order == 6) { v[7] += r4.y; v[8] += r5.x; v[9] += r5.y; }
+            const int j = __double2loint(r4.x);
+            c = __double2hiint(r4.x);
+            // slices are visited in ascending order by each lane, so strict < keeps the lowest address
+            if (r3.y < nn_d2 || (r3.y == nn_d2 && (unsigned)j < (unsigned)nn_j)) {
+                nn_d2 = r3.y;
+                nn_j = j;
+            }
+        }
+        cnt_total += c;
+        if (a.flags & S2_WANT_NGB) {
+            // compaction across slices: exclusive prefix of the (clamped) segment lengths in slice
+            // order = ascending j order, by warp shuffles; each lane copies its own segment.
+            const int len = min(c, a.segcap);
+            int incl = len;
+#pragma unroll
+            for (int m = 1; m < 32; m <<= 1) {
+                const int o = __shfl_up_sync(0xffffffffu, incl, m);
+                if (lane >= m) incl += o;
+            }
+            const int base = written + incl - len;
+            if (len > 0) {
+                const int *src = a.seg + ((size_t)i * S + s) * a.segcap;
+                int *dst = a.list + (size_t)i * a.ngb_cap;
+                for (int k = 0; k < len && base + k < a.ngb_cap; ++k) dst[base + k] = src[k];
+            }
+            written += __shfl_sync(0xffffffffu, incl, 31);
+        }
+    }
+
+#pragma unroll
+    for (int m = 1; m < 32; m <<= 1) {
+#pragma unroll
+        for (int c = 0; c < 10; ++c) v[c] += shfl_xor_d(v[c], m);
+        const double od2 = shfl_xor_d(nn_d2, m);
+        const int oj = __shfl_xor_sync(0xffffffffu, nn_j, m);
+        if (od2 < nn_d2 || (od2 == nn_d2 && (unsigned)oj < (unsigned)nn_j)) {
+            nn_d2 = od2;
+            nn_j = oj;
+        }
+        cnt_total += __shfl_xor_sync(0xffffffffu, cnt_total, m);
+    }
+
+    if (lane == 0) {
+        int nn = nn_j;
+        if ((a.flags & S2_WANT_NN) && nn >= 0) nn = __double2loint(a.jid_plane[nn].y);
+        if ((a.flags & S2_WANT_NGB) && cnt_total > a.ngb_cap) *a.overflow_flag = 1;
+        double2 *o = reinterpret_cast<double2 *>(a.out + (size_t)i * REC);
+        o[0] = make_double2(v[0], v[1]);
+        o[1] = make_double2(v[2], v[3]);
+        o[2] = make_double2(v[4], v[5]);
+        o[3] = make_double2(v[6], nn_d2);
+        o[4] = make_double2(__hiloint2double(cnt_total, nn), v[7]);
+        o[5] = make_double2(v[8], v[9]);
+    }
+}
+
+cudaError_t launch_reduce(const ReduceArgs &a, cudaStream_t st)
+{
+    if (a.ni <= 0) return cudaSuccess;
+    const int warps_per_block = 8;
+    reduce_kernel<<<(a.ni + warps_per_block - 1) / warps_per_block, 32 * warps_per_block, 0, st>>>(a);
+    return cudaGetLastError();
+}
+
+}  // namespace s2

@@ -1,0 +1,171 @@
+// s2_store.cu -- a1 (commit: scatter staged particles into the fp64 SoA j-store) and
+// a2 (Taylor predictor) kernels.  PAPER.md L88: "one copy kernel to move particles from CPU
+// buffers to GPU buffers, one kernel to predict the particles to the new time-step".
+// Both are pure streaming kernels: HBM-bound.
+#include "s2_internal.h"
+
+namespace s2 {
+
+// One thread per staged particle; consecutive threads read consecutive staged values
+// (coalesced) and write to `address` (contiguous when the host sends address-ordered sets).
+__global__ void __launch_bounds__(256) scatter_kernel(ScatterArgs a)
+{
+    int p = blockIdx.x * blockDim.x + threadIdx.x;
+    if (p >= a.n) return;
+    int addr = a.address[p];
+    if (addr < 0 || addr >= a.nj_cap) {
+        *a.erange_flag = 1;
+        return;
+    }
+    a.dst_id[addr] = a.id[p];
+#pragma unroll
+    for (int f = 0; f < kMaxFields; ++f) {
+        if (f < a.nfields) {
+            // staging layout: plain length-n arrays; user layout: scalars length n, vectors (n,3)
+            const double *src = a.src[f];
+            double v;
+            if (a.src_soa || f < 2)
+                v = src[p];
+            else
+                v = src[(size_t)3 * p];   // src already offset by the component
+            a.dst[f][addr] = v;
+        }
+    }
+}
+
+cudaError_t launch_scatter(const ScatterArgs &a, cudaStream_t st)
+{
+    if (a.n <= 0) return cudaSuccess;
+    scatter_kernel<<<(a.n + 255) / 256, 256, 0, st>>>(a);
+    return cudaGetLastError();
+}
+
+// ------------------------------------------------------------------------------------------
+// Predictor (reading P2), Horner form, fp64 FMA:
+//   4th: x_p = x + dt (v + dt/2 (a + dt/3 j));                 v_p = v + dt (a + dt/2 j)
+//   6th: x_p = x + dt (v + dt/2 (a + dt/3 (j + dt/4 (s + dt/5 c))))
+//        v_p = v + dt (a + dt/2 (j + dt/3 (s + dt/4 c)));      a_p = a + dt (j + dt/2 (s + dt/3 c))
+// One thread per j: 14 (20) coalesced 8-byte reads + id, 4 (6) coalesced 16-byte plane writes,
+// plus the float / double-single planes when the context computes in those precisions.
+
+__device__ __forceinline__ float2 split_ds(double x)
+{
+    float hi = __double2float_rn(x);
+    float lo = __double2float_rn(x - (double)hi);
+    return make_float2(hi, lo);
+}
+
+template <int ORDER>
+__global__ void __launch_bounds__(256) predict_kernel(PredictArgs a)
+{
+    int j = blockIdx.x * blockDim.x + threadIdx.x;
+    if (j >= a.nj) return;
+    const double dt = a.t - a.f[0][j];
+    const double m = a.f[1][j];
+    const int id = a.id[j];
+    const double h2 = 0.5 * dt, h3 = dt * (1.0 / 3.0);
+    double xp[3], vp[3], ap[3];
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+        const double x = a.f[2 + c][j], v = a.f[5 + c][j], ac = a.f[8 + c][j], jk = a.f[11 + c][j];
+        if (ORDER == 4) {
+            xp[c] = fma(dt, fma(h2, fma(h3, jk, ac), v), x);
+            vp[c] = fma(dt, fma(h2, jk, ac), v);
+            ap[c] = ac;
+        } else {
+            const double s = a.f[14 + c][j], cr = a.f[17 + c][j];
+            const double h4 = 0.25 * dt, h5 = 0.2 * dt;
+            xp[c] = fma(dt, fma(h2, fma(h3, fma(h4, fma(h5, cr, s), jk), ac), v), x);
+            vp[c] = fma(dt, fma(h2, fma(h3, fma(h4, cr, s), jk), ac), v);
+            ap[c] = fma(dt, fma(h2, fma(h3, cr, s), jk), ac);
+        }
+    }
+    const double idbits = __hiloint2double(0, id);
+    a.p[0][j] = make_double2(xp[0], xp[1]);
+    a.p[1][j] = make_double2(xp[2], m);
+    a.p[2][j] = make_double2(vp[0], vp[1]);
+    a.p[3][j] = make_double2(vp[2], idbits);
+    if (ORDER == 6) {
+        a.p[4][j] = make_double2(ap[0], ap[1]);
+        a.p[5][j] = make_double2(ap[2], 0.0);
+    }
+    if (a.precision == S2_FP32) {
+        float2 X = split_ds(xp[0]), Y = split_ds(xp[1]), Z = split_ds(xp[2]);
+        a.q[0][j] = make_float4(X.x, Y.x, Z.x, __double2float_rn(m));
+        a.q[1][j] = make_float4(X.y, Y.y, Z.y, __int_as_float(id));
+        a.q[2][j] = make_float4(__double2float_rn(vp[0]), __double2float_rn(vp[1]), __double2float_rn(vp[2]), 0.f);
+        if (ORDER == 6)
+            a.q[3][j] = make_float4(__double2float_rn(ap[0]), __double2float_rn(ap[1]), __double2float_rn(ap[2]), 0.f);
+    } else if (a.precision == S2_DS) {
+        float2 X = split_ds(xp[0]), Y = split_ds(xp[1]), Z = split_ds(xp[2]), M = split_ds(m);
+        float2 U = split_ds(vp[0]), V = split_ds(vp[1]), W = split_ds(vp[2]);
+        a.q[0][j] = make_float4(X.x, X.y, Y.x, Y.y);
+        a.q[1][j] = make_float4(Z.x, Z.y, M.x, M.y);
+        a.q[2][j] = make_float4(U.x, U.y, V.x, V.y);
+        a.q[3][j] = make_float4(W.x, W.y, __int_as_float(id), 0.f);
+        if (ORDER == 6) {
+            float2 A = split_ds(ap[0]), B = split_ds(ap[1]), Cc = split_ds(ap[2]);
+            a.q[4][j] = make_float4(A.x, A.y, B.x, B.y);
+            a.q[5][j] = make_float4(Cc.x, Cc.y, 0.f, 0.f);
+        }
+    }
+}
+
+cudaError_t launch_predict(const PredictArgs &a, cudaStream_t st)
+{
+    if (a.nj <= 0) return cudaSuccess;
+    const int grid = (a.nj + 255) / 256;
+    if (a.order == 6)
+        predict_kernel<6><<<grid, 256, 0, st>>>(a);
+    else
+        predict_kernel<4><<<grid, 256, 0, st>>>(a);
+    return cudaGetLastError();
+}
+
+// ------------------------------------------------------------------------------------------
+// Peak microbenchmarks (roofline denominators): 8 independent FMA chains per thread.
+template <typename T>
+__global__ void __launch_bounds__(256) peak_fma_kernel(T *out, int iters, T seed)
+{
+    T a0 = seed + threadIdx.x, a1 = a0 + 1, a2 = a0 + 2, a3 = a0 + 3, a4 = a0 + 4, a5 = a0 + 5, a6 = a0 + 6, a7 = a0 + 7;
+    const T b = (T)0.999999, c = (T)1e-7;
+    for (int i = 0; i < iters; ++i) {
+#pragma unroll
+        for (int u = 0; u < 16; ++u) {
+            a0 = fma(a0, b, c); a1 = fma(a1, b, c); a2 = fma(a2, b, c); a3 = fma(a3, b, c);
+            a4 = fma(a4, b, c); a5 = fma(a5, b, c); a6 = fma(a6, b, c); a7 = fma(a7, b, c);
+        }
+    }
+    T s = a0 + a1 + a2 + a3 + a4 + a5 + a6 + a7;
+    if (s == (T)123456.789) out[blockIdx.x * blockDim.x + threadIdx.x] = s;   // never true; keeps the chains live
+}
+
+cudaError_t run_peak_fma(int kind, int iters, int sm_count, cudaStream_t st, double *fma_per_s)
+{
+    cudaEvent_t e0, e1;
+    cudaError_t err;
+    if ((err = cudaEventCreate(&e0)) != cudaSuccess) return err;
+    if ((err = cudaEventCreate(&e1)) != cudaSuccess) return err;
+    const int grid = sm_count * 8, block = 256;   // 64 warps per SM
+    void *dummy = nullptr;
+    for (int rep = 0; rep < 2; ++rep) {           // first pass warms up
+        if (rep == 1) cudaEventRecord(e0, st);
+        if (kind == 0)
+            peak_fma_kernel<double><<<grid, block, 0, st>>>((double *)dummy, iters, 1.0);
+        else
+            peak_fma_kernel<float><<<grid, block, 0, st>>>((float *)dummy, iters, 1.0f);
+    }
+    cudaEventRecord(e1, st);
+    err = cudaEventSynchronize(e1);
+    if (err == cudaSuccess) err = cudaGetLastError();
+    float ms = 0.f;
+    cudaEventElapsedTime(&ms, e0, e1);
+    cudaEventDestroy(e0);
+    cudaEventDestroy(e1);
+    if (err != cudaSuccess) return err;
+    const double fmas = (double)grid * block * (double)iters * 16.0 * 8.0;
+    *fma_per_s = fmas / (ms * 1e-3);
+    return cudaSuccess;
+}
+
+}  // namespace s2

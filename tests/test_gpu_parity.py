@@ -1,0 +1,284 @@
+"""GPU parity tests: the CUDA library (through the C ABI) against the CPU oracle, element by
+element, on the same seeded inputs.  Run on the B200 box with  pytest -m gpu."""
+import numpy as np
+import pytest
+
+import oracle
+import paper_1510_04068_b200 as s2
+from workloads import make_config, lattice_workload
+
+from gpu_util import (TOL, check_forces, check_neighbour_lists, open_and_load, oracle_on_gpu_prediction, rel_err)
+
+pytestmark = pytest.mark.gpu
+
+NN, NGB = s2.S2_WANT_NN, s2.S2_WANT_NGB
+
+
+# ------------------------------------------------------------------------------- a1 / a2
+@pytest.mark.parametrize("cfg,order,N", [(1, 4, 1024), (4, 6, 5000)])
+def test_commit_roundtrip_and_predictor(cfg, order, N):
+    w = make_config(cfg, N=N)
+    ctx = open_and_load(w, order, chunks=3)
+    ident, t, mass, pos = s2.s2_get_j(ctx, 0, N)
+    assert np.array_equal(ident, w.ident) and np.array_equal(t, w.t_j)
+    assert np.array_equal(mass, w.mass) and np.array_equal(pos, w.pos)
+    s2.s2_predict(ctx, w.t_pred, N)
+    xp, vp, ap = s2.s2_get_predicted_j(ctx, 0, N)
+    oxp, ovp, oap = oracle.predict(order, w.t_pred, w.t_j, w.pos, w.vel, w.acc, w.jerk, w.snap, w.crackle)
+    # reading P1(i): within 2 ulp of the magnitude of the Taylor terms
+    dt = (w.t_pred - w.t_j)[:, None]
+    u = 2.0 ** -52
+    mx = np.abs(w.pos) + np.abs(w.vel * dt) + np.abs(w.acc * dt ** 2 / 2) + np.abs(w.jerk * dt ** 3 / 6)
+    mv = np.abs(w.vel) + np.abs(w.acc * dt) + np.abs(w.jerk * dt ** 2 / 2)
+    if order == 6:
+        mx += np.abs(w.snap * dt ** 4 / 24) + np.abs(w.crackle * dt ** 5 / 120)
+        mv += np.abs(w.snap * dt ** 3 / 6) + np.abs(w.crackle * dt ** 4 / 24)
+        ma = np.abs(w.acc) + np.abs(w.jerk * dt) + np.abs(w.snap * dt ** 2 / 2) + np.abs(w.crackle * dt ** 3 / 6)
+        assert (np.abs(ap - oap) <= 2 * u * ma).all()
+    assert (np.abs(xp - oxp) <= 2 * u * mx).all()
+    assert (np.abs(vp - ovp) <= 2 * u * mv).all()
+    # dt = 0 returns the input bit-exactly; a second commit of a subset overwrites only that subset
+    sub = np.arange(0, N, 7, dtype=np.int32)
+    s2.s2_set_j(ctx, sub, w.ident[sub], np.full(sub.size, 0.5), w.mass[sub], w.pos[sub] + 1.0, w.vel[sub], w.acc[sub],
+                w.jerk[sub], w.snap[sub] if order == 6 else None, w.crackle[sub] if order == 6 else None)
+    s2.s2_commit_j(ctx)
+    s2.s2_predict(ctx, 0.5, N)
+    xp2, vp2, _ = s2.s2_get_predicted_j(ctx, 0, N)
+    assert np.array_equal(xp2[sub], w.pos[sub] + 1.0) and np.array_equal(vp2[sub], w.vel[sub])
+    s2.s2_close(ctx)
+
+
+# ------------------------------------------------------------------------------- config 1
+def test_cfg1_fp64_all_active_with_nn():
+    """BASELINE config 1: N = 1024 Plummer, eps = 1e-3, all active, acc + jerk + pot + nn, fp64."""
+    w = make_config(1)
+    ctx = open_and_load(w)
+    s2.s2_predict(ctx, w.t_pred, w.N)
+    il = w.ilist(w.N)
+    s2.s2_calc_ilist(ctx, il, eps2=w.eps2, flags=NN)
+    res = s2.s2_get_results(ctx, w.N)
+    ref, _ = oracle_on_gpu_prediction(ctx, w, 4, il, w.eps2)
+    errs = check_forces(res, ref, s2.S2_FP64, 4, NN, "cfg1")
+    # end to end as well (oracle predictor + oracle forces; closest pair ~5e-3 -> P1)
+    oxp, ovp, _ = oracle.predict(4, w.t_pred, w.t_j, w.pos, w.vel, w.acc, w.jerk)
+    ref2 = oracle.forces_ilist(4, w.mass, w.ident, oxp, ovp, None, il, w.eps2)
+    assert rel_err(res["acc"], ref2.acc).max() < 1e-13 and rel_err(res["jerk"], ref2.jerk).max() < 1e-12
+    assert np.array_equal(res["nn_id"], ref2.nn_id)
+    print("cfg1 max rel errors:", {k: f"{v:.2e}" for k, v in errs.items()})
+    s2.s2_close(ctx)
+
+
+# ------------------------------------------------------------------------------- config 2
+def test_cfg2_small_n_sweep():
+    """BASELINE config 2: N = 64, eps = 1e-4, n_i = 1, 2, 4 ... 64 (j-split path at every n_i)."""
+    w = make_config(2)
+    ctx = open_and_load(w)
+    s2.s2_predict(ctx, w.t_pred, w.N)
+    for ni in (1, 2, 3, 4, 8, 16, 32, 33, 64):
+        il = w.ilist(ni)
+        s2.s2_calc_ilist(ctx, il, eps2=w.eps2, flags=NN)
+        res = s2.s2_get_results(ctx, ni)
+        ref, _ = oracle_on_gpu_prediction(ctx, w, 4, il, w.eps2)
+        check_forces(res, ref, s2.S2_FP64, 4, NN, f"cfg2 n_i={ni} shape={s2.s2_last_launch_info(ctx)}")
+    s2.s2_close(ctx)
+
+
+# ------------------------------------------------------------------------------- forced shapes
+@pytest.mark.parametrize("order", [4, 6])
+@pytest.mark.parametrize("flags", [0, NN, NN | NGB])
+def test_all_launch_shapes_ragged(order, flags):
+    """Every lanes-per-i / warp-column / slice shape on a ragged problem (N = 1000 is not a multiple
+    of any tile, n_i = 37 leaves idle lanes) against the oracle, neighbour lists included."""
+    w = make_config(4 if order == 6 else 5, N=1000, order=order)
+    ctx = open_and_load(w, order, ngb_cap=24)
+    s2.s2_predict(ctx, w.t_pred, w.N)
+    ni = 37
+    il = w.ilist(ni)
+    h2 = w.h2[il] * 0.6 if flags & NGB else None
+    ref, _ = oracle_on_gpu_prediction(ctx, w, order, il, w.eps2, h2, ngb_cap=24)
+    shapes = [(L, 1, S, tile) for L in (1, 2, 4, 8, 16, 32) for S, tile in ((1, 0), (3, 64), (13, 32))]
+    shapes += [(32, Wj, S, 0) for Wj in (2, 4, 8) for S in (1, 2, 5)]
+    for L, Wj, S, tile in shapes:
+        s2.s2_set_tuning(ctx, 1, L); s2.s2_set_tuning(ctx, 2, Wj); s2.s2_set_tuning(ctx, 0, S); s2.s2_set_tuning(ctx, 4, tile)
+        s2.s2_calc_ilist(ctx, il, h2, w.eps2, flags)
+        res = s2.s2_get_results(ctx, ni)
+        info = s2.s2_last_launch_info(ctx)
+        assert info["lanes_per_i"] == L and info["warp_columns"] == Wj
+        check_forces(res, ref, s2.S2_FP64, order, flags, f"shape {info}")
+        if flags & NGB:
+            assert res["overflow"] == bool((ref.ngb_count > 24).any())
+            check_neighbour_lists(ctx, ref, ni, 24, f"shape {info}")
+    s2.s2_close(ctx)
+
+
+def test_neighbour_overflow_and_single_list():
+    w = make_config(5, N=2048)
+    ctx = open_and_load(w, 4, ngb_cap=8)
+    s2.s2_predict(ctx, w.t_pred, w.N)
+    il = w.ilist(300)
+    h2 = w.h2[il]
+    ref, _ = oracle_on_gpu_prediction(ctx, w, 4, il, w.eps2, h2, ngb_cap=8)
+    assert (ref.ngb_count > 8).any()
+    for S in (0, 1, 7):
+        s2.s2_set_tuning(ctx, 0, S)
+        s2.s2_calc_ilist(ctx, il, h2, w.eps2, NN | NGB)
+        res = s2.s2_get_results(ctx, 300)
+        assert res["overflow"]
+        assert np.array_equal(res["ngb_count"], ref.ngb_count)      # true counts (P8)
+        check_neighbour_lists(ctx, ref, 300, 8, f"S={S}")              # the 8 lowest addresses, ascending
+        k = int(np.argmax(ref.ngb_count))
+        one = s2.s2_get_neighbours(ctx, k, 5)
+        assert np.array_equal(one, ref.ngb_list[k][:5])
+    s2.s2_close(ctx)
+
+
+# ------------------------------------------------------------------------------- config 3
+@pytest.mark.parametrize("ni", [1, 32, 256, 2048, 16384, 65536])
+def test_cfg3_blockstep_fp64(ni):
+    """BASELINE config 3 (fp64 leg): N = 65536, n_i in {1, 32, 256, 2048, 16384, 65536}, acc + jerk + pot.
+    Oracle on every i up to 2048, on a seeded sample of 2048 above that (oracle speed)."""
+    w = make_config(3)
+    ctx = open_and_load(w)
+    s2.s2_predict(ctx, w.t_pred, w.N)
+    il = w.ilist(ni)
+    s2.s2_calc_ilist(ctx, il, eps2=w.eps2, flags=0)
+    res = s2.s2_get_results(ctx, ni)
+    pick = np.arange(ni) if ni <= 2048 else np.sort(np.random.default_rng(3).choice(ni, 2048, replace=False))
+    ref, (xp, vp, _) = oracle_on_gpu_prediction(ctx, w, 4, il[pick], w.eps2)
+    sub = {k: (v[pick] if isinstance(v, np.ndarray) else v) for k, v in res.items()}
+    errs = check_forces(sub, ref, s2.S2_FP64, 4, 0, f"cfg3 n_i={ni} {s2.s2_last_launch_info(ctx)}")
+    print(f"cfg3 n_i={ni}", s2.s2_last_launch_info(ctx), {k: f"{v:.2e}" for k, v in errs.items()})
+    if ni == w.N:   # Newton's third law on the full GPU output
+        for q in ("acc", "jerk"):
+            tot = np.abs((w.mass[il, None] * res[q]).sum(0)).max()
+            scale = (w.mass[il] * np.linalg.norm(res[q], axis=1)).sum()
+            assert tot <= 1e-11 * scale
+    s2.s2_close(ctx)
+
+
+# ------------------------------------------------------------------------------- determinism
+def test_bit_reproducible_and_paths_agree():
+    w = make_config(3, N=8192)
+    ctx = open_and_load(w)
+    s2.s2_predict(ctx, w.t_pred, w.N)
+    il = w.ilist(96)
+    outs = {}
+    for S in (0, 1, 9):
+        s2.s2_set_tuning(ctx, 0, S)
+        runs = []
+        for _ in range(10):
+            s2.s2_calc_ilist(ctx, il, eps2=w.eps2, flags=NN)
+            r = s2.s2_get_results(ctx, 96)
+            runs.append(np.concatenate([r["acc"].ravel(), r["jerk"].ravel(), r["pot"], r["nn_r2"]]))
+        for r in runs[1:]:
+            assert np.array_equal(r, runs[0]), "results differ run to run"
+        outs[S] = runs[0]
+    assert np.allclose(outs[1], outs[9], rtol=1e-12, atol=0)
+    assert np.allclose(outs[0], outs[1], rtol=1e-12, atol=0)
+    s2.s2_close(ctx)
+
+
+# ------------------------------------------------------------------------------- ties
+def test_lattice_ties_and_strictness_gpu():
+    w = lattice_workload(4, 0.25)
+    ctx = open_and_load(w, 4, ngb_cap=32)
+    s2.s2_predict(ctx, 0.0, w.N)
+    il = w.ilist(w.N)
+    s2v = 0.25 ** 2
+    for h2v in (s2v, 2 * s2v, 2 * s2v * (1 + 2 ** -40)):
+        h2 = np.full(w.N, h2v)
+        ref, _ = oracle_on_gpu_prediction(ctx, w, 4, il, w.eps2, h2, ngb_cap=32)
+        for L in (0, 1, 8, 32):
+            s2.s2_set_tuning(ctx, 1, L)
+            s2.s2_calc_ilist(ctx, il, h2, w.eps2, NN | NGB)
+            res = s2.s2_get_results(ctx, w.N)
+            check_forces(res, ref, s2.S2_FP64, 4, NN | NGB, f"lattice h2={h2v} L={L}")
+            check_neighbour_lists(ctx, ref, w.N, 32)
+    s2.s2_close(ctx)
+
+
+# ------------------------------------------------------------------------------- explicit i, edge cases
+def test_explicit_sinks_and_degenerate_sizes():
+    w = make_config(1, N=300)
+    ctx = open_and_load(w, 4, ngb_cap=16)
+    s2.s2_predict(ctx, w.t_pred, w.N)
+    xp, vp, _ = s2.s2_get_predicted_j(ctx, 0, w.N)
+    rng = np.random.default_rng(5)
+    ni = 45
+    xi = rng.normal(size=(ni, 3)) * 0.5
+    vi = rng.normal(size=(ni, 3)) * 0.3
+    ids = np.full(ni, -1, np.int32)
+    ids[::3] = w.ident[:15]                 # some sinks coincide in id with a source: that source is skipped
+    h2 = np.full(ni, 0.05)
+    s2.s2_calc_explicit(ctx, ids, xi, vi, None, h2, w.eps2, NN | NGB)
+    res = s2.s2_get_results(ctx, ni)
+    ref = oracle.forces(4, w.mass, w.ident, xp, vp, None, ids, xi, vi, None, w.eps2, h2, 16)
+    check_forces(res, ref, s2.S2_FP64, 4, NN | NGB, "explicit")
+    check_neighbour_lists(ctx, ref, ni, 16)
+    s2.s2_close(ctx)
+
+    # N = 1 (only self): all zero, nn = -1 / +inf;  N = 2: each sees only the other
+    for N in (1, 2):
+        w = make_config(1, N=64)
+        ctx = open_and_load(w, 4, nj=N)
+        s2.s2_predict(ctx, w.t_pred, N)
+        il = np.arange(N, dtype=np.int32)
+        s2.s2_calc_ilist(ctx, il, np.full(N, 100.0), w.eps2, NN | NGB)
+        res = s2.s2_get_results(ctx, N)
+        ref, _ = oracle_on_gpu_prediction(ctx, w, 4, il, w.eps2, np.full(N, 100.0), nj=N)
+        if N == 1:
+            assert not res["acc"].any() and not res["jerk"].any() and res["pot"][0] == 0.0
+            assert res["nn_id"][0] == -1 and np.isinf(res["nn_r2"][0]) and res["ngb_count"][0] == 0
+        else:
+            check_forces(res, ref, s2.S2_FP64, 4, NN | NGB, "N=2")
+            assert list(res["ngb_count"]) == [1, 1]
+        s2.s2_close(ctx)
+
+
+def test_state_and_argument_errors():
+    w = make_config(1, N=64)
+    ctx = s2.s2_open(0, 4, s2.S2_FP64, nj_capacity=64, ngb_cap=0)
+    with pytest.raises(s2.S2Error) as e:
+        s2.s2_predict(ctx, 0.0, 64)
+    assert e.value.code == s2.S2_ESTATE
+    with pytest.raises(s2.S2Error) as e:
+        s2.s2_set_j(ctx, np.array([64], np.int32), w.ident[:1], w.t_j[:1], w.mass[:1], w.pos[:1], w.vel[:1], w.acc[:1], w.jerk[:1])
+    assert e.value.code == s2.S2_ERANGE
+    a = np.arange(64, dtype=np.int32)
+    s2.s2_set_j(ctx, a, w.ident, w.t_j, w.mass, w.pos, w.vel, w.acc, w.jerk)
+    with pytest.raises(s2.S2Error) as e:      # staged but not committed
+        s2.s2_predict(ctx, 0.0, 64)
+    assert e.value.code == s2.S2_ESTATE
+    s2.s2_commit_j(ctx)
+    with pytest.raises(s2.S2Error) as e:
+        s2.s2_calc_ilist(ctx, a[:4], eps2=1e-4)
+    assert e.value.code == s2.S2_ESTATE
+    s2.s2_predict(ctx, 0.0, 64)
+    with pytest.raises(s2.S2Error) as e:
+        s2.s2_get_results(ctx, 4)
+    assert e.value.code == s2.S2_ESTATE
+    with pytest.raises(s2.S2Error) as e:      # neighbour lists need ngb_cap > 0 and h2
+        s2.s2_calc_ilist(ctx, a[:4], np.ones(4), 1e-4, NGB)
+    assert e.value.code == s2.S2_EINVAL
+    with pytest.raises(s2.S2Error) as e:
+        s2.s2_calc_ilist(ctx, np.array([70], np.int32), eps2=1e-4)
+    assert e.value.code == s2.S2_ERANGE
+    s2.s2_calc_ilist(ctx, a[:4], eps2=1e-4)
+    assert s2.s2_get_results(ctx, 4)["pot"].shape == (4,)
+    assert s2.s2_kernel_launches(ctx) >= 3
+    s2.s2_close(ctx)
+
+
+# ------------------------------------------------------------------------------- config 4 (6th order)
+def test_cfg4_sixth_order_ni1024():
+    """BASELINE config 4: N = 262144 Salpeter Plummer, 6th order fp64, n_i = 1024 (full oracle)."""
+    w = make_config(4)
+    ctx = open_and_load(w, 6)
+    s2.s2_predict(ctx, w.t_pred, w.N)
+    il = w.ilist(1024)
+    s2.s2_calc_ilist(ctx, il, eps2=w.eps2)
+    res = s2.s2_get_results(ctx, 1024)
+    ref, _ = oracle_on_gpu_prediction(ctx, w, 6, il, w.eps2)
+    errs = check_forces(res, ref, s2.S2_FP64, 6, 0, f"cfg4 n_i=1024 {s2.s2_last_launch_info(ctx)}")
+    print("cfg4 n_i=1024", s2.s2_last_launch_info(ctx), {k: f"{v:.2e}" for k, v in errs.items()})
+    s2.s2_close(ctx)
