@@ -1,0 +1,324 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the direct-summation Hermite force path on B200.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--no-sweep]
+
+Metric (BASELINE.json): pair interactions per second (Ginteractions/s) and fraction of the FP64
+roofline.  Workload at N = 1 GPU: the north_star headline point -- N = n_i = 2^18 equal-mass
+Plummer sphere, eps = 1e-4, 4th-order Hermite, fp64, acc + jerk + pot (it fits one GPU).
+
+One "step" is one pass of the whole hot path: commit all N j-particles,
+predict them to t, force sweep for the i-list (+ deterministic reduce), results available.
+  value : inputs already resident in HBM (s2_commit_j_device / s2_calc_ilist_device), device timed.
+  e2e   : the same step through the host-buffer C-ABI calls (s2_set_j + s2_commit_j + s2_predict +
+          s2_calc_ilist + s2_get_results), H2D / D2H copies inside the timed region.
+Timing: CUDA events around every step on the library's stream, L2 flushed between steps,
+max over ranks.  --impl reference times the CPU oracle (as it stands) on a bounded sample.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import statistics
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+FLOP_PER_PAIR = {4: 60, 6: 97}          # stated convention (reading P16)
+FP64_INSTR_PER_PAIR = {4: 32, 6: 54}    # FP64-pipe instructions per pair in the SASS of the sweep (profiles/)
+SM_COUNT, FP64_LANES_PER_SM, SM_MAX_HZ = 148, 64, 1.965e9
+FP64_PEAK_TFLOPS = SM_COUNT * FP64_LANES_PER_SM * 2 * SM_MAX_HZ / 1e12     # 37.2
+# dram__bytes_read.sum + dram__bytes_write.sum of one force-sweep launch at the headline point,
+# from the ncu --set full capture summarised in profiles/ (None until a capture exists)
+FORCE_KERNEL_DRAM_BYTES = None
+
+
+def parse_args():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--no-sweep", action="store_true", help="skip the n_i sweep and the peak microbenchmarks")
+    ap.add_argument("--workload", default="H", help="config key: H (headline), 3, 4, 5 ...")
+    ap.add_argument("--N", type=int, default=0, help="override N (reduced sizes are for debugging only)")
+    return ap.parse_args()
+
+
+# ------------------------------------------------------------------------------------------- clocks
+class ClockSampler:
+    """Samples nvidia-smi clocks and throttle reasons during the timed region."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.index, self.rows, self.proc = index, [], None
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
+                                          "-i", str(self.index), "-lms", "100"], stdout=subprocess.PIPE, text=True)
+            threading.Thread(target=self._read, daemon=True).start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append([x.strip() for x in line.split(",")])
+
+    def stop(self) -> dict:
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        self.proc.terminate()
+        sm, mx, reasons = [], [], set()
+        for r in self.rows:
+            try:
+                sm.append(float(r[0])); mx.append(float(r[1]))
+            except Exception:
+                continue
+            for name, v in zip(("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"), r[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(name)
+        return {"sm_mhz": statistics.median(sm) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "samples": len(sm), "reasons": sorted(reasons)}
+
+
+# ------------------------------------------------------------------------------------------- reference arm
+def run_reference(args, w, rank, world):
+    """The CPU oracle, as it stands, on the host cores: each step = a bounded sample of the workload."""
+    if rank != 0:
+        return
+    import oracle
+    order = w.order
+    xp, vp, ap = oracle.predict(order, w.t_pred, w.t_j, w.pos, w.vel, w.acc, w.jerk, w.snap, w.crackle)
+    n_s = max(8, min(w.N, int(6.0e7 // w.N)))          # ~6e7 pairs per step
+    il = w.ilist(n_s)
+    times = []
+    for k in range(args.warmup + args.steps):
+        t0 = time.perf_counter()
+        oracle.predict(order, w.t_pred, w.t_j[:n_s], w.pos[:n_s], w.vel[:n_s], w.acc[:n_s], w.jerk[:n_s],
+                       w.snap[:n_s], w.crackle[:n_s])
+        oracle.forces_ilist(order, w.mass, w.ident, xp, vp, ap, il, w.eps2)
+        if k >= args.warmup:
+            times.append(time.perf_counter() - t0)
+    ms = 1e3 * sum(times) / len(times)
+    val = n_s * w.N / (ms * 1e-3) / 1e9
+    sample = f"{n_s} of {w.N} i-particles (seeded prefix of the active-set permutation) x all {w.N} j per step"
+    line = {"impl": "reference", "metric": "Ginteractions/s", "value": val, "unit": "Ginteractions/s",
+            "n_gpus": args.gpus, "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms,
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f80 (x87 long double)",
+            "data": "synthetic", "config": workload_config(w, w.N),
+            "cpu_baseline": {"value": val, "unit": "Ginteractions/s", "cores": oracle.max_threads(),
+                             "kind": "oracle", "sample": sample},
+            "e2e": {"value": val, "unit": "Ginteractions/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line), flush=True)
+
+
+def workload_config(w, ni):
+    return {"workload": f"{w.name}: Plummer sphere N={w.N}, n_i={ni}, {w.order}th-order Hermite, "
+                        f"eps={w.notes['eps']:.4g}, {'Salpeter' if w.notes['salpeter'] else 'equal'} masses, "
+                        f"acc+jerk{'+snap' if w.order == 6 else ''}+pot",
+            "N": w.N, "n_i": ni, "order": w.order, "precision": "fp64", "seed": w.seed,
+            "l2": "L2 flushed (256 MiB write) between timed steps; the predicted j-store (16 MiB) is re-read "
+                  "from L2 inside a step by design",
+            "parallelism": "j-store replicated, i-lists per rank (no data-path collective)"}
+
+
+# ------------------------------------------------------------------------------------------- our arm
+def main():
+    args = parse_args()
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+
+    from workloads import make_config
+    key = int(args.workload) if args.workload.isdigit() else args.workload
+    w = make_config(key, N=args.N or None)
+
+    if args.impl == "reference":
+        run_reference(args, w, rank, world)
+        return
+
+    import torch
+    import torch.distributed as dist
+    import paper_1510_04068_b200 as s2
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the library has no CPU fallback")
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+
+    order, N, ni = w.order, w.N, w.N
+    # i-list of this rank: its own rotation of the seeded permutation (same per-GPU work on every rank)
+    il_host = np.ascontiguousarray(np.roll(w.perm, -rank * (N // max(world, 1)))[:ni])
+
+    ctx = s2.s2_open(local, order, s2.S2_FP64, nj_capacity=N, ngb_cap=0)
+    s2.s2_enable_timing(ctx, True)
+    addr = np.arange(N, dtype=np.int32)
+    host = dict(address=addr, ident=w.ident, t=w.t_j, mass=w.mass, pos=w.pos, vel=w.vel, acc=w.acc, jerk=w.jerk,
+                snap=w.snap if order == 6 else None, crackle=w.crackle if order == 6 else None)
+    d = {k: (torch.from_numpy(v).to(dev) if v is not None else None) for k, v in host.items()}
+    d_il = torch.from_numpy(il_host).to(dev)
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)
+
+    def step_resident():
+        s2.s2_commit_j_device(ctx, d["address"], d["ident"], d["t"], d["mass"], d["pos"], d["vel"], d["acc"], d["jerk"],
+                              d["snap"], d["crackle"])
+        s2.s2_predict(ctx, w.t_pred, N)
+        s2.s2_calc_ilist_device(ctx, d_il, None, w.eps2, 0)
+
+    def step_e2e():
+        s2.s2_set_j(ctx, host["address"], host["ident"], host["t"], host["mass"], host["pos"], host["vel"], host["acc"],
+                    host["jerk"], host["snap"], host["crackle"])
+        s2.s2_commit_j(ctx)
+        s2.s2_predict(ctx, w.t_pred, N)
+        s2.s2_calc_ilist(ctx, il_host, None, w.eps2, 0)
+        return s2.s2_get_results(ctx, ni)
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    def timed(fn, steps, warmup, collect_kernel_times=False):
+        for _ in range(warmup):
+            fn()
+        torch.cuda.synchronize()
+        ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(steps)]
+        ktimes = []
+        barrier()
+        l0 = s2.s2_kernel_launches(ctx)
+        for a, b in ev:
+            flush.zero_()
+            a.record()
+            fn()
+            b.record()
+            if collect_kernel_times:
+                ktimes.append(s2.s2_get_timing(ctx))     # synchronises; outside the event pair
+        barrier()
+        launches = s2.s2_kernel_launches(ctx) - l0
+        ms = [a.elapsed_time(b) for a, b in ev]
+        return sum(ms), launches, ktimes
+
+    sampler = ClockSampler(local)
+    sampler.start()
+    tot_ms, launches, ktimes = timed(step_resident, args.steps, max(args.warmup, 3), True)
+    clocks = sampler.stop()
+    e2e_ms, _, _ = timed(step_e2e, args.steps, 1)
+
+    t = torch.tensor([tot_ms, e2e_ms], dtype=torch.float64, device=dev)
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    tot_ms, e2e_ms = float(t[0]), float(t[1])
+    pairs_step = float(ni) * N * world
+    value = pairs_step * args.steps / (tot_ms * 1e-3) / 1e9
+    e2e_value = pairs_step * args.steps / (e2e_ms * 1e-3) / 1e9
+
+    nf = 20 if order == 6 else 14
+    h2d = N * (nf * 8 + 8) + ni * 4
+    d2h = ni * 96 + 8
+
+    force_ms = statistics.mean(k["force_ms"] for k in ktimes)
+    achieved = ni * N * FLOP_PER_PAIR[order] / (force_ms * 1e-3) / 1e12
+    roofline = {"bound": "alu", "kernel": "force_sweep_kernel<PolicyF64>", "achieved": achieved,
+                "peak": FP64_PEAK_TFLOPS, "unit": "TFLOP/s", "frac": achieved / FP64_PEAK_TFLOPS,
+                "traffic": FORCE_KERNEL_DRAM_BYTES,
+                "peak_source": "derived: 148 SM x 64 FP64 FMA lanes x 2 flop x 1.965 GHz (DESIGN.md); not in MEASURED_PEAKS.json",
+                "convention": f"{FLOP_PER_PAIR[order]} flop per pair interaction (labelled convention, reading P16)",
+                "kernel_ms": force_ms, "kernel_share_of_step": force_ms * args.steps / tot_ms,
+                "fp64_instr_per_pair": FP64_INSTR_PER_PAIR[order],
+                "fp64_pipe_frac_nominal": ni * N * FP64_INSTR_PER_PAIR[order] / (force_ms * 1e-3)
+                                          / (SM_COUNT * FP64_LANES_PER_SM * SM_MAX_HZ),
+                "predict_ms": statistics.mean(k["predict_ms"] for k in ktimes),
+                "reduce_ms": statistics.mean(k["reduce_ms"] for k in ktimes)}
+
+    line = {"metric": "Ginteractions/s", "value": value, "unit": "Ginteractions/s", "n_gpus": world,
+            "steps": args.steps, "warmup": max(args.warmup, 3), "ms_per_step": tot_ms / args.steps,
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": workload_config(w, ni), "clocks": clocks,
+            "e2e": {"value": e2e_value, "unit": "Ginteractions/s", "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
+                    "ms_per_step": e2e_ms / args.steps},
+            "gpu_launches": int(launches), "roofline": roofline, "launch": s2.s2_last_launch_info(ctx)}
+
+    if rank == 0 and world == 1 and not args.no_sweep:
+        # measured FMA peaks in the same process (SURVEY sec 8(d) "clock risk")
+        dfma = s2.s2_peak_fma(ctx, 0, 4000)
+        roofline["measured_dfma_tflops"] = 2 * dfma / 1e12
+        roofline["frac_of_measured_dfma_pipe"] = (ni * N * FP64_INSTR_PER_PAIR[order] / (force_ms * 1e-3)) / dfma
+        line["sweep"] = ni_sweep(s2, torch, dev, order)
+        line["cpu_baseline"] = cpu_baseline(w)
+    if rank == 0:
+        print(json.dumps(line), flush=True)
+    s2.s2_close(ctx)
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def ni_sweep(s2, torch, dev, order):
+    """Ginteractions/s versus n_i at config 3's N = 65536 and at the headline N = 2^18 (4th order fp64),
+    kernel time only (force sweep + reduce), as in the paper's Fig. 2 protocol."""
+    from workloads import make_config
+    out = []
+    for key, nis in ((3, (1, 32, 256, 2048, 16384, 65536)), ("H", (1, 32, 256, 4096, 262144))):
+        w = make_config(key)
+        ctx = s2.s2_open(dev.index, 4, s2.S2_FP64, nj_capacity=w.N, ngb_cap=0)
+        a = np.arange(w.N, dtype=np.int32)
+        s2.s2_set_j(ctx, a, w.ident, w.t_j, w.mass, w.pos, w.vel, w.acc, w.jerk)
+        s2.s2_commit_j(ctx)
+        s2.s2_predict(ctx, w.t_pred, w.N)
+        s2.s2_enable_timing(ctx, True)
+        full = None
+        rows = []
+        for ni in nis[::-1]:
+            il = torch.from_numpy(w.ilist(ni)).to(dev)
+            reps = 3 if ni * w.N > 1e9 else 20
+            ts = []
+            for r in range(reps + 2):
+                s2.s2_calc_ilist_device(ctx, il, None, w.eps2, 0)
+                t = s2.s2_get_timing(ctx)
+                if r >= 2:
+                    ts.append(t["force_ms"] + t["reduce_ms"])
+            ms = statistics.median(ts)
+            g = ni * w.N / (ms * 1e-3) / 1e9
+            full = full or g
+            info = s2.s2_last_launch_info(ctx)
+            rows.append({"N": w.N, "n_i": ni, "kernel_us": ms * 1e3, "ginteractions_per_s": g,
+                         "frac_fp64_peak_60flop": g * 60e9 / 1e12 / FP64_PEAK_TFLOPS, "vs_full_rate": g / full,
+                         "S": info["S"], "lanes_per_i": info["lanes_per_i"], "warp_columns": info["warp_columns"]})
+        out.extend(rows[::-1])
+        s2.s2_close(ctx)
+    return out
+
+
+def cpu_baseline(w):
+    """The oracle as it stands, timed on the host cores on a bounded sample of the same workload."""
+    import oracle
+    xp, vp, ap = oracle.predict(w.order, w.t_pred, w.t_j, w.pos, w.vel, w.acc, w.jerk, w.snap, w.crackle)
+    # calibrate on 64 i, then size the sample for ~10 s
+    il = w.ilist(64)
+    t0 = time.perf_counter()
+    oracle.forces_ilist(w.order, w.mass, w.ident, xp, vp, ap, il, w.eps2)
+    rate = 64 * w.N / (time.perf_counter() - t0)
+    n_s = int(min(w.N, max(64, 10.0 * rate / w.N)))
+    il = w.ilist(n_s)
+    t0 = time.perf_counter()
+    oracle.forces_ilist(w.order, w.mass, w.ident, xp, vp, ap, il, w.eps2)
+    dt = time.perf_counter() - t0
+    return {"value": n_s * w.N / dt / 1e9, "unit": "Ginteractions/s", "cores": oracle.max_threads(), "kind": "oracle",
+            "sample": f"{n_s} of {w.N} i-particles (seeded prefix of the active-set permutation) x all {w.N} j, "
+                      f"long double, {dt:.1f} s"}
+
+
+if __name__ == "__main__":
+    main()
