@@ -24,7 +24,14 @@ struct PolicyF64 {
     static constexpr int ORDER = ORDER_;
     static constexpr bool NN = NN_, NGB = NGB_;
     static constexpr int NPL = ORDER == 6 ? 6 : 4;
-    static constexpr int kMinBlocks = 2;
+#ifndef S2_F64_MINBLOCKS
+#define S2_F64_MINBLOCKS 2
+#endif
+#ifndef S2_F64_UNROLL
+#define S2_F64_UNROLL 4
+#endif
+    static constexpr int kMinBlocks = S2_F64_MINBLOCKS;
+    static constexpr int kUnroll = S2_F64_UNROLL;   // pairs in flight per thread in the one-lane-per-i loop
 
     struct IState {
         double x, y, z, vx, vy, vz, ax, ay, az, h2, eps2;
@@ -58,6 +65,8 @@ struct PolicyF64 {
             o[7] = ORDER == 6 ? sx : 0.0; o[8] = ORDER == 6 ? sy : 0.0; o[9] = ORDER == 6 ? sz : 0.0;
         }
     };
+
+    using Part = Acc;   // fp64 partial sums per tile, added to fp64 totals
 
     static __device__ __forceinline__ void load_i(const ForceArgs &a, int i, IState &I)
     {
@@ -127,31 +136,6 @@ struct PolicyF64 {
         }
     }
 };
-
-template <class P>
-static cudaError_t launch_L(int L, dim3 grid, size_t smem, const ForceArgs &a, cudaStream_t st, bool query,
-                            int *ctas_per_sm)
-{
-#define S2_CASE(LL)                                                                                          \
-    case LL: {                                                                                               \
-        auto kern = force_sweep_kernel<P, LL>;                                                               \
-        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem); \
-        if (e != cudaSuccess) return e;                                                                      \
-        if (query) return cudaOccupancyMaxActiveBlocksPerMultiprocessor(ctas_per_sm, kern, kThreads, smem);  \
-        kern<<<grid, kThreads, smem, st>>>(a);                                                               \
-        return cudaGetLastError();                                                                           \
-    }
-    switch (L) {
-        S2_CASE(1)
-        S2_CASE(2)
-        S2_CASE(4)
-        S2_CASE(8)
-        S2_CASE(16)
-        S2_CASE(32)
-    }
-#undef S2_CASE
-    return cudaErrorInvalidValue;
-}
 
 cudaError_t dispatch_force_fp64(int order, unsigned flags, int L, dim3 grid, size_t smem, const ForceArgs &a,
                                 cudaStream_t st, bool query, int *ctas_per_sm)

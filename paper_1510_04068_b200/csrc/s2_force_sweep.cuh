@@ -66,9 +66,10 @@ __device__ __forceinline__ void decide(double d2, int jaddr, bool skip, double h
 // Policy interface (see PolicyF64 in s2_force_fp64.cu):
 //   NPL, kMinBlocks, NN, NGB, ORDER
 //   struct IState; static void load_i(const ForceArgs&, int i, IState&)
-//   struct Acc { void zero(); void add(const Acc&); void shfl_add(int mask); void to_f64(double out[10]) }
+//   struct Part { void zero(); }   per-tile partial sums, updated by pair()
+//   struct Acc { void zero(); void add(const Part&); void shfl_add(int mask); void to_f64(double out[10]) }
 //   template <int L, bool MASKED> static void pair(const unsigned char *stage, int tile, int k, bool valid,
-//                                                  int jaddr, const IState&, Acc&, Dec&, const Decomp&, int *seg, int segcap)
+//                                                  int jaddr, const IState&, Part&, Dec&, const Decomp&, int *seg, int segcap)
 template <class P, int L>
 __global__ void __launch_bounds__(kThreads, P::kMinBlocks) force_sweep_kernel(const ForceArgs a)
 {
@@ -108,7 +109,8 @@ __global__ void __launch_bounds__(kThreads, P::kMinBlocks) force_sweep_kernel(co
     typename P::IState I;
     P::load_i(a, d.i, I);
 
-    typename P::Acc tot, part;
+    typename P::Acc tot;     // running totals (fp64 / double-single)
+    typename P::Part part;   // per-tile partial sums in the pair-arithmetic type
     tot.zero();
     Dec D;
     D.nn_d2 = CUDART_INF;
@@ -133,7 +135,7 @@ __global__ void __launch_bounds__(kThreads, P::kMinBlocks) force_sweep_kernel(co
         const int len = end - beg;
         part.zero();
         if (L == 1) {
-#pragma unroll 4
+#pragma unroll P::kUnroll
             for (int k = beg; k < end; ++k)
                 P::template pair<L, false>(stage, tile, k, true, jt + k, I, part, D, d, seg, a.segcap);
         } else {
@@ -185,6 +187,33 @@ __global__ void __launch_bounds__(kThreads, P::kMinBlocks) force_sweep_kernel(co
         r2[4] = make_double2(__hiloint2double(D.cnt, nn), out[7]);
         r2[5] = make_double2(out[8], out[9]);
     }
+}
+
+// Host side: instantiate the kernel for a policy and launch it (or query its occupancy) for the
+// run-time lane count L.
+template <class P>
+cudaError_t launch_L(int L, dim3 grid, size_t smem, const ForceArgs &a, cudaStream_t st, bool query,
+                            int *ctas_per_sm)
+{
+#define S2_CASE(LL)                                                                                          \
+    case LL: {                                                                                               \
+        auto kern = force_sweep_kernel<P, LL>;                                                               \
+        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem); \
+        if (e != cudaSuccess) return e;                                                                      \
+        if (query) return cudaOccupancyMaxActiveBlocksPerMultiprocessor(ctas_per_sm, kern, kThreads, smem);  \
+        kern<<<grid, kThreads, smem, st>>>(a);                                                               \
+        return cudaGetLastError();                                                                           \
+    }
+    switch (L) {
+        S2_CASE(1)
+        S2_CASE(2)
+        S2_CASE(4)
+        S2_CASE(8)
+        S2_CASE(16)
+        S2_CASE(32)
+    }
+#undef S2_CASE
+    return cudaErrorInvalidValue;
 }
 
 }  // namespace s2

@@ -29,7 +29,10 @@ namespace s2 {
 constexpr int kMaxFields = 20;
 constexpr int kMaxPlanes = 8;      // up to 6 arithmetic planes + 2 fp64 position planes for decisions
 constexpr int REC = 12;            // doubles per result record (96 B = three 32-byte sectors)
-constexpr int kThreads = 256;      // threads per force CTA
+#ifndef S2_THREADS
+#define S2_THREADS 256
+#endif
+constexpr int kThreads = S2_THREADS;   // threads per force CTA
 constexpr int kWarps = kThreads / 32;
 
 inline int nfields(int order) { return order == 6 ? 20 : 14; }
