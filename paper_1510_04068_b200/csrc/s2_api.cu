@@ -500,11 +500,15 @@ static int choose_shape(s2_ctx *ctx, int ni, int nj, unsigned flags, ForceShape 
         }
     }
     if (S < 1 || S > 65535) return S2_EINVAL;
+    // largest tile whose two stages fit the 227 KB of shared memory one CTA may use
+    const int tile_max = std::min(2048, (int)((232448 - kSmemHeader) / (2 * npl * 16)) / 32 * 32);
+    if (tile > tile_max) return S2_EINVAL;
+    if (Wj > 1 && (nj + S - 1) / S > tile_max) S = (nj + tile_max - 1) / tile_max;   // one tile per CTA
     int slice_len = (nj + S - 1) / S;
     S = (nj + slice_len - 1) / slice_len;
+    if (S > 65535) return S2_EINVAL;
     if (Wj > 1) {
         tile = std::max(32, (slice_len + 31) / 32 * 32);
-        if (tile > 2048) return S2_EINVAL;
     } else if (slice_len < tile) {
         tile = std::max(32, (slice_len + 31) / 32 * 32);
     }

@@ -1,0 +1,162 @@
+// s2_force_fp32.cu -- single-precision pair arithmetic for the force sweep (j-particles
+// "converted to either float or double-single" on the device; L128-L132).
+//
+// Reading P10: "plain fp32" keeps every pair operation in fp32, but
+//   (a) positions are held as (hi, lo) float pairs and r is formed as (hi_j - hi_i) + (lo_j - lo_i), so the
+//       separation of a close pair does not inherit the 6e-8 |x| rounding of a float coordinate;
+//   (b) a thread sums in fp32 only over one j tile (<= 256 terms); tile sums are added to fp64 totals.
+// The two integer decisions (nearest neighbour, neighbour test) use the fp64 squared distance formed from
+// the fp64 predicted positions (planes P0, P1 staged next to the float planes) in every precision mode.
+//
+// j planes (float4 per particle): F0 (x_hi, y_hi, z_hi, m)  F1 (x_lo, y_lo, z_lo, id bits)  F2 (vx, vy, vz, 0)
+//                                 [6th order: F3 (ax, ay, az, 0)]  [NN/NGB: P0 (x, y) P1 (z, m) as double2]
+#include "s2_force_sweep.cuh"
+
+namespace s2 {
+
+__device__ __forceinline__ float rsqrt_f32(float s)
+{
+    float y;
+    asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(s));   // MUFU.RSQ, <= 2^-22.4 relative
+    return y;
+}
+
+template <int ORDER_, bool NN_, bool NGB_>
+struct PolicyF32 {
+    static constexpr int ORDER = ORDER_;
+    static constexpr bool NN = NN_, NGB = NGB_;
+    static constexpr bool DEC = NN || NGB;
+    static constexpr int NQ = ORDER == 6 ? 4 : 3;     // float planes
+    static constexpr int NPL = NQ + (DEC ? 2 : 0);    // + fp64 position planes for the decisions
+    static constexpr int kMinBlocks = 2;
+    static constexpr int kUnroll = 4;
+
+    struct IState {
+        float xh, yh, zh, xl, yl, zl, vx, vy, vz, ax, ay, az, eps2;
+        double x, y, z, h2;   // fp64 position for the decisions
+        int id;
+    };
+
+    struct Part {   // fp32 sums over one tile
+        float ax, ay, az, jx, jy, jz, pot, sx, sy, sz;
+        __device__ __forceinline__ void zero()
+        {
+            ax = ay = az = jx = jy = jz = pot = 0.f;
+            if (ORDER == 6) sx = sy = sz = 0.f;
+        }
+    };
+
+    struct Acc {    // fp64 totals
+        double ax, ay, az, jx, jy, jz, pot, sx, sy, sz;
+        __device__ __forceinline__ void zero()
+        {
+            ax = ay = az = jx = jy = jz = pot = 0.0;
+            if (ORDER == 6) sx = sy = sz = 0.0;
+        }
+        __device__ __forceinline__ void add(const Part &o)
+        {
+            ax += (double)o.ax; ay += (double)o.ay; az += (double)o.az;
+            jx += (double)o.jx; jy += (double)o.jy; jz += (double)o.jz;
+            pot += (double)o.pot;
+            if (ORDER == 6) { sx += (double)o.sx; sy += (double)o.sy; sz += (double)o.sz; }
+        }
+        __device__ __forceinline__ void shfl_add(int m)
+        {
+            ax += shfl_xor_d(ax, m); ay += shfl_xor_d(ay, m); az += shfl_xor_d(az, m);
+            jx += shfl_xor_d(jx, m); jy += shfl_xor_d(jy, m); jz += shfl_xor_d(jz, m);
+            pot += shfl_xor_d(pot, m);
+            if (ORDER == 6) { sx += shfl_xor_d(sx, m); sy += shfl_xor_d(sy, m); sz += shfl_xor_d(sz, m); }
+        }
+        __device__ __forceinline__ void to_f64(double o[10]) const
+        {
+            o[0] = ax; o[1] = ay; o[2] = az; o[3] = jx; o[4] = jy; o[5] = jz; o[6] = pot;
+            o[7] = ORDER == 6 ? sx : 0.0; o[8] = ORDER == 6 ? sy : 0.0; o[9] = ORDER == 6 ? sz : 0.0;
+        }
+    };
+
+    static __device__ __forceinline__ void load_i(const ForceArgs &a, int i, IState &I)
+    {
+        const int ia = a.i_addr ? a.i_addr[i] : i;
+        const float4 f0 = static_cast<const float4 *>(a.ip[0])[ia];
+        const float4 f1 = static_cast<const float4 *>(a.ip[1])[ia];
+        const float4 f2 = static_cast<const float4 *>(a.ip[2])[ia];
+        I.xh = f0.x; I.yh = f0.y; I.zh = f0.z;
+        I.xl = f1.x; I.yl = f1.y; I.zl = f1.z;
+        I.id = __float_as_int(f1.w);
+        I.vx = f2.x; I.vy = f2.y; I.vz = f2.z;
+        if (ORDER == 6) {
+            const float4 f3 = static_cast<const float4 *>(a.ip[3])[ia];
+            I.ax = f3.x; I.ay = f3.y; I.az = f3.z;
+        }
+        if (DEC) {
+            const double2 p0 = static_cast<const double2 *>(a.ip[NQ])[ia];
+            const double2 p1 = static_cast<const double2 *>(a.ip[NQ + 1])[ia];
+            I.x = p0.x; I.y = p0.y; I.z = p1.x;
+        }
+        I.h2 = (NGB && a.h2) ? a.h2[i] : 0.0;
+        I.eps2 = (float)a.eps2;
+    }
+
+    template <int L, bool MASKED>
+    static __device__ __forceinline__ void pair(const unsigned char *stage, int tile, int k, bool valid, int jaddr,
+                                                const IState &I, Part &A, Dec &D, const Decomp &d, int *seg,
+                                                int segcap)
+    {
+        const float4 *pl = reinterpret_cast<const float4 *>(stage);
+        const float4 f0 = pl[k], f1 = pl[tile + k], f2 = pl[2 * tile + k];
+        const bool skip = (__float_as_int(f1.w) == I.id) || (MASKED && !valid);
+
+        if (DEC) {
+            const double2 *pd = reinterpret_cast<const double2 *>(stage);
+            const double2 p0 = pd[NQ * tile + k], p1 = pd[(NQ + 1) * tile + k];
+            const double ex = p0.x - I.x, ey = p0.y - I.y, ez = p1.x - I.z;
+            const double d2 = __fma_rn(ez, ez, __fma_rn(ey, ey, __dmul_rn(ex, ex)));
+            decide<L, NN, NGB>(d2, jaddr, skip, I.h2, D, d, seg, segcap);
+        }
+
+        const float dx = (f0.x - I.xh) + (f1.x - I.xl);
+        const float dy = (f0.y - I.yh) + (f1.y - I.yl);
+        const float dz = (f0.z - I.zh) + (f1.z - I.zl);
+        const float dvx = f2.x - I.vx, dvy = f2.y - I.vy, dvz = f2.z - I.vz;
+        const float s = fmaf(dz, dz, fmaf(dy, dy, fmaf(dx, dx, I.eps2)));
+        const float rv = fmaf(dz, dvz, fmaf(dy, dvy, dx * dvx));
+        float y = rsqrt_f32(s);
+        y = skip ? 0.f : y;
+        const float y2 = y * y;
+        const float my = f0.w * y;
+        const float q = my * y2;
+        A.pot -= my;
+        const float alpha = rv * y2;
+        const float a3 = -3.f * alpha;
+        const float tx = fmaf(a3, dx, dvx), ty = fmaf(a3, dy, dvy), tz = fmaf(a3, dz, dvz);
+        A.ax = fmaf(q, dx, A.ax); A.ay = fmaf(q, dy, A.ay); A.az = fmaf(q, dz, A.az);
+        A.jx = fmaf(q, tx, A.jx); A.jy = fmaf(q, ty, A.jy); A.jz = fmaf(q, tz, A.jz);
+        if (ORDER == 6) {
+            const float4 f3 = pl[3 * tile + k];
+            const float dax = f3.x - I.ax, day = f3.y - I.ay, daz = f3.z - I.az;
+            const float w = fmaf(dvx, dvx, fmaf(dvy, dvy, fmaf(dvz, dvz, fmaf(dx, dax, fmaf(dy, day, dz * daz)))));
+            const float b3 = -3.f * fmaf(w, y2, alpha * alpha);
+            const float a6 = a3 + a3;
+            const float ux = fmaf(a6, tx, fmaf(b3, dx, dax));
+            const float uy = fmaf(a6, ty, fmaf(b3, dy, day));
+            const float uz = fmaf(a6, tz, fmaf(b3, dz, daz));
+            A.sx = fmaf(q, ux, A.sx); A.sy = fmaf(q, uy, A.sy); A.sz = fmaf(q, uz, A.sz);
+        }
+    }
+};
+
+cudaError_t dispatch_force_fp32(int order, unsigned flags, int L, dim3 grid, size_t smem, const ForceArgs &a,
+                                cudaStream_t st, bool query, int *ctas_per_sm)
+{
+    const bool ngb = flags & S2_WANT_NGB, nn = (flags & S2_WANT_NN) || ngb;
+    if (order == 4) {
+        if (ngb) return launch_L<PolicyF32<4, true, true>>(L, grid, smem, a, st, query, ctas_per_sm);
+        if (nn) return launch_L<PolicyF32<4, true, false>>(L, grid, smem, a, st, query, ctas_per_sm);
+        return launch_L<PolicyF32<4, false, false>>(L, grid, smem, a, st, query, ctas_per_sm);
+    }
+    if (ngb) return launch_L<PolicyF32<6, true, true>>(L, grid, smem, a, st, query, ctas_per_sm);
+    if (nn) return launch_L<PolicyF32<6, true, false>>(L, grid, smem, a, st, query, ctas_per_sm);
+    return launch_L<PolicyF32<6, false, false>>(L, grid, smem, a, st, query, ctas_per_sm);
+}
+
+}  // namespace s2

@@ -14,14 +14,4 @@ int force_nplanes(int precision, int order, unsigned flags)
     return 0;
 }
 
-// placeholders until the fp32 / double-single sweeps land
-cudaError_t dispatch_force_fp32(int, unsigned, int, dim3, size_t, const ForceArgs &, cudaStream_t, bool, int *)
-{
-    return cudaErrorNotSupported;
-}
-cudaError_t dispatch_force_ds(int, unsigned, int, dim3, size_t, const ForceArgs &, cudaStream_t, bool, int *)
-{
-    return cudaErrorNotSupported;
-}
-
 }  // namespace s2

@@ -1,0 +1,168 @@
+"""GPU parity of the double-single and fp32 force paths, and the large configurations (4, 5), against the
+CPU oracle through the C ABI.  Tolerances: BASELINE.json north_star (max over i): DS 1e-10, fp32 1e-5;
+nearest neighbour and neighbour sets exact in every mode (decisions are taken in fp64, reading P13)."""
+import numpy as np
+import pytest
+
+import oracle
+import paper_1510_04068_b200 as s2
+from workloads import make_config, lattice_workload
+
+from gpu_util import check_forces, check_neighbour_lists, open_and_load, oracle_on_gpu_prediction
+
+pytestmark = pytest.mark.gpu
+
+NN, NGB = s2.S2_WANT_NN, s2.S2_WANT_NGB
+PREC = {"ds": s2.S2_DS, "fp32": s2.S2_FP32}
+
+
+@pytest.mark.parametrize("prec", ["ds", "fp32"])
+@pytest.mark.parametrize("order", [4, 6])
+@pytest.mark.parametrize("flags", [0, NN | NGB])
+def test_precision_paths_all_shapes_ragged(prec, order, flags):
+    """Every launch shape on a ragged problem (N = 1000, n_i = 37), both orders, with and without the
+    decision outputs, in double-single and fp32."""
+    P = PREC[prec]
+    w = make_config(4 if order == 6 else 5, N=1000, order=order)
+    ctx = open_and_load(w, order, precision=P, ngb_cap=24)
+    s2.s2_predict(ctx, w.t_pred, w.N)
+    ni = 37
+    il = w.ilist(ni)
+    h2 = w.h2[il] * 0.6 if flags & NGB else None
+    ref, _ = oracle_on_gpu_prediction(ctx, w, order, il, w.eps2, h2, ngb_cap=24)
+    shapes = [(L, 1, S, tile) for L in (1, 2, 4, 8, 16, 32) for S, tile in ((1, 0), (3, 64), (13, 32))]
+    shapes += [(32, Wj, S, 0) for Wj in (2, 8) for S in (1, 5)]
+    worst = {}
+    for L, Wj, S, tile in shapes:
+        s2.s2_set_tuning(ctx, 1, L); s2.s2_set_tuning(ctx, 2, Wj); s2.s2_set_tuning(ctx, 0, S); s2.s2_set_tuning(ctx, 4, tile)
+        s2.s2_calc_ilist(ctx, il, h2, w.eps2, flags)
+        res = s2.s2_get_results(ctx, ni)
+        info = s2.s2_last_launch_info(ctx)
+        errs = check_forces(res, ref, P, order, flags, f"{prec} shape {info}")
+        for k, v in errs.items():
+            worst[k] = max(worst.get(k, 0.0), v)
+        if flags & NGB:
+            check_neighbour_lists(ctx, ref, ni, 24, f"{prec} shape {info}")
+    print(f"{prec} order {order} flags {flags}: worst rel errors", {k: f"{v:.2e}" for k, v in worst.items()})
+    s2.s2_close(ctx)
+
+
+@pytest.mark.parametrize("prec", ["ds", "fp32"])
+def test_cfg3_blockstep_ds_fp32(prec):
+    """BASELINE config 3, DS and fp32 legs: N = 65536, n_i in {1, 32, 256, 2048, 16384, 65536}."""
+    P = PREC[prec]
+    w = make_config(3)
+    ctx = open_and_load(w, 4, precision=P)
+    s2.s2_predict(ctx, w.t_pred, w.N)
+    for ni in (1, 32, 256, 2048, 16384, 65536):
+        il = w.ilist(ni)
+        s2.s2_calc_ilist(ctx, il, eps2=w.eps2, flags=0)
+        res = s2.s2_get_results(ctx, ni)
+        pick = np.arange(ni) if ni <= 1024 else np.sort(np.random.default_rng(3).choice(ni, 1024, replace=False))
+        ref, _ = oracle_on_gpu_prediction(ctx, w, 4, il[pick], w.eps2)
+        sub = {k: (v[pick] if isinstance(v, np.ndarray) else v) for k, v in res.items()}
+        errs = check_forces(sub, ref, P, 4, 0, f"cfg3 {prec} n_i={ni} {s2.s2_last_launch_info(ctx)}")
+        print(f"cfg3 {prec} n_i={ni}", {k: f"{v:.2e}" for k, v in errs.items()})
+    s2.s2_close(ctx)
+
+
+@pytest.mark.parametrize("prec", ["ds", "fp32"])
+def test_lattice_ties_exact_in_every_precision(prec):
+    """Exact ties on an integer lattice: nn tie-break and the strict neighbour test must be bit-exact in
+    every precision (reading P13)."""
+    P = PREC[prec]
+    w = lattice_workload(4, 0.25)
+    ctx = open_and_load(w, 4, precision=P, ngb_cap=32)
+    s2.s2_predict(ctx, 0.0, w.N)
+    il = w.ilist(w.N)
+    s2v = 0.25 ** 2
+    for h2v in (s2v, 2 * s2v, 2 * s2v * (1 + 2 ** -40)):
+        h2 = np.full(w.N, h2v)
+        ref, _ = oracle_on_gpu_prediction(ctx, w, 4, il, w.eps2, h2, ngb_cap=32)
+        for L in (0, 1, 8, 32):
+            s2.s2_set_tuning(ctx, 1, L)
+            s2.s2_calc_ilist(ctx, il, h2, w.eps2, NN | NGB)
+            res = s2.s2_get_results(ctx, w.N)
+            check_forces(res, ref, P, 4, NN | NGB, f"lattice {prec} h2={h2v} L={L}")
+            check_neighbour_lists(ctx, ref, w.N, 32)
+    s2.s2_close(ctx)
+
+
+@pytest.mark.parametrize("prec", ["ds", "fp32"])
+def test_explicit_sinks_ds_fp32(prec):
+    P = PREC[prec]
+    w = make_config(4, N=500, order=6)
+    ctx = open_and_load(w, 6, precision=P, ngb_cap=16)
+    s2.s2_predict(ctx, w.t_pred, w.N)
+    xp, vp, ap = s2.s2_get_predicted_j(ctx, 0, w.N)
+    rng = np.random.default_rng(11)
+    ni = 45
+    xi, vi, ai = rng.normal(size=(ni, 3)) * 0.5, rng.normal(size=(ni, 3)) * 0.3, rng.normal(size=(ni, 3))
+    ids = np.full(ni, -1, np.int32)
+    ids[::3] = w.ident[:15]
+    h2 = np.full(ni, 0.05)
+    s2.s2_calc_explicit(ctx, ids, xi, vi, ai, h2, w.eps2, NN | NGB)
+    res = s2.s2_get_results(ctx, ni)
+    ref = oracle.forces(6, w.mass, w.ident, xp, vp, ap, ids, xi, vi, ai, w.eps2, h2, 16)
+    check_forces(res, ref, P, 6, NN | NGB, f"explicit {prec}")
+    check_neighbour_lists(ctx, ref, ni, 16)
+    s2.s2_close(ctx)
+
+
+def test_cfg4_sixth_order_all_active_sampled():
+    """BASELINE config 4 at n_i = N = 262144 (6.9e10 pairs): oracle on a seeded sample of 1024 i, plus
+    Newton's third law on the full GPU output."""
+    w = make_config(4)
+    ctx = open_and_load(w, 6)
+    s2.s2_predict(ctx, w.t_pred, w.N)
+    il = w.ilist(w.N)
+    s2.s2_calc_ilist(ctx, il, eps2=w.eps2)
+    res = s2.s2_get_results(ctx, w.N)
+    pick = np.sort(np.random.default_rng(4).choice(w.N, 1024, replace=False))
+    ref, _ = oracle_on_gpu_prediction(ctx, w, 6, il[pick], w.eps2)
+    sub = {k: (v[pick] if isinstance(v, np.ndarray) else v) for k, v in res.items()}
+    errs = check_forces(sub, ref, s2.S2_FP64, 6, 0, f"cfg4 n_i=N {s2.s2_last_launch_info(ctx)}")
+    print("cfg4 n_i=N sample 1024 (seed 4)", {k: f"{v:.2e}" for k, v in errs.items()})
+    for q in ("acc", "jerk", "snap"):
+        tot = np.abs((w.mass[il, None] * res[q]).sum(0)).max()
+        scale = (w.mass[il] * np.linalg.norm(res[q], axis=1)).sum()
+        assert tot <= 1e-10 * scale, (q, tot, scale)
+    s2.s2_close(ctx)
+
+
+@pytest.mark.parametrize("prec", ["fp64", "fp32"])
+def test_cfg5_neighbour_path_sampled(prec):
+    """BASELINE config 5: N = n_i = 2^20 Salpeter Plummer, nn + neighbour lists (cap 256), fp64 and fp32.
+    Oracle on a seeded sample of 512 i (sets exact); counts, overflow flag and the pot-symmetry / third-law
+    invariants on the full output."""
+    P = s2.S2_FP64 if prec == "fp64" else s2.S2_FP32
+    w = make_config(5)
+    ctx = open_and_load(w, 4, precision=P, ngb_cap=256)
+    s2.s2_predict(ctx, w.t_pred, w.N)
+    il = w.ilist(w.N)
+    h2 = w.h2[il]
+    s2.s2_calc_ilist(ctx, il, h2, w.eps2, NN | NGB)
+    res = s2.s2_get_results(ctx, w.N)
+    pick = np.sort(np.random.default_rng(5).choice(w.N, 512, replace=False))
+    ref, _ = oracle_on_gpu_prediction(ctx, w, 4, il[pick], w.eps2, h2[pick], ngb_cap=256)
+    sub = {k: (v[pick] if isinstance(v, np.ndarray) else v) for k, v in res.items()}
+    errs = check_forces(sub, ref, P, 4, NN | NGB, f"cfg5 {prec}")
+    for k, i in enumerate(pick):
+        got = s2.s2_get_neighbours(ctx, int(i), 256)
+        want = ref.ngb_list[k][ref.ngb_list[k] >= 0][:256]
+        assert np.array_equal(got, want), f"cfg5 {prec}: neighbour list of i={i}"
+    cnt = res["ngb_count"]
+    print(f"cfg5 {prec}", {k: f"{v:.2e}" for k, v in errs.items()}, "mean/max neighbour count", cnt.mean(), cnt.max(),
+          "overflows", int((cnt > 256).sum()), s2.s2_last_launch_info(ctx))
+    assert res["overflow"] == bool((cnt > 256).any())
+    assert 8 < cnt.mean() < 128
+    tol = 1e-10 if prec == "fp64" else 1e-4
+    for q in ("acc", "jerk"):
+        tot = np.abs((w.mass[il, None] * res[q]).sum(0)).max()
+        scale = (w.mass[il] * np.linalg.norm(res[q], axis=1)).sum()
+        assert tot <= tol * scale, (q, tot, scale)
+    # symmetric nearest-neighbour sanity: the nn of i has i within the same distance
+    nn = res["nn_id"]
+    inv = np.empty(w.N, np.int64); inv[il] = np.arange(w.N)
+    assert (res["nn_r2"][inv[nn]] <= res["nn_r2"]).all()
+    s2.s2_close(ctx)
