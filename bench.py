@@ -161,7 +161,8 @@ def main():
 
     order, N, ni = w.order, w.N, w.N
     # i-list of this rank: its own rotation of the seeded permutation (same per-GPU work on every rank)
-    il_host = np.ascontiguousarray(np.roll(w.perm, -rank * (N // max(world, 1)))[:ni])
+    from paper_1510_04068_b200.sharding import max_over_ranks, rank_ilist
+    il_host = rank_ilist(w.perm, rank, world, ni)
 
     ctx = s2.s2_open(local, order, s2.S2_FP64, nj_capacity=N, ngb_cap=0)
     s2.s2_enable_timing(ctx, True)
@@ -217,10 +218,7 @@ def main():
     clocks = sampler.stop()
     e2e_ms, _, _ = timed(step_e2e, args.steps, 1)
 
-    t = torch.tensor([tot_ms, e2e_ms], dtype=torch.float64, device=dev)
-    if world > 1:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-    tot_ms, e2e_ms = float(t[0]), float(t[1])
+    tot_ms, e2e_ms = max_over_ranks([tot_ms, e2e_ms], device=dev)
     pairs_step = float(ni) * N * world
     value = pairs_step * args.steps / (tot_ms * 1e-3) / 1e9
     e2e_value = pairs_step * args.steps / (e2e_ms * 1e-3) / 1e9
@@ -256,6 +254,14 @@ def main():
         dfma = s2.s2_peak_fma(ctx, 0, 4000)
         roofline["measured_dfma_tflops"] = 2 * dfma / 1e12
         roofline["frac_of_measured_dfma_pipe"] = (ni * N * FP64_INSTR_PER_PAIR[order] / (force_ms * 1e-3)) / dfma
+        # FP64 operand-path model: lane-instruction rate of each operand pattern / nominal
+        nominal = SM_COUNT * FP64_LANES_PER_SM * SM_MAX_HZ
+        roofline["fp64_pipe_model"] = {
+            "dfma_const_operands": dfma / nominal,
+            "dfma_three_distinct_registers": s2.s2_peak_fma(ctx, 2, 4000) / nominal,
+            "dfma_one_operand_reused": s2.s2_peak_fma(ctx, 3, 4000) / nominal,
+            "dadd_two_registers": s2.s2_peak_fma(ctx, 4, 4000) / nominal,
+            "unit": "fraction of 148 SM x 64 lanes x 1.965 GHz lane-instructions/s"}
         line["sweep"] = ni_sweep(s2, torch, dev, order)
         line["cpu_baseline"] = cpu_baseline(w)
     if rank == 0:

@@ -165,10 +165,13 @@ int s2_get_j(s2_ctx *ctx, int first, int n, int *id, double *t, double *mass, do
 /* Launch-shape overrides for tests and tuning sweeps; value 0 restores the automatic choice.
  *   key 0: number of j-slices S      key 1: lanes per i-particle (1,2,4,..,32)
  *   key 2: warp columns over j (1,2,4,8; only with lanes == 32)
- *   key 3: CTAs per SM assumed by the balancer      key 4: j-tile length (multiple of 32) */
+ *   key 3: CTAs per SM assumed by the balancer      key 4: j-tile length (multiple of 32)
+ *   key 5: 1 = combine j-slices with the separate reduce kernel even when the fused combine applies
+ *   key 6: CTAs per thread-block cluster along the slice axis in the fused combine (1 = none, 2, 4, 8) */
 int s2_set_tuning(s2_ctx *ctx, int key, int value);
 /* Shape of the last force launch: out[0]=S, [1]=lanes per i, [2]=warp columns, [3]=grid size,
- * [4]=threads per CTA, [5]=dynamic shared memory bytes, [6]=1 if the reduce kernel ran,
+ * [4]=threads per CTA, [5]=dynamic shared memory bytes, [6]=0 no combine needed / 1 reduce kernel ran /
+ * 2 combine fused into the sweep launch (last CTA of each i-group reduces, fixed order),
  * [7]=resident CTAs per SM (occupancy query). */
 int s2_last_launch_info(const s2_ctx *ctx, int out[8]);
 /* Number of kernels this context has launched since s2_open. */
@@ -179,9 +182,12 @@ int s2_enable_timing(s2_ctx *ctx, int on);
  * (force sweep, reduce/compaction); 0 for kernels that did not run.  SYNC. */
 int s2_get_timing(s2_ctx *ctx, float *predict_ms, float *force_ms, float *reduce_ms);
 
-/* Peak microbenchmarks used as roofline denominators: a grid that fills the device runs
- * `iters` rounds of 8 independent dependent-FMA chains per thread.  kind 0 = DFMA (fp64),
- * 1 = FFMA (fp32).  Returns achieved FMA lane-instructions per second in *fma_per_s.  SYNC. */
+/* Peak microbenchmarks used as roofline denominators and for the FP64 operand-path model:
+ * a grid that fills the device runs `iters` rounds of 8 independent chains per thread.
+ *   kind 0 = DFMA with constant operands (nominal fp64 rate)      1 = FFMA (fp32)
+ *   kind 2 = DFMA with three distinct 64-bit register operands    3 = DFMA with one operand shared by
+ *   consecutive instructions (operand-reuse cache)                 4 = DADD with two distinct register operands
+ * Returns achieved lane-instructions per second in *fma_per_s.  SYNC. */
 int s2_peak_fma(s2_ctx *ctx, int kind, int iters, double *fma_per_s);
 
 const char *s2_strerror(int code);

@@ -45,7 +45,7 @@ struct s2_ctx {
     long long launches = 0;
 
     // device buffers
-    Buf base, planes, qplanes, stage_dev, iplanes, iqplanes, i_addr, i_h2, part, result, seg, list, flags;
+    Buf base, planes, qplanes, stage_dev, iplanes, iqplanes, i_addr, i_h2, part, result, seg, list, flags, counters;
     // pinned host buffers
     void *h_stage = nullptr;
     size_t h_stage_bytes = 0, h_stage_used = 0;
@@ -63,9 +63,10 @@ struct s2_ctx {
     double t_pred = 0.0;
 
     // tuning overrides and last launch
-    int tune[5] = {0, 0, 0, 0, 0};
+    int tune[7] = {0, 0, 0, 0, 0, 0, 0};
     int last_info[8] = {0, 0, 0, 0, 0, 0, 0, 0};
     std::map<long long, int> occ_cache;
+    std::map<long long, std::pair<ForceShape, int>> shape_cache;
 
     // timing
     bool timing = false;
@@ -223,7 +224,7 @@ extern "C" int s2_close(s2_ctx *ctx)
     cudaSetDevice(ctx->device);
     cudaStreamSynchronize(ctx->stream);
     for (Buf *b : {&ctx->base, &ctx->planes, &ctx->qplanes, &ctx->stage_dev, &ctx->iplanes, &ctx->iqplanes,
-                   &ctx->i_addr, &ctx->i_h2, &ctx->part, &ctx->result, &ctx->seg, &ctx->list, &ctx->flags})
+                   &ctx->i_addr, &ctx->i_h2, &ctx->part, &ctx->result, &ctx->seg, &ctx->list, &ctx->flags, &ctx->counters})
         dev_release(ctx, *b);
     if (ctx->h_stage) cudaFreeHost(ctx->h_stage);
     if (ctx->h_io) cudaFreeHost(ctx->h_io);
@@ -403,13 +404,6 @@ extern "C" int s2_predict(s2_ctx *ctx, double t, int nj)
 
 // ---- launch balancer ----------------------------------------------------------------------
 
-static int pow2_ceil(int x)
-{
-    int p = 1;
-    while (p < x) p <<= 1;
-    return p;
-}
-
 static cudaError_t dispatch(int precision, int order, unsigned flags, int L, dim3 grid, size_t smem,
                             const ForceArgs &a, cudaStream_t st, bool query, int *occ)
 {
@@ -421,45 +415,35 @@ static cudaError_t dispatch(int precision, int order, unsigned flags, int L, dim
     return cudaErrorInvalidValue;
 }
 
-// Chooses lanes per i (L), warp columns (Wj), number of j-slices (S) and the tile length so that
-// the grid fills 148 SMs x resident CTAs in an integral number of waves.
-static int choose_shape(s2_ctx *ctx, int ni, int nj, unsigned flags, ForceShape *out)
+// Launch-shape model.  All times in SM cycles:
+//   an SM receives n = ceil(CTAs / SMs) CTAs; with `occ` resident at a time it pays the fixed per-CTA latency
+//   (first bulk copy, i-gather, epilogue) once per residency round, and one CTA-iteration (256 lanes x 1 pair)
+//   costs t_iter cycles of the arithmetic pipe, whoever shares the SM;
+//   the combine costs one launch gap when it is a separate kernel, or a short serial tail in the last CTA of
+//   each i-group when it is fused.
+struct ShapeCost {
+    double t_iter, c_cta, c_row, c_launch;
+};
+static ShapeCost cost_params(int precision, int order)
 {
-    ForceShape sh{};
-    // lanes per i: minimise (number of i-groups) / L, i.e. the idle-lane waste; ties -> fewer lanes
-    int L = 1;
-    {
-        double best = 1e300;
-        for (int l = 1; l <= 32; l <<= 1) {
-            const int icta = kThreads / l;
-            const double c = (double)((ni + icta - 1) / icta) / l;
-            if (c < best * (1 - 1e-12)) {
-                best = c;
-                L = l;
-            }
-        }
-    }
-    if (ctx->tune[1] > 0) L = ctx->tune[1];
-    if (L < 1 || L > 32 || (L & (L - 1))) return S2_EINVAL;
-    int Wj = 1;
-    if (L == 32 && ni < kWarps) Wj = kWarps / pow2_ceil(ni);
-    if (ctx->tune[2] > 0) Wj = ctx->tune[2];
-    if (Wj < 1 || Wj > kWarps || (Wj & (Wj - 1)) || (Wj > 1 && L != 32)) return S2_EINVAL;
-    const int icta = (kWarps / Wj) * (32 / L);
-    const int Gi = (ni + icta - 1) / icta;
-    const int npl = force_nplanes(ctx->precision, ctx->order, flags);
+    ShapeCost c;
+    c.t_iter = precision == S2_FP64 ? 146.0 : (precision == S2_FP32 ? 100.0 : 1400.0);
+    if (order == 6) c.t_iter *= 1.7;
+    c.c_cta = 4000.0;     // ~2 us: launch ramp, first tile, i-gather, shuffles, record write
+    c.c_row = 1000.0;     // ~0.5 us per round of 32 partial rows (L2 latency bound)
+    c.c_launch = 4000.0;  // ~2 us: second launch (programmatic dependent launch hides part of it)
+    return c;
+}
 
-    int tile = ctx->tune[4] > 0 ? ctx->tune[4] : 256;
-    if (tile % 32 || tile < 32 || tile > 2048) return S2_EINVAL;
-
-    // resident CTAs per SM of this kernel variant (cached)
+static int query_occ(s2_ctx *ctx, unsigned flags, int L, int npl, int *occ_out)
+{
     int occ = ctx->tune[3];
     if (occ <= 0) {
-        const long long key = ((long long)flags << 32) | ((long long)L << 16) | tile;
+        const long long key = ((long long)flags << 32) | L;
         auto it = ctx->occ_cache.find(key);
         if (it == ctx->occ_cache.end()) {
             ForceArgs dummy{};
-            cudaError_t e = dispatch(ctx->precision, ctx->order, flags, L, dim3(1), force_smem_bytes(npl, tile, 2),
+            cudaError_t e = dispatch(ctx->precision, ctx->order, flags, L, dim3(1), force_smem_bytes(npl, 256, 2),
                                      dummy, ctx->stream, true, &occ);
             if (e != cudaSuccess) return fail_cuda(ctx, e);
             if (occ < 1) occ = 1;
@@ -468,57 +452,129 @@ static int choose_shape(s2_ctx *ctx, int ni, int nj, unsigned flags, ForceShape 
             occ = it->second;
         }
     }
-    const long long slots = (long long)ctx->sm_count * occ;
+    *occ_out = occ;
+    return S2_OK;
+}
 
-    int S;
-    if (ctx->tune[0] > 0) {
-        S = ctx->tune[0];
-    } else if (Wj > 1) {
-        // one tile per CTA; enough CTAs to fill the machine, slices no longer than the tile cap
-        S = (int)std::max<long long>(1, slots / Gi);
-        S = std::min(S, std::max(1, nj / (Wj * 4)));   // at least ~4 j per warp column
-        const int tcap = 512;
-        if ((nj + S - 1) / S > tcap) S = (nj + tcap - 1) / tcap;
-    } else {
-        // cost model: waves x (thread iterations per slice + fixed per-CTA overhead)
-        const double c0 = 24.0;
-        const int min_slice = std::max(32, 2 * L);
-        const int smax = (int)std::min<long long>(std::max(1, nj / min_slice),
-                                                  std::max<long long>(1, (8 * slots + Gi - 1) / Gi));
-        double best = 1e300;
-        S = 1;
-        for (int s = 1; s <= smax; ++s) {
-            const int sl = (nj + s - 1) / s;
-            const long long ctas = (long long)Gi * ((nj + sl - 1) / sl);
-            const double waves = (double)((ctas + slots - 1) / slots);
-            double cost = waves * ((double)((sl + L - 1) / L) + c0);
-            if (s > 1) cost *= 1.0 + 2e-3;   // a reduce pass follows
-            if (cost < best * (1 - 1e-9)) {
-                best = cost;
-                S = s;
+// Chooses lanes per i (L), warp columns (Wj), number of j-slices (S), the tile length and the number of tile
+// buffers.  Automatic choices are cached per (n_i, n_j, flags); s2_set_tuning overrides any of them.
+static int choose_shape(s2_ctx *ctx, int ni, int nj, unsigned flags, ForceShape *out)
+{
+    const bool tuned = ctx->tune[0] || ctx->tune[1] || ctx->tune[2] || ctx->tune[3] || ctx->tune[4] || ctx->tune[5] || ctx->tune[6];
+    const long long ckey = ((long long)ni << 34) ^ ((long long)nj << 3) ^ (long long)flags;
+    if (!tuned) {
+        auto it = ctx->shape_cache.find(ckey);
+        if (it != ctx->shape_cache.end()) {
+            *out = it->second.first;
+            ctx->last_info[7] = it->second.second;
+            return S2_OK;
+        }
+    }
+    const int npl = force_nplanes(ctx->precision, ctx->order, flags);
+    const ShapeCost C_ = cost_params(ctx->precision, ctx->order);
+    const bool want_ngb = flags & S2_WANT_NGB;
+    const int tile_max = std::min(2048, (int)((232448 - kSmemHeader) / (2 * npl * 16)) / 32 * 32);
+
+    double best = 1e300;
+    int bL = 1, bWj = 1, bS = 1, bocc = 1, bfused = 0, bC = 1;
+    for (int L = 1; L <= 32; L <<= 1) {
+        if (ctx->tune[1] > 0 && L != ctx->tune[1]) continue;
+        int occ;
+        int rc = query_occ(ctx, flags, L, npl, &occ);
+        if (rc != S2_OK) return rc;
+        for (int Wj = 1; Wj <= kWarps; Wj <<= 1) {
+            // warp columns: warps of a CTA share i-particles and split every tile (the paper's 2D blocks, L104);
+            // worth it only while the i-list does not fill the i-groups anyway
+            if (ctx->tune[2] > 0 ? Wj != ctx->tune[2] : (Wj > 1 && (L == 1 || (long long)ni * L * Wj > 2048))) continue;
+            if (Wj > 1 && L == 1) continue;
+            const int icta = (kWarps / Wj) * (32 / L);
+            const int Gi = (ni + icta - 1) / icta;
+            const int lanes_j = L * Wj;                         // lanes (over all warp columns) sharing one i
+            const int min_slice = std::max(32, 2 * lanes_j);
+            const int smax = std::min(65535, std::max(1, nj / min_slice));
+            // candidate slice counts: 1, and those that make the grid k x SMs (k = 1..16)
+            int cand[40], nc = 0;
+            if (ctx->tune[0] > 0) {
+                cand[nc++] = ctx->tune[0];
+            } else {
+                cand[nc++] = 1;
+                for (int k = 1; k <= 16; ++k) {
+                    const int s1 = (int)(((long long)k * ctx->sm_count) / Gi);          // floor: grid <= k SMs
+                    if (s1 >= 1 && s1 <= smax) cand[nc++] = s1;
+                }
+            }
+            for (int q = 0; q < nc; ++q) {
+                int S = cand[q];
+                // neighbour segments must stay ascending per record: a warp column may then only take a part of ONE tile
+                if (want_ngb && Wj > 1 && (nj + S - 1) / S > tile_max) S = (nj + tile_max - 1) / tile_max;
+                const bool fusable = !want_ngb && ctx->tune[5] == 0 && S * Wj > 1;
+                // clusters of C CTAs along the slice axis pre-combine their records through distributed shared
+                // memory (j-split shapes only: their record block, <= 128 x 96 B, always fits the tile buffers)
+                int C = 1;
+                if (fusable && lanes_j > 1 && S > 1) {
+                    C = ctx->tune[6] > 0 ? ctx->tune[6] : 1;   // opt-in: measured slower than no cluster
+                    if (C != 1 && C != 2 && C != 4 && C != 8) return S2_EINVAL;
+                    if (S < C) C = 1;
+                    S = S / C * C;
+                }
+                int sl = (nj + S - 1) / S;
+                if (C == 1) S = (nj + sl - 1) / sl;             // no empty slices (a cluster grid may keep some)
+                const long long ctas = (long long)Gi * S;
+                const double n_sm = (double)((ctas + ctx->sm_count - 1) / ctx->sm_count);
+                const double iters = (double)((sl + lanes_j - 1) / lanes_j);
+                // lanes that share an i read different j: LDS.128 is conflict-free up to 8 distinct addresses
+                // measured (profiles/r01_small_ni.md): a lone CTA per SM is latency-bound (~1.25x), lanes that
+                // share an i read different j (LDS.128 conflict-free up to L = 8, 2- and 4-way above)
+                const double t_iter = C_.t_iter * (n_sm >= 2 ? 1.0 : 1.25) * (1.0 + 0.01 * L) * (L > 8 ? 1.0 + 0.01 * L : 1.0);
+                // every i-group streams the whole j range from L2 (~2500 B per SM-cycle over the chip)
+                const double stream = (double)Gi * nj * npl * 16.0 / 2500.0;
+                double cost = std::ceil(n_sm / occ) * C_.c_cta + std::max(n_sm * iters * t_iter, stream);
+                const int nst = S * Wj;
+                int fused = 0;
+                if (nst > 1) {
+                    const double rounds_f = std::ceil(std::min(icta, ni) / (double)kWarps) * std::ceil((S / C) / 32.0);
+                    const double fused_cost = (1.0 + rounds_f) * C_.c_row + (C > 1 ? C_.c_row : 0.0);
+                    const double sep_cost = C_.c_launch + std::ceil(nst / 128.0) * C_.c_row +
+                                            (double)ni * nst * (REC * 8.0) / 2000.0;
+                    fused = fusable && (fused_cost < sep_cost || ctx->tune[6] > 1);
+                    if (!fused && C > 1) continue;              // a cluster shape only makes sense fused
+                    cost += fused ? fused_cost : sep_cost;
+                }
+                if (cost < best * (1 - 1e-9)) {
+                    best = cost;
+                    bL = L; bWj = Wj; bS = S; bocc = occ; bfused = fused; bC = fused ? C : 1;
+                }
             }
         }
     }
-    if (S < 1 || S > 65535) return S2_EINVAL;
-    // largest tile whose two stages fit the 227 KB of shared memory one CTA may use
-    const int tile_max = std::min(2048, (int)((232448 - kSmemHeader) / (2 * npl * 16)) / 32 * 32);
-    if (tile > tile_max) return S2_EINVAL;
-    if (Wj > 1 && (nj + S - 1) / S > tile_max) S = (nj + tile_max - 1) / tile_max;   // one tile per CTA
-    int slice_len = (nj + S - 1) / S;
-    S = (nj + slice_len - 1) / slice_len;
-    if (S > 65535) return S2_EINVAL;
-    if (Wj > 1) {
-        tile = std::max(32, (slice_len + 31) / 32 * 32);
-    } else if (slice_len < tile) {
-        tile = std::max(32, (slice_len + 31) / 32 * 32);
+    if (best >= 1e300) return S2_EINVAL;
+
+    ForceShape sh{};
+    sh.L = bL;
+    sh.Wj = bWj;
+    sh.S = bS;
+    sh.slice_len = (nj + bS - 1) / bS;
+    // tiles: a ring of up to 4 buffers (<= ~96 KB per CTA so two CTAs still fit an SM); short slices are cut
+    // into as many tiles as there are buffers so that every bulk copy is in flight from the start
+    int tile = ctx->tune[4] > 0 ? ctx->tune[4] : 256;
+    if (tile % 32 || tile < 32 || tile > tile_max) return S2_EINVAL;
+    int stages;
+    if (bWj > 1 && want_ngb) {   // one tile per CTA
+        tile = std::max(32, (sh.slice_len + 31) / 32 * 32);
+        if (tile > tile_max) return S2_EINVAL;
+        stages = 1;
+    } else {
+        if (bWj > 1 && ctx->tune[4] == 0) tile = std::min(tile_max, 64 * bWj);   // >= 64 j per warp column and tile
+        stages = std::max(2, std::min(4, (int)(98304 / ((size_t)npl * tile * 16))));
+        if (ctx->tune[4] == 0 && sh.slice_len < stages * tile)
+            tile = std::max(32, ((sh.slice_len + stages - 1) / stages + 31) / 32 * 32);
     }
-    sh.L = L;
-    sh.Wj = Wj;
-    sh.S = S;
-    sh.slice_len = slice_len;
     sh.tile = tile;
-    sh.stages = 2;
-    ctx->last_info[7] = occ;
+    sh.stages = stages;
+    sh.fused = bfused;
+    sh.cluster = bC;
+    ctx->last_info[7] = bocc;
+    if (!tuned) ctx->shape_cache[ckey] = std::make_pair(sh, bocc);
     *out = sh;
     return S2_OK;
 }
@@ -534,14 +590,22 @@ static int run_force(s2_ctx *ctx, int ni, const int *d_i_addr, const double *d_h
     const int nst = sh.S * sh.Wj;
     const bool want_ngb = flags & S2_WANT_NGB;
     const bool final_direct = nst == 1;
+    // without neighbour lists the combine is fused into the sweep launch (last CTA of an i-group reduces)
+    const int icta_ = (kWarps / sh.Wj) * (32 / sh.L);
+    const int Gi_ = (ni + icta_ - 1) / icta_;
+    const bool fused = sh.fused != 0;
 
     rc = dev_reserve(ctx, ctx->result, (size_t)ni * REC * sizeof(double));
     if (rc == S2_OK && !final_direct) rc = dev_reserve(ctx, ctx->part, (size_t)nst * ni * REC * sizeof(double));
+    if (rc == S2_OK && fused && (size_t)Gi_ * sizeof(unsigned) > ctx->counters.bytes) {
+        rc = dev_reserve(ctx, ctx->counters, (size_t)Gi_ * sizeof(unsigned));
+        if (rc == S2_OK) CU(cudaMemsetAsync(ctx->counters.p, 0, ctx->counters.bytes, ctx->stream));
+    }
     int segcap = 0;
     if (want_ngb) {
         if (ctx->ngb_cap <= 0) return S2_EINVAL;
-        const int jper = (sh.slice_len + sh.Wj - 1) / sh.Wj;   // longest j range one record covers
-        segcap = final_direct ? ctx->ngb_cap : std::min(ctx->ngb_cap, jper);
+        // a record covers at most one slice (a warp column takes a part of every tile of the slice)
+        segcap = final_direct ? ctx->ngb_cap : std::min(ctx->ngb_cap, sh.slice_len);
         if (rc == S2_OK) rc = dev_reserve(ctx, ctx->list, (size_t)ni * ctx->ngb_cap * sizeof(int));
         if (rc == S2_OK && !final_direct) rc = dev_reserve(ctx, ctx->seg, (size_t)ni * nst * segcap * sizeof(int));
     }
@@ -576,6 +640,7 @@ static int run_force(s2_ctx *ctx, int ni, const int *d_i_addr, const double *d_h
     a.slice_len = sh.slice_len;
     a.Wj = sh.Wj;
     a.tile = sh.tile;
+    a.stages = sh.stages;
     a.nslices_total = nst;
     a.is_final = final_direct ? 1 : 0;
     a.rec = final_direct ? (double *)ctx->result.p : (double *)ctx->part.p;
@@ -583,18 +648,24 @@ static int run_force(s2_ctx *ctx, int ni, const int *d_i_addr, const double *d_h
     a.segcap = segcap;
     a.overflow_flag = (int *)ctx->flags.p;
     a.ngb_cap = ctx->ngb_cap;
+    a.fused = fused ? 1 : 0;
+    a.cluster = fused ? sh.cluster : 1;
+    a.counters = (unsigned *)ctx->counters.p;
+    a.out_final = (double *)ctx->result.p;
+    a.order = ctx->order;
 
-    CU(cudaMemsetAsync(ctx->flags.p, 0, sizeof(int), ctx->stream));   // overflow flag of this call
+    if (want_ngb) CU(cudaMemsetAsync(ctx->flags.p, 0, sizeof(int), ctx->stream));   // overflow flag of this call
     const int icta = (kWarps / sh.Wj) * (32 / sh.L);
     dim3 grid((ni + icta - 1) / icta, sh.S);
-    const size_t smem = force_smem_bytes(force_nplanes(ctx->precision, ctx->order, flags), sh.tile, sh.stages);
+    size_t smem = force_smem_bytes(force_nplanes(ctx->precision, ctx->order, flags), sh.tile, sh.stages);
+    smem = std::max(smem, (size_t)kSmemHeader + (size_t)icta * sh.Wj * REC * sizeof(double));   // record block of the combines
     if (ctx->timing) CU(cudaEventRecord(ctx->ev_t[2], ctx->stream));
     CU(dispatch(ctx->precision, ctx->order, flags, sh.L, grid, smem, a, ctx->stream, false, nullptr));
     if (ctx->timing) CU(cudaEventRecord(ctx->ev_t[3], ctx->stream));
     ctx->launches++;
     ctx->ran_force = true;
     ctx->ran_reduce = false;
-    if (!final_direct) {
+    if (!final_direct && !fused) {
         ReduceArgs r{};
         r.part = (const double *)ctx->part.p;
         r.out = (double *)ctx->result.p;
@@ -616,7 +687,7 @@ static int run_force(s2_ctx *ctx, int ni, const int *d_i_addr, const double *d_h
     }
     int *li = ctx->last_info;
     li[0] = sh.S; li[1] = sh.L; li[2] = sh.Wj; li[3] = (int)(grid.x * grid.y); li[4] = kThreads;
-    li[5] = (int)smem; li[6] = final_direct ? 0 : 1;
+    li[5] = (int)smem; li[6] = final_direct ? 0 : (fused ? 2 : 1);
     ctx->calc_done = true;
     ctx->ni_last = ni;
     ctx->flags_last = flags;
@@ -900,7 +971,7 @@ extern "C" int s2_get_j(s2_ctx *ctx, int first, int n, int *id, double *t, doubl
 
 extern "C" int s2_set_tuning(s2_ctx *ctx, int key, int value)
 {
-    if (!ctx || key < 0 || key > 4 || value < 0) return S2_EINVAL;
+    if (!ctx || key < 0 || key > 6 || value < 0) return S2_EINVAL;
     ctx->tune[key] = value;
     return S2_OK;
 }
@@ -939,7 +1010,7 @@ extern "C" int s2_get_timing(s2_ctx *ctx, float *predict_ms, float *force_ms, fl
 
 extern "C" int s2_peak_fma(s2_ctx *ctx, int kind, int iters, double *fma_per_s)
 {
-    if (!ctx || !fma_per_s || iters <= 0 || kind < 0 || kind > 1) return S2_EINVAL;
+    if (!ctx || !fma_per_s || iters <= 0 || kind < 0 || kind > 4) return S2_EINVAL;
     CU(cudaSetDevice(ctx->device));
     CU(run_peak_fma(kind, iters, ctx->sm_count, ctx->stream, fma_per_s));
     ctx->launches += 2;

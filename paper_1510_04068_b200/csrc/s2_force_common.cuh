@@ -52,6 +52,27 @@ __device__ __forceinline__ void bulk_g2s(void *dst, const void *src, uint32_t by
                  : "memory");
 }
 
+// Thread-block cluster primitives (distributed shared memory)
+__device__ __forceinline__ uint32_t cluster_ctarank()
+{
+    uint32_t r;
+    asm volatile("mov.u32 %0, %%cluster_ctarank;" : "=r"(r));
+    return r;
+}
+__device__ __forceinline__ void cluster_sync()
+{
+    asm volatile("barrier.cluster.arrive.release.aligned;\n\tbarrier.cluster.wait.acquire.aligned;" ::: "memory");
+}
+// fp64 load from the shared memory of CTA `rank` of this cluster, at the same offset as local address saddr
+__device__ __forceinline__ double ld_dsmem_f64(uint32_t saddr, uint32_t rank)
+{
+    uint32_t ra;
+    double v;
+    asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(ra) : "r"(saddr), "r"(rank));
+    asm volatile("ld.shared::cluster.f64 %0, [%1];" : "=d"(v) : "r"(ra) : "memory");
+    return v;
+}
+
 // Work decomposition of one CTA:
 //   warp w -> (wi, wj) = (w / Wj, w % Wj);  lane -> (il, jl) = (lane / L, lane % L)
 //   i index  = (blockIdx.x * (kWarps / Wj) + wi) * (32 / L) + il

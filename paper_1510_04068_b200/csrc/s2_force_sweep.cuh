@@ -63,6 +63,73 @@ __device__ __forceinline__ void decide(double d2, int jaddr, bool skip, double h
     }
 }
 
+// Sum of the partial rows of one i-particle by one warp, in a fixed order (P17): lane l adds rows l, l+32, ...
+// sequentially, then the 32 lanes combine by an xor-butterfly; nn by (d2, address) lexicographic minimum.
+// Rows were written by other CTAs of the same launch: read through L2 (ld.global.cg), after a fence.
+template <bool NN>
+__device__ __forceinline__ void reduce_rows_warp(const double *part, double *outp, const double2 *jid_plane, int i,
+                                                 int ni, int rows, int order, int lane)
+{
+    double v[10];
+#pragma unroll
+    for (int c = 0; c < 10; ++c) v[c] = 0.0;
+    double nn_d2 = CUDART_INF;
+    int nn_j = -1;
+    // rows are fetched four at a time (independent loads in flight) and added in row order
+    for (int s0 = lane; s0 < rows; s0 += 4 * 32) {
+        double2 q[4][6];
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+            const int s = s0 + 32 * u;
+            if (s < rows) {
+                const double2 *r = reinterpret_cast<const double2 *>(part + ((size_t)s * ni + i) * REC);
+#pragma unroll
+                for (int c = 0; c < 5; ++c) q[u][c] = __ldcg(r + c);
+                if (order == 6) q[u][5] = __ldcg(r + 5);
+            }
+        }
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+            if (s0 + 32 * u < rows) {
+                v[0] += q[u][0].x; v[1] += q[u][0].y; v[2] += q[u][1].x; v[3] += q[u][1].y;
+                v[4] += q[u][2].x; v[5] += q[u][2].y; v[6] += q[u][3].x;
+                if (order == 6) { v[7] += q[u][4].y; v[8] += q[u][5].x; v[9] += q[u][5].y; }
+                if (NN) {
+                    const int j = __double2loint(q[u][4].x);
+                    if (q[u][3].y < nn_d2 || (q[u][3].y == nn_d2 && (unsigned)j < (unsigned)nn_j)) {
+                        nn_d2 = q[u][3].y;
+                        nn_j = j;
+                    }
+                }
+            }
+        }
+    }
+#pragma unroll
+    for (int m = 1; m < 32; m <<= 1) {
+#pragma unroll
+        for (int c = 0; c < 10; ++c) v[c] += shfl_xor_d(v[c], m);
+        if (NN) {
+            const double od2 = shfl_xor_d(nn_d2, m);
+            const int oj = __shfl_xor_sync(0xffffffffu, nn_j, m);
+            if (od2 < nn_d2 || (od2 == nn_d2 && (unsigned)oj < (unsigned)nn_j)) {
+                nn_d2 = od2;
+                nn_j = oj;
+            }
+        }
+    }
+    if (lane == 0) {
+        int nn = nn_j;
+        if (NN && nn >= 0) nn = __double2loint(jid_plane[nn].y);
+        double2 *o = reinterpret_cast<double2 *>(outp + (size_t)i * REC);
+        o[0] = make_double2(v[0], v[1]);
+        o[1] = make_double2(v[2], v[3]);
+        o[2] = make_double2(v[4], v[5]);
+        o[3] = make_double2(v[6], nn_d2);
+        o[4] = make_double2(__hiloint2double(0, nn), v[7]);
+        o[5] = make_double2(v[8], v[9]);
+    }
+}
+
 // Policy interface (see PolicyF64 in s2_force_fp64.cu):
 //   NPL, kMinBlocks, NN, NGB, ORDER
 //   struct IState; static void load_i(const ForceArgs&, int i, IState&)
@@ -77,7 +144,7 @@ __global__ void __launch_bounds__(kThreads, P::kMinBlocks) force_sweep_kernel(co
     uint64_t *full = reinterpret_cast<uint64_t *>(smem_raw);
     unsigned char *tiles = smem_raw + kSmemHeader;
     constexpr int NPL = P::NPL;
-    constexpr int ST = 2;   // stages
+    const int ST = a.stages;   // ring of ST tile buffers (2..kMaxStages), each filled by NPL bulk copies
 
     const Decomp d = decompose<L>(a.Wj, a.ni);
     const int tile = a.tile;
@@ -88,14 +155,13 @@ __global__ void __launch_bounds__(kThreads, P::kMinBlocks) force_sweep_kernel(co
     const int ntiles = j1 > j0 ? (j1 - j0 + tile - 1) / tile : 0;
 
     if (threadIdx.x == 0) {
-        mbar_init(&full[0], 1);
-        mbar_init(&full[1], 1);
+        for (int s = 0; s < ST; ++s) mbar_init(&full[s], 1);
         mbar_fence_init();
     }
     __syncthreads();
 
     auto issue = [&](int t) {
-        const int st = t & 1;
+        const int st = t % ST;
         const int jt = j0 + t * tile;
         const uint32_t bytes = (uint32_t)min(tile, j1 - jt) * 16u;
         mbar_arrive_expect_tx(&full[st], bytes * NPL);
@@ -104,7 +170,11 @@ __global__ void __launch_bounds__(kThreads, P::kMinBlocks) force_sweep_kernel(co
             bulk_g2s(tiles + st * stage_bytes + (size_t)p * tile * 16,
                      reinterpret_cast<const unsigned char *>(a.jp[p]) + (size_t)jt * 16, bytes, &full[st]);
     };
-    if (threadIdx.x == 0 && ntiles > 0) issue(0);
+    if (threadIdx.x == 0)
+        for (int t = 0; t < min(ntiles, ST - 1); ++t) issue(t);   // prologue: ST-1 tiles in flight
+    // let a dependent launch (the reduce kernel, launched with programmatic stream serialisation) be staged now;
+    // it waits for this grid's completion itself (griddepcontrol.wait)
+    asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
 
     typename P::IState I;
     P::load_i(a, d.i, I);
@@ -120,9 +190,10 @@ __global__ void __launch_bounds__(kThreads, P::kMinBlocks) force_sweep_kernel(co
     if (P::NGB) seg = a.seg + ((size_t)d.i * a.nslices_total + d.slice) * a.segcap;
 
     for (int t = 0; t < ntiles; ++t) {
-        if (threadIdx.x == 0 && t + 1 < ntiles) issue(t + 1);   // stage (t+1)&1 was released by the barrier ending tile t-1
-        mbar_wait(&full[t & 1], (t >> 1) & 1);
-        const unsigned char *stage = tiles + (t & 1) * stage_bytes;
+        // stage (t-1) % ST was released by the barrier that ended tile t-1: refill it with tile t+ST-1
+        if (threadIdx.x == 0 && t + ST - 1 < ntiles) issue(t + ST - 1);
+        mbar_wait(&full[t % ST], (t / ST) & 1);
+        const unsigned char *stage = tiles + (t % ST) * stage_bytes;
         const int jt = j0 + t * tile;
         const int cnt = min(tile, j1 - jt);
         // this warp column's sub-range of the tile
@@ -141,7 +212,7 @@ __global__ void __launch_bounds__(kThreads, P::kMinBlocks) force_sweep_kernel(co
         } else {
             const int nfull = len / L;
             int k = beg + d.jl;
-#pragma unroll 2
+#pragma unroll P::kUnroll
             for (int it = 0; it < nfull; ++it, k += L)
                 P::template pair<L, false>(stage, tile, k, true, jt + k, I, part, D, d, seg, a.segcap);
             if (len - nfull * L > 0) {   // ragged tail: lanes past the end re-read the last j, masked
@@ -151,7 +222,7 @@ __global__ void __launch_bounds__(kThreads, P::kMinBlocks) force_sweep_kernel(co
             }
         }
         tot.add(part);   // two-level accumulation: per-tile partial sums, then the running total
-        __syncthreads();
+        if (t + ST < ntiles) __syncthreads();   // only needed when this stage will be refilled
     }
 
     // combine the L lanes of each i in a fixed (butterfly) order
@@ -170,11 +241,98 @@ __global__ void __launch_bounds__(kThreads, P::kMinBlocks) force_sweep_kernel(co
         }
     }
 
-    if (d.jl == 0 && d.i_valid) {
-        double out[10];
-        tot.to_f64(out);
-        double *r = a.rec + ((size_t)d.slice * a.ni + d.i) * REC;
-        int nn = D.nn_j;
+    double out[10];
+    tot.to_f64(out);
+    int nn = D.nn_j;
+    int row = d.slice;                      // partial row this thread's record goes to
+    bool writer = d.jl == 0 && d.i_valid;
+
+    if (a.fused && a.Wj > 1) {
+        // warp columns: the Wj warps that hold the same i-particles (different j sub-ranges of every tile) add
+        // their records in shared memory, in column order 0, 1, ...; column 0 carries the sum on
+        double *sm = reinterpret_cast<double *>(tiles);
+        const int il_cta = d.wi * (32 / L) + d.il;         // index of this thread's i inside the CTA
+        __syncthreads();                                   // every warp is done reading the tile buffers
+        if (d.jl == 0) {
+            double *r = sm + (il_cta * a.Wj + d.wj) * REC;
+#pragma unroll
+            for (int c = 0; c < 10; ++c) r[c] = out[c];
+            r[10] = D.nn_d2;
+            r[11] = __hiloint2double(0, nn);
+        }
+        __syncthreads();
+        writer = writer && d.wj == 0;
+        if (d.jl == 0 && d.wj == 0) {
+            for (int c = 1; c < a.Wj; ++c) {
+                const double *r = sm + (il_cta * a.Wj + c) * REC;
+#pragma unroll
+                for (int k = 0; k < 10; ++k) out[k] += r[k];
+                if (P::NN) {
+                    const int oj = __double2loint(r[11]);
+                    if (r[10] < D.nn_d2 || (r[10] == D.nn_d2 && (unsigned)oj < (unsigned)nn)) {
+                        D.nn_d2 = r[10];
+                        nn = oj;
+                    }
+                }
+            }
+        }
+        row = blockIdx.y;
+    }
+
+    if (a.cluster > 1) {
+        // Thread-block cluster of a.cluster CTAs along the slice axis: every CTA parks its records in its own
+        // shared memory, the cluster synchronises, and CTA rank r sums the records of its share of the i-particles
+        // over the ranks 0, 1, ... in that order through distributed shared memory.  One partial row per cluster.
+        const int C = a.cluster;
+        const int icta = (kWarps / a.Wj) * (32 / L);
+        const int il_cta = d.wi * (32 / L) + d.il;            // index of this thread's i inside the CTA
+        double *sm = reinterpret_cast<double *>(tiles);
+        __syncthreads();                                       // tile buffers are dead from here on
+        if (d.jl == 0 && (a.Wj == 1 || d.wj == 0)) {
+            double *r = sm + il_cta * REC;
+#pragma unroll
+            for (int c = 0; c < 10; ++c) r[c] = out[c];
+            r[10] = D.nn_d2;
+            r[11] = __hiloint2double(0, nn);
+        }
+        cluster_sync();
+        const uint32_t rank = cluster_ctarank();
+        const int per = (icta + C - 1) / C;                    // i-particles summed by one rank
+        for (int t = threadIdx.x; t < per * REC; t += kThreads) {
+            const int li = t / REC, comp = t % REC;
+            const int il_sum = rank * per + li;
+            const int gi = blockIdx.x * icta + il_sum;
+            if (il_sum >= icta || gi >= a.ni || comp == 11) continue;
+            const uint32_t base = smem_u32(sm + il_sum * REC);
+            double v = ld_dsmem_f64(base + comp * 8, 0);
+            int bj = comp == 10 ? __double2loint(ld_dsmem_f64(base + 88, 0)) : 0;
+            for (int rk = 1; rk < C; ++rk) {
+                const double o = ld_dsmem_f64(base + comp * 8, rk);
+                if (comp < 10) {
+                    v += o;
+                } else {   // nearest neighbour: (d2, address) lexicographic minimum
+                    const int oj = __double2loint(ld_dsmem_f64(base + 88, rk));
+                    if (o < v || (o == v && (unsigned)oj < (unsigned)bj)) {
+                        v = o;
+                        bj = oj;
+                    }
+                }
+            }
+            // record layout: 0-2 acc, 3-5 jerk, 6 pot, 7 nn_d2, 8 {nn, count}, 9-11 snap
+            double *g = a.rec + ((size_t)(blockIdx.y / C) * a.ni + gi) * REC;
+            if (comp < 7) g[comp] = v;
+            else if (comp < 10) g[comp + 2] = v;
+            else {
+                g[7] = v;
+                g[8] = __hiloint2double(0, bj);
+            }
+        }
+        cluster_sync();                                        // nobody leaves while its shared memory is read
+        writer = false;
+    }
+
+    if (writer) {
+        double *r = a.rec + ((size_t)row * a.ni + d.i) * REC;
         if (a.is_final) {
             if (P::NN && nn >= 0) nn = __double2loint(a.jid_plane[nn].y);
             if (P::NGB && D.cnt > a.ngb_cap) *a.overflow_flag = 1;
@@ -186,6 +344,30 @@ __global__ void __launch_bounds__(kThreads, P::kMinBlocks) force_sweep_kernel(co
         r2[3] = make_double2(out[6], D.nn_d2);
         r2[4] = make_double2(__hiloint2double(D.cnt, nn), out[7]);
         r2[5] = make_double2(out[8], out[9]);
+    }
+
+    if (a.fused) {
+        // The last CTA of this i-group to arrive reduces the gridDim.y partial rows (fixed order: lane l adds
+        // rows l, l+32, ... then an xor-butterfly -- the same order as reduce_kernel).  No floating-point atomics.
+        __shared__ int s_last;
+        __threadfence();
+        __syncthreads();
+        if (threadIdx.x == 0) {
+            const unsigned prev = atomicAdd(&a.counters[blockIdx.x], 1u);
+            s_last = prev == gridDim.y - 1;
+        }
+        __syncthreads();
+        if (s_last) {
+            __threadfence();
+            const int icta = (kWarps / a.Wj) * (32 / L);
+            const int i0 = blockIdx.x * icta;
+            const int i1 = min(a.ni, i0 + icta);
+            const int rows = gridDim.y / max(1, a.cluster);
+            const int lane = threadIdx.x & 31;
+            for (int i = i0 + (threadIdx.x >> 5); i < i1; i += kWarps)
+                reduce_rows_warp<P::NN>(a.rec, a.out_final, a.jid_plane, i, a.ni, rows, a.order, lane);
+            if (threadIdx.x == 0) a.counters[blockIdx.x] = 0;
+        }
     }
 }
 
@@ -201,6 +383,15 @@ cudaError_t launch_L(int L, dim3 grid, size_t smem, const ForceArgs &a, cudaStre
         cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem); \
         if (e != cudaSuccess) return e;                                                                      \
         if (query) return cudaOccupancyMaxActiveBlocksPerMultiprocessor(ctas_per_sm, kern, kThreads, smem);  \
+        if (a.cluster > 1) {                                                                                 \
+            cudaLaunchConfig_t cfg = {};                                                                     \
+            cfg.gridDim = grid; cfg.blockDim = dim3(kThreads); cfg.dynamicSmemBytes = smem; cfg.stream = st; \
+            cudaLaunchAttribute at[1];                                                                       \
+            at[0].id = cudaLaunchAttributeClusterDimension;                                                  \
+            at[0].val.clusterDim.x = 1; at[0].val.clusterDim.y = a.cluster; at[0].val.clusterDim.z = 1;      \
+            cfg.attrs = at; cfg.numAttrs = 1;                                                                \
+            return cudaLaunchKernelEx(&cfg, kern, a);                                                        \
+        }                                                                                                    \
         kern<<<grid, kThreads, smem, st>>>(a);                                                               \
         return cudaGetLastError();                                                                           \
     }

@@ -76,6 +76,7 @@ struct ForceArgs {
     int slice_len;                 // j per CTA slice
     int Wj;                        // warp columns over j inside a CTA (1,2,4,8)
     int tile;                      // j per shared-memory tile
+    int stages;                    // tile buffers in the ring (2..kMaxStages)
     int nslices_total;             // S * Wj
     int is_final;                  // 1: write final records (nn as id), no reduce kernel follows
     double *rec;                   // [nslices_total][ni][REC]
@@ -83,6 +84,13 @@ struct ForceArgs {
     int segcap;
     int *overflow_flag;
     int ngb_cap;
+    // fused combine (no neighbour lists): the warp columns of a CTA are summed in shared memory, so there is one
+    // partial row per j-slice, and the last CTA of an i-group to finish reduces the S rows in a fixed order
+    int fused;
+    int cluster;                   // CTAs per cluster along the slice axis (1, 2, 4, 8); > 1 only when fused
+    unsigned *counters;            // [number of i-groups], zero between calls (the reducing CTA resets its entry)
+    double *out_final;             // [ni][REC]
+    int order;
 };
 
 struct ReduceArgs {
@@ -112,8 +120,11 @@ struct ForceShape {                // chosen by the balancer in s2_api.cu
     int slice_len;
     int tile;
     int stages;
+    int fused;                     // combine inside the sweep launch (last CTA of each i-group)
+    int cluster;                   // CTAs per cluster along the slice axis when fused (1 = no cluster)
 };
 constexpr int kSmemHeader = 64;   // mbarriers live in the first 64 bytes of dynamic shared memory
+constexpr int kMaxStages = 8;
 inline size_t force_smem_bytes(int nplanes, int tile, int stages)
 {
     return (size_t)kSmemHeader + (size_t)stages * nplanes * tile * 16;

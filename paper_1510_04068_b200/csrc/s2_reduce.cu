@@ -9,17 +9,26 @@
 // The kernel streams S*ni records of 96 bytes once: L2/HBM-bound, tiny.
 #include <math_constants.h>
 
-#include "s2_force_common.cuh"
+#include "s2_force_sweep.cuh"
 
 namespace s2 {
 
-__global__ void __launch_bounds__(256) reduce_kernel(ReduceArgs a)
+__global__ void __launch_bounds__(256) reduce_kernel(const ReduceArgs a)
 {
     const int warp = (blockIdx.x * blockDim.x + threadIdx.x) >> 5;
     const int lane = threadIdx.x & 31;
     if (warp >= a.ni) return;   // whole warp exits together
     const int i = warp;
     const int S = a.nslices_total;
+    // programmatic dependent launch: this grid may start while the sweep is still running; wait for its results
+    asm volatile("griddepcontrol.wait;" ::: "memory");
+    if (!(a.flags & S2_WANT_NGB)) {   // plain sums (+ nn): the same fixed-order routine the fused combine uses
+        if (a.flags & S2_WANT_NN)
+            reduce_rows_warp<true>(a.part, a.out, a.jid_plane, i, a.ni, S, a.order, lane);
+        else
+            reduce_rows_warp<false>(a.part, a.out, a.jid_plane, i, a.ni, S, a.order, lane);
+        return;
+    }
 
     double v[10];
 #pragma unroll
@@ -97,9 +106,17 @@ __global__ void __launch_bounds__(256) reduce_kernel(ReduceArgs a)
 cudaError_t launch_reduce(const ReduceArgs &a, cudaStream_t st)
 {
     if (a.ni <= 0) return cudaSuccess;
-    const int warps_per_block = 8;
-    reduce_kernel<<<(a.ni + warps_per_block - 1) / warps_per_block, 32 * warps_per_block, 0, st>>>(a);
-    return cudaGetLastError();
+    const int warps_per_block = a.ni <= 1024 ? 2 : 8;   // few i: spread the warps over more SMs
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3((a.ni + warps_per_block - 1) / warps_per_block);
+    cfg.blockDim = dim3(32 * warps_per_block);
+    cfg.stream = st;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;   // overlap this launch with the sweep's tail
+    at[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = at;
+    cfg.numAttrs = 1;
+    return cudaLaunchKernelEx(&cfg, reduce_kernel, a);
 }
 
 }  // namespace s2

@@ -123,20 +123,38 @@ cudaError_t launch_predict(const PredictArgs &a, cudaStream_t st)
 }
 
 // ------------------------------------------------------------------------------------------
-// Peak microbenchmarks (roofline denominators): 8 independent FMA chains per thread.
-template <typename T>
+// Peak microbenchmarks (roofline denominators and the FP64 operand-path model of DESIGN.md 5.2):
+// 8 independent chains per thread, 64 warps per SM.
+//   kind 0  DFMA  a = fma(a, c1, c2), c1/c2 compile-time constants       (nominal FP64 rate)
+//   kind 1  FFMA  same in fp32
+//   kind 2  DFMA  a_k = fma(b_k, b_k+1, a_k): three distinct 64-bit register operands
+//   kind 3  DFMA  a_k = fma(q, b_k, a_k): one operand shared by consecutive instructions (reuse cache)
+//   kind 4  DADD  a_k = a_k + b_k: two distinct register operands
+template <typename T, int MODE>
 __global__ void __launch_bounds__(256) peak_fma_kernel(T *out, int iters, T seed)
 {
-    T a0 = seed + threadIdx.x, a1 = a0 + 1, a2 = a0 + 2, a3 = a0 + 3, a4 = a0 + 4, a5 = a0 + 5, a6 = a0 + 6, a7 = a0 + 7;
-    const T b = (T)0.999999, c = (T)1e-7;
+    T a[8], b[8];
+    const T q = (T)0.999999 + seed * (T)1e-9;
+#pragma unroll
+    for (int k = 0; k < 8; ++k) {
+        a[k] = seed + (T)(threadIdx.x + k);
+        b[k] = (T)1.0 + (T)1e-9 * (T)(threadIdx.x + k) * seed;
+    }
     for (int i = 0; i < iters; ++i) {
 #pragma unroll
         for (int u = 0; u < 16; ++u) {
-            a0 = fma(a0, b, c); a1 = fma(a1, b, c); a2 = fma(a2, b, c); a3 = fma(a3, b, c);
-            a4 = fma(a4, b, c); a5 = fma(a5, b, c); a6 = fma(a6, b, c); a7 = fma(a7, b, c);
+#pragma unroll
+            for (int k = 0; k < 8; ++k) {
+                if (MODE == 0) a[k] = fma(a[k], (T)0.999999, (T)1e-7);
+                if (MODE == 2) a[k] = fma(b[k], b[(k + 1) & 7], a[k]);
+                if (MODE == 3) a[k] = fma(q, b[k], a[k]);
+                if (MODE == 4) a[k] = a[k] + b[k];
+            }
         }
     }
-    T s = a0 + a1 + a2 + a3 + a4 + a5 + a6 + a7;
+    T s = 0;
+#pragma unroll
+    for (int k = 0; k < 8; ++k) s += a[k] + b[k];
     if (s == (T)123456.789) out[blockIdx.x * blockDim.x + threadIdx.x] = s;   // never true; keeps the chains live
 }
 
@@ -150,10 +168,13 @@ cudaError_t run_peak_fma(int kind, int iters, int sm_count, cudaStream_t st, dou
     void *dummy = nullptr;
     for (int rep = 0; rep < 2; ++rep) {           // first pass warms up
         if (rep == 1) cudaEventRecord(e0, st);
-        if (kind == 0)
-            peak_fma_kernel<double><<<grid, block, 0, st>>>((double *)dummy, iters, 1.0);
-        else
-            peak_fma_kernel<float><<<grid, block, 0, st>>>((float *)dummy, iters, 1.0f);
+        switch (kind) {
+        case 0: peak_fma_kernel<double, 0><<<grid, block, 0, st>>>((double *)dummy, iters, 1.0); break;
+        case 1: peak_fma_kernel<float, 0><<<grid, block, 0, st>>>((float *)dummy, iters, 1.0f); break;
+        case 2: peak_fma_kernel<double, 2><<<grid, block, 0, st>>>((double *)dummy, iters, 1.0); break;
+        case 3: peak_fma_kernel<double, 3><<<grid, block, 0, st>>>((double *)dummy, iters, 1.0); break;
+        default: peak_fma_kernel<double, 4><<<grid, block, 0, st>>>((double *)dummy, iters, 1.0); break;
+        }
     }
     cudaEventRecord(e1, st);
     err = cudaEventSynchronize(e1);

@@ -98,13 +98,16 @@ def test_all_launch_shapes_ragged(order, flags):
     ref, _ = oracle_on_gpu_prediction(ctx, w, order, il, w.eps2, h2, ngb_cap=24)
     shapes = [(L, 1, S, tile) for L in (1, 2, 4, 8, 16, 32) for S, tile in ((1, 0), (3, 64), (13, 32))]
     shapes += [(32, Wj, S, 0) for Wj in (2, 4, 8) for S in (1, 2, 5)]
+    shapes += [(8, 4, 1, 0), (8, 8, 3, 64), (2, 2, 5, 128), (16, 2, 2, 32)]   # warp columns with several i per warp
     for L, Wj, S, tile in shapes:
         s2.s2_set_tuning(ctx, 1, L); s2.s2_set_tuning(ctx, 2, Wj); s2.s2_set_tuning(ctx, 0, S); s2.s2_set_tuning(ctx, 4, tile)
-        s2.s2_calc_ilist(ctx, il, h2, w.eps2, flags)
-        res = s2.s2_get_results(ctx, ni)
-        info = s2.s2_last_launch_info(ctx)
-        assert info["lanes_per_i"] == L and info["warp_columns"] == Wj
-        check_forces(res, ref, s2.S2_FP64, order, flags, f"shape {info}")
+        for unfused, cluster in ((0, 0), (0, 1), (0, 2), (0, 8), (1, 0)):   # fused (auto / no / 2 / 8 CTA clusters), separate reduce
+            s2.s2_set_tuning(ctx, 5, unfused); s2.s2_set_tuning(ctx, 6, cluster)
+            s2.s2_calc_ilist(ctx, il, h2, w.eps2, flags)
+            res = s2.s2_get_results(ctx, ni)
+            info = s2.s2_last_launch_info(ctx)
+            assert info["lanes_per_i"] == L and info["warp_columns"] == Wj
+            check_forces(res, ref, s2.S2_FP64, order, flags, f"shape {info}")
         if flags & NGB:
             assert res["overflow"] == bool((ref.ngb_count > 24).any())
             check_neighbour_lists(ctx, ref, ni, 24, f"shape {info}")
@@ -175,6 +178,16 @@ def test_bit_reproducible_and_paths_agree():
         outs[S] = runs[0]
     assert np.allclose(outs[1], outs[9], rtol=1e-12, atol=0)
     assert np.allclose(outs[0], outs[1], rtol=1e-12, atol=0)
+    # the fused combine (last CTA of an i-group reduces) and the separate reduce kernel add the slice
+    # partials in the same fixed order: bit-identical results
+    s2.s2_set_tuning(ctx, 0, 9)
+    s2.s2_calc_ilist(ctx, il, eps2=w.eps2, flags=NN)
+    assert s2.s2_last_launch_info(ctx)["reduced"] == 2
+    s2.s2_set_tuning(ctx, 5, 1)
+    s2.s2_calc_ilist(ctx, il, eps2=w.eps2, flags=NN)
+    assert s2.s2_last_launch_info(ctx)["reduced"] == 1
+    r = s2.s2_get_results(ctx, 96)
+    assert np.array_equal(np.concatenate([r["acc"].ravel(), r["jerk"].ravel(), r["pot"], r["nn_r2"]]), outs[9])
     s2.s2_close(ctx)
 
 

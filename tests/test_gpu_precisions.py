@@ -31,7 +31,7 @@ def test_precision_paths_all_shapes_ragged(prec, order, flags):
     h2 = w.h2[il] * 0.6 if flags & NGB else None
     ref, _ = oracle_on_gpu_prediction(ctx, w, order, il, w.eps2, h2, ngb_cap=24)
     shapes = [(L, 1, S, tile) for L in (1, 2, 4, 8, 16, 32) for S, tile in ((1, 0), (3, 64), (13, 32))]
-    shapes += [(32, Wj, S, 0) for Wj in (2, 8) for S in (1, 5)]
+    shapes += [(32, Wj, S, 0) for Wj in (2, 8) for S in (1, 5)] + [(8, 4, 3, 64), (4, 2, 1, 0)]
     worst = {}
     for L, Wj, S, tile in shapes:
         s2.s2_set_tuning(ctx, 1, L); s2.s2_set_tuning(ctx, 2, Wj); s2.s2_set_tuning(ctx, 0, S); s2.s2_set_tuning(ctx, 4, tile)
