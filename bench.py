@@ -123,6 +123,14 @@ def run_reference(args, w, rank, world):
     print(json.dumps(line), flush=True)
 
 
+def measured_peaks():
+    try:
+        with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as f:
+            return json.load(f)
+    except Exception:
+        return {}          # fallback figures of B200_PROFILING.md are then used ("of fallback")
+
+
 def workload_config(w, ni):
     return {"workload": f"{w.name}: Plummer sphere N={w.N}, n_i={ni}, {w.order}th-order Hermite, "
                         f"eps={w.notes['eps']:.4g}, {'Salpeter' if w.notes['salpeter'] else 'equal'} masses, "
@@ -263,6 +271,7 @@ def main():
             "dadd_two_registers": s2.s2_peak_fma(ctx, 4, 4000) / nominal,
             "unit": "fraction of 148 SM x 64 lanes x 1.965 GHz lane-instructions/s"}
         line["sweep"] = ni_sweep(s2, torch, dev, order)
+        line["hbm_kernels"] = hbm_kernels(s2, torch, dev, measured_peaks().get("hbm_gbs", 6650.0))
         line["cpu_baseline"] = cpu_baseline(w)
     if rank == 0:
         print(json.dumps(line), flush=True)
@@ -271,38 +280,102 @@ def main():
         dist.destroy_process_group()
 
 
+def graph_time_us(s2, torch, ctx, fn, calls=20, reps=7):
+    """Device time per call of `fn` (which only enqueues library calls): `calls` calls captured in one CUDA
+    graph on a side stream, replayed `reps` times between CUDA events; median.  Removes the host launch cost
+    and the ~6 us floor of an event pair around a single small kernel."""
+    st = torch.cuda.Stream()
+    s2.s2_set_stream(ctx, st.cuda_stream)
+    with torch.cuda.stream(st):
+        fn(); fn()                                   # warm-up: allocations and shape caches settle
+    st.synchronize()
+    g = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(g, stream=st):
+        for _ in range(calls):
+            fn()
+    ts = []
+    for _ in range(reps + 1):
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(); g.replay(); e1.record()
+        torch.cuda.synchronize()
+        ts.append(e0.elapsed_time(e1) / calls * 1e3)
+    s2.s2_set_stream(ctx, torch.cuda.current_stream().cuda_stream)
+    return statistics.median(ts[1:])
+
+
 def ni_sweep(s2, torch, dev, order):
-    """Ginteractions/s versus n_i at config 3's N = 65536 and at the headline N = 2^18 (4th order fp64),
-    kernel time only (force sweep + reduce), as in the paper's Fig. 2 protocol."""
+    """Ginteractions/s versus n_i (4th order): config 3 (N = 65536) in fp64, double-single and fp32, the
+    headline N = 2^18 in fp64, and config 2 (N = 64) latencies.  Device time of one s2_calc_ilist_device call
+    (force sweep + combine), as in the paper's Fig. 2 protocol (kernel time only).  Calls with
+    fewer than 2e8 pairs are timed by CUDA-graph replay of 20 calls, larger ones by CUDA events per call."""
     from workloads import make_config
     out = []
-    for key, nis in ((3, (1, 32, 256, 2048, 16384, 65536)), ("H", (1, 32, 256, 4096, 262144))):
+    plan = ((3, "fp64", s2.S2_FP64, (1, 32, 256, 2048, 16384, 65536)),
+            (3, "ds", s2.S2_DS, (1, 32, 256, 2048, 16384, 65536)),
+            (3, "fp32", s2.S2_FP32, (1, 32, 256, 2048, 16384, 65536)),
+            ("H", "fp64", s2.S2_FP64, (1, 32, 256, 4096, 262144)),
+            (2, "fp64", s2.S2_FP64, (1, 2, 4, 8, 16, 32, 64)))
+    for key, pname, prec, nis in plan:
         w = make_config(key)
-        ctx = s2.s2_open(dev.index, 4, s2.S2_FP64, nj_capacity=w.N, ngb_cap=0)
+        ctx = s2.s2_open(dev.index, 4, prec, nj_capacity=w.N, ngb_cap=0)
         a = np.arange(w.N, dtype=np.int32)
         s2.s2_set_j(ctx, a, w.ident, w.t_j, w.mass, w.pos, w.vel, w.acc, w.jerk)
         s2.s2_commit_j(ctx)
         s2.s2_predict(ctx, w.t_pred, w.N)
-        s2.s2_enable_timing(ctx, True)
         full = None
         rows = []
         for ni in nis[::-1]:
             il = torch.from_numpy(w.ilist(ni)).to(dev)
-            reps = 3 if ni * w.N > 1e9 else 20
-            ts = []
-            for r in range(reps + 2):
-                s2.s2_calc_ilist_device(ctx, il, None, w.eps2, 0)
-                t = s2.s2_get_timing(ctx)
-                if r >= 2:
-                    ts.append(t["force_ms"] + t["reduce_ms"])
-            ms = statistics.median(ts)
-            g = ni * w.N / (ms * 1e-3) / 1e9
+            if ni * w.N >= 2e8:
+                s2.s2_enable_timing(ctx, True)
+                reps = 3 if ni * w.N > 1e9 else 10
+                ts = []
+                for r in range(reps + 2):
+                    s2.s2_calc_ilist_device(ctx, il, None, w.eps2, 0)
+                    t = s2.s2_get_timing(ctx)
+                    if r >= 2:
+                        ts.append(t["force_ms"] + t["reduce_ms"])
+                s2.s2_enable_timing(ctx, False)
+                us, how = statistics.median(ts) * 1e3, "events"
+            else:
+                us, how = graph_time_us(s2, torch, ctx, lambda: s2.s2_calc_ilist_device(ctx, il, None, w.eps2, 0)), "graph"
+            g = ni * w.N / (us * 1e-6) / 1e9
             full = full or g
             info = s2.s2_last_launch_info(ctx)
-            rows.append({"N": w.N, "n_i": ni, "kernel_us": ms * 1e3, "ginteractions_per_s": g,
-                         "frac_fp64_peak_60flop": g * 60e9 / 1e12 / FP64_PEAK_TFLOPS, "vs_full_rate": g / full,
-                         "S": info["S"], "lanes_per_i": info["lanes_per_i"], "warp_columns": info["warp_columns"]})
+            rows.append({"cfg": str(key), "precision": pname, "N": w.N, "n_i": ni, "call_us": round(us, 2), "timing": how,
+                         "ginteractions_per_s": g, "vs_full_rate": g / full,
+                         "S": info["S"], "lanes_per_i": info["lanes_per_i"], "warp_columns": info["warp_columns"],
+                         "combine": ("none", "reduce kernel", "fused")[info["reduced"]]})
         out.extend(rows[::-1])
+        s2.s2_close(ctx)
+    return out
+
+
+def hbm_kernels(s2, torch, dev, hbm_gbs):
+    """Achieved HBM GB/s of the streaming kernels: the predictor (a2) and the commit scatter (a1, from device
+    arrays) at N = 2^20 with config 5's (4th order) and config 4's (6th order) particle recipe.
+    Algorithmic bytes per j are those of DESIGN.md 5.1; graph-replay timing."""
+    from workloads import make_config
+    out = []
+    for key, order in ((5, 4), (4, 6)):
+        w = make_config(key, N=1 << 20)            # both orders at N = 2^20: the working set exceeds the 126 MB L2
+        ctx = s2.s2_open(dev.index, order, s2.S2_FP64, nj_capacity=w.N, ngb_cap=0)
+        names = ["ident", "t_j", "mass", "pos", "vel", "acc", "jerk"] + (["snap", "crackle"] if order == 6 else [])
+        d = {k: torch.from_numpy(getattr(w, k)).to(dev) for k in names}
+        addr = torch.arange(w.N, dtype=torch.int32, device=dev)
+        args = [addr, d["ident"], d["t_j"], d["mass"], d["pos"], d["vel"], d["acc"], d["jerk"]]
+        args += [d["snap"], d["crackle"]] if order == 6 else [None, None]
+        commit = lambda: s2.s2_commit_j_device(ctx, *args)
+        commit()
+        us_c = graph_time_us(s2, torch, ctx, commit, calls=10)
+        us_p = graph_time_us(s2, torch, ctx, lambda: s2.s2_predict(ctx, w.t_pred, w.N), calls=10)
+        nf = 20 if order == 6 else 14
+        b_commit = w.N * ((nf * 8 + 8) + (nf * 8 + 4))
+        b_pred = w.N * ((nf * 8 + 4) + (96 if order == 6 else 64))
+        for name, us, b in (("scatter_kernel", us_c, b_commit), (f"predict_kernel<{order}>", us_p, b_pred)):
+            gbs = b / (us * 1e-6) / 1e9
+            out.append({"kernel": name, "N": w.N, "order": order, "bytes": b, "us": round(us, 2), "GB/s": gbs,
+                        "frac_of_measured_hbm": gbs / hbm_gbs})
         s2.s2_close(ctx)
     return out
 

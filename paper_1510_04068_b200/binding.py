@@ -74,7 +74,7 @@ def lib() -> C.CDLL:
         "s2_get_predicted_j": (C.c_int, [vp, C.c_int, C.c_int, dp, dp, dp]),
         "s2_get_j": (C.c_int, [vp, C.c_int, C.c_int, ip, dp, dp, dp]),
         "s2_set_tuning": (C.c_int, [vp, C.c_int, C.c_int]),
-        "s2_last_launch_info": (C.c_int, [vp, C.POINTER(C.c_int * 8)]),
+        "s2_last_launch_info": (C.c_int, [vp, C.POINTER(C.c_int * 10)]),
         "s2_kernel_launches": (C.c_longlong, [vp]),
         "s2_enable_timing": (C.c_int, [vp, C.c_int]),
         "s2_get_timing": (C.c_int, [vp, C.POINTER(C.c_float), C.POINTER(C.c_float), C.POINTER(C.c_float)]),
@@ -319,9 +319,10 @@ def s2_set_tuning(ctx, key: int, value: int):
 
 
 def s2_last_launch_info(ctx) -> dict:
-    arr = (C.c_int * 8)()
+    arr = (C.c_int * 10)()
     _check(lib().s2_last_launch_info(ctx.handle, C.byref(arr)), "s2_last_launch_info", ctx.handle)
-    keys = ("S", "lanes_per_i", "warp_columns", "grid", "threads", "smem", "reduced", "ctas_per_sm")
+    keys = ("S", "lanes_per_i", "warp_columns", "grid", "threads", "smem", "reduced", "ctas_per_sm", "i_per_thread",
+            "cluster")
     return dict(zip(keys, list(arr)))
 
 

@@ -63,8 +63,8 @@ struct s2_ctx {
     double t_pred = 0.0;
 
     // tuning overrides and last launch
-    int tune[7] = {0, 0, 0, 0, 0, 0, 0};
-    int last_info[8] = {0, 0, 0, 0, 0, 0, 0, 0};
+    int tune[8] = {0, 0, 0, 0, 0, 0, 0, 0};
+    int last_info[10] = {0, 0, 0, 0, 0, 0, 0, 0, 1, 1};
     std::map<long long, int> occ_cache;
     std::map<long long, std::pair<ForceShape, int>> shape_cache;
 
@@ -422,13 +422,14 @@ static cudaError_t dispatch(int precision, int order, unsigned flags, int L, dim
 //   the combine costs one launch gap when it is a separate kernel, or a short serial tail in the last CTA of
 //   each i-group when it is fused.
 struct ShapeCost {
-    double t_iter, c_cta, c_row, c_launch;
+    double t_iter, c_cta, c_row, c_launch, tiled_gain;
 };
 static ShapeCost cost_params(int precision, int order)
 {
     ShapeCost c;
     c.t_iter = precision == S2_FP64 ? 146.0 : (precision == S2_FP32 ? 100.0 : 1400.0);
     if (order == 6) c.t_iter *= 1.7;
+    c.tiled_gain = 0.93;  // measured: pairs of the register-tiled sweep cost this fraction of the plain ones
     c.c_cta = 4000.0;     // ~2 us: launch ramp, first tile, i-gather, shuffles, record write
     c.c_row = 1000.0;     // ~0.5 us per round of 32 partial rows (L2 latency bound)
     c.c_launch = 4000.0;  // ~2 us: second launch (programmatic dependent launch hides part of it)
@@ -460,7 +461,7 @@ static int query_occ(s2_ctx *ctx, unsigned flags, int L, int npl, int *occ_out)
 // buffers.  Automatic choices are cached per (n_i, n_j, flags); s2_set_tuning overrides any of them.
 static int choose_shape(s2_ctx *ctx, int ni, int nj, unsigned flags, ForceShape *out)
 {
-    const bool tuned = ctx->tune[0] || ctx->tune[1] || ctx->tune[2] || ctx->tune[3] || ctx->tune[4] || ctx->tune[5] || ctx->tune[6];
+    const bool tuned = ctx->tune[0] || ctx->tune[1] || ctx->tune[2] || ctx->tune[3] || ctx->tune[4] || ctx->tune[5] || ctx->tune[6] || ctx->tune[7];
     const long long ckey = ((long long)ni << 34) ^ ((long long)nj << 3) ^ (long long)flags;
     if (!tuned) {
         auto it = ctx->shape_cache.find(ckey);
@@ -477,19 +478,26 @@ static int choose_shape(s2_ctx *ctx, int ni, int nj, unsigned flags, ForceShape 
 
     double best = 1e300;
     int bL = 1, bWj = 1, bS = 1, bocc = 1, bfused = 0, bC = 1;
-    for (int L = 1; L <= 32; L <<= 1) {
-        if (ctx->tune[1] > 0 && L != ctx->tune[1]) continue;
+    const int ipt_max = force_ipt(ctx->precision);
+    for (int Lc = 0; Lc <= 6; ++Lc) {
+        // Lc = 0: register-tiled sweep (one lane per i, ipt_max i per thread); Lc = 1..6: L = 1, 2, 4, .., 32 lanes per i
+        const int L = Lc == 0 ? 0 : 1 << (Lc - 1);
+        const int ipt = L == 0 ? ipt_max : 1;
+        if (L == 0 && (ipt_max < 2 || ctx->tune[7] == 1)) continue;
+        if (ctx->tune[7] >= 2 && L != 0) continue;
+        if (ctx->tune[1] > 0 && (L == 0 ? 1 : L) != ctx->tune[1]) continue;
         int occ;
         int rc = query_occ(ctx, flags, L, npl, &occ);
         if (rc != S2_OK) return rc;
         for (int Wj = 1; Wj <= kWarps; Wj <<= 1) {
             // warp columns: warps of a CTA share i-particles and split every tile (the paper's 2D blocks, L104);
-            // worth it only while the i-list does not fill the i-groups anyway
-            if (ctx->tune[2] > 0 ? Wj != ctx->tune[2] : (Wj > 1 && (L == 1 || (long long)ni * L * Wj > 2048))) continue;
-            if (Wj > 1 && L == 1) continue;
-            const int icta = (kWarps / Wj) * (32 / L);
+            // used only while the i-list cannot fill one CTA with L lanes per i (measured: otherwise the extra
+            // i-groups re-stream the j range from L2 and lose, profiles/r01_small_ni.md)
+            if (ctx->tune[2] > 0 ? Wj != ctx->tune[2] : (Wj > 1 && (L <= 1 || (long long)ni * L * Wj > kThreads))) continue;
+            if (Wj > 1 && L <= 1) continue;
+            const int icta = L == 0 ? kThreads * ipt : (kWarps / Wj) * (32 / L);
             const int Gi = (ni + icta - 1) / icta;
-            const int lanes_j = L * Wj;                         // lanes (over all warp columns) sharing one i
+            const int lanes_j = std::max(1, L) * Wj;             // lanes (over all warp columns) sharing one i
             const int min_slice = std::max(32, 2 * lanes_j);
             const int smax = std::min(65535, std::max(1, nj / min_slice));
             // candidate slice counts: 1, and those that make the grid k x SMs (k = 1..16)
@@ -507,7 +515,7 @@ static int choose_shape(s2_ctx *ctx, int ni, int nj, unsigned flags, ForceShape 
                 int S = cand[q];
                 // neighbour segments must stay ascending per record: a warp column may then only take a part of ONE tile
                 if (want_ngb && Wj > 1 && (nj + S - 1) / S > tile_max) S = (nj + tile_max - 1) / tile_max;
-                const bool fusable = !want_ngb && ctx->tune[5] == 0 && S * Wj > 1;
+                const bool fusable = !want_ngb && ctx->tune[5] == 0 && S * Wj > 1 && L != 0;
                 // clusters of C CTAs along the slice axis pre-combine their records through distributed shared
                 // memory (j-split shapes only: their record block, <= 128 x 96 B, always fits the tile buffers)
                 int C = 1;
@@ -525,7 +533,8 @@ static int choose_shape(s2_ctx *ctx, int ni, int nj, unsigned flags, ForceShape 
                 // lanes that share an i read different j: LDS.128 is conflict-free up to 8 distinct addresses
                 // measured (profiles/r01_small_ni.md): a lone CTA per SM is latency-bound (~1.25x), lanes that
                 // share an i read different j (LDS.128 conflict-free up to L = 8, 2- and 4-way above)
-                const double t_iter = C_.t_iter * (n_sm >= 2 ? 1.0 : 1.25) * (1.0 + 0.01 * L) * (L > 8 ? 1.0 + 0.01 * L : 1.0);
+                double t_iter = C_.t_iter * (n_sm >= 2 ? 1.0 : 1.25) * (1.0 + 0.01 * L) * (L > 8 ? 1.0 + 0.01 * L : 1.0);
+                if (L == 0) t_iter = C_.t_iter * ipt * C_.tiled_gain;   // ipt pairs per lane and j, fewer shared-memory reads each
                 // every i-group streams the whole j range from L2 (~2500 B per SM-cycle over the chip)
                 const double stream = (double)Gi * nj * npl * 16.0 / 2500.0;
                 double cost = std::ceil(n_sm / occ) * C_.c_cta + std::max(n_sm * iters * t_iter, stream);
@@ -591,7 +600,7 @@ static int run_force(s2_ctx *ctx, int ni, const int *d_i_addr, const double *d_h
     const bool want_ngb = flags & S2_WANT_NGB;
     const bool final_direct = nst == 1;
     // without neighbour lists the combine is fused into the sweep launch (last CTA of an i-group reduces)
-    const int icta_ = (kWarps / sh.Wj) * (32 / sh.L);
+    const int icta_ = sh.L == 0 ? kThreads * force_ipt(ctx->precision) : (kWarps / sh.Wj) * (32 / sh.L);
     const int Gi_ = (ni + icta_ - 1) / icta_;
     const bool fused = sh.fused != 0;
 
@@ -655,7 +664,7 @@ static int run_force(s2_ctx *ctx, int ni, const int *d_i_addr, const double *d_h
     a.order = ctx->order;
 
     if (want_ngb) CU(cudaMemsetAsync(ctx->flags.p, 0, sizeof(int), ctx->stream));   // overflow flag of this call
-    const int icta = (kWarps / sh.Wj) * (32 / sh.L);
+    const int icta = icta_;
     dim3 grid((ni + icta - 1) / icta, sh.S);
     size_t smem = force_smem_bytes(force_nplanes(ctx->precision, ctx->order, flags), sh.tile, sh.stages);
     smem = std::max(smem, (size_t)kSmemHeader + (size_t)icta * sh.Wj * REC * sizeof(double));   // record block of the combines
@@ -686,8 +695,9 @@ static int run_force(s2_ctx *ctx, int ni, const int *d_i_addr, const double *d_h
         ctx->ran_reduce = true;
     }
     int *li = ctx->last_info;
-    li[0] = sh.S; li[1] = sh.L; li[2] = sh.Wj; li[3] = (int)(grid.x * grid.y); li[4] = kThreads;
+    li[0] = sh.S; li[1] = sh.L == 0 ? 1 : sh.L; li[2] = sh.Wj; li[3] = (int)(grid.x * grid.y); li[4] = kThreads;
     li[5] = (int)smem; li[6] = final_direct ? 0 : (fused ? 2 : 1);
+    li[8] = sh.L == 0 ? force_ipt(ctx->precision) : 1; li[9] = a.cluster;
     ctx->calc_done = true;
     ctx->ni_last = ni;
     ctx->flags_last = flags;
@@ -971,12 +981,12 @@ extern "C" int s2_get_j(s2_ctx *ctx, int first, int n, int *id, double *t, doubl
 
 extern "C" int s2_set_tuning(s2_ctx *ctx, int key, int value)
 {
-    if (!ctx || key < 0 || key > 6 || value < 0) return S2_EINVAL;
+    if (!ctx || key < 0 || key > 7 || value < 0) return S2_EINVAL;
     ctx->tune[key] = value;
     return S2_OK;
 }
 
-extern "C" int s2_last_launch_info(const s2_ctx *ctx, int out[8])
+extern "C" int s2_last_launch_info(const s2_ctx *ctx, int out[10])
 {
     if (!ctx || !out) return S2_EINVAL;
     memcpy(out, ctx->last_info, sizeof ctx->last_info);

@@ -105,6 +105,7 @@ struct PolicyDS {
     static constexpr int NPL = NQ + (DEC ? 2 : 0);
     static constexpr int kMinBlocks = 2;
     static constexpr int kUnroll = 1;
+    static constexpr int kIPT = kIptDS;          // no register tiling: a double-single pair is ~400 FP32 instructions
 
     struct IState {
         ds x, y, z, vx, vy, vz, ax, ay, az, eps2;

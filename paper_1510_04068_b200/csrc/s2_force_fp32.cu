@@ -30,6 +30,15 @@ struct PolicyF32 {
     static constexpr int NPL = NQ + (DEC ? 2 : 0);    // + fp64 position planes for the decisions
     static constexpr int kMinBlocks = 2;
     static constexpr int kUnroll = 4;
+    static constexpr int kIPT = kIptF32;          // i-particles per thread in the register-tiled sweep
+#ifndef S2_F32_UNROLL_TILED
+#define S2_F32_UNROLL_TILED 2
+#endif
+#ifndef S2_F32_MINBLOCKS_TILED
+#define S2_F32_MINBLOCKS_TILED 2
+#endif
+    static constexpr int kUnrollTiled = S2_F32_UNROLL_TILED;
+    static constexpr int kMinBlocksTiled = S2_F32_MINBLOCKS_TILED;
 
     struct IState {
         float xh, yh, zh, xl, yl, zl, vx, vy, vz, ax, ay, az, eps2;
@@ -97,18 +106,40 @@ struct PolicyF32 {
         I.eps2 = (float)a.eps2;
     }
 
+    struct JData {
+        float4 f0, f1, f2, f3;
+        double2 p0, p1;
+    };
+    static __device__ __forceinline__ void load_j(const unsigned char *stage, int tile, int k, JData &J)
+    {
+        const float4 *pl = reinterpret_cast<const float4 *>(stage);
+        J.f0 = pl[k]; J.f1 = pl[tile + k]; J.f2 = pl[2 * tile + k];
+        if (ORDER == 6) J.f3 = pl[3 * tile + k];
+        if (DEC) {
+            const double2 *pd = reinterpret_cast<const double2 *>(stage);
+            J.p0 = pd[NQ * tile + k]; J.p1 = pd[(NQ + 1) * tile + k];
+        }
+    }
+
     template <int L, bool MASKED>
     static __device__ __forceinline__ void pair(const unsigned char *stage, int tile, int k, bool valid, int jaddr,
                                                 const IState &I, Part &A, Dec &D, const Decomp &d, int *seg,
                                                 int segcap)
     {
-        const float4 *pl = reinterpret_cast<const float4 *>(stage);
-        const float4 f0 = pl[k], f1 = pl[tile + k], f2 = pl[2 * tile + k];
+        JData J;
+        load_j(stage, tile, k, J);
+        interact<L, MASKED>(J, valid, jaddr, I, A, D, d, seg, segcap);
+    }
+
+    template <int L, bool MASKED>
+    static __device__ __forceinline__ void interact(const JData &J, bool valid, int jaddr, const IState &I, Part &A,
+                                                    Dec &D, const Decomp &d, int *seg, int segcap)
+    {
+        const float4 f0 = J.f0, f1 = J.f1, f2 = J.f2;
         const bool skip = (__float_as_int(f1.w) == I.id) || (MASKED && !valid);
 
         if (DEC) {
-            const double2 *pd = reinterpret_cast<const double2 *>(stage);
-            const double2 p0 = pd[NQ * tile + k], p1 = pd[(NQ + 1) * tile + k];
+            const double2 p0 = J.p0, p1 = J.p1;
             const double ex = p0.x - I.x, ey = p0.y - I.y, ez = p1.x - I.z;
             const double d2 = __fma_rn(ez, ez, __fma_rn(ey, ey, __dmul_rn(ex, ex)));
             decide<L, NN, NGB>(d2, jaddr, skip, I.h2, D, d, seg, segcap);
@@ -132,7 +163,7 @@ struct PolicyF32 {
         A.ax = fmaf(q, dx, A.ax); A.ay = fmaf(q, dy, A.ay); A.az = fmaf(q, dz, A.az);
         A.jx = fmaf(q, tx, A.jx); A.jy = fmaf(q, ty, A.jy); A.jz = fmaf(q, tz, A.jz);
         if (ORDER == 6) {
-            const float4 f3 = pl[3 * tile + k];
+            const float4 f3 = J.f3;
             const float dax = f3.x - I.ax, day = f3.y - I.ay, daz = f3.z - I.az;
             const float w = fmaf(dvx, dvx, fmaf(dvy, dvy, fmaf(dvz, dvz, fmaf(dx, dax, fmaf(dy, day, dz * daz)))));
             const float b3 = -3.f * fmaf(w, y2, alpha * alpha);

@@ -32,6 +32,15 @@ struct PolicyF64 {
 #endif
     static constexpr int kMinBlocks = S2_F64_MINBLOCKS;
     static constexpr int kUnroll = S2_F64_UNROLL;   // pairs in flight per thread in the one-lane-per-i loop
+#ifndef S2_F64_UNROLL_TILED
+#define S2_F64_UNROLL_TILED 4
+#endif
+#ifndef S2_F64_MINBLOCKS_TILED
+#define S2_F64_MINBLOCKS_TILED 2
+#endif
+    static constexpr int kMinBlocksTiled = S2_F64_MINBLOCKS_TILED;
+    static constexpr int kIPT = kIptF64;                        // i-particles per thread in the register-tiled sweep
+    static constexpr int kUnrollTiled = S2_F64_UNROLL_TILED;    // j per unrolled step there (x kIPT pairs in flight)
 
     struct IState {
         double x, y, z, vx, vy, vz, ax, ay, az, h2, eps2;
@@ -87,13 +96,31 @@ struct PolicyF64 {
         I.eps2 = a.eps2;
     }
 
+    struct JData {   // one j-particle as read from the shared-memory planes
+        double2 p0, p1, p2, p3, p4, p5;
+    };
+    static __device__ __forceinline__ void load_j(const unsigned char *stage, int tile, int k, JData &J)
+    {
+        const double2 *pl = reinterpret_cast<const double2 *>(stage);
+        J.p0 = pl[k]; J.p1 = pl[tile + k]; J.p2 = pl[2 * tile + k]; J.p3 = pl[3 * tile + k];
+        if (ORDER == 6) { J.p4 = pl[4 * tile + k]; J.p5 = pl[5 * tile + k]; }
+    }
+
     template <int L, bool MASKED>
     static __device__ __forceinline__ void pair(const unsigned char *stage, int tile, int k, bool valid, int jaddr,
                                                 const IState &I, Acc &A, Dec &D, const Decomp &d, int *seg,
                                                 int segcap)
     {
-        const double2 *pl = reinterpret_cast<const double2 *>(stage);
-        const double2 p0 = pl[k], p1 = pl[tile + k], p2 = pl[2 * tile + k], p3 = pl[3 * tile + k];
+        JData J;
+        load_j(stage, tile, k, J);
+        interact<L, MASKED>(J, valid, jaddr, I, A, D, d, seg, segcap);
+    }
+
+    template <int L, bool MASKED>
+    static __device__ __forceinline__ void interact(const JData &J, bool valid, int jaddr, const IState &I, Acc &A,
+                                                    Dec &D, const Decomp &d, int *seg, int segcap)
+    {
+        const double2 p0 = J.p0, p1 = J.p1, p2 = J.p2, p3 = J.p3;
         const bool skip = (__double2loint(p3.y) == I.id) || (MASKED && !valid);
 
         const double dx = p0.x - I.x, dy = p0.y - I.y, dz = p1.x - I.z;
@@ -126,7 +153,7 @@ struct PolicyF64 {
         A.ax = fma(q, dx, A.ax); A.ay = fma(q, dy, A.ay); A.az = fma(q, dz, A.az);
         A.jx = fma(q, tx, A.jx); A.jy = fma(q, ty, A.jy); A.jz = fma(q, tz, A.jz);
         if (ORDER == 6) {
-            const double2 p4 = pl[4 * tile + k], p5 = pl[5 * tile + k];
+            const double2 p4 = J.p4, p5 = J.p5;
             const double dax = p4.x - I.ax, day = p4.y - I.ay, daz = p5.x - I.az;
             const double w = fma(dvx, dvx, fma(dvy, dvy, fma(dvz, dvz, fma(dx, dax, fma(dy, day, dz * daz)))));
             const double b3 = -3.0 * fma(w, y2, alpha * alpha);

@@ -130,6 +130,60 @@ __device__ __forceinline__ void reduce_rows_warp(const double *part, double *out
     }
 }
 
+// Ring of ST shared-memory tile buffers filled by 1-D bulk copies (one per plane) that complete on an mbarrier.
+// Thread 0 issues; everybody waits on the barrier of the tile it is about to read.
+template <int NPL>
+struct TilePipe {
+    uint64_t *full;
+    unsigned char *tiles;
+    const ForceArgs *a;
+    int ST, tile, j0, j1, ntiles;
+    size_t stage_bytes;
+
+    __device__ __forceinline__ void init(unsigned char *smem_raw, const ForceArgs &args)
+    {
+        a = &args;
+        full = reinterpret_cast<uint64_t *>(smem_raw);
+        tiles = smem_raw + kSmemHeader;
+        ST = args.stages;
+        tile = args.tile;
+        stage_bytes = (size_t)NPL * tile * 16;
+        j0 = blockIdx.y * args.slice_len;
+        j1 = min(args.nj, j0 + args.slice_len);
+        ntiles = j1 > j0 ? (j1 - j0 + tile - 1) / tile : 0;
+        if (threadIdx.x == 0) {
+            for (int s = 0; s < ST; ++s) mbar_init(&full[s], 1);
+            mbar_fence_init();
+        }
+        __syncthreads();
+        if (threadIdx.x == 0)
+            for (int t = 0; t < min(ntiles, ST - 1); ++t) issue(t);   // prologue: ST-1 tiles in flight
+    }
+    __device__ __forceinline__ void issue(int t) const
+    {
+        const int st = t % ST;
+        const int jt = j0 + t * tile;
+        const uint32_t bytes = (uint32_t)min(tile, j1 - jt) * 16u;
+        mbar_arrive_expect_tx(&full[st], bytes * NPL);
+#pragma unroll
+        for (int p = 0; p < NPL; ++p)
+            bulk_g2s(tiles + st * stage_bytes + (size_t)p * tile * 16,
+                     reinterpret_cast<const unsigned char *>(a->jp[p]) + (size_t)jt * 16, bytes, &full[st]);
+    }
+    // start of tile t: refill the stage released by the barrier that ended tile t-1, then wait for tile t
+    __device__ __forceinline__ const unsigned char *acquire(int t) const
+    {
+        if (threadIdx.x == 0 && t + ST - 1 < ntiles) issue(t + ST - 1);
+        mbar_wait(&full[t % ST], (t / ST) & 1);
+        return tiles + (t % ST) * stage_bytes;
+    }
+    // end of tile t: a barrier is only needed when this stage will be refilled
+    __device__ __forceinline__ void release(int t) const
+    {
+        if (t + ST < ntiles) __syncthreads();
+    }
+};
+
 // Policy interface (see PolicyF64 in s2_force_fp64.cu):
 //   NPL, kMinBlocks, NN, NGB, ORDER
 //   struct IState; static void load_i(const ForceArgs&, int i, IState&)
@@ -141,37 +195,12 @@ template <class P, int L>
 __global__ void __launch_bounds__(kThreads, P::kMinBlocks) force_sweep_kernel(const ForceArgs a)
 {
     extern __shared__ __align__(128) unsigned char smem_raw[];
-    uint64_t *full = reinterpret_cast<uint64_t *>(smem_raw);
-    unsigned char *tiles = smem_raw + kSmemHeader;
     constexpr int NPL = P::NPL;
-    const int ST = a.stages;   // ring of ST tile buffers (2..kMaxStages), each filled by NPL bulk copies
-
     const Decomp d = decompose<L>(a.Wj, a.ni);
-    const int tile = a.tile;
-    const size_t stage_bytes = (size_t)NPL * tile * 16;
-
-    const int j0 = blockIdx.y * a.slice_len;
-    const int j1 = min(a.nj, j0 + a.slice_len);
-    const int ntiles = j1 > j0 ? (j1 - j0 + tile - 1) / tile : 0;
-
-    if (threadIdx.x == 0) {
-        for (int s = 0; s < ST; ++s) mbar_init(&full[s], 1);
-        mbar_fence_init();
-    }
-    __syncthreads();
-
-    auto issue = [&](int t) {
-        const int st = t % ST;
-        const int jt = j0 + t * tile;
-        const uint32_t bytes = (uint32_t)min(tile, j1 - jt) * 16u;
-        mbar_arrive_expect_tx(&full[st], bytes * NPL);
-#pragma unroll
-        for (int p = 0; p < NPL; ++p)
-            bulk_g2s(tiles + st * stage_bytes + (size_t)p * tile * 16,
-                     reinterpret_cast<const unsigned char *>(a.jp[p]) + (size_t)jt * 16, bytes, &full[st]);
-    };
-    if (threadIdx.x == 0)
-        for (int t = 0; t < min(ntiles, ST - 1); ++t) issue(t);   // prologue: ST-1 tiles in flight
+    TilePipe<NPL> pipe;
+    pipe.init(smem_raw, a);
+    unsigned char *tiles = pipe.tiles;
+    const int tile = a.tile, j0 = pipe.j0, j1 = pipe.j1, ntiles = pipe.ntiles;
     // let a dependent launch (the reduce kernel, launched with programmatic stream serialisation) be staged now;
     // it waits for this grid's completion itself (griddepcontrol.wait)
     asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
@@ -190,10 +219,7 @@ __global__ void __launch_bounds__(kThreads, P::kMinBlocks) force_sweep_kernel(co
     if (P::NGB) seg = a.seg + ((size_t)d.i * a.nslices_total + d.slice) * a.segcap;
 
     for (int t = 0; t < ntiles; ++t) {
-        // stage (t-1) % ST was released by the barrier that ended tile t-1: refill it with tile t+ST-1
-        if (threadIdx.x == 0 && t + ST - 1 < ntiles) issue(t + ST - 1);
-        mbar_wait(&full[t % ST], (t / ST) & 1);
-        const unsigned char *stage = tiles + (t % ST) * stage_bytes;
+        const unsigned char *stage = pipe.acquire(t);
         const int jt = j0 + t * tile;
         const int cnt = min(tile, j1 - jt);
         // this warp column's sub-range of the tile
@@ -222,7 +248,7 @@ __global__ void __launch_bounds__(kThreads, P::kMinBlocks) force_sweep_kernel(co
             }
         }
         tot.add(part);   // two-level accumulation: per-tile partial sums, then the running total
-        if (t + ST < ntiles) __syncthreads();   // only needed when this stage will be refilled
+        pipe.release(t);
     }
 
     // combine the L lanes of each i in a fixed (butterfly) order
@@ -371,6 +397,81 @@ __global__ void __launch_bounds__(kThreads, P::kMinBlocks) force_sweep_kernel(co
     }
 }
 
+// Register-tiled full-occupancy sweep (a4): one lane per i as in force_sweep_kernel<P, 1>, but every thread holds
+// IPT i-particles, so each j read from shared memory (4-6 LDS.128 broadcasts) feeds IPT pair evaluations.
+// Measured on B200: an LDS.128 costs the FP64 path ~2.75 cycles of register-file bandwidth, so
+// halving the loads per pair is worth more than the occupancy it costs.  i-index of slot u of a thread:
+// (blockIdx.x * IPT + u) * kThreads + threadIdx.x.  No warp columns, no cluster, no fused combine on this path:
+// the grid is large, slices are combined by reduce_kernel (or there is a single slice).
+template <class P, int IPT>
+__global__ void __launch_bounds__(kThreads, P::kMinBlocksTiled) force_sweep_tiled_kernel(const ForceArgs a)
+{
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    constexpr int NPL = P::NPL;
+    TilePipe<NPL> pipe;
+    pipe.init(smem_raw, a);
+    const int tile = a.tile;
+    asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
+
+    Decomp d[IPT];
+    typename P::IState I[IPT];
+    typename P::Acc tot[IPT];
+    typename P::Part part[IPT];
+    Dec D[IPT];
+    int *seg[IPT];
+#pragma unroll
+    for (int u = 0; u < IPT; ++u) {
+        d[u].lane = threadIdx.x & 31;
+        d[u].il = d[u].lane; d[u].jl = 0; d[u].wi = threadIdx.x >> 5; d[u].wj = 0;
+        d[u].i = (blockIdx.x * IPT + u) * kThreads + threadIdx.x;
+        d[u].i_valid = d[u].i < a.ni;
+        if (!d[u].i_valid) d[u].i = a.ni - 1;   // padding slots recompute the last i and never write
+        d[u].slice = blockIdx.y;
+        P::load_i(a, d[u].i, I[u]);
+        tot[u].zero();
+        D[u].nn_d2 = CUDART_INF; D[u].nn_j = -1; D[u].cnt = 0;
+        seg[u] = P::NGB ? a.seg + ((size_t)d[u].i * a.nslices_total + d[u].slice) * a.segcap : nullptr;
+    }
+
+    for (int t = 0; t < pipe.ntiles; ++t) {
+        const unsigned char *stage = pipe.acquire(t);
+        const int jt = pipe.j0 + t * tile;
+        const int cnt = min(tile, pipe.j1 - jt);
+#pragma unroll
+        for (int u = 0; u < IPT; ++u) part[u].zero();
+#pragma unroll P::kUnrollTiled
+        for (int k = 0; k < cnt; ++k) {
+            typename P::JData J;
+            P::load_j(stage, tile, k, J);
+#pragma unroll
+            for (int u = 0; u < IPT; ++u)
+                P::template interact<1, false>(J, true, jt + k, I[u], part[u], D[u], d[u], seg[u], a.segcap);
+        }
+#pragma unroll
+        for (int u = 0; u < IPT; ++u) tot[u].add(part[u]);
+        pipe.release(t);
+    }
+
+#pragma unroll
+    for (int u = 0; u < IPT; ++u) {
+        if (!d[u].i_valid) continue;
+        double out[10];
+        tot[u].to_f64(out);
+        int nn = D[u].nn_j;
+        if (a.is_final) {
+            if (P::NN && nn >= 0) nn = __double2loint(a.jid_plane[nn].y);
+            if (P::NGB && D[u].cnt > a.ngb_cap) *a.overflow_flag = 1;
+        }
+        double2 *r2 = reinterpret_cast<double2 *>(a.rec + ((size_t)blockIdx.y * a.ni + d[u].i) * REC);
+        r2[0] = make_double2(out[0], out[1]);
+        r2[1] = make_double2(out[2], out[3]);
+        r2[2] = make_double2(out[4], out[5]);
+        r2[3] = make_double2(out[6], D[u].nn_d2);
+        r2[4] = make_double2(__hiloint2double(D[u].cnt, nn), out[7]);
+        r2[5] = make_double2(out[8], out[9]);
+    }
+}
+
 // Host side: instantiate the kernel for a policy and launch it (or query its occupancy) for the
 // run-time lane count L.
 template <class P>
@@ -394,6 +495,18 @@ cudaError_t launch_L(int L, dim3 grid, size_t smem, const ForceArgs &a, cudaStre
         }                                                                                                    \
         kern<<<grid, kThreads, smem, st>>>(a);                                                               \
         return cudaGetLastError();                                                                           \
+    }
+    if (L == 0) {   // register-tiled full-occupancy sweep, P::kIPT i-particles per thread
+        if constexpr (P::kIPT >= 2) {
+            auto kern = force_sweep_tiled_kernel<P, P::kIPT>;
+            cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+            if (e != cudaSuccess) return e;
+            if (query) return cudaOccupancyMaxActiveBlocksPerMultiprocessor(ctas_per_sm, kern, kThreads, smem);
+            kern<<<grid, kThreads, smem, st>>>(a);
+            return cudaGetLastError();
+        } else {
+            return cudaErrorInvalidValue;
+        }
     }
     switch (L) {
         S2_CASE(1)

@@ -34,6 +34,15 @@ constexpr int REC = 12;            // doubles per result record (96 B = three 32
 #endif
 constexpr int kThreads = S2_THREADS;   // threads per force CTA
 constexpr int kWarps = kThreads / 32;
+// i-particles per thread of the register-tiled full-occupancy sweep (force_sweep_tiled_kernel); 1 = not built
+#ifndef S2_F64_IPT
+#define S2_F64_IPT 2
+#endif
+#ifndef S2_F32_IPT
+#define S2_F32_IPT 2
+#endif
+constexpr int kIptF64 = S2_F64_IPT, kIptF32 = S2_F32_IPT, kIptDS = 1;
+inline int force_ipt(int precision) { return precision == S2_FP64 ? kIptF64 : (precision == S2_FP32 ? kIptF32 : kIptDS); }
 
 inline int nfields(int order) { return order == 6 ? 20 : 14; }
 inline int nplanes(int order) { return order == 6 ? 6 : 4; }

@@ -101,12 +101,15 @@ def test_all_launch_shapes_ragged(order, flags):
     shapes += [(8, 4, 1, 0), (8, 8, 3, 64), (2, 2, 5, 128), (16, 2, 2, 32)]   # warp columns with several i per warp
     for L, Wj, S, tile in shapes:
         s2.s2_set_tuning(ctx, 1, L); s2.s2_set_tuning(ctx, 2, Wj); s2.s2_set_tuning(ctx, 0, S); s2.s2_set_tuning(ctx, 4, tile)
-        for unfused, cluster in ((0, 0), (0, 1), (0, 2), (0, 8), (1, 0)):   # fused (auto / no / 2 / 8 CTA clusters), separate reduce
-            s2.s2_set_tuning(ctx, 5, unfused); s2.s2_set_tuning(ctx, 6, cluster)
+        # fused combine (auto / no / 2 / 8 CTA clusters), separate reduce kernel, and for one lane per i the
+        # register-tiled sweep (several i per thread)
+        modes = [(0, 0, 1), (0, 1, 1), (0, 2, 1), (0, 8, 1), (1, 0, 1)] + ([(0, 0, 2)] if L == 1 else [])
+        for unfused, cluster, tiled in modes:
+            s2.s2_set_tuning(ctx, 5, unfused); s2.s2_set_tuning(ctx, 6, cluster); s2.s2_set_tuning(ctx, 7, tiled)
             s2.s2_calc_ilist(ctx, il, h2, w.eps2, flags)
             res = s2.s2_get_results(ctx, ni)
             info = s2.s2_last_launch_info(ctx)
-            assert info["lanes_per_i"] == L and info["warp_columns"] == Wj
+            assert info["lanes_per_i"] == L and info["warp_columns"] == Wj and (info["i_per_thread"] > 1) == (tiled == 2)
             check_forces(res, ref, s2.S2_FP64, order, flags, f"shape {info}")
         if flags & NGB:
             assert res["overflow"] == bool((ref.ngb_count > 24).any())

@@ -33,8 +33,12 @@ def test_precision_paths_all_shapes_ragged(prec, order, flags):
     shapes = [(L, 1, S, tile) for L in (1, 2, 4, 8, 16, 32) for S, tile in ((1, 0), (3, 64), (13, 32))]
     shapes += [(32, Wj, S, 0) for Wj in (2, 8) for S in (1, 5)] + [(8, 4, 3, 64), (4, 2, 1, 0)]
     worst = {}
-    for L, Wj, S, tile in shapes:
+    shapes = [s + (1,) for s in shapes]
+    if P == s2.S2_FP32:                                   # register-tiled sweep (two i per thread) exists for fp32 and fp64
+        shapes += [(1, 1, 1, 0, 2), (1, 1, 3, 64, 2), (1, 1, 13, 32, 2)]
+    for L, Wj, S, tile, tiled in shapes:
         s2.s2_set_tuning(ctx, 1, L); s2.s2_set_tuning(ctx, 2, Wj); s2.s2_set_tuning(ctx, 0, S); s2.s2_set_tuning(ctx, 4, tile)
+        s2.s2_set_tuning(ctx, 7, tiled)
         s2.s2_calc_ilist(ctx, il, h2, w.eps2, flags)
         res = s2.s2_get_results(ctx, ni)
         info = s2.s2_last_launch_info(ctx)
