@@ -237,7 +237,7 @@ def main():
 
     force_ms = statistics.mean(k["force_ms"] for k in ktimes)
     achieved = ni * N * FLOP_PER_PAIR[order] / (force_ms * 1e-3) / 1e12
-    roofline = {"bound": "alu", "kernel": "force_sweep_kernel<PolicyF64>", "achieved": achieved,
+    roofline = {"bound": "alu", "kernel": "force_sweep_tiled_kernel<PolicyF64<4,0,0>,2>", "achieved": achieved,
                 "peak": FP64_PEAK_TFLOPS, "unit": "TFLOP/s", "frac": achieved / FP64_PEAK_TFLOPS,
                 "traffic": FORCE_KERNEL_DRAM_BYTES,
                 "peak_source": "derived: 148 SM x 64 FP64 FMA lanes x 2 flop x 1.965 GHz (DESIGN.md); not in MEASURED_PEAKS.json",
@@ -345,6 +345,7 @@ def ni_sweep(s2, torch, dev, order):
             rows.append({"cfg": str(key), "precision": pname, "N": w.N, "n_i": ni, "call_us": round(us, 2), "timing": how,
                          "ginteractions_per_s": g, "vs_full_rate": g / full,
                          "S": info["S"], "lanes_per_i": info["lanes_per_i"], "warp_columns": info["warp_columns"],
+                         "i_per_thread": info["i_per_thread"], "grid": info["grid"],
                          "combine": ("none", "reduce kernel", "fused")[info["reduced"]]})
         out.extend(rows[::-1])
         s2.s2_close(ctx)

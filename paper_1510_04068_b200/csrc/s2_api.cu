@@ -432,7 +432,7 @@ static ShapeCost cost_params(int precision, int order)
     c.tiled_gain = 0.93;  // measured: pairs of the register-tiled sweep cost this fraction of the plain ones
     c.c_cta = 4000.0;     // ~2 us: launch ramp, first tile, i-gather, shuffles, record write
     c.c_row = 1000.0;     // ~0.5 us per round of 32 partial rows (L2 latency bound)
-    c.c_launch = 4000.0;  // ~2 us: second launch (programmatic dependent launch hides part of it)
+    c.c_launch = 3000.0;  // ~1.5 us: second launch (programmatic dependent launch hides part of it)
     return c;
 }
 
@@ -533,8 +533,9 @@ static int choose_shape(s2_ctx *ctx, int ni, int nj, unsigned flags, ForceShape 
                 // lanes that share an i read different j: LDS.128 is conflict-free up to 8 distinct addresses
                 // measured (profiles/r01_small_ni.md): a lone CTA per SM is latency-bound (~1.25x), lanes that
                 // share an i read different j (LDS.128 conflict-free up to L = 8, 2- and 4-way above)
-                double t_iter = C_.t_iter * (n_sm >= 2 ? 1.0 : 1.25) * (1.0 + 0.01 * L) * (L > 8 ? 1.0 + 0.01 * L : 1.0);
-                if (L == 0) t_iter = C_.t_iter * ipt * C_.tiled_gain;   // ipt pairs per lane and j, fewer shared-memory reads each
+                double t_iter = C_.t_iter * (n_sm >= 2 ? 1.0 : 1.1) * (1.0 + 0.01 * L) * (L == 32 ? 1.3 : 1.0);   // 4-way LDS conflicts at L = 32
+                // register-tiled: ipt pairs per lane and j, fewer shared-memory reads each
+                if (L == 0) t_iter = C_.t_iter * ipt * C_.tiled_gain * (n_sm >= 2 ? 1.0 : 1.09);
                 // every i-group streams the whole j range from L2 (~2500 B per SM-cycle over the chip)
                 const double stream = (double)Gi * nj * npl * 16.0 / 2500.0;
                 double cost = std::ceil(n_sm / occ) * C_.c_cta + std::max(n_sm * iters * t_iter, stream);
@@ -543,7 +544,7 @@ static int choose_shape(s2_ctx *ctx, int ni, int nj, unsigned flags, ForceShape 
                 if (nst > 1) {
                     const double rounds_f = std::ceil(std::min(icta, ni) / (double)kWarps) * std::ceil((S / C) / 32.0);
                     const double fused_cost = (1.0 + rounds_f) * C_.c_row + (C > 1 ? C_.c_row : 0.0);
-                    const double sep_cost = C_.c_launch + std::ceil(nst / 128.0) * C_.c_row +
+                    const double sep_cost = C_.c_launch + std::ceil(nst / 32.0) * C_.c_row * 0.5 +
                                             (double)ni * nst * (REC * 8.0) / 2000.0;
                     fused = fusable && (fused_cost < sep_cost || ctx->tune[6] > 1);
                     if (!fused && C > 1) continue;              // a cluster shape only makes sense fused

@@ -40,7 +40,8 @@ struct PolicyF64 {
 #endif
     static constexpr int kMinBlocksTiled = S2_F64_MINBLOCKS_TILED;
     static constexpr int kIPT = kIptF64;                        // i-particles per thread in the register-tiled sweep
-    static constexpr int kUnrollTiled = S2_F64_UNROLL_TILED;    // j per unrolled step there (x kIPT pairs in flight)
+    // j per unrolled step there (x kIPT pairs in flight); the 6th-order pair holds 18 more live doubles
+    static constexpr int kUnrollTiled = ORDER == 6 ? 2 : S2_F64_UNROLL_TILED;
 
     struct IState {
         double x, y, z, vx, vy, vz, ax, ay, az, h2, eps2;

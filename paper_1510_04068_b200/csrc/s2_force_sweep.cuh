@@ -201,10 +201,6 @@ __global__ void __launch_bounds__(kThreads, P::kMinBlocks) force_sweep_kernel(co
     pipe.init(smem_raw, a);
     unsigned char *tiles = pipe.tiles;
     const int tile = a.tile, j0 = pipe.j0, j1 = pipe.j1, ntiles = pipe.ntiles;
-    // let a dependent launch (the reduce kernel, launched with programmatic stream serialisation) be staged now;
-    // it waits for this grid's completion itself (griddepcontrol.wait)
-    asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
-
     typename P::IState I;
     P::load_i(a, d.i, I);
 
@@ -250,6 +246,11 @@ __global__ void __launch_bounds__(kThreads, P::kMinBlocks) force_sweep_kernel(co
         tot.add(part);   // two-level accumulation: per-tile partial sums, then the running total
         pipe.release(t);
     }
+
+    // The sweep is over: let a dependent launch (the reduce kernel, launched with programmatic stream
+    // serialisation) be staged while the epilogue runs; it waits for this grid's completion itself
+    // (griddepcontrol.wait).  Not earlier: staged CTAs hold registers that a second sweep CTA per SM needs.
+    asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
 
     // combine the L lanes of each i in a fixed (butterfly) order
     if (L > 1) {
@@ -411,7 +412,6 @@ __global__ void __launch_bounds__(kThreads, P::kMinBlocksTiled) force_sweep_tile
     TilePipe<NPL> pipe;
     pipe.init(smem_raw, a);
     const int tile = a.tile;
-    asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
 
     Decomp d[IPT];
     typename P::IState I[IPT];
@@ -451,6 +451,7 @@ __global__ void __launch_bounds__(kThreads, P::kMinBlocksTiled) force_sweep_tile
         for (int u = 0; u < IPT; ++u) tot[u].add(part[u]);
         pipe.release(t);
     }
+    asm volatile("griddepcontrol.launch_dependents;" ::: "memory");   // see force_sweep_kernel
 
 #pragma unroll
     for (int u = 0; u < IPT; ++u) {
