@@ -37,7 +37,7 @@ SM_COUNT, FP64_LANES_PER_SM, SM_MAX_HZ = 148, 64, 1.965e9
 FP64_PEAK_TFLOPS = SM_COUNT * FP64_LANES_PER_SM * 2 * SM_MAX_HZ / 1e12     # 37.2
 # dram__bytes_read.sum + dram__bytes_write.sum of one force-sweep launch at the headline point,
 # from the ncu --set full capture summarised in profiles/ (None until a capture exists)
-FORCE_KERNEL_DRAM_BYTES = None
+FORCE_KERNEL_DRAM_BYTES = 20.99e6   # 18.02 MB read + 2.96 MB written (profiles/r01_force_fp64_ncu_full.md)
 
 
 def parse_args():
