@@ -49,6 +49,9 @@ def parse_args():
     ap.add_argument("--no-sweep", action="store_true", help="skip the n_i sweep and the peak microbenchmarks")
     ap.add_argument("--workload", default="H", help="config key: H (headline), 3, 4, 5 ...")
     ap.add_argument("--N", type=int, default=0, help="override N (reduced sizes are for debugging only)")
+    ap.add_argument("--blockstep", type=int, default=0, metavar="N",
+                    help="second workload (not the default line): block-time-step Hermite run of an N-particle Plummer "
+                         "sphere for 1/8 time unit in fp64 and double-single; prints one JSON line of statistics")
     return ap.parse_args()
 
 
@@ -154,6 +157,10 @@ def main():
 
     if args.impl == "reference":
         run_reference(args, w, rank, world)
+        return
+    if args.blockstep:
+        if rank == 0:
+            run_blockstep(args.blockstep)
         return
 
     import torch
@@ -278,6 +285,30 @@ def main():
     s2.s2_close(ctx)
     if world > 1:
         dist.destroy_process_group()
+
+
+def run_blockstep(n):
+    """PAPER.md sec 3.7 (L152-L168) in miniature: the host Hermite driver on the library, fp64 versus double-single."""
+    import paper_1510_04068_b200 as s2
+    from paper_1510_04068_b200.hermite import Hermite4, S2Backend
+    from workloads import make_config
+    w = make_config(3, N=n)
+    out = {"workload": f"block-time-step 4th-order Hermite, Plummer N={n}, eps={w.notes['eps']:.3g}, eta=0.01, t=0..1/8", "runs": []}
+    for name, prec in (("fp64", s2.S2_FP64), ("ds", s2.S2_DS)):
+        b = S2Backend(w.N, w.eps2, precision=prec)
+        h = Hermite4(b, w.mass, w.pos, w.vel)
+        e0 = h.energy()
+        b.calls = b.pairs = 0
+        t0 = time.perf_counter()
+        h.run_until(0.125)
+        wall = time.perf_counter() - t0
+        e1 = h.energy()
+        sizes = np.array(h.active_hist)
+        out["runs"].append({"precision": name, "block_steps": h.block_steps, "particle_steps": h.particle_steps,
+                            "n_i_min": int(sizes.min()), "n_i_median": float(np.median(sizes)), "n_i_max": int(sizes.max()),
+                            "wall_s": wall, "ginteractions_per_s_wall": b.pairs / wall / 1e9, "dE_over_E": (e1 - e0) / e0})
+        b.close()
+    print(json.dumps(out), flush=True)
 
 
 def graph_time_us(s2, torch, ctx, fn, calls=20, reps=7):

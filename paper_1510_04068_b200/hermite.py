@@ -1,0 +1,136 @@
+"""Block-time-step 4th-order Hermite integrator on top of the force library (host side).
+
+This is the layer the paper calls the host integrator (sec 3.7): it "picks the active set,
+corrects, computes time steps" on the CPU and leaves "predict, gravity, particle copy" to the GPU.  It is the
+second workload of SURVEY sec 8(f): it drives every entry point of include/s2b200.h the way a production code
+does -- partial j updates (s2_set_j + s2_commit_j of the corrected particles only), s2_predict to the block
+time, s2_calc_ilist for an i-list whose length varies between 1 and N, s2_get_results.
+
+All pairwise arithmetic and the Taylor prediction of the j-particles run in the CUDA kernels.  The host part
+below is the textbook corrector and time-step rule of the 4th-order Hermite scheme the paper names (ref [27],
+L92, L251), written for NumPy arrays of the active particles only:
+
+    corrector   v1 = v0 + (a0 + a1) dt / 2 + (j0 - j1) dt^2 / 12
+                x1 = x0 + (v0 + v1) dt / 2 + (a0 - a1) dt^2 / 12
+    derivatives s0 = (-6 (a0 - a1) - dt (4 j0 + 2 j1)) / dt^2,   c0 = (12 (a0 - a1) + 6 dt (j0 + j1)) / dt^3
+                s1 = s0 + c0 dt,  c1 = c0
+    time step   dt = sqrt(eta (|a1| |s1| + |j1|^2) / (|j1| |c1| + |s1|^2))      (Aarseth criterion, eta = 0.01, L152)
+                quantised to a power of two, block-aligned, at most doubled per step.
+
+The force source is a small backend object, so the same driver can be run against any implementation of
+`set_j / forces` (the tests run it against the CPU oracle to check the GPU run step by step).
+"""
+from __future__ import annotations
+
+import numpy as np
+
+
+class S2Backend:
+    """Forces from libs2b200 (4th order, any precision mode)."""
+
+    def __init__(self, n: int, eps2: float, precision: int = 0, device: int = 0):
+        from . import binding as s2
+        self.s2, self.n, self.eps2 = s2, n, float(eps2)
+        self.ctx = s2.s2_open(device, 4, precision, nj_capacity=n, ngb_cap=0)
+        self.ident = np.arange(n, dtype=np.int32)
+        self.calls = 0
+        self.pairs = 0
+
+    def set_j(self, idx, t, mass, pos, vel, acc, jerk):
+        s2 = self.s2
+        idx = np.ascontiguousarray(idx, dtype=np.int32)
+        s2.s2_set_j(self.ctx, idx, self.ident[idx], t, mass, pos, vel, acc, jerk)
+        s2.s2_commit_j(self.ctx)
+
+    def forces(self, t: float, idx):
+        s2 = self.s2
+        idx = np.ascontiguousarray(idx, dtype=np.int32)
+        s2.s2_predict(self.ctx, float(t), self.n)
+        s2.s2_calc_ilist(self.ctx, idx, None, self.eps2, 0)
+        r = s2.s2_get_results(self.ctx, idx.size)
+        self.calls += 1
+        self.pairs += idx.size * self.n
+        return r["acc"], r["jerk"], r["pot"]
+
+    def close(self):
+        self.s2.s2_close(self.ctx)
+
+
+def _pow2_floor(x):
+    """Largest power of two <= x (element-wise, x > 0)."""
+    return np.exp2(np.floor(np.log2(x)))
+
+
+class Hermite4:
+    """Individual (block) time steps, 4th-order Hermite predictor-corrector."""
+
+    def __init__(self, backend, mass, pos, vel, eta: float = 0.01, eta_start: float = 0.0025,
+                 dt_max: float = 2.0 ** -3, dt_min: float = 2.0 ** -40):
+        self.b = backend
+        self.n = mass.shape[0]
+        self.m = np.ascontiguousarray(mass, dtype=np.float64)
+        self.x = np.array(pos, dtype=np.float64, order="C")
+        self.v = np.array(vel, dtype=np.float64, order="C")
+        self.a = np.zeros_like(self.x)
+        self.j = np.zeros_like(self.x)
+        self.pot = np.zeros(self.n)
+        self.t = np.zeros(self.n)
+        self.dt = np.full(self.n, dt_max)
+        self.eta, self.dt_max, self.dt_min = eta, dt_max, dt_min
+        self.time = 0.0
+        self.block_steps = 0
+        self.particle_steps = 0
+        self.active_hist = []
+        # start-up: forces at t = 0 from positions and velocities alone, then dt = eta_s |a| / |j|
+        everyone = np.arange(self.n, dtype=np.int32)
+        self.b.set_j(everyone, self.t, self.m, self.x, self.v, self.a, self.j)
+        self.a, self.j, self.pot = (np.array(q) for q in self.b.forces(0.0, everyone))
+        an, jn = np.linalg.norm(self.a, axis=1), np.linalg.norm(self.j, axis=1)
+        raw = eta_start * an / np.maximum(jn, 1e-300)
+        self.dt = np.clip(_pow2_floor(np.maximum(raw, dt_min)), dt_min, dt_max)
+        self.b.set_j(everyone, self.t, self.m, self.x, self.v, self.a, self.j)
+
+    # ------------------------------------------------------------------ one block step
+    def step(self):
+        t_new = float((self.t + self.dt).min())
+        act = np.flatnonzero(self.t + self.dt == t_new).astype(np.int32)
+        a1, j1, pot = self.b.forces(t_new, act)
+        dt = self.dt[act][:, None]
+        x0, v0, a0, j0 = self.x[act], self.v[act], self.a[act], self.j[act]
+        v1 = v0 + (a0 + a1) * (dt / 2) + (j0 - j1) * (dt * dt / 12)
+        x1 = x0 + (v0 + v1) * (dt / 2) + (a0 - a1) * (dt * dt / 12)
+        s0 = (-6.0 * (a0 - a1) - dt * (4.0 * j0 + 2.0 * j1)) / (dt * dt)
+        c0 = (12.0 * (a0 - a1) + 6.0 * dt * (j0 + j1)) / (dt * dt * dt)
+        s1 = s0 + c0 * dt
+        nrm = lambda q: np.linalg.norm(q, axis=1)
+        an, jn, sn, cn = nrm(a1), nrm(j1), nrm(s1), nrm(c0)
+        raw = np.sqrt(self.eta * (an * sn + jn * jn) / np.maximum(jn * cn + sn * sn, 1e-300))
+        old = self.dt[act]
+        new = np.minimum(_pow2_floor(np.maximum(raw, self.dt_min)), 2.0 * old)
+        grow = new > old
+        new[grow & (np.fmod(t_new, 2.0 * old) != 0.0)] = old[grow & (np.fmod(t_new, 2.0 * old) != 0.0)]   # block alignment
+        new = np.clip(new, self.dt_min, self.dt_max)
+        self.x[act], self.v[act], self.a[act], self.j[act], self.pot[act] = x1, v1, a1, j1, pot
+        self.t[act] = t_new
+        self.dt[act] = new
+        self.b.set_j(act, self.t[act], self.m[act], x1, v1, a1, j1)   # only the corrected particles are re-sent (L88)
+        self.time = t_new
+        self.block_steps += 1
+        self.particle_steps += act.size
+        self.active_hist.append(act.size)
+        return act.size
+
+    def run_until(self, t_end: float):
+        """Advances until every particle sits at t_end (a multiple of dt_max)."""
+        assert np.fmod(t_end, self.dt_max) == 0.0, "t_end must be a multiple of dt_max"
+        while self.time < t_end:
+            self.step()
+        assert (self.t == t_end).all()
+
+    # ------------------------------------------------------------------ diagnostics
+    def energy(self):
+        """Total energy at a synchronisation time (all particles at the same t): T + 1/2 sum m pot."""
+        assert (self.t == self.t[0]).all(), "energy() needs a synchronisation time"
+        _, _, pot = self.b.forces(float(self.t[0]), np.arange(self.n, dtype=np.int32))
+        kin = 0.5 * float((self.m * (self.v * self.v).sum(axis=1)).sum())
+        return kin + 0.5 * float((self.m * pot).sum())
