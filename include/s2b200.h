@@ -192,6 +192,12 @@ int s2_get_timing(s2_ctx *ctx, float *predict_ms, float *force_ms, float *reduce
  * Returns achieved lane-instructions per second in *fma_per_s.  SYNC. */
 int s2_peak_fma(s2_ctx *ctx, int kind, int iters, double *fma_per_s);
 
+/* Test hook for the double-single arithmetic of the S2_DS path (reading P11): for k < n (host arrays) the operands
+ * a[k], b[k] are split into (hi, lo) float pairs on the device and out[8k .. 8k+7] receives, as fp64,
+ *   [0] the round trip of a   [1] a + b   [2] a - b (cancellation-safe form)   [3] a b   [4] a^2   [5] -3 a
+ *   [6] |a|^(-1/2)   [7] a b + a.   SYNC. */
+int s2_test_ds_ops(s2_ctx *ctx, int n, const double *a, const double *b, double *out);
+
 const char *s2_strerror(int code);
 /* cudaGetErrorString of the last CUDA failure seen by this context ("" if none). */
 const char *s2_last_cuda_error(const s2_ctx *ctx);

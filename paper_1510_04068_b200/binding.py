@@ -75,6 +75,7 @@ def lib() -> C.CDLL:
         "s2_get_j": (C.c_int, [vp, C.c_int, C.c_int, ip, dp, dp, dp]),
         "s2_set_tuning": (C.c_int, [vp, C.c_int, C.c_int]),
         "s2_last_launch_info": (C.c_int, [vp, C.POINTER(C.c_int * 10)]),
+        "s2_test_ds_ops": (C.c_int, [vp, C.c_int, dp, dp, dp]),
         "s2_kernel_launches": (C.c_longlong, [vp]),
         "s2_enable_timing": (C.c_int, [vp, C.c_int]),
         "s2_get_timing": (C.c_int, [vp, C.POINTER(C.c_float), C.POINTER(C.c_float), C.POINTER(C.c_float)]),
@@ -344,6 +345,17 @@ def s2_peak_fma(ctx, kind: int, iters: int = 2000) -> float:
     v = C.c_double()
     _check(lib().s2_peak_fma(ctx.handle, kind, iters, C.byref(v)), "s2_peak_fma", ctx.handle)
     return v.value
+
+
+def s2_test_ds_ops(ctx, a, b) -> np.ndarray:
+    a = np.ascontiguousarray(a, dtype=np.float64)
+    b = np.ascontiguousarray(b, dtype=np.float64)
+    if a.ndim != 1 or a.shape != b.shape:
+        raise ValueError("s2_test_ds_ops: a and b must be 1-D arrays of equal length")
+    out = np.empty((a.shape[0], 8), np.float64)
+    _check(lib().s2_test_ds_ops(ctx.handle, a.shape[0], a.ctypes.data_as(C.c_void_p), b.ctypes.data_as(C.c_void_p),
+                                out.ctypes.data_as(C.c_void_p)), "s2_test_ds_ops", ctx.handle)
+    return out
 
 
 def s2_last_cuda_error(ctx) -> str:

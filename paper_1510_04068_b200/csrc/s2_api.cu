@@ -21,6 +21,7 @@ cudaError_t dispatch_force_fp32(int order, unsigned flags, int L, dim3 grid, siz
 cudaError_t dispatch_force_ds(int order, unsigned flags, int L, dim3 grid, size_t smem, const ForceArgs &a,
                               cudaStream_t st, bool query, int *ctas_per_sm);
 int force_nplanes(int precision, int order, unsigned flags);
+cudaError_t run_ds_ops(int n, const double *d_a, const double *d_b, double *d_out, cudaStream_t st);
 }  // namespace s2
 
 using namespace s2;
@@ -1025,6 +1026,27 @@ extern "C" int s2_peak_fma(s2_ctx *ctx, int kind, int iters, double *fma_per_s)
     CU(cudaSetDevice(ctx->device));
     CU(run_peak_fma(kind, iters, ctx->sm_count, ctx->stream, fma_per_s));
     ctx->launches += 2;
+    return S2_OK;
+}
+
+extern "C" int s2_test_ds_ops(s2_ctx *ctx, int n, const double *a, const double *b, double *out)
+{
+    if (!ctx || n < 0 || (n > 0 && (!a || !b || !out))) return S2_EINVAL;
+    if (n == 0) return S2_OK;
+    CU(cudaSetDevice(ctx->device));
+    Buf tmp;
+    const size_t bytes = (size_t)n * sizeof(double);
+    int rc = dev_reserve(ctx, tmp, 10 * bytes);
+    if (rc != S2_OK) return rc;
+    double *d_a = (double *)tmp.p, *d_b = d_a + n, *d_out = d_b + n;
+    cudaError_t e = cudaMemcpyAsync(d_a, a, bytes, cudaMemcpyHostToDevice, ctx->stream);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(d_b, b, bytes, cudaMemcpyHostToDevice, ctx->stream);
+    if (e == cudaSuccess) e = run_ds_ops(n, d_a, d_b, d_out, ctx->stream);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(out, d_out, 8 * bytes, cudaMemcpyDeviceToHost, ctx->stream);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(ctx->stream);
+    ctx->launches++;
+    dev_release(ctx, tmp);
+    if (e != cudaSuccess) return fail_cuda(ctx, e);
     return S2_OK;
 }
 

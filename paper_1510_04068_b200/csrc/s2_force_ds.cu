@@ -235,4 +235,29 @@ cudaError_t dispatch_force_ds(int order, unsigned flags, int L, dim3 grid, size_
     return launch_L<PolicyDS<6, false, false>>(L, grid, smem, a, st, query, ctas_per_sm);
 }
 
+// Test hook (s2_test_ds_ops): every double-single primitive on n operand pairs, results as fp64.
+__global__ void ds_ops_kernel(int n, const double *a, const double *b, double *out)
+{
+    const int k = blockIdx.x * blockDim.x + threadIdx.x;
+    if (k >= n) return;
+    const ds x = ds_from_double(a[k]), y = ds_from_double(b[k]);
+    auto val = [](ds v) { return (double)v.hi + (double)v.lo; };
+    double *o = out + (size_t)k * 8;
+    o[0] = val(x);                              // fp64 -> DS -> fp64 round trip
+    o[1] = val(ds_add(x, y));
+    o[2] = val(ds_sub_cancel(x, y));
+    o[3] = val(ds_mul(x, y));
+    o[4] = val(ds_sqr(x));
+    o[5] = val(ds_mul_f(x, -3.0f));
+    o[6] = val(ds_rsqrt(ds{fabsf(x.hi), x.hi < 0.f ? -x.lo : x.lo}));   // of |a|
+    o[7] = val(ds_fma(x, y, x));
+}
+
+cudaError_t run_ds_ops(int n, const double *d_a, const double *d_b, double *d_out, cudaStream_t st)
+{
+    if (n <= 0) return cudaSuccess;
+    ds_ops_kernel<<<(n + 255) / 256, 256, 0, st>>>(n, d_a, d_b, d_out);
+    return cudaGetLastError();
+}
+
 }  // namespace s2

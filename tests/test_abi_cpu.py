@@ -1,0 +1,51 @@
+"""CPU-side checks of the boundary: the C-ABI library loads without a GPU, exports every symbol that
+include/s2b200.h declares, fails loudly without a device, and the product never touches the oracle."""
+import ctypes as C
+import os
+import re
+
+import pytest
+
+import paper_1510_04068_b200 as s2
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+def test_library_exports_every_declared_symbol():
+    L = s2.lib()
+    names = s2.header_symbols()
+    assert len(names) >= 25 and "s2_calc_ilist" in names and "s2_get_neighbours_csr" in names
+    missing = [n for n in names if not hasattr(L, n)]
+    assert not missing, missing
+    assert s2.s2_version().startswith("s2b200")
+    assert "order" in s2.s2_strerror(s2.S2_ESTATE) and "fallback" in s2.s2_strerror(s2.S2_ECUDA)
+    assert s2.s2_strerror(-99) == "unknown error code"
+
+
+def test_open_argument_checks_and_no_cpu_fallback():
+    L = s2.lib()
+    h = C.c_void_p()
+    assert L.s2_open(None, 0, 4, 0, 16, 0, None, None) == s2.S2_EINVAL
+    for order, prec, cap in ((5, 0, 16), (4, 7, 16), (4, 0, 0)):
+        assert L.s2_open(C.byref(h), 0, order, prec, cap, 0, None, None) == s2.S2_EINVAL
+    import torch
+    if not torch.cuda.is_available():
+        # no device: the raw ABI reports S2_ECUDA and the binding raises -- nothing falls back to the CPU
+        assert L.s2_open(C.byref(h), 0, 4, 0, 16, 0, None, None) == s2.S2_ECUDA
+        with pytest.raises(s2.S2Error) as e:
+            s2.s2_open(0, 4, s2.S2_FP64, nj_capacity=16)
+        assert e.value.code == s2.S2_ECUDA
+    assert L.s2_close(None) == s2.S2_EINVAL
+    assert L.s2_kernel_launches(None) == 0
+
+
+def test_product_never_imports_the_oracle_and_header_has_no_torch_types():
+    pkg = os.path.join(ROOT, "paper_1510_04068_b200")
+    for dirpath, _, files in os.walk(pkg):
+        for f in files:
+            if f.endswith((".py", ".cu", ".cuh", ".h")):
+                src = open(os.path.join(dirpath, f)).read()
+                assert not re.search(r"^\s*(from|import)\s+oracle\b", src, flags=re.M), f
+                assert "hermite_oracle" not in src and "liboracle" not in src, f
+    hdr = open(os.path.join(ROOT, "include", "s2b200.h")).read()
+    assert "torch" not in re.sub(r"/\*.*?\*/", "", hdr, flags=re.S).lower() and 'extern "C"' in hdr

@@ -170,3 +170,59 @@ def test_cfg5_neighbour_path_sampled(prec):
     inv = np.empty(w.N, np.int64); inv[il] = np.arange(w.N)
     assert (res["nn_r2"][inv[nn]] <= res["nn_r2"]).all()
     s2.s2_close(ctx)
+
+
+def test_headline_point_in_bench_configuration_sampled():
+    """The bench workload (north_star target point): N = n_i = 2^18 equal-mass Plummer, eps = 1e-4, 4th order fp64,
+    in the launch configuration bench.py times (device-resident i-list, automatic shape = register-tiled sweep).
+    Oracle on a seeded sample of 512 i; Newton's third law and the potential symmetry on the full output."""
+    import torch
+    w = make_config("H")
+    ctx = open_and_load(w, 4)
+    s2.s2_predict(ctx, w.t_pred, w.N)
+    il = w.ilist(w.N)
+    d_il = torch.from_numpy(il).cuda()
+    s2.s2_calc_ilist_device(ctx, d_il, None, w.eps2, 0)
+    info = s2.s2_last_launch_info(ctx)
+    assert info["i_per_thread"] == 2 and info["lanes_per_i"] == 1
+    res = s2.s2_get_results(ctx, w.N)
+    pick = np.sort(np.random.default_rng(6).choice(w.N, 512, replace=False))
+    ref, _ = oracle_on_gpu_prediction(ctx, w, 4, il[pick], w.eps2)
+    sub = {k: (v[pick] if isinstance(v, np.ndarray) else v) for k, v in res.items()}
+    errs = check_forces(sub, ref, s2.S2_FP64, 4, 0, f"headline {info}")
+    print("headline sample 512 (seed 6)", info, {k: f"{v:.2e}" for k, v in errs.items()})
+    for q in ("acc", "jerk"):
+        tot = np.abs((w.mass[il, None] * res[q]).sum(0)).max()
+        scale = (w.mass[il] * np.linalg.norm(res[q], axis=1)).sum()
+        assert tot <= 1e-11 * scale, (q, tot, scale)
+    # 1/2 sum m pot is the potential energy of a Plummer sphere in N-body units: -1/2 within sampling noise
+    assert abs(0.5 * (w.mass[il] * res["pot"]).sum() + 0.5) < 0.02
+    s2.s2_close(ctx)
+
+
+def test_double_single_primitives_against_long_double():
+    """Every double-single primitive of the S2_DS path on random operands against numpy long double
+    (SURVEY sec 8(c) pin "DS arithmetic": error <= 2^-44 relative; round trip <= 2^-48)."""
+    rng = np.random.default_rng(44)
+    n = 20000
+    a = rng.normal(size=n) * np.exp(rng.uniform(-8, 8, n))
+    b = rng.normal(size=n) * np.exp(rng.uniform(-8, 8, n))
+    b[: n // 4] = a[: n // 4] * (1 + rng.normal(size=n // 4) * 1e-6)       # nearly equal operands: cancellation in a - b
+    ctx = s2.s2_open(0, 4, s2.S2_DS, nj_capacity=16, ngb_cap=0)
+    out = s2.s2_test_ds_ops(ctx, a, b).astype(np.longdouble)
+    s2.s2_close(ctx)
+    A, B = a.astype(np.longdouble), b.astype(np.longdouble)
+    u44, u48 = np.longdouble(2.0) ** -44, np.longdouble(2.0) ** -48
+    assert (np.abs(out[:, 0] - A) <= u48 * np.abs(A)).all()
+    # the operands the device really works with are the round-tripped ones
+    Ar = out[:, 0]
+    hi = b.astype(np.float32)
+    Br = hi.astype(np.longdouble) + (b - hi.astype(np.float64)).astype(np.float32).astype(np.longdouble)
+    assert (np.abs(out[:, 1] - (Ar + Br)) <= u44 * (np.abs(Ar) + np.abs(Br))).all()
+    assert (np.abs(out[:, 2] - (Ar - Br)) <= u44 * (np.abs(Ar) + np.abs(Br))).all()
+    assert (np.abs(out[:, 3] - Ar * Br) <= u44 * np.abs(Ar * Br)).all()
+    assert (np.abs(out[:, 4] - Ar * Ar) <= u44 * Ar * Ar).all()
+    assert (np.abs(out[:, 5] + 3 * Ar) <= u44 * 3 * np.abs(Ar)).all()
+    rs = 1 / np.sqrt(np.abs(Ar))
+    assert (np.abs(out[:, 6] - rs) <= 4 * u44 * rs).all()
+    assert (np.abs(out[:, 7] - (Ar * Br + Ar)) <= u44 * (np.abs(Ar * Br) + np.abs(Ar))).all()
