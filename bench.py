@@ -31,8 +31,8 @@ import numpy as np
 ROOT = os.path.dirname(os.path.abspath(__file__))
 sys.path.insert(0, ROOT)
 
-FLOP_PER_PAIR = {4: 60, 6: 97}          # stated convention (reading P16)
-FP64_INSTR_PER_PAIR = {4: 32, 6: 54}    # FP64-pipe instructions per pair in the SASS of the sweep (profiles/)
+FLOP_PER_PAIR = {2: 38, 4: 60, 6: 97}   # stated convention (reading P16); 38 = the usual acc+pot count
+FP64_INSTR_PER_PAIR = {2: 18, 4: 32, 6: 54}    # FP64-pipe instructions per pair in the SASS of the sweep (profiles/)
 SM_COUNT, FP64_LANES_PER_SM, SM_MAX_HZ = 148, 64, 1.965e9
 FP64_PEAK_TFLOPS = SM_COUNT * FP64_LANES_PER_SM * 2 * SM_MAX_HZ / 1e12     # 37.2
 # dram__bytes_read.sum + dram__bytes_write.sum of one force-sweep launch at the headline point,
@@ -278,6 +278,7 @@ def main():
             "dadd_two_registers": s2.s2_peak_fma(ctx, 4, 4000) / nominal,
             "unit": "fraction of 148 SM x 64 lanes x 1.965 GHz lane-instructions/s"}
         line["sweep"] = ni_sweep(s2, torch, dev, order)
+        line["large_configs"] = neighbour_path(s2, torch, dev)
         line["hbm_kernels"] = hbm_kernels(s2, torch, dev, measured_peaks().get("hbm_gbs", 6650.0))
         line["cpu_baseline"] = cpu_baseline(w)
     if rank == 0:
@@ -379,6 +380,47 @@ def ni_sweep(s2, torch, dev, order):
                          "i_per_thread": info["i_per_thread"], "grid": info["grid"],
                          "combine": ("none", "reduce kernel", "fused")[info["reduced"]]})
         out.extend(rows[::-1])
+        s2.s2_close(ctx)
+    return out
+
+
+def neighbour_path(s2, torch, dev):
+    """Config 5 (a7 + a8): N = n_i = 2^20 Salpeter Plummer sphere, nearest neighbour + neighbour lists (cap 256,
+    mean 32 per i), fp64 and fp32; config 4's 6th-order fp64 sweep at n_i = N = 2^18; and the 2nd-order (acc + pot)
+    fp64 sweep on the headline particle set.  One warm-up call, then the median of 3 event-timed calls."""
+    from workloads import make_config
+    out = []
+    for key, order, pname, prec, flags in ((5, 4, "fp64", s2.S2_FP64, 3), (5, 4, "fp32", s2.S2_FP32, 3),
+                                           (4, 6, "fp64", s2.S2_FP64, 0), ("H", 2, "fp64", s2.S2_FP64, 0)):
+        w = make_config(key)
+        ctx = s2.s2_open(dev.index, order, prec, nj_capacity=w.N, ngb_cap=256 if flags else 0)
+        a = np.arange(w.N, dtype=np.int32)
+        s2.s2_set_j(ctx, a, w.ident, w.t_j, w.mass, w.pos, w.vel, w.acc, w.jerk,
+                    w.snap if order == 6 else None, w.crackle if order == 6 else None)
+        s2.s2_commit_j(ctx)
+        s2.s2_predict(ctx, w.t_pred, w.N)
+        il = w.ilist(w.N)
+        d_il = torch.from_numpy(il).to(dev)
+        d_h2 = torch.from_numpy(np.ascontiguousarray(w.h2[il])).to(dev) if flags else None
+        s2.s2_enable_timing(ctx, True)
+        ts = []
+        for r in range(4):
+            s2.s2_calc_ilist_device(ctx, d_il, d_h2, w.eps2, flags)
+            t = s2.s2_get_timing(ctx)
+            if r:
+                ts.append(t["force_ms"] + t["reduce_ms"])
+        ms = statistics.median(ts)
+        info = s2.s2_last_launch_info(ctx)
+        row = {"cfg": str(key), "order": order, "precision": pname, "N": w.N, "n_i": w.N,
+               "outputs": "acc+jerk+pot+nn+neighbour lists" if flags else {2: "acc+pot", 4: "acc+jerk+pot", 6: "acc+jerk+snap+pot"}[order],
+               "call_ms": ms,
+               "ginteractions_per_s": w.N * w.N / (ms * 1e-3) / 1e9,
+               "tflops_convention": w.N * w.N * FLOP_PER_PAIR[order] / (ms * 1e-3) / 1e12,
+               "S": info["S"], "i_per_thread": info["i_per_thread"], "grid": info["grid"]}
+        if flags:
+            cnt = s2.s2_get_results(ctx, w.N)["ngb_count"]
+            row.update(mean_neighbours=float(cnt.mean()), max_neighbours=int(cnt.max()), overflows=int((cnt > 256).sum()))
+        out.append(row)
         s2.s2_close(ctx)
     return out
 

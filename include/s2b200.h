@@ -84,7 +84,8 @@ typedef struct {
 /* --- life cycle ----------------------------------------------------------------------- */
 
 /* Creates a context on CUDA device `device`.
- *   order        4 (GRAPE-6 style: acc, jerk) or 6 (also snap; j carries snap and crackle) [L34, L76]
+ *   order        2 (GRAPE-5 style, L34: acc and pot only), 4 (GRAPE-6 style: acc, jerk) or
+ *                6 (also snap; j carries snap and crackle) [L34, L76]
  *   precision    S2_FP64 | S2_DS | S2_FP32
  *   nj_capacity  maximum number of j-particles (addresses 0 .. nj_capacity-1)
  *   ngb_cap      maximum neighbour-list length kept per i (e.g. 256); 0 disables lists
@@ -101,7 +102,8 @@ int s2_synchronize(s2_ctx *ctx);
 /* --- a1: set / commit j-particles ("copy kernel"; L76 fp64 storage) -------- */
 
 /* Stages n j-particles in pinned host memory (host pointers; pos..crackle are (n,3) row-major;
- * snap and crackle may be NULL when order == 4, in which case they are ignored).
+ * snap and crackle may be NULL when order <= 4, in which case they are ignored; acc and jerk may be NULL when
+ * order == 2 and are then stored as zero, so that the predictor reduces to x + v dt).
  * address[k] is the slot in the j-store, id[k] >= 0 the identity used for the self test.
  * May be called several times before one s2_commit_j.  Host-only, no GPU work. */
 int s2_set_j(s2_ctx *ctx, int n, const int *address, const int *id, const double *t,
@@ -120,7 +122,7 @@ int s2_commit_j_device(s2_ctx *ctx, int n, const int *d_address, const int *d_id
 /* --- a2: predict ("one kernel to predict the particles to the new time-step") */
 
 /* Taylor-predicts j-particles 0 .. nj-1 to time t (dt = t - t_j, any sign):
- *   4th order: x_p through jerk, v_p through jerk;  6th order: x_p, v_p, a_p through crackle.
+ *   2nd and 4th order: x_p through jerk, v_p through jerk;  6th order: x_p, v_p, a_p through crackle.
  * Subsequent s2_calc_* calls sum over exactly these nj particles.  ASYNC. */
 int s2_predict(s2_ctx *ctx, double t, int nj);
 
@@ -135,14 +137,16 @@ int s2_calc_ilist(s2_ctx *ctx, int ni, const int *i_address, const double *h2, d
 int s2_calc_ilist_device(s2_ctx *ctx, int ni, const int *d_i_address, const double *d_h2,
                          double eps2, unsigned flags);
 /* i-particles given explicitly (sinks need not be sources, L46).  id[k] < 0 matches no j.
- * acc is read only when order == 6 (relative acceleration for snap).  host pointers. ASYNC. */
+ * acc is read only when order == 6 (relative acceleration for snap); vel may be NULL when order == 2.
+ * host pointers. ASYNC. */
 int s2_calc_explicit(s2_ctx *ctx, int ni, const int *id, const double *pos, const double *vel,
                      const double *acc, const double *h2, double eps2, unsigned flags);
 
 /* --- a9: read results ("transfer of the force computation results") -------- */
 
 /* Results of the last s2_calc_* for i = 0 .. ni-1 (position in the i-list).  Any output
- * pointer may be NULL.  acc/jerk/snap are (ni,3); snap is written only when order == 6.
+ * pointer may be NULL.  acc/jerk/snap are (ni,3); snap is written only when order == 6; jerk is zero when
+ * order == 2.
  * nn_id/nn_r2 are meaningful only if S2_WANT_NN was set, ngb_count only if S2_WANT_NGB.
  * Returns S2_EOVERFLOW (results still written) if any list was truncated.  SYNC. */
 int s2_get_results(s2_ctx *ctx, int ni, double *acc, double *jerk, double *snap, double *pot,

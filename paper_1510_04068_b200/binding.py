@@ -207,7 +207,7 @@ def s2_synchronize(ctx):
     ctx._keep = []
 
 
-def s2_set_j(ctx, address, ident, t, mass, pos, vel, acc, jerk, snap=None, crackle=None):
+def s2_set_j(ctx, address, ident, t, mass, pos, vel, acc=None, jerk=None, snap=None, crackle=None):
     n = int(np.asarray(address).shape[0])
     i32, f64 = np.int32, np.float64
     keep = []

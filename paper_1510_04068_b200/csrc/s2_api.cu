@@ -172,7 +172,7 @@ extern "C" int s2_open(s2_ctx **out, int device, int order, int precision, int n
 {
     if (!out) return S2_EINVAL;
     *out = nullptr;
-    if ((order != 4 && order != 6) || precision < S2_FP64 || precision > S2_FP32 || nj_capacity <= 0 || ngb_cap < 0)
+    if ((order != 2 && order != 4 && order != 6) || precision < S2_FP64 || precision > S2_FP32 || nj_capacity <= 0 || ngb_cap < 0)
         return S2_EINVAL;
     int ndev = 0;
     if (cudaGetDeviceCount(&ndev) != cudaSuccess || device < 0 || device >= ndev) {
@@ -263,7 +263,8 @@ extern "C" int s2_set_j(s2_ctx *ctx, int n, const int *address, const int *id, c
 {
     if (!ctx || n < 0) return S2_EINVAL;
     if (n == 0) return S2_OK;
-    if (!address || !id || !t || !mass || !pos || !vel || !acc || !jerk) return S2_EINVAL;
+    if (!address || !id || !t || !mass || !pos || !vel) return S2_EINVAL;
+    if (ctx->order != 2 && (!acc || !jerk)) return S2_EINVAL;   // 2nd order: missing derivatives are stored as zero
     if (ctx->order == 6 && (!snap || !crackle)) return S2_EINVAL;
     if (n > ctx->nj_cap) return S2_ERANGE;
     for (int k = 0; k < n; ++k)
@@ -291,6 +292,10 @@ extern "C" int s2_set_j(s2_ctx *ctx, int n, const int *address, const int *id, c
     for (int v = 0; v < nvec; ++v) {
         double *d0 = f + (size_t)(2 + 3 * v) * n, *d1 = d0 + n, *d2 = d1 + n;
         const double *s = vecs[v];
+        if (!s) {   // 2nd-order context without acc / jerk
+            memset(d0, 0, (size_t)3 * n * sizeof(double));
+            continue;
+        }
         for (int k = 0; k < n; ++k) {
             d0[k] = s[3 * (size_t)k];
             d1[k] = s[3 * (size_t)k + 1];
@@ -430,6 +435,7 @@ static ShapeCost cost_params(int precision, int order)
     ShapeCost c;
     c.t_iter = precision == S2_FP64 ? 146.0 : (precision == S2_FP32 ? 100.0 : 1400.0);
     if (order == 6) c.t_iter *= 1.7;
+    if (order == 2) c.t_iter *= 0.6;
     c.tiled_gain = 0.93;  // measured: pairs of the register-tiled sweep cost this fraction of the plain ones
     c.c_cta = 4000.0;     // ~2 us: launch ramp, first tile, i-gather, shuffles, record write
     c.c_row = 1000.0;     // ~0.5 us per round of 32 partial rows (L2 latency bound)
@@ -624,21 +630,30 @@ static int run_force(s2_ctx *ctx, int ni, const int *d_i_addr, const double *d_h
 
     ForceArgs a{};
     const int np = nplanes(ctx->order), nq = n_qplanes(ctx->precision, ctx->order);
+    // planes staged per tile, in the order the policy reads them.  A 2nd-order sweep skips the velocity planes:
+    // fp64 P0 P1 P3, fp32 F0 F1, double-single D0 D1 D3 (P3 / D3 carry the id).
+    int nsel = 0;
+    int sel[kMaxPlanes];
     if (ctx->precision == S2_FP64) {
-        for (int k = 0; k < np; ++k) {
-            a.jp[k] = plane(ctx, k);
-            a.ip[k] = explicit_i ? (const void *)((double2 *)ctx->iplanes.p + (size_t)k * ni) : a.jp[k];
+        if (ctx->order == 2) { sel[0] = 0; sel[1] = 1; sel[2] = 3; nsel = 3; }
+        else for (int k = 0; k < np; ++k) sel[nsel++] = k;
+        for (int k = 0; k < nsel; ++k) {
+            a.jp[k] = plane(ctx, sel[k]);
+            a.ip[k] = explicit_i ? (const void *)((double2 *)ctx->iplanes.p + (size_t)sel[k] * ni) : a.jp[k];
         }
     } else {
-        for (int k = 0; k < nq; ++k) {
-            a.jp[k] = qplane(ctx, k);
-            a.ip[k] = explicit_i ? (const void *)((float4 *)ctx->iqplanes.p + (size_t)k * ni) : a.jp[k];
+        if (ctx->order == 2 && ctx->precision == S2_FP32) { sel[0] = 0; sel[1] = 1; nsel = 2; }
+        else if (ctx->order == 2) { sel[0] = 0; sel[1] = 1; sel[2] = 3; nsel = 3; }
+        else for (int k = 0; k < nq; ++k) sel[nsel++] = k;
+        for (int k = 0; k < nsel; ++k) {
+            a.jp[k] = qplane(ctx, sel[k]);
+            a.ip[k] = explicit_i ? (const void *)((float4 *)ctx->iqplanes.p + (size_t)sel[k] * ni) : a.jp[k];
         }
     }
     if (ctx->precision != S2_FP64 && flags) {   // decisions are taken on fp64 positions in every mode
         for (int k = 0; k < 2; ++k) {
-            a.jp[nq + k] = plane(ctx, k);
-            a.ip[nq + k] = explicit_i ? (const void *)((double2 *)ctx->iplanes.p + (size_t)k * ni) : a.jp[nq + k];
+            a.jp[nsel + k] = plane(ctx, k);
+            a.ip[nsel + k] = explicit_i ? (const void *)((double2 *)ctx->iplanes.p + (size_t)k * ni) : a.jp[nsel + k];
         }
     }
     a.i_addr = explicit_i ? nullptr : d_i_addr;
@@ -759,7 +774,7 @@ extern "C" int s2_calc_explicit(s2_ctx *ctx, int ni, const int *id, const double
 {
     int rc = check_calc(ctx, ni, flags, h2);
     if (rc != S2_OK) return rc;
-    if (!id || !pos || !vel || (ctx->order == 6 && !acc)) return S2_EINVAL;
+    if (!id || !pos || (ctx->order != 2 && !vel) || (ctx->order == 6 && !acc)) return S2_EINVAL;
     CU(cudaSetDevice(ctx->device));
     const bool ngb = flags & S2_WANT_NGB;
     const int np = nplanes(ctx->order), nq = n_qplanes(ctx->precision, ctx->order);
@@ -776,7 +791,8 @@ extern "C" int s2_calc_explicit(s2_ctx *ctx, int ni, const int *id, const double
     double2 *P = (double2 *)ctx->h_io;
     float4 *Q = (float4 *)((char *)ctx->h_io + b_p);
     for (int k = 0; k < ni; ++k) {
-        const double *x = pos + 3 * (size_t)k, *v = vel + 3 * (size_t)k;
+        static const double zero3[3] = {0.0, 0.0, 0.0};
+        const double *x = pos + 3 * (size_t)k, *v = vel ? vel + 3 * (size_t)k : zero3;
         int idk = id[k];
         double idbits;
         memset(&idbits, 0, sizeof idbits);

@@ -101,7 +101,8 @@ struct PolicyDS {
     static constexpr int ORDER = ORDER_;
     static constexpr bool NN = NN_, NGB = NGB_;
     static constexpr bool DEC = NN || NGB;
-    static constexpr int NQ = ORDER == 6 ? 6 : 4;
+    static constexpr int NQ = ORDER == 6 ? 6 : (ORDER == 2 ? 3 : 4);   // 2nd order stages D0, D1, D3 (D3 carries the id)
+    static constexpr int kIdPlane = ORDER == 2 ? 2 : 3;
     static constexpr int NPL = NQ + (DEC ? 2 : 0);
     static constexpr int kMinBlocks = 2;
     static constexpr int kUnroll = 1;
@@ -151,10 +152,12 @@ struct PolicyDS {
         const int ia = a.i_addr ? a.i_addr[i] : i;
         const float4 d0 = static_cast<const float4 *>(a.ip[0])[ia];
         const float4 d1 = static_cast<const float4 *>(a.ip[1])[ia];
-        const float4 d2 = static_cast<const float4 *>(a.ip[2])[ia];
-        const float4 d3 = static_cast<const float4 *>(a.ip[3])[ia];
+        const float4 d3 = static_cast<const float4 *>(a.ip[kIdPlane])[ia];
         I.x = {d0.x, d0.y}; I.y = {d0.z, d0.w}; I.z = {d1.x, d1.y};
-        I.vx = {d2.x, d2.y}; I.vy = {d2.z, d2.w}; I.vz = {d3.x, d3.y};
+        if (ORDER != 2) {
+            const float4 d2 = static_cast<const float4 *>(a.ip[2])[ia];
+            I.vx = {d2.x, d2.y}; I.vy = {d2.z, d2.w}; I.vz = {d3.x, d3.y};
+        }
         I.id = __float_as_int(d3.z);
         if (ORDER == 6) {
             const float4 d4 = static_cast<const float4 *>(a.ip[4])[ia];
@@ -176,7 +179,7 @@ struct PolicyDS {
                                                 int segcap)
     {
         const float4 *pl = reinterpret_cast<const float4 *>(stage);
-        const float4 d0 = pl[k], d1 = pl[tile + k], d2 = pl[2 * tile + k], d3 = pl[3 * tile + k];
+        const float4 d0 = pl[k], d1 = pl[tile + k], d2 = pl[2 * tile + k], d3 = ORDER == 2 ? d2 : pl[3 * tile + k];
         const bool skip = (__float_as_int(d3.z) == I.id) || (MASKED && !valid);
 
         if (DEC) {
@@ -189,21 +192,22 @@ struct PolicyDS {
 
         const ds dx = ds_sub_cancel({d0.x, d0.y}, I.x), dy = ds_sub_cancel({d0.z, d0.w}, I.y),
                  dz = ds_sub_cancel({d1.x, d1.y}, I.z);
-        const ds dvx = ds_sub_cancel({d2.x, d2.y}, I.vx), dvy = ds_sub_cancel({d2.z, d2.w}, I.vy),
-                 dvz = ds_sub_cancel({d3.x, d3.y}, I.vz);
         const ds m = {d1.z, d1.w};
         const ds s = ds_add(ds_add(ds_add(ds_sqr(dx), ds_sqr(dy)), ds_sqr(dz)), I.eps2);
-        const ds rv = ds_add(ds_add(ds_mul(dx, dvx), ds_mul(dy, dvy)), ds_mul(dz, dvz));
         ds y = ds_rsqrt(s);
         if (skip) y = ds{0.f, 0.f};
         const ds y2 = ds_sqr(y);
         const ds my = ds_mul(m, y);
         const ds q = ds_mul(my, y2);
         A.pot = ds_add(A.pot, ds_neg(my));
+        A.ax = ds_fma(q, dx, A.ax); A.ay = ds_fma(q, dy, A.ay); A.az = ds_fma(q, dz, A.az);
+        if (ORDER == 2) return;
+        const ds dvx = ds_sub_cancel({d2.x, d2.y}, I.vx), dvy = ds_sub_cancel({d2.z, d2.w}, I.vy),
+                 dvz = ds_sub_cancel({d3.x, d3.y}, I.vz);
+        const ds rv = ds_add(ds_add(ds_mul(dx, dvx), ds_mul(dy, dvy)), ds_mul(dz, dvz));
         const ds alpha = ds_mul(rv, y2);
         const ds a3 = ds_mul_f(alpha, -3.0f);
         const ds tx = ds_fma(a3, dx, dvx), ty = ds_fma(a3, dy, dvy), tz = ds_fma(a3, dz, dvz);
-        A.ax = ds_fma(q, dx, A.ax); A.ay = ds_fma(q, dy, A.ay); A.az = ds_fma(q, dz, A.az);
         A.jx = ds_fma(q, tx, A.jx); A.jy = ds_fma(q, ty, A.jy); A.jz = ds_fma(q, tz, A.jz);
         if (ORDER == 6) {
             const float4 d4 = pl[4 * tile + k], d5 = pl[5 * tile + k];
@@ -225,6 +229,11 @@ cudaError_t dispatch_force_ds(int order, unsigned flags, int L, dim3 grid, size_
                               cudaStream_t st, bool query, int *ctas_per_sm)
 {
     const bool ngb = flags & S2_WANT_NGB, nn = (flags & S2_WANT_NN) || ngb;
+    if (order == 2) {
+        if (ngb) return launch_L<PolicyDS<2, true, true>>(L, grid, smem, a, st, query, ctas_per_sm);
+        if (nn) return launch_L<PolicyDS<2, true, false>>(L, grid, smem, a, st, query, ctas_per_sm);
+        return launch_L<PolicyDS<2, false, false>>(L, grid, smem, a, st, query, ctas_per_sm);
+    }
     if (order == 4) {
         if (ngb) return launch_L<PolicyDS<4, true, true>>(L, grid, smem, a, st, query, ctas_per_sm);
         if (nn) return launch_L<PolicyDS<4, true, false>>(L, grid, smem, a, st, query, ctas_per_sm);

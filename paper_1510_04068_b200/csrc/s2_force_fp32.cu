@@ -26,7 +26,7 @@ struct PolicyF32 {
     static constexpr int ORDER = ORDER_;
     static constexpr bool NN = NN_, NGB = NGB_;
     static constexpr bool DEC = NN || NGB;
-    static constexpr int NQ = ORDER == 6 ? 4 : 3;     // float planes
+    static constexpr int NQ = ORDER == 6 ? 4 : (ORDER == 2 ? 2 : 3);     // float planes (2nd order: F0, F1 only)
     static constexpr int NPL = NQ + (DEC ? 2 : 0);    // + fp64 position planes for the decisions
     static constexpr int kMinBlocks = 2;
     static constexpr int kUnroll = 4;
@@ -88,11 +88,13 @@ struct PolicyF32 {
         const int ia = a.i_addr ? a.i_addr[i] : i;
         const float4 f0 = static_cast<const float4 *>(a.ip[0])[ia];
         const float4 f1 = static_cast<const float4 *>(a.ip[1])[ia];
-        const float4 f2 = static_cast<const float4 *>(a.ip[2])[ia];
         I.xh = f0.x; I.yh = f0.y; I.zh = f0.z;
         I.xl = f1.x; I.yl = f1.y; I.zl = f1.z;
         I.id = __float_as_int(f1.w);
-        I.vx = f2.x; I.vy = f2.y; I.vz = f2.z;
+        if (ORDER != 2) {
+            const float4 f2 = static_cast<const float4 *>(a.ip[2])[ia];
+            I.vx = f2.x; I.vy = f2.y; I.vz = f2.z;
+        }
         if (ORDER == 6) {
             const float4 f3 = static_cast<const float4 *>(a.ip[3])[ia];
             I.ax = f3.x; I.ay = f3.y; I.az = f3.z;
@@ -113,7 +115,8 @@ struct PolicyF32 {
     static __device__ __forceinline__ void load_j(const unsigned char *stage, int tile, int k, JData &J)
     {
         const float4 *pl = reinterpret_cast<const float4 *>(stage);
-        J.f0 = pl[k]; J.f1 = pl[tile + k]; J.f2 = pl[2 * tile + k];
+        J.f0 = pl[k]; J.f1 = pl[tile + k];
+        if (ORDER != 2) J.f2 = pl[2 * tile + k];
         if (ORDER == 6) J.f3 = pl[3 * tile + k];
         if (DEC) {
             const double2 *pd = reinterpret_cast<const double2 *>(stage);
@@ -148,19 +151,20 @@ struct PolicyF32 {
         const float dx = (f0.x - I.xh) + (f1.x - I.xl);
         const float dy = (f0.y - I.yh) + (f1.y - I.yl);
         const float dz = (f0.z - I.zh) + (f1.z - I.zl);
-        const float dvx = f2.x - I.vx, dvy = f2.y - I.vy, dvz = f2.z - I.vz;
         const float s = fmaf(dz, dz, fmaf(dy, dy, fmaf(dx, dx, I.eps2)));
-        const float rv = fmaf(dz, dvz, fmaf(dy, dvy, dx * dvx));
         float y = rsqrt_f32(s);
         y = skip ? 0.f : y;
         const float y2 = y * y;
         const float my = f0.w * y;
         const float q = my * y2;
         A.pot -= my;
+        A.ax = fmaf(q, dx, A.ax); A.ay = fmaf(q, dy, A.ay); A.az = fmaf(q, dz, A.az);
+        if (ORDER == 2) return;
+        const float dvx = f2.x - I.vx, dvy = f2.y - I.vy, dvz = f2.z - I.vz;
+        const float rv = fmaf(dz, dvz, fmaf(dy, dvy, dx * dvx));
         const float alpha = rv * y2;
         const float a3 = -3.f * alpha;
         const float tx = fmaf(a3, dx, dvx), ty = fmaf(a3, dy, dvy), tz = fmaf(a3, dz, dvz);
-        A.ax = fmaf(q, dx, A.ax); A.ay = fmaf(q, dy, A.ay); A.az = fmaf(q, dz, A.az);
         A.jx = fmaf(q, tx, A.jx); A.jy = fmaf(q, ty, A.jy); A.jz = fmaf(q, tz, A.jz);
         if (ORDER == 6) {
             const float4 f3 = J.f3;
@@ -180,6 +184,11 @@ cudaError_t dispatch_force_fp32(int order, unsigned flags, int L, dim3 grid, siz
                                 cudaStream_t st, bool query, int *ctas_per_sm)
 {
     const bool ngb = flags & S2_WANT_NGB, nn = (flags & S2_WANT_NN) || ngb;
+    if (order == 2) {
+        if (ngb) return launch_L<PolicyF32<2, true, true>>(L, grid, smem, a, st, query, ctas_per_sm);
+        if (nn) return launch_L<PolicyF32<2, true, false>>(L, grid, smem, a, st, query, ctas_per_sm);
+        return launch_L<PolicyF32<2, false, false>>(L, grid, smem, a, st, query, ctas_per_sm);
+    }
     if (order == 4) {
         if (ngb) return launch_L<PolicyF32<4, true, true>>(L, grid, smem, a, st, query, ctas_per_sm);
         if (nn) return launch_L<PolicyF32<4, true, false>>(L, grid, smem, a, st, query, ctas_per_sm);

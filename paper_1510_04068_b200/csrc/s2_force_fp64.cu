@@ -23,7 +23,10 @@ template <int ORDER_, bool NN_, bool NGB_>
 struct PolicyF64 {
     static constexpr int ORDER = ORDER_;
     static constexpr bool NN = NN_, NGB = NGB_;
-    static constexpr int NPL = ORDER == 6 ? 6 : 4;
+    // planes staged per tile: P0 P1 P2 P3 [P4 P5]; 2nd order (acc + pot only, GRAPE-5 style L34) needs no velocities:
+    // P0 P1 P3 (P3 carries the id)
+    static constexpr int NPL = ORDER == 6 ? 6 : (ORDER == 2 ? 3 : 4);
+    static constexpr int kIdPlane = ORDER == 2 ? 2 : 3;
 #ifndef S2_F64_MINBLOCKS
 #define S2_F64_MINBLOCKS 2
 #endif
@@ -83,10 +86,12 @@ struct PolicyF64 {
         const int ia = a.i_addr ? a.i_addr[i] : i;
         const double2 p0 = static_cast<const double2 *>(a.ip[0])[ia];
         const double2 p1 = static_cast<const double2 *>(a.ip[1])[ia];
-        const double2 p2 = static_cast<const double2 *>(a.ip[2])[ia];
-        const double2 p3 = static_cast<const double2 *>(a.ip[3])[ia];
+        const double2 p3 = static_cast<const double2 *>(a.ip[kIdPlane])[ia];
         I.x = p0.x; I.y = p0.y; I.z = p1.x;
-        I.vx = p2.x; I.vy = p2.y; I.vz = p3.x;
+        if (ORDER != 2) {
+            const double2 p2 = static_cast<const double2 *>(a.ip[2])[ia];
+            I.vx = p2.x; I.vy = p2.y; I.vz = p3.x;
+        }
         I.id = __double2loint(p3.y);
         if (ORDER == 6) {
             const double2 p4 = static_cast<const double2 *>(a.ip[4])[ia];
@@ -103,7 +108,8 @@ struct PolicyF64 {
     static __device__ __forceinline__ void load_j(const unsigned char *stage, int tile, int k, JData &J)
     {
         const double2 *pl = reinterpret_cast<const double2 *>(stage);
-        J.p0 = pl[k]; J.p1 = pl[tile + k]; J.p2 = pl[2 * tile + k]; J.p3 = pl[3 * tile + k];
+        J.p0 = pl[k]; J.p1 = pl[tile + k];
+        if (ORDER == 2) { J.p3 = pl[2 * tile + k]; } else { J.p2 = pl[2 * tile + k]; J.p3 = pl[3 * tile + k]; }
         if (ORDER == 6) { J.p4 = pl[4 * tile + k]; J.p5 = pl[5 * tile + k]; }
     }
 
@@ -125,7 +131,8 @@ struct PolicyF64 {
         const bool skip = (__double2loint(p3.y) == I.id) || (MASKED && !valid);
 
         const double dx = p0.x - I.x, dy = p0.y - I.y, dz = p1.x - I.z;
-        const double dvx = p2.x - I.vx, dvy = p2.y - I.vy, dvz = p3.x - I.vz;
+        double dvx = 0.0, dvy = 0.0, dvz = 0.0, rv = 0.0;
+        if (ORDER != 2) { dvx = p2.x - I.vx; dvy = p2.y - I.vy; dvz = p3.x - I.vz; }
         double s;
         if (NN || NGB) {
             const double d2 = __fma_rn(dz, dz, __fma_rn(dy, dy, __dmul_rn(dx, dx)));
@@ -134,7 +141,7 @@ struct PolicyF64 {
         } else {
             s = fma(dz, dz, fma(dy, dy, fma(dx, dx, I.eps2)));
         }
-        const double rv = fma(dz, dvz, fma(dy, dvy, dx * dvx));
+        if (ORDER != 2) rv = fma(dz, dvz, fma(dy, dvy, dx * dvx));
 
         // y = s^(-1/2): hardware seed + one third-order step  y <- y (1 + e/2 + 3 e^2 / 8), e = 1 - s y^2
         const double y0 = rsqrt_seed(s);
@@ -148,6 +155,10 @@ struct PolicyF64 {
         const double my = p1.y * y;
         const double q = my * y2;
         A.pot -= my;
+        if (ORDER == 2) {   // GRAPE-5 style: acceleration and potential only
+            A.ax = fma(q, dx, A.ax); A.ay = fma(q, dy, A.ay); A.az = fma(q, dz, A.az);
+            return;
+        }
         const double alpha = rv * y2;
         const double a3 = -3.0 * alpha;
         const double tx = fma(a3, dx, dvx), ty = fma(a3, dy, dvy), tz = fma(a3, dz, dvz);
@@ -171,6 +182,11 @@ cudaError_t dispatch_force_fp64(int order, unsigned flags, int L, dim3 grid, siz
                                 cudaStream_t st, bool query, int *ctas_per_sm)
 {
     const bool ngb = flags & S2_WANT_NGB, nn = (flags & S2_WANT_NN) || ngb;
+    if (order == 2) {
+        if (ngb) return launch_L<PolicyF64<2, true, true>>(L, grid, smem, a, st, query, ctas_per_sm);
+        if (nn) return launch_L<PolicyF64<2, true, false>>(L, grid, smem, a, st, query, ctas_per_sm);
+        return launch_L<PolicyF64<2, false, false>>(L, grid, smem, a, st, query, ctas_per_sm);
+    }
     if (order == 4) {
         if (ngb) return launch_L<PolicyF64<4, true, true>>(L, grid, smem, a, st, query, ctas_per_sm);
         if (nn) return launch_L<PolicyF64<4, true, false>>(L, grid, smem, a, st, query, ctas_per_sm);

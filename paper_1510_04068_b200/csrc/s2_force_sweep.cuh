@@ -482,8 +482,12 @@ cudaError_t launch_L(int L, dim3 grid, size_t smem, const ForceArgs &a, cudaStre
 #define S2_CASE(LL)                                                                                          \
     case LL: {                                                                                               \
         auto kern = force_sweep_kernel<P, LL>;                                                               \
-        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem); \
-        if (e != cudaSuccess) return e;                                                                      \
+        static int s_smem_attr = 0;   /* largest dynamic shared memory size this kernel was opted into */   \
+        if ((int)smem > s_smem_attr) {                                                                       \
+            cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem); \
+            if (e != cudaSuccess) return e;                                                                  \
+            s_smem_attr = (int)smem;                                                                         \
+        }                                                                                                    \
         if (query) return cudaOccupancyMaxActiveBlocksPerMultiprocessor(ctas_per_sm, kern, kThreads, smem);  \
         if (a.cluster > 1) {                                                                                 \
             cudaLaunchConfig_t cfg = {};                                                                     \
@@ -500,8 +504,12 @@ cudaError_t launch_L(int L, dim3 grid, size_t smem, const ForceArgs &a, cudaStre
     if (L == 0) {   // register-tiled full-occupancy sweep, P::kIPT i-particles per thread
         if constexpr (P::kIPT >= 2) {
             auto kern = force_sweep_tiled_kernel<P, P::kIPT>;
-            cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-            if (e != cudaSuccess) return e;
+            static int s_smem_attr = 0;
+            if ((int)smem > s_smem_attr) {
+                cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+                if (e != cudaSuccess) return e;
+                s_smem_attr = (int)smem;
+            }
             if (query) return cudaOccupancyMaxActiveBlocksPerMultiprocessor(ctas_per_sm, kern, kThreads, smem);
             kern<<<grid, kThreads, smem, st>>>(a);
             return cudaGetLastError();

@@ -44,6 +44,8 @@ constexpr int kWarps = kThreads / 32;
 constexpr int kIptF64 = S2_F64_IPT, kIptF32 = S2_F32_IPT, kIptDS = 1;
 inline int force_ipt(int precision) { return precision == S2_FP64 ? kIptF64 : (precision == S2_FP32 ? kIptF32 : kIptDS); }
 
+// a 2nd-order context (acc + pot only) stores and predicts like a 4th-order one (missing derivatives are zero);
+// only the force sweep differs (fewer planes staged, no jerk terms)
 inline int nfields(int order) { return order == 6 ? 20 : 14; }
 inline int nplanes(int order) { return order == 6 ? 6 : 4; }
 

@@ -226,3 +226,48 @@ def test_double_single_primitives_against_long_double():
     rs = 1 / np.sqrt(np.abs(Ar))
     assert (np.abs(out[:, 6] - rs) <= 4 * u44 * rs).all()
     assert (np.abs(out[:, 7] - (Ar * Br + Ar)) <= u44 * (np.abs(Ar * Br) + np.abs(Ar))).all()
+
+
+@pytest.mark.parametrize("prec", ["fp64", "ds", "fp32"])
+def test_second_order_acc_pot_only(prec):
+    """2nd-order (GRAPE-5 style) contexts: acc + pot (+ nn, neighbour lists) without jerk terms.
+    acc and pot of the pair sum do not depend on velocities, so the oracle's 4th-order acc / pot on the GPU's
+    predicted positions is the reference; the predictor with acc = jerk = NULL reduces to x + v dt."""
+    P = {"fp64": s2.S2_FP64, "ds": s2.S2_DS, "fp32": s2.S2_FP32}[prec]
+    w = make_config(5, N=3000)
+    ctx = s2.s2_open(0, 2, P, nj_capacity=w.N, ngb_cap=24)
+    addr = np.arange(w.N, dtype=np.int32)
+    s2.s2_set_j(ctx, addr, w.ident, w.t_j, w.mass, w.pos, w.vel)          # no acc / jerk
+    s2.s2_commit_j(ctx)
+    s2.s2_predict(ctx, w.t_pred, w.N)
+    xp, vp, _ = s2.s2_get_predicted_j(ctx, 0, w.N)
+    dt = (w.t_pred - w.t_j)[:, None]
+    assert np.abs(xp - (w.pos + w.vel * dt)).max() <= 4e-16 * np.abs(w.pos).max() and np.array_equal(vp, w.vel)
+    from gpu_util import TOL, rel_err
+    for ni, flags, tune in ((w.N, 0, {}), (w.N, NN | NGB, {}), (37, NN | NGB, {1: 8, 0: 5}), (37, 0, {1: 32, 2: 8, 0: 3}),
+                            (700, NN, {7: 1, 1: 1, 0: 3}), (1, NN, {})):
+        for k in range(8):
+            s2.s2_set_tuning(ctx, k, tune.get(k, 0))
+        il = w.ilist(ni)
+        h2 = w.h2[il] * 0.6 if flags & NGB else None
+        s2.s2_calc_ilist(ctx, il, h2, w.eps2, flags)
+        res = s2.s2_get_results(ctx, ni)
+        ref = oracle.forces_ilist(4, w.mass, w.ident, xp, vp, None, il, w.eps2, h2, 24)
+        what = f"order 2 {prec} n_i={ni} flags={flags} {s2.s2_last_launch_info(ctx)}"
+        assert rel_err(res["acc"], ref.acc).max() <= TOL[P]["acc"], what
+        assert rel_err(res["pot"], ref.pot).max() <= TOL[P]["pot"], what
+        assert not res["jerk"].any(), what
+        if flags:
+            assert np.array_equal(res["nn_id"], ref.nn_id) and np.array_equal(res["nn_r2"], ref.nn_d2), what
+        if flags & NGB:
+            assert np.array_equal(res["ngb_count"], ref.ngb_count), what
+            check_neighbour_lists(ctx, ref, ni, 24, what)
+    # explicit sinks without velocities
+    rng = np.random.default_rng(2)
+    xi = rng.normal(size=(20, 3)) * 0.4
+    ids = np.full(20, -1, np.int32)
+    s2.s2_calc_explicit(ctx, ids, xi, None, None, None, w.eps2, 0)
+    res = s2.s2_get_results(ctx, 20)
+    ref = oracle.forces(4, w.mass, w.ident, xp, vp, None, ids, xi, np.zeros((20, 3)), None, w.eps2)
+    assert rel_err(res["acc"], ref.acc).max() <= TOL[P]["acc"] and rel_err(res["pot"], ref.pot).max() <= TOL[P]["pot"]
+    s2.s2_close(ctx)
