@@ -298,3 +298,20 @@ def test_cfg4_sixth_order_ni1024():
     errs = check_forces(res, ref, s2.S2_FP64, 6, 0, f"cfg4 n_i=1024 {s2.s2_last_launch_info(ctx)}")
     print("cfg4 n_i=1024", s2.s2_last_launch_info(ctx), {k: f"{v:.2e}" for k, v in errs.items()})
     s2.s2_close(ctx)
+
+
+def test_sharded_forces_single_rank():
+    """The j-sharding wrapper with a world of one rank: explicit sinks against the local
+    shard, identity combine.  The two-rank combine itself is covered on CPU (tests/test_multirank_cpu.py)."""
+    from paper_1510_04068_b200.sharding import ShardedForces
+    w = make_config(1, N=500)
+    sf = ShardedForces(w.N, order=4)
+    assert sf.world == 1 and np.array_equal(sf.mine, np.arange(w.N))
+    sf.set_all_j(w.ident, w.t_j, w.mass, w.pos, w.vel, w.acc, w.jerk)
+    oxp, ovp, _ = oracle.predict(4, w.t_pred, w.t_j, w.pos, w.vel, w.acc, w.jerk)
+    il = w.ilist(60)
+    res = sf.forces(w.t_pred, w.ident[il], oxp[il], ovp[il], None, w.eps2)
+    ref = oracle.forces_ilist(4, w.mass, w.ident, oxp, ovp, None, il, w.eps2)
+    assert rel_err(res["acc"], ref.acc).max() < 1e-13 and rel_err(res["jerk"], ref.jerk).max() < 1e-12
+    assert np.array_equal(res["nn_id"], ref.nn_id)
+    sf.close()
