@@ -35,6 +35,7 @@ FLOP_PER_PAIR = {2: 38, 4: 60, 6: 97}   # stated convention (reading P
 FP64_INSTR_PER_PAIR = {2: 18, 4: 32, 6: 54}    # FP64-pipe instructions per pair in the SASS of the sweep (profiles/)
 SM_COUNT, FP64_LANES_PER_SM, SM_MAX_HZ = 148, 64, 1.965e9
 FP64_PEAK_TFLOPS = SM_COUNT * FP64_LANES_PER_SM * 2 * SM_MAX_HZ / 1e12     # 37.2
+FP32_PEAK_TFLOPS = 2 * FP64_PEAK_TFLOPS                                    # 128 FP32 lanes per SM: 74.5
 # dram__bytes_read.sum + dram__bytes_write.sum of one force-sweep launch at the headline point,
 # from the ncu --set full capture summarised in profiles/ (None until a capture exists)
 FORCE_KERNEL_DRAM_BYTES = 20.99e6   # 18.02 MB read + 2.96 MB written (profiles/r01_force_fp64_ncu_full.md)
@@ -49,6 +50,10 @@ def parse_args():
     ap.add_argument("--no-sweep", action="store_true", help="skip the n_i sweep and the peak microbenchmarks")
     ap.add_argument("--workload", default="H", help="config key: H (headline), 3, 4, 5 ...")
     ap.add_argument("--N", type=int, default=0, help="override N (reduced sizes are for debugging only)")
+    ap.add_argument("--precision", default="fp64", choices=["fp64", "ds", "fp32"],
+                    help="pair-arithmetic precision of the timed step (the default bench line is fp64)")
+    ap.add_argument("--section", default="all", choices=["all", "hbm"],
+                    help="hbm: only the streaming-kernel (predictor / scatter) measurement, for ncu captures")
     ap.add_argument("--blockstep", type=int, default=0, metavar="N",
                     help="second workload (not the default line): block-time-step Hermite run of an N-particle Plummer "
                          "sphere for 1/8 time unit in fp64 and double-single; prints one JSON line of statistics")
@@ -134,11 +139,11 @@ def measured_peaks():
         return {}          # fallback figures of B200_PROFILING.md are then used ("of fallback")
 
 
-def workload_config(w, ni):
+def workload_config(w, ni, precision="fp64"):
     return {"workload": f"{w.name}: Plummer sphere N={w.N}, n_i={ni}, {w.order}th-order Hermite, "
                         f"eps={w.notes['eps']:.4g}, {'Salpeter' if w.notes['salpeter'] else 'equal'} masses, "
                         f"acc+jerk{'+snap' if w.order == 6 else ''}+pot",
-            "N": w.N, "n_i": ni, "order": w.order, "precision": "fp64", "seed": w.seed,
+            "N": w.N, "n_i": ni, "order": w.order, "precision": precision, "seed": w.seed,
             "l2": "L2 flushed (256 MiB write) between timed steps; the predicted j-store (16 MiB) is re-read "
                   "from L2 inside a step by design",
             "parallelism": "j-store replicated, i-lists per rank (no data-path collective)"}
@@ -162,6 +167,13 @@ def main():
         if rank == 0:
             run_blockstep(args.blockstep)
         return
+    if args.section == "hbm":
+        if rank == 0:
+            import torch
+            import paper_1510_04068_b200 as s2
+            print(json.dumps({"hbm_kernels": hbm_kernels(s2, torch, torch.device("cuda", local),
+                                                         measured_peaks().get("hbm_gbs", 6650.0))}), flush=True)
+        return
 
     import torch
     import torch.distributed as dist
@@ -179,7 +191,8 @@ def main():
     from paper_1510_04068_b200.sharding import max_over_ranks, rank_ilist
     il_host = rank_ilist(w.perm, rank, world, ni)
 
-    ctx = s2.s2_open(local, order, s2.S2_FP64, nj_capacity=N, ngb_cap=0)
+    prec = {"fp64": s2.S2_FP64, "ds": s2.S2_DS, "fp32": s2.S2_FP32}[args.precision]
+    ctx = s2.s2_open(local, order, prec, nj_capacity=N, ngb_cap=0)
     s2.s2_enable_timing(ctx, True)
     addr = np.arange(N, dtype=np.int32)
     host = dict(address=addr, ident=w.ident, t=w.t_j, mass=w.mass, pos=w.pos, vel=w.vel, acc=w.acc, jerk=w.jerk,
@@ -244,27 +257,35 @@ def main():
 
     force_ms = statistics.mean(k["force_ms"] for k in ktimes)
     achieved = ni * N * FLOP_PER_PAIR[order] / (force_ms * 1e-3) / 1e12
-    roofline = {"bound": "alu", "kernel": "force_sweep_tiled_kernel<PolicyF64<4,0,0>,2>", "achieved": achieved,
-                "peak": FP64_PEAK_TFLOPS, "unit": "TFLOP/s", "frac": achieved / FP64_PEAK_TFLOPS,
-                "traffic": FORCE_KERNEL_DRAM_BYTES,
-                "peak_source": "derived: 148 SM x 64 FP64 FMA lanes x 2 flop x 1.965 GHz (DESIGN.md); not in MEASURED_PEAKS.json",
+    info = s2.s2_last_launch_info(ctx)
+    fp64_path = args.precision == "fp64"
+    peak = FP64_PEAK_TFLOPS if fp64_path else FP32_PEAK_TFLOPS
+    kname = {"fp64": "PolicyF64", "ds": "PolicyDS", "fp32": "PolicyF32"}[args.precision]
+    kname = (f"force_sweep_tiled_kernel<{kname}<{order},0,0>,{info['i_per_thread']}>" if info["i_per_thread"] > 1
+             else f"force_sweep_kernel<{kname}<{order},0,0>,{info['lanes_per_i']}>")
+    roofline = {"bound": "alu", "kernel": kname, "achieved": achieved,
+                "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak,
+                "traffic": FORCE_KERNEL_DRAM_BYTES if fp64_path else None,
+                "peak_source": ("derived: 148 SM x 64 FP64 FMA lanes x 2 flop x 1.965 GHz" if fp64_path else
+                                "derived: 148 SM x 128 FP32 FMA lanes x 2 flop x 1.965 GHz") + " (DESIGN.md 5.2); not in MEASURED_PEAKS.json",
                 "convention": f"{FLOP_PER_PAIR[order]} flop per pair interaction (labelled convention, reading P16)",
                 "kernel_ms": force_ms, "kernel_share_of_step": force_ms * args.steps / tot_ms,
-                "fp64_instr_per_pair": FP64_INSTR_PER_PAIR[order],
-                "fp64_pipe_frac_nominal": ni * N * FP64_INSTR_PER_PAIR[order] / (force_ms * 1e-3)
-                                          / (SM_COUNT * FP64_LANES_PER_SM * SM_MAX_HZ),
                 "predict_ms": statistics.mean(k["predict_ms"] for k in ktimes),
                 "reduce_ms": statistics.mean(k["reduce_ms"] for k in ktimes)}
+    if fp64_path:
+        roofline["fp64_instr_per_pair"] = FP64_INSTR_PER_PAIR[order]
+        roofline["fp64_pipe_frac_nominal"] = (ni * N * FP64_INSTR_PER_PAIR[order] / (force_ms * 1e-3)
+                                              / (SM_COUNT * FP64_LANES_PER_SM * SM_MAX_HZ))
 
     line = {"metric": "Ginteractions/s", "value": value, "unit": "Ginteractions/s", "n_gpus": world,
             "steps": args.steps, "warmup": max(args.warmup, 3), "ms_per_step": tot_ms / args.steps,
-            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-            "config": workload_config(w, ni), "clocks": clocks,
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": {"fp64": "f64", "ds": "f32x2 (double-single)", "fp32": "f32"}[args.precision],
+            "data": "synthetic", "config": workload_config(w, ni, args.precision), "clocks": clocks,
             "e2e": {"value": e2e_value, "unit": "Ginteractions/s", "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
                     "ms_per_step": e2e_ms / args.steps},
             "gpu_launches": int(launches), "roofline": roofline, "launch": s2.s2_last_launch_info(ctx)}
 
-    if rank == 0 and world == 1 and not args.no_sweep:
+    if rank == 0 and world == 1 and not args.no_sweep and fp64_path:
         # measured FMA peaks in the same process (SURVEY sec 8(d) "clock risk")
         dfma = s2.s2_peak_fma(ctx, 0, 4000)
         roofline["measured_dfma_tflops"] = 2 * dfma / 1e12
