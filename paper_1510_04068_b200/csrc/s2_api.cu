@@ -287,20 +287,15 @@ extern "C" int s2_set_j(s2_ctx *ctx, int n, const int *address, const int *id, c
     double *f = (double *)(blk + ints);
     memcpy(f, t, (size_t)n * sizeof(double));
     memcpy(f + n, mass, (size_t)n * sizeof(double));
+    // vector fields are staged verbatim, (n,3) row-major; the scatter kernel does the transposition into the SoA
     const double *vecs[6] = {pos, vel, acc, jerk, snap, crackle};
     const int nvec = ctx->order == 6 ? 6 : 4;
     for (int v = 0; v < nvec; ++v) {
-        double *d0 = f + (size_t)(2 + 3 * v) * n, *d1 = d0 + n, *d2 = d1 + n;
-        const double *s = vecs[v];
-        if (!s) {   // 2nd-order context without acc / jerk
-            memset(d0, 0, (size_t)3 * n * sizeof(double));
-            continue;
-        }
-        for (int k = 0; k < n; ++k) {
-            d0[k] = s[3 * (size_t)k];
-            d1[k] = s[3 * (size_t)k + 1];
-            d2[k] = s[3 * (size_t)k + 2];
-        }
+        double *dst = f + (size_t)(2 + 3 * v) * n;
+        if (vecs[v])
+            memcpy(dst, vecs[v], (size_t)3 * n * sizeof(double));
+        else   // 2nd-order context without acc / jerk
+            memset(dst, 0, (size_t)3 * n * sizeof(double));
     }
     ctx->batches.push_back({off, n});
     ctx->h_stage_used = off + bytes;
@@ -323,15 +318,15 @@ extern "C" int s2_commit_j(s2_ctx *ctx)
         a.address = (const int *)blk;
         a.id = a.address + b.n;
         const double *f = (const double *)(blk + align16((size_t)2 * b.n * sizeof(int)));
-        for (int k = 0; k < nf; ++k) {
-            a.src[k] = f + (size_t)k * b.n;
-            a.dst[k] = base_field(ctx, k);
-        }
+        a.src[0] = f;
+        a.src[1] = f + b.n;
+        for (int k = 2; k < nf; ++k)   // component c of vector field v: row-major (n,3) block, stride 3
+            a.src[k] = f + (size_t)(2 + 3 * ((k - 2) / 3)) * b.n + (k - 2) % 3;
+        for (int k = 0; k < nf; ++k) a.dst[k] = base_field(ctx, k);
         a.dst_id = base_id(ctx);
         a.n = b.n;
         a.nfields = nf;
         a.nj_cap = ctx->nj_cap;
-        a.src_soa = 1;
         a.erange_flag = (int *)ctx->flags.p + 1;
         CU(launch_scatter(a, ctx->stream));
         ctx->launches++;
@@ -369,7 +364,6 @@ extern "C" int s2_commit_j_device(s2_ctx *ctx, int n, const int *d_address, cons
     a.n = n;
     a.nfields = nf;
     a.nj_cap = ctx->nj_cap;
-    a.src_soa = 0;
     a.erange_flag = (int *)ctx->flags.p + 1;
     CU(launch_scatter(a, ctx->stream));
     ctx->launches++;
@@ -537,10 +531,9 @@ static int choose_shape(s2_ctx *ctx, int ni, int nj, unsigned flags, ForceShape 
                 const long long ctas = (long long)Gi * S;
                 const double n_sm = (double)((ctas + ctx->sm_count - 1) / ctx->sm_count);
                 const double iters = (double)((sl + lanes_j - 1) / lanes_j);
-                // lanes that share an i read different j: LDS.128 is conflict-free up to 8 distinct addresses
-                // measured (profiles/r01_small_ni.md): a lone CTA per SM is latency-bound (~1.25x), lanes that
-                // share an i read different j (LDS.128 conflict-free up to L = 8, 2- and 4-way above)
-                double t_iter = C_.t_iter * (n_sm >= 2 ? 1.0 : 1.1) * (1.0 + 0.01 * L) * (L == 32 ? 1.3 : 1.0);   // 4-way LDS conflicts at L = 32
+                // measured (profiles/r01_small_ni.md): a lone CTA per SM is latency-bound (~1.1x); lanes that share an i
+                // read different j, and LDS.128 is conflict-free only up to 8 distinct addresses (4-way at L = 32)
+                double t_iter = C_.t_iter * (n_sm >= 2 ? 1.0 : 1.1) * (1.0 + 0.01 * L) * (L == 32 ? 1.3 : 1.0);
                 // register-tiled: ipt pairs per lane and j, fewer shared-memory reads each
                 if (L == 0) t_iter = C_.t_iter * ipt * C_.tiled_gain * (n_sm >= 2 ? 1.0 : 1.09);
                 // every i-group streams the whole j range from L2 (~2500 B per SM-cycle over the chip)

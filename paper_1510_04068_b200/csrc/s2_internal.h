@@ -69,7 +69,6 @@ struct ScatterArgs {
     int n;
     int nfields;
     int nj_cap;
-    int src_soa;                   // 1: every src field is a plain length-n array (staging layout)
     int *erange_flag;
 };
 

@@ -6,8 +6,8 @@
 
 namespace s2 {
 
-// One thread per staged particle; consecutive threads read consecutive staged values
-// (coalesced) and write to `address` (contiguous when the host sends address-ordered sets).
+// One thread per staged particle; a warp reads contiguous rows of the staged arrays and writes to `address`
+// (contiguous when the host sends address-ordered sets).
 __global__ void __launch_bounds__(256) scatter_kernel(ScatterArgs a)
 {
     int p = blockIdx.x * blockDim.x + threadIdx.x;
@@ -21,13 +21,9 @@ __global__ void __launch_bounds__(256) scatter_kernel(ScatterArgs a)
 #pragma unroll
     for (int f = 0; f < kMaxFields; ++f) {
         if (f < a.nfields) {
-            // staging layout: plain length-n arrays; user layout: scalars length n, vectors (n,3)
-            const double *src = a.src[f];
-            double v;
-            if (a.src_soa || f < 2)
-                v = src[p];
-            else
-                v = src[(size_t)3 * p];   // src already offset by the component
+            // scalars (t, m): plain length-n arrays; vector components: (n,3) row-major, src already offset by the
+            // component, so the three loads of a thread cover one contiguous 24-byte row
+            const double v = f < 2 ? a.src[f][p] : a.src[f][(size_t)3 * p];
             a.dst[f][addr] = v;
         }
     }
