@@ -395,11 +395,22 @@ def ni_sweep(s2, torch, dev, order):
             g = ni * w.N / (us * 1e-6) / 1e9
             full = full or g
             info = s2.s2_last_launch_info(ctx)
+            host_us = None
+            if key == 2:      # config 2: per-call latency as the host sees it (host i-list in, results out, synchronised)
+                il_h = w.ilist(ni)
+                for _ in range(20):
+                    s2.s2_calc_ilist(ctx, il_h, None, w.eps2, 0); s2.s2_get_results(ctx, ni)
+                t0 = time.perf_counter()
+                for _ in range(300):
+                    s2.s2_calc_ilist(ctx, il_h, None, w.eps2, 0); s2.s2_get_results(ctx, ni)
+                host_us = (time.perf_counter() - t0) / 300 * 1e6
             rows.append({"cfg": str(key), "precision": pname, "N": w.N, "n_i": ni, "call_us": round(us, 2), "timing": how,
                          "ginteractions_per_s": g, "vs_full_rate": g / full,
                          "S": info["S"], "lanes_per_i": info["lanes_per_i"], "warp_columns": info["warp_columns"],
                          "i_per_thread": info["i_per_thread"], "grid": info["grid"],
                          "combine": ("none", "reduce kernel", "fused")[info["reduced"]]})
+            if host_us is not None:
+                rows[-1]["host_roundtrip_us"] = round(host_us, 1)
         out.extend(rows[::-1])
         s2.s2_close(ctx)
     return out
