@@ -182,16 +182,19 @@ struct PolicyDS {
         const float4 d0 = pl[k], d1 = pl[tile + k], d2 = pl[2 * tile + k], d3 = ORDER == 2 ? d2 : pl[3 * tile + k];
         const bool skip = (__float_as_int(d3.z) == I.id) || (MASKED && !valid);
 
-        if (DEC) {
-            const double2 *pd = reinterpret_cast<const double2 *>(stage);
-            const double2 p0 = pd[NQ * tile + k], p1 = pd[(NQ + 1) * tile + k];
-            const double ex = p0.x - I.px, ey = p0.y - I.py, ez = p1.x - I.pz;
-            const double dd = __fma_rn(ez, ez, __fma_rn(ey, ey, __dmul_rn(ex, ex)));
-            decide<L, NN, NGB>(dd, jaddr, skip, I.h2, D, d, seg, segcap);
-        }
-
         const ds dx = ds_sub_cancel({d0.x, d0.y}, I.x), dy = ds_sub_cancel({d0.z, d0.w}, I.y),
                  dz = ds_sub_cancel({d1.x, d1.y}, I.z);
+        if (DEC) {
+            // fp64 decisions (reading P13), behind an fp32 prefilter on the one-lane-per-i path
+            const float d2f = fmaf(dz.hi, dz.hi, fmaf(dy.hi, dy.hi, dx.hi * dx.hi));
+            if (L > 1 || d2f < D.thrf) {
+                const double2 *pd = reinterpret_cast<const double2 *>(stage);
+                const double2 p0 = pd[NQ * tile + k], p1 = pd[(NQ + 1) * tile + k];
+                const double ex = p0.x - I.px, ey = p0.y - I.py, ez = p1.x - I.pz;
+                const double dd = __fma_rn(ez, ez, __fma_rn(ey, ey, __dmul_rn(ex, ex)));
+                decide<L, NN, NGB>(dd, jaddr, skip, I.h2, D, d, seg, segcap);
+            }
+        }
         const ds m = {d1.z, d1.w};
         const ds s = ds_add(ds_add(ds_add(ds_sqr(dx), ds_sqr(dy)), ds_sqr(dz)), I.eps2);
         ds y = ds_rsqrt(s);

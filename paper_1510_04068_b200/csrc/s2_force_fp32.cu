@@ -141,17 +141,24 @@ struct PolicyF32 {
         const float4 f0 = J.f0, f1 = J.f1, f2 = J.f2;
         const bool skip = (__float_as_int(f1.w) == I.id) || (MASKED && !valid);
 
-        if (DEC) {
-            const double2 p0 = J.p0, p1 = J.p1;
-            const double ex = p0.x - I.x, ey = p0.y - I.y, ez = p1.x - I.z;
-            const double d2 = __fma_rn(ez, ez, __fma_rn(ey, ey, __dmul_rn(ex, ex)));
-            decide<L, NN, NGB>(d2, jaddr, skip, I.h2, D, d, seg, segcap);
-        }
-
         const float dx = (f0.x - I.xh) + (f1.x - I.xl);
         const float dy = (f0.y - I.yh) + (f1.y - I.yl);
         const float dz = (f0.z - I.zh) + (f1.z - I.zl);
-        const float s = fmaf(dz, dz, fmaf(dy, dy, fmaf(dx, dx, I.eps2)));
+        float s;
+        if (DEC) {
+            // the decisions are taken on the fp64 d2 (reading P13), but only for pairs whose fp32 estimate comes
+            // within the guard band of the rejection threshold (one-lane-per-i paths; L > 1 lanes vote together)
+            const float d2f = fmaf(dz, dz, fmaf(dy, dy, dx * dx));
+            s = d2f + I.eps2;
+            if (L > 1 || d2f < D.thrf) {
+                const double2 p0 = J.p0, p1 = J.p1;
+                const double ex = p0.x - I.x, ey = p0.y - I.y, ez = p1.x - I.z;
+                const double d2 = __fma_rn(ez, ez, __fma_rn(ey, ey, __dmul_rn(ex, ex)));
+                decide<L, NN, NGB>(d2, jaddr, skip, I.h2, D, d, seg, segcap);
+            }
+        } else {
+            s = fmaf(dz, dz, fmaf(dy, dy, fmaf(dx, dx, I.eps2)));
+        }
         float y = rsqrt_f32(s);
         y = skip ? 0.f : y;
         const float y2 = y * y;

@@ -25,11 +25,30 @@
 
 namespace s2 {
 
-// decision state: nearest neighbour (squared distance, j address) and neighbour count
+// decision state: nearest neighbour (squared distance, j address) and neighbour count, plus the rejection
+// threshold of the one-lane-per-i paths: a pair can only change a decision if d2 < thr = max(h2, nn_d2), which is
+// rare (a few dozen neighbours and ~ln N nearest-neighbour updates per i), so everything else sits behind one compare
 struct Dec {
     double nn_d2;
+    double thr;    // max(h2 if neighbour lists are wanted, nn_d2 if the nearest neighbour is wanted)
+    float thrf;    // thr rounded up with a 2^-10 guard band: prefilter on an fp32 estimate of d2 (fp32 / DS sweeps)
     int nn_j;
     int cnt;
+
+    template <bool NN, bool NGB>
+    __device__ __forceinline__ void set_thr(double h2)
+    {
+        thr = NN ? (NGB ? fmax(h2, nn_d2) : nn_d2) : h2;
+        thrf = __double2float_ru(thr) * 1.0009765625f;
+    }
+    template <bool NN, bool NGB>
+    __device__ __forceinline__ void init(double h2)
+    {
+        nn_d2 = CUDART_INF;
+        nn_j = -1;
+        cnt = 0;
+        set_thr<NN, NGB>(h2);
+    }
 };
 
 // d2: unsoftened squared distance in fp64 (reading R-D2); skip: self or padding lane.
@@ -37,11 +56,15 @@ template <int L, bool NN, bool NGB>
 __device__ __forceinline__ void decide(double d2, int jaddr, bool skip, double h2, Dec &D,
                                        const Decomp &d, int *seg, int segcap)
 {
+    if (L == 1) {
+        if (!(d2 < D.thr)) return;   // exact: no decision below can fire when d2 >= max(h2, nn_d2)
+    }
     const double d2m = skip ? CUDART_INF : d2;
     if (NN) {
         if (d2m < D.nn_d2) {   // strict: the first (lowest-address) minimum of this lane is kept
             D.nn_d2 = d2m;
             D.nn_j = jaddr;
+            if (L == 1) D.template set_thr<NN, NGB>(h2);
         }
     }
     if (NGB) {
@@ -208,9 +231,7 @@ __global__ void __launch_bounds__(kThreads, P::kMinBlocks) force_sweep_kernel(co
     typename P::Part part;   // per-tile partial sums in the pair-arithmetic type
     tot.zero();
     Dec D;
-    D.nn_d2 = CUDART_INF;
-    D.nn_j = -1;
-    D.cnt = 0;
+    D.template init<P::NN, P::NGB>(I.h2);
     int *seg = nullptr;
     if (P::NGB) seg = a.seg + ((size_t)d.i * a.nslices_total + d.slice) * a.segcap;
 
@@ -429,7 +450,7 @@ __global__ void __launch_bounds__(kThreads, P::kMinBlocksTiled) force_sweep_tile
         d[u].slice = blockIdx.y;
         P::load_i(a, d[u].i, I[u]);
         tot[u].zero();
-        D[u].nn_d2 = CUDART_INF; D[u].nn_j = -1; D[u].cnt = 0;
+        D[u].template init<P::NN, P::NGB>(I[u].h2);
         seg[u] = P::NGB ? a.seg + ((size_t)d[u].i * a.nslices_total + d[u].slice) * a.segcap : nullptr;
     }
 
