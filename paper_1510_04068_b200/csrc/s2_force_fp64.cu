@@ -41,10 +41,18 @@ struct PolicyF64 {
 #ifndef S2_F64_MINBLOCKS_TILED
 #define S2_F64_MINBLOCKS_TILED 2
 #endif
-    static constexpr int kMinBlocksTiled = S2_F64_MINBLOCKS_TILED;
+#ifndef S2_F64_MINBLOCKS_TILED6
+#define S2_F64_MINBLOCKS_TILED6 1
+#endif
+#ifndef S2_F64_UNROLL_TILED6
+#define S2_F64_UNROLL_TILED6 4
+#endif
+    static constexpr int kMinBlocksTiled = ORDER == 6 ? S2_F64_MINBLOCKS_TILED6 : S2_F64_MINBLOCKS_TILED;
     static constexpr int kIPT = kIptF64;                        // i-particles per thread in the register-tiled sweep
-    // j per unrolled step there (x kIPT pairs in flight); the 6th-order pair holds 18 more live doubles
-    static constexpr int kUnrollTiled = ORDER == 6 ? 2 : S2_F64_UNROLL_TILED;
+    // j per unrolled step there (x kIPT pairs in flight).  The 6th-order pair holds 18 more live doubles: with
+    // 128 registers the totals spill inside the loop, so that variant runs one CTA per SM with 208 registers
+    // (measured 290 vs 277 Gpairs/s)
+    static constexpr int kUnrollTiled = ORDER == 6 ? S2_F64_UNROLL_TILED6 : S2_F64_UNROLL_TILED;
 
     struct IState {
         double x, y, z, vx, vy, vz, ax, ay, az, h2, eps2;
