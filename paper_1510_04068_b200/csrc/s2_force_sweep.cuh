@@ -3,20 +3,24 @@
 // PAPER.md sec 2.1 (L46-L54): sinks (i) x sources (j); "parallelisation over the sink particles"
 // when there are many sinks, Sapporo1's "parallelize over the source particles ... split into
 // subsets" when there are few, and sec 3.1 (L104) "2D thread-blocks ... multiple threads per
-// i-particle whereby each thread computes a part of the j-particles".  Here one kernel template
-// covers the whole range:
+// i-particle whereby each thread computes a part of the j-particles".  Two kernel templates cover
+// the whole range:
+//   force_sweep_tiled_kernel<P, IPT>  full-occupancy path: one lane per i, IPT i-particles per thread,
+//                                     so every j read from shared memory feeds IPT pair evaluations;
+//   force_sweep_kernel<P, L>          j-split path: L lanes share one i-particle and take interleaved j
+//                                     (L = 1: plain one lane per i); when the i-list cannot fill a CTA the
+//                                     8 warps also become warp columns (Wj) that split every tile.
+// Common to both:
 //   - a CTA owns a group of i-particles (blockIdx.x) and a contiguous j-slice (blockIdx.y);
-//   - inside a warp, L lanes share one i-particle and take interleaved j (L = 1: one lane per i,
-//     every lane reads the same j from shared memory as a broadcast);
-//   - for very few i (L = 32) the 8 warps may additionally be arranged as warp columns (Wj) that
-//     take contiguous sub-ranges of the CTA's (single) tile;
-//   - j tiles are staged global -> shared with 1-D bulk async copies (TMA, cp.async.bulk) that
-//     complete on an mbarrier, double buffered;
-//   - i-particles and accumulators live in registers; the L lanes combine with xor-shuffles in a
-//     fixed order; each (slice, i) writes one 96-byte record.  Slices are combined by the
-//     deterministic reduce kernel (s2_reduce.cu), never by atomics.
-//   - neighbour hits are appended in ascending j order: per thread for L = 1, and for L > 1 by
-//     warp ballot + population-count prefix inside the lane group.
+//   - j tiles are staged global -> shared with 1-D bulk async copies (TMA, cp.async.bulk) that complete on
+//     an mbarrier, in a ring of up to 4 buffers (TilePipe);
+//   - i-particles and accumulators live in registers; per-tile partial sums are added to running totals;
+//     each (slice, i) writes one 96-byte record;
+//   - slices are combined in a fixed order, never by floating-point atomics: by reduce_kernel
+//     (s2_reduce.cu, launched with programmatic dependent launch) or, for small i-groups, by the last CTA
+//     of the i-group inside the sweep launch (fused), optionally after a cluster / DSMEM pre-combine;
+//   - nearest-neighbour and neighbour decisions sit behind one exact compare (Dec::thr); hits are appended in
+//     ascending j order: per thread for L = 1, by warp ballot + population-count prefix for L > 1.
 #pragma once
 
 #include <math_constants.h>

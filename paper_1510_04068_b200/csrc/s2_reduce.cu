@@ -5,8 +5,11 @@
 // partial results"; Sapporo2 merged them with atomics.  This build keeps the second kernel
 // because floating-point atomics make the summation order (and the last digit, L84, L164)
 // run-dependent; here the order is fixed: lane l of the warp that owns i adds slices
-// l, l+32, l+64, ... in sequence, then the 32 lanes are combined by an xor-butterfly.
-// The kernel streams S*ni records of 96 bytes once: L2/HBM-bound, tiny.
+// l, l+32, l+64, ... in sequence, then the 32 lanes are combined by an xor-butterfly
+// (reduce_rows_warp, shared with the fused combine of the sweep, so both give the same bits).
+// The kernel streams S*ni records of 96 bytes once: L2/HBM-bound, tiny.  It is launched with
+// programmatic stream serialisation: the sweep triggers it after its j loop and this grid waits
+// for the sweep's completion itself (griddepcontrol.wait).
 #include <math_constants.h>
 
 #include "s2_force_sweep.cuh"
