@@ -1,4 +1,4 @@
-"""Block-time-step 4th-order Hermite integrator on top of the force library (host side).
+"""Block-time-step 4th- and 6th-order Hermite integrators on top of the force library (host side).
 
 This is the layer the paper calls the host integrator (sec 3.7): it "picks the active set,
 corrects, computes time steps" on the CPU and leaves "predict, gravity, particle copy" to the GPU.  It is the
@@ -26,23 +26,24 @@ import numpy as np
 
 
 class S2Backend:
-    """Forces from libs2b200 (4th order, any precision mode)."""
+    """Forces from libs2b200 (4th or 6th order, any precision mode)."""
 
-    def __init__(self, n: int, eps2: float, precision: int = 0, device: int = 0):
+    def __init__(self, n: int, eps2: float, precision: int = 0, device: int = 0, order: int = 4):
         from . import binding as s2
-        self.s2, self.n, self.eps2 = s2, n, float(eps2)
-        self.ctx = s2.s2_open(device, 4, precision, nj_capacity=n, ngb_cap=0)
+        self.s2, self.n, self.eps2, self.order = s2, n, float(eps2), order
+        self.ctx = s2.s2_open(device, order, precision, nj_capacity=n, ngb_cap=0)
         self.ident = np.arange(n, dtype=np.int32)
         self.calls = 0
         self.pairs = 0
 
-    def set_j(self, idx, t, mass, pos, vel, acc, jerk):
+    def set_j(self, idx, t, mass, pos, vel, acc, jerk, snap=None, crackle=None):
         s2 = self.s2
         idx = np.ascontiguousarray(idx, dtype=np.int32)
-        s2.s2_set_j(self.ctx, idx, self.ident[idx], t, mass, pos, vel, acc, jerk)
+        s2.s2_set_j(self.ctx, idx, self.ident[idx], t, mass, pos, vel, acc, jerk, snap, crackle)
         s2.s2_commit_j(self.ctx)
 
     def forces(self, t: float, idx):
+        """acc, jerk, pot (and snap for order 6) of the listed particles at time t."""
         s2 = self.s2
         idx = np.ascontiguousarray(idx, dtype=np.int32)
         s2.s2_predict(self.ctx, float(t), self.n)
@@ -50,6 +51,8 @@ class S2Backend:
         r = s2.s2_get_results(self.ctx, idx.size)
         self.calls += 1
         self.pairs += idx.size * self.n
+        if self.order == 6:
+            return r["acc"], r["jerk"], r["pot"], r["snap"]
         return r["acc"], r["jerk"], r["pot"]
 
     def close(self):
@@ -131,6 +134,85 @@ class Hermite4:
     def energy(self):
         """Total energy at a synchronisation time (all particles at the same t): T + 1/2 sum m pot."""
         assert (self.t == self.t[0]).all(), "energy() needs a synchronisation time"
-        _, _, pot = self.b.forces(float(self.t[0]), np.arange(self.n, dtype=np.int32))
+        pot = self.b.forces(float(self.t[0]), np.arange(self.n, dtype=np.int32))[2]
         kin = 0.5 * float((self.m * (self.v * self.v).sum(axis=1)).sum())
         return kin + 0.5 * float((self.m * pot).sum())
+
+
+class Hermite6(Hermite4):
+    """6th-order Hermite scheme (the paper's sec 3.7 integrator, ref [5]; L152-L156): forces, jerks and snaps at
+    both ends of a step define a 5th-degree interpolation polynomial of the acceleration.  With h = dt / 2,
+    A+- = a1 +- a0, J+- = h (j1 +- j0), S+- = h^2 (s1 +- s0):
+
+        v1 = v0 + h (A+ - 2/5 J- + 1/15 S+)
+        x1 = x0 + h (v1 + v0) - 2/5 h^2 (a1 - a0) + 1/15 h^3 (j1 + j0)
+        F5 = (S- - 3 J+ + 3 A-) / 16,  F4 = (S+ - J-) / 16,  F3 = (5 J+ - 5 A- - S-) / 8     (F_k = h^k a^(k)_mid / k!)
+        at t1:  a^(3) = 6 (F3 + 4 F4 + 10 F5) / h^3,  a^(4) = 24 (F4 + 5 F5) / h^4,  a^(5) = 120 F5 / h^5
+        dt = eta (A1 / A4)^(1/3),  A_k = sqrt(|a^(k-1)| |a^(k+1)| + |a^(k)|^2)            (generalised Aarseth)
+
+    The library's 6th-order predictor uses the stored snap and the interpolated crackle a^(3)."""
+
+    def __init__(self, backend, mass, pos, vel, eta: float = 0.1, eta_start: float = 0.01,
+                 dt_max: float = 2.0 ** -3, dt_min: float = 2.0 ** -40):
+        self.b = backend
+        self.n = mass.shape[0]
+        self.m = np.ascontiguousarray(mass, dtype=np.float64)
+        self.x = np.array(pos, dtype=np.float64, order="C")
+        self.v = np.array(vel, dtype=np.float64, order="C")
+        z = np.zeros_like(self.x)
+        self.a, self.j, self.s, self.c = z.copy(), z.copy(), z.copy(), z.copy()
+        self.pot = np.zeros(self.n)
+        self.t = np.zeros(self.n)
+        self.eta, self.dt_max, self.dt_min = eta, dt_max, dt_min
+        self.time = 0.0
+        self.block_steps = 0
+        self.particle_steps = 0
+        self.active_hist = []
+        everyone = np.arange(self.n, dtype=np.int32)
+        # start-up: acc and jerk first; the snap needs every particle's acceleration, so a second pass
+        self.b.set_j(everyone, self.t, self.m, self.x, self.v, self.a, self.j, self.s, self.c)
+        self.a, self.j, _, _ = (np.array(q) for q in self.b.forces(0.0, everyone))
+        self.b.set_j(everyone, self.t, self.m, self.x, self.v, self.a, self.j, self.s, self.c)
+        self.a, self.j, self.pot, self.s = (np.array(q) for q in self.b.forces(0.0, everyone))
+        an, jn = np.linalg.norm(self.a, axis=1), np.linalg.norm(self.j, axis=1)
+        raw = eta_start * an / np.maximum(jn, 1e-300)
+        self.dt = np.clip(_pow2_floor(np.maximum(raw, dt_min)), dt_min, dt_max)
+        self.b.set_j(everyone, self.t, self.m, self.x, self.v, self.a, self.j, self.s, self.c)
+
+    def step(self):
+        t_new = float((self.t + self.dt).min())
+        act = np.flatnonzero(self.t + self.dt == t_new).astype(np.int32)
+        a1, j1, pot, s1 = self.b.forces(t_new, act)
+        dt = self.dt[act][:, None]
+        h = 0.5 * dt
+        x0, v0, a0, j0, s0 = self.x[act], self.v[act], self.a[act], self.j[act], self.s[act]
+        Ap, Am = a1 + a0, a1 - a0
+        Jp, Jm = h * (j1 + j0), h * (j1 - j0)
+        Sp, Sm = h * h * (s1 + s0), h * h * (s1 - s0)
+        v1 = v0 + h * (Ap - 0.4 * Jm + Sp / 15.0)
+        x1 = x0 + h * (v1 + v0) - 0.4 * h * h * Am + (h * h * h / 15.0) * (j1 + j0)
+        F5 = (Sm - 3.0 * Jp + 3.0 * Am) / 16.0
+        F4 = (Sp - Jm) / 16.0
+        F3 = (5.0 * Jp - 5.0 * Am - Sm) / 8.0
+        c1 = 6.0 * (F3 + 4.0 * F4 + 10.0 * F5) / h ** 3          # crackle a^(3) at t1
+        p1 = 24.0 * (F4 + 5.0 * F5) / h ** 4                     # a^(4)
+        q1 = 120.0 * F5 / h ** 5                                 # a^(5), constant over the step
+        nrm = lambda q: np.linalg.norm(q, axis=1)
+        A1 = np.sqrt(nrm(a1) * nrm(s1) + nrm(j1) ** 2)
+        A4 = np.sqrt(nrm(c1) * nrm(q1) + nrm(p1) ** 2)
+        raw = self.eta * np.cbrt(A1 / np.maximum(A4, 1e-300))
+        old = self.dt[act]
+        new = np.minimum(_pow2_floor(np.maximum(raw, self.dt_min)), 2.0 * old)
+        blocked = (new > old) & (np.fmod(t_new, 2.0 * old) != 0.0)
+        new[blocked] = old[blocked]
+        new = np.clip(new, self.dt_min, self.dt_max)
+        self.x[act], self.v[act], self.a[act], self.j[act], self.s[act], self.c[act] = x1, v1, a1, j1, s1, c1
+        self.pot[act] = pot
+        self.t[act] = t_new
+        self.dt[act] = new
+        self.b.set_j(act, self.t[act], self.m[act], x1, v1, a1, j1, s1, c1)
+        self.time = t_new
+        self.block_steps += 1
+        self.particle_steps += act.size
+        self.active_hist.append(act.size)
+        return act.size

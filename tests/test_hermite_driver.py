@@ -5,7 +5,7 @@ active sets.  GPU part: the same driver on libs2b200 follows the oracle-driven r
 import numpy as np
 import pytest
 
-from paper_1510_04068_b200.hermite import Hermite4
+from paper_1510_04068_b200.hermite import Hermite4, Hermite6
 from workloads import make_config
 
 from hermite_util import OracleBackend
@@ -55,4 +55,39 @@ def test_driver_gpu_follows_oracle_run(precision, tol):
     print(f"{precision}: block steps {g.block_steps}, mean active {np.mean(g.active_hist):.1f}, "
           f"force calls {gb.calls}, dE/E = {(e1 - e0) / e0:.2e}, max |dx| vs oracle run {np.abs(g.x - o.x).max():.2e}")
     assert abs((e1 - e0) / e0) < 1e-6
+    gb.close()
+
+
+def test_sixth_order_driver_on_oracle_conserves_energy():
+    """6th-order scheme (sec 3.7: eta_6 = 0.1) driven by the oracle: energy and a 4th-order cross-check."""
+    w = _plummer(64)
+    h6 = Hermite6(OracleBackend(w.N, w.eps2, order=6), w.mass, w.pos, w.vel, eta=0.1)
+    e0 = h6.energy()
+    h6.run_until(0.25)
+    e1 = h6.energy()
+    assert abs((e1 - e0) / e0) < 1e-8, (e0, e1)
+    h4 = Hermite4(OracleBackend(w.N, w.eps2), w.mass, w.pos, w.vel, eta=0.002)      # a tight 4th-order run
+    h4.run_until(0.25)
+    assert np.abs(h6.x - h4.x).max() < 2e-6                                         # same trajectory
+    assert min(h6.active_hist) < w.N // 4 and max(h6.active_hist) == w.N
+
+
+@pytest.mark.gpu
+def test_sixth_order_driver_gpu_follows_oracle_run():
+    import paper_1510_04068_b200 as s2
+    from paper_1510_04068_b200.hermite import S2Backend
+    w = _plummer(256)
+    gb = S2Backend(w.N, w.eps2, precision=s2.S2_FP64, order=6)
+    g = Hermite6(gb, w.mass, w.pos, w.vel)
+    o = Hermite6(OracleBackend(w.N, w.eps2, order=6), w.mass, w.pos, w.vel)
+    e0 = g.energy()
+    for _ in range(120):
+        na, nb = g.step(), o.step()
+        assert na == nb and g.time == o.time
+    assert np.array_equal(g.dt, o.dt)
+    assert np.abs(g.x - o.x).max() < 1e-10 and np.abs(g.v - o.v).max() < 1e-9
+    g.run_until(0.125)
+    e1 = g.energy()
+    print(f"6th order: block steps {g.block_steps}, mean active {np.mean(g.active_hist):.1f}, dE/E = {(e1 - e0) / e0:.2e}")
+    assert abs((e1 - e0) / e0) < 1e-8
     gb.close()
