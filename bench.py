@@ -261,7 +261,8 @@ def main():
     fp64_path = args.precision == "fp64"
     peak = FP64_PEAK_TFLOPS if fp64_path else FP32_PEAK_TFLOPS
     kname = {"fp64": "PolicyF64", "ds": "PolicyDS", "fp32": "PolicyF32"}[args.precision]
-    kname = (f"force_sweep_tiled_kernel<{kname}<{order},0,0>,{info['i_per_thread']}>" if info["i_per_thread"] > 1
+    kname = (f"force_sweep_bank_kernel<{kname}<{order},0,0>>" if info["reduced"] == 3
+             else f"force_sweep_tiled_kernel<{kname}<{order},0,0>,{info['i_per_thread']}>" if info["i_per_thread"] > 1
              else f"force_sweep_kernel<{kname}<{order},0,0>,{info['lanes_per_i']}>")
     roofline = {"bound": "alu", "kernel": kname, "achieved": achieved,
                 "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak,
@@ -408,7 +409,7 @@ def ni_sweep(s2, torch, dev, order):
                          "ginteractions_per_s": g, "vs_full_rate": g / full,
                          "S": info["S"], "lanes_per_i": info["lanes_per_i"], "warp_columns": info["warp_columns"],
                          "i_per_thread": info["i_per_thread"], "grid": info["grid"],
-                         "combine": ("none", "reduce kernel", "fused")[info["reduced"]]})
+                         "combine": ("none", "reduce kernel", "fused", "none (chunk launches)")[info["reduced"]]})
             if host_us is not None:
                 rows[-1]["host_roundtrip_us"] = round(host_us, 1)
         out.extend(rows[::-1])

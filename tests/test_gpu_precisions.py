@@ -174,7 +174,7 @@ def test_cfg5_neighbour_path_sampled(prec):
 
 def test_headline_point_in_bench_configuration_sampled():
     """The bench workload (north_star target point): N = n_i = 2^18 equal-mass Plummer, eps = 1e-4, 4th order fp64,
-    in the launch configuration bench.py times (device-resident i-list, automatic shape = register-tiled sweep).
+    in the launch configuration bench.py times (device-resident i-list, automatic shape = uniform-operand sweep).
     Oracle on a seeded sample of 512 i; Newton's third law and the potential symmetry on the full output."""
     import torch
     w = make_config("H")
@@ -184,7 +184,7 @@ def test_headline_point_in_bench_configuration_sampled():
     d_il = torch.from_numpy(il).cuda()
     s2.s2_calc_ilist_device(ctx, d_il, None, w.eps2, 0)
     info = s2.s2_last_launch_info(ctx)
-    assert info["i_per_thread"] == 2 and info["lanes_per_i"] == 1
+    assert info["reduced"] == 3 and info["lanes_per_i"] == 1 and info["S"] == w.N // 1024   # one launch per chunk
     res = s2.s2_get_results(ctx, w.N)
     pick = np.sort(np.random.default_rng(6).choice(w.N, 512, replace=False))
     ref, _ = oracle_on_gpu_prediction(ctx, w, 4, il[pick], w.eps2)
