@@ -38,7 +38,9 @@ FP64_PEAK_TFLOPS = SM_COUNT * FP64_LANES_PER_SM * 2 * SM_MAX_HZ / 1e12     # 37.
 FP32_PEAK_TFLOPS = 2 * FP64_PEAK_TFLOPS                                    # 128 FP32 lanes per SM: 74.5
 # dram__bytes_read.sum + dram__bytes_write.sum of one force-sweep launch at the headline point,
 # from the ncu --set full capture summarised in profiles/ (None until a capture exists)
-FORCE_KERNEL_DRAM_BYTES = 20.99e6   # 18.02 MB read + 2.96 MB written (profiles/r01_force_fp64_ncu_full.md)
+FORCE_KERNEL_DRAM_BYTES = 20.99e6   # tiled sweep: 18.02 MB read + 2.96 MB written (profiles/r01_force_fp64_ncu_full.md)
+BANK_KERNEL_DRAM_BYTES = 29.44e6    # uniform-operand sweep, per chunk launch: 29.44 MB read (parked i-state + running
+                                    # sums, cold L2 under ncu) + 0 written (profiles/r01_force_bank_ncu_full.md)
 
 
 def parse_args():
@@ -266,13 +268,20 @@ def main():
              else f"force_sweep_kernel<{kname}<{order},0,0>,{info['lanes_per_i']}>")
     roofline = {"bound": "alu", "kernel": kname, "achieved": achieved,
                 "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak,
-                "traffic": FORCE_KERNEL_DRAM_BYTES if fp64_path else None,
+                "traffic": (BANK_KERNEL_DRAM_BYTES if info["reduced"] == 3 else FORCE_KERNEL_DRAM_BYTES) if fp64_path else None,
                 "peak_source": ("derived: 148 SM x 64 FP64 FMA lanes x 2 flop x 1.965 GHz" if fp64_path else
                                 "derived: 148 SM x 128 FP32 FMA lanes x 2 flop x 1.965 GHz") + " (DESIGN.md 5.2); not in MEASURED_PEAKS.json",
                 "convention": f"{FLOP_PER_PAIR[order]} flop per pair interaction (labelled convention, reading P16)",
                 "kernel_ms": force_ms, "kernel_share_of_step": force_ms * args.steps / tot_ms,
                 "predict_ms": statistics.mean(k["predict_ms"] for k in ktimes),
                 "reduce_ms": statistics.mean(k["reduce_ms"] for k in ktimes)}
+    if info["reduced"] == 3:
+        # one launch per chunk of the constant bank; achieved = (n_i x chunk x flop) / (mean duration of a chunk
+        # launch INCLUDING the copy that refills the bank before it) -- the same ratio as the whole sweep's
+        roofline["launches_per_sweep"] = info["S"]
+        roofline["pairs_per_launch"] = ni * N // info["S"]
+        roofline["ms_per_launch"] = force_ms / info["S"]
+        roofline["traffic_note"] = "per chunk launch, cold L2 under ncu; the state it re-reads stays in L2 between launches"
     if fp64_path:
         roofline["fp64_instr_per_pair"] = FP64_INSTR_PER_PAIR[order]
         roofline["fp64_pipe_frac_nominal"] = (ni * N * FP64_INSTR_PER_PAIR[order] / (force_ms * 1e-3)
