@@ -418,7 +418,7 @@ def ni_sweep(s2, torch, dev, order):
                          "ginteractions_per_s": g, "vs_full_rate": g / full,
                          "S": info["S"], "lanes_per_i": info["lanes_per_i"], "warp_columns": info["warp_columns"],
                          "i_per_thread": info["i_per_thread"], "grid": info["grid"],
-                         "combine": ("none", "reduce kernel", "fused", "none (chunk launches)")[info["reduced"]]})
+                         "combine": ("none", "reduce kernel", "fused", "none (chunk launches)", "atomics")[info["reduced"]]})
             if host_us is not None:
                 rows[-1]["host_roundtrip_us"] = round(host_us, 1)
         out.extend(rows[::-1])

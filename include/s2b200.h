@@ -170,7 +170,9 @@ int s2_get_j(s2_ctx *ctx, int first, int n, int *id, double *t, double *mass, do
  *   key 0: number of j-slices S      key 1: lanes per i-particle (1,2,4,..,32)
  *   key 2: warp columns over j (1,2,4,8; only with lanes == 32)
  *   key 3: CTAs per SM assumed by the balancer      key 4: j-tile length (multiple of 32)
- *   key 5: 1 = combine j-slices with the separate reduce kernel even when the fused combine applies
+ *   key 5: 1 = combine j-slices with the separate reduce kernel even when the fused combine applies,
+ *          2 = combine them with fp64 atomics on the final records instead (the paper's Sapporo2 scheme, L88): one
+ *          launch, but the last bits then vary run to run; ignored when NN / neighbour lists are requested
  *   key 6: CTAs per thread-block cluster along the slice axis in the fused combine (1 = none, 2, 4, 8)
  *   key 7: 1 = never use the register-tiled sweep (several i per thread), 2 = always use it
  *   key 8: 1 = never use the uniform-operand sweep (j-particles read chunk by chunk from the constant bank, one
@@ -179,7 +181,8 @@ int s2_set_tuning(s2_ctx *ctx, int key, int value);
 /* Shape of the last force launch: out[0]=S, [1]=lanes per i, [2]=warp columns, [3]=grid size,
  * [4]=threads per CTA, [5]=dynamic shared memory bytes, [6]=0 no combine needed / 1 reduce kernel ran /
  * 2 combine fused into the sweep launch (last CTA of each i-group reduces, fixed order) / 3 uniform-operand
- * sweep: out[0] is then the number of chunk launches (sums carried in address order, nothing to combine),
+ * sweep: out[0] is then the number of chunk launches (sums carried in address order, nothing to combine) /
+ * 4 combined by atomics (key 5 = 2),
  * [7]=resident CTAs per SM (occupancy query), [8]=i-particles per thread (register-tiled sweep when > 1),
  * [9]=CTAs per cluster. */
 int s2_last_launch_info(const s2_ctx *ctx, int out[10]);

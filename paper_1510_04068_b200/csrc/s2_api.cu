@@ -696,9 +696,11 @@ static int run_force(s2_ctx *ctx, int ni, const int *d_i_addr, const double *d_h
     const int icta_ = sh.L == 0 ? kThreads * force_ipt(ctx->precision) : (kWarps / sh.Wj) * (32 / sh.L);
     const int Gi_ = (ni + icta_ - 1) / icta_;
     const bool fused = sh.fused != 0;
+    // opt-in (s2_set_tuning key 5 = 2): combine the j-slices with fp64 atomics instead of the reduce kernel
+    const bool atomic = ctx->tune[5] == 2 && flags == 0 && nst > 1 && !fused && !bank;
 
     rc = dev_reserve(ctx, ctx->result, (size_t)ni * REC * sizeof(double));
-    if (rc == S2_OK && !final_direct) rc = dev_reserve(ctx, ctx->part, (size_t)nst * ni * REC * sizeof(double));
+    if (rc == S2_OK && !final_direct && !atomic) rc = dev_reserve(ctx, ctx->part, (size_t)nst * ni * REC * sizeof(double));
     if (rc == S2_OK && fused && (size_t)Gi_ * sizeof(unsigned) > ctx->counters.bytes) {
         rc = dev_reserve(ctx, ctx->counters, (size_t)Gi_ * sizeof(unsigned));
         if (rc == S2_OK) CU(cudaMemsetAsync(ctx->counters.p, 0, ctx->counters.bytes, ctx->stream));
@@ -764,6 +766,8 @@ static int run_force(s2_ctx *ctx, int ni, const int *d_i_addr, const double *d_h
     a.counters = (unsigned *)ctx->counters.p;
     a.out_final = (double *)ctx->result.p;
     a.order = ctx->order;
+    a.atomic = atomic ? 1 : 0;
+    if (atomic) CU(cudaMemsetAsync(ctx->result.p, 0, (size_t)ni * REC * sizeof(double), ctx->stream));
 
     if (want_ngb) CU(cudaMemsetAsync(ctx->flags.p, 0, sizeof(int), ctx->stream));   // overflow flag of this call
     if (bank) {
@@ -786,7 +790,7 @@ static int run_force(s2_ctx *ctx, int ni, const int *d_i_addr, const double *d_h
     ctx->launches++;
     ctx->ran_force = true;
     ctx->ran_reduce = false;
-    if (!final_direct && !fused) {
+    if (!final_direct && !fused && !atomic) {
         ReduceArgs r{};
         r.part = (const double *)ctx->part.p;
         r.out = (double *)ctx->result.p;
@@ -808,7 +812,7 @@ static int run_force(s2_ctx *ctx, int ni, const int *d_i_addr, const double *d_h
     }
     int *li = ctx->last_info;
     li[0] = sh.S; li[1] = sh.L == 0 ? 1 : sh.L; li[2] = sh.Wj; li[3] = (int)(grid.x * grid.y); li[4] = kThreads;
-    li[5] = (int)smem; li[6] = final_direct ? 0 : (fused ? 2 : 1);
+    li[5] = (int)smem; li[6] = final_direct ? 0 : (fused ? 2 : (atomic ? 4 : 1));
     li[8] = sh.L == 0 ? force_ipt(ctx->precision) : 1; li[9] = a.cluster;
     ctx->calc_done = true;
     ctx->ni_last = ni;

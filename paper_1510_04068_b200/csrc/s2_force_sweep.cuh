@@ -90,6 +90,23 @@ __device__ __forceinline__ void decide(double d2, int jaddr, bool skip, double h
     }
 }
 
+// Opt-in combine by atomics (sec 2.2.4: Sapporo2 "uses atomic operations" instead of a second kernel):
+// every (slice, i) record is added to the zeroed final record.  The order of the additions is whatever the
+// hardware makes it, so the last bits differ run to run (L84, L164) -- which is why it is not the default.
+__device__ __forceinline__ void atomic_add_record(double *r, const double out[10], int order, bool first_slice)
+{
+#pragma unroll
+    for (int c = 0; c < 7; ++c) atomicAdd(r + c, out[c]);
+    if (order == 6) {
+#pragma unroll
+        for (int c = 0; c < 3; ++c) atomicAdd(r + 9 + c, out[7 + c]);
+    }
+    if (first_slice) {   // decisions are not computed on this path: "none"
+        r[7] = CUDART_INF;
+        r[8] = __hiloint2double(0, -1);
+    }
+}
+
 // Sum of the partial rows of one i-particle by one warp, in a fixed order (P17): lane l adds rows l, l+32, ...
 // sequentially, then the 32 lanes combine by an xor-butterfly; nn by (d2, address) lexicographic minimum.
 // Rows were written by other CTAs of the same launch: read through L2 (ld.global.cg), after a fence.
@@ -383,7 +400,9 @@ __global__ void __launch_bounds__(kThreads, P::kMinBlocks) force_sweep_kernel(co
         writer = false;
     }
 
-    if (writer) {
+    if (writer && a.atomic) {
+        atomic_add_record(a.out_final + (size_t)d.i * REC, out, a.order, row == 0);
+    } else if (writer) {
         double *r = a.rec + ((size_t)row * a.ni + d.i) * REC;
         if (a.is_final) {
             if (P::NN && nn >= 0) nn = __double2loint(a.jid_plane[nn].y);
@@ -483,6 +502,10 @@ __global__ void __launch_bounds__(kThreads, P::kMinBlocksTiled) force_sweep_tile
         if (!d[u].i_valid) continue;
         double out[10];
         tot[u].to_f64(out);
+        if (a.atomic) {
+            atomic_add_record(a.out_final + (size_t)d[u].i * REC, out, a.order, blockIdx.y == 0);
+            continue;
+        }
         int nn = D[u].nn_j;
         if (a.is_final) {
             if (P::NN && nn >= 0) nn = __double2loint(a.jid_plane[nn].y);

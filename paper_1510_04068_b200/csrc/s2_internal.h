@@ -101,6 +101,8 @@ struct ForceArgs {
     unsigned *counters;            // [number of i-groups], zero between calls (the reducing CTA resets its entry)
     double *out_final;             // [ni][REC]
     int order;
+    int atomic;                    // 1: j-slices add their sums to the zeroed final records with fp64 atomics (opt-in,
+                                   // the paper's Sapporo2 combine L88; not bit-reproducible; no NN / neighbour lists)
     // uniform-operand sweep (force_sweep_bank_kernel): the chunk of j now in the constant bank
     int bank_j0, bank_cnt;         // address of its first particle, number of particles
     int bank_first, bank_last;     // first chunk: start from zero; last chunk: write final records to rec

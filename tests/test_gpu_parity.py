@@ -194,6 +194,39 @@ def test_bit_reproducible_and_paths_agree():
     s2.s2_close(ctx)
 
 
+def test_atomic_combine_option():
+    """the paper's single-kernel combine by atomics (L88) as an opt-in (s2_set_tuning key 5 = 2).
+    Within tolerance of the oracle, equal to the deterministic combine up to summation order, and never used when
+    nearest neighbours are requested (those need the ordered min-by-address combine)."""
+    w = make_config(3, N=8192)
+    ctx = open_and_load(w)
+    s2.s2_predict(ctx, w.t_pred, w.N)
+    for ni, shape in ((96, {0: 9}), (700, {0: 5, 1: 1}), (3000, {0: 3, 7: 2})):
+        il = w.ilist(ni)
+        for k in range(9):
+            s2.s2_set_tuning(ctx, k, 0)
+        for k, v in shape.items():
+            s2.s2_set_tuning(ctx, k, v)
+        s2.s2_set_tuning(ctx, 5, 1)
+        s2.s2_calc_ilist(ctx, il, eps2=w.eps2)
+        det = s2.s2_get_results(ctx, ni)
+        assert s2.s2_last_launch_info(ctx)["reduced"] == 1
+        s2.s2_set_tuning(ctx, 5, 2)
+        s2.s2_calc_ilist(ctx, il, eps2=w.eps2)
+        info = s2.s2_last_launch_info(ctx)
+        assert info["reduced"] == 4, info
+        res = s2.s2_get_results(ctx, ni)
+        ref, _ = oracle_on_gpu_prediction(ctx, w, 4, il, w.eps2)
+        check_forces(res, ref, s2.S2_FP64, 4, 0, f"atomic combine {info}")
+        assert np.allclose(res["acc"], det["acc"], rtol=1e-12, atol=0) and np.allclose(res["pot"], det["pot"], rtol=1e-13)
+        assert (res["nn_id"] == -1).all() and np.isinf(res["nn_r2"]).all()
+        s2.s2_calc_ilist(ctx, il, eps2=w.eps2, flags=NN)     # decisions requested: deterministic combine
+        assert s2.s2_last_launch_info(ctx)["reduced"] == 1
+        ref, _ = oracle_on_gpu_prediction(ctx, w, 4, il, w.eps2)
+        check_forces(s2.s2_get_results(ctx, ni), ref, s2.S2_FP64, 4, NN, "atomic option with NN")
+    s2.s2_close(ctx)
+
+
 # ------------------------------------------------------------------------------- ties
 def test_lattice_ties_and_strictness_gpu():
     w = lattice_workload(4, 0.25)
