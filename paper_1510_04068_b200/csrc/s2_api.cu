@@ -647,7 +647,12 @@ static int run_force_bank(s2_ctx *ctx, ForceArgs &a, int ni, unsigned flags)
     std::lock_guard<std::mutex> lock(g_bank_mu);
     BankOwner &own = g_bank[ctx->device];
     if (!own.ev) CU(cudaEventCreateWithFlags(&own.ev, cudaEventDisableTiming));
-    if (own.used && own.stream != ctx->stream) CU(cudaStreamWaitEvent(ctx->stream, own.ev, 0));
+    // inside a stream capture (CUDA graph) events cannot tie the graph to work outside it: the caller orders
+    // replays of such a graph against other users of the bank himself
+    cudaStreamCaptureStatus cap = cudaStreamCaptureStatusNone;
+    CU(cudaStreamIsCapturing(ctx->stream, &cap));
+    const bool capturing = cap != cudaStreamCaptureStatusNone;
+    if (!capturing && own.used && own.stream != ctx->stream) CU(cudaStreamWaitEvent(ctx->stream, own.ev, 0));
     if (ctx->timing) CU(cudaEventRecord(ctx->ev_t[2], ctx->stream));
     for (int c = 0; c < nchunks; ++c) {
         a.bank_j0 = c * chunk;
@@ -666,9 +671,11 @@ static int run_force_bank(s2_ctx *ctx, ForceArgs &a, int ni, unsigned flags)
         ctx->launches++;
     }
     if (ctx->timing) CU(cudaEventRecord(ctx->ev_t[3], ctx->stream));
-    CU(cudaEventRecord(own.ev, ctx->stream));
-    own.stream = ctx->stream;
-    own.used = true;
+    if (!capturing) {
+        CU(cudaEventRecord(own.ev, ctx->stream));
+        own.stream = ctx->stream;
+        own.used = true;
+    }
 
     int *li = ctx->last_info;
     li[0] = nchunks; li[1] = 1; li[2] = 1; li[3] = (ni + geom[1] - 1) / geom[1]; li[4] = geom[1]; li[5] = 0; li[6] = 3;
