@@ -8,7 +8,7 @@ import oracle
 import paper_1510_04068_b200 as s2
 from workloads import make_config, lattice_workload
 
-from gpu_util import check_forces, check_neighbour_lists, open_and_load, oracle_on_gpu_prediction
+from gpu_util import check_forces, check_neighbour_lists, open_and_load, oracle_on_gpu_prediction, rel_err
 
 pytestmark = pytest.mark.gpu
 
@@ -270,4 +270,25 @@ def test_second_order_acc_pot_only(prec):
     res = s2.s2_get_results(ctx, 20)
     ref = oracle.forces(4, w.mass, w.ident, xp, vp, None, ids, xi, np.zeros((20, 3)), None, w.eps2)
     assert rel_err(res["acc"], ref.acc).max() <= TOL[P]["acc"] and rel_err(res["pot"], ref.pot).max() <= TOL[P]["pot"]
+    s2.s2_close(ctx)
+
+
+def test_largest_store_small_ilist_sampled():
+    """Maximum-size edge case: N = 2^22 j-particles (4x config 5; base store 0.5 GB, 10^4 times the 32-particle
+    i-list), j-split path with many slices, NN + neighbour lists; and one explicit-sink call.  Full oracle (1.3e8 pairs)."""
+    w = make_config(5, N=1 << 22)
+    ctx = open_and_load(w, 4, ngb_cap=64, chunks=3)
+    s2.s2_predict(ctx, w.t_pred, w.N)
+    il = w.ilist(32)
+    h2 = w.h2[il]
+    s2.s2_calc_ilist(ctx, il, h2, w.eps2, NN | NGB)
+    res = s2.s2_get_results(ctx, 32)
+    info = s2.s2_last_launch_info(ctx)
+    ref, (xp, vp, _) = oracle_on_gpu_prediction(ctx, w, 4, il, w.eps2, h2, ngb_cap=64)
+    check_forces(res, ref, s2.S2_FP64, 4, NN | NGB, f"N=2^22 n_i=32 {info}")
+    check_neighbour_lists(ctx, ref, 32, 64, "N=2^22 n_i=32")
+    assert info["S"] * info["warp_columns"] > 1            # the j range really was split
+    s2.s2_calc_ilist(ctx, il[:1], None, w.eps2, 0)          # one active particle against 4M sources
+    r1 = s2.s2_get_results(ctx, 1)
+    assert rel_err(r1["acc"], ref.acc[:1]).max() <= 1e-13 and rel_err(r1["jerk"], ref.jerk[:1]).max() <= 1e-12
     s2.s2_close(ctx)
