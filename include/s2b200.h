@@ -176,7 +176,9 @@ int s2_get_j(s2_ctx *ctx, int first, int n, int *id, double *t, double *mass, do
  *   key 6: CTAs per thread-block cluster along the slice axis in the fused combine (1 = none, 2, 4, 8)
  *   key 7: 1 = never use the register-tiled sweep (several i per thread), 2 = always use it
  *   key 8: 1 = never use the uniform-operand sweep (j-particles read chunk by chunk from the constant bank, one
- *          launch per chunk; fp64 only), 2 = always use it when the context computes in fp64 */
+ *          launch per chunk; fp64 only), 2 = always use it when the context computes in fp64
+ *   key 9: 1 = never use the zero-copy path of small host calls (n_i <= 128 with host arrays: the kernels read the
+ *          i-list from, and write the final records to, pinned host memory, so no copy is enqueued) */
 int s2_set_tuning(s2_ctx *ctx, int key, int value);
 /* Shape of the last force launch: out[0]=S, [1]=lanes per i, [2]=warp columns, [3]=grid size,
  * [4]=threads per CTA, [5]=dynamic shared memory bytes, [6]=0 no combine needed / 1 reduce kernel ran /

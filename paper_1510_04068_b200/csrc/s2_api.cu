@@ -57,6 +57,16 @@ struct s2_ctx {
     void *h_io = nullptr;
     size_t h_io_bytes = 0;
     int *h_flags = nullptr;           // pinned, 4 ints
+    // zero-copy small calls (n_i <= kZeroCopyNi): the kernels read the i-list from, and write the final records to,
+    // pinned host memory directly (device-accessible under unified addressing) -- no copy operations on the stream
+    void *h_res = nullptr;            // final records of the last small call
+    size_t h_res_bytes = 0;
+    bool res_on_host = false;
+    void *h_il[2] = {nullptr, nullptr};   // i-list (+ h2) of small calls, alternating so that a call can be
+    size_t h_il_bytes[2] = {0, 0};        // prepared while the previous one still runs
+    cudaEvent_t ev_il[2] = {nullptr, nullptr};
+    int il_turn = 0;
+    bool flags_dirty = false;         // a device-side commit may have raised the range flag
     cudaEvent_t ev_stage = nullptr;   // H2D of the staging buffer finished
     cudaEvent_t ev_io = nullptr;      // H2D of the i-list upload finished
     std::vector<Batch> batches;
@@ -68,7 +78,7 @@ struct s2_ctx {
     double t_pred = 0.0;
 
     // tuning overrides and last launch
-    int tune[9] = {0, 0, 0, 0, 0, 0, 0, 0, 0};
+    int tune[10] = {0, 0, 0, 0, 0, 0, 0, 0, 0, 0};
     int last_info[10] = {0, 0, 0, 0, 0, 0, 0, 0, 1, 1};
     std::map<long long, int> occ_cache;
     std::map<long long, std::pair<ForceShape, int>> shape_cache;
@@ -232,6 +242,8 @@ extern "C" int s2_open(s2_ctx **out, int device, int order, int precision, int n
         if (e == cudaSuccess) e = cudaHostAlloc((void **)&ctx->h_flags, 64, cudaHostAllocDefault);
         if (e == cudaSuccess) e = cudaEventCreateWithFlags(&ctx->ev_stage, cudaEventDisableTiming);
         if (e == cudaSuccess) e = cudaEventCreateWithFlags(&ctx->ev_io, cudaEventDisableTiming);
+        if (e == cudaSuccess) e = cudaEventCreateWithFlags(&ctx->ev_il[0], cudaEventDisableTiming);
+        if (e == cudaSuccess) e = cudaEventCreateWithFlags(&ctx->ev_il[1], cudaEventDisableTiming);
         for (int k = 0; k < 6 && e == cudaSuccess; ++k) e = cudaEventCreate(&ctx->ev_t[k]);
         if (e == cudaSuccess) e = cudaStreamSynchronize(ctx->stream);
         if (e != cudaSuccess) rc = fail_cuda(ctx, e);
@@ -257,6 +269,11 @@ extern "C" int s2_close(s2_ctx *ctx)
     if (ctx->h_flags) cudaFreeHost(ctx->h_flags);
     if (ctx->ev_stage) cudaEventDestroy(ctx->ev_stage);
     if (ctx->ev_io) cudaEventDestroy(ctx->ev_io);
+    for (int k = 0; k < 2; ++k) {
+        if (ctx->ev_il[k]) cudaEventDestroy(ctx->ev_il[k]);
+        if (ctx->h_il[k]) cudaFreeHost(ctx->h_il[k]);
+    }
+    if (ctx->h_res) cudaFreeHost(ctx->h_res);
     for (auto &e : ctx->ev_t)
         if (e) cudaEventDestroy(e);
     cudaGetLastError();
@@ -393,6 +410,7 @@ extern "C" int s2_commit_j_device(s2_ctx *ctx, int n, const int *d_address, cons
     CU(launch_scatter(a, ctx->stream));
     ctx->launches++;
     ctx->have_j = true;
+    ctx->flags_dirty = true;   // the scatter kernel raises flag 1 on an out-of-range address
     ctx->predicted = false;
     return S2_OK;
 }
@@ -705,8 +723,14 @@ static int run_force_bank(s2_ctx *ctx, ForceArgs &a, int ni, unsigned flags)
     return S2_OK;
 }
 
+// Calls with at most this many i-particles keep their i-list and their final records in pinned host memory that the
+// kernels access directly (transfers dominate small calls).  Measured host round trip
+// (calc + get_results): N = 64: 38-41 -> 26 us; N = 65536, n_i = 1: 37 -> 27.5, n_i = 32: 40 -> 34, n_i = 256: 72 -> 73
+// (the record writes over the host link start to cost more than the copy they save), hence the limit
+constexpr int kZeroCopyNi = 128;
+
 static int run_force(s2_ctx *ctx, int ni, const int *d_i_addr, const double *d_h2, bool explicit_i, double eps2,
-                     unsigned flags)
+                     unsigned flags, bool host_call)
 {
     const bool bank = bank_applies(ctx, ni, ctx->nj_pred);
     ForceShape sh{};
@@ -727,8 +751,13 @@ static int run_force(s2_ctx *ctx, int ni, const int *d_i_addr, const double *d_h
     const bool fused = sh.fused != 0;
     // opt-in (s2_set_tuning key 5 = 2): combine the j-slices with fp64 atomics instead of the reduce kernel
     const bool atomic = ctx->tune[5] == 2 && flags == 0 && nst > 1 && !fused && !bank;
+    // small calls: the final records are written straight into pinned host memory
+    // (calls made with host arrays only: a caller that keeps its i-list on the device is not latency-bound by copies)
+    const bool host_res = host_call && ni <= kZeroCopyNi && !bank && !atomic && ctx->tune[9] != 1 && ctx->tune[9] != 3;
 
-    rc = dev_reserve(ctx, ctx->result, (size_t)ni * REC * sizeof(double));
+    rc = host_res ? pinned_reserve(ctx, &ctx->h_res, &ctx->h_res_bytes, 0, (size_t)kZeroCopyNi * REC * sizeof(double))
+                  : dev_reserve(ctx, ctx->result, (size_t)ni * REC * sizeof(double));
+    double *const resp = host_res ? (double *)ctx->h_res : (double *)ctx->result.p;
     if (rc == S2_OK && !final_direct && !atomic) rc = dev_reserve(ctx, ctx->part, (size_t)nst * ni * REC * sizeof(double));
     if (rc == S2_OK && fused && (size_t)Gi_ * sizeof(unsigned) > ctx->counters.bytes) {
         rc = dev_reserve(ctx, ctx->counters, (size_t)Gi_ * sizeof(unsigned));
@@ -774,6 +803,20 @@ static int run_force(s2_ctx *ctx, int ni, const int *d_i_addr, const double *d_h
     }
     a.i_addr = explicit_i ? nullptr : d_i_addr;
     a.h2 = d_h2;
+    if (host_call && !explicit_i && ni <= kZeroCopyNi && ctx->tune[9] != 1) {
+        // d_i_addr / d_h2 point into pinned host memory (s2_calc_ilist).  A few CTAs read them in place; a wide grid
+        // (every CTA of every j-slice gathers its i-particles) would queue a thousand reads on the host link
+        // (measured +11 us at 148 CTAs), so there they are copied once to the device first
+        const long long ctas = (long long)Gi_ * sh.S;
+        if (ctas > 8 || ctx->tune[9] == 2) {
+            const size_t b_addr = align16((size_t)ni * sizeof(int)), b_h2 = d_h2 ? (size_t)ni * sizeof(double) : 0;
+            rc = dev_reserve(ctx, ctx->i_addr, b_addr + b_h2);
+            if (rc != S2_OK) return rc;
+            CU(cudaMemcpyAsync(ctx->i_addr.p, d_i_addr, b_addr + b_h2, cudaMemcpyHostToDevice, ctx->stream));
+            a.i_addr = (const int *)ctx->i_addr.p;
+            a.h2 = d_h2 ? (const double *)((char *)ctx->i_addr.p + b_addr) : nullptr;
+        }
+    }
     a.jid_plane = plane(ctx, 3);
     a.ni = ni;
     a.nj = ctx->nj_pred;
@@ -785,7 +828,7 @@ static int run_force(s2_ctx *ctx, int ni, const int *d_i_addr, const double *d_h
     a.stages = sh.stages;
     a.nslices_total = nst;
     a.is_final = final_direct ? 1 : 0;
-    a.rec = final_direct ? (double *)ctx->result.p : (double *)ctx->part.p;
+    a.rec = final_direct ? resp : (double *)ctx->part.p;
     a.seg = final_direct ? (int *)ctx->list.p : (int *)ctx->seg.p;
     a.segcap = segcap;
     a.overflow_flag = (int *)ctx->flags.p;
@@ -793,7 +836,7 @@ static int run_force(s2_ctx *ctx, int ni, const int *d_i_addr, const double *d_h
     a.fused = fused ? 1 : 0;
     a.cluster = fused ? sh.cluster : 1;
     a.counters = (unsigned *)ctx->counters.p;
-    a.out_final = (double *)ctx->result.p;
+    a.out_final = resp;
     a.order = ctx->order;
     a.atomic = atomic ? 1 : 0;
     if (atomic) CU(cudaMemsetAsync(ctx->result.p, 0, (size_t)ni * REC * sizeof(double), ctx->stream));
@@ -805,6 +848,7 @@ static int run_force(s2_ctx *ctx, int ni, const int *d_i_addr, const double *d_h
         ctx->ran_force = true;
         ctx->ran_reduce = false;
         ctx->calc_done = true;
+        ctx->res_on_host = false;
         ctx->ni_last = ni;
         ctx->flags_last = flags;
         return S2_OK;
@@ -822,7 +866,7 @@ static int run_force(s2_ctx *ctx, int ni, const int *d_i_addr, const double *d_h
     if (!final_direct && !fused && !atomic) {
         ReduceArgs r{};
         r.part = (const double *)ctx->part.p;
-        r.out = (double *)ctx->result.p;
+        r.out = resp;
         r.seg = (const int *)ctx->seg.p;
         r.list = (int *)ctx->list.p;
         r.jid_plane = plane(ctx, 3);
@@ -844,6 +888,7 @@ static int run_force(s2_ctx *ctx, int ni, const int *d_i_addr, const double *d_h
     li[5] = (int)smem; li[6] = final_direct ? 0 : (fused ? 2 : (atomic ? 4 : 1));
     li[8] = sh.L == 0 ? force_ipt(ctx->precision) : 1; li[9] = a.cluster;
     ctx->calc_done = true;
+    ctx->res_on_host = host_res;
     ctx->ni_last = ni;
     ctx->flags_last = flags;
     return S2_OK;
@@ -865,7 +910,7 @@ extern "C" int s2_calc_ilist_device(s2_ctx *ctx, int ni, const int *d_i_address,
     if (rc != S2_OK) return rc;
     if (!d_i_address) return S2_EINVAL;
     CU(cudaSetDevice(ctx->device));
-    return run_force(ctx, ni, d_i_address, d_h2, false, eps2, flags);
+    return run_force(ctx, ni, d_i_address, d_h2, false, eps2, flags, false);
 }
 
 extern "C" int s2_calc_ilist(s2_ctx *ctx, int ni, const int *i_address, const double *h2, double eps2,
@@ -879,6 +924,23 @@ extern "C" int s2_calc_ilist(s2_ctx *ctx, int ni, const int *i_address, const do
     CU(cudaSetDevice(ctx->device));
     const bool ngb = flags & S2_WANT_NGB;
     const size_t b_addr = align16((size_t)ni * sizeof(int)), b_h2 = ngb ? (size_t)ni * sizeof(double) : 0;
+    if (ni <= kZeroCopyNi && ctx->tune[9] != 1) {
+        // small call: the kernels read the i-list (and h2) from pinned host memory; two buffers alternate, each
+        // guarded by an event recorded behind the kernels that read it
+        const int k = ctx->il_turn;
+        ctx->il_turn ^= 1;
+        CU(cudaEventSynchronize(ctx->ev_il[k]));
+        rc = pinned_reserve(ctx, &ctx->h_il[k], &ctx->h_il_bytes[k], 0,
+                            align16((size_t)kZeroCopyNi * sizeof(int)) + (size_t)kZeroCopyNi * sizeof(double));
+        if (rc != S2_OK) return rc;
+        memcpy(ctx->h_il[k], i_address, (size_t)ni * sizeof(int));
+        if (ngb) memcpy((char *)ctx->h_il[k] + b_addr, h2, b_h2);
+        rc = run_force(ctx, ni, (const int *)ctx->h_il[k], ngb ? (const double *)((char *)ctx->h_il[k] + b_addr) : nullptr,
+                       false, eps2, flags, true);
+        if (rc != S2_OK) return rc;
+        CU(cudaEventRecord(ctx->ev_il[k], ctx->stream));
+        return S2_OK;
+    }
     CU(cudaEventSynchronize(ctx->ev_io));
     rc = pinned_reserve(ctx, &ctx->h_io, &ctx->h_io_bytes, 0, b_addr + b_h2);
     if (rc == S2_OK) rc = dev_reserve(ctx, ctx->i_addr, b_addr + b_h2);
@@ -888,7 +950,7 @@ extern "C" int s2_calc_ilist(s2_ctx *ctx, int ni, const int *i_address, const do
     CU(cudaMemcpyAsync(ctx->i_addr.p, ctx->h_io, b_addr + b_h2, cudaMemcpyHostToDevice, ctx->stream));
     CU(cudaEventRecord(ctx->ev_io, ctx->stream));
     return run_force(ctx, ni, (const int *)ctx->i_addr.p,
-                     ngb ? (const double *)((char *)ctx->i_addr.p + b_addr) : nullptr, false, eps2, flags);
+                     ngb ? (const double *)((char *)ctx->i_addr.p + b_addr) : nullptr, false, eps2, flags, true);
 }
 
 static inline void split_ds_host(double x, float *hi, float *lo)
@@ -965,14 +1027,21 @@ extern "C" int s2_calc_explicit(s2_ctx *ctx, int ni, const int *id, const double
     if (nq) CU(cudaMemcpyAsync(ctx->iqplanes.p, (char *)ctx->h_io + b_p, b_q, cudaMemcpyHostToDevice, ctx->stream));
     if (ngb) CU(cudaMemcpyAsync(ctx->i_h2.p, (char *)ctx->h_io + b_p + b_q, b_h2, cudaMemcpyHostToDevice, ctx->stream));
     CU(cudaEventRecord(ctx->ev_io, ctx->stream));
-    return run_force(ctx, ni, nullptr, ngb ? (const double *)ctx->i_h2.p : nullptr, true, eps2, flags);
+    return run_force(ctx, ni, nullptr, ngb ? (const double *)ctx->i_h2.p : nullptr, true, eps2, flags, true);
 }
 
 // ---- a9: results --------------------------------------------------------------------------
 
+// flag 0: a neighbour list overflowed in the last call; flag 1: a device-side commit dropped an address.  Neither
+// can be set unless lists were asked for or s2_commit_j_device ran, and then the copy is skipped (small calls)
 static int fetch_flags(s2_ctx *ctx)
 {
+    if (!(ctx->flags_last & S2_WANT_NGB) && !ctx->flags_dirty) {
+        ctx->h_flags[0] = ctx->h_flags[1] = 0;
+        return S2_OK;
+    }
     CU(cudaMemcpyAsync(ctx->h_flags, ctx->flags.p, 2 * sizeof(int), cudaMemcpyDeviceToHost, ctx->stream));
+    ctx->flags_dirty = false;
     return S2_OK;
 }
 
@@ -994,15 +1063,18 @@ extern "C" int s2_get_results(s2_ctx *ctx, int ni, double *acc, double *jerk, do
     if (ni > ctx->ni_last) return S2_ERANGE;
     CU(cudaSetDevice(ctx->device));
     const size_t bytes = (size_t)ni * REC * sizeof(double);
-    CU(cudaEventSynchronize(ctx->ev_io));
-    int rc = pinned_reserve(ctx, &ctx->h_io, &ctx->h_io_bytes, 0, bytes);
-    if (rc != S2_OK) return rc;
-    if (ni) CU(cudaMemcpyAsync(ctx->h_io, ctx->result.p, bytes, cudaMemcpyDeviceToHost, ctx->stream));
+    int rc = S2_OK;
+    if (!ctx->res_on_host) {
+        CU(cudaEventSynchronize(ctx->ev_io));
+        rc = pinned_reserve(ctx, &ctx->h_io, &ctx->h_io_bytes, 0, bytes);
+        if (rc != S2_OK) return rc;
+        if (ni) CU(cudaMemcpyAsync(ctx->h_io, ctx->result.p, bytes, cudaMemcpyDeviceToHost, ctx->stream));
+    }
     rc = fetch_flags(ctx);
     if (rc != S2_OK) return rc;
     CU(cudaStreamSynchronize(ctx->stream));
     CU(cudaGetLastError());
-    const double *r0 = (const double *)ctx->h_io;
+    const double *r0 = (const double *)(ctx->res_on_host ? ctx->h_res : ctx->h_io);   // small calls: written by the kernels
     const int order = ctx->order;
     par_ranges((size_t)ni, (size_t)16384, [=](size_t lo, size_t hi) {
     const double *r = r0 + lo * REC;
@@ -1028,9 +1100,11 @@ extern "C" int s2_get_neighbours(s2_ctx *ctx, int i, int cap, int *n_out, int *l
     if (i < 0 || i >= ctx->ni_last) return S2_ERANGE;
     CU(cudaSetDevice(ctx->device));
     double rec8 = 0.0;
-    CU(cudaMemcpyAsync(&rec8, (double *)ctx->result.p + (size_t)i * REC + 8, sizeof(double), cudaMemcpyDeviceToHost,
-                       ctx->stream));
+    if (!ctx->res_on_host)
+        CU(cudaMemcpyAsync(&rec8, (double *)ctx->result.p + (size_t)i * REC + 8, sizeof(double), cudaMemcpyDeviceToHost,
+                           ctx->stream));
     CU(cudaStreamSynchronize(ctx->stream));
+    if (ctx->res_on_host) rec8 = ((const double *)ctx->h_res)[(size_t)i * REC + 8];
     int packed[2];
     memcpy(packed, &rec8, sizeof packed);
     const int have = std::min(packed[1], ctx->ngb_cap);
@@ -1057,11 +1131,12 @@ extern "C" int s2_get_neighbours_csr(s2_ctx *ctx, int ni, long long *offsets, in
     int rc = pinned_reserve(ctx, &ctx->h_io, &ctx->h_io_bytes, 0, b_rec + b_list);
     if (rc != S2_OK) return rc;
     if (ni) {
-        CU(cudaMemcpyAsync(ctx->h_io, ctx->result.p, (size_t)ni * REC * sizeof(double), cudaMemcpyDeviceToHost, ctx->stream));
+        if (!ctx->res_on_host)
+            CU(cudaMemcpyAsync(ctx->h_io, ctx->result.p, (size_t)ni * REC * sizeof(double), cudaMemcpyDeviceToHost, ctx->stream));
         CU(cudaMemcpyAsync((char *)ctx->h_io + b_rec, ctx->list.p, b_list, cudaMemcpyDeviceToHost, ctx->stream));
     }
     CU(cudaStreamSynchronize(ctx->stream));
-    const double *r = (const double *)ctx->h_io;
+    const double *r = (const double *)(ctx->res_on_host ? ctx->h_res : ctx->h_io);
     const int *L = (const int *)((const char *)ctx->h_io + b_rec);
     long long tot = 0;
     bool overflow = false;
@@ -1131,7 +1206,7 @@ extern "C" int s2_get_j(s2_ctx *ctx, int first, int n, int *id, double *t, doubl
 
 extern "C" int s2_set_tuning(s2_ctx *ctx, int key, int value)
 {
-    if (!ctx || key < 0 || key > 8 || value < 0) return S2_EINVAL;
+    if (!ctx || key < 0 || key > 9 || value < 0) return S2_EINVAL;
     ctx->tune[key] = value;
     return S2_OK;
 }

@@ -227,6 +227,38 @@ def test_atomic_combine_option():
     s2.s2_close(ctx)
 
 
+def test_zero_copy_small_calls_equal_copied_ones():
+    """Small host calls (n_i <= 128) let the kernels read the i-list from and write the records to pinned host memory
+    (no copy operation enqueued).  Results, neighbour lists and error codes are bit-identical to the copied path
+    (s2_set_tuning key 9 = 1), also when several calls are enqueued back to back (alternating i-list buffers)."""
+    for cfg, N in ((2, 64), (3, 8192)):
+        w = make_config(cfg, N=N)
+        ctx = open_and_load(w, 4, ngb_cap=8)
+        s2.s2_predict(ctx, w.t_pred, w.N)
+        for ni in (1, 7, 64, 128, 129):
+            ni = min(ni, N)
+            il = w.ilist(ni)
+            h2 = w.h2[il] * 4.0
+            out = {}
+            for zc in (1, 0):
+                s2.s2_set_tuning(ctx, 9, zc)
+                for junk in (w.ilist(min(N, 3)), w.ilist(min(N, 100))):      # enqueued before, never read back
+                    s2.s2_calc_ilist(ctx, junk, None, w.eps2, 0)
+                s2.s2_calc_ilist(ctx, il, h2, w.eps2, NN | NGB)
+                r = s2.s2_get_results(ctx, ni)
+                off, lst = s2.s2_get_neighbours_csr(ctx, ni)
+                one = s2.s2_get_neighbours(ctx, ni - 1, 8)
+                out[zc] = (r, off, lst, one)
+            a, b = out[1], out[0]
+            for k in ("acc", "jerk", "pot", "nn_id", "nn_r2", "ngb_count"):
+                assert np.array_equal(a[0][k], b[0][k]), (cfg, ni, k)
+            assert a[0]["overflow"] == b[0]["overflow"]
+            assert np.array_equal(a[1], b[1]) and np.array_equal(a[2], b[2]) and np.array_equal(a[3], b[3])
+            ref, _ = oracle_on_gpu_prediction(ctx, w, 4, il, w.eps2, h2, ngb_cap=8)
+            check_forces(b[0], ref, s2.S2_FP64, 4, NN | NGB, f"zero-copy cfg {cfg} n_i {ni}")
+        s2.s2_close(ctx)
+
+
 # ------------------------------------------------------------------------------- ties
 def test_lattice_ties_and_strictness_gpu():
     w = lattice_workload(4, 0.25)
