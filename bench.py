@@ -493,6 +493,30 @@ def hbm_kernels(s2, torch, dev, hbm_gbs):
             out.append({"kernel": name, "N": w.N, "order": order, "bytes": b, "us": round(us, 2), "GB/s": gbs,
                         "frac_of_measured_hbm": gbs / hbm_gbs})
         s2.s2_close(ctx)
+        if order == 4:
+            # the combine of the j-slices (a6): 2^20 explicit sinks against a 4096-particle store in 4 forced slices,
+            # so that the 4 x 2^20 partial records (403 MB) exceed L2; kernel time from the library's events
+            S, nj = 4, 4096
+            ctx = s2.s2_open(dev.index, 4, s2.S2_FP64, nj_capacity=nj, ngb_cap=0)
+            a = np.arange(nj, dtype=np.int32)
+            s2.s2_set_j(ctx, a, w.ident[:nj], w.t_j[:nj], w.mass[:nj], w.pos[:nj], w.vel[:nj], w.acc[:nj], w.jerk[:nj])
+            s2.s2_commit_j(ctx)
+            s2.s2_predict(ctx, w.t_pred, nj)
+            s2.s2_enable_timing(ctx, True)
+            for k, v in ((0, S), (5, 1), (7, 2)):
+                s2.s2_set_tuning(ctx, k, v)
+            ids = np.full(w.N, -1, dtype=np.int32)
+            best = 1e9
+            for _ in range(3):
+                s2.s2_calc_explicit(ctx, ids, w.pos, w.vel, None, None, w.eps2, 0)
+                best = min(best, s2.s2_get_timing(ctx)["reduce_ms"])
+            info = s2.s2_last_launch_info(ctx)
+            b = (info["S"] + 1) * w.N * 96
+            gbs = b / (best * 1e-3) / 1e9
+            out.append({"kernel": f"reduce_thread_kernel<{info['S']}>", "n_i": w.N, "rows": info["S"], "order": 4, "bytes": b,
+                        "us": round(best * 1e3, 2), "GB/s": gbs, "frac_of_measured_hbm": gbs / hbm_gbs,
+                        "timing": "CUDA events around the launch"})
+            s2.s2_close(ctx)
     return out
 
 

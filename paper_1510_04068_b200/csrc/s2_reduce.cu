@@ -106,9 +106,95 @@ __global__ void __launch_bounds__(256) reduce_kernel(const ReduceArgs a)
     }
 }
 
+// Few partial rows, many i-particles (the full-occupancy sweeps with 2-16 j-slices): one THREAD per i streams its
+// rows with coalesced loads instead of one warp per i with 2-16 active lanes.  The additions follow the same balanced
+// tree the warp butterfly of reduce_rows_warp forms (rows beyond NST are its zero lanes), so the sums have the same bits:
+//   T(lo, w) = T(lo, w/2) + T(lo + w/2, w/2),  T(l, 1) = row l.
+struct RowSum {
+    double v[10];
+    double nn_d2;
+    int nn_j;
+};
+
+template <int NST, int LO, int W, bool NN>
+__device__ __forceinline__ void tree_rows(const double *part, size_t ni, size_t i, int order, RowSum &out)
+{
+    if constexpr (W == 1) {
+        const double2 *r = reinterpret_cast<const double2 *>(part + ((size_t)LO * ni + i) * REC);
+        const double2 r0 = r[0], r1 = r[1], r2 = r[2], r3 = r[3], r4 = r[4];
+        out.v[0] = r0.x; out.v[1] = r0.y; out.v[2] = r1.x; out.v[3] = r1.y; out.v[4] = r2.x; out.v[5] = r2.y;
+        out.v[6] = r3.x;
+        out.v[7] = out.v[8] = out.v[9] = 0.0;
+        if (order == 6) {
+            const double2 r5 = r[5];
+            out.v[7] = r4.y; out.v[8] = r5.x; out.v[9] = r5.y;
+        }
+        out.nn_d2 = r3.y;
+        out.nn_j = __double2loint(r4.x);
+    } else {
+        tree_rows<NST, LO, W / 2, NN>(part, ni, i, order, out);
+        if constexpr (LO + W / 2 < NST) {
+            RowSum o;
+            tree_rows<NST, LO + W / 2, W / 2, NN>(part, ni, i, order, o);
+#pragma unroll
+            for (int c = 0; c < 10; ++c) out.v[c] += o.v[c];
+            if (NN && (o.nn_d2 < out.nn_d2 || (o.nn_d2 == out.nn_d2 && (unsigned)o.nn_j < (unsigned)out.nn_j))) {
+                out.nn_d2 = o.nn_d2;
+                out.nn_j = o.nn_j;
+            }
+        }
+    }
+}
+
+template <int NST, bool NN>
+__global__ void __launch_bounds__(256) reduce_thread_kernel(const ReduceArgs a)
+{
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= a.ni) return;
+    RowSum t;
+    tree_rows<NST, 0, (NST > 8 ? 16 : 8), NN>(a.part, (size_t)a.ni, (size_t)i, a.order, t);
+    int nn = NN ? t.nn_j : -1;
+    if (NN && nn >= 0) nn = __double2loint(a.jid_plane[nn].y);
+    double2 *o = reinterpret_cast<double2 *>(a.out + (size_t)i * REC);
+    o[0] = make_double2(t.v[0], t.v[1]);
+    o[1] = make_double2(t.v[2], t.v[3]);
+    o[2] = make_double2(t.v[4], t.v[5]);
+    o[3] = make_double2(t.v[6], NN ? t.nn_d2 : CUDART_INF);
+    o[4] = make_double2(__hiloint2double(0, nn), t.v[7]);
+    o[5] = make_double2(t.v[8], t.v[9]);
+}
+
+template <int NST>
+static cudaError_t launch_reduce_thread(const ReduceArgs &a, cudaStream_t st)
+{
+    const dim3 grid((a.ni + 255) / 256);
+    if (a.flags & S2_WANT_NN) reduce_thread_kernel<NST, true><<<grid, 256, 0, st>>>(a);
+    else reduce_thread_kernel<NST, false><<<grid, 256, 0, st>>>(a);
+    return cudaGetLastError();
+}
+
 cudaError_t launch_reduce(const ReduceArgs &a, cudaStream_t st)
 {
     if (a.ni <= 0) return cudaSuccess;
+    if (!(a.flags & S2_WANT_NGB) && a.nslices_total <= 16 && a.ni >= 4096) {
+        switch (a.nslices_total) {   // ordinary stream order (no programmatic launch): the rows are read through L1
+        case 2: return launch_reduce_thread<2>(a, st);
+        case 3: return launch_reduce_thread<3>(a, st);
+        case 4: return launch_reduce_thread<4>(a, st);
+        case 5: return launch_reduce_thread<5>(a, st);
+        case 6: return launch_reduce_thread<6>(a, st);
+        case 7: return launch_reduce_thread<7>(a, st);
+        case 8: return launch_reduce_thread<8>(a, st);
+        case 9: return launch_reduce_thread<9>(a, st);
+        case 10: return launch_reduce_thread<10>(a, st);
+        case 11: return launch_reduce_thread<11>(a, st);
+        case 12: return launch_reduce_thread<12>(a, st);
+        case 13: return launch_reduce_thread<13>(a, st);
+        case 14: return launch_reduce_thread<14>(a, st);
+        case 15: return launch_reduce_thread<15>(a, st);
+        case 16: return launch_reduce_thread<16>(a, st);
+        }
+    }
     const int warps_per_block = a.ni <= 1024 ? 2 : 8;   // few i: spread the warps over more SMs
     cudaLaunchConfig_t cfg = {};
     cfg.gridDim = dim3((a.ni + warps_per_block - 1) / warps_per_block);

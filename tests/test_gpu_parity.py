@@ -194,6 +194,30 @@ def test_bit_reproducible_and_paths_agree():
     s2.s2_close(ctx)
 
 
+@pytest.mark.parametrize("order", [4, 6])
+def test_thread_per_i_reduce_has_the_bits_of_the_warp_reduce(order):
+    """With 2-16 partial rows and >= 4096 i-particles reduce_thread_kernel (one thread per i, coalesced) replaces
+    reduce_kernel (one warp per i); it adds the rows in the tree order of the warp butterfly, so an i-particle gets
+    the same bits from a 4095-particle call (warp kernel) and a 4096-particle call (thread kernel)."""
+    w = make_config(4 if order == 6 else 3, N=8192)
+    ctx = open_and_load(w, order)
+    s2.s2_predict(ctx, w.t_pred, w.N)
+    il = w.ilist(4096)
+    for S in (2, 3, 5, 8, 9, 13, 16):
+        for flags in (0, NN):
+            s2.s2_set_tuning(ctx, 0, S); s2.s2_set_tuning(ctx, 1, 1); s2.s2_set_tuning(ctx, 7, 1); s2.s2_set_tuning(ctx, 5, 1)
+            s2.s2_calc_ilist(ctx, il[:4095], eps2=w.eps2, flags=flags)
+            a = s2.s2_get_results(ctx, 4095)
+            s2.s2_calc_ilist(ctx, il, eps2=w.eps2, flags=flags)
+            assert s2.s2_last_launch_info(ctx)["reduced"] == 1 and s2.s2_last_launch_info(ctx)["S"] == S
+            b = s2.s2_get_results(ctx, 4096)
+            for k in ("acc", "jerk", "pot", "nn_id", "nn_r2") + (("snap",) if order == 6 else ()):
+                assert np.array_equal(a[k], b[k][:4095]), (S, flags, k)
+            ref, _ = oracle_on_gpu_prediction(ctx, w, order, il, w.eps2)
+            check_forces(b, ref, s2.S2_FP64, order, flags, f"thread reduce S={S}")
+    s2.s2_close(ctx)
+
+
 def test_atomic_combine_option():
     """the paper's single-kernel combine by atomics (L88) as an opt-in (s2_set_tuning key 5 = 2).
     Within tolerance of the oracle, equal to the deterministic combine up to summation order, and never used when
