@@ -373,7 +373,8 @@ def ni_sweep(s2, torch, dev, order):
     fewer than 2e8 pairs are timed by CUDA-graph replay of 20 calls, larger ones by CUDA events per call."""
     from workloads import make_config
     out = []
-    plan = ((3, "fp64", s2.S2_FP64, (1, 32, 256, 2048, 16384, 65536)),
+    pow2 = tuple(1 << k for k in range(17))    # fp64 at config 3's N: every power of two from 1 to N (Fig. 2's axis)
+    plan = ((3, "fp64", s2.S2_FP64, pow2),
             (3, "ds", s2.S2_DS, (1, 32, 256, 2048, 16384, 65536)),
             (3, "fp32", s2.S2_FP32, (1, 32, 256, 2048, 16384, 65536)),
             ("H", "fp64", s2.S2_FP64, (1, 32, 256, 4096, 262144)),
@@ -414,8 +415,10 @@ def ni_sweep(s2, torch, dev, order):
                 for _ in range(300):
                     s2.s2_calc_ilist(ctx, il_h, None, w.eps2, 0); s2.s2_get_results(ctx, ni)
                 host_us = (time.perf_counter() - t0) / 300 * 1e6
+            peak = FP64_PEAK_TFLOPS if pname == "fp64" else FP32_PEAK_TFLOPS
             rows.append({"cfg": str(key), "precision": pname, "N": w.N, "n_i": ni, "call_us": round(us, 2), "timing": how,
                          "ginteractions_per_s": g, "vs_full_rate": g / full,
+                         "frac_of_peak_60flop": g * 1e9 * FLOP_PER_PAIR[4] / 1e12 / peak,
                          "S": info["S"], "lanes_per_i": info["lanes_per_i"], "warp_columns": info["warp_columns"],
                          "i_per_thread": info["i_per_thread"], "grid": info["grid"],
                          "combine": ("none", "reduce kernel", "fused", "none (chunk launches)", "atomics")[info["reduced"]]})

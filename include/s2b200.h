@@ -172,7 +172,8 @@ int s2_get_j(s2_ctx *ctx, int first, int n, int *id, double *t, double *mass, do
  *   key 3: CTAs per SM assumed by the balancer      key 4: j-tile length (multiple of 32)
  *   key 5: 1 = combine j-slices with the separate reduce kernel even when the fused combine applies,
  *          2 = combine them with fp64 atomics on the final records instead (the paper's Sapporo2 scheme, L88): one
- *          launch, but the last bits then vary run to run; ignored when NN / neighbour lists are requested
+ *          launch, but the last bits then vary run to run; ignored when NN / neighbour lists are requested,
+ *          3 = use the fused combine (last CTA of each i-group) whenever the shape allows it
  *   key 6: CTAs per thread-block cluster along the slice axis in the fused combine (1 = none, 2, 4, 8)
  *   key 7: 1 = never use the register-tiled sweep (several i per thread), 2 = always use it
  *   key 8: 1 = never use the uniform-operand sweep (j-particles read chunk by chunk from the constant bank, one

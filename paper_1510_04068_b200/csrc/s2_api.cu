@@ -559,7 +559,7 @@ static int choose_shape(s2_ctx *ctx, int ni, int nj, unsigned flags, ForceShape 
                 int S = cand[q];
                 // neighbour segments must stay ascending per record: a warp column may then only take a part of ONE tile
                 if (want_ngb && Wj > 1 && (nj + S - 1) / S > tile_max) S = (nj + tile_max - 1) / tile_max;
-                const bool fusable = !want_ngb && ctx->tune[5] == 0 && S * Wj > 1 && L != 0;
+                const bool fusable = !want_ngb && (ctx->tune[5] == 0 || ctx->tune[5] == 3) && S * Wj > 1 && L != 0;
                 // clusters of C CTAs along the slice axis pre-combine their records through distributed shared
                 // memory (j-split shapes only: their record block, <= 128 x 96 B, always fits the tile buffers)
                 int C = 1;
@@ -586,11 +586,17 @@ static int choose_shape(s2_ctx *ctx, int ni, int nj, unsigned flags, ForceShape 
                 int fused = 0;
                 if (nst > 1) {
                     const double rounds_f = std::ceil(std::min(icta, ni) / (double)kWarps) * std::ceil((S / C) / 32.0);
-                    const double fused_cost = (1.0 + rounds_f) * C_.c_row + (C > 1 ? C_.c_row : 0.0);
+                    // the fused tail (fence, arrival counter, the last CTA's serial reduce; nothing overlaps it) costs
+                    // ~2 us more than the same rounds in the separate launch, whose latency programmatic dependent
+                    // launch hides (measured at N = 65536, same sweep shape: n_i = 8: 12.0 vs 9.9 us, n_i = 1: 8.9 vs 8.5)
+                    const double fused_cost = (1.0 + rounds_f) * C_.c_row + (C > 1 ? C_.c_row : 0.0) + 4000.0;
                     const double sep_cost = C_.c_launch + std::ceil(nst / 32.0) * C_.c_row * 0.5 +
                                             (double)ni * nst * (REC * 8.0) / 2000.0;
-                    fused = fusable && (fused_cost < sep_cost || ctx->tune[6] > 1);
+                    fused = fusable && (fused_cost < sep_cost || ctx->tune[6] > 1 || ctx->tune[5] == 3);
                     if (!fused && C > 1) continue;              // a cluster shape only makes sense fused
+                    // warp columns only pay when the CTA adds them up in shared memory (the fused path); unfused, every
+                    // column writes its own partial row (measured at N = 2^18, n_i = 1: 16.7 us against 10.4 us fused)
+                    if (!fused && Wj > 1 && !want_ngb && ctx->tune[2] == 0 && ctx->tune[5] == 0) continue;
                     cost += fused ? fused_cost : sep_cost;
                 }
                 if (cost < best * (1 - 1e-9)) {
