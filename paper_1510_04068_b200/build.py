@@ -41,7 +41,11 @@ def build(force: bool = False, verbose: bool = False) -> str:
         s = os.path.join(CSRC, src)
         o = os.path.join(OBJ, src[:-3] + ".o")
         objs.append(o)
-        if force or not os.path.exists(o) or os.path.getmtime(o) < max(os.path.getmtime(s), hdr_m):
+        src_m = os.path.getmtime(s)
+        for line in open(s):   # a .cu that includes another .cu (second instance of a module) depends on it
+            if line.startswith('#include "') and line.rstrip().endswith('.cu"'):
+                src_m = max(src_m, os.path.getmtime(os.path.join(CSRC, line.split('"')[1])))
+        if force or not os.path.exists(o) or os.path.getmtime(o) < max(src_m, hdr_m):
             jobs.append([NVCC, *FLAGS, "-c", s, "-o", o])
 
     def run(cmd):

@@ -20,9 +20,16 @@ __device__ __forceinline__ double rsqrt_seed(double s)
 }
 
 // j-bank of the uniform-operand sweep (force_sweep_bank_kernel below): the whole 64 KB constant bank of this
-// module holds one chunk of predicted j-particles, plane p at c_jbank[p * kChunk ..]
+// module holds one chunk of predicted j-particles, plane p at c_jbank[p * kChunk ..].  Every translation unit is a
+// CUDA module of its own with its own bank, so this file is compiled twice (S2_BANK_ID 0 here, 1 through
+// s2_force_fp64_bank1.cu): while the sweep reads one bank, the next chunk is copied into the other.
+#ifndef S2_BANK_ID
+#define S2_BANK_ID 0
+#endif
+#define S2_CAT2(a, b) a##b
+#define S2_CAT(a, b) S2_CAT2(a, b)
 constexpr int kBankBytes = 65536;
-__constant__ double2 c_jbank[kBankBytes / 16];
+static __constant__ double2 c_jbank[kBankBytes / 16];
 
 template <int ORDER_, bool NN_, bool NGB_>
 struct PolicyF64 {
@@ -243,6 +250,7 @@ struct PolicyF64 {
     }
 };
 
+#ifndef S2_BANK_ONLY
 cudaError_t dispatch_force_fp64(int order, unsigned flags, int L, dim3 grid, size_t smem, const ForceArgs &a,
                                 cudaStream_t st, bool query, int *ctas_per_sm)
 {
@@ -262,6 +270,8 @@ cudaError_t dispatch_force_fp64(int order, unsigned flags, int L, dim3 grid, siz
     return launch_L<PolicyF64<6, false, false>>(L, grid, smem, a, st, query, ctas_per_sm);
 }
 
+#endif   // S2_BANK_ONLY
+
 // ---- uniform-operand sweep (a4 at the largest n_i) ------------------------------------------------------------
 // Every lane of a warp reads the same j-particle, so j is warp-uniform data.  Here it is not staged through
 // shared memory at all: a chunk of the predicted j-store is copied into the module's constant bank between
@@ -270,7 +280,7 @@ cudaError_t dispatch_force_fp64(int order, unsigned flags, int L, dim3 grid, siz
 // each and every barrier: warps are fully independent, one i-particle per lane, eight pairs in
 // flight per thread.  The price is one launch per chunk (1024 j at 4th order), with the running sums carried
 // through an SoA state buffer; sums are added in address order chunk by chunk, so results are bit-reproducible.
-template <class P>
+template <class P, int BANK>   // BANK only makes the kernels of the two translation units distinct symbols
 __global__ void __launch_bounds__(P::kBankThreads, P::kMinBlocksBank) force_sweep_bank_kernel(const ForceArgs a)
 {
     constexpr int NC = P::ORDER == 6 ? 10 : 7;   // running sums carried per i
@@ -358,12 +368,12 @@ static cudaError_t launch_bank(const ForceArgs &a, cudaStream_t st, int *geom)
 {
     if (geom) { geom[0] = P::kChunk; geom[1] = P::kBankThreads; geom[2] = P::kMinBlocksBank; return cudaSuccess; }
     const dim3 grid((a.ni + P::kBankThreads - 1) / P::kBankThreads);
-    force_sweep_bank_kernel<P><<<grid, P::kBankThreads, 0, st>>>(a);
+    force_sweep_bank_kernel<P, S2_BANK_ID><<<grid, P::kBankThreads, 0, st>>>(a);
     return cudaGetLastError();
 }
 
 // geom != nullptr: only report {chunk length of this order's bank layout, threads per CTA, CTAs per SM aimed at}
-cudaError_t dispatch_force_fp64_bank(int order, unsigned flags, const ForceArgs &a, cudaStream_t st, int *geom)
+cudaError_t S2_CAT(dispatch_force_fp64_bank, S2_BANK_ID)(int order, unsigned flags, const ForceArgs &a, cudaStream_t st, int *geom)
 {
     const bool ngb = flags & S2_WANT_NGB, nn = (flags & S2_WANT_NN) || ngb;
     if (order == 2) {
@@ -382,6 +392,6 @@ cudaError_t dispatch_force_fp64_bank(int order, unsigned flags, const ForceArgs 
 }
 
 // device address of the constant bank (target of the per-chunk device-to-device copies)
-cudaError_t force_bank_address(void **p) { return cudaGetSymbolAddress(p, c_jbank); }
+cudaError_t S2_CAT(force_bank_address, S2_BANK_ID)(void **p) { return cudaGetSymbolAddress(p, c_jbank); }
 
 }  // namespace s2
