@@ -655,6 +655,8 @@ struct BankOwner {
     cudaEvent_t ev = nullptr;
     cudaStream_t stream = nullptr;
     bool used = false;
+    unsigned *flags = nullptr;   // device words {ready[2], done[2], arrived[2]} (flag hand-shake, see run_force_bank)
+    unsigned ticket = 0;         // tickets handed out so far (chunk sequence numbers, cyclic)
 };
 static std::mutex g_bank_mu;
 static std::map<int, BankOwner> g_bank;
@@ -666,7 +668,7 @@ static std::map<int, BankOwner> g_bank;
 static bool bank_applies(const s2_ctx *ctx, int ni, int nj)
 {
     if (ctx->precision != S2_FP64 || ctx->tune[8] == 1) return false;
-    if (ctx->tune[8] == 2) return true;
+    if (ctx->tune[8] >= 2) return true;   // 3: forced, without programmatic dependent launch (A/B measurements)
     for (int k = 0; k < 8; ++k)
         if (ctx->tune[k]) return false;   // an explicit launch shape was asked for
     if (ctx->order != 4 || nj < 8192) return false;
@@ -681,9 +683,37 @@ static cudaError_t dispatch_bank(int b, int order, unsigned flags, const ForceAr
     return b ? dispatch_force_fp64_bank1(order, flags, a, st, geom) : dispatch_force_fp64_bank0(order, flags, a, st, geom);
 }
 
-// Chunk c lives in bank c & 1.  The refills run on a side stream: the copy of chunk c waits for the launch that read
-// chunk c - 2 out of the same bank, the launch of chunk c waits for its copy -- so a refill overlaps the sweep of the
-// other bank (measured: the exposed copies were 0.9 % of the sweep at n_i = 2^18).
+// Stream memory operations of the driver (wait until a device word reaches a value / write a device word), fetched
+// through the runtime so that the library does not link libcuda: they let the refill stream and the sweep kernels hand
+// the banks over through flags in device memory, with no event operation between two chunk launches.
+typedef int (*StreamValueFn)(cudaStream_t, unsigned long long, unsigned, unsigned);
+static StreamValueFn g_wait_value = nullptr, g_write_value = nullptr;
+static bool g_value_ops_probed = false;
+static bool stream_value_ops()
+{
+    if (!g_value_ops_probed) {
+        g_value_ops_probed = true;
+        void *w = nullptr, *x = nullptr;
+        cudaDriverEntryPointQueryResult q1, q2;
+        if (cudaGetDriverEntryPoint("cuStreamWaitValue32", &w, cudaEnableDefault, &q1) == cudaSuccess &&
+            cudaGetDriverEntryPoint("cuStreamWriteValue32", &x, cudaEnableDefault, &q2) == cudaSuccess &&
+            q1 == cudaDriverEntryPointSuccess && q2 == cudaDriverEntryPointSuccess && w && x) {
+            g_wait_value = (StreamValueFn)w;
+            g_write_value = (StreamValueFn)x;
+        }
+        cudaGetLastError();
+    }
+    return g_wait_value && g_write_value;
+}
+
+// Chunk c lives in bank c & 1 and carries ticket base + c + 1.  The refills run on a side stream.  Hand-over of a bank:
+//   flag path (default): the last CTA of the launch that swept chunk c stores done[bank] = ticket(c); the side stream
+//     waits for that value, copies chunk c + 2 and writes ready[bank] = ticket(c + 2); the launch of chunk c + 2 spins
+//     on ready[bank] before it reads the bank.  Nothing sits between two chunk launches in the main stream, so they are
+//     launched with programmatic stream serialisation: the next launch fills the SMs while this one drains, and every
+//     CTA reads the previous launch's totals behind griddepcontrol.wait (499 -> 519 Gpairs/s at n_i = 2^18);
+//   event path (stream capture, or no stream memory operations): events order copies and launches (no overlap of
+//     launches).
 static int run_force_bank(s2_ctx *ctx, ForceArgs &a, int ni, unsigned flags)
 {
     int geom[3] = {0, 0, 0};
@@ -723,14 +753,27 @@ static int run_force_bank(s2_ctx *ctx, ForceArgs &a, int ni, unsigned flags)
     cudaStreamCaptureStatus cap = cudaStreamCaptureStatusNone;
     CU(cudaStreamIsCapturing(ctx->stream, &cap));
     const bool capturing = cap != cudaStreamCaptureStatusNone;
+    const bool by_flags = !capturing && ctx->tune[8] != 3 && stream_value_ops();
+    if (by_flags && !own.flags) {
+        CU(cudaMalloc((void **)&own.flags, 64));
+        CU(cudaMemset(own.flags, 0, 64));
+    }
     if (!capturing && own.used && own.stream != ctx->stream) CU(cudaStreamWaitEvent(ctx->stream, own.ev, 0));
     if (ctx->timing) CU(cudaEventRecord(ctx->ev_t[2], ctx->stream));
     // fork: the side stream starts behind everything enqueued so far (the predictor, earlier sweeps on the banks)
     CU(cudaEventRecord(ctx->ev_bank_fork, ctx->stream));
     CU(cudaStreamWaitEvent(ctx->bank_stream, ctx->ev_bank_fork, 0));
+    const unsigned base = own.ticket;
+    own.ticket += (unsigned)nchunks;
     auto refill = [&](int c) -> int {
         const int b = c & 1, j0 = c * chunk, cnt = std::min(chunk, nj - j0);
-        if (c >= 2) CU(cudaStreamWaitEvent(ctx->bank_stream, ctx->ev_bank_done[b], 0));   // chunk c - 2 has been swept
+        if (c >= 2) {   // chunk c - 2 has been swept out of this bank
+            if (by_flags) {
+                if (g_wait_value(ctx->bank_stream, (unsigned long long)(own.flags + 2 + b), base + (unsigned)c - 1u, 0u) != 0) return S2_ECUDA;
+            } else {
+                CU(cudaStreamWaitEvent(ctx->bank_stream, ctx->ev_bank_done[b], 0));
+            }
+        }
         if (equal_stride) {   // one strided copy moves the chunk of every plane
             CU(cudaMemcpy2DAsync(bank[b], (size_t)chunk * sizeof(double2), (const double2 *)a.jp[0] + j0, pitch,
                                  (size_t)cnt * sizeof(double2), npl, cudaMemcpyDeviceToDevice, ctx->bank_stream));
@@ -739,9 +782,19 @@ static int run_force_bank(s2_ctx *ctx, ForceArgs &a, int ni, unsigned flags)
                 CU(cudaMemcpyAsync((double2 *)bank[b] + (size_t)p * chunk, (const double2 *)a.jp[p] + j0,
                                    (size_t)cnt * sizeof(double2), cudaMemcpyDeviceToDevice, ctx->bank_stream));
         }
-        CU(cudaEventRecord(ctx->ev_bank_copy[b], ctx->bank_stream));
+        if (by_flags) {
+            if (g_write_value(ctx->bank_stream, (unsigned long long)(own.flags + b), base + (unsigned)c + 1u, 0u) != 0) return S2_ECUDA;
+        } else {
+            CU(cudaEventRecord(ctx->ev_bank_copy[b], ctx->bank_stream));
+        }
         return S2_OK;
     };
+    // launch -1 sweeps nothing: it gathers the i-particles, parks them and zeroes the running state, so that every
+    // chunk launch finds its inputs complete and may overlap its predecessor
+    a.bank_j0 = 0; a.bank_cnt = 0; a.bank_first = 1; a.bank_last = 0; a.bank_pdl = 0; a.bank_wait_early = 0;
+    a.bank_id = 0; a.bank_flags = nullptr; a.bank_ticket = 0;
+    CU(dispatch_bank(0, ctx->order, flags, a, ctx->stream, nullptr));
+    ctx->launches++;
     int rc = refill(0);
     if (rc == S2_OK && nchunks > 1) rc = refill(1);
     if (rc != S2_OK) return rc;
@@ -749,13 +802,18 @@ static int run_force_bank(s2_ctx *ctx, ForceArgs &a, int ni, unsigned flags)
         const int b = c & 1;
         a.bank_j0 = c * chunk;
         a.bank_cnt = std::min(chunk, nj - a.bank_j0);
-        a.bank_first = c == 0;
+        a.bank_first = 0;
         a.bank_last = c == nchunks - 1;
-        CU(cudaStreamWaitEvent(ctx->stream, ctx->ev_bank_copy[b], 0));   // join: chunk c is in its bank
+        a.bank_id = b;
+        a.bank_flags = by_flags ? own.flags : nullptr;
+        a.bank_ticket = base + (unsigned)c + 1u;
+        a.bank_pdl = by_flags && c > 0;
+        a.bank_wait_early = c == 0 || flags != 0;   // decisions (thresholds) are carried from chunk to chunk
+        if (!by_flags) CU(cudaStreamWaitEvent(ctx->stream, ctx->ev_bank_copy[b], 0));   // join: chunk c is in its bank
         CU(dispatch_bank(b, ctx->order, flags, a, ctx->stream, nullptr));
         ctx->launches++;
-        if (c + 2 < nchunks) {
-            CU(cudaEventRecord(ctx->ev_bank_done[b], ctx->stream));
+        if (c + 2 < nchunks) {   // the refill after next goes to the side stream (which paces itself on done[bank])
+            if (!by_flags) CU(cudaEventRecord(ctx->ev_bank_done[b], ctx->stream));
             rc = refill(c + 2);
             if (rc != S2_OK) return rc;
         }

@@ -290,6 +290,22 @@ __global__ void __launch_bounds__(P::kBankThreads, P::kMinBlocksBank) force_swee
     d.i = blockIdx.x * P::kBankThreads + threadIdx.x;
     d.i_valid = d.i < a.ni;
     if (!d.i_valid) d.i = a.ni - 1;   // padding lanes recompute the last i and never write
+    // programmatic dependent launch (chunks >= 1): the next chunk launch may start filling the SMs as soon as every
+    // CTA of this one has started; whatever depends on the previous launch is read behind griddepcontrol.wait
+    asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
+    if (a.bank_wait_early) asm volatile("griddepcontrol.wait;" ::: "memory");
+    if (a.bank_flags) {
+        // this chunk's refill (side stream: wait value, copy, write value) may still be in flight when an early CTA of
+        // an overlapped launch arrives: spin until ready[bank] has reached this chunk's ticket (cyclic compare)
+        if (threadIdx.x == 0) {
+            unsigned r;
+            do {
+                asm volatile("ld.acquire.sys.global.u32 %0, [%1];" : "=r"(r) : "l"(a.bank_flags + a.bank_id) : "memory");
+                if ((int)(r - a.bank_ticket) < 0) __nanosleep(200);
+            } while ((int)(r - a.bank_ticket) < 0);
+        }
+        __syncthreads();
+    }
     const size_t ni = (size_t)a.ni;
     double *st = a.bank_state + d.i;   // SoA: component c of particle i at bank_state[c * ni + i]
     double *ist = st + REC * ni;       // parked i-state behind the REC running components
@@ -329,9 +345,22 @@ __global__ void __launch_bounds__(P::kBankThreads, P::kMinBlocksBank) force_swee
         P::load_j_bank(k, J);
         P::template interact<1, false>(J, true, j0 + k, I, part, D, d, seg, a.segcap);
     }
+    if (a.bank_flags) {
+        // the bank is free for the refill after next once every CTA of this launch is through its loop
+        __syncthreads();
+        if (threadIdx.x == 0) {
+            const unsigned prev = atomicAdd(a.bank_flags + 4 + a.bank_id, 1u);
+            if (prev == gridDim.x - 1) {
+                a.bank_flags[4 + a.bank_id] = 0u;
+                __threadfence_system();
+                asm volatile("st.release.sys.global.u32 [%0], %1;" ::"l"(a.bank_flags + 2 + a.bank_id), "r"(a.bank_ticket) : "memory");
+            }
+        }
+    }
     if (a.bank_first) {
         tot.zero();
     } else {
+        if (!a.bank_wait_early) asm volatile("griddepcontrol.wait;" ::: "memory");   // the previous chunk's totals
         double o[10];
 #pragma unroll
         for (int c = 0; c < NC; ++c) o[c] = st[c * ni];
@@ -367,9 +396,16 @@ template <class P>
 static cudaError_t launch_bank(const ForceArgs &a, cudaStream_t st, int *geom)
 {
     if (geom) { geom[0] = P::kChunk; geom[1] = P::kBankThreads; geom[2] = P::kMinBlocksBank; return cudaSuccess; }
-    const dim3 grid((a.ni + P::kBankThreads - 1) / P::kBankThreads);
-    force_sweep_bank_kernel<P, S2_BANK_ID><<<grid, P::kBankThreads, 0, st>>>(a);
-    return cudaGetLastError();
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3((a.ni + P::kBankThreads - 1) / P::kBankThreads);
+    cfg.blockDim = dim3(P::kBankThreads);
+    cfg.stream = st;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    at[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = at;
+    cfg.numAttrs = a.bank_pdl ? 1 : 0;
+    return cudaLaunchKernelEx(&cfg, force_sweep_bank_kernel<P, S2_BANK_ID>, a);
 }
 
 // geom != nullptr: only report {chunk length of this order's bank layout, threads per CTA, CTAs per SM aimed at}

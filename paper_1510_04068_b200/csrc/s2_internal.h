@@ -107,6 +107,13 @@ struct ForceArgs {
     int bank_j0, bank_cnt;         // address of its first particle, number of particles
     int bank_first, bank_last;     // first chunk: start from zero; last chunk: write final records to rec
     double *bank_state;            // [REC][ni] running sums and decisions between chunk launches (SoA)
+    int bank_id;                   // which of the two constant banks (modules) this launch reads
+    unsigned *bank_flags;          // device words {ready[2], done[2], arrived[2]} of the flag hand-shake with the refill
+                                   // stream, or nullptr when events order the refills (no overlap of launches then)
+    unsigned bank_ticket;          // sequence number of this chunk: ready[bank] >= ticket before the bank is read,
+                                   // done[bank] = ticket once every CTA has swept it
+    int bank_pdl;                  // launch with programmatic stream serialisation (overlaps the previous chunk's tail)
+    int bank_wait_early;           // wait for the previous launch before anything is read (decisions carried, chunk 0)
 };
 
 struct ReduceArgs {
