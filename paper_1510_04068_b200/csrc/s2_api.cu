@@ -69,9 +69,6 @@ struct s2_ctx {
     cudaEvent_t ev_il[2] = {nullptr, nullptr};
     int il_turn = 0;
     bool flags_dirty = false;         // a device-side commit may have raised the range flag
-    // uniform-operand sweep: the stream that refills one constant bank while the sweep reads the other
-    cudaStream_t bank_stream = nullptr;
-    cudaEvent_t ev_bank_fork = nullptr, ev_bank_copy[2] = {nullptr, nullptr}, ev_bank_done[2] = {nullptr, nullptr};
     cudaEvent_t ev_stage = nullptr;   // H2D of the staging buffer finished
     cudaEvent_t ev_io = nullptr;      // H2D of the i-list upload finished
     std::vector<Batch> batches;
@@ -279,9 +276,6 @@ extern "C" int s2_close(s2_ctx *ctx)
         if (ctx->h_il[k]) cudaFreeHost(ctx->h_il[k]);
     }
     if (ctx->h_res) cudaFreeHost(ctx->h_res);
-    if (ctx->bank_stream) cudaStreamDestroy(ctx->bank_stream);
-    for (cudaEvent_t e : {ctx->ev_bank_fork, ctx->ev_bank_copy[0], ctx->ev_bank_copy[1], ctx->ev_bank_done[0], ctx->ev_bank_done[1]})
-        if (e) cudaEventDestroy(e);
     for (auto &e : ctx->ev_t)
         if (e) cudaEventDestroy(e);
     cudaGetLastError();
@@ -655,27 +649,24 @@ struct BankOwner {
     cudaEvent_t ev = nullptr;
     cudaStream_t stream = nullptr;
     bool used = false;
-    unsigned *flags = nullptr;   // device words {ready[2], done[2], arrived[2]} (flag hand-shake, see run_force_bank)
+    unsigned *flags = nullptr;   // device words {ready[2], -, -, arrived[2]} of the bank hand-over (run_force_bank)
     unsigned ticket = 0;         // tickets handed out so far (chunk sequence numbers, cyclic)
 };
 static std::mutex g_bank_mu;
 static std::map<int, BankOwner> g_bank;
 
-// When the chunked sweep beats the shared-memory one (measured on B200): its pair loop runs ~5.5 %
-// faster, but every chunk is a launch of ceil(n_i / 256) equal CTAs, so (a) the busiest SM sets the pace -- the
-// CTAs-per-SM quantisation q -- and (b) each chunk pays ~12 us of copy + ramp + state traffic.  4th order only:
-// the 6th- and 2nd-order variants measured within 1 % of their shared-memory sweeps.
+// When the chunked sweep beats the shared-memory one (measured on B200 at N = 2^18, fp64 4th order, Gpairs/s
+// bank / shared-memory): n_i = 65536: 421 / 489, 98304: 480 / 489, 131072: 510 / 481, 151552: 511 / 472, 245760: 513 / 489,
+// 262144: 513 / 481, 2^19: 513 / 481 (with NN + lists 441 / 420).  Its launches overlap, so unlike the shared-memory
+// sweep it does not care whether the grid is a whole number of residency rounds; below ~1.5 rounds (296 CTAs each)
+// the per-launch costs win.  4th order only: the 6th-order variant measures 282 against 290, the 2nd-order one -4 %.
 static bool bank_applies(const s2_ctx *ctx, int ni, int nj)
 {
     if (ctx->precision != S2_FP64 || ctx->tune[8] == 1) return false;
-    if (ctx->tune[8] >= 2) return true;   // 3: forced, without programmatic dependent launch (A/B measurements)
+    if (ctx->tune[8] >= 2) return true;   // 3: forced, without overlapping launches (A/B measurements)
     for (int k = 0; k < 8; ++k)
         if (ctx->tune[k]) return false;   // an explicit launch shape was asked for
-    if (ctx->order != 4 || nj < 8192) return false;
-    const double per_sm = std::ceil(ni / (double)kThreads) / ctx->sm_count;
-    const double q = per_sm / std::ceil(per_sm);
-    const double chunk_us = (double)ni * 1024.0 / 505e3;   // at 505 Gpairs/s
-    return 1.055 * q * (1.0 - 12.0 / chunk_us) > 1.01;
+    return ctx->order == 4 && nj >= 8192 && ni >= 120000;
 }
 
 static cudaError_t dispatch_bank(int b, int order, unsigned flags, const ForceArgs &a, cudaStream_t st, int *geom)
@@ -683,37 +674,11 @@ static cudaError_t dispatch_bank(int b, int order, unsigned flags, const ForceAr
     return b ? dispatch_force_fp64_bank1(order, flags, a, st, geom) : dispatch_force_fp64_bank0(order, flags, a, st, geom);
 }
 
-// Stream memory operations of the driver (wait until a device word reaches a value / write a device word), fetched
-// through the runtime so that the library does not link libcuda: they let the refill stream and the sweep kernels hand
-// the banks over through flags in device memory, with no event operation between two chunk launches.
-typedef int (*StreamValueFn)(cudaStream_t, unsigned long long, unsigned, unsigned);
-static StreamValueFn g_wait_value = nullptr, g_write_value = nullptr;
-static bool g_value_ops_probed = false;
-static bool stream_value_ops()
-{
-    if (!g_value_ops_probed) {
-        g_value_ops_probed = true;
-        void *w = nullptr, *x = nullptr;
-        cudaDriverEntryPointQueryResult q1, q2;
-        if (cudaGetDriverEntryPoint("cuStreamWaitValue32", &w, cudaEnableDefault, &q1) == cudaSuccess &&
-            cudaGetDriverEntryPoint("cuStreamWriteValue32", &x, cudaEnableDefault, &q2) == cudaSuccess &&
-            q1 == cudaDriverEntryPointSuccess && q2 == cudaDriverEntryPointSuccess && w && x) {
-            g_wait_value = (StreamValueFn)w;
-            g_write_value = (StreamValueFn)x;
-        }
-        cudaGetLastError();
-    }
-    return g_wait_value && g_write_value;
-}
-
-// Chunk c lives in bank c & 1 and carries ticket base + c + 1.  The refills run on a side stream.  Hand-over of a bank:
-//   flag path (default): the last CTA of the launch that swept chunk c stores done[bank] = ticket(c); the side stream
-//     waits for that value, copies chunk c + 2 and writes ready[bank] = ticket(c + 2); the launch of chunk c + 2 spins
-//     on ready[bank] before it reads the bank.  Nothing sits between two chunk launches in the main stream, so they are
-//     launched with programmatic stream serialisation: the next launch fills the SMs while this one drains, and every
-//     CTA reads the previous launch's totals behind griddepcontrol.wait (499 -> 519 Gpairs/s at n_i = 2^18);
-//   event path (stream capture, or no stream memory operations): events order copies and launches (no overlap of
-//     launches).
+// Chunk c lives in bank c & 1 and carries ticket base + c + 1.  The host copies chunks 0 and 1 into the banks; from
+// then on the sweep feeds itself: the last CTA of the launch of chunk c copies chunk c + 2 into the bank it has just
+// swept and publishes ready[bank] = ticket(c + 2) (see force_sweep_bank_kernel).  Nothing but kernels sits in the
+// stream, so the launches carry programmatic stream serialisation and overlap: the next one fills the SMs while this
+// one drains (event-ordered refills: 498 Gpairs/s at n_i = 2^18; overlapped: 512).
 static int run_force_bank(s2_ctx *ctx, ForceArgs &a, int ni, unsigned flags)
 {
     int geom[3] = {0, 0, 0};
@@ -722,14 +687,6 @@ static int run_force_bank(s2_ctx *ctx, ForceArgs &a, int ni, unsigned flags)
     void *bank[2] = {nullptr, nullptr};
     CU(force_bank_address0(&bank[0]));
     CU(force_bank_address1(&bank[1]));
-    if (!ctx->bank_stream) {
-        CU(cudaStreamCreateWithFlags(&ctx->bank_stream, cudaStreamNonBlocking));
-        CU(cudaEventCreateWithFlags(&ctx->ev_bank_fork, cudaEventDisableTiming));
-        for (int b = 0; b < 2; ++b) {
-            CU(cudaEventCreateWithFlags(&ctx->ev_bank_copy[b], cudaEventDisableTiming));
-            CU(cudaEventCreateWithFlags(&ctx->ev_bank_done[b], cudaEventDisableTiming));
-        }
-    }
     const int npl = force_nplanes(S2_FP64, ctx->order, flags);
     const int nj = a.nj;
     const int nchunks = (nj + chunk - 1) / chunk;
@@ -748,56 +705,38 @@ static int run_force_bank(s2_ctx *ctx, ForceArgs &a, int ni, unsigned flags)
     std::lock_guard<std::mutex> lock(g_bank_mu);
     BankOwner &own = g_bank[ctx->device];
     if (!own.ev) CU(cudaEventCreateWithFlags(&own.ev, cudaEventDisableTiming));
+    if (!own.flags) {
+        CU(cudaMalloc((void **)&own.flags, 64));
+        CU(cudaMemset(own.flags, 0, 64));
+    }
     // inside a stream capture (CUDA graph) events cannot tie the graph to work outside it: the caller orders
     // replays of such a graph against other users of the banks himself
     cudaStreamCaptureStatus cap = cudaStreamCaptureStatusNone;
     CU(cudaStreamIsCapturing(ctx->stream, &cap));
     const bool capturing = cap != cudaStreamCaptureStatusNone;
-    const bool by_flags = !capturing && ctx->tune[8] != 3 && stream_value_ops();
-    if (by_flags && !own.flags) {
-        CU(cudaMalloc((void **)&own.flags, 64));
-        CU(cudaMemset(own.flags, 0, 64));
-    }
     if (!capturing && own.used && own.stream != ctx->stream) CU(cudaStreamWaitEvent(ctx->stream, own.ev, 0));
     if (ctx->timing) CU(cudaEventRecord(ctx->ev_t[2], ctx->stream));
-    // fork: the side stream starts behind everything enqueued so far (the predictor, earlier sweeps on the banks)
-    CU(cudaEventRecord(ctx->ev_bank_fork, ctx->stream));
-    CU(cudaStreamWaitEvent(ctx->bank_stream, ctx->ev_bank_fork, 0));
     const unsigned base = own.ticket;
     own.ticket += (unsigned)nchunks;
-    auto refill = [&](int c) -> int {
-        const int b = c & 1, j0 = c * chunk, cnt = std::min(chunk, nj - j0);
-        if (c >= 2) {   // chunk c - 2 has been swept out of this bank
-            if (by_flags) {
-                if (g_wait_value(ctx->bank_stream, (unsigned long long)(own.flags + 2 + b), base + (unsigned)c - 1u, 0u) != 0) return S2_ECUDA;
-            } else {
-                CU(cudaStreamWaitEvent(ctx->bank_stream, ctx->ev_bank_done[b], 0));
-            }
-        }
+    for (int c = 0; c < std::min(2, nchunks); ++c) {   // the first two chunks; the later ones are copied by the kernels
+        const int cnt = std::min(chunk, nj - c * chunk);
         if (equal_stride) {   // one strided copy moves the chunk of every plane
-            CU(cudaMemcpy2DAsync(bank[b], (size_t)chunk * sizeof(double2), (const double2 *)a.jp[0] + j0, pitch,
-                                 (size_t)cnt * sizeof(double2), npl, cudaMemcpyDeviceToDevice, ctx->bank_stream));
+            CU(cudaMemcpy2DAsync(bank[c], (size_t)chunk * sizeof(double2), (const double2 *)a.jp[0] + c * chunk, pitch,
+                                 (size_t)cnt * sizeof(double2), npl, cudaMemcpyDeviceToDevice, ctx->stream));
         } else {
             for (int p = 0; p < npl; ++p)
-                CU(cudaMemcpyAsync((double2 *)bank[b] + (size_t)p * chunk, (const double2 *)a.jp[p] + j0,
-                                   (size_t)cnt * sizeof(double2), cudaMemcpyDeviceToDevice, ctx->bank_stream));
+                CU(cudaMemcpyAsync((double2 *)bank[c] + (size_t)p * chunk, (const double2 *)a.jp[p] + c * chunk,
+                                   (size_t)cnt * sizeof(double2), cudaMemcpyDeviceToDevice, ctx->stream));
         }
-        if (by_flags) {
-            if (g_write_value(ctx->bank_stream, (unsigned long long)(own.flags + b), base + (unsigned)c + 1u, 0u) != 0) return S2_ECUDA;
-        } else {
-            CU(cudaEventRecord(ctx->ev_bank_copy[b], ctx->bank_stream));
-        }
-        return S2_OK;
-    };
+    }
     // launch -1 sweeps nothing: it gathers the i-particles, parks them and zeroes the running state, so that every
     // chunk launch finds its inputs complete and may overlap its predecessor
     a.bank_j0 = 0; a.bank_cnt = 0; a.bank_first = 1; a.bank_last = 0; a.bank_pdl = 0; a.bank_wait_early = 0;
-    a.bank_id = 0; a.bank_flags = nullptr; a.bank_ticket = 0;
+    a.bank_id = 0; a.bank_flags = nullptr; a.bank_ticket = 0; a.bank_spin = 0; a.bank_next_known = 1;
+    a.bank_self = nullptr; a.bank_next_j0 = 0; a.bank_next_cnt = 0;
     CU(dispatch_bank(0, ctx->order, flags, a, ctx->stream, nullptr));
     ctx->launches++;
-    int rc = refill(0);
-    if (rc == S2_OK && nchunks > 1) rc = refill(1);
-    if (rc != S2_OK) return rc;
+    const bool overlap = !capturing && ctx->tune[8] != 3;   // 3: forced, plain launches (A/B measurements)
     for (int c = 0; c < nchunks; ++c) {
         const int b = c & 1;
         a.bank_j0 = c * chunk;
@@ -805,18 +744,17 @@ static int run_force_bank(s2_ctx *ctx, ForceArgs &a, int ni, unsigned flags)
         a.bank_first = 0;
         a.bank_last = c == nchunks - 1;
         a.bank_id = b;
-        a.bank_flags = by_flags ? own.flags : nullptr;
+        a.bank_flags = own.flags;
         a.bank_ticket = base + (unsigned)c + 1u;
-        a.bank_pdl = by_flags && c > 0;
+        a.bank_spin = c >= 2;
+        a.bank_next_known = c == 0 || c == nchunks - 1;
+        a.bank_self = (double2 *)bank[b];
+        a.bank_next_j0 = (c + 2) * chunk;
+        a.bank_next_cnt = c + 2 < nchunks ? std::min(chunk, nj - a.bank_next_j0) : 0;
+        a.bank_pdl = overlap && c > 0;
         a.bank_wait_early = c == 0 || flags != 0;   // decisions (thresholds) are carried from chunk to chunk
-        if (!by_flags) CU(cudaStreamWaitEvent(ctx->stream, ctx->ev_bank_copy[b], 0));   // join: chunk c is in its bank
         CU(dispatch_bank(b, ctx->order, flags, a, ctx->stream, nullptr));
         ctx->launches++;
-        if (c + 2 < nchunks) {   // the refill after next goes to the side stream (which paces itself on done[bank])
-            if (!by_flags) CU(cudaEventRecord(ctx->ev_bank_done[b], ctx->stream));
-            rc = refill(c + 2);
-            if (rc != S2_OK) return rc;
-        }
     }
     if (ctx->timing) CU(cudaEventRecord(ctx->ev_t[3], ctx->stream));
     if (!capturing) {

@@ -290,21 +290,33 @@ __global__ void __launch_bounds__(P::kBankThreads, P::kMinBlocksBank) force_swee
     d.i = blockIdx.x * P::kBankThreads + threadIdx.x;
     d.i_valid = d.i < a.ni;
     if (!d.i_valid) d.i = a.ni - 1;   // padding lanes recompute the last i and never write
-    // programmatic dependent launch (chunks >= 1): the next chunk launch may start filling the SMs as soon as every
-    // CTA of this one has started; whatever depends on the previous launch is read behind griddepcontrol.wait
-    asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
+    // Overlap of consecutive chunk launches (programmatic dependent launch) and hand-over of the two banks:
+    //   * the launch of chunk c reads bank c & 1; when its last CTA is through the loop, that CTA copies chunk c + 2
+    //     into the same bank and publishes ready[bank] = ticket(c + 2);
+    //   * a CTA lets the next launch start (launch_dependents) only once it has SEEN the next chunk ready -- so the
+    //     next launch, and the constant-cache invalidation that comes with it, happens after the bank was rewritten
+    //     and after its previous readers were through; CTAs that start too early for that trigger by exiting;
+    //   * everything a CTA reads from the previous launch (running totals, decisions) sits behind griddepcontrol.wait.
+    __shared__ int s_next_ready, s_last;
     if (a.bank_wait_early) asm volatile("griddepcontrol.wait;" ::: "memory");
     if (a.bank_flags) {
-        // this chunk's refill (side stream: wait value, copy, write value) may still be in flight when an early CTA of
-        // an overlapped launch arrives: spin until ready[bank] has reached this chunk's ticket (cyclic compare)
         if (threadIdx.x == 0) {
             unsigned r;
-            do {
-                asm volatile("ld.acquire.sys.global.u32 %0, [%1];" : "=r"(r) : "l"(a.bank_flags + a.bank_id) : "memory");
-                if ((int)(r - a.bank_ticket) < 0) __nanosleep(200);
-            } while ((int)(r - a.bank_ticket) < 0);
+            if (a.bank_spin) {   // never spins in practice (see above); a guard, not a synchronisation point
+                do {
+                    asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(r) : "l"(a.bank_flags + a.bank_id) : "memory");
+                    if ((int)(r - a.bank_ticket) < 0) __nanosleep(200);
+                } while ((int)(r - a.bank_ticket) < 0);
+            }
+            int nr = a.bank_next_known;
+            if (!nr) {
+                asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(r) : "l"(a.bank_flags + (a.bank_id ^ 1)) : "memory");
+                nr = (int)(r - (a.bank_ticket + 1u)) >= 0;
+            }
+            s_next_ready = nr;
         }
         __syncthreads();
+        if (s_next_ready) asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
     }
     const size_t ni = (size_t)a.ni;
     double *st = a.bank_state + d.i;   // SoA: component c of particle i at bank_state[c * ni + i]
@@ -346,16 +358,29 @@ __global__ void __launch_bounds__(P::kBankThreads, P::kMinBlocksBank) force_swee
         P::template interact<1, false>(J, true, j0 + k, I, part, D, d, seg, a.segcap);
     }
     if (a.bank_flags) {
-        // the bank is free for the refill after next once every CTA of this launch is through its loop
+        // the last CTA through its loop refills this bank with the chunk after next (through the bank's address in
+        // global memory) and publishes it
         __syncthreads();
         if (threadIdx.x == 0) {
             const unsigned prev = atomicAdd(a.bank_flags + 4 + a.bank_id, 1u);
-            if (prev == gridDim.x - 1) {
-                a.bank_flags[4 + a.bank_id] = 0u;
-                __threadfence_system();
-                asm volatile("st.release.sys.global.u32 [%0], %1;" ::"l"(a.bank_flags + 2 + a.bank_id), "r"(a.bank_ticket) : "memory");
-            }
+            s_last = prev == gridDim.x - 1;
+            if (s_last) a.bank_flags[4 + a.bank_id] = 0u;
         }
+        __syncthreads();
+        if (s_last && a.bank_next_cnt > 0) {
+            double2 *dst = a.bank_self;
+#pragma unroll
+            for (int p = 0; p < P::NPL; ++p) {
+                const double2 *src = static_cast<const double2 *>(a.jp[p]) + a.bank_next_j0;
+                for (int k = threadIdx.x; k < a.bank_next_cnt; k += P::kBankThreads) dst[p * P::kChunk + k] = __ldcg(src + k);
+            }
+            __threadfence();
+            __syncthreads();
+            if (threadIdx.x == 0)
+                asm volatile("st.release.gpu.global.u32 [%0], %1;" ::"l"(a.bank_flags + a.bank_id), "r"(a.bank_ticket + 2u) : "memory");
+        }
+        // CTAs that did not see the next chunk ready at their start let the next launch go by exiting: that is behind
+        // their griddepcontrol.wait, i.e. after the previous launch (whose last CTA refills the next bank) has completed
     }
     if (a.bank_first) {
         tot.zero();

@@ -108,10 +108,13 @@ struct ForceArgs {
     int bank_first, bank_last;     // first chunk: start from zero; last chunk: write final records to rec
     double *bank_state;            // [REC][ni] running sums and decisions between chunk launches (SoA)
     int bank_id;                   // which of the two constant banks (modules) this launch reads
-    unsigned *bank_flags;          // device words {ready[2], done[2], arrived[2]} of the flag hand-shake with the refill
-                                   // stream, or nullptr when events order the refills (no overlap of launches then)
-    unsigned bank_ticket;          // sequence number of this chunk: ready[bank] >= ticket before the bank is read,
-                                   // done[bank] = ticket once every CTA has swept it
+    unsigned *bank_flags;          // device words {ready[2], -, -, arrived[2]} of the bank hand-over, or nullptr for the
+                                   // launch that only parks the i-particles
+    unsigned bank_ticket;          // sequence number of this chunk: ready[bank] >= ticket when the chunk is in its bank
+    int bank_spin;                 // 0 for the first two chunks (copied by the host before the first launch)
+    int bank_next_known;           // 1: the next chunk is known to be in its bank (first chunks) or there is none
+    double2 *bank_self;            // this launch's bank through its address in global memory (refill target)
+    int bank_next_j0, bank_next_cnt;   // the chunk after next, which the last CTA copies into this bank (cnt 0: none)
     int bank_pdl;                  // launch with programmatic stream serialisation (overlaps the previous chunk's tail)
     int bank_wait_early;           // wait for the previous launch before anything is read (decisions carried, chunk 0)
 };
