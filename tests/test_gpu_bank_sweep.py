@@ -150,3 +150,35 @@ def test_bank_sweep_reproducible_agrees_with_tiled_and_is_shared_safely():
     assert rel_err(r2["acc"], ref2.acc).max() <= 1e-13 and np.array_equal(r2["nn_id"], ref2.nn_id)
     s2.s2_close(ctx2)
     s2.s2_close(ctx)
+
+
+@pytest.mark.timeout(300)
+def test_bank_sweep_overlapping_launches_at_residency_boundaries():
+    """The chunk launches overlap (programmatic dependent launch) and hand the two banks over through device flags.
+    Grids just below, at and above whole residency rounds (296 CTAs of 256 i on a 148-SM part) and a 1-CTA grid,
+    several sweeps back to back without synchronising: equal to the shared-memory sweep within rounding, bit-identical
+    from call to call, and no launch waits on work that is not resident (the test would hang)."""
+    import torch
+    N = 8192                                      # 8 chunks
+    w = make_config(3, N=N)
+    ctx = open_and_load(w)
+    s2.s2_predict(ctx, w.t_pred, N)
+    rng = np.random.default_rng(12)
+    for ni in (1, 255, 295 * 256, 296 * 256, 297 * 256 + 3, 2 * 296 * 256, 3 * 296 * 256 - 1):
+        il = torch.from_numpy(rng.integers(0, N, ni).astype(np.int32)).cuda()     # i-particles may repeat
+        for flags in (0, NN):
+            s2.s2_set_tuning(ctx, 8, 1)
+            s2.s2_calc_ilist_device(ctx, il, None, w.eps2, flags)
+            ref = s2.s2_get_results(ctx, ni)
+            s2.s2_set_tuning(ctx, 8, 2)
+            for _ in range(3):
+                s2.s2_calc_ilist_device(ctx, il, None, w.eps2, flags)
+            a = s2.s2_get_results(ctx, ni)
+            assert s2.s2_last_launch_info(ctx)["reduced"] == 3
+            s2.s2_calc_ilist_device(ctx, il, None, w.eps2, flags)
+            b = s2.s2_get_results(ctx, ni)
+            for k in ("acc", "jerk", "pot", "nn_id", "nn_r2"):
+                assert np.array_equal(a[k], b[k]), (ni, flags, k)
+            assert rel_err(a["acc"], ref["acc"]).max() < 1e-13 and rel_err(a["jerk"], ref["jerk"]).max() < 1e-12
+            assert np.array_equal(a["nn_id"], ref["nn_id"])
+    s2.s2_close(ctx)
