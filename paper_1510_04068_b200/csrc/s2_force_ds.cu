@@ -119,6 +119,7 @@ struct PolicyDS {
     static constexpr int kMinBlocks = 2;
     static constexpr int kUnroll = 1;
     static constexpr int kIPT = kIptDS;          // no register tiling: a double-single pair is ~400 FP32 instructions
+    static constexpr bool kPacked2 = false;
 
     struct IState {
         ds x, y, z, vx, vy, vz, ax, ay, az, eps2;

@@ -21,6 +21,46 @@ __device__ __forceinline__ float rsqrt_f32(float s)
     return y;
 }
 
+// Packed fp32 pairs (sm_100a: FADD2 / FMUL2 / FFMA2, PTX add/mul/fma.rn.f32x2): one issue slot carries the same IEEE
+// operation for two i-particles of a thread.  The FP32 pipe does not get wider (a packed instruction occupies it for
+// two cycles), but the sweep is ISSUE-bound (33 FP32 + ~6 other slots per pair, FP32 pipe width = issue width), so
+// halving the FP32 issue slots frees the scheduler for the loads, MUFU and selects.  Each element is rounded exactly
+// like the scalar instruction, so the results keep the bits of the scalar sweeps.  A scalar operand that is the same
+// for both halves (the j-particle) is written as a (v, v) pack, which ptxas turns into a broadcast operand (R.F32).
+typedef unsigned long long f32x2;
+__device__ __forceinline__ f32x2 pk2(float lo, float hi)
+{
+    f32x2 r;
+    asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(lo), "f"(hi));
+    return r;
+}
+__device__ __forceinline__ void upk2(f32x2 v, float &lo, float &hi) { asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(v)); }
+__device__ __forceinline__ f32x2 bc2(float v) { return pk2(v, v); }
+__device__ __forceinline__ f32x2 add2(f32x2 a, f32x2 b)
+{
+    f32x2 d;
+    asm("add.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b));
+    return d;
+}
+__device__ __forceinline__ f32x2 sub2(f32x2 a, f32x2 b)
+{
+    f32x2 d;
+    asm("sub.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b));
+    return d;
+}
+__device__ __forceinline__ f32x2 mul2(f32x2 a, f32x2 b)
+{
+    f32x2 d;
+    asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b));
+    return d;
+}
+__device__ __forceinline__ f32x2 fma2(f32x2 a, f32x2 b, f32x2 c)
+{
+    f32x2 d;
+    asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(d) : "l"(a), "l"(b), "l"(c));
+    return d;
+}
+
 template <int ORDER_, bool NN_, bool NGB_>
 struct PolicyF32 {
     static constexpr int ORDER = ORDER_;
@@ -183,6 +223,81 @@ struct PolicyF32 {
             const float uy = fmaf(a6, ty, fmaf(b3, dy, day));
             const float uz = fmaf(a6, tz, fmaf(b3, dz, daz));
             A.sx = fmaf(q, ux, A.sx); A.sy = fmaf(q, uy, A.sy); A.sz = fmaf(q, uz, A.sz);
+        }
+    }
+
+    // Two i-particles of one thread against the same j, every FP32 operation packed (see f32x2 above).  Same
+    // operations in the same order as interact<1, false> for each half.
+    static constexpr bool kPacked2 = true;
+    static __device__ __forceinline__ void interact2(const JData &J, int jaddr, const IState (&I)[2], Part (&A)[2],
+                                                     Dec (&D)[2], const Decomp (&d)[2], int *(&seg)[2], int segcap)
+    {
+        const float4 f0 = J.f0, f1 = J.f1, f2 = J.f2;
+        const int jid = __float_as_int(f1.w);
+        const bool skip0 = jid == I[0].id, skip1 = jid == I[1].id;
+
+        const f32x2 dx = add2(sub2(bc2(f0.x), pk2(I[0].xh, I[1].xh)), sub2(bc2(f1.x), pk2(I[0].xl, I[1].xl)));
+        const f32x2 dy = add2(sub2(bc2(f0.y), pk2(I[0].yh, I[1].yh)), sub2(bc2(f1.y), pk2(I[0].yl, I[1].yl)));
+        const f32x2 dz = add2(sub2(bc2(f0.z), pk2(I[0].zh, I[1].zh)), sub2(bc2(f1.z), pk2(I[0].zl, I[1].zl)));
+        f32x2 s;
+        if (DEC) {
+            const f32x2 d2f = fma2(dz, dz, fma2(dy, dy, mul2(dx, dx)));
+            s = add2(d2f, bc2(I[0].eps2));
+            float e0, e1;
+            upk2(d2f, e0, e1);
+            if (e0 < D[0].thrf || e1 < D[1].thrf) {
+                const double2 p0 = J.p0, p1 = J.p1;
+#pragma unroll
+                for (int u = 0; u < 2; ++u) {
+                    if ((u ? e1 : e0) < D[u].thrf) {
+                        const double ex = p0.x - I[u].x, ey = p0.y - I[u].y, ez = p1.x - I[u].z;
+                        const double d2 = __fma_rn(ez, ez, __fma_rn(ey, ey, __dmul_rn(ex, ex)));
+                        decide<1, NN, NGB>(d2, jaddr, u ? skip1 : skip0, I[u].h2, D[u], d[u], seg[u], segcap);
+                    }
+                }
+            }
+        } else {
+            s = fma2(dz, dz, fma2(dy, dy, fma2(dx, dx, bc2(I[0].eps2))));
+        }
+        float s0, s1;
+        upk2(s, s0, s1);
+        float y0 = rsqrt_f32(s0), y1 = rsqrt_f32(s1);
+        y0 = skip0 ? 0.f : y0;
+        y1 = skip1 ? 0.f : y1;
+        const f32x2 y = pk2(y0, y1);
+        const f32x2 y2 = mul2(y, y);
+        const f32x2 my = mul2(bc2(f0.w), y);
+        const f32x2 q = mul2(my, y2);
+        f32x2 apot = pk2(A[0].pot, A[1].pot), aax = pk2(A[0].ax, A[1].ax), aay = pk2(A[0].ay, A[1].ay), aaz = pk2(A[0].az, A[1].az);
+        apot = sub2(apot, my);
+        aax = fma2(q, dx, aax); aay = fma2(q, dy, aay); aaz = fma2(q, dz, aaz);
+        upk2(apot, A[0].pot, A[1].pot);
+        upk2(aax, A[0].ax, A[1].ax); upk2(aay, A[0].ay, A[1].ay); upk2(aaz, A[0].az, A[1].az);
+        if (ORDER == 2) return;
+        const f32x2 dvx = sub2(bc2(f2.x), pk2(I[0].vx, I[1].vx));
+        const f32x2 dvy = sub2(bc2(f2.y), pk2(I[0].vy, I[1].vy));
+        const f32x2 dvz = sub2(bc2(f2.z), pk2(I[0].vz, I[1].vz));
+        const f32x2 rv = fma2(dz, dvz, fma2(dy, dvy, mul2(dx, dvx)));
+        const f32x2 alpha = mul2(rv, y2);
+        const f32x2 a3 = mul2(bc2(-3.f), alpha);
+        const f32x2 tx = fma2(a3, dx, dvx), ty = fma2(a3, dy, dvy), tz = fma2(a3, dz, dvz);
+        f32x2 ajx = pk2(A[0].jx, A[1].jx), ajy = pk2(A[0].jy, A[1].jy), ajz = pk2(A[0].jz, A[1].jz);
+        ajx = fma2(q, tx, ajx); ajy = fma2(q, ty, ajy); ajz = fma2(q, tz, ajz);
+        upk2(ajx, A[0].jx, A[1].jx); upk2(ajy, A[0].jy, A[1].jy); upk2(ajz, A[0].jz, A[1].jz);
+        if (ORDER == 6) {
+            const float4 f3 = J.f3;
+            const f32x2 dax = sub2(bc2(f3.x), pk2(I[0].ax, I[1].ax));
+            const f32x2 day = sub2(bc2(f3.y), pk2(I[0].ay, I[1].ay));
+            const f32x2 daz = sub2(bc2(f3.z), pk2(I[0].az, I[1].az));
+            const f32x2 w = fma2(dvx, dvx, fma2(dvy, dvy, fma2(dvz, dvz, fma2(dx, dax, fma2(dy, day, mul2(dz, daz))))));
+            const f32x2 b3 = mul2(bc2(-3.f), fma2(w, y2, mul2(alpha, alpha)));
+            const f32x2 a6 = add2(a3, a3);
+            const f32x2 ux = fma2(a6, tx, fma2(b3, dx, dax));
+            const f32x2 uy = fma2(a6, ty, fma2(b3, dy, day));
+            const f32x2 uz = fma2(a6, tz, fma2(b3, dz, daz));
+            f32x2 asx = pk2(A[0].sx, A[1].sx), asy = pk2(A[0].sy, A[1].sy), asz = pk2(A[0].sz, A[1].sz);
+            asx = fma2(q, ux, asx); asy = fma2(q, uy, asy); asz = fma2(q, uz, asz);
+            upk2(asx, A[0].sx, A[1].sx); upk2(asy, A[0].sy, A[1].sy); upk2(asz, A[0].sz, A[1].sz);
         }
     }
 };

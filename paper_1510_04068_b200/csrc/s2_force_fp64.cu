@@ -81,6 +81,7 @@ struct PolicyF64 {
 #endif
     static constexpr int kMinBlocksTiled = ORDER == 6 ? S2_F64_MINBLOCKS_TILED6 : S2_F64_MINBLOCKS_TILED;
     static constexpr int kIPT = kIptF64;                        // i-particles per thread in the register-tiled sweep
+    static constexpr bool kPacked2 = false;
     // j per unrolled step there (x kIPT pairs in flight).  The 6th-order pair holds 18 more live doubles: with
     // 128 registers the totals spill inside the loop, so that variant runs one CTA per SM with 208 registers
     // (measured 290 vs 277 Gpairs/s)

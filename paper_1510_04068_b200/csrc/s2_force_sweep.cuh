@@ -487,9 +487,13 @@ __global__ void __launch_bounds__(kThreads, P::kMinBlocksTiled) force_sweep_tile
         for (int k = 0; k < cnt; ++k) {
             typename P::JData J;
             P::load_j(stage, tile, k, J);
+            if constexpr (IPT == 2 && P::kPacked2) {
+                P::interact2(J, jt + k, I, part, D, d, seg, a.segcap);
+            } else {
 #pragma unroll
-            for (int u = 0; u < IPT; ++u)
-                P::template interact<1, false>(J, true, jt + k, I[u], part[u], D[u], d[u], seg[u], a.segcap);
+                for (int u = 0; u < IPT; ++u)
+                    P::template interact<1, false>(J, true, jt + k, I[u], part[u], D[u], d[u], seg[u], a.segcap);
+            }
         }
 #pragma unroll
         for (int u = 0; u < IPT; ++u) tot[u].add(part[u]);
