@@ -72,7 +72,7 @@ struct PolicyF32 {
     static constexpr int kUnroll = 4;
     static constexpr int kIPT = kIptF32;          // i-particles per thread in the register-tiled sweep
 #ifndef S2_F32_UNROLL_TILED
-#define S2_F32_UNROLL_TILED 2
+#define S2_F32_UNROLL_TILED 4
 #endif
 #ifndef S2_F32_MINBLOCKS_TILED
 #define S2_F32_MINBLOCKS_TILED 2
@@ -229,8 +229,8 @@ struct PolicyF32 {
     // Two i-particles of one thread against the same j, every FP32 operation packed (see f32x2 above).  Same
     // operations in the same order as interact<1, false> for each half.
     static constexpr bool kPacked2 = true;
-    static __device__ __forceinline__ void interact2(const JData &J, int jaddr, const IState (&I)[2], Part (&A)[2],
-                                                     Dec (&D)[2], const Decomp (&d)[2], int *(&seg)[2], int segcap)
+    static __device__ __forceinline__ void interact2(const JData &J, int jaddr, const IState *I, Part *A, Dec *D,
+                                                     const Decomp *d, int *const *seg, int segcap)
     {
         const float4 f0 = J.f0, f1 = J.f1, f2 = J.f2;
         const int jid = __float_as_int(f1.w);

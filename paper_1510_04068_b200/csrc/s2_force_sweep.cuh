@@ -487,8 +487,10 @@ __global__ void __launch_bounds__(kThreads, P::kMinBlocksTiled) force_sweep_tile
         for (int k = 0; k < cnt; ++k) {
             typename P::JData J;
             P::load_j(stage, tile, k, J);
-            if constexpr (IPT == 2 && P::kPacked2) {
-                P::interact2(J, jt + k, I, part, D, d, seg, a.segcap);
+            if constexpr (IPT % 2 == 0 && P::kPacked2) {   // i-particles two by two in packed instructions
+#pragma unroll
+                for (int u = 0; u < IPT; u += 2)
+                    P::interact2(J, jt + k, I + u, part + u, D + u, d + u, seg + u, a.segcap);
             } else {
 #pragma unroll
                 for (int u = 0; u < IPT; ++u)

@@ -292,3 +292,38 @@ def test_largest_store_small_ilist_sampled():
     r1 = s2.s2_get_results(ctx, 1)
     assert rel_err(r1["acc"], ref.acc[:1]).max() <= 1e-13 and rel_err(r1["jerk"], ref.jerk[:1]).max() <= 1e-12
     s2.s2_close(ctx)
+
+
+@pytest.mark.parametrize("order", [2, 4, 6])
+@pytest.mark.parametrize("flags", [0, NN | NGB])
+def test_fp32_packed_tiled_sweep_has_the_bits_of_the_scalar_sweep(order, flags):
+    """The register-tiled fp32 sweep evaluates the two i-particles of a thread in packed FP32 instructions
+    (FADD2 / FMUL2 / FFMA2); every half is rounded like the scalar instruction, so with the same slices and tiles
+    it must return exactly the bits of the one-lane-per-i scalar sweep -- and both must match the oracle."""
+    w = make_config(4 if order == 6 else 5, N=3000, order=max(order, 4))
+    if order == 2:
+        ctx = s2.s2_open(0, 2, s2.S2_FP32, nj_capacity=w.N, ngb_cap=24)
+        s2.s2_set_j(ctx, np.arange(w.N, dtype=np.int32), w.ident, w.t_j, w.mass, w.pos, w.vel)
+        s2.s2_commit_j(ctx)
+    else:
+        ctx = open_and_load(w, order, precision=s2.S2_FP32, ngb_cap=24)
+    s2.s2_predict(ctx, w.t_pred, w.N)
+    ni = 700                                              # two CTAs of 2 x 256 i-slots, ragged second one
+    il = w.ilist(ni)
+    h2 = w.h2[il] * 0.6 if flags & NGB else None
+    keys = ("acc", "pot") + (("jerk",) if order >= 4 else ()) + (("snap",) if order == 6 else ())
+    keys += ("nn_id", "nn_r2", "ngb_count") if flags else ()
+    for S, tile in ((1, 0), (3, 64), (7, 256)):
+        got = {}
+        for tiled in (1, 2):
+            s2.s2_set_tuning(ctx, 1, 1); s2.s2_set_tuning(ctx, 2, 1); s2.s2_set_tuning(ctx, 0, S)
+            s2.s2_set_tuning(ctx, 4, tile); s2.s2_set_tuning(ctx, 7, tiled)
+            s2.s2_calc_ilist(ctx, il, h2, w.eps2, flags)
+            got[tiled] = s2.s2_get_results(ctx, ni)
+            assert s2.s2_last_launch_info(ctx)["i_per_thread"] == tiled
+        for k in keys:
+            assert np.array_equal(got[1][k], got[2][k]), (order, flags, S, tile, k)
+    if order >= 4:
+        ref, _ = oracle_on_gpu_prediction(ctx, w, order, il, w.eps2, h2, ngb_cap=24)
+        check_forces(got[2], ref, s2.S2_FP32, order, flags, f"fp32 packed order {order}")
+    s2.s2_close(ctx)
