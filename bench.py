@@ -295,6 +295,20 @@ def main():
                     "ms_per_step": e2e_ms / args.steps},
             "gpu_launches": int(launches), "roofline": roofline, "launch": s2.s2_last_launch_info(ctx)}
 
+    if rank == 0 and world == 1 and args.precision == "fp32":
+        # FP32 pipe, measured in the same process: scalar FFMA and the packed forms the tiled sweep issues
+        nominal32 = SM_COUNT * 128 * SM_MAX_HZ
+        ffma = s2.s2_peak_fma(ctx, 1, 4000)
+        roofline["measured_ffma_tflops"] = 2 * ffma / 1e12
+        roofline["fp32_lane_ops_per_pair"] = 33
+        roofline["fp32_pipe_frac_nominal"] = ni * N * 33 / (force_ms * 1e-3) / nominal32
+        roofline["fp32_pipe_model"] = {
+            "ffma_const_operands": ffma / nominal32,
+            "ffma2_const_operands": s2.s2_peak_fma(ctx, 5, 4000) / nominal32,
+            "ffma2_three_distinct_register_pairs": s2.s2_peak_fma(ctx, 6, 4000) / nominal32,
+            "ffma2_broadcast_operand": s2.s2_peak_fma(ctx, 7, 4000) / nominal32,
+            "fadd2_two_register_pairs": s2.s2_peak_fma(ctx, 8, 4000) / nominal32,
+            "unit": "fraction of 148 SM x 128 lanes x 1.965 GHz lane-operations/s"}
     if rank == 0 and world == 1 and not args.no_sweep and fp64_path:
         # measured FMA peaks in the same process (SURVEY sec 8(d) "clock risk")
         dfma = s2.s2_peak_fma(ctx, 0, 4000)

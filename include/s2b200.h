@@ -202,6 +202,9 @@ int s2_get_timing(s2_ctx *ctx, float *predict_ms, float *force_ms, float *reduce
  *   kind 0 = DFMA with constant operands (nominal fp64 rate)      1 = FFMA (fp32)
  *   kind 2 = DFMA with three distinct 64-bit register operands    3 = DFMA with one operand shared by
  *   consecutive instructions (operand-reuse cache)                 4 = DADD with two distinct register operands
+ *   kind 5-8 = packed FP32 (two lane-operations per instruction, both counted): 5 = FFMA2 with constant operands,
+ *   6 = FFMA2 with three distinct register pairs, 7 = FFMA2 with a 32-bit register broadcast to both halves,
+ *   8 = FADD2 with two distinct register pairs
  * Returns achieved lane-instructions per second in *fma_per_s.  SYNC. */
 int s2_peak_fma(s2_ctx *ctx, int kind, int iters, double *fma_per_s);
 

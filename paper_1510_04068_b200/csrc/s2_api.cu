@@ -1291,7 +1291,7 @@ extern "C" int s2_get_timing(s2_ctx *ctx, float *predict_ms, float *force_ms, fl
 
 extern "C" int s2_peak_fma(s2_ctx *ctx, int kind, int iters, double *fma_per_s)
 {
-    if (!ctx || !fma_per_s || iters <= 0 || kind < 0 || kind > 4) return S2_EINVAL;
+    if (!ctx || !fma_per_s || iters <= 0 || kind < 0 || kind > 8) return S2_EINVAL;
     CU(cudaSetDevice(ctx->device));
     CU(run_peak_fma(kind, iters, ctx->sm_count, ctx->stream, fma_per_s));
     ctx->launches += 2;

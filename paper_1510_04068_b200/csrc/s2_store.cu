@@ -154,6 +154,61 @@ __global__ void __launch_bounds__(256) peak_fma_kernel(T *out, int iters, T seed
     if (s == (T)123456.789) out[blockIdx.x * blockDim.x + threadIdx.x] = s;   // never true; keeps the chains live
 }
 
+// Packed FP32 (FFMA2 / FADD2, PTX fma/add.rn.f32x2): the same 8 chains per thread, each a register PAIR, so one
+// instruction carries two lane-operations; *fma_per_s counts lane-operations (2 per lane and instruction).
+//   kind 5  FFMA2  a = fma2(a, c1, c2), constants                       (packed rate with free operands)
+//   kind 6  FFMA2  a_k = fma2(b_k, b_k+1, a_k): three distinct register pairs
+//   kind 7  FFMA2  a_k = fma2(q, b_k, a_k), q a 32-bit register broadcast to both halves (the j operand of the sweep)
+//   kind 8  FADD2  a_k = a_k + b_k: two distinct register pairs
+typedef unsigned long long pk_f32x2;
+__device__ __forceinline__ pk_f32x2 pk_make(float lo, float hi)
+{
+    pk_f32x2 r;
+    asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(lo), "f"(hi));
+    return r;
+}
+__device__ __forceinline__ pk_f32x2 pk_fma(pk_f32x2 a, pk_f32x2 b, pk_f32x2 c)
+{
+    pk_f32x2 d;
+    asm volatile("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(d) : "l"(a), "l"(b), "l"(c));
+    return d;
+}
+__device__ __forceinline__ pk_f32x2 pk_add(pk_f32x2 a, pk_f32x2 b)
+{
+    pk_f32x2 d;
+    asm volatile("add.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b));
+    return d;
+}
+template <int MODE>
+__global__ void __launch_bounds__(256) peak_fma2_kernel(float *out, int iters, float seed)
+{
+    pk_f32x2 a[8], b[8];
+    const float qs = 0.999999f + seed * 1e-9f;
+    const pk_f32x2 q = pk_make(qs, qs);
+    const pk_f32x2 c1 = pk_make(0.999999f, 0.999999f), c2 = pk_make(1e-7f, 1e-7f);
+#pragma unroll
+    for (int k = 0; k < 8; ++k) {
+        a[k] = pk_make(seed + (float)(threadIdx.x + k), seed + (float)(threadIdx.x + k + 8));
+        b[k] = pk_make(1.0f + 1e-7f * (float)(threadIdx.x + k) * seed, 1.0f + 1e-7f * (float)(threadIdx.x + k + 8) * seed);
+    }
+    for (int i = 0; i < iters; ++i) {
+#pragma unroll
+        for (int u = 0; u < 16; ++u) {
+#pragma unroll
+            for (int k = 0; k < 8; ++k) {
+                if (MODE == 5) a[k] = pk_fma(a[k], c1, c2);
+                if (MODE == 6) a[k] = pk_fma(b[k], b[(k + 1) & 7], a[k]);
+                if (MODE == 7) a[k] = pk_fma(q, b[k], a[k]);
+                if (MODE == 8) a[k] = pk_add(a[k], b[k]);
+            }
+        }
+    }
+    pk_f32x2 s = 0;
+#pragma unroll
+    for (int k = 0; k < 8; ++k) s ^= a[k] ^ b[k];
+    if (s == 0x123456789abcdefull) out[blockIdx.x * blockDim.x + threadIdx.x] = 1.f;   // never true; keeps the chains live
+}
+
 cudaError_t run_peak_fma(int kind, int iters, int sm_count, cudaStream_t st, double *fma_per_s)
 {
     cudaEvent_t e0, e1;
@@ -169,6 +224,10 @@ cudaError_t run_peak_fma(int kind, int iters, int sm_count, cudaStream_t st, dou
         case 1: peak_fma_kernel<float, 0><<<grid, block, 0, st>>>((float *)dummy, iters, 1.0f); break;
         case 2: peak_fma_kernel<double, 2><<<grid, block, 0, st>>>((double *)dummy, iters, 1.0); break;
         case 3: peak_fma_kernel<double, 3><<<grid, block, 0, st>>>((double *)dummy, iters, 1.0); break;
+        case 5: peak_fma2_kernel<5><<<grid, block, 0, st>>>((float *)dummy, iters, 1.0f); break;
+        case 6: peak_fma2_kernel<6><<<grid, block, 0, st>>>((float *)dummy, iters, 1.0f); break;
+        case 7: peak_fma2_kernel<7><<<grid, block, 0, st>>>((float *)dummy, iters, 1.0f); break;
+        case 8: peak_fma2_kernel<8><<<grid, block, 0, st>>>((float *)dummy, iters, 1.0f); break;
         default: peak_fma_kernel<double, 4><<<grid, block, 0, st>>>((double *)dummy, iters, 1.0); break;
         }
     }
@@ -180,7 +239,7 @@ cudaError_t run_peak_fma(int kind, int iters, int sm_count, cudaStream_t st, dou
     cudaEventDestroy(e0);
     cudaEventDestroy(e1);
     if (err != cudaSuccess) return err;
-    const double fmas = (double)grid * block * (double)iters * 16.0 * 8.0;
+    const double fmas = (double)grid * block * (double)iters * 16.0 * 8.0 * (kind >= 5 && kind <= 8 ? 2.0 : 1.0);
     *fma_per_s = fmas / (ms * 1e-3);
     return cudaSuccess;
 }
