@@ -656,17 +656,19 @@ static std::mutex g_bank_mu;
 static std::map<int, BankOwner> g_bank;
 
 // When the chunked sweep beats the shared-memory one (measured on B200 at N = 2^18, fp64 4th order, Gpairs/s
-// bank / shared-memory): n_i = 65536: 421 / 489, 98304: 480 / 489, 131072: 510 / 481, 151552: 511 / 472, 245760: 513 / 489,
-// 262144: 513 / 481, 2^19: 513 / 481 (with NN + lists 441 / 420).  Its launches overlap, so unlike the shared-memory
-// sweep it does not care whether the grid is a whole number of residency rounds; below ~1.5 rounds (296 CTAs each)
-// the per-launch costs win.  4th order only: the 6th-order variant measures 282 against 290, the 2nd-order one -4 %.
+// bank / shared-memory): n_i = 49152: 481 / 488, 57344: 492 / 487, 61440: 502 / 489, 65536: 506 / 489, 81920: 510 / 489,
+// 114688: 513 / 478, 131072: 517 / 482, 262144: 518 / 482 (with NN + lists 441 / 420).  Its launches overlap and a
+// launch moves into the CTA slots its predecessor leaves free (the CTAs look for the next chunk's ticket at their
+// start and 15 more times on their way through the chunk), so unlike the shared-memory sweep it does not care whether
+// the grid is a whole number of residency rounds; below ~0.8 rounds (296 CTAs each) the per-launch costs win.
+// 4th order only: the 6th-order variant measures 282 against 290, the 2nd-order one -4 %.
 static bool bank_applies(const s2_ctx *ctx, int ni, int nj)
 {
     if (ctx->precision != S2_FP64 || ctx->tune[8] == 1) return false;
     if (ctx->tune[8] >= 2) return true;   // 3: forced, without overlapping launches (A/B measurements)
     for (int k = 0; k < 8; ++k)
         if (ctx->tune[k]) return false;   // an explicit launch shape was asked for
-    return ctx->order == 4 && nj >= 8192 && ni >= 120000;
+    return ctx->order == 4 && nj >= 8192 && ni >= 60000;
 }
 
 static cudaError_t dispatch_bank(int b, int order, unsigned flags, const ForceArgs &a, cudaStream_t st, int *geom)

@@ -281,6 +281,12 @@ cudaError_t dispatch_force_fp64(int order, unsigned flags, int L, dim3 grid, siz
 // each and every barrier: warps are fully independent, one i-particle per lane, eight pairs in
 // flight per thread.  The price is one launch per chunk (1024 j at 4th order), with the running sums carried
 // through an SoA state buffer; sums are added in address order chunk by chunk, so results are bit-reproducible.
+#ifndef S2_BANK_LOOKS
+#define S2_BANK_LOOKS 15
+#endif
+constexpr int kBankLooks = S2_BANK_LOOKS;   // later looks at the next chunk's ticket inside a chunk (0: only at the start);
+                                            // measured at n_i = 65536 / 81920 / 2^18: 0: 421 / 480 / 513, 3: 494 / - / 518, 7: 501 / 503 / 518,
+                                            // 15: 506 / 510 / 518, 31: 507 / 511 / 518, 63: 501 / 504 / 512 Gpairs/s
 template <class P, int BANK>   // BANK only makes the kernels of the two translation units distinct symbols
 __global__ void __launch_bounds__(P::kBankThreads, P::kMinBlocksBank) force_sweep_bank_kernel(const ForceArgs a)
 {
@@ -352,8 +358,24 @@ __global__ void __launch_bounds__(P::kBankThreads, P::kMinBlocksBank) force_swee
     int *seg = P::NGB ? a.seg + (size_t)d.i * a.segcap : nullptr;
 
     const int cnt = a.bank_cnt, j0 = a.bank_j0;
+    // A CTA that started before the next chunk was published (every CTA of a launch of one residency round or less:
+    // they start while the last CTA of the previous launch is still refilling) looks again a few times on its way
+    // through the chunk -- warp by warp, no barrier -- so that the next launch can move into the free CTA slots
+    // instead of waiting for this CTA to exit.  Same condition as at the start, only observed later.
+    // (a launch that waits for its predecessor right at its start gains nothing from being launched earlier)
+    bool trig = a.bank_flags == nullptr || a.bank_wait_early || __ballot_sync(0xffffffffu, s_next_ready != 0) != 0u;   // warp-uniform
+    constexpr int kLooks = (P::NN || P::NGB) ? 0 : kBankLooks;   // decision launches wait at their start: no looks compiled in
+    constexpr int kLookEvery = P::kChunk / (kLooks + 1) / 8 * 8;
 #pragma unroll P::kUnrollBank
     for (int k = 0; k < cnt; ++k) {
+        if (kLooks > 0 && k > 0 && k % kLookEvery == 0 && !trig) {
+            unsigned r;
+            asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(r) : "l"(a.bank_flags + (a.bank_id ^ 1)) : "memory");
+            if (__ballot_sync(0xffffffffu, (int)(r - (a.bank_ticket + 1u)) >= 0) != 0u) {
+                trig = true;
+                asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
+            }
+        }
         typename P::JData J;
         P::load_j_bank(k, J);
         P::template interact<1, false>(J, true, j0 + k, I, part, D, d, seg, a.segcap);
