@@ -164,7 +164,9 @@ def test_bank_sweep_overlapping_launches_at_residency_boundaries():
     ctx = open_and_load(w)
     s2.s2_predict(ctx, w.t_pred, N)
     rng = np.random.default_rng(12)
-    for ni in (1, 255, 295 * 256, 296 * 256, 297 * 256 + 3, 2 * 296 * 256, 3 * 296 * 256 - 1):
+    # 100 and 256 CTAs: launches of less than one round, whose CTAs find the next ticket only by looking again inside
+    # the chunk, and whose successors then share the round with them
+    for ni in (1, 255, 100 * 256 + 17, 256 * 256, 295 * 256, 296 * 256, 297 * 256 + 3, 2 * 296 * 256, 3 * 296 * 256 - 1):
         il = torch.from_numpy(rng.integers(0, N, ni).astype(np.int32)).cuda()     # i-particles may repeat
         for flags in (0, NN):
             s2.s2_set_tuning(ctx, 8, 1)
