@@ -660,7 +660,8 @@ static std::map<int, BankOwner> g_bank;
 // 114688: 513 / 478, 131072: 517 / 482, 262144: 518 / 482 (with NN + lists 441 / 420).  Its launches overlap and a
 // launch moves into the CTA slots its predecessor leaves free (the CTAs look for the next chunk's ticket at their
 // start and 15 more times on their way through the chunk), so unlike the shared-memory sweep it does not care whether
-// the grid is a whole number of residency rounds; below ~0.8 rounds (296 CTAs each) the per-launch costs win.
+// the grid is a whole number of residency rounds; below ~0.6 rounds (296 CTAs of 256 threads each) the per-launch
+// costs win (n_i = 40960: 452 / 488 with 128-thread CTAs, 49152: 502 / 488).
 // 4th order only: the 6th-order variant measures 282 against 290, the 2nd-order one -4 %.
 static bool bank_applies(const s2_ctx *ctx, int ni, int nj)
 {
@@ -668,7 +669,7 @@ static bool bank_applies(const s2_ctx *ctx, int ni, int nj)
     if (ctx->tune[8] >= 2) return true;   // 3: forced, without overlapping launches (A/B measurements)
     for (int k = 0; k < 8; ++k)
         if (ctx->tune[k]) return false;   // an explicit launch shape was asked for
-    return ctx->order == 4 && nj >= 8192 && ni >= 60000;
+    return ctx->order == 4 && nj >= 8192 && ni >= 48000;
 }
 
 static cudaError_t dispatch_bank(int b, int order, unsigned flags, const ForceArgs &a, cudaStream_t st, int *geom)
@@ -692,6 +693,11 @@ static int run_force_bank(s2_ctx *ctx, ForceArgs &a, int ni, unsigned flags)
     const int npl = force_nplanes(S2_FP64, ctx->order, flags);
     const int nj = a.nj;
     const int nchunks = (nj + chunk - 1) / chunk;
+    // CTAs of 128 threads (4 per SM) fill the rounds that consecutive launches share more finely; measured at N = 2^18
+    // (128 / 256 threads, Gpairs/s): n_i = 49152: 502 / 481, 65536: 512 / 506, 81920: 514 / 510, 131072: 518 / 517,
+    // 262144: 516 / 518.  Launches with decisions do not share rounds (they wait at their start): 256.
+    const int threads = (flags == 0 && ctx->order == 4 && ni < 200000 && ctx->tune[8] != 3) ? 128 : geom[1];
+    a.bank_threads = threads;
     a.bank_state = (double *)ctx->part.p;
     a.is_final = 1;
     a.rec = (double *)ctx->result.p;
@@ -766,8 +772,8 @@ static int run_force_bank(s2_ctx *ctx, ForceArgs &a, int ni, unsigned flags)
     }
 
     int *li = ctx->last_info;
-    li[0] = nchunks; li[1] = 1; li[2] = 1; li[3] = (ni + geom[1] - 1) / geom[1]; li[4] = geom[1]; li[5] = 0; li[6] = 3;
-    li[7] = geom[2]; li[8] = 1; li[9] = 1;
+    li[0] = nchunks; li[1] = 1; li[2] = 1; li[3] = (ni + threads - 1) / threads; li[4] = threads; li[5] = 0; li[6] = 3;
+    li[7] = geom[2] * geom[1] / threads; li[8] = 1; li[9] = 1;
     return S2_OK;
 }
 

@@ -287,14 +287,14 @@ cudaError_t dispatch_force_fp64(int order, unsigned flags, int L, dim3 grid, siz
 constexpr int kBankLooks = S2_BANK_LOOKS;   // later looks at the next chunk's ticket inside a chunk (0: only at the start);
                                             // measured at n_i = 65536 / 81920 / 2^18: 0: 421 / 480 / 513, 3: 494 / - / 518, 7: 501 / 503 / 518,
                                             // 15: 506 / 510 / 518, 31: 507 / 511 / 518, 63: 501 / 504 / 512 Gpairs/s
-template <class P, int BANK>   // BANK only makes the kernels of the two translation units distinct symbols
-__global__ void __launch_bounds__(P::kBankThreads, P::kMinBlocksBank) force_sweep_bank_kernel(const ForceArgs a)
+template <class P, int BANK, int THREADS>   // BANK only makes the kernels of the two translation units distinct symbols
+__global__ void __launch_bounds__(THREADS, P::kMinBlocksBank * P::kBankThreads / THREADS) force_sweep_bank_kernel(const ForceArgs a)
 {
     constexpr int NC = P::ORDER == 6 ? 10 : 7;   // running sums carried per i
     Decomp d;
     d.lane = threadIdx.x & 31;
     d.il = d.lane; d.jl = 0; d.wi = threadIdx.x >> 5; d.wj = 0; d.slice = 0;
-    d.i = blockIdx.x * P::kBankThreads + threadIdx.x;
+    d.i = blockIdx.x * THREADS + threadIdx.x;   // 256 threads (2 CTAs per SM) or 128 (4 per SM: finer fill of shared rounds)
     d.i_valid = d.i < a.ni;
     if (!d.i_valid) d.i = a.ni - 1;   // padding lanes recompute the last i and never write
     // Overlap of consecutive chunk launches (programmatic dependent launch) and hand-over of the two banks:
@@ -395,7 +395,7 @@ __global__ void __launch_bounds__(P::kBankThreads, P::kMinBlocksBank) force_swee
 #pragma unroll
             for (int p = 0; p < P::NPL; ++p) {
                 const double2 *src = static_cast<const double2 *>(a.jp[p]) + a.bank_next_j0;
-                for (int k = threadIdx.x; k < a.bank_next_cnt; k += P::kBankThreads) dst[p * P::kChunk + k] = __ldcg(src + k);
+                for (int k = threadIdx.x; k < a.bank_next_cnt; k += THREADS) dst[p * P::kChunk + k] = __ldcg(src + k);
             }
             __threadfence();
             __syncthreads();
@@ -445,15 +445,20 @@ static cudaError_t launch_bank(const ForceArgs &a, cudaStream_t st, int *geom)
 {
     if (geom) { geom[0] = P::kChunk; geom[1] = P::kBankThreads; geom[2] = P::kMinBlocksBank; return cudaSuccess; }
     cudaLaunchConfig_t cfg = {};
-    cfg.gridDim = dim3((a.ni + P::kBankThreads - 1) / P::kBankThreads);
-    cfg.blockDim = dim3(P::kBankThreads);
+    // the 128-thread instance exists for the plain 4th-order sweep only (s2_api.cu asks for it at mid-sized i-lists)
+    constexpr bool kHasSmall = P::ORDER == 4 && !P::NN && !P::NGB && P::kBankThreads == 256;
+    const int threads = (kHasSmall && a.bank_threads == 128) ? 128 : P::kBankThreads;
+    cfg.gridDim = dim3((a.ni + threads - 1) / threads);
+    cfg.blockDim = dim3(threads);
     cfg.stream = st;
     cudaLaunchAttribute at[1];
     at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
     at[0].val.programmaticStreamSerializationAllowed = 1;
     cfg.attrs = at;
     cfg.numAttrs = a.bank_pdl ? 1 : 0;
-    return cudaLaunchKernelEx(&cfg, force_sweep_bank_kernel<P, S2_BANK_ID>, a);
+    if constexpr (kHasSmall)
+        if (threads == 128) return cudaLaunchKernelEx(&cfg, force_sweep_bank_kernel<P, S2_BANK_ID, 128>, a);
+    return cudaLaunchKernelEx(&cfg, force_sweep_bank_kernel<P, S2_BANK_ID, P::kBankThreads>, a);
 }
 
 // geom != nullptr: only report {chunk length of this order's bank layout, threads per CTA, CTAs per SM aimed at}

@@ -117,6 +117,7 @@ struct ForceArgs {
     int bank_next_j0, bank_next_cnt;   // the chunk after next, which the last CTA copies into this bank (cnt 0: none)
     int bank_pdl;                  // launch with programmatic stream serialisation (overlaps the previous chunk's tail)
     int bank_wait_early;           // wait for the previous launch before anything is read (decisions carried, chunk 0)
+    int bank_threads;              // threads per CTA of the chunk launches (128 or 256; 0: the policy's default)
 };
 
 struct ReduceArgs {
