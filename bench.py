@@ -429,6 +429,7 @@ def ni_sweep(s2, torch, dev, order):
                 for _ in range(300):
                     s2.s2_calc_ilist(ctx, il_h, None, w.eps2, 0); s2.s2_get_results(ctx, ni)
                 host_us = (time.perf_counter() - t0) / 300 * 1e6
+                host_c_us = s2.s2_time_host_roundtrip(ctx, il_h, w.eps2, 0, 1000)
             peak = FP64_PEAK_TFLOPS if pname == "fp64" else FP32_PEAK_TFLOPS
             rows.append({"cfg": str(key), "precision": pname, "N": w.N, "n_i": ni, "call_us": round(us, 2), "timing": how,
                          "ginteractions_per_s": g, "vs_full_rate": g / full,
@@ -437,7 +438,8 @@ def ni_sweep(s2, torch, dev, order):
                          "i_per_thread": info["i_per_thread"], "grid": info["grid"],
                          "combine": ("none", "reduce kernel", "fused", "none (chunk launches)", "atomics")[info["reduced"]]})
             if host_us is not None:
-                rows[-1]["host_roundtrip_us"] = round(host_us, 1)
+                rows[-1]["host_roundtrip_us"] = round(host_us, 1)          # through the Python binding (ctypes)
+                rows[-1]["host_roundtrip_c_us"] = round(host_c_us, 1)      # the same two calls timed inside the library
         out.extend(rows[::-1])
         s2.s2_close(ctx)
     return out

@@ -197,6 +197,13 @@ int s2_enable_timing(s2_ctx *ctx, int on);
  * (force sweep, reduce/compaction); 0 for kernels that did not run.  SYNC. */
 int s2_get_timing(s2_ctx *ctx, float *predict_ms, float *force_ms, float *reduce_ms);
 
+/* Host wall time, in microseconds per call, of s2_calc_ilist + s2_get_results (all outputs but neighbour lists)
+ * repeated `reps` times after 3 warm-up calls, measured inside the library with the steady clock: the latency of
+ * a small force call as a C caller sees it (BASELINE config 2; PAPER.md L114, L124 on small-n_i overheads), without
+ * any binding layer.  i_address: host array of ni addresses.  S2_WANT_NGB is not accepted.  SYNC. */
+int s2_time_host_roundtrip(s2_ctx *ctx, int ni, const int *i_address, double eps2, unsigned flags, int reps,
+                           double *us_per_call);
+
 /* Peak microbenchmarks used as roofline denominators and for the FP64 operand-path model:
  * a grid that fills the device runs `iters` rounds of 8 independent chains per thread.
  *   kind 0 = DFMA with constant operands (nominal fp64 rate)      1 = FFMA (fp32)

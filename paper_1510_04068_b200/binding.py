@@ -80,6 +80,7 @@ def lib() -> C.CDLL:
         "s2_enable_timing": (C.c_int, [vp, C.c_int]),
         "s2_get_timing": (C.c_int, [vp, C.POINTER(C.c_float), C.POINTER(C.c_float), C.POINTER(C.c_float)]),
         "s2_peak_fma": (C.c_int, [vp, C.c_int, C.c_int, C.POINTER(C.c_double)]),
+        "s2_time_host_roundtrip": (C.c_int, [vp, C.c_int, C.POINTER(C.c_int), C.c_double, C.c_uint, C.c_int, C.POINTER(C.c_double)]),
         "s2_strerror": (C.c_char_p, [C.c_int]),
         "s2_last_cuda_error": (C.c_char_p, [vp]),
         "s2_version": (C.c_char_p, []),
@@ -339,6 +340,15 @@ def s2_get_timing(ctx) -> dict:
     a, b, c = C.c_float(), C.c_float(), C.c_float()
     _check(lib().s2_get_timing(ctx.handle, C.byref(a), C.byref(b), C.byref(c)), "s2_get_timing", ctx.handle)
     return dict(predict_ms=a.value, force_ms=b.value, reduce_ms=c.value)
+
+
+def s2_time_host_roundtrip(ctx, i_address, eps2: float = 0.0, flags: int = 0, reps: int = 1000) -> float:
+    """Microseconds per (s2_calc_ilist + s2_get_results) as timed inside the library (no binding in the loop)."""
+    ia = np.ascontiguousarray(i_address, dtype=np.int32)
+    v = C.c_double()
+    _check(lib().s2_time_host_roundtrip(ctx.handle, ia.size, ia.ctypes.data_as(C.POINTER(C.c_int)), float(eps2), int(flags),
+                                        int(reps), C.byref(v)), "s2_time_host_roundtrip", ctx.handle)
+    return v.value
 
 
 def s2_peak_fma(ctx, kind: int, iters: int = 2000) -> float:

@@ -8,10 +8,12 @@
 #include <string.h>
 
 #include <algorithm>
+#include <chrono>
 #include <map>
 #include <mutex>
 #include <string>
 #include <thread>
+#include <vector>
 
 #include "s2_internal.h"
 
@@ -1294,6 +1296,32 @@ extern "C" int s2_get_timing(s2_ctx *ctx, float *predict_ms, float *force_ms, fl
     if (predict_ms) *predict_ms = v[0];
     if (force_ms) *force_ms = v[1];
     if (reduce_ms) *reduce_ms = v[2];
+    return S2_OK;
+}
+
+// Host wall time of one small force call as a C caller sees it: s2_calc_ilist + s2_get_results (which synchronises),
+// `reps` times in a row, measured with the steady clock here so that no binding layer is in the loop.
+extern "C" int s2_time_host_roundtrip(s2_ctx *ctx, int ni, const int *i_address, double eps2, unsigned flags, int reps,
+                                      double *us_per_call)
+{
+    if (!ctx || !i_address || !us_per_call || ni <= 0 || reps <= 0 || (flags & S2_WANT_NGB)) return S2_EINVAL;
+    std::vector<double> acc((size_t)ni * 3), jerk((size_t)ni * 3), snap((size_t)ni * 3), pot((size_t)ni), nn_r2((size_t)ni);
+    std::vector<int> nn_id((size_t)ni);
+    for (int k = 0; k < 3; ++k) {   // warm-up: shape cache, pinned buffers
+        int rc = s2_calc_ilist(ctx, ni, i_address, nullptr, eps2, flags);
+        if (rc != S2_OK) return rc;
+        rc = s2_get_results(ctx, ni, acc.data(), jerk.data(), snap.data(), pot.data(), nn_id.data(), nn_r2.data(), nullptr);
+        if (rc != S2_OK) return rc;
+    }
+    const auto t0 = std::chrono::steady_clock::now();
+    for (int k = 0; k < reps; ++k) {
+        int rc = s2_calc_ilist(ctx, ni, i_address, nullptr, eps2, flags);
+        if (rc != S2_OK) return rc;
+        rc = s2_get_results(ctx, ni, acc.data(), jerk.data(), snap.data(), pot.data(), nn_id.data(), nn_r2.data(), nullptr);
+        if (rc != S2_OK) return rc;
+    }
+    const auto t1 = std::chrono::steady_clock::now();
+    *us_per_call = std::chrono::duration<double, std::micro>(t1 - t0).count() / reps;
     return S2_OK;
 }
 
