@@ -39,8 +39,10 @@ FP32_PEAK_TFLOPS = 2 * FP64_PEAK_TFLOPS                                    # 128
 # dram__bytes_read.sum + dram__bytes_write.sum of one force-sweep launch at the headline point,
 # from the ncu --set full capture summarised in profiles/ (None until a capture exists)
 FORCE_KERNEL_DRAM_BYTES = 20.99e6   # tiled sweep: 18.02 MB read + 2.96 MB written (profiles/r01_force_fp64_ncu_full.md)
-BANK_KERNEL_DRAM_BYTES = 29.44e6    # uniform-operand sweep, per chunk launch: 29.44 MB read (parked i-state + running
+BANK_KERNEL_DRAM_BYTES = 29.51e6    # uniform-operand sweep, per chunk launch: 29.51 MB read (parked i-state + running
                                     # sums, cold L2 under ncu) + 0 written (profiles/r01_force_bank_ncu_full.md)
+FP32_KERNEL_DRAM_BYTES = 16.24e6    # packed fp32 tiled sweep at N = n_i = 2^18: 13.71 MB read + 2.52 MB written
+                                    # (profiles/r01_predict_and_fp32_ncu.md)
 
 
 def parse_args():
@@ -268,7 +270,8 @@ def main():
              else f"force_sweep_kernel<{kname}<{order},0,0>,{info['lanes_per_i']}>")
     roofline = {"bound": "alu", "kernel": kname, "achieved": achieved,
                 "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak,
-                "traffic": (BANK_KERNEL_DRAM_BYTES if info["reduced"] == 3 else FORCE_KERNEL_DRAM_BYTES) if fp64_path else None,
+                "traffic": ((BANK_KERNEL_DRAM_BYTES if info["reduced"] == 3 else FORCE_KERNEL_DRAM_BYTES) if fp64_path else
+                            FP32_KERNEL_DRAM_BYTES if (args.precision == "fp32" and info["i_per_thread"] > 1) else None),
                 "peak_source": ("derived: 148 SM x 64 FP64 FMA lanes x 2 flop x 1.965 GHz" if fp64_path else
                                 "derived: 148 SM x 128 FP32 FMA lanes x 2 flop x 1.965 GHz") + " (DESIGN.md 5.2); not in MEASURED_PEAKS.json",
                 "convention": f"{FLOP_PER_PAIR[order]} flop per pair interaction (labelled convention, reading P16)",
