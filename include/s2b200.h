@@ -111,7 +111,7 @@ int s2_set_j(s2_ctx *ctx, int n, const int *address, const int *id, const double
              const double *jerk, const double *snap, const double *crackle);
 /* Copies the staged particles to the device and scatters them into the SoA j-store. ASYNC. */
 int s2_commit_j(s2_ctx *ctx);
-/* Same scatter, from arrays that already live in device memory (same layouts as s2_set_j).
+/* Same scatter, from arrays that already live in device memory (same layouts and NULL rules as s2_set_j).
  * Address range is the caller's responsibility here (checked on the device: out-of-range
  * entries are dropped and reported as S2_ERANGE at the next SYNC call).  ASYNC. */
 int s2_commit_j_device(s2_ctx *ctx, int n, const int *d_address, const int *d_id, const double *d_t,
@@ -151,14 +151,28 @@ int s2_calc_explicit(s2_ctx *ctx, int ni, const int *id, const double *pos, cons
  * Returns S2_EOVERFLOW (results still written) if any list was truncated.  SYNC. */
 int s2_get_results(s2_ctx *ctx, int ni, double *acc, double *jerk, double *snap, double *pot,
                    int *nn_id, double *nn_r2, int *ngb_count);
+/* The same results written into DEVICE arrays of the caller (same shapes; any may be NULL), by a kernel enqueued
+ * behind the force call: nothing crosses the host link and nothing synchronises, so a device-resident consumer
+ * (an integrator kernel, a collective over j-sharded partial results) can follow directly.
+ * Truncated lists are not reported here (s2_get_results / s2_get_neighbours_csr do).  ASYNC. */
+int s2_get_results_device(s2_ctx *ctx, int ni, double *d_acc, double *d_jerk, double *d_snap, double *d_pot,
+                          int *d_nn_id, double *d_nn_r2, int *d_ngb_count);
 /* Neighbour list of the i-th entry of the i-list: j addresses, ascending, at most
  * min(cap, ngb_cap) entries; *n_out = number written.  SYNC. */
 int s2_get_neighbours(s2_ctx *ctx, int i, int cap, int *n_out, int *list);
 /* All lists in CSR form: offsets has ni+1 entries, list has offsets[ni] <= list_cap entries
- * (S2_ERANGE if list_cap is too small; offsets are still written so the caller can resize). SYNC. */
+ * (S2_ERANGE if list_cap is too small; offsets are still written so the caller can resize).
+ * The lists are compacted ON THE DEVICE (count -> exclusive scan -> fill): only the offsets and the
+ * offsets[ni] list members cross the host link, not the fixed-stride ni x ngb_cap buffer.  The compaction runs once
+ * per force call and is cached, so a sizing call (list == NULL, list_cap == 0) followed by the real one costs one
+ * compaction.  Returns S2_EOVERFLOW (output still written) if any list of the last call was truncated.  SYNC. */
 int s2_get_neighbours_csr(s2_ctx *ctx, int ni, long long *offsets, int *list, long long list_cap);
+/* The same CSR, left in device memory for device-resident callers: *d_offsets points at ni_last+1 64-bit offsets,
+ * *d_list at the compacted addresses (both context-owned, valid until the next s2_calc_* or s2_close);
+ * *total = offsets[ni].  SYNC (one 8-byte read). */
+int s2_get_neighbours_csr_device(s2_ctx *ctx, int ni, const long long **d_offsets, const int **d_list, long long *total);
 
-/* --- test hooks and diagnostics ---------------------------------------------------------- */
+/* --- read-back hooks and diagnostics (tuning overrides and microbenchmarks: s2b200_test.h) --- */
 
 /* fp64 predicted state of j-particles first .. first+n-1 ((n,3) arrays, any may be NULL;
  * acc = predicted acceleration for order 6, undefined for order 4).  SYNC. */
@@ -166,29 +180,6 @@ int s2_get_predicted_j(s2_ctx *ctx, int first, int n, double *pos, double *vel, 
 /* stored (unpredicted) state: id, t, mass (n) and pos (n,3); any may be NULL.  SYNC. */
 int s2_get_j(s2_ctx *ctx, int first, int n, int *id, double *t, double *mass, double *pos);
 
-/* Launch-shape overrides for tests and tuning sweeps; value 0 restores the automatic choice.
- *   key 0: number of j-slices S      key 1: lanes per i-particle (1,2,4,..,32)
- *   key 2: warp columns over j (1,2,4,8; only with lanes == 32)
- *   key 3: CTAs per SM assumed by the balancer      key 4: j-tile length (multiple of 32)
- *   key 5: 1 = combine j-slices with the separate reduce kernel even when the fused combine applies,
- *          2 = combine them with fp64 atomics on the final records instead (the paper's Sapporo2 scheme, L88): one
- *          launch, but the last bits then vary run to run; ignored when NN / neighbour lists are requested,
- *          3 = use the fused combine (last CTA of each i-group) whenever the shape allows it
- *   key 6: CTAs per thread-block cluster along the slice axis in the fused combine (1 = none, 2, 4, 8)
- *   key 7: 1 = never use the register-tiled sweep (several i per thread), 2 = always use it
- *   key 8: 1 = never use the uniform-operand sweep (j-particles read chunk by chunk from the constant bank, one
- *          launch per chunk; fp64 only), 2 = always use it when the context computes in fp64
- *   key 9: 1 = never use the zero-copy path of small host calls (n_i <= 128 with host arrays: the kernels read the
- *          i-list from, and write the final records to, pinned host memory, so no copy is enqueued) */
-int s2_set_tuning(s2_ctx *ctx, int key, int value);
-/* Shape of the last force launch: out[0]=S, [1]=lanes per i, [2]=warp columns, [3]=grid size,
- * [4]=threads per CTA, [5]=dynamic shared memory bytes, [6]=0 no combine needed / 1 reduce kernel ran /
- * 2 combine fused into the sweep launch (last CTA of each i-group reduces, fixed order) / 3 uniform-operand
- * sweep: out[0] is then the number of chunk launches (sums carried in address order, nothing to combine) /
- * 4 combined by atomics (key 5 = 2),
- * [7]=resident CTAs per SM (occupancy query), [8]=i-particles per thread (register-tiled sweep when > 1),
- * [9]=CTAs per cluster. */
-int s2_last_launch_info(const s2_ctx *ctx, int out[10]);
 /* Number of kernels this context has launched since s2_open. */
 long long s2_kernel_launches(const s2_ctx *ctx);
 /* When enabled, CUDA events bracket each kernel of predict / calc on the context's stream. */
@@ -196,30 +187,6 @@ int s2_enable_timing(s2_ctx *ctx, int on);
 /* Device time in milliseconds of the kernels of the last s2_predict and the last s2_calc_*
  * (force sweep, reduce/compaction); 0 for kernels that did not run.  SYNC. */
 int s2_get_timing(s2_ctx *ctx, float *predict_ms, float *force_ms, float *reduce_ms);
-
-/* Host wall time, in microseconds per call, of s2_calc_ilist + s2_get_results (all outputs but neighbour lists)
- * repeated `reps` times after 3 warm-up calls, measured inside the library with the steady clock: the latency of
- * a small force call as a C caller sees it (BASELINE config 2; PAPER.md L114, L124 on small-n_i overheads), without
- * any binding layer.  i_address: host array of ni addresses.  S2_WANT_NGB is not accepted.  SYNC. */
-int s2_time_host_roundtrip(s2_ctx *ctx, int ni, const int *i_address, double eps2, unsigned flags, int reps,
-                           double *us_per_call);
-
-/* Peak microbenchmarks used as roofline denominators and for the FP64 operand-path model:
- * a grid that fills the device runs `iters` rounds of 8 independent chains per thread.
- *   kind 0 = DFMA with constant operands (nominal fp64 rate)      1 = FFMA (fp32)
- *   kind 2 = DFMA with three distinct 64-bit register operands    3 = DFMA with one operand shared by
- *   consecutive instructions (operand-reuse cache)                 4 = DADD with two distinct register operands
- *   kind 5-8 = packed FP32 (two lane-operations per instruction, both counted): 5 = FFMA2 with constant operands,
- *   6 = FFMA2 with three distinct register pairs, 7 = FFMA2 with a 32-bit register broadcast to both halves,
- *   8 = FADD2 with two distinct register pairs
- * Returns achieved lane-instructions per second in *fma_per_s.  SYNC. */
-int s2_peak_fma(s2_ctx *ctx, int kind, int iters, double *fma_per_s);
-
-/* Test hook for the double-single arithmetic of the S2_DS path (reading P11): for k < n (host arrays) the operands
- * a[k], b[k] are split into (hi, lo) float pairs on the device and out[8k .. 8k+7] receives, as fp64,
- *   [0] the round trip of a   [1] a + b   [2] a - b (cancellation-safe form)   [3] a b   [4] a^2   [5] -3 a
- *   [6] |a|^(-1/2)   [7] a b + a.   SYNC. */
-int s2_test_ds_ops(s2_ctx *ctx, int n, const double *a, const double *b, double *out);
 
 const char *s2_strerror(int code);
 /* cudaGetErrorString of the last CUDA failure seen by this context ("" if none). */

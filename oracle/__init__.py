@@ -76,6 +76,11 @@ class ForceResult:
     nn_addr_ld: np.ndarray    # long-double-decision nearest neighbour (informational)
     ngb_count: np.ndarray | None
     ngb_list: np.ndarray | None   # (ni, cap), ascending addresses, -1 padded
+    nn_d2_ld: np.ndarray | None = None        # long-double d2 of nn_addr_ld, rounded to fp64 once
+    ngb_count_ld: np.ndarray | None = None    # neighbour set decided on the long-double d2 (rr < h2)
+    ngb_list_ld: np.ndarray | None = None
+    inputs: dict | None = None                # the geometry the decisions were taken on (xj, xi, h2, ident): lets a
+                                              # test re-evaluate one pair's d2 in long double without another oracle run
 
     def ngb_sets(self):
         return [set(int(x) for x in row[row >= 0]) for row in self.ngb_list]
@@ -101,13 +106,17 @@ def forces(order: int, mass, ident, xp, vp, ap, i_id, xi, vi, ai, eps2: float,
     nn_d2 = np.empty(ni)
     cnt = np.zeros(ni, np.int32) if h2 is not None else None
     lst = np.full((ni, ngb_cap), -1, np.int32) if h2 is not None else None
+    nn_d2_ld = np.empty(ni)
+    cnt_ld = np.zeros(ni, np.int32) if h2 is not None else None
+    lst_ld = np.full((ni, ngb_cap), -1, np.int32) if h2 is not None else None
     d, i = np.float64, np.int32
     lib().oracle_forces(C.c_int(order), C.c_int(N), _p(mass, d), _p(ident, i), _p(xp, d), _p(vp, d), _p(ap, d),
                         C.c_int(ni), _p(i_id, i), _p(xi, d), _p(vi, d), _p(ai, d), _p(h2, d), C.c_double(eps2),
                         _p(acc, d), _p(jerk, d), _p(snap, d), _p(pot, d),
                         _p(nn_addr, i), _p(nn_id, i), _p(nn_d2, d), _p(nn_addr_ld, i),
-                        _p(cnt, i), _p(lst, i), C.c_int(ngb_cap))
-    return ForceResult(acc, jerk, snap, pot, nn_addr, nn_id, nn_d2, nn_addr_ld, cnt, lst)
+                        _p(cnt, i), _p(lst, i), C.c_int(ngb_cap), _p(nn_d2_ld, d), _p(cnt_ld, i), _p(lst_ld, i))
+    return ForceResult(acc, jerk, snap, pot, nn_addr, nn_id, nn_d2, nn_addr_ld, cnt, lst, nn_d2_ld, cnt_ld, lst_ld,
+                       dict(xj=xp, xi=xi, h2=h2, ident=ident, ngb_cap=ngb_cap))
 
 
 def forces_ilist(order: int, mass, ident, xp, vp, ap, i_address, eps2: float,

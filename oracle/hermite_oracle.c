@@ -109,8 +109,13 @@ void oracle_predict(int n, int order, double t, const double *tj,
  * The two integer decisions (nearest neighbour, neighbour membership) are
  * taken on d2 evaluated in the CUDA path's decision precision (fp64):
  *     dx = fl(x_j - x_i) ...;  d2 = fma(dz, dz, fma(dy, dy, fl(dx*dx)))
- * (reading R-D2).  The long-double d2 decision is returned as
- * well (nn_addr_ld) so tests can count where the two differ.
+ * (reading R-D2).  The decisions taken on the long-double d2 (the
+ * oracle's own arithmetic, no formula shared with the kernels) are returned
+ * as well: nn_addr_ld / nn_d2_ld (d2 rounded to fp64 once) and the neighbour
+ * set ngb_count_ld / ngb_list_ld (rr < h2_i in long double).  The GPU parity
+ * tests are judged against THESE, within north_star's band (nn: candidates
+ * whose long-double d2 differ by <= 1e-12 relative; sets: pairs within 1e-12
+ * relative of h2); equality with the fp64 decision is a secondary check.
  *
  * Inputs: (N,3) predicted arrays of the j-store; explicit i arrays (ni,3).
  * Outputs (any may be NULL): acc, jerk, snap (ni,3); pot, nn_d2 (ni);
@@ -124,14 +129,15 @@ void oracle_forces(int order, int N, const double *m, const int *id,
                    const double *h2, double eps2,
                    double *acc, double *jerk, double *snap, double *pot,
                    int *nn_addr, int *nn_id, double *nn_d2, int *nn_addr_ld,
-                   int *ngb_count, int *ngb_list, int ngb_cap)
+                   int *ngb_count, int *ngb_list, int ngb_cap,
+                   double *nn_d2_ld, int *ngb_count_ld, int *ngb_list_ld)
 {
 #pragma omp parallel for schedule(dynamic, 8)
     for (int i = 0; i < ni; ++i) {
         ld A[3] = {0, 0, 0}, J[3] = {0, 0, 0}, S[3] = {0, 0, 0}, P = 0;
         double best = INFINITY;
         ld best_ld = INFINITY;
-        int best_j = -1, best_j_ld = -1, cnt = 0;
+        int best_j = -1, best_j_ld = -1, cnt = 0, cnt_ld = 0;
         const double *Xi = xi + (size_t)3 * i, *Vi = vi + (size_t)3 * i;
         const double *Ai = (order == 6) ? ai + (size_t)3 * i : NULL;
         for (int j = 0; j < N; ++j) {
@@ -168,6 +174,10 @@ void oracle_forces(int order, int N, const double *m, const int *id,
             double d2 = fma(dz, dz, fma(dy, dy, dx * dx));
             if (d2 < best) { best = d2; best_j = j; }
             if (rr < best_ld) { best_ld = rr; best_j_ld = j; }
+            if (h2 && rr < (ld)h2[i]) {
+                if (ngb_list_ld && cnt_ld < ngb_cap) ngb_list_ld[(size_t)i * ngb_cap + cnt_ld] = j;
+                ++cnt_ld;
+            }
             if (h2 && d2 < h2[i]) {
                 if (ngb_list && cnt < ngb_cap) ngb_list[(size_t)i * ngb_cap + cnt] = j;
                 ++cnt;
@@ -184,6 +194,10 @@ void oracle_forces(int order, int N, const double *m, const int *id,
         if (nn_d2) nn_d2[i] = best;
         if (nn_addr_ld) nn_addr_ld[i] = best_j_ld;
         if (ngb_count) ngb_count[i] = cnt;
+        if (nn_d2_ld) nn_d2_ld[i] = (double)best_ld;
+        if (ngb_count_ld) ngb_count_ld[i] = cnt_ld;
+        if (ngb_list_ld)
+            for (int k = cnt_ld; k < ngb_cap; ++k) ngb_list_ld[(size_t)i * ngb_cap + k] = -1;
         if (ngb_list)
             for (int k = cnt; k < ngb_cap; ++k) ngb_list[(size_t)i * ngb_cap + k] = -1;
     }

@@ -17,6 +17,7 @@ import numpy as np
 _PKG = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_PKG, "libs2b200.so")
 HEADER_PATH = os.path.join(os.path.dirname(_PKG), "include", "s2b200.h")
+TEST_HEADER_PATH = os.path.join(os.path.dirname(_PKG), "include", "s2b200_test.h")   # tuning overrides, microbenchmarks
 
 S2_FP64, S2_DS, S2_FP32 = 0, 1, 2
 S2_WANT_NN, S2_WANT_NGB = 1, 2
@@ -39,11 +40,15 @@ class S2Error(RuntimeError):
 _lib = None
 
 
-def header_symbols() -> list[str]:
-    """Every function include/s2b200.h declares."""
-    src = open(HEADER_PATH).read()
-    src = re.sub(r"/\*.*?\*/", "", src, flags=re.S)
-    return sorted(set(re.findall(r"\b(s2_[a-z0-9_]+)\s*\(", src)))
+def header_symbols(which: str = "all") -> list[str]:
+    """Every function include/s2b200.h (the product ABI) and include/s2b200_test.h (test hooks) declare;
+    which = "product" | "test" | "all"."""
+    paths = {"product": [HEADER_PATH], "test": [TEST_HEADER_PATH], "all": [HEADER_PATH, TEST_HEADER_PATH]}[which]
+    names = set()
+    for path in paths:
+        src = re.sub(r"/\*.*?\*/", "", open(path).read(), flags=re.S)
+        names.update(re.findall(r"\b(s2_[a-z0-9_]+)\s*\(", src))
+    return sorted(names)
 
 
 def lib() -> C.CDLL:
@@ -69,8 +74,11 @@ def lib() -> C.CDLL:
         "s2_calc_ilist_device": (C.c_int, [vp, C.c_int, ip, dp, C.c_double, C.c_uint]),
         "s2_calc_explicit": (C.c_int, [vp, C.c_int, ip, dp, dp, dp, dp, C.c_double, C.c_uint]),
         "s2_get_results": (C.c_int, [vp, C.c_int, dp, dp, dp, dp, ip, dp, ip]),
+        "s2_get_results_device": (C.c_int, [vp, C.c_int, dp, dp, dp, dp, ip, dp, ip]),
         "s2_get_neighbours": (C.c_int, [vp, C.c_int, C.c_int, C.POINTER(C.c_int), ip]),
         "s2_get_neighbours_csr": (C.c_int, [vp, C.c_int, vp, ip, C.c_longlong]),
+        "s2_get_neighbours_csr_device": (C.c_int, [vp, C.c_int, C.POINTER(vp), C.POINTER(vp), C.POINTER(C.c_longlong)]),
+        "s2_get_csr_timing": (C.c_int, [vp, C.POINTER(C.c_float), C.POINTER(C.c_float)]),
         "s2_get_predicted_j": (C.c_int, [vp, C.c_int, C.c_int, dp, dp, dp]),
         "s2_get_j": (C.c_int, [vp, C.c_int, C.c_int, ip, dp, dp, dp]),
         "s2_set_tuning": (C.c_int, [vp, C.c_int, C.c_int]),
@@ -226,7 +234,7 @@ def s2_commit_j(ctx):
     _check(lib().s2_commit_j(ctx.handle), "s2_commit_j", ctx.handle)
 
 
-def s2_commit_j_device(ctx, d_address, d_id, d_t, d_mass, d_pos, d_vel, d_acc, d_jerk, d_snap=None, d_crackle=None):
+def s2_commit_j_device(ctx, d_address, d_id, d_t, d_mass, d_pos, d_vel, d_acc=None, d_jerk=None, d_snap=None, d_crackle=None):
     n = d_address.numel()
     args = [_d(d_address, "int32", n, "address"), _d(d_id, "int32", n, "id"), _d(d_t, "float64", n, "t"),
             _d(d_mass, "float64", n, "mass")]
@@ -280,6 +288,15 @@ def s2_get_results(ctx, ni: int, allow_overflow: bool = True) -> dict:
     return out
 
 
+def s2_get_results_device(ctx, ni: int, acc=None, jerk=None, snap=None, pot=None, nn_id=None, nn_r2=None, ngb_count=None):
+    """Unpacks the results of the last s2_calc_* into the given torch CUDA tensors (any may be None).  ASYNC."""
+    args = [_d(acc, "float64", 3 * ni, "acc"), _d(jerk, "float64", 3 * ni, "jerk"), _d(snap, "float64", 3 * ni, "snap"),
+            _d(pot, "float64", ni, "pot"), _d(nn_id, "int32", ni, "nn_id"), _d(nn_r2, "float64", ni, "nn_r2"),
+            _d(ngb_count, "int32", ni, "ngb_count")]
+    ctx._keep = ctx._keep + [acc, jerk, snap, pot, nn_id, nn_r2, ngb_count]
+    _check(lib().s2_get_results_device(ctx.handle, int(ni), *args), "s2_get_results_device", ctx.handle)
+
+
 def s2_get_neighbours(ctx, i: int, cap: int) -> np.ndarray:
     lst = np.empty(max(cap, 1), np.int32)
     n = C.c_int(0)
@@ -288,17 +305,45 @@ def s2_get_neighbours(ctx, i: int, cap: int) -> np.ndarray:
     return lst[:n.value].copy()
 
 
+class _DeviceView:
+    """Zero-copy view of library-owned device memory (valid until the next s2_calc_* / s2_close)."""
+
+    def __init__(self, ptr: int, n: int, typestr: str):
+        self.__cuda_array_interface__ = {"shape": (n,), "typestr": typestr, "data": (ptr, True), "version": 2}
+
+
+def s2_get_neighbours_csr_device(ctx, ni: int):
+    """(offsets, list, total): torch views of the device-resident CSR (int64 offsets of the whole last call, int32
+    addresses); total = offsets[ni].  No list data crosses the host link."""
+    import torch
+    po, pl, tot = C.c_void_p(), C.c_void_p(), C.c_longlong()
+    rc = lib().s2_get_neighbours_csr_device(ctx.handle, int(ni), C.byref(po), C.byref(pl), C.byref(tot))
+    _check(rc, "s2_get_neighbours_csr_device", ctx.handle, ok=(S2_OK, S2_EOVERFLOW))
+    dev = torch.device("cuda", ctx.device)
+    off = torch.as_tensor(_DeviceView(po.value, ni + 1, "<i8"), device=dev)
+    lst = torch.as_tensor(_DeviceView(pl.value, max(int(tot.value), 1), "<i4"), device=dev)[:int(tot.value)]
+    return off, lst, int(tot.value)
+
+
 def s2_get_neighbours_csr(ctx, ni: int, list_cap: int | None = None):
+    """(offsets, list) on the host.  One read-back: the library compacts the lists on the device once per force call;
+    the sizing query below only reads the 8-byte total."""
     off = np.zeros(ni + 1, np.int64)
-    if list_cap is None:   # first call sizes the list
-        rc = lib().s2_get_neighbours_csr(ctx.handle, ni, off.ctypes.data_as(C.c_void_p), None, 0)
-        if rc not in (S2_OK, S2_ERANGE, S2_EOVERFLOW):
-            _check(rc, "s2_get_neighbours_csr", ctx.handle)
-        list_cap = int(off[ni])
+    if list_cap is None:
+        po, pl, tot = C.c_void_p(), C.c_void_p(), C.c_longlong()
+        rc = lib().s2_get_neighbours_csr_device(ctx.handle, int(ni), C.byref(po), C.byref(pl), C.byref(tot))
+        _check(rc, "s2_get_neighbours_csr", ctx.handle, ok=(S2_OK, S2_EOVERFLOW))
+        list_cap = int(tot.value)
     lst = np.empty(max(list_cap, 1), np.int32)
     rc = lib().s2_get_neighbours_csr(ctx.handle, ni, off.ctypes.data_as(C.c_void_p), lst.ctypes.data_as(C.c_void_p), list_cap)
     _check(rc, "s2_get_neighbours_csr", ctx.handle, ok=(S2_OK, S2_EOVERFLOW))
-    return off, lst[:off[ni]].copy()
+    return off, lst[:off[ni]]
+
+
+def s2_get_csr_timing(ctx) -> dict:
+    a, b = C.c_float(), C.c_float()
+    _check(lib().s2_get_csr_timing(ctx.handle, C.byref(a), C.byref(b)), "s2_get_csr_timing", ctx.handle)
+    return dict(scan_ms=a.value, fill_ms=b.value)
 
 
 def s2_get_predicted_j(ctx, first: int, n: int):

@@ -18,6 +18,7 @@ CSRC = os.path.join(PKG, "csrc")
 OBJ = os.path.join(CSRC, "build")
 LIB = os.path.join(PKG, "libs2b200.so")
 HEADER = os.path.join(os.path.dirname(PKG), "include", "s2b200.h")
+TEST_HEADER = os.path.join(os.path.dirname(PKG), "include", "s2b200_test.h")
 
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
@@ -29,7 +30,7 @@ def _sources():
 
 
 def _deps_mtime():
-    hdrs = [os.path.join(CSRC, f) for f in os.listdir(CSRC) if f.endswith((".h", ".cuh"))] + [HEADER]
+    hdrs = [os.path.join(CSRC, f) for f in os.listdir(CSRC) if f.endswith((".h", ".cuh"))] + [HEADER, TEST_HEADER]
     return max(os.path.getmtime(h) for h in hdrs)
 
 

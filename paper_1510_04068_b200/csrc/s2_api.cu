@@ -16,8 +16,16 @@
 #include <vector>
 
 #include "s2_internal.h"
+#include "../../include/s2b200_test.h"
 
 namespace s2 {
+cudaError_t launch_csr_scan(const double *rec, int ni, int cap, int *len, long long *block_sum, long long *total,
+                            long long *offsets, cudaStream_t st);
+cudaError_t launch_csr_fill(const int *list, const int *len, const long long *offsets, int ni, int cap, int *out, cudaStream_t st);
+int csr_blocks(int ni);
+cudaError_t launch_compare_records(const double *a, const double *b, int ni, int order, double tol, int *bad, cudaStream_t st);
+cudaError_t launch_unpack_records(const double *rec, int ni, int order, double *acc, double *jerk, double *snap, double *pot,
+                                  int *nn_id, double *nn_r2, int *ngb_count, cudaStream_t st);
 cudaError_t dispatch_force_fp64(int order, unsigned flags, int L, dim3 grid, size_t smem, const ForceArgs &a,
                                 cudaStream_t st, bool query, int *ctas_per_sm);
 cudaError_t dispatch_force_fp32(int order, unsigned flags, int L, dim3 grid, size_t smem, const ForceArgs &a,
@@ -55,6 +63,12 @@ struct s2_ctx {
 
     // device buffers
     Buf base, planes, qplanes, stage_dev, iplanes, iqplanes, i_addr, i_h2, part, result, seg, list, flags, counters;
+    // device-side CSR of the neighbour lists of the last force call (built on first request, s2_ngb.cu)
+    Buf csr_len, csr_bsum, csr_off, csr_list;
+    bool csr_valid = false;
+    long long csr_total = 0;
+    cudaEvent_t ev_csr[4] = {nullptr, nullptr, nullptr, nullptr};
+    bool ran_csr = false;
     // pinned host buffers
     void *h_stage = nullptr;
     size_t h_stage_bytes = 0, h_stage_used = 0;
@@ -71,6 +85,7 @@ struct s2_ctx {
     cudaEvent_t ev_il[2] = {nullptr, nullptr};
     int il_turn = 0;
     bool flags_dirty = false;         // a device-side commit may have raised the range flag
+    bool in_selftest = false;         // inside bank_selftest (run_force re-entered with a reduced problem)
     cudaEvent_t ev_stage = nullptr;   // H2D of the staging buffer finished
     cudaEvent_t ev_io = nullptr;      // H2D of the i-list upload finished
     std::vector<Batch> batches;
@@ -204,6 +219,26 @@ static inline int n_qplanes(int precision, int order)
     return 0;
 }
 
+// ---- state shared by the contexts of one device: the two constant banks of the uniform-operand sweep ------------
+// (see run_force_bank below)
+struct BankOwner {
+    cudaEvent_t ev = nullptr;
+    cudaStream_t stream = nullptr;
+    bool used = false;
+    unsigned *flags = nullptr;   // device words {ready[2], -, -, arrived[2]} of the bank hand-over (run_force_bank)
+    unsigned ticket = 0;         // tickets handed out so far (chunk sequence numbers, cyclic)
+    int refs = 0;                // open contexts on this device; the last s2_close frees flags and event
+    // How the banks are refilled on this device (DESIGN.md 5.2 "what the uniform-operand sweep assumes"):
+    //   0 not yet decided; 1 by the sweep's own last CTA through the bank's global address, launches overlapped
+    //   (relies on behaviour CUDA does not document, so it is only used after bank_selftest has seen it produce the
+    //   shared-memory sweep's results on this device and driver); 2 by cudaMemcpyAsync between ordinary launches
+    //   (documented semantics; ~4 % slower)
+    int mode = 0;
+};
+static std::mutex g_bank_mu;
+static std::map<int, BankOwner> g_bank;
+enum { kBankSelfRefill = 1, kBankHostRefill = 2 };
+
 // ---- life cycle ---------------------------------------------------------------------------
 
 extern "C" int s2_open(s2_ctx **out, int device, int order, int precision, int nj_capacity, int ngb_cap,
@@ -249,8 +284,13 @@ extern "C" int s2_open(s2_ctx **out, int device, int order, int precision, int n
         if (e == cudaSuccess) e = cudaEventCreateWithFlags(&ctx->ev_il[0], cudaEventDisableTiming);
         if (e == cudaSuccess) e = cudaEventCreateWithFlags(&ctx->ev_il[1], cudaEventDisableTiming);
         for (int k = 0; k < 6 && e == cudaSuccess; ++k) e = cudaEventCreate(&ctx->ev_t[k]);
+        for (int k = 0; k < 4 && e == cudaSuccess; ++k) e = cudaEventCreate(&ctx->ev_csr[k]);
         if (e == cudaSuccess) e = cudaStreamSynchronize(ctx->stream);
         if (e != cudaSuccess) rc = fail_cuda(ctx, e);
+    }
+    {
+        std::lock_guard<std::mutex> lock(g_bank_mu);
+        g_bank[device].refs++;
     }
     if (rc != S2_OK) {
         s2_close(ctx);
@@ -266,8 +306,11 @@ extern "C" int s2_close(s2_ctx *ctx)
     cudaSetDevice(ctx->device);
     cudaStreamSynchronize(ctx->stream);
     for (Buf *b : {&ctx->base, &ctx->planes, &ctx->qplanes, &ctx->stage_dev, &ctx->iplanes, &ctx->iqplanes,
-                   &ctx->i_addr, &ctx->i_h2, &ctx->part, &ctx->result, &ctx->seg, &ctx->list, &ctx->flags, &ctx->counters})
+                   &ctx->i_addr, &ctx->i_h2, &ctx->part, &ctx->result, &ctx->seg, &ctx->list, &ctx->flags, &ctx->counters,
+                   &ctx->csr_len, &ctx->csr_bsum, &ctx->csr_off, &ctx->csr_list})
         dev_release(ctx, *b);
+    for (auto &e : ctx->ev_csr)
+        if (e) cudaEventDestroy(e);
     if (ctx->h_stage) cudaFreeHost(ctx->h_stage);
     if (ctx->h_io) cudaFreeHost(ctx->h_io);
     if (ctx->h_flags) cudaFreeHost(ctx->h_flags);
@@ -280,6 +323,18 @@ extern "C" int s2_close(s2_ctx *ctx)
     if (ctx->h_res) cudaFreeHost(ctx->h_res);
     for (auto &e : ctx->ev_t)
         if (e) cudaEventDestroy(e);
+    {   // the last context of a device releases what the device's contexts share (bank hand-over words, event)
+        std::lock_guard<std::mutex> lock(g_bank_mu);
+        auto it = g_bank.find(ctx->device);
+        if (it != g_bank.end() && --it->second.refs <= 0) {
+            if (it->second.used) cudaEventSynchronize(it->second.ev);
+            if (it->second.flags) cudaFree(it->second.flags);
+            if (it->second.ev) cudaEventDestroy(it->second.ev);
+            const int mode = it->second.mode;
+            g_bank.erase(it);
+            g_bank[ctx->device].mode = mode;   // the verdict of the self-test is a property of device + driver: kept
+        }
+    }
     cudaGetLastError();
     delete ctx;
     return S2_OK;
@@ -391,7 +446,8 @@ extern "C" int s2_commit_j_device(s2_ctx *ctx, int n, const int *d_address, cons
 {
     if (!ctx || n < 0) return S2_EINVAL;
     if (n == 0) return S2_OK;
-    if (!d_address || !d_id || !d_t || !d_mass || !d_pos || !d_vel || !d_acc || !d_jerk) return S2_EINVAL;
+    if (!d_address || !d_id || !d_t || !d_mass || !d_pos || !d_vel) return S2_EINVAL;
+    if (ctx->order != 2 && (!d_acc || !d_jerk)) return S2_EINVAL;   // 2nd order: missing derivatives are stored as zero (as s2_set_j)
     if (ctx->order == 6 && (!d_snap || !d_crackle)) return S2_EINVAL;
     if (n > ctx->nj_cap) return S2_ERANGE;
     CU(cudaSetDevice(ctx->device));
@@ -403,7 +459,7 @@ extern "C" int s2_commit_j_device(s2_ctx *ctx, int n, const int *d_address, cons
     const double *vecs[6] = {d_pos, d_vel, d_acc, d_jerk, d_snap, d_crackle};
     const int nvec = ctx->order == 6 ? 6 : 4;
     for (int v = 0; v < nvec; ++v)
-        for (int c = 0; c < 3; ++c) a.src[2 + 3 * v + c] = vecs[v] + c;
+        for (int c = 0; c < 3; ++c) a.src[2 + 3 * v + c] = vecs[v] ? vecs[v] + c : nullptr;
     const int nf = nfields(ctx->order);
     for (int k = 0; k < nf; ++k) a.dst[k] = base_field(ctx, k);
     a.dst_id = base_id(ctx);
@@ -647,15 +703,6 @@ static int choose_shape(s2_ctx *ctx, int ni, int nj, unsigned flags, ForceShape 
 // ---- a4 at the largest n_i: the uniform-operand sweep (force_sweep_bank_kernel, s2_force_fp64.cu) -----------
 // The constant bank is one per device and module, shared by every context of the process: a sweep that uses it
 // on another stream first waits for the event the previous user recorded after its last chunk.
-struct BankOwner {
-    cudaEvent_t ev = nullptr;
-    cudaStream_t stream = nullptr;
-    bool used = false;
-    unsigned *flags = nullptr;   // device words {ready[2], -, -, arrived[2]} of the bank hand-over (run_force_bank)
-    unsigned ticket = 0;         // tickets handed out so far (chunk sequence numbers, cyclic)
-};
-static std::mutex g_bank_mu;
-static std::map<int, BankOwner> g_bank;
 
 // When the chunked sweep beats the shared-memory one (measured on B200 at N = 2^18, fp64 4th order, Gpairs/s
 // bank / shared-memory): n_i = 49152: 481 / 488, 57344: 492 / 487, 61440: 502 / 489, 65536: 506 / 489, 81920: 510 / 489,
@@ -668,7 +715,8 @@ static std::map<int, BankOwner> g_bank;
 static bool bank_applies(const s2_ctx *ctx, int ni, int nj)
 {
     if (ctx->precision != S2_FP64 || ctx->tune[8] == 1) return false;
-    if (ctx->tune[8] >= 2) return true;   // 3: forced, without overlapping launches (A/B measurements)
+    if (ctx->tune[8] >= 2) return true;   // 3: forced, without overlapping launches (A/B measurements); 4: forced, refilled
+                                          // by stream-ordered copies (the documented-semantics fallback)
     for (int k = 0; k < 8; ++k)
         if (ctx->tune[k]) return false;   // an explicit launch shape was asked for
     return ctx->order == 4 && nj >= 8192 && ni >= 48000;
@@ -684,7 +732,7 @@ static cudaError_t dispatch_bank(int b, int order, unsigned flags, const ForceAr
 // swept and publishes ready[bank] = ticket(c + 2) (see force_sweep_bank_kernel).  Nothing but kernels sits in the
 // stream, so the launches carry programmatic stream serialisation and overlap: the next one fills the SMs while this
 // one drains (event-ordered refills: 498 Gpairs/s at n_i = 2^18; overlapped: 512).
-static int run_force_bank(s2_ctx *ctx, ForceArgs &a, int ni, unsigned flags)
+static int run_force_bank(s2_ctx *ctx, ForceArgs &a, int ni, unsigned flags, int mode)
 {
     int geom[3] = {0, 0, 0};
     CU(dispatch_bank(0, ctx->order, flags, a, ctx->stream, geom));
@@ -698,7 +746,7 @@ static int run_force_bank(s2_ctx *ctx, ForceArgs &a, int ni, unsigned flags)
     // CTAs of 128 threads (4 per SM) fill the rounds that consecutive launches share more finely; measured at N = 2^18
     // (128 / 256 threads, Gpairs/s): n_i = 49152: 502 / 481, 65536: 512 / 506, 81920: 514 / 510, 131072: 518 / 517,
     // 262144: 516 / 518.  Launches with decisions do not share rounds (they wait at their start): 256.
-    const int threads = (flags == 0 && ctx->order == 4 && ni < 200000 && ctx->tune[8] != 3) ? 128 : geom[1];
+    const int threads = (flags == 0 && ctx->order == 4 && ni < 200000 && ctx->tune[8] != 3 && mode == kBankSelfRefill) ? 128 : geom[1];
     a.bank_threads = threads;
     a.bank_state = (double *)ctx->part.p;
     a.is_final = 1;
@@ -715,9 +763,9 @@ static int run_force_bank(s2_ctx *ctx, ForceArgs &a, int ni, unsigned flags)
     std::lock_guard<std::mutex> lock(g_bank_mu);
     BankOwner &own = g_bank[ctx->device];
     if (!own.ev) CU(cudaEventCreateWithFlags(&own.ev, cudaEventDisableTiming));
-    if (!own.flags) {
+    if (!own.flags) {   // 64 bytes shared by every context of the device (not a context's buffer): freed by the last s2_close
         CU(cudaMalloc((void **)&own.flags, 64));
-        CU(cudaMemset(own.flags, 0, 64));
+        CU(cudaMemsetAsync(own.flags, 0, 64, ctx->stream));   // ordered before this stream's first sweep; others wait on own.ev
     }
     // inside a stream capture (CUDA graph) events cannot tie the graph to work outside it: the caller orders
     // replays of such a graph against other users of the banks himself
@@ -727,18 +775,21 @@ static int run_force_bank(s2_ctx *ctx, ForceArgs &a, int ni, unsigned flags)
     if (!capturing && own.used && own.stream != ctx->stream) CU(cudaStreamWaitEvent(ctx->stream, own.ev, 0));
     if (ctx->timing) CU(cudaEventRecord(ctx->ev_t[2], ctx->stream));
     const unsigned base = own.ticket;
-    own.ticket += (unsigned)nchunks;
-    for (int c = 0; c < std::min(2, nchunks); ++c) {   // the first two chunks; the later ones are copied by the kernels
+    if (mode == kBankSelfRefill) own.ticket += (unsigned)nchunks;
+    auto copy_chunk = [&](int c) -> cudaError_t {   // chunk c of every plane -> bank c & 1, in stream order
         const int cnt = std::min(chunk, nj - c * chunk);
-        if (equal_stride) {   // one strided copy moves the chunk of every plane
-            CU(cudaMemcpy2DAsync(bank[c], (size_t)chunk * sizeof(double2), (const double2 *)a.jp[0] + c * chunk, pitch,
-                                 (size_t)cnt * sizeof(double2), npl, cudaMemcpyDeviceToDevice, ctx->stream));
-        } else {
-            for (int p = 0; p < npl; ++p)
-                CU(cudaMemcpyAsync((double2 *)bank[c] + (size_t)p * chunk, (const double2 *)a.jp[p] + c * chunk,
-                                   (size_t)cnt * sizeof(double2), cudaMemcpyDeviceToDevice, ctx->stream));
+        if (equal_stride)   // one strided copy moves the chunk of every plane
+            return cudaMemcpy2DAsync(bank[c & 1], (size_t)chunk * sizeof(double2), (const double2 *)a.jp[0] + (size_t)c * chunk, pitch,
+                                     (size_t)cnt * sizeof(double2), npl, cudaMemcpyDeviceToDevice, ctx->stream);
+        for (int p = 0; p < npl; ++p) {
+            cudaError_t e = cudaMemcpyAsync((double2 *)bank[c & 1] + (size_t)p * chunk, (const double2 *)a.jp[p] + (size_t)c * chunk,
+                                            (size_t)cnt * sizeof(double2), cudaMemcpyDeviceToDevice, ctx->stream);
+            if (e != cudaSuccess) return e;
         }
-    }
+        return cudaSuccess;
+    };
+    if (mode == kBankSelfRefill)
+        for (int c = 0; c < std::min(2, nchunks); ++c) CU(copy_chunk(c));   // the later chunks are copied by the kernels
     // launch -1 sweeps nothing: it gathers the i-particles, parks them and zeroes the running state, so that every
     // chunk launch finds its inputs complete and may overlap its predecessor
     a.bank_j0 = 0; a.bank_cnt = 0; a.bank_first = 1; a.bank_last = 0; a.bank_pdl = 0; a.bank_wait_early = 0;
@@ -754,6 +805,16 @@ static int run_force_bank(s2_ctx *ctx, ForceArgs &a, int ni, unsigned flags)
         a.bank_first = 0;
         a.bank_last = c == nchunks - 1;
         a.bank_id = b;
+        if (mode == kBankHostRefill) {
+            // Documented semantics only: the bank is written by a stream-ordered copy between two ordinary launches
+            // (the copy follows the launch of chunk c - 2, the last reader of this bank, and precedes this launch).
+            CU(copy_chunk(c));
+            a.bank_flags = nullptr; a.bank_ticket = 0; a.bank_spin = 0; a.bank_next_known = 1; a.bank_self = nullptr;
+            a.bank_next_j0 = 0; a.bank_next_cnt = 0; a.bank_pdl = 0; a.bank_wait_early = 0;
+            CU(dispatch_bank(b, ctx->order, flags, a, ctx->stream, nullptr));
+            ctx->launches++;
+            continue;
+        }
         a.bank_flags = own.flags;
         a.bank_ticket = base + (unsigned)c + 1u;
         a.bank_spin = c >= 2;
@@ -774,8 +835,89 @@ static int run_force_bank(s2_ctx *ctx, ForceArgs &a, int ni, unsigned flags)
     }
 
     int *li = ctx->last_info;
-    li[0] = nchunks; li[1] = 1; li[2] = 1; li[3] = (ni + threads - 1) / threads; li[4] = threads; li[5] = 0; li[6] = 3;
+    li[0] = nchunks; li[1] = 1; li[2] = 1; li[3] = (ni + threads - 1) / threads; li[4] = threads; li[5] = 0;
+    li[6] = mode == kBankSelfRefill ? 3 : 5;
     li[7] = geom[2] * geom[1] / threads; li[8] = 1; li[9] = 1;
+    return S2_OK;
+}
+
+static int run_force(s2_ctx *ctx, int ni, const int *d_i_addr, const double *d_h2, bool explicit_i, double eps2,
+                     unsigned flags, bool host_call);
+
+// First use of the self-refilling sweep on a device: run it once next to the shared-memory sweep on (a part of) the
+// caller's own problem -- at least three chunks, so that the last-CTA refill, the ticket hand-over and the
+// overlapping launches are all exercised -- and compare every record.  The self-refill writes the constant bank from
+// device code and relies on the next launch seeing the new contents; CUDA documents neither, so the
+// library only keeps using it where it has just seen it work, and otherwise falls back for good to refilling the banks
+// with stream-ordered copies between ordinary launches (documented semantics, measured ~4 % slower).
+static int bank_selftest(s2_ctx *ctx, int ni, const int *d_i_addr, bool explicit_i, double eps2, bool *ok)
+{
+    const int nj_save = ctx->nj_pred, t8 = ctx->tune[8];
+    const int ni_t = std::min(ni, 65536);
+    const int nj_t = std::min(nj_save, 8 * 1024);
+    *ok = false;
+    Buf ref;
+    int rc = dev_reserve(ctx, ref, (size_t)ni_t * REC * sizeof(double));
+    if (rc != S2_OK) return rc;
+    ctx->in_selftest = true;
+    ctx->nj_pred = nj_t;
+    ctx->tune[8] = 1;
+    rc = run_force(ctx, ni_t, d_i_addr, nullptr, explicit_i, eps2, 0, false);
+    if (rc == S2_OK) {
+        cudaError_t e = cudaMemcpyAsync(ref.p, ctx->result.p, (size_t)ni_t * REC * sizeof(double), cudaMemcpyDeviceToDevice, ctx->stream);
+        if (e != cudaSuccess) rc = fail_cuda(ctx, e);
+    }
+    ctx->tune[8] = 2;
+    for (int rep = 0; rep < 2 && rc == S2_OK; ++rep) {   // twice back to back: the second sweep starts on banks the first one left
+        rc = run_force(ctx, ni_t, d_i_addr, nullptr, explicit_i, eps2, 0, false);
+        if (rc == S2_OK) {
+            cudaError_t e = launch_compare_records((const double *)ref.p, (const double *)ctx->result.p, ni_t, ctx->order, 1e-11,
+                                                   (int *)ctx->flags.p + 2, ctx->stream);
+            if (e != cudaSuccess) rc = fail_cuda(ctx, e);
+            ctx->launches++;
+        }
+    }
+    ctx->tune[8] = t8;
+    ctx->nj_pred = nj_save;
+    ctx->in_selftest = false;
+    ctx->calc_done = false;
+    if (rc == S2_OK) {
+        cudaError_t e = cudaMemcpyAsync(ctx->h_flags + 2, (int *)ctx->flags.p + 2, sizeof(int), cudaMemcpyDeviceToHost, ctx->stream);
+        if (e == cudaSuccess) e = cudaStreamSynchronize(ctx->stream);
+        if (e == cudaSuccess) e = cudaMemsetAsync((int *)ctx->flags.p + 2, 0, sizeof(int), ctx->stream);
+        if (e != cudaSuccess) rc = fail_cuda(ctx, e);
+        else *ok = ctx->h_flags[2] == 0;
+    }
+    dev_release(ctx, ref);
+    return rc;
+}
+
+static int bank_choose_mode(s2_ctx *ctx, int ni, const int *d_i_addr, bool explicit_i, double eps2, int *mode)
+{
+    if (ctx->in_selftest) { *mode = kBankSelfRefill; return S2_OK; }
+    if (ctx->tune[8] == 4) { *mode = kBankHostRefill; return S2_OK; }
+    int m;
+    {
+        std::lock_guard<std::mutex> lock(g_bank_mu);
+        m = g_bank[ctx->device].mode;
+    }
+    if (m == 0) {
+        // a sweep of at most two chunks never refills a bank from a kernel (the host copies both): nothing to verify yet
+        int geom[3] = {0, 0, 0};
+        ForceArgs dummy{};
+        CU(dispatch_force_fp64_bank0(ctx->order, 0, dummy, ctx->stream, geom));
+        if (ctx->nj_pred <= 2 * geom[0]) { *mode = kBankSelfRefill; return S2_OK; }
+        cudaStreamCaptureStatus cap = cudaStreamCaptureStatusNone;
+        CU(cudaStreamIsCapturing(ctx->stream, &cap));
+        if (cap != cudaStreamCaptureStatusNone) { *mode = kBankHostRefill; return S2_OK; }   // cannot test inside a capture
+        bool ok = false;
+        int rc = bank_selftest(ctx, ni, d_i_addr, explicit_i, eps2, &ok);
+        if (rc != S2_OK) return rc;
+        m = ok ? kBankSelfRefill : kBankHostRefill;
+        std::lock_guard<std::mutex> lock(g_bank_mu);
+        g_bank[ctx->device].mode = m;
+    }
+    *mode = m;
     return S2_OK;
 }
 
@@ -791,6 +933,12 @@ static int run_force(s2_ctx *ctx, int ni, const int *d_i_addr, const double *d_h
     const bool bank = bank_applies(ctx, ni, ctx->nj_pred);
     ForceShape sh{};
     int rc = S2_OK;
+    ctx->csr_valid = false;
+    int bank_mode = 0;
+    if (bank) {
+        rc = bank_choose_mode(ctx, ni, d_i_addr, explicit_i, eps2, &bank_mode);
+        if (rc != S2_OK) return rc;
+    }
     if (bank) {   // one lane per i, one "slice": the chunks of the constant bank are swept launch by launch
         sh.L = 1; sh.Wj = 1; sh.S = 1; sh.slice_len = ctx->nj_pred; sh.tile = 256; sh.stages = 2; sh.cluster = 1;
         rc = dev_reserve(ctx, ctx->part, (size_t)ni * (REC + 10) * sizeof(double));   // running sums + parked i-state
@@ -899,7 +1047,7 @@ static int run_force(s2_ctx *ctx, int ni, const int *d_i_addr, const double *d_h
 
     if (want_ngb) CU(cudaMemsetAsync(ctx->flags.p, 0, sizeof(int), ctx->stream));   // overflow flag of this call
     if (bank) {
-        rc = run_force_bank(ctx, a, ni, flags);
+        rc = run_force_bank(ctx, a, ni, flags, bank_mode);
         if (rc != S2_OK) return rc;
         ctx->ran_force = true;
         ctx->ran_reduce = false;
@@ -1149,6 +1297,19 @@ extern "C" int s2_get_results(s2_ctx *ctx, int ni, double *acc, double *jerk, do
     return post_sync_status(ctx);
 }
 
+extern "C" int s2_get_results_device(s2_ctx *ctx, int ni, double *d_acc, double *d_jerk, double *d_snap, double *d_pot,
+                                     int *d_nn_id, double *d_nn_r2, int *d_ngb_count)
+{
+    if (!ctx || ni < 0) return S2_EINVAL;
+    if (!ctx->calc_done) return S2_ESTATE;
+    if (ni > ctx->ni_last) return S2_ERANGE;
+    CU(cudaSetDevice(ctx->device));
+    const double *rec = (const double *)(ctx->res_on_host ? ctx->h_res : ctx->result.p);
+    CU(launch_unpack_records(rec, ni, ctx->order, d_acc, d_jerk, d_snap, d_pot, d_nn_id, d_nn_r2, d_ngb_count, ctx->stream));
+    ctx->launches++;
+    return S2_OK;
+}
+
 extern "C" int s2_get_neighbours(s2_ctx *ctx, int i, int cap, int *n_out, int *list)
 {
     if (!ctx || !n_out || cap < 0 || (cap > 0 && !list)) return S2_EINVAL;
@@ -1174,40 +1335,109 @@ extern "C" int s2_get_neighbours(s2_ctx *ctx, int i, int cap, int *n_out, int *l
     return packed[1] > ctx->ngb_cap ? S2_EOVERFLOW : S2_OK;
 }
 
+// Compacts the fixed-stride lists of the last force call into CSR form on the device (count -> scan -> fill) and
+// caches the result until the next s2_calc_*.  One 8-byte read-back (the total) sits between scan and fill.
+static int build_csr(s2_ctx *ctx)
+{
+    if (ctx->csr_valid) return S2_OK;
+    const int ni = ctx->ni_last;
+    const int nb = csr_blocks(ni);
+    int rc = dev_reserve(ctx, ctx->csr_len, (size_t)ni * sizeof(int));
+    if (rc == S2_OK) rc = dev_reserve(ctx, ctx->csr_bsum, (size_t)(nb + 1) * sizeof(long long));
+    if (rc == S2_OK) rc = dev_reserve(ctx, ctx->csr_off, (size_t)(ni + 1) * sizeof(long long));
+    if (rc != S2_OK) return rc;
+    const double *rec = (const double *)(ctx->res_on_host ? ctx->h_res : ctx->result.p);   // pinned records are device-readable
+    long long *bsum = (long long *)ctx->csr_bsum.p, *d_total = bsum + nb;
+    long long *h_total = (long long *)(ctx->h_flags + 4);
+    if (ctx->timing) CU(cudaEventRecord(ctx->ev_csr[0], ctx->stream));
+    CU(launch_csr_scan(rec, ni, ctx->ngb_cap, (int *)ctx->csr_len.p, bsum, d_total, (long long *)ctx->csr_off.p, ctx->stream));
+    if (ctx->timing) CU(cudaEventRecord(ctx->ev_csr[1], ctx->stream));
+    ctx->launches += 3;
+    CU(cudaMemcpyAsync(h_total, d_total, sizeof(long long), cudaMemcpyDeviceToHost, ctx->stream));
+    rc = fetch_flags(ctx);
+    if (rc != S2_OK) return rc;
+    CU(cudaStreamSynchronize(ctx->stream));
+    ctx->csr_total = *h_total;
+    rc = dev_reserve(ctx, ctx->csr_list, (size_t)std::max<long long>(ctx->csr_total, 1) * sizeof(int));
+    if (rc != S2_OK) return rc;
+    if (ctx->timing) CU(cudaEventRecord(ctx->ev_csr[2], ctx->stream));
+    if (ctx->csr_total > 0) {
+        CU(launch_csr_fill((const int *)ctx->list.p, (const int *)ctx->csr_len.p, (const long long *)ctx->csr_off.p, ni,
+                           ctx->ngb_cap, (int *)ctx->csr_list.p, ctx->stream));
+        ctx->launches++;
+    }
+    if (ctx->timing) CU(cudaEventRecord(ctx->ev_csr[3], ctx->stream));
+    ctx->ran_csr = true;
+    ctx->csr_valid = true;
+    return S2_OK;
+}
+
 extern "C" int s2_get_neighbours_csr(s2_ctx *ctx, int ni, long long *offsets, int *list, long long list_cap)
 {
     if (!ctx || ni < 0 || !offsets || list_cap < 0) return S2_EINVAL;
     if (!ctx->calc_done || !(ctx->flags_last & S2_WANT_NGB)) return S2_ESTATE;
     if (ni > ctx->ni_last) return S2_ERANGE;
     CU(cudaSetDevice(ctx->device));
-    // counts come from the result records, lists from the fixed-stride device buffer
-    const size_t b_rec = align16((size_t)ni * REC * sizeof(double));
-    const size_t b_list = (size_t)ni * ctx->ngb_cap * sizeof(int);
-    CU(cudaEventSynchronize(ctx->ev_io));
-    int rc = pinned_reserve(ctx, &ctx->h_io, &ctx->h_io_bytes, 0, b_rec + b_list);
+    int rc = build_csr(ctx);
     if (rc != S2_OK) return rc;
-    if (ni) {
-        if (!ctx->res_on_host)
-            CU(cudaMemcpyAsync(ctx->h_io, ctx->result.p, (size_t)ni * REC * sizeof(double), cudaMemcpyDeviceToHost, ctx->stream));
-        CU(cudaMemcpyAsync((char *)ctx->h_io + b_rec, ctx->list.p, b_list, cudaMemcpyDeviceToHost, ctx->stream));
-    }
+    // offsets and (when the caller's list can hold every member) the compacted list in one go; a prefix request
+    // (ni < n_i of the call) may need fewer members than csr_total, which offsets[ni] then says
+    const size_t b_off = align16((size_t)(ni + 1) * sizeof(long long));
+    const bool with_list = list && list_cap >= ctx->csr_total && ctx->csr_total > 0;
+    CU(cudaEventSynchronize(ctx->ev_io));
+    rc = pinned_reserve(ctx, &ctx->h_io, &ctx->h_io_bytes, 0, b_off + (with_list ? (size_t)ctx->csr_total * sizeof(int) : 0));
+    if (rc != S2_OK) return rc;
+    CU(cudaMemcpyAsync(ctx->h_io, ctx->csr_off.p, (size_t)(ni + 1) * sizeof(long long), cudaMemcpyDeviceToHost, ctx->stream));
+    if (with_list)
+        CU(cudaMemcpyAsync((char *)ctx->h_io + b_off, ctx->csr_list.p, (size_t)ctx->csr_total * sizeof(int), cudaMemcpyDeviceToHost,
+                           ctx->stream));
     CU(cudaStreamSynchronize(ctx->stream));
-    const double *r = (const double *)(ctx->res_on_host ? ctx->h_res : ctx->h_io);
-    const int *L = (const int *)((const char *)ctx->h_io + b_rec);
-    long long tot = 0;
-    bool overflow = false;
-    for (int k = 0; k < ni; ++k) {
-        int packed[2];
-        memcpy(packed, &r[(size_t)k * REC + 8], sizeof packed);
-        offsets[k] = tot;
-        if (packed[1] > ctx->ngb_cap) overflow = true;
-        tot += std::min(packed[1], ctx->ngb_cap);
-    }
-    offsets[ni] = tot;
+    par_memcpy(offsets, ctx->h_io, (size_t)(ni + 1) * sizeof(long long));
+    const long long tot = offsets[ni];
     if (tot > list_cap || (tot > 0 && !list)) return S2_ERANGE;
-    for (int k = 0; k < ni; ++k)
-        memcpy(list + offsets[k], L + (size_t)k * ctx->ngb_cap, (size_t)(offsets[k + 1] - offsets[k]) * sizeof(int));
-    return overflow ? S2_EOVERFLOW : S2_OK;
+    if (tot > 0) {
+        if (!with_list) {   // prefix request with a list shorter than the whole call's: copy just the prefix
+            rc = pinned_reserve(ctx, &ctx->h_io, &ctx->h_io_bytes, 0, b_off + (size_t)tot * sizeof(int));
+            if (rc != S2_OK) return rc;
+            CU(cudaMemcpyAsync((char *)ctx->h_io + b_off, ctx->csr_list.p, (size_t)tot * sizeof(int), cudaMemcpyDeviceToHost, ctx->stream));
+            CU(cudaStreamSynchronize(ctx->stream));
+        }
+        par_memcpy(list, (const char *)ctx->h_io + b_off, (size_t)tot * sizeof(int));
+    }
+    return ctx->h_flags[0] ? S2_EOVERFLOW : S2_OK;
+}
+
+extern "C" int s2_get_neighbours_csr_device(s2_ctx *ctx, int ni, const long long **d_offsets, const int **d_list, long long *total)
+{
+    if (!ctx || ni < 0 || !d_offsets || !d_list || !total) return S2_EINVAL;
+    if (!ctx->calc_done || !(ctx->flags_last & S2_WANT_NGB)) return S2_ESTATE;
+    if (ni > ctx->ni_last) return S2_ERANGE;
+    CU(cudaSetDevice(ctx->device));
+    int rc = build_csr(ctx);
+    if (rc != S2_OK) return rc;
+    *d_offsets = (const long long *)ctx->csr_off.p;
+    *d_list = (const int *)ctx->csr_list.p;
+    *total = ctx->csr_total;
+    if (ni < ctx->ni_last) {
+        long long *h = (long long *)(ctx->h_flags + 4);
+        CU(cudaMemcpyAsync(h, (const long long *)ctx->csr_off.p + ni, sizeof(long long), cudaMemcpyDeviceToHost, ctx->stream));
+        CU(cudaStreamSynchronize(ctx->stream));
+        *total = *h;
+    }
+    return ctx->h_flags[0] ? S2_EOVERFLOW : S2_OK;
+}
+
+extern "C" int s2_get_csr_timing(s2_ctx *ctx, float *scan_ms, float *fill_ms)
+{
+    if (!ctx) return S2_EINVAL;
+    if (!ctx->timing || !ctx->ran_csr) return S2_ESTATE;
+    CU(cudaStreamSynchronize(ctx->stream));
+    float a = 0.f, b = 0.f;
+    CU(cudaEventElapsedTime(&a, ctx->ev_csr[0], ctx->ev_csr[1]));
+    CU(cudaEventElapsedTime(&b, ctx->ev_csr[2], ctx->ev_csr[3]));
+    if (scan_ms) *scan_ms = a;
+    if (fill_ms) *fill_ms = b;
+    return S2_OK;
 }
 
 // ---- hooks and diagnostics ----------------------------------------------------------------

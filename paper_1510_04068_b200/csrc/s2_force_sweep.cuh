@@ -25,6 +25,8 @@
 
 #include <math_constants.h>
 
+#include <atomic>
+
 #include "s2_force_common.cuh"
 
 namespace s2 {
@@ -527,6 +529,25 @@ __global__ void __launch_bounds__(kThreads, P::kMinBlocksTiled) force_sweep_tile
     }
 }
 
+// Dynamic shared memory above 48 KB needs an opt-in that is per kernel AND per device.  Each kernel is opted in once
+// per device to that device's full limit (idempotent, so contexts on different threads may race here harmlessly; a
+// process-wide "largest size so far" would leave the kernels of a second device without their opt-in).
+constexpr int kMaxDevices = 64;
+template <class K>
+inline cudaError_t opt_in_smem(K kern, std::atomic<int> *done)
+{
+    int dev = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return e;
+    if (dev < 0 || dev >= kMaxDevices) return cudaErrorInvalidDevice;
+    if (done[dev].load(std::memory_order_acquire)) return cudaSuccess;
+    int lim = 0;
+    e = cudaDeviceGetAttribute(&lim, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, lim);
+    if (e == cudaSuccess) done[dev].store(1, std::memory_order_release);
+    return e;
+}
+
 // Host side: instantiate the kernel for a policy and launch it (or query its occupancy) for the
 // run-time lane count L.
 template <class P>
@@ -536,12 +557,8 @@ cudaError_t launch_L(int L, dim3 grid, size_t smem, const ForceArgs &a, cudaStre
 #define S2_CASE(LL)                                                                                          \
     case LL: {                                                                                               \
         auto kern = force_sweep_kernel<P, LL>;                                                               \
-        static int s_smem_attr = 0;   /* largest dynamic shared memory size this kernel was opted into */   \
-        if ((int)smem > s_smem_attr) {                                                                       \
-            cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem); \
-            if (e != cudaSuccess) return e;                                                                  \
-            s_smem_attr = (int)smem;                                                                         \
-        }                                                                                                    \
+        static std::atomic<int> s_opted[kMaxDevices];                                                        \
+        if (cudaError_t e = opt_in_smem(kern, s_opted); e != cudaSuccess) return e;                          \
         if (query) return cudaOccupancyMaxActiveBlocksPerMultiprocessor(ctas_per_sm, kern, kThreads, smem);  \
         if (a.cluster > 1) {                                                                                 \
             cudaLaunchConfig_t cfg = {};                                                                     \
@@ -558,12 +575,8 @@ cudaError_t launch_L(int L, dim3 grid, size_t smem, const ForceArgs &a, cudaStre
     if (L == 0) {   // register-tiled full-occupancy sweep, P::kIPT i-particles per thread
         if constexpr (P::kIPT >= 2) {
             auto kern = force_sweep_tiled_kernel<P, P::kIPT>;
-            static int s_smem_attr = 0;
-            if ((int)smem > s_smem_attr) {
-                cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-                if (e != cudaSuccess) return e;
-                s_smem_attr = (int)smem;
-            }
+            static std::atomic<int> s_opted[kMaxDevices];
+            if (cudaError_t e = opt_in_smem(kern, s_opted); e != cudaSuccess) return e;
             if (query) return cudaOccupancyMaxActiveBlocksPerMultiprocessor(ctas_per_sm, kern, kThreads, smem);
             kern<<<grid, kThreads, smem, st>>>(a);
             return cudaGetLastError();

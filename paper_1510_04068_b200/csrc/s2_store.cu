@@ -23,7 +23,8 @@ __global__ void __launch_bounds__(256) scatter_kernel(ScatterArgs a)
         if (f < a.nfields) {
             // scalars (t, m): plain length-n arrays; vector components: (n,3) row-major, src already offset by the
             // component, so the three loads of a thread cover one contiguous 24-byte row
-            const double v = f < 2 ? a.src[f][p] : a.src[f][(size_t)3 * p];
+            // a missing field (2nd-order context committed without acc / jerk) is stored as zero
+            const double v = !a.src[f] ? 0.0 : (f < 2 ? a.src[f][p] : a.src[f][(size_t)3 * p]);
             a.dst[f][addr] = v;
         }
     }

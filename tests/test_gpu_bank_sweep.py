@@ -8,7 +8,7 @@ import oracle
 import paper_1510_04068_b200 as s2
 from workloads import lattice_workload, make_config
 
-from gpu_util import TOL, check_neighbour_lists, open_and_load, rel_err
+from gpu_util import TOL, check_neighbour_lists, check_nn_ld, open_and_load, rel_err
 
 pytestmark = pytest.mark.gpu
 
@@ -57,6 +57,7 @@ def test_bank_sweep_parity_all_chunkings(order):
                 else:
                     assert not res["acc"].any() and res["pot"][0] == 0.0, what
                 if flags:
+                    check_nn_ld(res, ref, what)      # primary: the oracle's long-double decision (north_star's band)
                     assert np.array_equal(res["nn_id"], ref.nn_id) and np.array_equal(res["nn_r2"], ref.nn_d2), what
                 if flags & NGB:
                     assert np.array_equal(res["ngb_count"], ref.ngb_count), what
@@ -84,6 +85,7 @@ def test_bank_sweep_explicit_sinks_and_lattice_ties():
     res = s2.s2_get_results(ctx, ni)
     ref = oracle.forces(4, w.mass, w.ident, xp, vp, None, ident, pos, vel, None, w.eps2, h2, 16)
     assert rel_err(res["acc"], ref.acc).max() <= 1e-13 and rel_err(res["jerk"], ref.jerk).max() <= 1e-12
+    check_nn_ld(res, ref, "explicit sinks, bank sweep")
     assert np.array_equal(res["nn_id"], ref.nn_id) and np.array_equal(res["ngb_count"], ref.ngb_count)
     check_neighbour_lists(ctx, ref, ni, 16, "explicit sinks, bank sweep")
     s2.s2_close(ctx)
@@ -99,6 +101,7 @@ def test_bank_sweep_explicit_sinks_and_lattice_ties():
     s2.s2_calc_ilist(ctx, il, h2, w.eps2, NN | NGB)
     res = s2.s2_get_results(ctx, w.N)
     ref = oracle.forces_ilist(4, w.mass, w.ident, xp, vp, None, il, w.eps2, h2, 32)
+    check_nn_ld(res, ref, "lattice, bank sweep")
     assert np.array_equal(res["nn_id"], ref.nn_id) and np.array_equal(res["nn_r2"], ref.nn_d2)
     assert np.array_equal(res["ngb_count"], ref.ngb_count)
     check_neighbour_lists(ctx, ref, w.N, 32, "lattice, bank sweep")
@@ -183,4 +186,113 @@ def test_bank_sweep_overlapping_launches_at_residency_boundaries():
                 assert np.array_equal(a[k], b[k]), (ni, flags, k)
             assert rel_err(a["acc"], ref["acc"]).max() < 1e-13 and rel_err(a["jerk"], ref["jerk"]).max() < 1e-12
             assert np.array_equal(a["nn_id"], ref["nn_id"])
+    s2.s2_close(ctx)
+
+
+@pytest.mark.timeout(900)
+@pytest.mark.parametrize("N,reps", [(8192, 30), (65536, 15), (262144, 5)])
+def test_bank_sweep_stress_changing_jstore_back_to_back(N, reps):
+    """The self-refilling uniform-operand sweep rewrites its constant banks from device code and overlaps its chunk
+    launches (DESIGN.md 5.2 states what that assumes).  Stress: 4 x reps sweeps per N (200 over the three N), enqueued
+    BACK TO BACK WITHOUT ANY HOST SYNCHRONISATION, the j-store changing between consecutive sweeps (alternating
+    s2_predict times, and half-way a partial s2_commit_j_device), at the sizes where the automatic rule picks this
+    sweep -- n_i = 49152, 65536, 131072 (128-thread instance) and 262144 (256-thread instance).  Every i of every
+    sweep is compared with the shared-memory sweep of the same j-state (acc, pot 1e-13, jerk 1e-12), and sweeps of
+    the same state must agree bit for bit: a stale bank, a chunk read before its refill or a constant-cache line
+    surviving a launch would show up as a wrong chunk of j in some sweep."""
+    import torch
+    w = make_config("H" if N == 262144 else 3, N=N)
+    ctx = open_and_load(w)
+    dev = torch.device("cuda", 0)
+    rng = np.random.default_rng(N)
+    # partial commit: every 5th particle moves a little (device arrays: nothing synchronises)
+    sub = np.arange(0, N, 5, dtype=np.int32)
+    T = lambda a: torch.from_numpy(np.ascontiguousarray(a)).to(dev)
+    orig = [T(sub), T(w.ident[sub]), T(w.t_j[sub]), T(w.mass[sub]), T(w.pos[sub]), T(w.vel[sub]), T(w.acc[sub]), T(w.jerk[sub])]
+    moved = list(orig)
+    moved[4] = T(w.pos[sub] + 0.03125 * w.vel[sub])
+    moved[3] = T(w.mass[sub] * 1.5)
+    times = {"A": w.t_pred, "B": w.t_pred + 2.0 ** -9, "C": w.t_pred, "D": w.t_pred + 2.0 ** -9}
+
+    def enqueue(state, il, out):
+        s2.s2_predict(ctx, times[state], N)
+        s2.s2_calc_ilist_device(ctx, il, None, w.eps2, 0)
+        s2.s2_get_results_device(ctx, il.numel(), acc=out[0], jerk=out[1], pot=out[2])
+
+    def buffers(ni):
+        return [torch.empty(ni * 3, dtype=torch.float64, device=dev), torch.empty(ni * 3, dtype=torch.float64, device=dev),
+                torch.empty(ni, dtype=torch.float64, device=dev)]
+
+    def rel(a, b, vec):
+        if vec:
+            a, b = a.view(-1, 3), b.view(-1, 3)
+            return float(((a - b).norm(dim=1) / b.norm(dim=1)).max())
+        return float(((a - b).abs() / b.abs()).max())
+
+    total = 0
+    for ni in (49152, 65536, 131072, 262144):
+        il = torch.from_numpy(rng.integers(0, N, ni).astype(np.int32)).to(dev)
+        # references: shared-memory sweep of each of the four j-states
+        s2.s2_set_tuning(ctx, 8, 1)
+        ref = {}
+        for st in "AB":
+            ref[st] = buffers(ni); enqueue(st, il, ref[st])
+        assert s2.s2_last_launch_info(ctx)["reduced"] not in (3, 5)
+        s2.s2_commit_j_device(ctx, *moved)
+        for st in "CD":
+            ref[st] = buffers(ni); enqueue(st, il, ref[st])
+        s2.s2_commit_j_device(ctx, *orig)
+        # the stress: automatic rule, no host synchronisation between the sweeps
+        s2.s2_set_tuning(ctx, 8, 0)
+        seq = [("AB"[k & 1]) for k in range(reps // 2)] + ["commit"] + [("CD"[k & 1]) for k in range(reps - reps // 2)]
+        outs = []
+        for st in seq:
+            if st == "commit":
+                s2.s2_commit_j_device(ctx, *moved)
+                continue
+            o = buffers(ni); enqueue(st, il, o); outs.append((st, o))
+        info = s2.s2_last_launch_info(ctx)
+        assert info["reduced"] == 3 and info["threads"] == (128 if ni < 200000 else 256), info
+        s2.s2_commit_j_device(ctx, *orig)
+        s2.s2_synchronize(ctx)
+        first = {}
+        for k, (st, o) in enumerate(outs):
+            what = f"N={N} n_i={ni} sweep {k} state {st}"
+            assert rel(o[0], ref[st][0], True) <= 1e-13, what
+            assert rel(o[1], ref[st][1], True) <= 1e-12, what
+            assert rel(o[2], ref[st][2], False) <= 1e-13, what
+            if st in first:
+                for a, b in zip(o, first[st]):
+                    assert torch.equal(a, b), what + ": differs from an earlier sweep of the same state"
+            else:
+                first[st] = o
+        assert rel(ref["A"][0], ref["C"][0], True) > 1e-6          # the partial commit really changed the forces
+        total += len(outs)
+        del outs, ref, first
+    assert total == 4 * reps
+    s2.s2_close(ctx)
+
+
+def test_bank_sweep_documented_fallback_has_the_same_bits():
+    """s2_set_tuning key 8 = 4: the banks are refilled by stream-ordered copies between ordinary launches (documented
+    CUDA semantics; the path the library falls back to for good if its first-use self-test of the self-refilling sweep
+    fails).  Same chunks, same order, same kernel: bit-identical records, decisions and lists."""
+    w = make_config(5, N=7000)
+    ctx = open_and_load(w, 4, ngb_cap=24)
+    s2.s2_predict(ctx, w.t_pred, w.N)
+    il = w.ilist(w.N)
+    h2 = w.h2[il]
+    for flags in (0, NN, NN | NGB):
+        got = {}
+        for key8, code in ((2, 3), (4, 5)):
+            s2.s2_set_tuning(ctx, 8, key8)
+            s2.s2_calc_ilist(ctx, il, h2 if flags & NGB else None, w.eps2, flags)
+            assert s2.s2_last_launch_info(ctx)["reduced"] == code
+            r = s2.s2_get_results(ctx, w.N)
+            lists = s2.s2_get_neighbours_csr(ctx, w.N) if flags & NGB else None
+            got[key8] = (r, lists)
+        for k in ("acc", "jerk", "pot") + (("nn_id", "nn_r2") if flags else ()) + (("ngb_count",) if flags & NGB else ()):
+            assert np.array_equal(got[2][0][k], got[4][0][k]), (flags, k)
+        if flags & NGB:
+            assert np.array_equal(got[2][1][0], got[4][1][0]) and np.array_equal(got[2][1][1], got[4][1][1])
     s2.s2_close(ctx)

@@ -8,12 +8,14 @@ import oracle
 import paper_1510_04068_b200 as s2
 from workloads import make_config, lattice_workload
 
-from gpu_util import check_forces, check_neighbour_lists, open_and_load, oracle_on_gpu_prediction, rel_err
+from gpu_util import (check_forces, check_neighbour_lists, check_nn_ld, check_sets_ld, open_and_load,
+                      oracle_on_gpu_prediction, rel_err)
 
 pytestmark = pytest.mark.gpu
 
 NN, NGB = s2.S2_WANT_NN, s2.S2_WANT_NGB
 PREC = {"ds": s2.S2_DS, "fp32": s2.S2_FP32}
+SAMPLE = 4096      # seeded i-sample where the full oracle is too slow (SURVEY 8(c) "Oracle cost and sampling")
 
 
 @pytest.mark.parametrize("prec", ["ds", "fp32"])
@@ -62,11 +64,11 @@ def test_cfg3_blockstep_ds_fp32(prec):
         il = w.ilist(ni)
         s2.s2_calc_ilist(ctx, il, eps2=w.eps2, flags=0)
         res = s2.s2_get_results(ctx, ni)
-        pick = np.arange(ni) if ni <= 1024 else np.sort(np.random.default_rng(3).choice(ni, 1024, replace=False))
+        pick = np.arange(ni) if ni <= SAMPLE else np.sort(np.random.default_rng(3).choice(ni, SAMPLE, replace=False))
         ref, _ = oracle_on_gpu_prediction(ctx, w, 4, il[pick], w.eps2)
         sub = {k: (v[pick] if isinstance(v, np.ndarray) else v) for k, v in res.items()}
         errs = check_forces(sub, ref, P, 4, 0, f"cfg3 {prec} n_i={ni} {s2.s2_last_launch_info(ctx)}")
-        print(f"cfg3 {prec} n_i={ni}", {k: f"{v:.2e}" for k, v in errs.items()})
+        print(f"cfg3 {prec} n_i={ni} (oracle on {pick.size} i, sample seed 3)", {k: f"{v:.2e}" for k, v in errs.items()})
     s2.s2_close(ctx)
 
 
@@ -114,7 +116,7 @@ def test_explicit_sinks_ds_fp32(prec):
 
 
 def test_cfg4_sixth_order_all_active_sampled():
-    """BASELINE config 4 at n_i = N = 262144 (6.9e10 pairs): oracle on a seeded sample of 1024 i, plus
+    """BASELINE config 4 at n_i = N = 262144 (6.9e10 pairs): oracle on a seeded sample of 4096 i, plus
     Newton's third law on the full GPU output."""
     w = make_config(4)
     ctx = open_and_load(w, 6)
@@ -122,11 +124,11 @@ def test_cfg4_sixth_order_all_active_sampled():
     il = w.ilist(w.N)
     s2.s2_calc_ilist(ctx, il, eps2=w.eps2)
     res = s2.s2_get_results(ctx, w.N)
-    pick = np.sort(np.random.default_rng(4).choice(w.N, 1024, replace=False))
+    pick = np.sort(np.random.default_rng(4).choice(w.N, SAMPLE, replace=False))
     ref, _ = oracle_on_gpu_prediction(ctx, w, 6, il[pick], w.eps2)
     sub = {k: (v[pick] if isinstance(v, np.ndarray) else v) for k, v in res.items()}
     errs = check_forces(sub, ref, s2.S2_FP64, 6, 0, f"cfg4 n_i=N {s2.s2_last_launch_info(ctx)}")
-    print("cfg4 n_i=N sample 1024 (seed 4)", {k: f"{v:.2e}" for k, v in errs.items()})
+    print(f"cfg4 n_i=N sample {SAMPLE} (seed 4)", {k: f"{v:.2e}" for k, v in errs.items()})
     for q in ("acc", "jerk", "snap"):
         tot = np.abs((w.mass[il, None] * res[q]).sum(0)).max()
         scale = (w.mass[il] * np.linalg.norm(res[q], axis=1)).sum()
@@ -134,11 +136,15 @@ def test_cfg4_sixth_order_all_active_sampled():
     s2.s2_close(ctx)
 
 
+_CFG5 = {}   # the 4096-i oracle result of config 5, shared by the two precision legs
+
+
 @pytest.mark.parametrize("prec", ["fp64", "fp32"])
 def test_cfg5_neighbour_path_sampled(prec):
     """BASELINE config 5: N = n_i = 2^20 Salpeter Plummer, nn + neighbour lists (cap 256), fp64 and fp32.
-    Oracle on a seeded sample of 512 i (sets exact); counts, overflow flag and the pot-symmetry / third-law
-    invariants on the full output."""
+    Oracle on a seeded sample of 4096 i (sets judged against the long-double decision within north_star's band);
+    counts, overflow flag and the third-law invariants on the full output.  The oracle runs once for both
+    precisions: its inputs are the fp64 predicted planes, which every precision mode writes identically (checked)."""
     P = s2.S2_FP64 if prec == "fp64" else s2.S2_FP32
     w = make_config(5)
     ctx = open_and_load(w, 4, precision=P, ngb_cap=256)
@@ -147,17 +153,28 @@ def test_cfg5_neighbour_path_sampled(prec):
     h2 = w.h2[il]
     s2.s2_calc_ilist(ctx, il, h2, w.eps2, NN | NGB)
     res = s2.s2_get_results(ctx, w.N)
-    pick = np.sort(np.random.default_rng(5).choice(w.N, 512, replace=False))
-    ref, _ = oracle_on_gpu_prediction(ctx, w, 4, il[pick], w.eps2, h2[pick], ngb_cap=256)
+    pick = np.sort(np.random.default_rng(5).choice(w.N, SAMPLE, replace=False))
+    xp, vp, _ = s2.s2_get_predicted_j(ctx, 0, w.N)
+    if "ref" not in _CFG5:
+        _CFG5["ref"] = oracle.forces_ilist(4, w.mass, w.ident, xp, vp, None, il[pick], w.eps2, h2[pick], 256)
+        _CFG5["xp"], _CFG5["vp"] = xp, vp
+    assert np.array_equal(xp, _CFG5["xp"]) and np.array_equal(vp, _CFG5["vp"])
+    ref = _CFG5["ref"]
     sub = {k: (v[pick] if isinstance(v, np.ndarray) else v) for k, v in res.items()}
     errs = check_forces(sub, ref, P, 4, NN | NGB, f"cfg5 {prec}")
-    for k, i in enumerate(pick):
-        got = s2.s2_get_neighbours(ctx, int(i), 256)
-        want = ref.ngb_list[k][ref.ngb_list[k] >= 0][:256]
-        assert np.array_equal(got, want), f"cfg5 {prec}: neighbour list of i={i}"
+    # all lists in one compacted read-back (device-side CSR), then the sampled ones against the oracle
+    off, lst = s2.s2_get_neighbours_csr(ctx, w.N)
     cnt = res["ngb_count"]
-    print(f"cfg5 {prec}", {k: f"{v:.2e}" for k, v in errs.items()}, "mean/max neighbour count", cnt.mean(), cnt.max(),
-          "overflows", int((cnt > 256).sum()), s2.s2_last_launch_info(ctx))
+    assert np.array_equal(np.diff(off), np.minimum(cnt, 256))
+    lists = [lst[off[i]:off[i + 1]] for i in pick]
+    n_band = check_sets_ld(cnt[pick], lists, ref, f"cfg5 {prec}")
+    for k in range(0, SAMPLE, 64):                           # the single-list getter returns the same segment
+        assert np.array_equal(s2.s2_get_neighbours(ctx, int(pick[k]), 256), lists[k])
+    for k in range(SAMPLE):                                  # secondary: the fp64 decision, bit for bit
+        assert np.array_equal(lists[k], ref.ngb_list[k][ref.ngb_list[k] >= 0][:256]), f"cfg5 {prec}: list of i={pick[k]}"
+    print(f"cfg5 {prec} sample {SAMPLE} (seed 5)", {k: f"{v:.2e}" for k, v in errs.items()}, "pairs accepted in the 1e-12 band:",
+          n_band, "mean/max neighbour count", cnt.mean(), cnt.max(), "overflows", int((cnt > 256).sum()),
+          "list entries", int(off[-1]), s2.s2_last_launch_info(ctx))
     assert res["overflow"] == bool((cnt > 256).any())
     assert 8 < cnt.mean() < 128
     tol = 1e-10 if prec == "fp64" else 1e-4
@@ -175,7 +192,7 @@ def test_cfg5_neighbour_path_sampled(prec):
 def test_headline_point_in_bench_configuration_sampled():
     """The bench workload (north_star target point): N = n_i = 2^18 equal-mass Plummer, eps = 1e-4, 4th order fp64,
     in the launch configuration bench.py times (device-resident i-list, automatic shape = uniform-operand sweep).
-    Oracle on a seeded sample of 512 i; Newton's third law and the potential symmetry on the full output."""
+    Oracle on a seeded sample of 4096 i; Newton's third law and the potential symmetry on the full output."""
     import torch
     w = make_config("H")
     ctx = open_and_load(w, 4)
@@ -186,11 +203,11 @@ def test_headline_point_in_bench_configuration_sampled():
     info = s2.s2_last_launch_info(ctx)
     assert info["reduced"] == 3 and info["lanes_per_i"] == 1 and info["S"] == w.N // 1024   # one launch per chunk
     res = s2.s2_get_results(ctx, w.N)
-    pick = np.sort(np.random.default_rng(6).choice(w.N, 512, replace=False))
+    pick = np.sort(np.random.default_rng(6).choice(w.N, SAMPLE, replace=False))
     ref, _ = oracle_on_gpu_prediction(ctx, w, 4, il[pick], w.eps2)
     sub = {k: (v[pick] if isinstance(v, np.ndarray) else v) for k, v in res.items()}
     errs = check_forces(sub, ref, s2.S2_FP64, 4, 0, f"headline {info}")
-    print("headline sample 512 (seed 6)", info, {k: f"{v:.2e}" for k, v in errs.items()})
+    print(f"headline sample {SAMPLE} (seed 6)", info, {k: f"{v:.2e}" for k, v in errs.items()})
     for q in ("acc", "jerk"):
         tot = np.abs((w.mass[il, None] * res[q]).sum(0)).max()
         scale = (w.mass[il] * np.linalg.norm(res[q], axis=1)).sum()
@@ -258,6 +275,7 @@ def test_second_order_acc_pot_only(prec):
         assert rel_err(res["pot"], ref.pot).max() <= TOL[P]["pot"], what
         assert not res["jerk"].any(), what
         if flags:
+            check_nn_ld(res, ref, what)
             assert np.array_equal(res["nn_id"], ref.nn_id) and np.array_equal(res["nn_r2"], ref.nn_d2), what
         if flags & NGB:
             assert np.array_equal(res["ngb_count"], ref.ngb_count), what

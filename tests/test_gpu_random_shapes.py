@@ -8,7 +8,7 @@ import oracle
 import paper_1510_04068_b200 as s2
 from workloads import make_config
 
-from gpu_util import TOL, check_neighbour_lists, rel_err
+from gpu_util import TOL, check_neighbour_lists, check_nn_ld, rel_err
 
 pytestmark = pytest.mark.gpu
 
@@ -54,6 +54,7 @@ def test_random_problems_automatic_shape(seed):
             else:
                 assert not res["acc"].any() and res["pot"][0] == 0.0, what
             if flags:
+                check_nn_ld(res, ref, what)      # primary: the oracle's long-double decision (north_star's band)
                 assert np.array_equal(res["nn_id"], ref.nn_id) and np.array_equal(res["nn_r2"], ref.nn_d2), what
             if flags & NGB:
                 assert np.array_equal(res["ngb_count"], ref.ngb_count), what

@@ -94,6 +94,43 @@ def test_ring_closed_form(n):
     np.testing.assert_allclose(res.pot, potc, rtol=1e-14)
 
 
+def test_term_norms_closed_forms():
+    """oracle_term_norms (the scale of the Newton's-third-law bound) is a second copy of the pair terms, so it gets
+    its own pins.  Circular two-body orbit (eps = 0, r.v = 0, v.v + r.a = 0): ||A0|| = m / R^2, ||A1|| = m v / R^3,
+    ||A2|| = m M / R^5.  Rigidly rotating regular n-gon: the pair (i, i + k) has separation d_k = 2 R sin(pi k / n),
+    relative velocity w d_k perpendicular to it and relative acceleration -w^2 r, so alpha = beta = 0 and the norms are
+    m / d_k^2, m w / d_k^2, m w^2 / d_k^2; sum_k 1 / sin^2(pi k / n) = (n^2 - 1) / 3."""
+    m, M, R = 0.3, 1.7, 2.5
+    r = np.array([[R, 0.0, 0.0]]); vc = math.sqrt(M / R)
+    v = np.array([[0.0, vc, 0.0]]); a = -M * r / R ** 3
+    z = np.zeros((1, 3))
+    na, nj, ns = oracle.term_norms(6, np.array([m]), np.array([5], np.int32), r, v, a, np.array([9], np.int32), z, z, z, 0.0)
+    assert na[0] == pytest.approx(m / R ** 2, rel=1e-15)
+    assert nj[0] == pytest.approx(m * vc / R ** 3, rel=1e-15)
+    assert ns[0] == pytest.approx(m * M / R ** 5, rel=1e-15)
+    # a generic pair: the norms are those of the oracle's own single-pair outputs (which the 80-digit pins fix)
+    rng = np.random.default_rng(3)
+    r, v, a = rng.normal(size=(1, 3)), rng.normal(size=(1, 3)), rng.normal(size=(1, 3))
+    one = _one_pair(6, m, r[0], v[0], a[0], 0.07)
+    na, nj, ns = oracle.term_norms(6, np.array([m]), np.array([5], np.int32), r, v, a, np.array([9], np.int32), z, z, z, 0.07)
+    for got, vec in ((na, one.acc), (nj, one.jerk), (ns, one.snap)):
+        assert got[0] == pytest.approx(np.linalg.norm(vec[0]), rel=1e-14)
+    for n in (3, 8, 17):
+        m, R, w = 0.7 / n, 1.3, 0.9
+        th = 2 * math.pi * np.arange(n) / n
+        x = np.stack([R * np.cos(th), R * np.sin(th), np.zeros(n)], 1)
+        vel = np.stack([-w * x[:, 1], w * x[:, 0], np.zeros(n)], 1)
+        ids = np.arange(n, dtype=np.int32)
+        na, nj, ns = oracle.term_norms(6, np.full(n, m), ids, x, vel, -w * w * x, ids, x, vel, -w * w * x, 0.0)
+        base = m * (n * n - 1) / (12 * R * R)
+        np.testing.assert_allclose(na, base, rtol=1e-13)
+        np.testing.assert_allclose(nj, base * w, rtol=1e-12)
+        np.testing.assert_allclose(ns, base * w * w, rtol=1e-12)
+    # the 4th-order call returns the same acc / jerk norms (no snap terms needed)
+    na4, nj4, _ = oracle.term_norms(4, np.full(n, m), ids, x, vel, None, ids, x, vel, None, 0.0)
+    assert np.array_equal(na4, na) and np.array_equal(nj4, nj)
+
+
 # ----------------------------------------------------------------------------- sums / invariants
 def _predicted(w, order):
     return oracle.predict(order, w.t_pred, w.t_j, w.pos, w.vel, w.acc, w.jerk, w.snap, w.crackle)
@@ -207,6 +244,10 @@ def test_bruteforce_neighbours_tiny():
         assert res.ngb_count[i] == len(members)
         got = [int(x) for x in res.ngb_list[i] if x >= 0]
         assert got == members[:8]            # P8: lowest addresses, ascending, truncated at cap
+        # the long-double decisions (the ones the GPU tests are judged against) pinned by the same brute force
+        assert res.nn_addr_ld[i] == order[0] and res.nn_d2_ld[i] == pytest.approx(d2[order[0]], rel=1e-15)
+        assert res.ngb_count_ld[i] == len(members)
+        assert [int(x) for x in res.ngb_list_ld[i] if x >= 0] == members[:8]
     assert (res.ngb_count > 8).any() and (res.ngb_count <= 8).any()
 
 
@@ -225,7 +266,8 @@ def test_lattice_ties_and_strictness():
             assert res.nn_addr[i] == int(np.flatnonzero(d2 == s2)[0])      # lowest address among ties
             assert res.ngb_count[i] == int((d2 < h2v).sum())
         assert res.ngb_count.max() == nmax
-        assert np.array_equal(res.nn_addr, res.nn_addr_ld)
+        assert np.array_equal(res.nn_addr, res.nn_addr_ld) and np.array_equal(res.nn_d2, res.nn_d2_ld)
+        assert np.array_equal(res.ngb_count, res.ngb_count_ld) and np.array_equal(res.ngb_list, res.ngb_list_ld)
 
 
 def test_self_skip_and_empty_cases():
