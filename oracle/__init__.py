@@ -116,7 +116,8 @@ def forces(order: int, mass, ident, xp, vp, ap, i_id, xi, vi, ai, eps2: float,
                         _p(nn_addr, i), _p(nn_id, i), _p(nn_d2, d), _p(nn_addr_ld, i),
                         _p(cnt, i), _p(lst, i), C.c_int(ngb_cap), _p(nn_d2_ld, d), _p(cnt_ld, i), _p(lst_ld, i))
     return ForceResult(acc, jerk, snap, pot, nn_addr, nn_id, nn_d2, nn_addr_ld, cnt, lst, nn_d2_ld, cnt_ld, lst_ld,
-                       dict(xj=xp, xi=xi, h2=h2, ident=ident, ngb_cap=ngb_cap))
+                       dict(xj=xp, xi=xi, h2=h2, ident=ident, ngb_cap=ngb_cap, order=order, mass=mass, vj=vp, aj=ap,
+                            i_id=i_id, vi=vi, ai=ai, eps2=eps2))
 
 
 def forces_ilist(order: int, mass, ident, xp, vp, ap, i_address, eps2: float,
@@ -128,8 +129,9 @@ def forces_ilist(order: int, mass, ident, xp, vp, ap, i_address, eps2: float,
                   None if ap is None else np.asarray(ap)[ia], eps2, h2_i, ngb_cap)
 
 
-def term_norms(order: int, mass, ident, xp, vp, ap, i_id, xi, vi, ai, eps2: float):
-    """Per-i sum over j of the norms of the individual pair terms (error norm of reading P12)."""
+def term_norms(order: int, mass, ident, xp, vp, ap, i_id, xi, vi, ai, eps2: float, rms: bool = False):
+    """Per-i sum over j of the norms of the individual pair terms (error norm of reading P12): (nacc, njerk, nsnap).
+    rms=True returns instead the roots of the sums of their squares (error norm of reading R-F32)."""
     mass, xp, vp = _f64(mass), _f64(xp), _f64(vp)
     ident, i_id = _i32(ident), _i32(i_id)
     xi, vi = _f64(xi), _f64(vi)
@@ -139,8 +141,9 @@ def term_norms(order: int, mass, ident, xp, vp, ap, i_id, xi, vi, ai, eps2: floa
     else:
         ap = ai = None
     na, nj, ns = np.empty(ni), np.empty(ni), np.empty(ni)
+    ra, rj, rs = np.empty(ni), np.empty(ni), np.empty(ni)
     d, i = np.float64, np.int32
     lib().oracle_term_norms(C.c_int(order), C.c_int(N), _p(mass, d), _p(ident, i), _p(xp, d), _p(vp, d), _p(ap, d),
                             C.c_int(ni), _p(i_id, i), _p(xi, d), _p(vi, d), _p(ai, d), C.c_double(eps2),
-                            _p(na, d), _p(nj, d), _p(ns, d))
-    return na, nj, ns
+                            _p(na, d), _p(nj, d), _p(ns, d), _p(ra, d), _p(rj, d), _p(rs, d))
+    return (ra, rj, rs) if rms else (na, nj, ns)

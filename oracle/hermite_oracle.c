@@ -23,7 +23,8 @@
  * Parity pins (tests/test_oracle_pins.py): two-body closed form, circular-orbit
  * closed form, regular n-gon closed form, Newton's third law, finite-difference
  * jerk and snap along the predictor polynomials, exact rational evaluation of
- * the predictor, brute-force neighbour sets, integer-lattice ties.
+ * the predictor, brute-force neighbour sets, integer-lattice ties; oracle_term_norms
+ * on the circular two-body orbit, the rotating n-gon and a generic single pair.
  * Conventions P3-P9 versus the real Sapporo2 library: parity unpinned (the
  * library is not available and the paper does not state them).
  */
@@ -204,15 +205,19 @@ void oracle_forces(int order, int N, const double *m, const int *id,
 }
 
 /* Sum over j of the Euclidean norms of the individual pair terms, per i (for the
- * symmetric-case error norm of reading P12: ||delta|| <= tol * sum_j ||term_j||). */
+ * symmetric-case error norm of reading P12: ||delta|| <= tol * sum_j ||term_j||), and
+ * the root of the sum of their squares (racc, rjerk, rsnap; any may be NULL): the
+ * scale of the rounding error of a sum whose terms are each evaluated to a fixed
+ * relative accuracy (reading R-F32, the fp32 path's error norm). */
 void oracle_term_norms(int order, int N, const double *m, const int *id,
                        const double *xp, const double *vp, const double *ap,
                        int ni, const int *i_id, const double *xi, const double *vi, const double *ai,
-                       double eps2, double *nacc, double *njerk, double *nsnap)
+                       double eps2, double *nacc, double *njerk, double *nsnap,
+                       double *racc, double *rjerk, double *rsnap)
 {
 #pragma omp parallel for schedule(dynamic, 8)
     for (int i = 0; i < ni; ++i) {
-        ld NA = 0, NJ = 0, NS = 0;
+        ld NA = 0, NJ = 0, NS = 0, QA = 0, QJ = 0, QS = 0;
         for (int j = 0; j < N; ++j) {
             if (id[j] == i_id[i]) continue;
             ld r[3], v[3], a[3] = {0, 0, 0};
@@ -234,9 +239,13 @@ void oracle_term_norms(int order, int N, const double *m, const int *id,
                 n0 += A0 * A0; n1 += A1 * A1; n2 += A2 * A2;
             }
             NA += sqrtl(n0); NJ += sqrtl(n1); NS += sqrtl(n2);
+            QA += n0; QJ += n1; QS += n2;
         }
         if (nacc) nacc[i] = (double)NA;
         if (njerk) njerk[i] = (double)NJ;
         if (nsnap) nsnap[i] = (double)NS;
+        if (racc) racc[i] = (double)sqrtl(QA);
+        if (rjerk) rjerk[i] = (double)sqrtl(QJ);
+        if (rsnap) rsnap[i] = (double)sqrtl(QS);
     }
 }

@@ -542,8 +542,11 @@ inline cudaError_t opt_in_smem(K kern, std::atomic<int> *done)
     if (dev < 0 || dev >= kMaxDevices) return cudaErrorInvalidDevice;
     if (done[dev].load(std::memory_order_acquire)) return cudaSuccess;
     int lim = 0;
+    cudaFuncAttributes fa;
     e = cudaDeviceGetAttribute(&lim, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev);
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, lim);
+    if (e == cudaSuccess) e = cudaFuncGetAttributes(&fa, kern);
+    // static + dynamic shared memory together must stay within the device's opt-in limit
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, lim - (int)fa.sharedSizeBytes);
     if (e == cudaSuccess) done[dev].store(1, std::memory_order_release);
     return e;
 }

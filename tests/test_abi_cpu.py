@@ -17,6 +17,12 @@ def test_library_exports_every_declared_symbol():
     assert len(names) >= 25 and "s2_calc_ilist" in names and "s2_get_neighbours_csr" in names
     missing = [n for n in names if not hasattr(L, n)]
     assert not missing, missing
+    # the product header carries the hot-path calls; tuning overrides and microbenchmarks live in s2b200_test.h only
+    prod, test = set(s2.header_symbols("product")), set(s2.header_symbols("test"))
+    assert {"s2_open", "s2_set_j", "s2_commit_j", "s2_predict", "s2_calc_ilist", "s2_calc_explicit", "s2_get_results",
+            "s2_get_results_device", "s2_get_neighbours", "s2_get_neighbours_csr", "s2_get_neighbours_csr_device"} <= prod
+    assert {"s2_set_tuning", "s2_peak_fma", "s2_test_ds_ops", "s2_time_host_roundtrip", "s2_last_launch_info"} <= test
+    assert not (prod & test)
     assert s2.s2_version().startswith("s2b200")
     assert "order" in s2.s2_strerror(s2.S2_ESTATE) and "fallback" in s2.s2_strerror(s2.S2_ECUDA)
     assert s2.s2_strerror(-99) == "unknown error code"

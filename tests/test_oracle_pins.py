@@ -113,8 +113,10 @@ def test_term_norms_closed_forms():
     r, v, a = rng.normal(size=(1, 3)), rng.normal(size=(1, 3)), rng.normal(size=(1, 3))
     one = _one_pair(6, m, r[0], v[0], a[0], 0.07)
     na, nj, ns = oracle.term_norms(6, np.array([m]), np.array([5], np.int32), r, v, a, np.array([9], np.int32), z, z, z, 0.07)
-    for got, vec in ((na, one.acc), (nj, one.jerk), (ns, one.snap)):
+    ra, rj, rs = oracle.term_norms(6, np.array([m]), np.array([5], np.int32), r, v, a, np.array([9], np.int32), z, z, z, 0.07, rms=True)
+    for got, got_rms, vec in ((na, ra, one.acc), (nj, rj, one.jerk), (ns, rs, one.snap)):
         assert got[0] == pytest.approx(np.linalg.norm(vec[0]), rel=1e-14)
+        assert got_rms[0] == pytest.approx(np.linalg.norm(vec[0]), rel=1e-14)      # one term: both norms are its length
     for n in (3, 8, 17):
         m, R, w = 0.7 / n, 1.3, 0.9
         th = 2 * math.pi * np.arange(n) / n
@@ -126,6 +128,12 @@ def test_term_norms_closed_forms():
         np.testing.assert_allclose(na, base, rtol=1e-13)
         np.testing.assert_allclose(nj, base * w, rtol=1e-12)
         np.testing.assert_allclose(ns, base * w * w, rtol=1e-12)
+        # root of the sum of squares (reading R-F32): sum_k 1 / sin^4(pi k / n) = (n^2 - 1)(n^2 + 11) / 45
+        ra, rj, rs = oracle.term_norms(6, np.full(n, m), ids, x, vel, -w * w * x, ids, x, vel, -w * w * x, 0.0, rms=True)
+        rbase = m / (4 * R * R) * math.sqrt((n * n - 1) * (n * n + 11) / 45)
+        np.testing.assert_allclose(ra, rbase, rtol=1e-13)
+        np.testing.assert_allclose(rj, rbase * w, rtol=1e-12)
+        np.testing.assert_allclose(rs, rbase * w * w, rtol=1e-12)
     # the 4th-order call returns the same acc / jerk norms (no snap terms needed)
     na4, nj4, _ = oracle.term_norms(4, np.full(n, m), ids, x, vel, None, ids, x, vel, None, 0.0)
     assert np.array_equal(na4, na) and np.array_equal(nj4, nj)
