@@ -172,6 +172,42 @@ int s2_get_neighbours_csr(s2_ctx *ctx, int ni, long long *offsets, int *list, lo
  * *total = offsets[ni].  SYNC (one 8-byte read). */
 int s2_get_neighbours_csr_device(s2_ctx *ctx, int ni, const long long **d_offsets, const int **d_list, long long *total);
 
+/* --- block-time-step Hermite integrator on the device (sec 3.7) -------- */
+
+/* The second workload of the paper: a 4th- or 6th-order Hermite predictor-corrector with block (power-of-two,
+ * block-aligned) individual time steps, which calls the hot path above with an active set that varies between 1 and N
+ * from step to step.  Everything runs in kernels on the context's stream: the particle state is the context's own
+ * j-store (the corrector updates it in place, so nothing is re-sent), the corrector and the time-step criterion
+ * (Aarseth, L152: eta_4 = 0.01, eta_6 = 0.1), the choice of the next block time and the compaction of the next
+ * active list.  Per block step the host reads back 12 bytes (next time, next active count) after one stream
+ * synchronisation -- it needs the count to shape the next force launch.  paper_1510_04068_b200/hermite.py is the host
+ * reference driver of the same schemes (textbook formulas, refs [27] and [5]).
+ * The integrator takes over the j-store of `ctx` (addresses 0 .. n-1, id == address); between s2_bts_run calls the
+ * ordinary calls (s2_predict, s2_calc_*, s2_get_*) may be used on the same context, s2_set_j / s2_commit_j may not. */
+typedef struct s2_bts s2_bts; /* opaque */
+
+/* ctx: an order-4 or order-6 context (any precision) with nj_capacity >= n.  dt_max, dt_min: powers of two <= 1.
+ * eta: accuracy parameter of the step criterion; eta_start: that of the first step, dt = eta_start |a| / |jerk|. */
+int s2_bts_open(s2_bts **out, s2_ctx *ctx, int n, double eps2, double eta, double eta_start, double dt_max, double dt_min);
+int s2_bts_close(s2_bts *b);
+/* Initial conditions at t = 0: host arrays mass (n), pos, vel (n,3).  Runs the start-up force evaluation (two passes
+ * for order 6: the snap needs every particle's acceleration), sets the first steps and the first active list.  SYNC. */
+int s2_bts_init(s2_bts *b, const double *mass, const double *pos, const double *vel);
+/* Advances block step by block step while the next block time is <= t_end, at most max_block_steps steps
+ * (*steps_done, may be NULL).  If t_end is a multiple of dt_max every particle ends at exactly t_end.
+ * time_device != 0 also accumulates the device time of the steps' kernels between CUDA events (s2_bts_stats).  SYNC. */
+int s2_bts_run(s2_bts *b, double t_end, long long max_block_steps, int time_device, long long *steps_done);
+/* Per-particle state, each particle at its own time t[i] (host arrays of n or (n,3); any may be NULL).  SYNC. */
+int s2_bts_get_state(s2_bts *b, double *time, double *t, double *dt, double *pos, double *vel, double *acc, double *jerk,
+                     double *pot);
+/* Counters since s2_bts_init (any pointer may be NULL): current time, next block time and its active count, block
+ * steps, particle steps (sum of the active counts), host wall time inside s2_bts_run, and -- for steps run with
+ * time_device -- the summed device time and their number. */
+int s2_bts_stats(const s2_bts *b, double *time, double *t_next, int *n_next, long long *block_steps,
+                 long long *particle_steps, double *wall_ms, double *device_ms, long long *timed_steps);
+/* Active counts of block steps first .. first+count-1 since s2_bts_init. */
+int s2_bts_get_history(const s2_bts *b, long long first, int count, int *n_active);
+
 /* --- read-back hooks and diagnostics (tuning overrides and microbenchmarks: s2b200_test.h) --- */
 
 /* fp64 predicted state of j-particles first .. first+n-1 ((n,3) arrays, any may be NULL;

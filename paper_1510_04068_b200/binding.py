@@ -89,6 +89,14 @@ def lib() -> C.CDLL:
         "s2_get_timing": (C.c_int, [vp, C.POINTER(C.c_float), C.POINTER(C.c_float), C.POINTER(C.c_float)]),
         "s2_peak_fma": (C.c_int, [vp, C.c_int, C.c_int, C.POINTER(C.c_double)]),
         "s2_time_host_roundtrip": (C.c_int, [vp, C.c_int, C.POINTER(C.c_int), C.c_double, C.c_uint, C.c_int, C.POINTER(C.c_double)]),
+        "s2_bts_open": (C.c_int, [C.POINTER(vp), vp, C.c_int] + [C.c_double] * 5),
+        "s2_bts_close": (C.c_int, [vp]),
+        "s2_bts_init": (C.c_int, [vp, dp, dp, dp]),
+        "s2_bts_run": (C.c_int, [vp, C.c_double, C.c_longlong, C.c_int, C.POINTER(C.c_longlong)]),
+        "s2_bts_get_state": (C.c_int, [vp, C.POINTER(C.c_double)] + [dp] * 7),
+        "s2_bts_stats": (C.c_int, [vp, C.POINTER(C.c_double), C.POINTER(C.c_double), C.POINTER(C.c_int), C.POINTER(C.c_longlong),
+                                   C.POINTER(C.c_longlong), C.POINTER(C.c_double), C.POINTER(C.c_double), C.POINTER(C.c_longlong)]),
+        "s2_bts_get_history": (C.c_int, [vp, C.c_longlong, C.c_int, ip]),
         "s2_strerror": (C.c_char_p, [C.c_int]),
         "s2_last_cuda_error": (C.c_char_p, [vp]),
         "s2_version": (C.c_char_p, []),
@@ -411,6 +419,70 @@ def s2_test_ds_ops(ctx, a, b) -> np.ndarray:
     _check(lib().s2_test_ds_ops(ctx.handle, a.shape[0], a.ctypes.data_as(C.c_void_p), b.ctypes.data_as(C.c_void_p),
                                 out.ctypes.data_as(C.c_void_p)), "s2_test_ds_ops", ctx.handle)
     return out
+
+
+# ---- block-time-step integrator (include/s2b200.h, s2_bts_*) ------------------------------------------------
+
+class s2_bts:
+    def __init__(self, handle, ctx, n):
+        self.handle, self.ctx, self.n = handle, ctx, n
+
+
+def s2_bts_open(ctx, n: int, eps2: float, eta: float, eta_start: float, dt_max: float = 2.0 ** -3, dt_min: float = 2.0 ** -40):
+    h = C.c_void_p()
+    _check(lib().s2_bts_open(C.byref(h), ctx.handle, int(n), float(eps2), float(eta), float(eta_start), float(dt_max),
+                             float(dt_min)), "s2_bts_open", ctx.handle)
+    return s2_bts(h, ctx, int(n))
+
+
+def s2_bts_close(b):
+    if b.handle:
+        _check(lib().s2_bts_close(b.handle), "s2_bts_close")
+        b.handle = None
+
+
+def s2_bts_init(b, mass, pos, vel):
+    pm, k0 = _h(mass, np.float64, (), b.n, "mass")
+    pp, k1 = _h(pos, np.float64, (3,), b.n, "pos")
+    pv, k2 = _h(vel, np.float64, (3,), b.n, "vel")
+    _check(lib().s2_bts_init(b.handle, pm, pp, pv), "s2_bts_init", b.ctx.handle)
+
+
+def s2_bts_run(b, t_end: float, max_block_steps: int = 1 << 62, time_device: bool = False) -> int:
+    done = C.c_longlong()
+    _check(lib().s2_bts_run(b.handle, float(t_end), int(max_block_steps), int(time_device), C.byref(done)), "s2_bts_run",
+           b.ctx.handle)
+    return done.value
+
+
+def s2_bts_get_state(b) -> dict:
+    n = b.n
+    out = dict(t=np.empty(n), dt=np.empty(n), pos=np.empty((n, 3)), vel=np.empty((n, 3)), acc=np.empty((n, 3)),
+               jerk=np.empty((n, 3)), pot=np.empty(n))
+    tm = C.c_double()
+    p = lambda a: a.ctypes.data_as(C.c_void_p)
+    _check(lib().s2_bts_get_state(b.handle, C.byref(tm), p(out["t"]), p(out["dt"]), p(out["pos"]), p(out["vel"]), p(out["acc"]),
+                                  p(out["jerk"]), p(out["pot"])), "s2_bts_get_state", b.ctx.handle)
+    out["time"] = tm.value
+    return out
+
+
+def s2_bts_stats(b) -> dict:
+    tm, tn, wall, dev = C.c_double(), C.c_double(), C.c_double(), C.c_double()
+    nn = C.c_int()
+    bs, ps, ts = C.c_longlong(), C.c_longlong(), C.c_longlong()
+    _check(lib().s2_bts_stats(b.handle, C.byref(tm), C.byref(tn), C.byref(nn), C.byref(bs), C.byref(ps), C.byref(wall), C.byref(dev),
+                              C.byref(ts)), "s2_bts_stats")
+    return dict(time=tm.value, t_next=tn.value, n_next=nn.value, block_steps=bs.value, particle_steps=ps.value,
+                wall_ms=wall.value, device_ms=dev.value, timed_steps=ts.value)
+
+
+def s2_bts_get_history(b, first: int = 0, count: int | None = None) -> np.ndarray:
+    if count is None:
+        count = s2_bts_stats(b)["block_steps"] - first
+    out = np.empty(max(count, 1), np.int32)
+    _check(lib().s2_bts_get_history(b.handle, int(first), int(count), out.ctypes.data_as(C.c_void_p)), "s2_bts_get_history")
+    return out[:count]
 
 
 def s2_last_cuda_error(ctx) -> str:

@@ -42,86 +42,17 @@ cudaError_t run_ds_ops(int n, const double *d_a, const double *d_b, double *d_ou
 
 using namespace s2;
 
-struct Buf {
-    void *p = nullptr;
-    size_t bytes = 0;
-};
-
-struct Batch {
-    size_t offset;   // byte offset of the batch block in the staging buffer
-    int n;
-};
-
-struct s2_ctx {
-    int device = 0, order = 4, precision = S2_FP64, nj_cap = 0, ngb_cap = 0;
-    s2_allocator alloc{};
-    bool has_alloc = false;
-    cudaStream_t stream = nullptr;
-    int sm_count = 148;
-    std::string cuda_err;
-    long long launches = 0;
-
-    // device buffers
-    Buf base, planes, qplanes, stage_dev, iplanes, iqplanes, i_addr, i_h2, part, result, seg, list, flags, counters;
-    // device-side CSR of the neighbour lists of the last force call (built on first request, s2_ngb.cu)
-    Buf csr_len, csr_bsum, csr_off, csr_list;
-    bool csr_valid = false;
-    long long csr_total = 0;
-    cudaEvent_t ev_csr[4] = {nullptr, nullptr, nullptr, nullptr};
-    bool ran_csr = false;
-    // pinned host buffers
-    void *h_stage = nullptr;
-    size_t h_stage_bytes = 0, h_stage_used = 0;
-    void *h_io = nullptr;
-    size_t h_io_bytes = 0;
-    int *h_flags = nullptr;           // pinned, 4 ints
-    // zero-copy small calls (n_i <= kZeroCopyNi): the kernels read the i-list from, and write the final records to,
-    // pinned host memory directly (device-accessible under unified addressing) -- no copy operations on the stream
-    void *h_res = nullptr;            // final records of the last small call
-    size_t h_res_bytes = 0;
-    bool res_on_host = false;
-    void *h_il[2] = {nullptr, nullptr};   // i-list (+ h2) of small calls, alternating so that a call can be
-    size_t h_il_bytes[2] = {0, 0};        // prepared while the previous one still runs
-    cudaEvent_t ev_il[2] = {nullptr, nullptr};
-    int il_turn = 0;
-    bool flags_dirty = false;         // a device-side commit may have raised the range flag
-    bool in_selftest = false;         // inside bank_selftest (run_force re-entered with a reduced problem)
-    cudaEvent_t ev_stage = nullptr;   // H2D of the staging buffer finished
-    cudaEvent_t ev_io = nullptr;      // H2D of the i-list upload finished
-    std::vector<Batch> batches;
-
-    // state
-    bool have_j = false, predicted = false, calc_done = false, results_fetched = false;
-    int nj_pred = 0, ni_last = 0;
-    unsigned flags_last = 0;
-    double t_pred = 0.0;
-
-    // tuning overrides and last launch
-    int tune[10] = {0, 0, 0, 0, 0, 0, 0, 0, 0, 0};
-    int last_info[10] = {0, 0, 0, 0, 0, 0, 0, 0, 1, 1};
-    std::map<long long, int> occ_cache;
-    std::map<long long, std::pair<ForceShape, int>> shape_cache;
-
-    // timing
-    bool timing = false;
-    cudaEvent_t ev_t[6] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};
-    bool ran_predict = false, ran_force = false, ran_reduce = false;
-};
+#include "s2_ctx.h"
 
 // ---- helpers ----------------------------------------------------------------------------
 
-static int fail_cuda(s2_ctx *c, cudaError_t e)
+int fail_cuda(s2_ctx *c, cudaError_t e)
 {
     if (c) c->cuda_err = cudaGetErrorString(e);
     return S2_ECUDA;
 }
-#define CU(call)                                           \
-    do {                                                   \
-        cudaError_t e__ = (call);                          \
-        if (e__ != cudaSuccess) return fail_cuda(ctx, e__); \
-    } while (0)
 
-static int dev_reserve(s2_ctx *ctx, Buf &b, size_t bytes)
+int dev_reserve(s2_ctx *ctx, Buf &b, size_t bytes)
 {
     if (bytes <= b.bytes) return S2_OK;
     // grow-only; contents are not preserved (callers refill)
@@ -154,7 +85,7 @@ static int dev_reserve(s2_ctx *ctx, Buf &b, size_t bytes)
     return S2_OK;
 }
 
-static void dev_release(s2_ctx *ctx, Buf &b)
+void dev_release(s2_ctx *ctx, Buf &b)
 {
     if (!b.p) return;
     if (ctx->has_alloc)
@@ -165,7 +96,7 @@ static void dev_release(s2_ctx *ctx, Buf &b)
     b.bytes = 0;
 }
 
-static int pinned_reserve(s2_ctx *ctx, void **p, size_t *have, size_t used, size_t bytes)
+int pinned_reserve(s2_ctx *ctx, void **p, size_t *have, size_t used, size_t bytes)
 {
     if (bytes <= *have) return S2_OK;
     size_t want = std::max(bytes + bytes / 2, (size_t)1 << 16);
@@ -207,17 +138,6 @@ static void par_memcpy(void *dst, const void *src, size_t bytes)
 }
 
 static inline size_t align16(size_t x) { return (x + 15) & ~(size_t)15; }
-
-static inline double *base_field(const s2_ctx *c, int f) { return (double *)c->base.p + (size_t)f * c->nj_cap; }
-static inline int *base_id(const s2_ctx *c) { return (int *)((double *)c->base.p + (size_t)nfields(c->order) * c->nj_cap); }
-static inline double2 *plane(const s2_ctx *c, int p) { return (double2 *)c->planes.p + (size_t)p * c->nj_cap; }
-static inline float4 *qplane(const s2_ctx *c, int p) { return (float4 *)c->qplanes.p + (size_t)p * c->nj_cap; }
-static inline int n_qplanes(int precision, int order)
-{
-    if (precision == S2_FP32) return order == 6 ? 4 : 3;
-    if (precision == S2_DS) return order == 6 ? 6 : 4;
-    return 0;
-}
 
 // ---- state shared by the contexts of one device: the two constant banks of the uniform-operand sweep ------------
 // (see run_force_bank below)
@@ -841,8 +761,6 @@ static int run_force_bank(s2_ctx *ctx, ForceArgs &a, int ni, unsigned flags, int
     return S2_OK;
 }
 
-static int run_force(s2_ctx *ctx, int ni, const int *d_i_addr, const double *d_h2, bool explicit_i, double eps2,
-                     unsigned flags, bool host_call);
 
 // First use of the self-refilling sweep on a device: run it once next to the shared-memory sweep on (a part of) the
 // caller's own problem -- at least three chunks, so that the last-CTA refill, the ticket hand-over and the
@@ -927,8 +845,8 @@ static int bank_choose_mode(s2_ctx *ctx, int ni, const int *d_i_addr, bool expli
 // (the record writes over the host link start to cost more than the copy they save), hence the limit
 constexpr int kZeroCopyNi = 128;
 
-static int run_force(s2_ctx *ctx, int ni, const int *d_i_addr, const double *d_h2, bool explicit_i, double eps2,
-                     unsigned flags, bool host_call)
+int run_force(s2_ctx *ctx, int ni, const int *d_i_addr, const double *d_h2, bool explicit_i, double eps2,
+              unsigned flags, bool host_call)
 {
     const bool bank = bank_applies(ctx, ni, ctx->nj_pred);
     ForceShape sh{};

@@ -1,0 +1,516 @@
+// s2_bts.cu -- device-resident block-time-step Hermite integrator (sec 3.7
+// L152-L168: "sixth order Hermite integrator with block time-steps", Plummer spheres, energy errors 1e-12 / 1e-10).
+//
+// The paper's point in L156-L164 is that in a block-step run the time goes into everything AROUND the force kernel:
+// picking the active set, the corrector, the time-step rule, and the traffic between host and device.  Here all of it
+// stays on the GPU.  The particle state IS the library's base j-store (t_j, m, x, v, a, jerk [, snap, crackle] at each
+// particle's own time): the corrector reads a particle's old state there and writes the new one in place, so there is
+// no commit copy at all.  One block step is
+//     predict_kernel (all j to t_next, the time read from device memory)     -- enqueued BEFORE the host knows t_next
+//     force sweep (+ reduce) for the active list                              -- s2_api.cu run_force, shape by n_active
+//     bts_correct_kernel   corrector + time-step rule + write-back, level histogram by integer atomics
+//     bts_select_kernel    next block time from the histogram, ordered compaction of the next active list,
+//                          {t_next, n_next} written to pinned host memory
+// and the host reads 12 bytes after one stream synchronisation (it needs n_next to shape the next sweep).
+//
+// Block time steps are powers of two and block-aligned (t_i is a multiple of dt_i), hence
+//     t_next = t_now + min_i dt_i        and        i is active at t_next  <=>  t_next is a multiple of dt_i,
+// so neither a t_i + dt_i array nor a global min-reduction over particles is needed: the smallest step follows from a
+// 64-bin histogram of step levels that the corrector keeps up to date.
+//
+// Corrector and time-step rule are the textbook ones of the schemes the paper names (4th order ref [27], 6th order
+// ref [5]); they are written out in paper_1510_04068_b200/hermite.py (the host reference driver, which the tests run
+// against the oracle in lock-step with this one) and repeated at the kernels below.
+#include <math_constants.h>
+
+#include <chrono>
+
+#include "s2_ctx.h"
+
+using namespace s2;
+
+namespace {
+
+constexpr int kLevels = 64;          // dt = 2^-level, level 0 .. 63
+constexpr int kSelThreads = 256;
+constexpr int kSelPerThread = 8;
+constexpr int kSelPerBlock = kSelThreads * kSelPerThread;
+
+struct BtsCtl {                      // device control block (also mirrored to pinned host memory by the select kernel)
+    double t_next;                   // time of the block step that is about to run
+    int n_next;                      // number of active particles of that step
+    int pad;
+};
+
+struct BtsArgs {
+    double *f[kMaxFields];           // base j-store fields (t, m, x, v, a, jerk [, snap, crackle])
+    double *dt;                      // [n] current step of every particle
+    double *pot;                     // [n] potential at the particle's last force evaluation
+    const double *rec;               // result records of the force call on the active list
+    int *ilist;                      // active list (addresses, ascending)
+    int *stage;                      // [n] per-block compaction staging of the select kernel
+    int *bcnt;                       // [nblocks] active particles found by each block
+    unsigned *arrive;                // arrival counter of the select kernel (zero between launches)
+    int *hist;                       // [kLevels] particles per step level
+    BtsCtl *ctl;                     // device control block
+    BtsCtl *h_ctl;                   // the same, in pinned host memory
+    int n, n_act, order;
+    double eta, eta_start, dt_max, dt_min;
+};
+
+__device__ __forceinline__ double pow2_floor(double x)   // largest power of two <= x, x > 0 finite
+{
+    return __hiloint2double(__double2hiint(x) & 0xfff00000, 0);
+}
+__device__ __forceinline__ int level_of(double dt)       // dt = 2^-level
+{
+    return 1023 - ((__double2hiint(dt) >> 20) & 0x7ff);
+}
+__device__ __forceinline__ double norm3(const double a[3]) { return sqrt(a[0] * a[0] + a[1] * a[1] + a[2] * a[2]); }
+
+// new step from the raw criterion value: power of two, at most doubled, doubled only at an even block boundary
+__device__ __forceinline__ double next_step(double raw, double old, double t_new, double dt_min, double dt_max)
+{
+    double nw = fmin(pow2_floor(fmax(raw, dt_min)), 2.0 * old);
+    if (nw > old) {
+        const double x = t_new / (2.0 * old);            // exact: division by a power of two
+        if (x != floor(x)) nw = old;
+    }
+    return fmin(fmax(nw, dt_min), dt_max);
+}
+
+// ---- start-up: first steps from acc and jerk alone, dt = eta_s |a| / |j| (hermite.py __init__) -------------------
+__global__ void __launch_bounds__(256) bts_init_kernel(BtsArgs a, int final_pass)
+{
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= a.n) return;
+    const double *r = a.rec + (size_t)i * REC;             // the start-up i-list is 0 .. n-1
+    double ac[3] = {r[0], r[1], r[2]}, jk[3] = {r[3], r[4], r[5]};
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+        a.f[8 + c][i] = ac[c];
+        a.f[11 + c][i] = jk[c];
+        if (a.order == 6 && final_pass) a.f[14 + c][i] = r[9 + c];   // snap needs every particle's acceleration: second pass
+    }
+    a.pot[i] = r[6];
+    if (!final_pass) return;
+    const double raw = a.eta_start * norm3(ac) / fmax(norm3(jk), 1e-300);
+    const double dt = fmin(fmax(pow2_floor(fmax(raw, a.dt_min)), a.dt_min), a.dt_max);
+    a.dt[i] = dt;
+    atomicAdd(&a.hist[level_of(dt)], 1);
+}
+
+// ---- corrector + time-step rule on the active particles ---------------------------------------------------------
+// 4th order (ref [27]):  v1 = v0 + (a0 + a1) dt/2 + (j0 - j1) dt^2/12;  x1 = x0 + (v0 + v1) dt/2 + (a0 - a1) dt^2/12
+//   s0 = (-6 (a0 - a1) - dt (4 j0 + 2 j1)) / dt^2,  c0 = (12 (a0 - a1) + 6 dt (j0 + j1)) / dt^3,  s1 = s0 + c0 dt
+//   dt' = sqrt(eta (|a1| |s1| + |j1|^2) / (|j1| |c0| + |s1|^2))                                   (Aarseth criterion)
+// 6th order (ref [5]), h = dt/2, A+- = a1 +- a0, J+- = h (j1 +- j0), S+- = h^2 (s1 +- s0):
+//   v1 = v0 + h (A+ - 2/5 J- + 1/15 S+);  x1 = x0 + h (v1 + v0) - 2/5 h^2 A- + h^3/15 (j1 + j0)
+//   F5 = (S- - 3 J+ + 3 A-)/16, F4 = (S+ - J-)/16, F3 = (5 J+ - 5 A- - S-)/8
+//   a3 = 6 (F3 + 4 F4 + 10 F5)/h^3 (stored as crackle), a4 = 24 (F4 + 5 F5)/h^4, a5 = 120 F5/h^5
+//   dt' = eta (A1 / A4)^(1/3),  A1 = sqrt(|a1||s1| + |j1|^2),  A4 = sqrt(|a3||a5| + |a4|^2)
+__global__ void __launch_bounds__(128) bts_correct_kernel(BtsArgs a)
+{
+    const int k = blockIdx.x * blockDim.x + threadIdx.x;
+    if (k >= a.n_act) return;
+    const int i = a.ilist[k];
+    const double t_new = a.ctl->t_next;
+    const double *r = a.rec + (size_t)k * REC;
+    const double dt = a.dt[i];
+    double x0[3], v0[3], a0[3], j0[3], a1[3], j1[3], x1[3], v1[3];
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+        x0[c] = a.f[2 + c][i]; v0[c] = a.f[5 + c][i]; a0[c] = a.f[8 + c][i]; j0[c] = a.f[11 + c][i];
+        a1[c] = r[c]; j1[c] = r[3 + c];
+    }
+    double raw;
+    if (a.order != 6) {
+        double s1[3], c0[3];
+        const double h = 0.5 * dt, d2 = dt * dt;
+#pragma unroll
+        for (int c = 0; c < 3; ++c) {
+            v1[c] = v0[c] + (a0[c] + a1[c]) * h + (j0[c] - j1[c]) * (d2 / 12.0);
+            x1[c] = x0[c] + (v0[c] + v1[c]) * h + (a0[c] - a1[c]) * (d2 / 12.0);
+            const double s0 = (-6.0 * (a0[c] - a1[c]) - dt * (4.0 * j0[c] + 2.0 * j1[c])) / d2;
+            c0[c] = (12.0 * (a0[c] - a1[c]) + 6.0 * dt * (j0[c] + j1[c])) / (d2 * dt);
+            s1[c] = s0 + c0[c] * dt;
+        }
+        const double an = norm3(a1), jn = norm3(j1), sn = norm3(s1), cn = norm3(c0);
+        raw = sqrt(a.eta * (an * sn + jn * jn) / fmax(jn * cn + sn * sn, 1e-300));
+    } else {
+        double s1[3], c1[3], p1[3], q1[3];
+        const double h = 0.5 * dt, h2 = h * h, h3 = h2 * h;
+#pragma unroll
+        for (int c = 0; c < 3; ++c) {
+            const double s0 = a.f[14 + c][i];
+            s1[c] = r[9 + c];
+            const double Ap = a1[c] + a0[c], Am = a1[c] - a0[c];
+            const double Jp = h * (j1[c] + j0[c]), Jm = h * (j1[c] - j0[c]);
+            const double Sp = h2 * (s1[c] + s0), Sm = h2 * (s1[c] - s0);
+            v1[c] = v0[c] + h * (Ap - 0.4 * Jm + Sp / 15.0);
+            x1[c] = x0[c] + h * (v1[c] + v0[c]) - 0.4 * h2 * Am + (h3 / 15.0) * (j1[c] + j0[c]);
+            const double F5 = (Sm - 3.0 * Jp + 3.0 * Am) / 16.0, F4 = (Sp - Jm) / 16.0, F3 = (5.0 * Jp - 5.0 * Am - Sm) / 8.0;
+            c1[c] = 6.0 * (F3 + 4.0 * F4 + 10.0 * F5) / h3;
+            p1[c] = 24.0 * (F4 + 5.0 * F5) / (h2 * h2);
+            q1[c] = 120.0 * F5 / (h2 * h3);
+            a.f[14 + c][i] = s1[c];
+            a.f[17 + c][i] = c1[c];
+        }
+        const double A1 = sqrt(norm3(a1) * norm3(s1) + norm3(j1) * norm3(j1));
+        const double A4 = sqrt(norm3(c1) * norm3(q1) + norm3(p1) * norm3(p1));
+        raw = a.eta * cbrt(A1 / fmax(A4, 1e-300));
+    }
+    const double nw = next_step(raw, dt, t_new, a.dt_min, a.dt_max);
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+        a.f[2 + c][i] = x1[c]; a.f[5 + c][i] = v1[c]; a.f[8 + c][i] = a1[c]; a.f[11 + c][i] = j1[c];
+    }
+    a.f[0][i] = t_new;
+    a.pot[i] = r[6];
+    if (nw != dt) {
+        a.dt[i] = nw;
+        atomicSub(&a.hist[level_of(dt)], 1);     // integer atomics: the histogram does not depend on their order
+        atomicAdd(&a.hist[level_of(nw)], 1);
+    }
+}
+
+// ---- next block time and next active list --------------------------------------------------------------------
+// Every block derives dt_min from the level histogram (64 loads), hence t_next = t_now + dt_min, compacts the active
+// particles of its 2048-particle slice (ascending) into its staging segment and publishes its count; the last block
+// to arrive concatenates the segments in block order -- the list is ascending by address whatever the arrival
+// order -- and writes {t_next, n_next} to the device control block and to pinned host memory.
+__global__ void __launch_bounds__(kSelThreads) bts_select_kernel(BtsArgs a, double t_now_host, int use_host_time)
+{
+    __shared__ int s_w[kSelThreads / 32];
+    __shared__ int s_last;
+    __shared__ double s_tnext;
+    if (threadIdx.x == 0) {
+        int lev = 0;
+        for (int l = kLevels - 1; l >= 0; --l)
+            if (a.hist[l] > 0) { lev = l; break; }
+        const double t_now = use_host_time ? t_now_host : a.ctl->t_next;
+        s_tnext = t_now + scalbn(1.0, -lev);
+    }
+    __syncthreads();
+    const double t_next = s_tnext;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int i0 = blockIdx.x * kSelPerBlock + threadIdx.x * kSelPerThread;
+    unsigned mask = 0;
+    int cnt = 0;
+#pragma unroll
+    for (int k = 0; k < kSelPerThread; ++k) {
+        const int i = i0 + k;
+        if (i < a.n) {
+            const double x = t_next / a.dt[i];           // exact: dt is a power of two
+            if (x == floor(x)) { mask |= 1u << k; ++cnt; }
+        }
+    }
+    int incl = cnt;
+#pragma unroll
+    for (int m = 1; m < 32; m <<= 1) {
+        const int o = __shfl_up_sync(0xffffffffu, incl, m);
+        if (lane >= m) incl += o;
+    }
+    if (lane == 31) s_w[warp] = incl;
+    __syncthreads();
+    int base = incl - cnt;
+    for (int w = 0; w < warp; ++w) base += s_w[w];
+    int *seg = a.stage + (size_t)blockIdx.x * kSelPerBlock;
+#pragma unroll
+    for (int k = 0; k < kSelPerThread; ++k)
+        if (mask & (1u << k)) seg[base++] = i0 + k;
+    if (threadIdx.x == kSelThreads - 1) {
+        a.bcnt[blockIdx.x] = base;                       // the last thread's running position = the block's count
+        __threadfence();
+        const unsigned prev = atomicAdd(a.arrive, 1u);
+        s_last = prev == gridDim.x - 1;
+    }
+    __syncthreads();
+    if (!s_last) return;
+    __threadfence();
+    // last block: concatenate the staging segments in block order
+    int off = 0;
+    for (int b = 0; b < (int)gridDim.x; ++b) {
+        const int c = __ldcg(a.bcnt + b);
+        const int *src = a.stage + (size_t)b * kSelPerBlock;
+        for (int k = threadIdx.x; k < c; k += kSelThreads) a.ilist[off + k] = __ldcg(src + k);
+        off += c;
+    }
+    if (threadIdx.x == 0) {
+        *a.arrive = 0u;
+        a.ctl->t_next = t_next;
+        a.ctl->n_next = off;
+        a.h_ctl->t_next = t_next;
+        a.h_ctl->n_next = off;
+    }
+}
+
+__global__ void bts_iota_kernel(int *p, int n)
+{
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < n) p[i] = i;
+}
+
+}  // namespace
+
+namespace s2 {
+cudaError_t launch_predict(const PredictArgs &a, cudaStream_t st);
+}
+
+struct s2_bts {
+    s2_ctx *ctx = nullptr;
+    int n = 0;
+    double eps2 = 0, eta = 0, eta_start = 0, dt_max = 0, dt_min = 0;
+    Buf dt, pot, ilist, stage, bcnt, misc;    // misc: {BtsCtl ctl; unsigned arrive; int hist[64]}
+    BtsCtl *h_ctl = nullptr;                  // pinned
+    bool ready = false;
+    double time = 0.0;
+    long long block_steps = 0, particle_steps = 0;
+    double device_ms = 0.0, wall_ms = 0.0;
+    long long timed_steps = 0;
+    std::vector<int> hist_ni;
+    cudaEvent_t ev[2] = {nullptr, nullptr};
+};
+
+static BtsArgs bts_args(s2_bts *b)
+{
+    s2_ctx *ctx = b->ctx;
+    BtsArgs a{};
+    for (int k = 0; k < nfields(ctx->order); ++k) a.f[k] = base_field(ctx, k);
+    a.dt = (double *)b->dt.p;
+    a.pot = (double *)b->pot.p;
+    a.rec = (const double *)ctx->result.p;
+    a.ilist = (int *)b->ilist.p;
+    a.stage = (int *)b->stage.p;
+    a.bcnt = (int *)b->bcnt.p;
+    a.ctl = (BtsCtl *)b->misc.p;
+    a.arrive = (unsigned *)((char *)b->misc.p + 32);
+    a.hist = (int *)((char *)b->misc.p + 64);
+    a.h_ctl = b->h_ctl;
+    a.n = b->n;
+    a.order = ctx->order;
+    a.eta = b->eta; a.eta_start = b->eta_start; a.dt_max = b->dt_max; a.dt_min = b->dt_min;
+    return a;
+}
+
+static int bts_predict_dev_time(s2_bts *b)   // predict every j to the device-resident t_next
+{
+    s2_ctx *ctx = b->ctx;
+    PredictArgs p{};
+    const int nf = nfields(ctx->order), np = nplanes(ctx->order), nq = n_qplanes(ctx->precision, ctx->order);
+    for (int k = 0; k < nf; ++k) p.f[k] = base_field(ctx, k);
+    p.id = base_id(ctx);
+    for (int k = 0; k < np; ++k) p.p[k] = plane(ctx, k);
+    for (int k = 0; k < nq; ++k) p.q[k] = qplane(ctx, k);
+    p.t = 0.0;
+    p.t_dev = &((BtsCtl *)b->misc.p)->t_next;
+    p.nj = b->n;
+    p.order = ctx->order;
+    p.precision = ctx->precision;
+    CU(launch_predict(p, ctx->stream));
+    ctx->launches++;
+    ctx->predicted = true;
+    ctx->nj_pred = b->n;
+    ctx->calc_done = false;
+    return S2_OK;
+}
+
+static int bts_select(s2_bts *b, double t_now, bool host_time)
+{
+    s2_ctx *ctx = b->ctx;
+    const int nb = (b->n + kSelPerBlock - 1) / kSelPerBlock;
+    bts_select_kernel<<<nb, kSelThreads, 0, ctx->stream>>>(bts_args(b), t_now, host_time ? 1 : 0);
+    CU(cudaGetLastError());
+    ctx->launches++;
+    return S2_OK;
+}
+
+// ---- the ABI (include/s2b200.h, "block-time-step integrator") ------------------------------------------------------
+
+extern "C" int s2_bts_open(s2_bts **out, s2_ctx *ctx, int n, double eps2, double eta, double eta_start, double dt_max,
+                           double dt_min)
+{
+    if (!out) return S2_EINVAL;
+    *out = nullptr;
+    if (!ctx || n <= 0 || n > ctx->nj_cap || (ctx->order != 4 && ctx->order != 6)) return S2_EINVAL;
+    int e1, e2;
+    if (!(eta > 0) || !(eta_start > 0) || !(dt_min > 0) || !(dt_max >= dt_min) || dt_max > 1.0 || eps2 < 0) return S2_EINVAL;
+    if (frexp(dt_max, &e1) != 0.5 || frexp(dt_min, &e2) != 0.5 || e2 < -62) return S2_EINVAL;   // powers of two, level <= 63
+    CU(cudaSetDevice(ctx->device));
+    s2_bts *b = new s2_bts();
+    b->ctx = ctx; b->n = n; b->eps2 = eps2; b->eta = eta; b->eta_start = eta_start; b->dt_max = dt_max; b->dt_min = dt_min;
+    const int nb = (n + kSelPerBlock - 1) / kSelPerBlock;
+    int rc = dev_reserve(ctx, b->dt, (size_t)n * sizeof(double));
+    if (rc == S2_OK) rc = dev_reserve(ctx, b->pot, (size_t)n * sizeof(double));
+    if (rc == S2_OK) rc = dev_reserve(ctx, b->ilist, (size_t)n * sizeof(int));
+    if (rc == S2_OK) rc = dev_reserve(ctx, b->stage, (size_t)nb * kSelPerBlock * sizeof(int));
+    if (rc == S2_OK) rc = dev_reserve(ctx, b->bcnt, (size_t)nb * sizeof(int));
+    if (rc == S2_OK) rc = dev_reserve(ctx, b->misc, 64 + kLevels * sizeof(int));
+    if (rc == S2_OK) {
+        cudaError_t e = cudaHostAlloc((void **)&b->h_ctl, sizeof(BtsCtl), cudaHostAllocDefault);
+        if (e == cudaSuccess) e = cudaEventCreate(&b->ev[0]);
+        if (e == cudaSuccess) e = cudaEventCreate(&b->ev[1]);
+        if (e != cudaSuccess) rc = fail_cuda(ctx, e);
+    }
+    if (rc != S2_OK) {
+        s2_bts_close(b);
+        return rc;
+    }
+    *out = b;
+    return S2_OK;
+}
+
+extern "C" int s2_bts_close(s2_bts *b)
+{
+    if (!b) return S2_EINVAL;
+    s2_ctx *ctx = b->ctx;
+    cudaSetDevice(ctx->device);
+    cudaStreamSynchronize(ctx->stream);
+    for (Buf *q : {&b->dt, &b->pot, &b->ilist, &b->stage, &b->bcnt, &b->misc}) dev_release(ctx, *q);
+    if (b->h_ctl) cudaFreeHost(b->h_ctl);
+    for (auto &e : b->ev)
+        if (e) cudaEventDestroy(e);
+    delete b;
+    return S2_OK;
+}
+
+// Initial conditions at t = 0 (host arrays), start-up force evaluation(s), first steps, first active list.
+extern "C" int s2_bts_init(s2_bts *b, const double *mass, const double *pos, const double *vel)
+{
+    if (!b || !mass || !pos || !vel) return S2_EINVAL;
+    s2_ctx *ctx = b->ctx;
+    const int n = b->n;
+    CU(cudaSetDevice(ctx->device));
+    std::vector<int> addr(n);
+    std::vector<double> zero((size_t)3 * n, 0.0), tz(n, 0.0);
+    for (int i = 0; i < n; ++i) addr[i] = i;
+    int rc = s2_set_j(ctx, n, addr.data(), addr.data(), tz.data(), mass, pos, vel, zero.data(), zero.data(),
+                      ctx->order == 6 ? zero.data() : nullptr, ctx->order == 6 ? zero.data() : nullptr);
+    if (rc == S2_OK) rc = s2_commit_j(ctx);
+    if (rc != S2_OK) return rc;
+    CU(cudaMemsetAsync(b->misc.p, 0, b->misc.bytes, ctx->stream));
+    bts_iota_kernel<<<(n + 255) / 256, 256, 0, ctx->stream>>>((int *)b->ilist.p, n);
+    CU(cudaGetLastError());
+    const int passes = ctx->order == 6 ? 2 : 1;
+    for (int p = 0; p < passes; ++p) {
+        rc = s2_predict(ctx, 0.0, n);
+        if (rc == S2_OK) rc = run_force(ctx, n, (const int *)b->ilist.p, nullptr, false, b->eps2, 0, false);
+        if (rc != S2_OK) return rc;
+        BtsArgs a = bts_args(b);
+        bts_init_kernel<<<(n + 255) / 256, 256, 0, ctx->stream>>>(a, p == passes - 1);
+        CU(cudaGetLastError());
+        ctx->launches += 1;
+    }
+    b->time = 0.0;
+    b->block_steps = b->particle_steps = 0;
+    b->hist_ni.clear();
+    rc = bts_select(b, 0.0, true);
+    if (rc == S2_OK) rc = bts_predict_dev_time(b);
+    if (rc != S2_OK) return rc;
+    CU(cudaStreamSynchronize(ctx->stream));
+    CU(cudaGetLastError());
+    b->ready = true;
+    return S2_OK;
+}
+
+// Advances block step by block step until the next block time would exceed t_end or max_block_steps are done.
+// time_device != 0: CUDA events bracket the kernels of every step and their elapsed times are accumulated
+// (s2_bts_stats), at the price of two event records per step.
+extern "C" int s2_bts_run(s2_bts *b, double t_end, long long max_block_steps, int time_device, long long *steps_done)
+{
+    if (!b || max_block_steps < 0) return S2_EINVAL;
+    if (!b->ready) return S2_ESTATE;
+    s2_ctx *ctx = b->ctx;
+    CU(cudaSetDevice(ctx->device));
+    long long done = 0;
+    const auto w0 = std::chrono::steady_clock::now();
+    // ordinary calls on the context since the last run (an energy evaluation, say) may have re-predicted the j-store
+    // to another time: predict to the pending block time again (one launch per s2_bts_run, not per step)
+    if (int rc = bts_predict_dev_time(b); rc != S2_OK) return rc;
+    while (done < max_block_steps && b->h_ctl->t_next <= t_end) {
+        const double t_new = b->h_ctl->t_next;
+        const int n_act = b->h_ctl->n_next;
+        if (n_act <= 0 || n_act > b->n) return S2_ESTATE;
+        // the j-particles were already predicted to t_new (enqueued behind the previous select)
+        if (time_device) CU(cudaEventRecord(b->ev[0], ctx->stream));
+        int rc = run_force(ctx, n_act, (const int *)b->ilist.p, nullptr, false, b->eps2, 0, false);
+        if (rc != S2_OK) return rc;
+        BtsArgs a = bts_args(b);
+        a.n_act = n_act;
+        bts_correct_kernel<<<(n_act + 127) / 128, 128, 0, ctx->stream>>>(a);
+        CU(cudaGetLastError());
+        ctx->launches++;
+        rc = bts_select(b, 0.0, false);
+        if (rc == S2_OK) rc = bts_predict_dev_time(b);
+        if (rc != S2_OK) return rc;
+        if (time_device) CU(cudaEventRecord(b->ev[1], ctx->stream));
+        CU(cudaStreamSynchronize(ctx->stream));          // the one synchronisation of a block step: 12 bytes in pinned memory
+        if (time_device) {
+            float ms = 0.f;
+            CU(cudaEventElapsedTime(&ms, b->ev[0], b->ev[1]));
+            b->device_ms += ms;
+            b->timed_steps++;
+        }
+        b->time = t_new;
+        b->block_steps++;
+        b->particle_steps += n_act;
+        b->hist_ni.push_back(n_act);
+        ++done;
+    }
+    CU(cudaGetLastError());
+    b->wall_ms += std::chrono::duration<double, std::milli>(std::chrono::steady_clock::now() - w0).count();
+    if (steps_done) *steps_done = done;
+    return S2_OK;
+}
+
+extern "C" int s2_bts_get_state(s2_bts *b, double *time, double *t, double *dt, double *pos, double *vel, double *acc,
+                                double *jerk, double *pot)
+{
+    if (!b) return S2_EINVAL;
+    if (!b->ready) return S2_ESTATE;
+    s2_ctx *ctx = b->ctx;
+    const int n = b->n;
+    CU(cudaSetDevice(ctx->device));
+    std::vector<double> h((size_t)15 * n);
+    CU(cudaMemcpyAsync(h.data(), base_field(ctx, 0), (size_t)n * sizeof(double), cudaMemcpyDeviceToHost, ctx->stream));
+    for (int f = 2; f < 14; ++f)
+        CU(cudaMemcpyAsync(h.data() + (size_t)(f - 1) * n, base_field(ctx, f), (size_t)n * sizeof(double), cudaMemcpyDeviceToHost,
+                           ctx->stream));
+    CU(cudaMemcpyAsync(h.data() + (size_t)13 * n, b->dt.p, (size_t)n * sizeof(double), cudaMemcpyDeviceToHost, ctx->stream));
+    CU(cudaMemcpyAsync(h.data() + (size_t)14 * n, b->pot.p, (size_t)n * sizeof(double), cudaMemcpyDeviceToHost, ctx->stream));
+    CU(cudaStreamSynchronize(ctx->stream));
+    if (time) *time = b->time;
+    double *vecs[4] = {pos, vel, acc, jerk};
+    for (int i = 0; i < n; ++i) {
+        if (t) t[i] = h[i];
+        if (dt) dt[i] = h[(size_t)13 * n + i];
+        if (pot) pot[i] = h[(size_t)14 * n + i];
+        for (int v = 0; v < 4; ++v)
+            if (vecs[v])
+                for (int c = 0; c < 3; ++c) vecs[v][3 * (size_t)i + c] = h[(size_t)(1 + 3 * v + c) * n + i];
+    }
+    return S2_OK;
+}
+
+extern "C" int s2_bts_stats(const s2_bts *b, double *time, double *t_next, int *n_next, long long *block_steps,
+                            long long *particle_steps, double *wall_ms, double *device_ms, long long *timed_steps)
+{
+    if (!b) return S2_EINVAL;
+    if (time) *time = b->time;
+    if (t_next) *t_next = b->ready ? b->h_ctl->t_next : 0.0;
+    if (n_next) *n_next = b->ready ? b->h_ctl->n_next : 0;
+    if (block_steps) *block_steps = b->block_steps;
+    if (particle_steps) *particle_steps = b->particle_steps;
+    if (wall_ms) *wall_ms = b->wall_ms;
+    if (device_ms) *device_ms = b->device_ms;
+    if (timed_steps) *timed_steps = b->timed_steps;
+    return S2_OK;
+}
+
+extern "C" int s2_bts_get_history(const s2_bts *b, long long first, int count, int *n_active)
+{
+    if (!b || first < 0 || count < 0 || (count > 0 && !n_active)) return S2_EINVAL;
+    if (first + count > (long long)b->hist_ni.size()) return S2_ERANGE;
+    for (int k = 0; k < count; ++k) n_active[k] = b->hist_ni[(size_t)first + k];
+    return S2_OK;
+}

@@ -55,6 +55,7 @@ struct PredictArgs {
     double2 *p[kMaxPlanes];        // fp64 planes (always written)
     float4 *q[kMaxPlanes];         // precision-specific planes or nullptr
     double t;
+    const double *t_dev;           // when non-null the prediction time is read from device memory (block-step integrator)
     int nj;
     int order;
     int precision;

@@ -57,7 +57,7 @@ __global__ void __launch_bounds__(256) predict_kernel(PredictArgs a)
 {
     int j = blockIdx.x * blockDim.x + threadIdx.x;
     if (j >= a.nj) return;
-    const double dt = a.t - a.f[0][j];
+    const double dt = (a.t_dev ? *a.t_dev : a.t) - a.f[0][j];
     const double m = a.f[1][j];
     const int id = a.id[j];
     const double h2 = 0.5 * dt, h3 = dt * (1.0 / 3.0);

@@ -216,3 +216,57 @@ class Hermite6(Hermite4):
         self.particle_steps += act.size
         self.active_hist.append(act.size)
         return act.size
+
+
+class DeviceHermite:
+    """The same two schemes with everything on the device (include/s2b200.h, s2_bts_*): the library's j-store is the
+    particle state, corrector / time-step rule / active-set selection are kernels, and a block step costs the host one
+    12-byte read.  Hermite4 / Hermite6 above are its host reference (the tests run both in lock-step)."""
+
+    def __init__(self, mass, pos, vel, eps2: float, order: int = 4, precision: int = 0, eta: float | None = None,
+                 eta_start: float | None = None, dt_max: float = 2.0 ** -3, dt_min: float = 2.0 ** -40, device: int = 0):
+        from . import binding as s2
+        self.s2, self.order, self.eps2 = s2, order, float(eps2)
+        self.n = int(np.asarray(mass).shape[0])
+        self.m = np.ascontiguousarray(mass, dtype=np.float64)
+        eta = (0.01 if order == 4 else 0.1) if eta is None else eta
+        eta_start = (0.0025 if order == 4 else 0.01) if eta_start is None else eta_start
+        self.ctx = s2.s2_open(device, order, precision, nj_capacity=self.n, ngb_cap=0)
+        self.bts = s2.s2_bts_open(self.ctx, self.n, eps2, eta, eta_start, dt_max, dt_min)
+        s2.s2_bts_init(self.bts, self.m, pos, vel)
+
+    def step(self) -> int:
+        """One block step; returns its active count."""
+        assert self.s2.s2_bts_run(self.bts, np.inf, 1) == 1
+        return int(self.s2.s2_bts_get_history(self.bts, self.stats()["block_steps"] - 1, 1)[0])
+
+    def run_until(self, t_end: float, time_device: bool = False) -> int:
+        return self.s2.s2_bts_run(self.bts, float(t_end), time_device=time_device)
+
+    def state(self) -> dict:
+        return self.s2.s2_bts_get_state(self.bts)
+
+    def stats(self) -> dict:
+        return self.s2.s2_bts_stats(self.bts)
+
+    def history(self) -> np.ndarray:
+        return self.s2.s2_bts_get_history(self.bts)
+
+    @property
+    def time(self) -> float:
+        return self.stats()["time"]
+
+    def energy(self) -> float:
+        """T + 1/2 sum m pot at a synchronisation time (every particle at the same t), potential from a force call."""
+        s2 = self.s2
+        st = self.state()
+        assert (st["t"] == st["t"][0]).all(), "energy() needs a synchronisation time"
+        s2.s2_predict(self.ctx, float(st["t"][0]), self.n)
+        s2.s2_calc_ilist(self.ctx, np.arange(self.n, dtype=np.int32), None, self.eps2, 0)
+        pot = s2.s2_get_results(self.ctx, self.n)["pot"]
+        kin = 0.5 * float((self.m * (st["vel"] * st["vel"]).sum(axis=1)).sum())
+        return kin + 0.5 * float((self.m * pot).sum())
+
+    def close(self):
+        self.s2.s2_bts_close(self.bts)
+        self.s2.s2_close(self.ctx)

@@ -91,3 +91,55 @@ def test_sixth_order_driver_gpu_follows_oracle_run():
     print(f"6th order: block steps {g.block_steps}, mean active {np.mean(g.active_hist):.1f}, dE/E = {(e1 - e0) / e0:.2e}")
     assert abs((e1 - e0) / e0) < 1e-8
     gb.close()
+
+
+@pytest.mark.gpu
+@pytest.mark.parametrize("order,precision,steps,tol", [(4, "fp64", 300, 1e-9), (4, "ds", 150, 1e-7), (6, "fp64", 150, 1e-9)])
+def test_device_integrator_follows_host_reference_in_lockstep(order, precision, steps, tol):
+    """The device-resident integrator (s2_bts_*: corrector, time-step rule and active-set selection in kernels, the
+    j-store as particle state) against hermite.py driven by the ORACLE, block step by block step: same active counts and
+    block times at every step, identical t and dt arrays, positions and velocities within tol."""
+    import paper_1510_04068_b200 as s2
+    from paper_1510_04068_b200.hermite import DeviceHermite
+    w = _plummer(256)
+    P = {"fp64": s2.S2_FP64, "ds": s2.S2_DS}[precision]
+    d = DeviceHermite(w.mass, w.pos, w.vel, w.eps2, order=order, precision=P)
+    H = Hermite4 if order == 4 else Hermite6
+    o = H(OracleBackend(w.N, w.eps2, order=order), w.mass, w.pos, w.vel)
+    st = d.state()
+    assert np.array_equal(st["dt"], o.dt) and np.allclose(st["acc"], o.a, rtol=1e-9, atol=0)
+    for k in range(steps):
+        na, nb = d.step(), o.step()
+        assert na == nb and d.time == o.time, (k, na, nb, d.time, o.time)
+    st = d.state()
+    assert np.array_equal(st["t"], o.t) and np.array_equal(st["dt"], o.dt)
+    assert np.abs(st["pos"] - o.x).max() < tol and np.abs(st["vel"] - o.v).max() < tol
+    assert np.array_equal(d.history(), np.array(o.active_hist))
+    stats = d.stats()
+    assert stats["block_steps"] == steps and stats["particle_steps"] == sum(o.active_hist)
+    d.close()
+
+
+@pytest.mark.gpu
+def test_device_integrator_conserves_energy_and_reaches_t_end():
+    import paper_1510_04068_b200 as s2
+    from paper_1510_04068_b200.hermite import DeviceHermite
+    w = make_config(1, N=1024)
+    for order, lim in ((4, 1e-6), (6, 1e-7)):
+        d = DeviceHermite(w.mass, w.pos, w.vel, w.eps2, order=order)
+        e0 = d.energy()
+        d.run_until(0.125)
+        st = d.state()
+        assert (st["t"] == 0.125).all() and st["time"] == 0.125
+        assert np.all(np.log2(st["dt"]) == np.round(np.log2(st["dt"]))) and np.all(np.fmod(st["t"], st["dt"]) == 0.0)
+        e1 = d.energy()
+        d.run_until(0.25, time_device=True)            # continues after the energy evaluation re-predicted the store
+        e2 = d.energy()
+        hist = d.history()
+        stats = d.stats()
+        print(f"order {order}: {stats['block_steps']} block steps, n_i min/median/max {hist.min()}/{np.median(hist)}/{hist.max()}, "
+              f"dE/E {(e1 - e0) / e0:.2e} {(e2 - e0) / e0:.2e}, wall/step {stats['wall_ms'] / stats['block_steps'] * 1e3:.1f} us, "
+              f"device/step {stats['device_ms'] / max(1, stats['timed_steps']) * 1e3:.1f} us")
+        assert abs((e1 - e0) / e0) < lim and abs((e2 - e0) / e0) < lim
+        assert hist.min() < w.N // 8 and hist.max() == w.N
+        d.close()
