@@ -60,8 +60,12 @@ def parse_args():
     ap.add_argument("--section", default="all", choices=["all", "hbm"],
                     help="hbm: only the streaming-kernel (predictor / scatter) measurement, for ncu captures")
     ap.add_argument("--blockstep", type=int, default=0, metavar="N",
-                    help="second workload (not the default line): block-time-step Hermite run of an N-particle Plummer "
-                         "sphere for 1/8 time unit in fp64 and double-single; prints one JSON line of statistics")
+                    help="second workload (not the default line): block-time-step Hermite runs of an N-particle Plummer "
+                         "sphere with the device-resident integrator, 4th and 6th order, fp64 and double-single; prints one "
+                         "JSON line of statistics")
+    ap.add_argument("--bs-tend", type=float, default=1.0, help="end time of the --blockstep runs (N-body time units)")
+    ap.add_argument("--bs-orders", default="4,6")
+    ap.add_argument("--bs-precisions", default="fp64,ds")
     return ap.parse_args()
 
 
@@ -170,7 +174,8 @@ def main():
         return
     if args.blockstep:
         if rank == 0:
-            run_blockstep(args.blockstep)
+            run_blockstep(args.blockstep, args.bs_tend, tuple(int(x) for x in args.bs_orders.split(",")),
+                          tuple(args.bs_precisions.split(",")))
         return
     if args.section == "hbm":
         if rank == 0:
@@ -359,27 +364,63 @@ def main():
         dist.destroy_process_group()
 
 
-def run_blockstep(n):
-    """PAPER.md sec 3.7 (L152-L168) in miniature: the host Hermite driver on the library, fp64 versus double-single."""
+def run_blockstep(n, t_end=1.0, orders=(4, 6), precisions=("fp64", "ds"), host_reference=True):
+    """PAPER.md sec 3.7 (L152-L168), the second workload: block-time-step Hermite runs of an N-particle Plummer sphere
+    for t_end N-body time units with the device-resident integrator (s2_bts_*), 4th order (eta = 0.01) and 6th order
+    (eta = 0.1, the paper's scheme), fp64 and double-single.  Reports wall time per block step, the summed device time
+    of the same steps (second, event-timed run over the first 1/8 time unit), the active-set statistics and dE/E (the
+    paper quotes ~1e-12 in double and ~1e-10 in double-single for its 6th-order runs, L164: context).  The host driver
+    of round 1 (hermite.py on s2_set_j / s2_calc_ilist / s2_get_results) runs the first 1/8 time unit for comparison."""
     import paper_1510_04068_b200 as s2
-    from paper_1510_04068_b200.hermite import Hermite4, S2Backend
+    from paper_1510_04068_b200.hermite import DeviceHermite, Hermite4, Hermite6, S2Backend
     from workloads import make_config
     w = make_config(3, N=n)
-    out = {"workload": f"block-time-step 4th-order Hermite, Plummer N={n}, eps={w.notes['eps']:.3g}, eta=0.01, t=0..1/8", "runs": []}
-    for name, prec in (("fp64", s2.S2_FP64), ("ds", s2.S2_DS)):
-        b = S2Backend(w.N, w.eps2, precision=prec)
-        h = Hermite4(b, w.mass, w.pos, w.vel)
-        e0 = h.energy()
-        b.calls = b.pairs = 0
-        t0 = time.perf_counter()
-        h.run_until(0.125)
-        wall = time.perf_counter() - t0
-        e1 = h.energy()
-        sizes = np.array(h.active_hist)
-        out["runs"].append({"precision": name, "block_steps": h.block_steps, "particle_steps": h.particle_steps,
-                            "n_i_min": int(sizes.min()), "n_i_median": float(np.median(sizes)), "n_i_max": int(sizes.max()),
-                            "wall_s": wall, "ginteractions_per_s_wall": b.pairs / wall / 1e9, "dE_over_E": (e1 - e0) / e0})
-        b.close()
+    P = {"fp64": s2.S2_FP64, "ds": s2.S2_DS, "fp32": s2.S2_FP32}
+    out = {"workload": f"block-time-step Hermite, Plummer N={n}, eps={w.notes['eps']:.3g}, t=0..{t_end}, eta4=0.01 eta6=0.1, "
+                       f"dt_max=1/8", "runs": []}
+    for order in orders:
+        for name in precisions:
+            d = DeviceHermite(w.mass, w.pos, w.vel, w.eps2, order=order, precision=P[name])
+            e0 = d.energy()
+            t0 = time.perf_counter()
+            d.run_until(t_end)
+            wall = time.perf_counter() - t0
+            e1 = d.energy()
+            st, hist = d.stats(), d.history()
+            d.close()
+            # the same steps again, event-timed, for the summed device time (first 1/8 time unit)
+            d = DeviceHermite(w.mass, w.pos, w.vel, w.eps2, order=order, precision=P[name])
+            d.run_until(min(t_end, 0.125), time_device=True)
+            sd = d.stats()
+            d.close()
+            d = DeviceHermite(w.mass, w.pos, w.vel, w.eps2, order=order, precision=P[name])
+            t0 = time.perf_counter()
+            d.run_until(min(t_end, 0.125))
+            wall8 = time.perf_counter() - t0
+            d.close()
+            row = {"integrator": "device (s2_bts)", "order": order, "precision": name, "block_steps": st["block_steps"],
+                   "particle_steps": st["particle_steps"], "n_i_min": int(hist.min()), "n_i_median": float(np.median(hist)),
+                   "n_i_mean": float(hist.mean()), "n_i_max": int(hist.max()), "wall_s": wall,
+                   "wall_us_per_block_step": wall / st["block_steps"] * 1e6,
+                   "ginteractions_per_s_wall": st["particle_steps"] * n / wall / 1e9, "dE_over_E": (e1 - e0) / e0,
+                   "first_eighth": {"block_steps": sd["block_steps"], "wall_us_per_block_step": wall8 / sd["block_steps"] * 1e6,
+                                    "device_us_per_block_step": sd["device_ms"] / sd["timed_steps"] * 1e3,
+                                    "wall_over_device": wall8 * 1e3 / sd["device_ms"]}}
+            out["runs"].append(row)
+            print(json.dumps(row), file=sys.stderr, flush=True)
+    if host_reference:
+        for order, H in ((4, Hermite4), (6, Hermite6)):
+            if order not in orders:
+                continue
+            b = S2Backend(w.N, w.eps2, precision=s2.S2_FP64, order=order)
+            h = H(b, w.mass, w.pos, w.vel)
+            b.calls = b.pairs = 0
+            t0 = time.perf_counter()
+            h.run_until(min(t_end, 0.125))
+            wall = time.perf_counter() - t0
+            out["runs"].append({"integrator": "host driver (hermite.py), first 1/8 time unit", "order": order, "precision": "fp64",
+                                "block_steps": h.block_steps, "wall_s": wall, "wall_us_per_block_step": wall / h.block_steps * 1e6})
+            b.close()
     print(json.dumps(out), flush=True)
 
 

@@ -26,6 +26,7 @@
 #include <chrono>
 
 #include "s2_ctx.h"
+#include "s2_predict.cuh"
 
 using namespace s2;
 
@@ -33,8 +34,7 @@ namespace {
 
 constexpr int kLevels = 64;          // dt = 2^-level, level 0 .. 63
 constexpr int kSelThreads = 256;
-constexpr int kSelPerThread = 8;
-constexpr int kSelPerBlock = kSelThreads * kSelPerThread;
+constexpr int kSelPerBlock = kSelThreads;   // particles per block of the select kernel (one per thread)
 
 struct BtsCtl {                      // device control block (also mirrored to pinned host memory by the select kernel)
     double t_next;                   // time of the block step that is about to run
@@ -111,6 +111,10 @@ __global__ void __launch_bounds__(256) bts_init_kernel(BtsArgs a, int final_pass
 //   dt' = eta (A1 / A4)^(1/3),  A1 = sqrt(|a1||s1| + |j1|^2),  A4 = sqrt(|a3||a5| + |a4|^2)
 __global__ void __launch_bounds__(128) bts_correct_kernel(BtsArgs a)
 {
+    // programmatic dependent launch along the chain sweep -> (reduce) -> correct -> select -> predict: every kernel lets
+    // its successor be staged at once and waits for its predecessor's results itself
+    asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
+    asm volatile("griddepcontrol.wait;" ::: "memory");
     const int k = blockIdx.x * blockDim.x + threadIdx.x;
     if (k >= a.n_act) return;
     const int i = a.ilist[k];
@@ -174,67 +178,87 @@ __global__ void __launch_bounds__(128) bts_correct_kernel(BtsArgs a)
     }
 }
 
-// ---- next block time and next active list --------------------------------------------------------------------
-// Every block derives dt_min from the level histogram (64 loads), hence t_next = t_now + dt_min, compacts the active
-// particles of its 2048-particle slice (ascending) into its staging segment and publishes its count; the last block
-// to arrive concatenates the segments in block order -- the list is ascending by address whatever the arrival
-// order -- and writes {t_next, n_next} to the device control block and to pinned host memory.
-__global__ void __launch_bounds__(kSelThreads) bts_select_kernel(BtsArgs a, double t_now_host, int use_host_time)
+// ---- next block time, next active list, and the prediction of the j-store to that time: one launch -------------
+// Every block (256 particles, one per thread) derives dt_min from the level histogram (64 parallel loads and two
+// ballots), hence t_next = t_now + dt_min; predicts its particles to t_next (predict_one: the same arithmetic as
+// predict_kernel); compacts its active particles (ascending) into its staging segment by ballot + popc and publishes
+// its count.  The last block to arrive concatenates the segments in block order -- the list is ascending by address
+// whatever the arrival order -- and writes {t_next, n_next} to the device control block and to pinned host memory.
+template <int ORDER>
+__global__ void __launch_bounds__(kSelThreads) bts_select_predict_kernel(BtsArgs a, PredictArgs pa, double t_now_host, int use_host_time)
 {
     __shared__ int s_w[kSelThreads / 32];
+    __shared__ unsigned s_hist[2];
     __shared__ int s_last;
-    __shared__ double s_tnext;
-    if (threadIdx.x == 0) {
-        int lev = 0;
-        for (int l = kLevels - 1; l >= 0; --l)
-            if (a.hist[l] > 0) { lev = l; break; }
-        const double t_now = use_host_time ? t_now_host : a.ctl->t_next;
-        s_tnext = t_now + scalbn(1.0, -lev);
-    }
-    __syncthreads();
-    const double t_next = s_tnext;
+    __shared__ int s_off[kSelThreads + 1];
+    asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
+    asm volatile("griddepcontrol.wait;" ::: "memory");
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    const int i0 = blockIdx.x * kSelPerBlock + threadIdx.x * kSelPerThread;
-    unsigned mask = 0;
-    int cnt = 0;
-#pragma unroll
-    for (int k = 0; k < kSelPerThread; ++k) {
-        const int i = i0 + k;
-        if (i < a.n) {
-            const double x = t_next / a.dt[i];           // exact: dt is a power of two
-            if (x == floor(x)) { mask |= 1u << k; ++cnt; }
-        }
+    if (threadIdx.x < kLevels) {
+        const unsigned b = __ballot_sync(0xffffffffu, a.hist[threadIdx.x] > 0);
+        if (lane == 0) s_hist[warp] = b;
     }
-    int incl = cnt;
-#pragma unroll
-    for (int m = 1; m < 32; m <<= 1) {
-        const int o = __shfl_up_sync(0xffffffffu, incl, m);
-        if (lane >= m) incl += o;
-    }
-    if (lane == 31) s_w[warp] = incl;
     __syncthreads();
-    int base = incl - cnt;
-    for (int w = 0; w < warp; ++w) base += s_w[w];
-    int *seg = a.stage + (size_t)blockIdx.x * kSelPerBlock;
+    const int lev = s_hist[1] ? 63 - __clz(s_hist[1]) : 31 - __clz(s_hist[0] | 1u);   // highest occupied level = smallest step
+    const double t_next = (use_host_time ? t_now_host : a.ctl->t_next) + scalbn(1.0, -lev);
+    const int i = blockIdx.x * kSelThreads + threadIdx.x;
+    bool act = false;
+    if (i < a.n) {
+        const double x = t_next / a.dt[i];               // exact: dt is a power of two
+        act = x == floor(x);
+        predict_one<ORDER>(pa, i, t_next);
+    }
+    const unsigned bal = __ballot_sync(0xffffffffu, act);
+    if (lane == 0) s_w[warp] = __popc(bal);
+    __syncthreads();
+    int base = __popc(bal & ((1u << lane) - 1u));
+    int total = 0;
 #pragma unroll
-    for (int k = 0; k < kSelPerThread; ++k)
-        if (mask & (1u << k)) seg[base++] = i0 + k;
-    if (threadIdx.x == kSelThreads - 1) {
-        a.bcnt[blockIdx.x] = base;                       // the last thread's running position = the block's count
-        __threadfence();
+    for (int w = 0; w < kSelThreads / 32; ++w) {
+        if (w < warp) base += s_w[w];
+        total += s_w[w];
+    }
+    if (act) a.stage[(size_t)blockIdx.x * kSelThreads + base] = i;
+    if (threadIdx.x == 0) a.bcnt[blockIdx.x] = total;
+    __threadfence();
+    __syncthreads();
+    if (threadIdx.x == 0) {
         const unsigned prev = atomicAdd(a.arrive, 1u);
         s_last = prev == gridDim.x - 1;
     }
     __syncthreads();
     if (!s_last) return;
     __threadfence();
-    // last block: concatenate the staging segments in block order
+    // last block: exclusive scan of the block counts, kSelThreads at a time, then a flat copy of each chunk's members
     int off = 0;
-    for (int b = 0; b < (int)gridDim.x; ++b) {
-        const int c = __ldcg(a.bcnt + b);
-        const int *src = a.stage + (size_t)b * kSelPerBlock;
-        for (int k = threadIdx.x; k < c; k += kSelThreads) a.ilist[off + k] = __ldcg(src + k);
-        off += c;
+    for (int b0 = 0; b0 < (int)gridDim.x; b0 += kSelThreads) {
+        const int b = b0 + threadIdx.x;
+        const int c = b < (int)gridDim.x ? __ldcg(a.bcnt + b) : 0;
+        int incl = c;
+#pragma unroll
+        for (int m = 1; m < 32; m <<= 1) {
+            const int o = __shfl_up_sync(0xffffffffu, incl, m);
+            if (lane >= m) incl += o;
+        }
+        __syncthreads();
+        if (lane == 31) s_w[warp] = incl;
+        __syncthreads();
+        int wb = 0;
+        for (int w = 0; w < warp; ++w) wb += s_w[w];
+        s_off[threadIdx.x] = wb + incl - c;
+        if (threadIdx.x == kSelThreads - 1) s_off[kSelThreads] = wb + incl;
+        __syncthreads();
+        const int chunk_total = s_off[kSelThreads];
+        for (int k = threadIdx.x; k < chunk_total; k += kSelThreads) {
+            int lo = 0, hi = kSelThreads - 1;            // block of member k: last lb with s_off[lb] <= k
+            while (lo < hi) {
+                const int mid = (lo + hi + 1) >> 1;
+                if (s_off[mid] <= k) lo = mid; else hi = mid - 1;
+            }
+            a.ilist[off + k] = __ldcg(a.stage + (size_t)(b0 + lo) * kSelThreads + (k - s_off[lo]));
+        }
+        off += chunk_total;
+        __syncthreads();
     }
     if (threadIdx.x == 0) {
         *a.arrive = 0u;
@@ -255,6 +279,18 @@ __global__ void bts_iota_kernel(int *p, int n)
 
 namespace s2 {
 cudaError_t launch_predict(const PredictArgs &a, cudaStream_t st);
+}
+
+template <class K, class A, class... R>
+static cudaError_t launch_pdl(K kern, dim3 grid, dim3 block, cudaStream_t st, const A &a, R... rest)
+{
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = grid; cfg.blockDim = block; cfg.stream = st;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    at[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = at; cfg.numAttrs = 1;
+    return cudaLaunchKernelEx(&cfg, kern, a, rest...);
 }
 
 struct s2_bts {
@@ -293,7 +329,7 @@ static BtsArgs bts_args(s2_bts *b)
     return a;
 }
 
-static int bts_predict_dev_time(s2_bts *b)   // predict every j to the device-resident t_next
+static PredictArgs bts_predict_args(s2_bts *b)
 {
     s2_ctx *ctx = b->ctx;
     PredictArgs p{};
@@ -307,7 +343,14 @@ static int bts_predict_dev_time(s2_bts *b)   // predict every j to the device-re
     p.nj = b->n;
     p.order = ctx->order;
     p.precision = ctx->precision;
-    CU(launch_predict(p, ctx->stream));
+    p.pdl = 1;
+    return p;
+}
+
+static int bts_predict_dev_time(s2_bts *b)   // predict every j to the device-resident t_next (stand-alone launch)
+{
+    s2_ctx *ctx = b->ctx;
+    CU(launch_predict(bts_predict_args(b), ctx->stream));
     ctx->launches++;
     ctx->predicted = true;
     ctx->nj_pred = b->n;
@@ -315,13 +358,19 @@ static int bts_predict_dev_time(s2_bts *b)   // predict every j to the device-re
     return S2_OK;
 }
 
-static int bts_select(s2_bts *b, double t_now, bool host_time)
+// next block time + next active list + prediction to that time, one launch
+static int bts_select_predict(s2_bts *b, double t_now, bool host_time)
 {
     s2_ctx *ctx = b->ctx;
     const int nb = (b->n + kSelPerBlock - 1) / kSelPerBlock;
-    bts_select_kernel<<<nb, kSelThreads, 0, ctx->stream>>>(bts_args(b), t_now, host_time ? 1 : 0);
-    CU(cudaGetLastError());
+    if (ctx->order == 6)
+        CU(launch_pdl(bts_select_predict_kernel<6>, dim3(nb), dim3(kSelThreads), ctx->stream, bts_args(b), bts_predict_args(b), t_now, host_time ? 1 : 0));
+    else
+        CU(launch_pdl(bts_select_predict_kernel<4>, dim3(nb), dim3(kSelThreads), ctx->stream, bts_args(b), bts_predict_args(b), t_now, host_time ? 1 : 0));
     ctx->launches++;
+    ctx->predicted = true;
+    ctx->nj_pred = b->n;
+    ctx->calc_done = false;
     return S2_OK;
 }
 
@@ -404,8 +453,7 @@ extern "C" int s2_bts_init(s2_bts *b, const double *mass, const double *pos, con
     b->time = 0.0;
     b->block_steps = b->particle_steps = 0;
     b->hist_ni.clear();
-    rc = bts_select(b, 0.0, true);
-    if (rc == S2_OK) rc = bts_predict_dev_time(b);
+    rc = bts_select_predict(b, 0.0, true);
     if (rc != S2_OK) return rc;
     CU(cudaStreamSynchronize(ctx->stream));
     CU(cudaGetLastError());
@@ -437,11 +485,9 @@ extern "C" int s2_bts_run(s2_bts *b, double t_end, long long max_block_steps, in
         if (rc != S2_OK) return rc;
         BtsArgs a = bts_args(b);
         a.n_act = n_act;
-        bts_correct_kernel<<<(n_act + 127) / 128, 128, 0, ctx->stream>>>(a);
-        CU(cudaGetLastError());
+        CU(launch_pdl(bts_correct_kernel, dim3((n_act + 127) / 128), dim3(128), ctx->stream, a));
         ctx->launches++;
-        rc = bts_select(b, 0.0, false);
-        if (rc == S2_OK) rc = bts_predict_dev_time(b);
+        rc = bts_select_predict(b, 0.0, false);
         if (rc != S2_OK) return rc;
         if (time_device) CU(cudaEventRecord(b->ev[1], ctx->stream));
         CU(cudaStreamSynchronize(ctx->stream));          // the one synchronisation of a block step: 12 bytes in pinned memory

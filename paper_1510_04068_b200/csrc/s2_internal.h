@@ -56,6 +56,7 @@ struct PredictArgs {
     float4 *q[kMaxPlanes];         // precision-specific planes or nullptr
     double t;
     const double *t_dev;           // when non-null the prediction time is read from device memory (block-step integrator)
+    int pdl;                       // launch with programmatic stream serialisation (the kernel waits for its predecessor itself)
     int nj;
     int order;
     int precision;

@@ -24,6 +24,8 @@ __global__ void __launch_bounds__(256) reduce_kernel(const ReduceArgs a)
     const int i = warp;
     const int S = a.nslices_total;
     // programmatic dependent launch: this grid may start while the sweep is still running; wait for its results
+    // (and let a dependent launch of its own -- the integrator's corrector -- be staged meanwhile)
+    asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
     asm volatile("griddepcontrol.wait;" ::: "memory");
     if (!(a.flags & S2_WANT_NGB)) {   // plain sums (+ nn): the same fixed-order routine the fused combine uses
         if (a.flags & S2_WANT_NN)

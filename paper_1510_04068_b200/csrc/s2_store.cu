@@ -3,6 +3,7 @@
 // buffers to GPU buffers, one kernel to predict the particles to the new time-step".
 // Both are pure streaming kernels: HBM-bound.
 #include "s2_internal.h"
+#include "s2_predict.cuh"
 
 namespace s2 {
 
@@ -38,80 +39,30 @@ cudaError_t launch_scatter(const ScatterArgs &a, cudaStream_t st)
 }
 
 // ------------------------------------------------------------------------------------------
-// Predictor (reading P2), Horner form, fp64 FMA:
-//   4th: x_p = x + dt (v + dt/2 (a + dt/3 j));                 v_p = v + dt (a + dt/2 j)
-//   6th: x_p = x + dt (v + dt/2 (a + dt/3 (j + dt/4 (s + dt/5 c))))
-//        v_p = v + dt (a + dt/2 (j + dt/3 (s + dt/4 c)));      a_p = a + dt (j + dt/2 (s + dt/3 c))
-// One thread per j: 14 (20) coalesced 8-byte reads + id, 4 (6) coalesced 16-byte plane writes,
-// plus the float / double-single planes when the context computes in those precisions.
-
-__device__ __forceinline__ float2 split_ds(double x)
-{
-    float hi = __double2float_rn(x);
-    float lo = __double2float_rn(x - (double)hi);
-    return make_float2(hi, lo);
-}
+// Predictor (a2): one thread per j, arithmetic in predict_one (s2_predict.cuh).
 
 template <int ORDER>
 __global__ void __launch_bounds__(256) predict_kernel(PredictArgs a)
 {
+    asm volatile("griddepcontrol.wait;" ::: "memory");   // no-op unless launched with programmatic stream serialisation
     int j = blockIdx.x * blockDim.x + threadIdx.x;
     if (j >= a.nj) return;
-    const double dt = (a.t_dev ? *a.t_dev : a.t) - a.f[0][j];
-    const double m = a.f[1][j];
-    const int id = a.id[j];
-    const double h2 = 0.5 * dt, h3 = dt * (1.0 / 3.0);
-    double xp[3], vp[3], ap[3];
-#pragma unroll
-    for (int c = 0; c < 3; ++c) {
-        const double x = a.f[2 + c][j], v = a.f[5 + c][j], ac = a.f[8 + c][j], jk = a.f[11 + c][j];
-        if (ORDER == 4) {
-            xp[c] = fma(dt, fma(h2, fma(h3, jk, ac), v), x);
-            vp[c] = fma(dt, fma(h2, jk, ac), v);
-            ap[c] = ac;
-        } else {
-            const double s = a.f[14 + c][j], cr = a.f[17 + c][j];
-            const double h4 = 0.25 * dt, h5 = 0.2 * dt;
-            xp[c] = fma(dt, fma(h2, fma(h3, fma(h4, fma(h5, cr, s), jk), ac), v), x);
-            vp[c] = fma(dt, fma(h2, fma(h3, fma(h4, cr, s), jk), ac), v);
-            ap[c] = fma(dt, fma(h2, fma(h3, cr, s), jk), ac);
-        }
-    }
-    const double idbits = __hiloint2double(0, id);
-    a.p[0][j] = make_double2(xp[0], xp[1]);
-    a.p[1][j] = make_double2(xp[2], m);
-    a.p[2][j] = make_double2(vp[0], vp[1]);
-    a.p[3][j] = make_double2(vp[2], idbits);
-    if (ORDER == 6) {
-        a.p[4][j] = make_double2(ap[0], ap[1]);
-        a.p[5][j] = make_double2(ap[2], 0.0);
-    }
-    if (a.precision == S2_FP32) {
-        float2 X = split_ds(xp[0]), Y = split_ds(xp[1]), Z = split_ds(xp[2]);
-        a.q[0][j] = make_float4(X.x, Y.x, Z.x, __double2float_rn(m));
-        a.q[1][j] = make_float4(X.y, Y.y, Z.y, __int_as_float(id));
-        a.q[2][j] = make_float4(__double2float_rn(vp[0]), __double2float_rn(vp[1]), __double2float_rn(vp[2]), 0.f);
-        if (ORDER == 6)
-            a.q[3][j] = make_float4(__double2float_rn(ap[0]), __double2float_rn(ap[1]), __double2float_rn(ap[2]), 0.f);
-    } else if (a.precision == S2_DS) {
-        float2 X = split_ds(xp[0]), Y = split_ds(xp[1]), Z = split_ds(xp[2]), M = split_ds(m);
-        float2 U = split_ds(vp[0]), V = split_ds(vp[1]), W = split_ds(vp[2]);
-        a.q[0][j] = make_float4(X.x, X.y, Y.x, Y.y);
-        a.q[1][j] = make_float4(Z.x, Z.y, M.x, M.y);
-        a.q[2][j] = make_float4(U.x, U.y, V.x, V.y);
-        a.q[3][j] = make_float4(W.x, W.y, __int_as_float(id), 0.f);
-        if (ORDER == 6) {
-            float2 A = split_ds(ap[0]), B = split_ds(ap[1]), Cc = split_ds(ap[2]);
-            a.q[4][j] = make_float4(A.x, A.y, B.x, B.y);
-            a.q[5][j] = make_float4(Cc.x, Cc.y, 0.f, 0.f);
-        }
-    }
+    predict_one<ORDER>(a, j, a.t_dev ? *a.t_dev : a.t);
 }
 
 cudaError_t launch_predict(const PredictArgs &a, cudaStream_t st)
 {
     if (a.nj <= 0) return cudaSuccess;
     const int grid = (a.nj + 255) / 256;
+    if (a.pdl) {
+        cudaLaunchConfig_t cfg = {};
+        cfg.gridDim = dim3(grid); cfg.blockDim = dim3(256); cfg.stream = st;
+        cudaLaunchAttribute at[1];
+        at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+        at[0].val.programmaticStreamSerializationAllowed = 1;
+        cfg.attrs = at; cfg.numAttrs = 1;
+        return a.order == 6 ? cudaLaunchKernelEx(&cfg, predict_kernel<6>, a) : cudaLaunchKernelEx(&cfg, predict_kernel<4>, a);
+    }
     if (a.order == 6)
         predict_kernel<6><<<grid, 256, 0, st>>>(a);
     else
