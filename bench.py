@@ -59,6 +59,10 @@ def parse_args():
                     help="pair-arithmetic precision of the timed step (the default bench line is fp64)")
     ap.add_argument("--section", default="all", choices=["all", "hbm"],
                     help="hbm: only the streaming-kernel (predictor / scatter) measurement, for ncu captures")
+    ap.add_argument("--shard", default="i", choices=["i", "j"],
+                    help="multi-GPU decomposition: i = every rank its own i-list against the whole store (independent units, "
+                         "weak scaling, the default line); j = the paper's scheme (L84): every rank sums ALL i over its own block "
+                         "of j and the partial results are combined by an all-reduce on device tensors (strong scaling)")
     ap.add_argument("--blockstep", type=int, default=0, metavar="N",
                     help="second workload (not the default line): block-time-step Hermite runs of an N-particle Plummer "
                          "sphere with the device-resident integrator, 4th and 6th order, fp64 and double-single; prints one "
@@ -199,11 +203,18 @@ def main():
     order, N, ni = w.order, w.N, w.N
     # i-list of this rank: its own rotation of the seeded permutation (same per-GPU work on every rank)
     from paper_1510_04068_b200.sharding import max_over_ranks, rank_ilist
-    il_host = rank_ilist(w.perm, rank, world, ni)
+    jshard = args.shard == "j"
+    il_host = w.ilist(ni) if jshard else rank_ilist(w.perm, rank, world, ni)
 
     prec = {"fp64": s2.S2_FP64, "ds": s2.S2_DS, "fp32": s2.S2_FP32}[args.precision]
     ctx = s2.s2_open(local, order, prec, nj_capacity=N, ngb_cap=0)
     s2.s2_enable_timing(ctx, True)
+    if jshard:
+        from paper_1510_04068_b200.sharding import block_shard, combine_partials
+        s2.s2_set_j_range(ctx, *block_shard(N, rank, world))
+        comb = dict(acc=torch.empty(ni * 3, dtype=torch.float64, device=dev), jerk=torch.empty(ni * 3, dtype=torch.float64, device=dev),
+                    pot=torch.empty(ni, dtype=torch.float64, device=dev))
+        h_comb = {k: torch.empty(v.shape, dtype=v.dtype).pin_memory() for k, v in comb.items()}
     addr = np.arange(N, dtype=np.int32)
     host = dict(address=addr, ident=w.ident, t=w.t_j, mass=w.mass, pos=w.pos, vel=w.vel, acc=w.acc, jerk=w.jerk,
                 snap=w.snap if order == 6 else None, crackle=w.crackle if order == 6 else None)
@@ -216,6 +227,9 @@ def main():
                               d["snap"], d["crackle"])
         s2.s2_predict(ctx, w.t_pred, N)
         s2.s2_calc_ilist_device(ctx, d_il, None, w.eps2, 0)
+        if jshard:   # the one exchange step of the paper's scheme: partial results of all i added over the ranks
+            s2.s2_get_results_device(ctx, ni, acc=comb["acc"], jerk=comb["jerk"], pot=comb["pot"])
+            combine_partials(comb["acc"], comb["jerk"], comb["pot"])
 
     def step_e2e():
         s2.s2_set_j(ctx, host["address"], host["ident"], host["t"], host["mass"], host["pos"], host["vel"], host["acc"],
@@ -223,6 +237,13 @@ def main():
         s2.s2_commit_j(ctx)
         s2.s2_predict(ctx, w.t_pred, N)
         s2.s2_calc_ilist(ctx, il_host, None, w.eps2, 0)
+        if jshard:
+            s2.s2_get_results_device(ctx, ni, acc=comb["acc"], jerk=comb["jerk"], pot=comb["pot"])
+            combine_partials(comb["acc"], comb["jerk"], comb["pot"])
+            for k in comb:
+                h_comb[k].copy_(comb[k], non_blocking=True)
+            torch.cuda.current_stream().synchronize()
+            return h_comb
         return s2.s2_get_results(ctx, ni)
 
     def barrier():
@@ -259,7 +280,7 @@ def main():
     # whole-job numbers: the slowest rank decides (sum, median and best of the per-step device times, each max over ranks)
     tot_ms, e2e_ms, med_ms, best_ms, e2e_med_ms = max_over_ranks(
         [sum(step_ms), sum(e2e_step_ms), statistics.median(step_ms), min(step_ms), statistics.median(e2e_step_ms)], device=dev)
-    pairs_step = float(ni) * N * world
+    pairs_step = float(ni) * N * (1 if jshard else world)     # j-sharding: the ranks share ONE n_i x N problem
     value = pairs_step * args.steps / (tot_ms * 1e-3) / 1e9
     e2e_value = pairs_step * args.steps / (e2e_ms * 1e-3) / 1e9
 
@@ -313,11 +334,18 @@ def main():
             "steps": args.steps, "warmup": max(args.warmup, 3), "ms_per_step": tot_ms / args.steps,
             "ms_per_step_median": med_ms, "ms_per_step_best": best_ms,
             "value_median": pairs_step / (med_ms * 1e-3) / 1e9, "value_best": pairs_step / (best_ms * 1e-3) / 1e9,
-            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": {"fp64": "f64", "ds": "f32x2 (double-single)", "fp32": "f32"}[args.precision],
+            "higher_is_better": True, "scaling": "strong" if jshard else "weak", "vs_baseline": None, "dtype": {"fp64": "f64", "ds": "f32x2 (double-single)", "fp32": "f32"}[args.precision],
             "data": "synthetic", "config": workload_config(w, ni, args.precision), "clocks": clocks,
             "e2e": {"value": e2e_value, "unit": "Ginteractions/s", "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
                     "ms_per_step": e2e_ms / args.steps, "ms_per_step_median": e2e_med_ms},
             "gpu_launches": int(launches), "roofline": roofline, "launch": s2.s2_last_launch_info(ctx)}
+    if jshard:
+        line["config"]["parallelism"] = (f"j-sharded over {world} rank(s) (PAPER.md L84): whole store on every rank, each sums all i over "
+                                         f"its own block of N/{world} j; all-reduce of acc/jerk/pot on device tensors (NCCL)")
+        # the sweep of one rank covers n_i x N/world pairs
+        for k in ("achieved", "frac", "fp64_pipe_frac_nominal"):
+            if k in roofline:
+                roofline[k] /= world
 
     if rank == 0 and world == 1 and args.precision == "fp32":
         # FP32 pipe, measured in the same process: scalar FFMA and the packed forms the tiled sweep issues
@@ -380,7 +408,7 @@ def run_blockstep(n, t_end=1.0, orders=(4, 6), precisions=("fp64", "ds"), host_r
                        f"dt_max=1/8", "runs": []}
     for order in orders:
         for name in precisions:
-            d = DeviceHermite(w.mass, w.pos, w.vel, w.eps2, order=order, precision=P[name])
+            d = DeviceHermite(w.mass, w.pos, w.vel, w.eps2, order=order, precision=P[name], averaged=order == 6)
             e0 = d.energy()
             t0 = time.perf_counter()
             d.run_until(t_end)
@@ -389,16 +417,16 @@ def run_blockstep(n, t_end=1.0, orders=(4, 6), precisions=("fp64", "ds"), host_r
             st, hist = d.stats(), d.history()
             d.close()
             # the same steps again, event-timed, for the summed device time (first 1/8 time unit)
-            d = DeviceHermite(w.mass, w.pos, w.vel, w.eps2, order=order, precision=P[name])
+            d = DeviceHermite(w.mass, w.pos, w.vel, w.eps2, order=order, precision=P[name], averaged=order == 6)
             d.run_until(min(t_end, 0.125), time_device=True)
             sd = d.stats()
             d.close()
-            d = DeviceHermite(w.mass, w.pos, w.vel, w.eps2, order=order, precision=P[name])
+            d = DeviceHermite(w.mass, w.pos, w.vel, w.eps2, order=order, precision=P[name], averaged=order == 6)
             t0 = time.perf_counter()
             d.run_until(min(t_end, 0.125))
             wall8 = time.perf_counter() - t0
             d.close()
-            row = {"integrator": "device (s2_bts)", "order": order, "precision": name, "block_steps": st["block_steps"],
+            row = {"integrator": "device (s2_bts)", "order": order, "criterion": "Aarseth" if order == 4 else "mean of Aarseth(eta4) and generalised(eta6) (L156)", "precision": name, "block_steps": st["block_steps"],
                    "particle_steps": st["particle_steps"], "n_i_min": int(hist.min()), "n_i_median": float(np.median(hist)),
                    "n_i_mean": float(hist.mean()), "n_i_max": int(hist.max()), "wall_s": wall,
                    "wall_us_per_block_step": wall / st["block_steps"] * 1e6,
@@ -413,7 +441,7 @@ def run_blockstep(n, t_end=1.0, orders=(4, 6), precisions=("fp64", "ds"), host_r
             if order not in orders:
                 continue
             b = S2Backend(w.N, w.eps2, precision=s2.S2_FP64, order=order)
-            h = H(b, w.mass, w.pos, w.vel)
+            h = H(b, w.mass, w.pos, w.vel, **({'averaged': True} if order == 6 else {}))
             b.calls = b.pairs = 0
             t0 = time.perf_counter()
             h.run_until(min(t_end, 0.125))

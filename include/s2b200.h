@@ -126,6 +126,13 @@ int s2_commit_j_device(s2_ctx *ctx, int n, const int *d_address, const int *d_id
  * Subsequent s2_calc_* calls sum over exactly these nj particles.  ASYNC. */
 int s2_predict(s2_ctx *ctx, double t, int nj);
 
+/* Restricts the j-sum of subsequent s2_calc_* calls to the addresses first .. first+count-1 of the predicted store
+ * (count == 0: every predicted particle again, the default).  This is one device's share when the j-particles are
+ * distributed over several GPUs and the partial results added (sec 2.2.3, sec 3.6): each
+ * rank keeps the whole store -- 116 bytes per particle -- predicts all of it, and sums over its own block; nearest-
+ * neighbour and list addresses stay global.  The range must lie inside the predicted particles (else S2_ERANGE). */
+int s2_set_j_range(s2_ctx *ctx, int first, int count);
+
 /* --- a3-a8: forces on an i-list ---------------------------------- */
 
 /* i-particles given as addresses into the predicted j-store (their state is the device-
@@ -187,8 +194,13 @@ int s2_get_neighbours_csr_device(s2_ctx *ctx, int ni, const long long **d_offset
 typedef struct s2_bts s2_bts; /* opaque */
 
 /* ctx: an order-4 or order-6 context (any precision) with nj_capacity >= n.  dt_max, dt_min: powers of two <= 1.
- * eta: accuracy parameter of the step criterion; eta_start: that of the first step, dt = eta_start |a| / |jerk|. */
-int s2_bts_open(s2_bts **out, s2_ctx *ctx, int n, double eps2, double eta, double eta_start, double dt_max, double dt_min);
+ * eta: accuracy parameter of the step criterion (4th order: Aarseth; 6th order: its generalisation, ref [5]);
+ * eta_start: that of the first step, dt = eta_start |a| / |jerk|.
+ * averaged != 0 (order 6 only): the step is the mean of the generalised criterion and the 4th-order Aarseth step with
+ * accuracy parameter eta4 -- the choice of the paper's runs (L156), which keeps double-single forces from driving the
+ * step to zero. */
+int s2_bts_open(s2_bts **out, s2_ctx *ctx, int n, double eps2, double eta, double eta_start, double dt_max, double dt_min,
+                int averaged, double eta4);
 int s2_bts_close(s2_bts *b);
 /* Initial conditions at t = 0: host arrays mass (n), pos, vel (n,3).  Runs the start-up force evaluation (two passes
  * for order 6: the snap needs every particle's acceleration), sets the first steps and the first active list.  SYNC. */

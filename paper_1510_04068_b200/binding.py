@@ -70,6 +70,7 @@ def lib() -> C.CDLL:
         "s2_commit_j": (C.c_int, [vp]),
         "s2_commit_j_device": (C.c_int, [vp, C.c_int, ip, ip] + [dp] * 8),
         "s2_predict": (C.c_int, [vp, C.c_double, C.c_int]),
+        "s2_set_j_range": (C.c_int, [vp, C.c_int, C.c_int]),
         "s2_calc_ilist": (C.c_int, [vp, C.c_int, ip, dp, C.c_double, C.c_uint]),
         "s2_calc_ilist_device": (C.c_int, [vp, C.c_int, ip, dp, C.c_double, C.c_uint]),
         "s2_calc_explicit": (C.c_int, [vp, C.c_int, ip, dp, dp, dp, dp, C.c_double, C.c_uint]),
@@ -89,7 +90,7 @@ def lib() -> C.CDLL:
         "s2_get_timing": (C.c_int, [vp, C.POINTER(C.c_float), C.POINTER(C.c_float), C.POINTER(C.c_float)]),
         "s2_peak_fma": (C.c_int, [vp, C.c_int, C.c_int, C.POINTER(C.c_double)]),
         "s2_time_host_roundtrip": (C.c_int, [vp, C.c_int, C.POINTER(C.c_int), C.c_double, C.c_uint, C.c_int, C.POINTER(C.c_double)]),
-        "s2_bts_open": (C.c_int, [C.POINTER(vp), vp, C.c_int] + [C.c_double] * 5),
+        "s2_bts_open": (C.c_int, [C.POINTER(vp), vp, C.c_int] + [C.c_double] * 5 + [C.c_int, C.c_double]),
         "s2_bts_close": (C.c_int, [vp]),
         "s2_bts_init": (C.c_int, [vp, dp, dp, dp]),
         "s2_bts_run": (C.c_int, [vp, C.c_double, C.c_longlong, C.c_int, C.POINTER(C.c_longlong)]),
@@ -256,6 +257,10 @@ def s2_predict(ctx, t: float, nj: int):
     _check(lib().s2_predict(ctx.handle, float(t), int(nj)), "s2_predict", ctx.handle)
 
 
+def s2_set_j_range(ctx, first: int, count: int):
+    _check(lib().s2_set_j_range(ctx.handle, int(first), int(count)), "s2_set_j_range", ctx.handle)
+
+
 def s2_calc_ilist(ctx, i_address, h2=None, eps2: float = 0.0, flags: int = 0):
     ni = int(np.asarray(i_address).shape[0])
     pa, ka = _h(i_address, np.int32, (), ni, "i_address")
@@ -317,7 +322,7 @@ class _DeviceView:
     """Zero-copy view of library-owned device memory (valid until the next s2_calc_* / s2_close)."""
 
     def __init__(self, ptr: int, n: int, typestr: str):
-        self.__cuda_array_interface__ = {"shape": (n,), "typestr": typestr, "data": (ptr, True), "version": 2}
+        self.__cuda_array_interface__ = {"shape": (n,), "typestr": typestr, "data": (ptr, False), "version": 2}
 
 
 def s2_get_neighbours_csr_device(ctx, ni: int):
@@ -428,10 +433,11 @@ class s2_bts:
         self.handle, self.ctx, self.n = handle, ctx, n
 
 
-def s2_bts_open(ctx, n: int, eps2: float, eta: float, eta_start: float, dt_max: float = 2.0 ** -3, dt_min: float = 2.0 ** -40):
+def s2_bts_open(ctx, n: int, eps2: float, eta: float, eta_start: float, dt_max: float = 2.0 ** -3, dt_min: float = 2.0 ** -40,
+                averaged: bool = False, eta4: float = 0.01):
     h = C.c_void_p()
     _check(lib().s2_bts_open(C.byref(h), ctx.handle, int(n), float(eps2), float(eta), float(eta_start), float(dt_max),
-                             float(dt_min)), "s2_bts_open", ctx.handle)
+                             float(dt_min), int(averaged), float(eta4)), "s2_bts_open", ctx.handle)
     return s2_bts(h, ctx, int(n))
 
 

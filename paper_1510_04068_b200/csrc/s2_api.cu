@@ -425,6 +425,15 @@ extern "C" int s2_predict(s2_ctx *ctx, double t, int nj)
     return S2_OK;
 }
 
+extern "C" int s2_set_j_range(s2_ctx *ctx, int first, int count)
+{
+    if (!ctx || first < 0 || count < 0) return S2_EINVAL;
+    if ((long long)first + count > ctx->nj_cap) return S2_ERANGE;
+    ctx->j_first = count > 0 ? first : 0;
+    ctx->j_count = count;
+    return S2_OK;
+}
+
 // ---- launch balancer ----------------------------------------------------------------------
 
 static cudaError_t dispatch(int precision, int order, unsigned flags, int L, dim3 grid, size_t smem,
@@ -699,10 +708,10 @@ static int run_force_bank(s2_ctx *ctx, ForceArgs &a, int ni, unsigned flags, int
     auto copy_chunk = [&](int c) -> cudaError_t {   // chunk c of every plane -> bank c & 1, in stream order
         const int cnt = std::min(chunk, nj - c * chunk);
         if (equal_stride)   // one strided copy moves the chunk of every plane
-            return cudaMemcpy2DAsync(bank[c & 1], (size_t)chunk * sizeof(double2), (const double2 *)a.jp[0] + (size_t)c * chunk, pitch,
+            return cudaMemcpy2DAsync(bank[c & 1], (size_t)chunk * sizeof(double2), (const double2 *)a.jp[0] + a.j_first + (size_t)c * chunk, pitch,
                                      (size_t)cnt * sizeof(double2), npl, cudaMemcpyDeviceToDevice, ctx->stream);
         for (int p = 0; p < npl; ++p) {
-            cudaError_t e = cudaMemcpyAsync((double2 *)bank[c & 1] + (size_t)p * chunk, (const double2 *)a.jp[p] + (size_t)c * chunk,
+            cudaError_t e = cudaMemcpyAsync((double2 *)bank[c & 1] + (size_t)p * chunk, (const double2 *)a.jp[p] + a.j_first + (size_t)c * chunk,
                                             (size_t)cnt * sizeof(double2), cudaMemcpyDeviceToDevice, ctx->stream);
             if (e != cudaSuccess) return e;
         }
@@ -720,8 +729,8 @@ static int run_force_bank(s2_ctx *ctx, ForceArgs &a, int ni, unsigned flags, int
     const bool overlap = !capturing && ctx->tune[8] != 3;   // 3: forced, plain launches (A/B measurements)
     for (int c = 0; c < nchunks; ++c) {
         const int b = c & 1;
-        a.bank_j0 = c * chunk;
-        a.bank_cnt = std::min(chunk, nj - a.bank_j0);
+        a.bank_j0 = a.j_first + c * chunk;
+        a.bank_cnt = std::min(chunk, nj - c * chunk);
         a.bank_first = 0;
         a.bank_last = c == nchunks - 1;
         a.bank_id = b;
@@ -740,8 +749,8 @@ static int run_force_bank(s2_ctx *ctx, ForceArgs &a, int ni, unsigned flags, int
         a.bank_spin = c >= 2;
         a.bank_next_known = c == 0 || c == nchunks - 1;
         a.bank_self = (double2 *)bank[b];
-        a.bank_next_j0 = (c + 2) * chunk;
-        a.bank_next_cnt = c + 2 < nchunks ? std::min(chunk, nj - a.bank_next_j0) : 0;
+        a.bank_next_j0 = a.j_first + (c + 2) * chunk;
+        a.bank_next_cnt = c + 2 < nchunks ? std::min(chunk, nj - (c + 2) * chunk) : 0;
         a.bank_pdl = overlap && c > 0;
         a.bank_wait_early = c == 0 || flags != 0;   // decisions (thresholds) are carried from chunk to chunk
         CU(dispatch_bank(b, ctx->order, flags, a, ctx->stream, nullptr));
@@ -770,7 +779,8 @@ static int run_force_bank(s2_ctx *ctx, ForceArgs &a, int ni, unsigned flags, int
 // with stream-ordered copies between ordinary launches (documented semantics, measured ~4 % slower).
 static int bank_selftest(s2_ctx *ctx, int ni, const int *d_i_addr, bool explicit_i, double eps2, bool *ok)
 {
-    const int nj_save = ctx->nj_pred, t8 = ctx->tune[8];
+    const int nj_save = ctx->nj_pred, t8 = ctx->tune[8], jc_save = ctx->j_count;
+    ctx->j_count = 0;
     const int ni_t = std::min(ni, 65536);
     const int nj_t = std::min(nj_save, 8 * 1024);
     *ok = false;
@@ -797,6 +807,7 @@ static int bank_selftest(s2_ctx *ctx, int ni, const int *d_i_addr, bool explicit
     }
     ctx->tune[8] = t8;
     ctx->nj_pred = nj_save;
+    ctx->j_count = jc_save;
     ctx->in_selftest = false;
     ctx->calc_done = false;
     if (rc == S2_OK) {
@@ -824,7 +835,7 @@ static int bank_choose_mode(s2_ctx *ctx, int ni, const int *d_i_addr, bool expli
         int geom[3] = {0, 0, 0};
         ForceArgs dummy{};
         CU(dispatch_force_fp64_bank0(ctx->order, 0, dummy, ctx->stream, geom));
-        if (ctx->nj_pred <= 2 * geom[0]) { *mode = kBankSelfRefill; return S2_OK; }
+        if ((ctx->j_count > 0 ? ctx->j_count : ctx->nj_pred) <= 2 * geom[0]) { *mode = kBankSelfRefill; return S2_OK; }
         cudaStreamCaptureStatus cap = cudaStreamCaptureStatusNone;
         CU(cudaStreamIsCapturing(ctx->stream, &cap));
         if (cap != cudaStreamCaptureStatusNone) { *mode = kBankHostRefill; return S2_OK; }   // cannot test inside a capture
@@ -848,7 +859,11 @@ constexpr int kZeroCopyNi = 128;
 int run_force(s2_ctx *ctx, int ni, const int *d_i_addr, const double *d_h2, bool explicit_i, double eps2,
               unsigned flags, bool host_call)
 {
-    const bool bank = bank_applies(ctx, ni, ctx->nj_pred);
+    // the j-range summed over: all predicted particles, or one rank's share under j-sharding (s2_set_j_range)
+    const int j_first = ctx->j_count > 0 ? ctx->j_first : 0;
+    const int nj_eff = ctx->j_count > 0 ? ctx->j_count : ctx->nj_pred;
+    if ((long long)j_first + nj_eff > ctx->nj_pred) return S2_ERANGE;
+    const bool bank = bank_applies(ctx, ni, nj_eff);
     ForceShape sh{};
     int rc = S2_OK;
     ctx->csr_valid = false;
@@ -858,10 +873,10 @@ int run_force(s2_ctx *ctx, int ni, const int *d_i_addr, const double *d_h2, bool
         if (rc != S2_OK) return rc;
     }
     if (bank) {   // one lane per i, one "slice": the chunks of the constant bank are swept launch by launch
-        sh.L = 1; sh.Wj = 1; sh.S = 1; sh.slice_len = ctx->nj_pred; sh.tile = 256; sh.stages = 2; sh.cluster = 1;
+        sh.L = 1; sh.Wj = 1; sh.S = 1; sh.slice_len = nj_eff; sh.tile = 256; sh.stages = 2; sh.cluster = 1;
         rc = dev_reserve(ctx, ctx->part, (size_t)ni * (REC + 10) * sizeof(double));   // running sums + parked i-state
     } else {
-        rc = choose_shape(ctx, ni, ctx->nj_pred, flags, &sh);
+        rc = choose_shape(ctx, ni, nj_eff, flags, &sh);
     }
     if (rc != S2_OK) return rc;
     const int nst = sh.S * sh.Wj;
@@ -941,7 +956,8 @@ int run_force(s2_ctx *ctx, int ni, const int *d_i_addr, const double *d_h2, bool
     }
     a.jid_plane = plane(ctx, 3);
     a.ni = ni;
-    a.nj = ctx->nj_pred;
+    a.nj = nj_eff;
+    a.j_first = j_first;
     a.eps2 = eps2;
     a.S = sh.S;
     a.slice_len = sh.slice_len;

@@ -56,6 +56,8 @@ struct BtsArgs {
     BtsCtl *h_ctl;                   // the same, in pinned host memory
     int n, n_act, order;
     double eta, eta_start, dt_max, dt_min;
+    double eta4;                     // 6th order, averaged criterion: eta of the 4th-order Aarseth step it is averaged with
+    int averaged;
 };
 
 __device__ __forceinline__ double pow2_floor(double x)   // largest power of two <= x, x > 0 finite
@@ -163,6 +165,13 @@ __global__ void __launch_bounds__(128) bts_correct_kernel(BtsArgs a)
         const double A1 = sqrt(norm3(a1) * norm3(s1) + norm3(j1) * norm3(j1));
         const double A4 = sqrt(norm3(c1) * norm3(q1) + norm3(p1) * norm3(p1));
         raw = a.eta * cbrt(A1 / fmax(A4, 1e-300));
+        if (a.averaged) {
+            // the generalised criterion "is unstable when the force computation is not accurate enough",
+            // so the paper's runs take "the average of the Aarseth fourth order method and the sixth order extension"
+            const double jn = norm3(j1), sn = norm3(s1), cn = norm3(c1);
+            const double raw4 = sqrt(a.eta4 * (norm3(a1) * sn + jn * jn) / fmax(jn * cn + sn * sn, 1e-300));
+            raw = 0.5 * (raw + raw4);
+        }
     }
     const double nw = next_step(raw, dt, t_new, a.dt_min, a.dt_max);
 #pragma unroll
@@ -296,7 +305,8 @@ static cudaError_t launch_pdl(K kern, dim3 grid, dim3 block, cudaStream_t st, co
 struct s2_bts {
     s2_ctx *ctx = nullptr;
     int n = 0;
-    double eps2 = 0, eta = 0, eta_start = 0, dt_max = 0, dt_min = 0;
+    double eps2 = 0, eta = 0, eta_start = 0, dt_max = 0, dt_min = 0, eta4 = 0;
+    int averaged = 0;
     Buf dt, pot, ilist, stage, bcnt, misc;    // misc: {BtsCtl ctl; unsigned arrive; int hist[64]}
     BtsCtl *h_ctl = nullptr;                  // pinned
     bool ready = false;
@@ -326,6 +336,7 @@ static BtsArgs bts_args(s2_bts *b)
     a.n = b->n;
     a.order = ctx->order;
     a.eta = b->eta; a.eta_start = b->eta_start; a.dt_max = b->dt_max; a.dt_min = b->dt_min;
+    a.eta4 = b->eta4; a.averaged = b->averaged;
     return a;
 }
 
@@ -377,17 +388,19 @@ static int bts_select_predict(s2_bts *b, double t_now, bool host_time)
 // ---- the ABI (include/s2b200.h, "block-time-step integrator") ------------------------------------------------------
 
 extern "C" int s2_bts_open(s2_bts **out, s2_ctx *ctx, int n, double eps2, double eta, double eta_start, double dt_max,
-                           double dt_min)
+                           double dt_min, int averaged, double eta4)
 {
     if (!out) return S2_EINVAL;
     *out = nullptr;
     if (!ctx || n <= 0 || n > ctx->nj_cap || (ctx->order != 4 && ctx->order != 6)) return S2_EINVAL;
     int e1, e2;
     if (!(eta > 0) || !(eta_start > 0) || !(dt_min > 0) || !(dt_max >= dt_min) || dt_max > 1.0 || eps2 < 0) return S2_EINVAL;
+    if (averaged && (ctx->order != 6 || !(eta4 > 0))) return S2_EINVAL;
     if (frexp(dt_max, &e1) != 0.5 || frexp(dt_min, &e2) != 0.5 || e2 < -62) return S2_EINVAL;   // powers of two, level <= 63
     CU(cudaSetDevice(ctx->device));
     s2_bts *b = new s2_bts();
     b->ctx = ctx; b->n = n; b->eps2 = eps2; b->eta = eta; b->eta_start = eta_start; b->dt_max = dt_max; b->dt_min = dt_min;
+    b->averaged = averaged ? 1 : 0; b->eta4 = eta4;
     const int nb = (n + kSelPerBlock - 1) / kSelPerBlock;
     int rc = dev_reserve(ctx, b->dt, (size_t)n * sizeof(double));
     if (rc == S2_OK) rc = dev_reserve(ctx, b->pot, (size_t)n * sizeof(double));

@@ -62,6 +62,7 @@ struct s2_ctx {
     // state
     bool have_j = false, predicted = false, calc_done = false, results_fetched = false;
     int nj_pred = 0, ni_last = 0;
+    int j_first = 0, j_count = 0;     // j-range of the force sums (s2_set_j_range); count 0 = every predicted particle
     unsigned flags_last = 0;
     double t_pred = 0.0;
 

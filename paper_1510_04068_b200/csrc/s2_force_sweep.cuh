@@ -194,8 +194,8 @@ struct TilePipe {
         ST = args.stages;
         tile = args.tile;
         stage_bytes = (size_t)NPL * tile * 16;
-        j0 = blockIdx.y * args.slice_len;
-        j1 = min(args.nj, j0 + args.slice_len);
+        j0 = args.j_first + blockIdx.y * args.slice_len;
+        j1 = min(args.j_first + args.nj, j0 + args.slice_len);
         ntiles = j1 > j0 ? (j1 - j0 + tile - 1) / tile : 0;
         if (threadIdx.x == 0) {
             for (int s = 0; s < ST; ++s) mbar_init(&full[s], 1);

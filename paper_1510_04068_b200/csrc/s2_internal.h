@@ -82,7 +82,8 @@ struct ForceArgs {
     const double *h2;              // per i, or nullptr
     const double2 *jid_plane;      // fp64 plane P3 of j (id lookup for final nn)
     int ni;
-    int nj;
+    int nj;                        // number of j-particles summed over ...
+    int j_first;                   // ... starting at this address of the predicted store
     double eps2;
     int S;                         // CTA slices over j
     int slice_len;                 // j per CTA slice

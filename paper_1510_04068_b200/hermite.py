@@ -153,7 +153,9 @@ class Hermite6(Hermite4):
     The library's 6th-order predictor uses the stored snap and the interpolated crackle a^(3)."""
 
     def __init__(self, backend, mass, pos, vel, eta: float = 0.1, eta_start: float = 0.01,
-                 dt_max: float = 2.0 ** -3, dt_min: float = 2.0 ** -40):
+                 dt_max: float = 2.0 ** -3, dt_min: float = 2.0 ** -40, averaged: bool = False, eta4: float = 0.01):
+        # averaged: the paper's runs (L156) take the mean of this generalised step and the 4th-order Aarseth step
+        self.averaged, self.eta4 = averaged, eta4
         self.b = backend
         self.n = mass.shape[0]
         self.m = np.ascontiguousarray(mass, dtype=np.float64)
@@ -201,6 +203,10 @@ class Hermite6(Hermite4):
         A1 = np.sqrt(nrm(a1) * nrm(s1) + nrm(j1) ** 2)
         A4 = np.sqrt(nrm(c1) * nrm(q1) + nrm(p1) ** 2)
         raw = self.eta * np.cbrt(A1 / np.maximum(A4, 1e-300))
+        if self.averaged:
+            jn, sn, cn = nrm(j1), nrm(s1), nrm(c1)
+            raw4 = np.sqrt(self.eta4 * (nrm(a1) * sn + jn * jn) / np.maximum(jn * cn + sn * sn, 1e-300))
+            raw = 0.5 * (raw + raw4)
         old = self.dt[act]
         new = np.minimum(_pow2_floor(np.maximum(raw, self.dt_min)), 2.0 * old)
         blocked = (new > old) & (np.fmod(t_new, 2.0 * old) != 0.0)
@@ -224,7 +230,8 @@ class DeviceHermite:
     12-byte read.  Hermite4 / Hermite6 above are its host reference (the tests run both in lock-step)."""
 
     def __init__(self, mass, pos, vel, eps2: float, order: int = 4, precision: int = 0, eta: float | None = None,
-                 eta_start: float | None = None, dt_max: float = 2.0 ** -3, dt_min: float = 2.0 ** -40, device: int = 0):
+                 eta_start: float | None = None, dt_max: float = 2.0 ** -3, dt_min: float = 2.0 ** -40, device: int = 0,
+                 averaged: bool = False, eta4: float = 0.01):
         from . import binding as s2
         self.s2, self.order, self.eps2 = s2, order, float(eps2)
         self.n = int(np.asarray(mass).shape[0])
@@ -232,7 +239,7 @@ class DeviceHermite:
         eta = (0.01 if order == 4 else 0.1) if eta is None else eta
         eta_start = (0.0025 if order == 4 else 0.01) if eta_start is None else eta_start
         self.ctx = s2.s2_open(device, order, precision, nj_capacity=self.n, ngb_cap=0)
-        self.bts = s2.s2_bts_open(self.ctx, self.n, eps2, eta, eta_start, dt_max, dt_min)
+        self.bts = s2.s2_bts_open(self.ctx, self.n, eps2, eta, eta_start, dt_max, dt_min, averaged, eta4)
         s2.s2_bts_init(self.bts, self.m, pos, vel)
 
     def step(self) -> int:

@@ -152,7 +152,7 @@ def check_forces(res, ref, precision, order, flags, what=""):
                 pot=rel_err(res["pot"], ref.pot).max())
     if order == 6:
         errs["snap"] = rel_err(res["snap"], ref.snap).max()
-    for k, v in errs.items():
+    for k, v in list(errs.items()):
         if v > tol[k] and precision == s2.S2_FP32 and k in ("acc", "jerk", "snap"):
             errs[k + "_by_rms_bound"] = check_fp32_rms_bound(k, res[k], getattr(ref, k), ref, tol[k], what)
             continue

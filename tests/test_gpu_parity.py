@@ -389,18 +389,98 @@ def test_cfg4_sixth_order_ni1024():
     s2.s2_close(ctx)
 
 
-def test_sharded_forces_single_rank():
-    """The j-sharding wrapper with a world of one rank: explicit sinks against the local
-    shard, identity combine.  The two-rank combine itself is covered on CPU (tests/test_multirank_cpu.py)."""
+@pytest.mark.parametrize("kind", ["plummer", "lattice"])
+def test_j_sharded_partials_combine_to_the_unsharded_result(kind):
+    """j-sharding: three "ranks" run one after the other on this GPU, each a context that
+    holds the whole store and sums over its own address block (s2_set_j_range).  Their partial results, combined the
+    way sharding.combine_partials / combine_neighbour_lists do across ranks (sum; nn by smallest r2, ties to the lower
+    rank; lists concatenated in rank order, truncated to the cap), must equal the oracle over all j: sums within
+    tolerance, nearest neighbours, counts and lists exactly -- exact ties on the lattice included."""
+    import torch
+    from paper_1510_04068_b200.sharding import ShardedForces, merge_rank_lists
+    w = make_config(5, N=5000) if kind == "plummer" else lattice_workload(12, 0.25)
+    cap = 16
+    world = 3
+    ni = 700
+    il = w.ilist(ni)
+    h2 = w.h2[il] * (2.0 if kind == "plummer" else 1.0)
+    d_il, d_h2 = torch.from_numpy(il).cuda(), torch.from_numpy(np.ascontiguousarray(h2)).cuda()
+    parts = []
+    for r in range(world):
+        sf = ShardedForces(w.N, order=4, ngb_cap=cap, rank=r, world=world)
+        sf.set_all_j(w.ident, w.t_j, w.mass, w.pos, w.vel, w.acc, w.jerk)
+        p = sf.partial(w.t_pred, d_il, d_h2, w.eps2, NN | NGB)
+        parts.append({k: (v.clone() if v is not None else None) for k, v in p.items()})
+        if r == 0:
+            xp, vp, _ = s2.s2_get_predicted_j(sf.ctx, 0, w.N)
+        sf.close()
+    acc = sum(p["acc"] for p in parts).view(-1, 3).cpu().numpy()
+    jerk = sum(p["jerk"] for p in parts).view(-1, 3).cpu().numpy()
+    pot = sum(p["pot"] for p in parts).cpu().numpy()
+    cnt = sum(p["ngb_count"] for p in parts).cpu().numpy()
+    best_r2, best_id = parts[0]["nn_r2"].clone(), parts[0]["nn_id"].clone()
+    for p in parts[1:]:
+        better = p["nn_r2"] < best_r2
+        best_r2, best_id = torch.where(better, p["nn_r2"], best_r2), torch.where(better, p["nn_id"], best_id)
+    off, lst = merge_rank_lists([(p["offsets"][1:] - p["offsets"][:-1]) for p in parts], [p["list"] for p in parts], cap)
+    off, lst = off.cpu().numpy(), lst.cpu().numpy()
+    ref = oracle.forces_ilist(4, w.mass, w.ident, xp, vp, None, il, w.eps2, h2, cap)
+    res = dict(acc=acc, jerk=jerk, pot=pot, nn_id=best_id.cpu().numpy(), nn_r2=best_r2.cpu().numpy(), ngb_count=cnt)
+    check_forces(res, ref, s2.S2_FP64, 4, NN | NGB, f"j-sharded {kind}")
+    assert (ref.ngb_count > cap).any() or kind == "lattice"
+    for i in range(ni):
+        want = ref.ngb_list[i][ref.ngb_list[i] >= 0]
+        assert np.array_equal(lst[off[i]:off[i + 1]], want), (kind, i)
+
+
+def _nccl_jshard_worker(rank, world, port, q):
+    import os
+    import torch
+    import torch.distributed as dist
     from paper_1510_04068_b200.sharding import ShardedForces
-    w = make_config(1, N=500)
-    sf = ShardedForces(w.N, order=4)
-    assert sf.world == 1 and np.array_equal(sf.mine, np.arange(w.N))
+    os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port), RANK=str(rank), WORLD_SIZE=str(world))
+    torch.cuda.set_device(rank)
+    dist.init_process_group("nccl", rank=rank, world_size=world, device_id=torch.device("cuda", rank))
+    w = make_config(5, N=5000)
+    il = w.ilist(700)
+    sf = ShardedForces(w.N, order=4, device=rank, ngb_cap=16)
     sf.set_all_j(w.ident, w.t_j, w.mass, w.pos, w.vel, w.acc, w.jerk)
-    oxp, ovp, _ = oracle.predict(4, w.t_pred, w.t_j, w.pos, w.vel, w.acc, w.jerk)
-    il = w.ilist(60)
-    res = sf.forces(w.t_pred, w.ident[il], oxp[il], ovp[il], None, w.eps2)
-    ref = oracle.forces_ilist(4, w.mass, w.ident, oxp, ovp, None, il, w.eps2)
-    assert rel_err(res["acc"], ref.acc).max() < 1e-13 and rel_err(res["jerk"], ref.jerk).max() < 1e-12
-    assert np.array_equal(res["nn_id"], ref.nn_id)
+    dev = torch.device("cuda", rank)
+    out = sf.forces(w.t_pred, torch.from_numpy(il).to(dev), torch.from_numpy(np.ascontiguousarray(w.h2[il] * 2.0)).to(dev),
+                    w.eps2, NN | NGB)
+    if rank == 0:
+        xp, vp, _ = s2.s2_get_predicted_j(sf.ctx, 0, w.N)
+        q.put(({k: (v.cpu().numpy() if v is not None else None) for k, v in out.items()}, xp, vp))
+    dist.barrier()
     sf.close()
+    dist.destroy_process_group()
+
+
+def test_j_sharded_forces_two_ranks_nccl():
+    """The same combine through NCCL with one process per GPU; needs two devices (skips on the one-GPU test box)."""
+    import socket
+    import torch
+    import torch.multiprocessing as mp
+    if torch.cuda.device_count() < 2:
+        pytest.skip("needs two GPUs")
+    with socket.socket() as sk:
+        sk.bind(("127.0.0.1", 0))
+        port = sk.getsockname()[1]
+    ctx = mp.get_context("spawn")
+    q = ctx.Queue()
+    procs = [ctx.Process(target=_nccl_jshard_worker, args=(r, 2, port, q)) for r in range(2)]
+    for p in procs:
+        p.start()
+    got, xp, vp = q.get(timeout=300)
+    for p in procs:
+        p.join(timeout=120)
+        assert p.exitcode == 0
+    w = make_config(5, N=5000)
+    il = w.ilist(700)
+    ref = oracle.forces_ilist(4, w.mass, w.ident, xp, vp, None, il, w.eps2, w.h2[il] * 2.0, 16)
+    res = dict(acc=got["acc"].reshape(-1, 3), jerk=got["jerk"].reshape(-1, 3), pot=got["pot"], nn_id=got["nn_id"],
+               nn_r2=got["nn_r2"], ngb_count=got["ngb_count"])
+    check_forces(res, ref, s2.S2_FP64, 4, NN | NGB, "j-sharded, 2 ranks over NCCL")
+    for i in range(il.size):
+        want = ref.ngb_list[i][ref.ngb_list[i] >= 0]
+        assert np.array_equal(got["list"][got["offsets"][i]:got["offsets"][i + 1]], want), i

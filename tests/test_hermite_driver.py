@@ -94,8 +94,10 @@ def test_sixth_order_driver_gpu_follows_oracle_run():
 
 
 @pytest.mark.gpu
-@pytest.mark.parametrize("order,precision,steps,tol", [(4, "fp64", 300, 1e-9), (4, "ds", 150, 1e-7), (6, "fp64", 150, 1e-9)])
-def test_device_integrator_follows_host_reference_in_lockstep(order, precision, steps, tol):
+@pytest.mark.parametrize("order,precision,steps,tol,averaged", [(4, "fp64", 300, 1e-9, False), (4, "ds", 150, 1e-7, False),
+                                                                (6, "fp64", 150, 1e-9, False), (6, "fp64", 150, 1e-9, True),
+                                                                (6, "ds", 100, 1e-7, True)])
+def test_device_integrator_follows_host_reference_in_lockstep(order, precision, steps, tol, averaged):
     """The device-resident integrator (s2_bts_*: corrector, time-step rule and active-set selection in kernels, the
     j-store as particle state) against hermite.py driven by the ORACLE, block step by block step: same active counts and
     block times at every step, identical t and dt arrays, positions and velocities within tol."""
@@ -103,9 +105,9 @@ def test_device_integrator_follows_host_reference_in_lockstep(order, precision, 
     from paper_1510_04068_b200.hermite import DeviceHermite
     w = _plummer(256)
     P = {"fp64": s2.S2_FP64, "ds": s2.S2_DS}[precision]
-    d = DeviceHermite(w.mass, w.pos, w.vel, w.eps2, order=order, precision=P)
-    H = Hermite4 if order == 4 else Hermite6
-    o = H(OracleBackend(w.N, w.eps2, order=order), w.mass, w.pos, w.vel)
+    d = DeviceHermite(w.mass, w.pos, w.vel, w.eps2, order=order, precision=P, averaged=averaged)
+    o = (Hermite4(OracleBackend(w.N, w.eps2), w.mass, w.pos, w.vel) if order == 4 else
+         Hermite6(OracleBackend(w.N, w.eps2, order=6), w.mass, w.pos, w.vel, averaged=averaged))
     st = d.state()
     assert np.array_equal(st["dt"], o.dt) and np.allclose(st["acc"], o.a, rtol=1e-9, atol=0)
     for k in range(steps):
