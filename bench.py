@@ -479,7 +479,7 @@ def ni_sweep(s2, torch, dev, order):
     """Ginteractions/s versus n_i (4th order): config 3 (N = 65536) in fp64, double-single and fp32, the
     headline N = 2^18 in fp64, and config 2 (N = 64) latencies.  Device time of one s2_calc_ilist_device call
     (force sweep + combine), as in the paper's Fig. 2 protocol (kernel time only).  Calls with
-    fewer than 2e8 pairs are timed by CUDA-graph replay of 20 calls, larger ones by CUDA events per call."""
+    fewer than 1e9 pairs are timed by CUDA-graph replay of 20 (4 above 2e8 pairs) calls, larger ones by CUDA events per call."""
     from workloads import make_config
     out = []
     pow2 = tuple(1 << k for k in range(17))    # fp64 at config 3's N: every power of two from 1 to N (Fig. 2's axis)
@@ -499,7 +499,7 @@ def ni_sweep(s2, torch, dev, order):
         rows = []
         for ni in nis[::-1]:
             il = torch.from_numpy(w.ilist(ni)).to(dev)
-            if ni * w.N >= 2e8:
+            if ni * w.N >= 1e9:
                 s2.s2_enable_timing(ctx, True)
                 reps = 3 if ni * w.N > 1e9 else 10
                 ts = []
@@ -511,7 +511,8 @@ def ni_sweep(s2, torch, dev, order):
                 s2.s2_enable_timing(ctx, False)
                 us, how = statistics.median(ts) * 1e3, "events"
             else:
-                us, how = graph_time_us(s2, torch, ctx, lambda: s2.s2_calc_ilist_device(ctx, il, None, w.eps2, 0)), "graph"
+                us, how = graph_time_us(s2, torch, ctx, lambda: s2.s2_calc_ilist_device(ctx, il, None, w.eps2, 0),
+                                        calls=20 if ni * w.N < 2e8 else 4), "graph"
             g = ni * w.N / (us * 1e-6) / 1e9
             full = full or g
             info = s2.s2_last_launch_info(ctx)
@@ -536,6 +537,15 @@ def ni_sweep(s2, torch, dev, order):
                 rows[-1]["host_roundtrip_us"] = round(host_us, 1)          # through the Python binding (ctypes)
                 rows[-1]["host_roundtrip_c_us"] = round(host_c_us, 1)      # the same two calls timed inside the library
                 rows[-1]["host_roundtrip_c_reps"] = 100000
+                # k such calls in one launch sequence and one synchronisation (s2_calc_ilist_batch): host us per i-list
+                for kb in (8, 64):
+                    lists = [il_h] * kb
+                    for _ in range(20):
+                        s2.s2_calc_ilist_batch(ctx, lists, None, w.eps2, 0); s2.s2_get_results(ctx, ni * kb)
+                    t0 = time.perf_counter()
+                    for _ in range(200):
+                        s2.s2_calc_ilist_batch(ctx, lists, None, w.eps2, 0); s2.s2_get_results(ctx, ni * kb)
+                    rows[-1][f"host_us_per_list_batch{kb}"] = round((time.perf_counter() - t0) / 200 / kb * 1e6, 2)
         out.extend(rows[::-1])
         s2.s2_close(ctx)
     return out

@@ -140,6 +140,16 @@ int s2_set_j_range(s2_ctx *ctx, int first, int count);
  * host-pointer form: ASYNC after an internal pinned copy. */
 int s2_calc_ilist(s2_ctx *ctx, int ni, const int *i_address, const double *h2, double eps2,
                   unsigned flags);
+/* k i-lists against the same predicted j-store in ONE launch sequence (a small call is bound by
+ * launch, copy and synchronisation latency, not by arithmetic).  i_address holds the lists back to back (ni[0] + ... +
+ * ni[k-1] entries, h2 likewise); the results of list b are entries offset_b .. offset_b + ni[b] - 1 of the next
+ * s2_get_results / s2_get_neighbours* call over the concatenation, offset_b = ni[0] + ... + ni[b-1].  i-particles are
+ * independent of one another, so this is the force call on the concatenated list (the launch shape, hence the
+ * summation order and the last bits, are those of that list; decisions and lists are identical).  Host pointers.
+ * ASYNC.  (Device-resident callers reach the same effect by capturing s2_calc_ilist_device calls in a CUDA graph: the
+ * library enqueues nothing but kernels on that path.) */
+int s2_calc_ilist_batch(s2_ctx *ctx, int k, const int *ni, const int *i_address, const double *h2, double eps2,
+                        unsigned flags);
 /* device-pointer form of the same call (arrays must stay valid until the next SYNC). ASYNC. */
 int s2_calc_ilist_device(s2_ctx *ctx, int ni, const int *d_i_address, const double *d_h2,
                          double eps2, unsigned flags);

@@ -73,6 +73,7 @@ def lib() -> C.CDLL:
         "s2_set_j_range": (C.c_int, [vp, C.c_int, C.c_int]),
         "s2_calc_ilist": (C.c_int, [vp, C.c_int, ip, dp, C.c_double, C.c_uint]),
         "s2_calc_ilist_device": (C.c_int, [vp, C.c_int, ip, dp, C.c_double, C.c_uint]),
+        "s2_calc_ilist_batch": (C.c_int, [vp, C.c_int, ip, ip, dp, C.c_double, C.c_uint]),
         "s2_calc_explicit": (C.c_int, [vp, C.c_int, ip, dp, dp, dp, dp, C.c_double, C.c_uint]),
         "s2_get_results": (C.c_int, [vp, C.c_int, dp, dp, dp, dp, ip, dp, ip]),
         "s2_get_results_device": (C.c_int, [vp, C.c_int, dp, dp, dp, dp, ip, dp, ip]),
@@ -266,6 +267,17 @@ def s2_calc_ilist(ctx, i_address, h2=None, eps2: float = 0.0, flags: int = 0):
     pa, ka = _h(i_address, np.int32, (), ni, "i_address")
     ph, kh = _h(h2, np.float64, (), ni, "h2")
     _check(lib().s2_calc_ilist(ctx.handle, ni, pa, ph, float(eps2), int(flags)), "s2_calc_ilist", ctx.handle)
+
+
+def s2_calc_ilist_batch(ctx, lists, h2_lists=None, eps2: float = 0.0, flags: int = 0) -> np.ndarray:
+    """k i-lists in one launch sequence; returns the offsets (k + 1) of each list's results in the next s2_get_results."""
+    ni = np.array([len(x) for x in lists], dtype=np.int32)
+    cat = np.ascontiguousarray(np.concatenate([np.asarray(x, dtype=np.int32) for x in lists]))
+    h2 = None if h2_lists is None else np.ascontiguousarray(np.concatenate([np.asarray(x, dtype=np.float64) for x in h2_lists]))
+    _check(lib().s2_calc_ilist_batch(ctx.handle, len(lists), ni.ctypes.data_as(C.c_void_p), cat.ctypes.data_as(C.c_void_p),
+                                     None if h2 is None else h2.ctypes.data_as(C.c_void_p), float(eps2), int(flags)),
+           "s2_calc_ilist_batch", ctx.handle)
+    return np.concatenate([[0], np.cumsum(ni)])
 
 
 def s2_calc_ilist_device(ctx, d_i_address, d_h2=None, eps2: float = 0.0, flags: int = 0):

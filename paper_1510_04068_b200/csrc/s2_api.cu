@@ -579,8 +579,10 @@ static int choose_shape(s2_ctx *ctx, int ni, int nj, unsigned flags, ForceShape 
                     // ~2 us more than the same rounds in the separate launch, whose latency programmatic dependent
                     // launch hides (measured at N = 65536, same sweep shape: n_i = 8: 12.0 vs 9.9 us, n_i = 1: 8.9 vs 8.5)
                     const double fused_cost = (1.0 + rounds_f) * C_.c_row + (C > 1 ? C_.c_row : 0.0) + 4000.0;
+                    // the partial records are written by every CTA at the end of a one-wave sweep and read back by the
+                    // reduce: ~600 B per cycle for the round trip (measured: n_i = 512, 296 rows: 14.5 MB, +12 us)
                     const double sep_cost = C_.c_launch + std::ceil(nst / 32.0) * C_.c_row * 0.5 +
-                                            (double)ni * nst * (REC * 8.0) / 2000.0;
+                                            (double)ni * nst * (REC * 8.0) / 600.0;
                     fused = fusable && (fused_cost < sep_cost || ctx->tune[6] > 1 || ctx->tune[5] == 3);
                     if (!fused && C > 1) continue;              // a cluster shape only makes sense fused
                     // warp columns only pay when the CTA adds them up in shared memory (the fused path); unfused, every
@@ -1089,6 +1091,20 @@ extern "C" int s2_calc_ilist(s2_ctx *ctx, int ni, const int *i_address, const do
     CU(cudaEventRecord(ctx->ev_io, ctx->stream));
     return run_force(ctx, ni, (const int *)ctx->i_addr.p,
                      ngb ? (const double *)((char *)ctx->i_addr.p + b_addr) : nullptr, false, eps2, flags, true);
+}
+
+extern "C" int s2_calc_ilist_batch(s2_ctx *ctx, int k, const int *ni, const int *i_address, const double *h2, double eps2,
+                                   unsigned flags)
+{
+    if (!ctx || k <= 0 || !ni) return S2_EINVAL;
+    long long tot = 0;
+    for (int b = 0; b < k; ++b) {
+        if (ni[b] <= 0) return S2_EINVAL;
+        tot += ni[b];
+    }
+    if (tot > 0x7fffffffLL) return S2_ERANGE;
+    // i-particles are independent of one another: the concatenation is one i-list
+    return s2_calc_ilist(ctx, (int)tot, i_address, h2, eps2, flags);
 }
 
 static inline void split_ds_host(double x, float *hi, float *lo)

@@ -119,17 +119,35 @@ __global__ void __launch_bounds__(kCsrThreads) csr_offsets_kernel(const int *len
     if (blockIdx.x == gridDim.x - 1 && threadIdx.x == 0) offsets[ni] = *total;
 }
 
-// one warp per i: a segment of <= cap addresses, written where the scan says
+// one warp per kFillPerWarp consecutive i: each segment (<= cap addresses) is read with all its loads issued before the
+// stores of the group, so that a warp keeps several rows in flight (rows are a fixed stride apart: a row of ~32
+// members is four sectors of its own)
+constexpr int kFillPerWarp = 4;
 __global__ void __launch_bounds__(256) csr_fill_kernel(const int *list, const int *len, const long long *offsets, int ni, int cap,
                                                        int *out)
 {
-    const int i = (blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+    const int w = (blockIdx.x * blockDim.x + threadIdx.x) >> 5;
     const int lane = threadIdx.x & 31;
-    if (i >= ni) return;
-    const int n = len[i];
-    const int *src = list + (size_t)i * cap;
-    int *dst = out + offsets[i];
-    for (int k = lane; k < n; k += 32) dst[k] = src[k];
+    const int i0 = w * kFillPerWarp;
+    if (i0 >= ni) return;
+    int n[kFillPerWarp], v[kFillPerWarp];
+    long long off[kFillPerWarp];
+#pragma unroll
+    for (int u = 0; u < kFillPerWarp; ++u) {
+        const int i = i0 + u;
+        n[u] = i < ni ? len[i] : 0;
+        off[u] = i < ni ? offsets[i] : 0;
+    }
+#pragma unroll
+    for (int u = 0; u < kFillPerWarp; ++u)
+        v[u] = lane < n[u] ? list[(size_t)(i0 + u) * cap + lane] : 0;
+#pragma unroll
+    for (int u = 0; u < kFillPerWarp; ++u) {
+        int *dst = out + off[u];
+        if (lane < n[u]) dst[lane] = v[u];
+        const int *src = list + (size_t)(i0 + u) * cap;
+        for (int k = lane + 32; k < n[u]; k += 32) dst[k] = src[k];   // segments longer than a warp (rare)
+    }
 }
 
 cudaError_t launch_csr_scan(const double *rec, int ni, int cap, int *len, long long *block_sum, long long *total,
@@ -146,7 +164,7 @@ cudaError_t launch_csr_scan(const double *rec, int ni, int cap, int *len, long l
 cudaError_t launch_csr_fill(const int *list, const int *len, const long long *offsets, int ni, int cap, int *out, cudaStream_t st)
 {
     if (ni <= 0) return cudaSuccess;
-    const long long threads = (long long)ni * 32;
+    const long long threads = (long long)((ni + kFillPerWarp - 1) / kFillPerWarp) * 32;
     csr_fill_kernel<<<(unsigned)((threads + 255) / 256), 256, 0, st>>>(list, len, offsets, ni, cap, out);
     return cudaGetLastError();
 }

@@ -484,3 +484,33 @@ def test_j_sharded_forces_two_ranks_nccl():
     for i in range(il.size):
         want = ref.ngb_list[i][ref.ngb_list[i] >= 0]
         assert np.array_equal(got["list"][got["offsets"][i]:got["offsets"][i + 1]], want), i
+
+
+def test_batched_small_calls_match_single_calls():
+    """s2_calc_ilist_batch: k i-lists in one launch sequence and one synchronisation (config 2's regime: a small call is
+    latency-bound).  Each list's segment of the results equals the list's own call within rounding, decisions and
+    neighbour lists exactly, and the whole matches the oracle."""
+    w = make_config(2)
+    ctx = open_and_load(w, 4, ngb_cap=16)
+    s2.s2_predict(ctx, w.t_pred, w.N)
+    rng = np.random.default_rng(8)
+    lists = [rng.permutation(w.N)[:n].astype(np.int32) for n in (1, 7, 64, 3, 32, 1, 20)]
+    h2s = [w.h2[l] * 3.0 for l in lists]
+    off = s2.s2_calc_ilist_batch(ctx, lists, h2s, w.eps2, NN | NGB)
+    tot = int(off[-1])
+    res = s2.s2_get_results(ctx, tot)
+    coff, clst = s2.s2_get_neighbours_csr(ctx, tot)
+    cat, h2 = np.concatenate(lists), np.concatenate(h2s)
+    ref, _ = oracle_on_gpu_prediction(ctx, w, 4, cat, w.eps2, h2, ngb_cap=16)
+    check_forces(res, ref, s2.S2_FP64, 4, NN | NGB, "batch")
+    check_neighbour_lists(ctx, ref, tot, 16, "batch", counts=res["ngb_count"])
+    for b, (l, hh) in enumerate(zip(lists, h2s)):
+        s2.s2_calc_ilist(ctx, l, hh, w.eps2, NN | NGB)
+        one = s2.s2_get_results(ctx, l.size)
+        o1, l1 = s2.s2_get_neighbours_csr(ctx, l.size)
+        seg = slice(off[b], off[b + 1])
+        assert rel_err(res["acc"][seg], one["acc"]).max() < 1e-13 and rel_err(res["jerk"][seg], one["jerk"]).max() < 1e-12
+        for k in ("nn_id", "nn_r2", "ngb_count"):
+            assert np.array_equal(res[k][seg], one[k]), (b, k)
+        assert np.array_equal(clst[coff[off[b]]:coff[off[b + 1]]], l1)
+    s2.s2_close(ctx)
