@@ -57,8 +57,9 @@ def parse_args():
     ap.add_argument("--N", type=int, default=0, help="override N (reduced sizes are for debugging only)")
     ap.add_argument("--precision", default="fp64", choices=["fp64", "ds", "fp32"],
                     help="pair-arithmetic precision of the timed step (the default bench line is fp64)")
-    ap.add_argument("--section", default="all", choices=["all", "hbm"],
-                    help="hbm: only the streaming-kernel (predictor / scatter) measurement, for ncu captures")
+    ap.add_argument("--section", default="all", choices=["all", "hbm", "shapes"],
+                    help="hbm: only the streaming-kernel (predictor / scatter) measurement, for ncu captures; shapes: the "
+                         "launch-shape space around n_i = 32 and the atomics-versus-reduce A/B (profiles/r02_small_ni.md)")
     ap.add_argument("--shard", default="i", choices=["i", "j"],
                     help="multi-GPU decomposition: i = every rank its own i-list against the whole store (independent units, "
                          "weak scaling, the default line); j = the paper's scheme (L84): every rank sums ALL i over its own block "
@@ -180,6 +181,12 @@ def main():
         if rank == 0:
             run_blockstep(args.blockstep, args.bs_tend, tuple(int(x) for x in args.bs_orders.split(",")),
                           tuple(args.bs_precisions.split(",")))
+        return
+    if args.section == "shapes":
+        if rank == 0:
+            import torch
+            import paper_1510_04068_b200 as s2
+            print(json.dumps(shape_space(s2, torch, torch.device("cuda", local))), flush=True)
         return
     if args.section == "hbm":
         if rank == 0:
@@ -475,6 +482,43 @@ def graph_time_us(s2, torch, ctx, fn, calls=20, reps=7):
     return statistics.median(ts[1:])
 
 
+def shape_space(s2, torch, dev):
+    """Evidence behind the launch balancer and the choice of the deterministic combine, config 3
+    (N = 65536, fp64, 4th order), graph-timed device time per s2_calc_ilist_device call:
+      (a) n_i = 32: the automatic shape against forced neighbours in (lanes per i, warp columns, j-slices);
+      (b) combine by reduce kernel / fused / fp64 atomics (s2_set_tuning key 5) at n_i = 32 ... 16384."""
+    from workloads import make_config
+    w = make_config(3)
+    ctx = s2.s2_open(dev.index, 4, s2.S2_FP64, nj_capacity=w.N, ngb_cap=0)
+    a = np.arange(w.N, dtype=np.int32)
+    s2.s2_set_j(ctx, a, w.ident, w.t_j, w.mass, w.pos, w.vel, w.acc, w.jerk)
+    s2.s2_commit_j(ctx)
+    s2.s2_predict(ctx, w.t_pred, w.N)
+
+    def timed(ni, tune):
+        for k in range(9):
+            s2.s2_set_tuning(ctx, k, tune.get(k, 0))
+        il = torch.from_numpy(w.ilist(ni)).to(dev)
+        us = graph_time_us(s2, torch, ctx, lambda: s2.s2_calc_ilist_device(ctx, il, None, w.eps2, 0),
+                           calls=20 if ni * w.N < 2e8 else 4, reps=9)
+        info = s2.s2_last_launch_info(ctx)
+        return {"n_i": ni, "forced": {str(k): v for k, v in tune.items()}, "us": round(us, 2),
+                "ginteractions_per_s": round(ni * w.N / us / 1e3, 1), "S": info["S"], "lanes_per_i": info["lanes_per_i"],
+                "warp_columns": info["warp_columns"], "grid": info["grid"], "i_per_thread": info["i_per_thread"],
+                "combine": ("none", "reduce kernel", "fused", "chunk launches", "atomics", "chunk launches")[info["reduced"]]}
+
+    out = {"workload": "config 3: N = 65536, fp64, 4th order; graph-timed (20 calls per graph, median of 9 replays)",
+           "ni32_shapes": [timed(32, {})], "combine_ab": []}
+    for L, Wj, S in ((16, 1, 148), (16, 1, 111), (16, 1, 92), (32, 1, 37), (32, 1, 74), (32, 1, 55), (32, 1, 148), (8, 1, 148),
+                     (8, 1, 296), (16, 2, 74), (32, 2, 37)):
+        out["ni32_shapes"].append(timed(32, {0: S, 1: L, 2: Wj}))
+    for ni in (32, 256, 2048, 16384):
+        for key5 in (0, 1, 2):
+            out["combine_ab"].append(timed(ni, {5: key5} if key5 else {}))
+    s2.s2_close(ctx)
+    return out
+
+
 def ni_sweep(s2, torch, dev, order):
     """Ginteractions/s versus n_i (4th order): config 3 (N = 65536) in fp64, double-single and fp32, the
     headline N = 2^18 in fp64, and config 2 (N = 64) latencies.  Device time of one s2_calc_ilist_device call
@@ -576,6 +620,8 @@ def neighbour_path(s2, torch, dev, hbm_gbs):
             t = s2.s2_get_timing(ctx)
             if r:
                 ts.append(t["force_ms"] + t["reduce_ms"])
+            if flags and r == 2:
+                s2.s2_get_neighbours_csr_device(ctx, w.N)     # warm-up of the compaction kernels (first launch, allocations)
         ms = statistics.median(ts)
         info = s2.s2_last_launch_info(ctx)
         row = {"cfg": str(key), "order": order, "precision": pname, "N": w.N, "n_i": w.N,

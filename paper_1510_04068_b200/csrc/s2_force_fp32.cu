@@ -71,14 +71,8 @@ struct PolicyF32 {
     static constexpr int kMinBlocks = 2;
     static constexpr int kUnroll = 4;
     static constexpr int kIPT = kIptF32;          // i-particles per thread in the register-tiled sweep
-#ifndef S2_F32_UNROLL_TILED
-#define S2_F32_UNROLL_TILED 4
-#endif
-#ifndef S2_F32_MINBLOCKS_TILED
-#define S2_F32_MINBLOCKS_TILED 2
-#endif
-    static constexpr int kUnrollTiled = S2_F32_UNROLL_TILED;
-    static constexpr int kMinBlocksTiled = S2_F32_MINBLOCKS_TILED;
+    static constexpr int kUnrollTiled = 4;
+    static constexpr int kMinBlocksTiled = 2;
 
     struct IState {
         float xh, yh, zh, xl, yl, zl, vx, vy, vz, ax, ay, az, eps2;

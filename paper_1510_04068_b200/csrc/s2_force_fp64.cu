@@ -41,51 +41,18 @@ struct PolicyF64 {
     static constexpr int kIdPlane = ORDER == 2 ? 2 : 3;
     // j-particles per chunk of the constant bank (1024 / 680 / 1360 for 4th / 6th / 2nd order)
     static constexpr int kChunk = kBankBytes / (NPL * 16) / 8 * 8;
-#ifndef S2_F64_UNROLL_BANK
-#define S2_F64_UNROLL_BANK 8
-#endif
-#ifndef S2_F64_UNROLL_BANK6
-#define S2_F64_UNROLL_BANK6 4
-#endif
-#ifndef S2_F64_MINBLOCKS_BANK6
-#define S2_F64_MINBLOCKS_BANK6 1
-#endif
-    static constexpr int kUnrollBank = ORDER == 6 ? S2_F64_UNROLL_BANK6 : S2_F64_UNROLL_BANK;   // pairs in flight there
-#ifndef S2_F64_MINBLOCKS_BANK
-#define S2_F64_MINBLOCKS_BANK 2
-#endif
-#ifndef S2_BANK_THREADS
-#define S2_BANK_THREADS 256
-#endif
-    static constexpr int kMinBlocksBank = ORDER == 6 ? S2_F64_MINBLOCKS_BANK6 : S2_F64_MINBLOCKS_BANK;
-    static constexpr int kBankThreads = S2_BANK_THREADS;   // threads per CTA of the uniform-operand sweep
-#ifndef S2_F64_MINBLOCKS
-#define S2_F64_MINBLOCKS 2
-#endif
-#ifndef S2_F64_UNROLL
-#define S2_F64_UNROLL 4
-#endif
-    static constexpr int kMinBlocks = S2_F64_MINBLOCKS;
-    static constexpr int kUnroll = S2_F64_UNROLL;   // pairs in flight per thread in the one-lane-per-i loop
-#ifndef S2_F64_UNROLL_TILED
-#define S2_F64_UNROLL_TILED 4
-#endif
-#ifndef S2_F64_MINBLOCKS_TILED
-#define S2_F64_MINBLOCKS_TILED 2
-#endif
-#ifndef S2_F64_MINBLOCKS_TILED6
-#define S2_F64_MINBLOCKS_TILED6 1
-#endif
-#ifndef S2_F64_UNROLL_TILED6
-#define S2_F64_UNROLL_TILED6 4
-#endif
-    static constexpr int kMinBlocksTiled = ORDER == 6 ? S2_F64_MINBLOCKS_TILED6 : S2_F64_MINBLOCKS_TILED;
+    static constexpr int kUnrollBank = ORDER == 6 ? 4 : 8;   // pairs in flight there
+    static constexpr int kMinBlocksBank = ORDER == 6 ? 1 : 2;
+    static constexpr int kBankThreads = 256;   // threads per CTA of the uniform-operand sweep
+    static constexpr int kMinBlocks = 2;
+    static constexpr int kUnroll = 4;   // pairs in flight per thread in the one-lane-per-i loop
+    static constexpr int kMinBlocksTiled = ORDER == 6 ? 1 : 2;
     static constexpr int kIPT = kIptF64;                        // i-particles per thread in the register-tiled sweep
     static constexpr bool kPacked2 = false;
     // j per unrolled step there (x kIPT pairs in flight).  The 6th-order pair holds 18 more live doubles: with
     // 128 registers the totals spill inside the loop, so that variant runs one CTA per SM with 208 registers
     // (measured 290 vs 277 Gpairs/s)
-    static constexpr int kUnrollTiled = ORDER == 6 ? S2_F64_UNROLL_TILED6 : S2_F64_UNROLL_TILED;
+    static constexpr int kUnrollTiled = 4;
 
     struct IState {
         double x, y, z, vx, vy, vz, ax, ay, az, h2, eps2;
@@ -281,10 +248,7 @@ cudaError_t dispatch_force_fp64(int order, unsigned flags, int L, dim3 grid, siz
 // each and every barrier: warps are fully independent, one i-particle per lane, eight pairs in
 // flight per thread.  The price is one launch per chunk (1024 j at 4th order), with the running sums carried
 // through an SoA state buffer; sums are added in address order chunk by chunk, so results are bit-reproducible.
-#ifndef S2_BANK_LOOKS
-#define S2_BANK_LOOKS 15
-#endif
-constexpr int kBankLooks = S2_BANK_LOOKS;   // later looks at the next chunk's ticket inside a chunk (0: only at the start);
+constexpr int kBankLooks = 15;   // later looks at the next chunk's ticket inside a chunk (0: only at the start);
                                             // measured at n_i = 65536 / 81920 / 2^18: 0: 421 / 480 / 513, 3: 494 / - / 518, 7: 501 / 503 / 518,
                                             // 15: 506 / 510 / 518, 31: 507 / 511 / 518, 63: 501 / 504 / 512 Gpairs/s
 template <class P, int BANK, int THREADS>   // BANK only makes the kernels of the two translation units distinct symbols

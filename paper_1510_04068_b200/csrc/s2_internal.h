@@ -29,19 +29,10 @@ namespace s2 {
 constexpr int kMaxFields = 20;
 constexpr int kMaxPlanes = 8;      // up to 6 arithmetic planes + 2 fp64 position planes for decisions
 constexpr int REC = 12;            // doubles per result record (96 B = three 32-byte sectors)
-#ifndef S2_THREADS
-#define S2_THREADS 256
-#endif
-constexpr int kThreads = S2_THREADS;   // threads per force CTA
+constexpr int kThreads = 256;   // threads per force CTA
 constexpr int kWarps = kThreads / 32;
 // i-particles per thread of the register-tiled full-occupancy sweep (force_sweep_tiled_kernel); 1 = not built
-#ifndef S2_F64_IPT
-#define S2_F64_IPT 2
-#endif
-#ifndef S2_F32_IPT
-#define S2_F32_IPT 2
-#endif
-constexpr int kIptF64 = S2_F64_IPT, kIptF32 = S2_F32_IPT, kIptDS = 1;
+constexpr int kIptF64 = 2, kIptF32 = 2, kIptDS = 1;
 inline int force_ipt(int precision) { return precision == S2_FP64 ? kIptF64 : (precision == S2_FP32 ? kIptF32 : kIptDS); }
 
 // a 2nd-order context (acc + pot only) stores and predicts like a 4th-order one (missing derivatives are zero);

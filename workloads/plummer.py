@@ -20,7 +20,9 @@ Recipe (SURVEY.md §8(d) "Synthetic inputs", restated in DESIGN.md):
      t = 1 - 2^-13 (all dt exactly representable);
   9. id_j = address_j = j; active sets = prefixes of one seeded permutation.
 
-Nothing in this file evaluates a pairwise interaction or a Taylor predictor.
+No particle-particle interaction and no Taylor predictor is evaluated here.  Step 7 does write out the closed-form
+first and second time derivatives of ONE smooth field (a unit point mass with softening a_P at the origin) to give the
+stored derivatives plausible magnitudes: that is generator data, never an expected value.
 """
 from __future__ import annotations
 
