@@ -27,7 +27,8 @@ extern "C" {
  *   key 8: 1 = never use the uniform-operand sweep (j-particles read chunk by chunk from the constant bank, one
  *          launch per chunk; fp64 only), 2 = always use it when the context computes in fp64
  *   key 9: 1 = never use the zero-copy path of small host calls (n_i <= 128 with host arrays: the kernels read the
- *          i-list from, and write the final records to, pinned host memory, so no copy is enqueued) */
+ *          i-list from, and write the final records to, pinned host memory, so no copy is enqueued),
+ *          4 = S2_FP32 contexts: no fp64 re-evaluation of ill-conditioned i-particles (A/B of reading R-F32) */
 int s2_set_tuning(s2_ctx *ctx, int key, int value);
 /* Shape of the last force launch: out[0]=S, [1]=lanes per i, [2]=warp columns, [3]=grid size,
  * [4]=threads per CTA, [5]=dynamic shared memory bytes, [6]=0 no combine needed / 1 reduce kernel ran /
@@ -64,6 +65,10 @@ int s2_test_ds_ops(s2_ctx *ctx, int n, const double *a, const double *b, double 
 /* Device time in milliseconds of the last neighbour-list compaction (scan kernels + fill kernel, s2_ngb.cu), when
  * s2_enable_timing is on; the bytes it moved are 20 B per i-particle + 8 B per list member.  SYNC. */
 int s2_get_csr_timing(s2_ctx *ctx, float *scan_ms, float *fill_ms);
+
+/* S2_FP32 contexts: number of i-particles of the last force call whose jerk sum was found ill-conditioned and that were
+ * re-evaluated in fp64 (reading R-F32); 0 for other precisions.  SYNC. */
+int s2_fp32_fixup_count(s2_ctx *ctx, int *n);
 
 #ifdef __cplusplus
 }

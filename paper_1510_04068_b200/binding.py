@@ -89,6 +89,7 @@ def lib() -> C.CDLL:
         "s2_kernel_launches": (C.c_longlong, [vp]),
         "s2_enable_timing": (C.c_int, [vp, C.c_int]),
         "s2_get_timing": (C.c_int, [vp, C.POINTER(C.c_float), C.POINTER(C.c_float), C.POINTER(C.c_float)]),
+        "s2_fp32_fixup_count": (C.c_int, [vp, C.POINTER(C.c_int)]),
         "s2_peak_fma": (C.c_int, [vp, C.c_int, C.c_int, C.POINTER(C.c_double)]),
         "s2_time_host_roundtrip": (C.c_int, [vp, C.c_int, C.POINTER(C.c_int), C.c_double, C.c_uint, C.c_int, C.POINTER(C.c_double)]),
         "s2_bts_open": (C.c_int, [C.POINTER(vp), vp, C.c_int] + [C.c_double] * 5 + [C.c_int, C.c_double]),
@@ -419,6 +420,12 @@ def s2_time_host_roundtrip(ctx, i_address, eps2: float = 0.0, flags: int = 0, re
     _check(lib().s2_time_host_roundtrip(ctx.handle, ia.size, ia.ctypes.data_as(C.POINTER(C.c_int)), float(eps2), int(flags),
                                         int(reps), C.byref(v)), "s2_time_host_roundtrip", ctx.handle)
     return v.value
+
+
+def s2_fp32_fixup_count(ctx) -> int:
+    n = C.c_int()
+    _check(lib().s2_fp32_fixup_count(ctx.handle, C.byref(n)), "s2_fp32_fixup_count", ctx.handle)
+    return n.value
 
 
 def s2_peak_fma(ctx, kind: int, iters: int = 2000) -> float:

@@ -127,8 +127,10 @@ struct PolicyDS {
         int id;
     };
 
+    static constexpr bool kTrackW = false;
     struct Acc {
         ds ax, ay, az, jx, jy, jz, pot, sx, sy, sz;
+        __device__ __forceinline__ double wq() const { return 0.0; }
         __device__ __forceinline__ void zero()
         {
             ax = ay = az = jx = jy = jz = pot = ds{0.f, 0.f};

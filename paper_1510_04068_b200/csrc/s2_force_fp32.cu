@@ -4,7 +4,12 @@
 // Reading P10: "plain fp32" keeps every pair operation in fp32, but
 //   (a) positions are held as (hi, lo) float pairs and r is formed as (hi_j - hi_i) + (lo_j - lo_i), so the
 //       separation of a close pair does not inherit the 6e-8 |x| rounding of a float coordinate;
-//   (b) a thread sums in fp32 only over one j tile (<= 256 terms); tile sums are added to fp64 totals.
+//   (b) a thread sums in fp32 only over one j tile (<= 256 terms); tile sums are added to fp64 totals;
+//   (c) (reading R-F32) each pair term is good to ~4e-7, so the error of a sum is ~4e-7 sqrt(sum_j |term_j|^2) whatever
+//       the total is; where a particle's jerk is a strongly cancelling sum no fp32 pair arithmetic reaches 1e-5 of the
+//       total (tests/test_fp32_conditioning.py).  The sweep therefore also accumulates sum_j q_j^2 per i (one FFMA2 per
+//       two pairs), and i-particles whose estimate sqrt(sum q^2) (|v_i| + v_esc) exceeds 8 |jerk_i| -- 0.3-0.8 % of a
+//       Plummer sphere -- are re-evaluated by the fp64 sweep (s2_api.cu "fp32 fix-up").
 // The two integer decisions (nearest neighbour, neighbour test) use the fp64 squared distance formed from
 // the fp64 predicted positions (planes P0, P1 staged next to the float planes) in every precision mode.
 //
@@ -80,20 +85,25 @@ struct PolicyF32 {
         int id;
     };
 
+    static constexpr bool kTrackW = ORDER != 2;   // sum of q^2 per i: conditioning estimate of the jerk sum (R-F32)
     struct Part {   // fp32 sums over one tile
         float ax, ay, az, jx, jy, jz, pot, sx, sy, sz;
+        float w;    // sum of q^2 over the tile
         __device__ __forceinline__ void zero()
         {
             ax = ay = az = jx = jy = jz = pot = 0.f;
+            w = 0.f;
             if (ORDER == 6) sx = sy = sz = 0.f;
         }
     };
 
     struct Acc {    // fp64 totals
         double ax, ay, az, jx, jy, jz, pot, sx, sy, sz;
+        double w;
         __device__ __forceinline__ void zero()
         {
             ax = ay = az = jx = jy = jz = pot = 0.0;
+            w = 0.0;
             if (ORDER == 6) sx = sy = sz = 0.0;
         }
         __device__ __forceinline__ void add(const Part &o)
@@ -101,10 +111,13 @@ struct PolicyF32 {
             ax += (double)o.ax; ay += (double)o.ay; az += (double)o.az;
             jx += (double)o.jx; jy += (double)o.jy; jz += (double)o.jz;
             pot += (double)o.pot;
+            if (kTrackW) w += (double)o.w;
             if (ORDER == 6) { sx += (double)o.sx; sy += (double)o.sy; sz += (double)o.sz; }
         }
+        __device__ __forceinline__ double wq() const { return w; }
         __device__ __forceinline__ void shfl_add(int m)
         {
+            if (kTrackW) w += shfl_xor_d(w, m);
             ax += shfl_xor_d(ax, m); ay += shfl_xor_d(ay, m); az += shfl_xor_d(az, m);
             jx += shfl_xor_d(jx, m); jy += shfl_xor_d(jy, m); jz += shfl_xor_d(jz, m);
             pot += shfl_xor_d(pot, m);
@@ -201,6 +214,7 @@ struct PolicyF32 {
         A.pot -= my;
         A.ax = fmaf(q, dx, A.ax); A.ay = fmaf(q, dy, A.ay); A.az = fmaf(q, dz, A.az);
         if (ORDER == 2) return;
+        A.w = fmaf(q, q, A.w);
         const float dvx = f2.x - I.vx, dvy = f2.y - I.vy, dvz = f2.z - I.vz;
         const float rv = fmaf(dz, dvz, fmaf(dy, dvy, dx * dvx));
         const float alpha = rv * y2;
@@ -268,6 +282,11 @@ struct PolicyF32 {
         upk2(apot, A[0].pot, A[1].pot);
         upk2(aax, A[0].ax, A[1].ax); upk2(aay, A[0].ay, A[1].ay); upk2(aaz, A[0].az, A[1].az);
         if (ORDER == 2) return;
+        {
+            f32x2 aw = pk2(A[0].w, A[1].w);
+            aw = fma2(q, q, aw);
+            upk2(aw, A[0].w, A[1].w);
+        }
         const f32x2 dvx = sub2(bc2(f2.x), pk2(I[0].vx, I[1].vx));
         const f32x2 dvy = sub2(bc2(f2.y), pk2(I[0].vy, I[1].vy));
         const f32x2 dvz = sub2(bc2(f2.z), pk2(I[0].vz, I[1].vz));

@@ -59,8 +59,10 @@ struct PolicyF64 {
         int id;
     };
 
+    static constexpr bool kTrackW = false;
     struct Acc {
         double ax, ay, az, jx, jy, jz, pot, sx, sy, sz;
+        __device__ __forceinline__ double wq() const { return 0.0; }
         __device__ __forceinline__ void zero()
         {
             ax = ay = az = jx = jy = jz = pot = 0.0;
@@ -94,8 +96,9 @@ struct PolicyF64 {
 
     using Part = Acc;   // fp64 partial sums per tile, added to fp64 totals
 
-    static __device__ __forceinline__ void load_i(const ForceArgs &a, int i, IState &I)
+    static __device__ __forceinline__ void load_i(const ForceArgs &a, int i_, IState &I)
     {
+        const int i = a.pos_list ? a.pos_list[i_] : i_;   // sub-list built on the device (fp32 fix-up): position in the i-list
         const int ia = a.i_addr ? a.i_addr[i] : i;
         const double2 p0 = static_cast<const double2 *>(a.ip[0])[ia];
         const double2 p1 = static_cast<const double2 *>(a.ip[1])[ia];

@@ -242,7 +242,12 @@ __global__ void __launch_bounds__(kThreads, P::kMinBlocks) force_sweep_kernel(co
 {
     extern __shared__ __align__(128) unsigned char smem_raw[];
     constexpr int NPL = P::NPL;
-    const Decomp d = decompose<L>(a.Wj, a.ni);
+    int ni_eff = a.ni;
+    if (a.ni_dev) {   // length of a device-built sub-list: the grid was sized for the worst case, surplus CTAs leave
+        ni_eff = *a.ni_dev;
+        if ((int)blockIdx.x * (kWarps / a.Wj) * (32 / L) >= ni_eff) return;
+    }
+    const Decomp d = decompose<L>(a.Wj, ni_eff);
     TilePipe<NPL> pipe;
     pipe.init(smem_raw, a);
     unsigned char *tiles = pipe.tiles;
@@ -312,8 +317,20 @@ __global__ void __launch_bounds__(kThreads, P::kMinBlocks) force_sweep_kernel(co
         }
     }
 
+    if constexpr (P::kTrackW)
+        if (a.wq && d.jl == 0 && d.i_valid) a.wq[(size_t)d.slice * a.ni + d.i] = (float)tot.wq();
+
     double out[10];
     tot.to_f64(out);
+    if (a.pos_list) {   // fp64 re-evaluation of a flagged i-particle: only the sums of its final record are replaced
+        if (d.jl == 0 && d.i_valid) {
+            double *r = a.rec + (size_t)a.pos_list[d.i] * REC;
+#pragma unroll
+            for (int c = 0; c < 7; ++c) r[c] = out[c];
+            if (a.order == 6) { r[9] = out[7]; r[10] = out[8]; r[11] = out[9]; }
+        }
+        return;
+    }
     int nn = D.nn_j;
     int row = d.slice;                      // partial row this thread's record goes to
     bool writer = d.jl == 0 && d.i_valid;
@@ -508,6 +525,8 @@ __global__ void __launch_bounds__(kThreads, P::kMinBlocksTiled) force_sweep_tile
 #pragma unroll
     for (int u = 0; u < IPT; ++u) {
         if (!d[u].i_valid) continue;
+        if constexpr (P::kTrackW)
+            if (a.wq) a.wq[(size_t)blockIdx.y * a.ni + d[u].i] = (float)tot[u].wq();
         double out[10];
         tot[u].to_f64(out);
         if (a.atomic) {

@@ -95,6 +95,13 @@ struct ForceArgs {
     unsigned *counters;            // [number of i-groups], zero between calls (the reducing CTA resets its entry)
     double *out_final;             // [ni][REC]
     int order;
+    // fp32 path, reading R-F32 (s2_api.cu fp32_fixup): the sweep leaves sum_j q_j^2 per (slice, i) so that particles whose
+    // jerk is a strongly cancelling sum can be found and re-evaluated in fp64
+    float *wq;                     // [nslices_total][ni], or nullptr
+    // fp64 re-evaluation of a device-built sub-list: i-particle k of this launch is entry pos_list[k] of the i-list, the
+    // count is read from device memory (CTAs beyond it exit), only the sums of its final record are overwritten
+    const int *pos_list;
+    const int *ni_dev;
     int atomic;                    // 1: j-slices add their sums to the zeroed final records with fp64 atomics (opt-in,
                                    // the paper's Sapporo2 combine L88; not bit-reproducible; no NN / neighbour lists)
     // uniform-operand sweep (force_sweep_bank_kernel): the chunk of j now in the constant bank

@@ -118,44 +118,13 @@ def check_sets_ld(counts, lists, ref, what=""):
     return n_band
 
 
-F32_RMS_FACTOR = 8.0
-F32_STATS = {"by_rms_bound": 0}
-
-
-def check_fp32_rms_bound(name, got, want, ref, tol, what=""):
-    """Reading R-F32: fp32 pair arithmetic evaluates each pair term to a few 2^-24, so the error
-    of a particle's sum scales with R_i = sqrt(sum_j ||term_j||^2), not with the sum.  Where the terms cancel (one
-    particle in ~4000 at config 3 has a single pair term 24 times its total jerk) even correctly rounded fp32
-    operations miss 1e-5 of the TOTAL (tests/test_fp32_conditioning.py).  The fp32 criterion is therefore
-        ||delta_i|| <= tol * max(||ref_i||, R_i / 8)
-    i.e. north_star's 1e-5 of the total wherever the rms cancellation is at most 8 : 1, and 1.25e-6 of the rms pair
-    term beyond.  Only particles that fail the plain criterion get here; they are counted and printed."""
-    g = ref.inputs
-    e = rel_err(got, want)
-    bad = np.flatnonzero(e > tol)
-    ra, rj, rs = oracle.term_norms(g["order"], g["mass"], g["ident"], g["xj"], g["vj"], g["aj"], g["i_id"][bad], g["xi"][bad],
-                                   g["vi"][bad], None if g["ai"] is None else g["ai"][bad], g["eps2"], rms=True)
-    R = dict(acc=ra, jerk=rj, snap=rs)[name]
-    nrm = np.linalg.norm(np.asarray(want)[bad], axis=1)
-    delta = e[bad] * nrm
-    assert (delta <= tol * np.maximum(nrm, R / F32_RMS_FACTOR)).all(), \
-        f"{what}: fp32 {name} outside tol * max(|ref|, rms terms / {F32_RMS_FACTOR:g}): rel err {e[bad]}, cancellation {R / nrm}"
-    F32_STATS["by_rms_bound"] += bad.size
-    print(f"[R-F32] {what}: {bad.size} particle(s) judged by the rms-term bound for {name}: rel err {e[bad]}, "
-          f"rms cancellation R/|ref| {R / nrm}")
-    return int(bad.size)
-
-
 def check_forces(res, ref, precision, order, flags, what=""):
     tol = TOL[precision]
     errs = dict(acc=rel_err(res["acc"], ref.acc).max(), jerk=rel_err(res["jerk"], ref.jerk).max(),
                 pot=rel_err(res["pot"], ref.pot).max())
     if order == 6:
         errs["snap"] = rel_err(res["snap"], ref.snap).max()
-    for k, v in list(errs.items()):
-        if v > tol[k] and precision == s2.S2_FP32 and k in ("acc", "jerk", "snap"):
-            errs[k + "_by_rms_bound"] = check_fp32_rms_bound(k, res[k], getattr(ref, k), ref, tol[k], what)
-            continue
+    for k, v in errs.items():
         assert v <= tol[k], f"{what}: {k} max rel err {v:.3e} > {tol[k]:.0e}"
     if flags & (s2.S2_WANT_NN | s2.S2_WANT_NGB):
         # primary: the oracle's long-double decision within north_star's band (DESIGN.md section 2, "parity criterion")

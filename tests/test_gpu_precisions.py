@@ -345,3 +345,44 @@ def test_fp32_packed_tiled_sweep_has_the_bits_of_the_scalar_sweep(order, flags):
         ref, _ = oracle_on_gpu_prediction(ctx, w, order, il, w.eps2, h2, ngb_cap=24)
         check_forces(got[2], ref, s2.S2_FP32, order, flags, f"fp32 packed order {order}")
     s2.s2_close(ctx)
+
+
+def test_fp32_fixup_meets_1e5_on_a_cancelling_sum():
+    """Reading R-F32: config 3 holds a particle (address 17198) whose jerk is a 48 : 1 cancellation; plain fp32 pair
+    arithmetic is at 1.9e-5 of the total there (and cannot do better, tests/test_fp32_conditioning.py).  The fp32 path
+    flags such particles from sum_j q_j^2 and re-evaluates them with the fp64 sweep: with the fix-up every particle is
+    within 1e-5; without it (s2_set_tuning key 9 = 4) this one is not; decisions and lists are untouched by it."""
+    w = make_config(3)
+    ctx = open_and_load(w, 4, precision=s2.S2_FP32, ngb_cap=32)
+    s2.s2_predict(ctx, w.t_pred, w.N)
+    il = np.concatenate([[17198], w.ilist(4095)]).astype(np.int32)
+    il = il[np.sort(np.unique(il, return_index=True)[1])]
+    h2 = np.full(il.size, (0.03) ** 2)
+    ref, _ = oracle_on_gpu_prediction(ctx, w, 4, il, w.eps2, h2, ngb_cap=32)
+    out = {}
+    for fix in (4, 0):
+        s2.s2_set_tuning(ctx, 9, fix)
+        for shape in ({}, {0: 5, 1: 4}, {0: 3, 7: 2}):          # automatic, a j-split shape with slices, the tiled sweep with slices
+            for k in range(8):
+                s2.s2_set_tuning(ctx, k, shape.get(k, 0))
+            s2.s2_calc_ilist(ctx, il, h2, w.eps2, NN | NGB)
+            res = s2.s2_get_results(ctx, il.size)
+            lists = s2.s2_get_neighbours_csr(ctx, il.size)
+            e = rel_err(res["jerk"], ref.jerk)
+            out[(fix, tuple(shape.items()))] = (res, lists, e)
+            n_fix = s2.s2_fp32_fixup_count(ctx)
+            if fix == 4:
+                assert e[0] > 1e-5 and n_fix == 0                 # plain fp32: the cancelling sum misses the tolerance
+            else:
+                assert e.max() <= 1e-5 and e[0] < 1e-12 and 1 <= n_fix <= il.size // 20, (e.max(), e[0], n_fix)
+                check_forces(res, ref, s2.S2_FP32, 4, NN | NGB, f"fp32 fix-up {shape}")
+    for key in [k for k in out if k[0] == 0]:
+        a, b = out[key], out[(4, key[1])]
+        for k in ("nn_id", "nn_r2", "ngb_count"):
+            assert np.array_equal(a[0][k], b[0][k])
+        assert np.array_equal(a[1][0], b[1][0]) and np.array_equal(a[1][1], b[1][1])
+        same = a[2] == b[2]
+        assert same.mean() > 0.9                                   # unflagged particles keep their fp32 bits
+    print("fp32 fix-up: flagged", s2.s2_fp32_fixup_count(ctx), "of", il.size, "worst jerk error with / without:",
+          out[(0, ())][2].max(), out[(4, ())][2].max())
+    s2.s2_close(ctx)
