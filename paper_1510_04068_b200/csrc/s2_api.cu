@@ -475,7 +475,7 @@ static int query_occ(s2_ctx *ctx, unsigned flags, int L, int npl, int *occ_out)
 {
     int occ = ctx->tune[3];
     if (occ <= 0) {
-        const long long key = ((long long)flags << 32) | L;
+        const long long key = ((long long)flags << 32) | (unsigned)(L & 0xffff);
         auto it = ctx->occ_cache.find(key);
         if (it == ctx->occ_cache.end()) {
             ForceArgs dummy{};
@@ -512,17 +512,23 @@ static int choose_shape(s2_ctx *ctx, int ni, int nj, unsigned flags, ForceShape 
     const int tile_max = std::min(2048, (int)((232448 - kSmemHeader) / (2 * npl * 16)) / 32 * 32);
 
     double best = 1e300;
-    int bL = 1, bWj = 1, bS = 1, bocc = 1, bfused = 0, bC = 1;
+    int bL = 1, bTL = 0, bWj = 1, bS = 1, bocc = 1, bfused = 0, bC = 1;
     const int ipt_max = force_ipt(ctx->precision);
-    for (int Lc = 0; Lc <= 6; ++Lc) {
-        // Lc = 0: register-tiled sweep (one lane per i, ipt_max i per thread); Lc = 1..6: L = 1, 2, 4, .., 32 lanes per i
-        const int L = Lc == 0 ? 0 : 1 << (Lc - 1);
+    for (int Lc = -5; Lc <= 6; ++Lc) {
+        // Lc <= 0: register-tiled sweep (ipt_max i per thread) with TL = 1, 2, .., 32 lanes per i-slot (TL > 1: plain sums
+        // only); Lc = 1..6: one i per thread, L = 1, 2, 4, .., 32 lanes per i
+        const int L = Lc <= 0 ? 0 : 1 << (Lc - 1);
+        const int TL = Lc <= 0 ? 1 << (-Lc) : 0;
         const int ipt = L == 0 ? ipt_max : 1;
-        if (L == 0 && (ipt_max < 2 || ctx->tune[7] == 1)) continue;
+        if (L == 0 && (ipt_max < 2 || ctx->tune[7] == 1 || (TL > 1 && flags != 0))) continue;
+        // lanes per i-slot pay in fp32, where the tiled sweep's packed FFMA2 pairs halve the issue slots (measured at
+        // N = 65536: n_i = 256: 32.1 -> 27.8 us, 1024: 101.9 -> 88.9 us); in fp64 they measure within 1 % of the one-i-per-
+        // thread shapes (the LDS.128 they save is a small part of an FP64-pipe-bound loop), so there only when forced
+        if (L == 0 && TL > 1 && ctx->precision != S2_FP32 && ctx->tune[7] < 2) continue;
         if (ctx->tune[7] >= 2 && L != 0) continue;
-        if (ctx->tune[1] > 0 && (L == 0 ? 1 : L) != ctx->tune[1]) continue;
+        if (ctx->tune[1] > 0 && (L == 0 ? TL : L) != ctx->tune[1]) continue;
         int occ;
-        int rc = query_occ(ctx, flags, L, npl, &occ);
+        int rc = query_occ(ctx, flags, L == 0 ? (TL > 1 ? -TL : 0) : L, npl, &occ);
         if (rc != S2_OK) return rc;
         for (int Wj = 1; Wj <= kWarps; Wj <<= 1) {
             // warp columns: warps of a CTA share i-particles and split every tile (the paper's 2D blocks, L104);
@@ -530,9 +536,9 @@ static int choose_shape(s2_ctx *ctx, int ni, int nj, unsigned flags, ForceShape 
             // i-groups re-stream the j range from L2 and lose, profiles/r01_small_ni.md)
             if (ctx->tune[2] > 0 ? Wj != ctx->tune[2] : (Wj > 1 && (L <= 1 || (long long)ni * L * Wj > kThreads))) continue;
             if (Wj > 1 && L <= 1) continue;
-            const int icta = L == 0 ? kThreads * ipt : (kWarps / Wj) * (32 / L);
+            const int icta = L == 0 ? kThreads * ipt / TL : (kWarps / Wj) * (32 / L);
             const int Gi = (ni + icta - 1) / icta;
-            const int lanes_j = std::max(1, L) * Wj;             // lanes (over all warp columns) sharing one i
+            const int lanes_j = (L == 0 ? TL : L) * Wj;          // lanes (over all warp columns) sharing one i
             const int min_slice = std::max(32, 2 * lanes_j);
             const int smax = std::min(65535, std::max(1, nj / min_slice));
             // candidate slice counts: 1, and those that make the grid k x SMs (k = 1..16)
@@ -569,7 +575,7 @@ static int choose_shape(s2_ctx *ctx, int ni, int nj, unsigned flags, ForceShape 
                 // read different j, and LDS.128 is conflict-free only up to 8 distinct addresses (4-way at L = 32)
                 double t_iter = C_.t_iter * (n_sm >= 2 ? 1.0 : 1.1) * (1.0 + 0.01 * L) * (L == 32 ? 1.3 : 1.0);
                 // register-tiled: ipt pairs per lane and j, fewer shared-memory reads each
-                if (L == 0) t_iter = C_.t_iter * ipt * C_.tiled_gain * (n_sm >= 2 ? 1.0 : 1.09);
+                if (L == 0) t_iter = C_.t_iter * ipt * C_.tiled_gain * (n_sm >= 2 ? 1.0 : 1.09) * (1.0 + 0.03 * (-Lc)) * (TL == 32 ? 1.3 : 1.0);
                 // every i-group streams the whole j range from L2 (~2500 B per SM-cycle over the chip)
                 const double stream = (double)Gi * nj * npl * 16.0 / 2500.0;
                 double cost = std::ceil(n_sm / occ) * C_.c_cta + std::max(n_sm * iters * t_iter, stream);
@@ -594,7 +600,7 @@ static int choose_shape(s2_ctx *ctx, int ni, int nj, unsigned flags, ForceShape 
                 }
                 if (cost < best * (1 - 1e-9)) {
                     best = cost;
-                    bL = L; bWj = Wj; bS = S; bocc = occ; bfused = fused; bC = fused ? C : 1;
+                    bL = L; bTL = TL; bWj = Wj; bS = S; bocc = occ; bfused = fused; bC = fused ? C : 1;
                 }
             }
         }
@@ -603,6 +609,7 @@ static int choose_shape(s2_ctx *ctx, int ni, int nj, unsigned flags, ForceShape 
 
     ForceShape sh{};
     sh.L = bL;
+    sh.TL = bTL;
     sh.Wj = bWj;
     sh.S = bS;
     sh.slice_len = (nj + bS - 1) / bS;
@@ -882,7 +889,7 @@ int run_force(s2_ctx *ctx, int ni, const int *d_i_addr, const double *d_h2, bool
         if (rc != S2_OK) return rc;
     }
     if (bank) {   // one lane per i, one "slice": the chunks of the constant bank are swept launch by launch
-        sh.L = 1; sh.Wj = 1; sh.S = 1; sh.slice_len = nj_eff; sh.tile = 256; sh.stages = 2; sh.cluster = 1;
+        sh.L = 1; sh.TL = 0; sh.Wj = 1; sh.S = 1; sh.slice_len = nj_eff; sh.tile = 256; sh.stages = 2; sh.cluster = 1;
         rc = dev_reserve(ctx, ctx->part, (size_t)ni * (REC + 10) * sizeof(double));   // running sums + parked i-state
     } else {
         rc = choose_shape(ctx, ni, nj_eff, flags, &sh);
@@ -892,7 +899,7 @@ int run_force(s2_ctx *ctx, int ni, const int *d_i_addr, const double *d_h2, bool
     const bool want_ngb = flags & S2_WANT_NGB;
     const bool final_direct = nst == 1;
     // without neighbour lists the combine is fused into the sweep launch (last CTA of an i-group reduces)
-    const int icta_ = sh.L == 0 ? kThreads * force_ipt(ctx->precision) : (kWarps / sh.Wj) * (32 / sh.L);
+    const int icta_ = sh.L == 0 ? kThreads * force_ipt(ctx->precision) / std::max(1, sh.TL) : (kWarps / sh.Wj) * (32 / sh.L);
     const int Gi_ = (ni + icta_ - 1) / icta_;
     const bool fused = sh.fused != 0;
     // opt-in (s2_set_tuning key 5 = 2): combine the j-slices with fp64 atomics instead of the reduce kernel
@@ -1015,7 +1022,7 @@ int run_force(s2_ctx *ctx, int ni, const int *d_i_addr, const double *d_h2, bool
     size_t smem = force_smem_bytes(force_nplanes(ctx->precision, ctx->order, flags), sh.tile, sh.stages);
     smem = std::max(smem, (size_t)kSmemHeader + (size_t)icta * sh.Wj * REC * sizeof(double));   // record block of the combines
     if (ctx->timing) CU(cudaEventRecord(ctx->ev_t[2], ctx->stream));
-    CU(dispatch(ctx->precision, ctx->order, flags, sh.L, grid, smem, a, ctx->stream, false, nullptr));
+    CU(dispatch(ctx->precision, ctx->order, flags, sh.L == 0 ? (sh.TL > 1 ? -sh.TL : 0) : sh.L, grid, smem, a, ctx->stream, false, nullptr));
     if (ctx->timing) CU(cudaEventRecord(ctx->ev_t[3], ctx->stream));
     ctx->launches++;
     ctx->ran_force = true;
@@ -1064,7 +1071,7 @@ int run_force(s2_ctx *ctx, int ni, const int *d_i_addr, const double *d_h2, bool
         ctx->fix_last = -1;
     }
     int *li = ctx->last_info;
-    li[0] = sh.S; li[1] = sh.L == 0 ? 1 : sh.L; li[2] = sh.Wj; li[3] = (int)(grid.x * grid.y); li[4] = kThreads;
+    li[0] = sh.S; li[1] = sh.L == 0 ? std::max(1, sh.TL) : sh.L; li[2] = sh.Wj; li[3] = (int)(grid.x * grid.y); li[4] = kThreads;
     li[5] = (int)smem; li[6] = final_direct ? 0 : (fused ? 2 : (atomic ? 4 : 1));
     li[8] = sh.L == 0 ? force_ipt(ctx->precision) : 1; li[9] = a.cluster;
     ctx->calc_done = true;

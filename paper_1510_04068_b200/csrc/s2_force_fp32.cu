@@ -237,12 +237,12 @@ struct PolicyF32 {
     // Two i-particles of one thread against the same j, every FP32 operation packed (see f32x2 above).  Same
     // operations in the same order as interact<1, false> for each half.
     static constexpr bool kPacked2 = true;
-    static __device__ __forceinline__ void interact2(const JData &J, int jaddr, const IState *I, Part *A, Dec *D,
+    static __device__ __forceinline__ void interact2(const JData &J, bool jvalid, int jaddr, const IState *I, Part *A, Dec *D,
                                                      const Decomp *d, int *const *seg, int segcap)
     {
         const float4 f0 = J.f0, f1 = J.f1, f2 = J.f2;
         const int jid = __float_as_int(f1.w);
-        const bool skip0 = jid == I[0].id, skip1 = jid == I[1].id;
+        const bool skip0 = jid == I[0].id || !jvalid, skip1 = jid == I[1].id || !jvalid;   // jvalid: false on a masked tail lane
 
         const f32x2 dx = add2(sub2(bc2(f0.x), pk2(I[0].xh, I[1].xh)), sub2(bc2(f1.x), pk2(I[0].xl, I[1].xl)));
         const f32x2 dy = add2(sub2(bc2(f0.y), pk2(I[0].yh, I[1].yh)), sub2(bc2(f1.y), pk2(I[0].yl, I[1].yl)));

@@ -467,9 +467,15 @@ __global__ void __launch_bounds__(kThreads, P::kMinBlocks) force_sweep_kernel(co
 // halving the loads per pair is worth more than the occupancy it costs.  i-index of slot u of a thread:
 // (blockIdx.x * IPT + u) * kThreads + threadIdx.x.  No warp columns, no cluster, no fused combine on this path:
 // the grid is large, slices are combined by reduce_kernel (or there is a single slice).
-template <class P, int IPT>
+// TL > 1 (plain sums only, no NN / neighbour lists): TL lanes share the IPT i-particles of a thread slot and take
+// interleaved j, combined by an xor-butterfly like the lanes of force_sweep_kernel -- the register-tiled pair arithmetic
+// (packed FFMA2 pairs in fp32, half the LDS.128 per pair in fp64) for i-lists too short to fill the chip with one lane per i.
+template <class P, int IPT, int TL>
 __global__ void __launch_bounds__(kThreads, P::kMinBlocksTiled) force_sweep_tiled_kernel(const ForceArgs a)
 {
+    static_assert(TL == 1 || (!P::NN && !P::NGB), "lanes per i-slot > 1: plain sums only");
+    constexpr int IPC = kThreads / TL;   // i-slots per CTA (each holds IPT i-particles)
+    const int jl = (threadIdx.x & 31) % TL;
     extern __shared__ __align__(128) unsigned char smem_raw[];
     constexpr int NPL = P::NPL;
     TilePipe<NPL> pipe;
@@ -485,8 +491,8 @@ __global__ void __launch_bounds__(kThreads, P::kMinBlocksTiled) force_sweep_tile
 #pragma unroll
     for (int u = 0; u < IPT; ++u) {
         d[u].lane = threadIdx.x & 31;
-        d[u].il = d[u].lane; d[u].jl = 0; d[u].wi = threadIdx.x >> 5; d[u].wj = 0;
-        d[u].i = (blockIdx.x * IPT + u) * kThreads + threadIdx.x;
+        d[u].il = d[u].lane / TL; d[u].jl = jl; d[u].wi = threadIdx.x >> 5; d[u].wj = 0;
+        d[u].i = (blockIdx.x * IPT + u) * IPC + threadIdx.x / TL;
         d[u].i_valid = d[u].i < a.ni;
         if (!d[u].i_valid) d[u].i = a.ni - 1;   // padding slots recompute the last i and never write
         d[u].slice = blockIdx.y;
@@ -502,18 +508,35 @@ __global__ void __launch_bounds__(kThreads, P::kMinBlocksTiled) force_sweep_tile
         const int cnt = min(tile, pipe.j1 - jt);
 #pragma unroll
         for (int u = 0; u < IPT; ++u) part[u].zero();
+        const int nfull = cnt / TL;
+        int k = jl;
 #pragma unroll P::kUnrollTiled
-        for (int k = 0; k < cnt; ++k) {
+        for (int it = 0; it < nfull; ++it, k += TL) {
             typename P::JData J;
             P::load_j(stage, tile, k, J);
             if constexpr (IPT % 2 == 0 && P::kPacked2) {   // i-particles two by two in packed instructions
 #pragma unroll
                 for (int u = 0; u < IPT; u += 2)
-                    P::interact2(J, jt + k, I + u, part + u, D + u, d + u, seg + u, a.segcap);
+                    P::interact2(J, true, jt + k, I + u, part + u, D + u, d + u, seg + u, a.segcap);
             } else {
 #pragma unroll
                 for (int u = 0; u < IPT; ++u)
                     P::template interact<1, false>(J, true, jt + k, I[u], part[u], D[u], d[u], seg[u], a.segcap);
+            }
+        }
+        if (TL > 1 && cnt - nfull * TL > 0) {   // ragged tail: lanes past the end re-read the last j, masked
+            const bool valid = k < cnt;
+            const int kk = valid ? k : cnt - 1;
+            typename P::JData J;
+            P::load_j(stage, tile, kk, J);
+            if constexpr (IPT % 2 == 0 && P::kPacked2) {
+#pragma unroll
+                for (int u = 0; u < IPT; u += 2)
+                    P::interact2(J, valid, jt + kk, I + u, part + u, D + u, d + u, seg + u, a.segcap);
+            } else {
+#pragma unroll
+                for (int u = 0; u < IPT; ++u)
+                    P::template interact<1, true>(J, valid, jt + kk, I[u], part[u], D[u], d[u], seg[u], a.segcap);
             }
         }
 #pragma unroll
@@ -522,9 +545,17 @@ __global__ void __launch_bounds__(kThreads, P::kMinBlocksTiled) force_sweep_tile
     }
     asm volatile("griddepcontrol.launch_dependents;" ::: "memory");   // see force_sweep_kernel
 
+    if (TL > 1) {   // combine the TL lanes of every i-slot in a fixed (butterfly) order
+#pragma unroll
+        for (int m = 1; m < TL; m <<= 1) {
+#pragma unroll
+            for (int u = 0; u < IPT; ++u) tot[u].shfl_add(m);
+        }
+    }
+
 #pragma unroll
     for (int u = 0; u < IPT; ++u) {
-        if (!d[u].i_valid) continue;
+        if (!d[u].i_valid || jl != 0) continue;
         if constexpr (P::kTrackW)
             if (a.wq) a.wq[(size_t)blockIdx.y * a.ni + d[u].i] = (float)tot[u].wq();
         double out[10];
@@ -594,14 +625,32 @@ cudaError_t launch_L(int L, dim3 grid, size_t smem, const ForceArgs &a, cudaStre
         kern<<<grid, kThreads, smem, st>>>(a);                                                               \
         return cudaGetLastError();                                                                           \
     }
-    if (L == 0) {   // register-tiled full-occupancy sweep, P::kIPT i-particles per thread
+    if (L <= 0) {   // register-tiled sweep, P::kIPT i-particles per thread, -L (or 1) lanes per i-slot
         if constexpr (P::kIPT >= 2) {
-            auto kern = force_sweep_tiled_kernel<P, P::kIPT>;
-            static std::atomic<int> s_opted[kMaxDevices];
-            if (cudaError_t e = opt_in_smem(kern, s_opted); e != cudaSuccess) return e;
-            if (query) return cudaOccupancyMaxActiveBlocksPerMultiprocessor(ctas_per_sm, kern, kThreads, smem);
-            kern<<<grid, kThreads, smem, st>>>(a);
-            return cudaGetLastError();
+#define S2_TCASE(TLL)                                                                                        \
+    case TLL: {                                                                                              \
+        auto kern = force_sweep_tiled_kernel<P, P::kIPT, TLL>;                                               \
+        static std::atomic<int> s_opted[kMaxDevices];                                                        \
+        if (cudaError_t e = opt_in_smem(kern, s_opted); e != cudaSuccess) return e;                          \
+        if (query) return cudaOccupancyMaxActiveBlocksPerMultiprocessor(ctas_per_sm, kern, kThreads, smem);  \
+        kern<<<grid, kThreads, smem, st>>>(a);                                                               \
+        return cudaGetLastError();                                                                           \
+    }
+            const int TL = L == 0 ? 1 : -L;
+            if constexpr (!P::NN && !P::NGB) {
+                switch (TL) {
+                    S2_TCASE(1)
+                    S2_TCASE(2)
+                    S2_TCASE(4)
+                    S2_TCASE(8)
+                    S2_TCASE(16)
+                    S2_TCASE(32)
+                }
+            } else {
+                switch (TL) { S2_TCASE(1) }
+            }
+#undef S2_TCASE
+            return cudaErrorInvalidValue;
         } else {
             return cudaErrorInvalidValue;
         }

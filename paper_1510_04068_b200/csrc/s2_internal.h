@@ -142,7 +142,8 @@ cudaError_t launch_predict(const PredictArgs &a, cudaStream_t st);
 cudaError_t launch_reduce(const ReduceArgs &a, cudaStream_t st);
 
 struct ForceShape {                // chosen by the balancer in s2_api.cu
-    int L;                         // lanes per i (1..32)
+    int L;                         // lanes per i (1..32); 0: register-tiled sweep (several i per thread)
+    int TL;                        // register-tiled sweep: lanes per i-slot (1..32)
     int Wj;                        // warp columns
     int S;
     int slice_len;

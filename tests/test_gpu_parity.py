@@ -103,7 +103,8 @@ def test_all_launch_shapes_ragged(order, flags):
         s2.s2_set_tuning(ctx, 1, L); s2.s2_set_tuning(ctx, 2, Wj); s2.s2_set_tuning(ctx, 0, S); s2.s2_set_tuning(ctx, 4, tile)
         # fused combine (auto / no / 2 / 8 CTA clusters), separate reduce kernel, and for one lane per i the
         # register-tiled sweep (several i per thread)
-        modes = [(0, 0, 1), (3, 0, 1), (0, 2, 1), (0, 8, 1), (1, 0, 1)] + ([(0, 0, 2)] if L == 1 else [])
+        # ... register-tiled sweep (several i per thread; with L > 1 lanes per i-slot for plain sums)
+        modes = [(0, 0, 1), (3, 0, 1), (0, 2, 1), (0, 8, 1), (1, 0, 1)] + ([(0, 0, 2)] if (L == 1 or flags == 0) and Wj == 1 else [])
         for unfused, cluster, tiled in modes:
             s2.s2_set_tuning(ctx, 5, unfused); s2.s2_set_tuning(ctx, 6, cluster); s2.s2_set_tuning(ctx, 7, tiled)
             s2.s2_calc_ilist(ctx, il, h2, w.eps2, flags)

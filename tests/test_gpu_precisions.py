@@ -38,6 +38,8 @@ def test_precision_paths_all_shapes_ragged(prec, order, flags):
     shapes = [s + (1,) for s in shapes]
     if P == s2.S2_FP32:                                   # register-tiled sweep (two i per thread) exists for fp32 and fp64
         shapes += [(1, 1, 1, 0, 2), (1, 1, 3, 64, 2), (1, 1, 13, 32, 2)]
+        if flags == 0:                                    # ... with several lanes per i-slot (plain sums)
+            shapes += [(L, 1, S, tile, 2) for L in (2, 8, 32) for S, tile in ((1, 0), (5, 64))]
     for L, Wj, S, tile, tiled in shapes:
         s2.s2_set_tuning(ctx, 1, L); s2.s2_set_tuning(ctx, 2, Wj); s2.s2_set_tuning(ctx, 0, S); s2.s2_set_tuning(ctx, 4, tile)
         s2.s2_set_tuning(ctx, 7, tiled)
@@ -331,14 +333,14 @@ def test_fp32_packed_tiled_sweep_has_the_bits_of_the_scalar_sweep(order, flags):
     h2 = w.h2[il] * 0.6 if flags & NGB else None
     keys = ("acc", "pot") + (("jerk",) if order >= 4 else ()) + (("snap",) if order == 6 else ())
     keys += ("nn_id", "nn_r2", "ngb_count") if flags else ()
-    for S, tile in ((1, 0), (3, 64), (7, 256)):
+    for S, tile, L in ((1, 0, 1), (3, 64, 1), (7, 256, 1)) + (((1, 0, 4), (5, 64, 16)) if flags == 0 else ()):
         got = {}
         for tiled in (1, 2):
-            s2.s2_set_tuning(ctx, 1, 1); s2.s2_set_tuning(ctx, 2, 1); s2.s2_set_tuning(ctx, 0, S)
+            s2.s2_set_tuning(ctx, 1, L); s2.s2_set_tuning(ctx, 2, 1); s2.s2_set_tuning(ctx, 0, S)
             s2.s2_set_tuning(ctx, 4, tile); s2.s2_set_tuning(ctx, 7, tiled)
             s2.s2_calc_ilist(ctx, il, h2, w.eps2, flags)
             got[tiled] = s2.s2_get_results(ctx, ni)
-            assert s2.s2_last_launch_info(ctx)["i_per_thread"] == tiled
+            assert s2.s2_last_launch_info(ctx)["i_per_thread"] == tiled and s2.s2_last_launch_info(ctx)["lanes_per_i"] == L
         for k in keys:
             assert np.array_equal(got[1][k], got[2][k]), (order, flags, S, tile, k)
     if order >= 4:
