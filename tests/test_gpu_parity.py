@@ -515,3 +515,31 @@ def test_batched_small_calls_match_single_calls():
             assert np.array_equal(res[k][seg], one[k]), (b, k)
         assert np.array_equal(clst[coff[off[b]]:coff[off[b + 1]]], l1)
     s2.s2_close(ctx)
+
+
+def test_contexts_on_two_devices_in_one_process():
+    """The > 48 KB shared-memory opt-in and the bank hand-over state are per device: contexts on two devices of one
+    process (the paper's multi-GPU mode is single-process, L80) must both run the large-tile sweeps and the
+    uniform-operand sweep.  Needs two GPUs (skips on the one-GPU test box)."""
+    import torch
+    if torch.cuda.device_count() < 2:
+        pytest.skip("needs two GPUs")
+    w = make_config(3, N=9000)
+    il = w.ilist(w.N)
+    out = []
+    for dev in (0, 1):
+        with torch.cuda.device(dev):
+            ctx = s2.s2_open(dev, 4, s2.S2_FP64, nj_capacity=w.N, ngb_cap=0)
+            a = np.arange(w.N, dtype=np.int32)
+            s2.s2_set_j(ctx, a, w.ident, w.t_j, w.mass, w.pos, w.vel, w.acc, w.jerk)
+            s2.s2_commit_j(ctx)
+            s2.s2_predict(ctx, w.t_pred, w.N)
+            res = {}
+            for key8 in (1, 2):
+                s2.s2_set_tuning(ctx, 8, key8)
+                s2.s2_calc_ilist(ctx, il, None, w.eps2, 0)
+                res[key8] = s2.s2_get_results(ctx, w.N)
+            out.append(res)
+            s2.s2_close(ctx)
+    for k in ("acc", "jerk", "pot"):
+        assert np.array_equal(out[0][1][k], out[1][1][k]) and np.array_equal(out[0][2][k], out[1][2][k])
