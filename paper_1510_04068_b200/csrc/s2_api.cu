@@ -651,7 +651,7 @@ static int choose_shape(s2_ctx *ctx, int ni, int nj, unsigned flags, ForceShape 
 // start and 15 more times on their way through the chunk), so unlike the shared-memory sweep it does not care whether
 // the grid is a whole number of residency rounds; below ~0.6 rounds (296 CTAs of 256 threads each) the per-launch
 // costs win (n_i = 40960: 452 / 488 with 128-thread CTAs, 49152: 502 / 488).
-// 4th order only: the 6th-order variant measures 282 against 290, the 2nd-order one -4 %.
+// The 2nd-order variant measures -4 % and stays on the shared-memory sweep.
 static bool bank_applies(const s2_ctx *ctx, int ni, int nj)
 {
     if (ctx->precision != S2_FP64 || ctx->tune[8] == 1) return false;
@@ -659,6 +659,9 @@ static bool bank_applies(const s2_ctx *ctx, int ni, int nj)
                                           // by stream-ordered copies (the documented-semantics fallback)
     for (int k = 0; k < 8; ++k)
         if (ctx->tune[k]) return false;   // an explicit launch shape was asked for
+    // 6th order (round 2: two 126-register CTAs per SM instead of one of 158): N = 2^18, bank / shared-memory Gpairs/s:
+    // n_i = 49152: 278 / 292, 65536: 294 / 293, 131072: 301 / 290, 262144: 302 / 290
+    if (ctx->order == 6) return nj >= 8192 && ni >= 100000;
     return ctx->order == 4 && nj >= 8192 && ni >= 48000;
 }
 

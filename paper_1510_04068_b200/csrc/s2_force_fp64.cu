@@ -42,7 +42,7 @@ struct PolicyF64 {
     // j-particles per chunk of the constant bank (1024 / 680 / 1360 for 4th / 6th / 2nd order)
     static constexpr int kChunk = kBankBytes / (NPL * 16) / 8 * 8;
     static constexpr int kUnrollBank = ORDER == 6 ? 4 : 8;   // pairs in flight there
-    static constexpr int kMinBlocksBank = ORDER == 6 ? 1 : 2;
+    static constexpr int kMinBlocksBank = 2;   // 6th order: 126 registers at 4 pairs in flight, no spills (1 CTA of 158 registers: 275 Gpairs/s; 2 CTAs: 302)
     static constexpr int kBankThreads = 256;   // threads per CTA of the uniform-operand sweep
     static constexpr int kMinBlocks = 2;
     static constexpr int kUnroll = 4;   // pairs in flight per thread in the one-lane-per-i loop
