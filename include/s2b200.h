@@ -189,6 +189,26 @@ int s2_get_neighbours_csr(s2_ctx *ctx, int ni, long long *offsets, int *list, lo
  * *total = offsets[ni].  SYNC (one 8-byte read). */
 int s2_get_neighbours_csr_device(s2_ctx *ctx, int ni, const long long **d_offsets, const int **d_list, long long *total);
 
+/* --- a5 + a6 without any allocation (PAPER.md L52-L54 j-split, L88 combine of the partial results) ------------ */
+
+/* For callers that cannot call cudaMalloc (code under CUDA-graph capture, tight serving loops, harnesses that forbid
+ * it): 4th-order fp64 acc, jerk and pot of ni i-particles from nj predicted j-particles, as a j-split sweep plus a
+ * fixed-order combine whose partial sums live in a STATIC device array of the library (4 MiB; every GPU that loads
+ * the library holds it until the process exits).  Needs no context.  It calls no cudaMalloc, cudaFree or allocating
+ * library routine: cudaSetDevice(device), once per device a symbol-address lookup, two kernel launches.
+ *   device pointers, caller-owned: d_pos, d_vel (nj,3) predicted state; d_mass, d_id (nj); d_i_address (ni) addresses
+ *   into those arrays (an address outside [0, nj) gives NaN results for that i, nothing faults);
+ *   outputs d_acc, d_jerk (ni,3), d_pot (ni).  Conventions as above (self skipped by id, pot negative, G = 1).
+ * Limit: ni <= 4096 (s2_noalloc_limits); larger i-lists return S2_ERANGE -- use the context calls for those.
+ * The scratch array is shared by all calls on a device and keeps the last call's contents; nothing in it needs
+ * clearing (every row read was written by the same call).  Calls that overlap on the GPU (two streams, two threads)
+ * RACE on it: the caller serialises them.  Results are bit-reproducible run to run.  ASYNC on cuda_stream. */
+int s2_forces_noalloc(int device, void *cuda_stream, int nj, const double *d_pos, const double *d_vel,
+                      const double *d_mass, const int *d_id, int ni, const int *d_i_address, double eps2,
+                      double *d_acc, double *d_jerk, double *d_pot);
+/* The fixed maxima of s2_forces_noalloc: largest ni, and the bytes of the static scratch array (either may be NULL). */
+int s2_noalloc_limits(int *max_ni, long long *scratch_bytes);
+
 /* --- block-time-step Hermite integrator on the device (sec 3.7) -------- */
 
 /* The second workload of the paper: a 4th- or 6th-order Hermite predictor-corrector with block (power-of-two,

@@ -100,6 +100,8 @@ def lib() -> C.CDLL:
         "s2_bts_stats": (C.c_int, [vp, C.POINTER(C.c_double), C.POINTER(C.c_double), C.POINTER(C.c_int), C.POINTER(C.c_longlong),
                                    C.POINTER(C.c_longlong), C.POINTER(C.c_double), C.POINTER(C.c_double), C.POINTER(C.c_longlong)]),
         "s2_bts_get_history": (C.c_int, [vp, C.c_longlong, C.c_int, ip]),
+        "s2_forces_noalloc": (C.c_int, [C.c_int, vp, C.c_int, dp, dp, dp, ip, C.c_int, ip, C.c_double, dp, dp, dp]),
+        "s2_noalloc_limits": (C.c_int, [C.POINTER(C.c_int), C.POINTER(C.c_longlong)]),
         "s2_strerror": (C.c_char_p, [C.c_int]),
         "s2_last_cuda_error": (C.c_char_p, [vp]),
         "s2_version": (C.c_char_p, []),
@@ -508,6 +510,30 @@ def s2_bts_get_history(b, first: int = 0, count: int | None = None) -> np.ndarra
     out = np.empty(max(count, 1), np.int32)
     _check(lib().s2_bts_get_history(b.handle, int(first), int(count), out.ctypes.data_as(C.c_void_p)), "s2_bts_get_history")
     return out[:count]
+
+
+# ---- allocation-free entry point (include/s2b200.h, s2_forces_noalloc) -----------------------------------
+
+def s2_noalloc_limits() -> dict:
+    n, b = C.c_int(), C.c_longlong()
+    _check(lib().s2_noalloc_limits(C.byref(n), C.byref(b)), "s2_noalloc_limits")
+    return dict(max_ni=n.value, scratch_bytes=b.value)
+
+
+def s2_forces_noalloc(d_pos, d_vel, d_mass, d_id, d_i_address, eps2, d_acc, d_jerk, d_pot, device: int = 0, stream=None):
+    """acc, jerk, pot (torch CUDA tensors the caller owns) of the listed i-particles; the library allocates nothing."""
+    nj, ni = d_mass.numel(), d_i_address.numel()
+    if stream is None:
+        import torch
+        stream = torch.cuda.current_stream(device).cuda_stream
+    rc = lib().s2_forces_noalloc(int(device), C.c_void_p(stream), nj, _d(d_pos, "float64", 3 * nj, "pos"),
+                                 _d(d_vel, "float64", 3 * nj, "vel"), _d(d_mass, "float64", nj, "mass"), _d(d_id, "int32", nj, "id"),
+                                 ni, _d(d_i_address, "int32", ni, "i_address"), float(eps2), _d(d_acc, "float64", 3 * ni, "acc"),
+                                 _d(d_jerk, "float64", 3 * ni, "jerk"), _d(d_pot, "float64", ni, "pot"))
+    if rc == S2_ERANGE:
+        raise S2Error(rc, "s2_forces_noalloc", f"n_i = {ni} exceeds the fixed maximum of {s2_noalloc_limits()['max_ni']} "
+                                               f"(static scratch); use s2_calc_ilist for larger i-lists")
+    _check(rc, "s2_forces_noalloc")
 
 
 def s2_last_cuda_error(ctx) -> str:
