@@ -28,7 +28,8 @@ extern "C" {
  *          launch per chunk; fp64 only), 2 = always use it when the context computes in fp64
  *   key 9: 1 = never use the zero-copy path of small host calls (n_i <= 128 with host arrays: the kernels read the
  *          i-list from, and write the final records to, pinned host memory, so no copy is enqueued),
- *          4 = S2_FP32 contexts: no fp64 re-evaluation of ill-conditioned i-particles (A/B of reading R-F32) */
+ *          4 = S2_FP32 contexts: no fp64 re-evaluation of ill-conditioned i-particles (A/B of reading R-F32),
+ *          5 = S2_FP32 contexts: re-evaluate EVERY i-particle in fp64 (tests of the fix-up kernels: the sums are then fp64-accurate) */
 int s2_set_tuning(s2_ctx *ctx, int key, int value);
 /* Shape of the last force launch: out[0]=S, [1]=lanes per i, [2]=warp columns, [3]=grid size,
  * [4]=threads per CTA, [5]=dynamic shared memory bytes, [6]=0 no combine needed / 1 reduce kernel ran /

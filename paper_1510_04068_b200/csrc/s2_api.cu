@@ -23,8 +23,8 @@ cudaError_t launch_csr_scan(const double *rec, int ni, int cap, int *len, long l
                             long long *offsets, cudaStream_t st);
 cudaError_t launch_csr_fill(const int *list, const int *len, const long long *offsets, int ni, int cap, int *out, cudaStream_t st);
 int csr_blocks(int ni);
-cudaError_t launch_fp32_flag(const double *rec, const float *wq, int nst, int ni, const double2 *v2, const double2 *v3,
-                             const int *i_addr, double thresh, int *pos_list, int *count, cudaStream_t st);
+cudaError_t launch_fp32_fix(const ForceArgs &a, int sm_count, cudaStream_t st);
+cudaError_t launch_fp32_flag(const double *rec, const F32Flag &f, int ni, cudaStream_t st);
 cudaError_t launch_compare_records(const double *a, const double *b, int ni, int order, double tol, int *bad, cudaStream_t st);
 cudaError_t launch_unpack_records(const double *rec, int ni, int order, double *acc, double *jerk, double *snap, double *pot,
                                   int *nn_id, double *nn_r2, int *ngb_count, cudaStream_t st);
@@ -229,7 +229,7 @@ extern "C" int s2_close(s2_ctx *ctx)
     cudaStreamSynchronize(ctx->stream);
     for (Buf *b : {&ctx->base, &ctx->planes, &ctx->qplanes, &ctx->stage_dev, &ctx->iplanes, &ctx->iqplanes,
                    &ctx->i_addr, &ctx->i_h2, &ctx->part, &ctx->result, &ctx->seg, &ctx->list, &ctx->flags, &ctx->counters,
-                   &ctx->csr_len, &ctx->csr_bsum, &ctx->csr_off, &ctx->csr_list, &ctx->wq, &ctx->fix})
+                   &ctx->csr_len, &ctx->csr_bsum, &ctx->csr_off, &ctx->csr_list, &ctx->wq, &ctx->fix, &ctx->fixpart, &ctx->fixarr})
         dev_release(ctx, *b);
     for (auto &e : ctx->ev_csr)
         if (e) cudaEventDestroy(e);
@@ -999,12 +999,44 @@ int run_force(s2_ctx *ctx, int ni, const int *d_i_addr, const double *d_h2, bool
     // fp32, reading R-F32: the sweep leaves sum_j q_j^2 per (slice, i); particles whose jerk is a strongly cancelling sum
     // are then re-evaluated in fp64 (tune key 9 = 4 switches the fix-up off, for A/B measurements)
     const bool fixup = ctx->precision == S2_FP32 && ctx->order != 2 && !atomic && ctx->tune[9] != 4;
+    F32Flag f32{};
+    int fix_S = 1, fix_slice = nj_eff, fix_kcap = 2;
     if (fixup) {
+        // j-slices of the fix-up sweep: <= 256 particles each, so that even one flagged particle is spread over many
+        // warps; at most 2^20 partial rows [slice][flagged particle], with room for n_i / 16 flagged particles (any beyond
+        // that are swept unsliced by the same kernel)
+        fix_kcap = std::min((ni + 1) / 2 * 2, std::max(64, ni / 16 / 2 * 2));   // room for 6 % flagged (measured: 0.3-0.8 %)
+        // slice length: ~4096 j keeps the sweep near 290 Gpairs/s once there is an item per warp (measured: n_i = 65536,
+        // N = 65536: 185 Gpairs/s with 4096-particle slices, 83 with 256-particle ones; N = n_i = 2^18: 291 against 195 with
+        // 65536-particle ones); a short i-list flags a handful of particles (~n_i / 200), which want short slices instead
+        {
+            const int warps = 16 * ctx->sm_count, groups = std::max(1, ni / 400);
+            const int s_long = std::max(1, nj_eff / 4096), s_short = std::max(1, (nj_eff + 255) / 256);
+            fix_S = (long long)groups * s_long >= warps ? s_long : std::min(s_short, std::max(s_long, (warps + groups - 1) / groups));
+            fix_S = std::max(1, std::min(fix_S, std::max(1, (1 << 20) / fix_kcap)));
+        }
+        fix_slice = (nj_eff + fix_S - 1) / fix_S;
+        fix_S = (nj_eff + fix_slice - 1) / fix_slice;
         rc = dev_reserve(ctx, ctx->wq, (size_t)nst * ni * sizeof(float));
         if (rc == S2_OK) rc = dev_reserve(ctx, ctx->fix, 16 + (size_t)ni * sizeof(int));
+        // arrival counters of the fix-up groups: a buffer of their own (nothing else is ever written there), zeroed when
+        // it is allocated; the kernel resets every counter it used, so they are zero between calls
+        const size_t b_arr = (size_t)(ni / 2 + 1) * sizeof(unsigned);
+        if (rc == S2_OK && b_arr > ctx->fixarr.bytes) {
+            rc = dev_reserve(ctx, ctx->fixarr, b_arr);
+            if (rc == S2_OK) CU(cudaMemsetAsync(ctx->fixarr.p, 0, ctx->fixarr.bytes, ctx->stream));
+        }
+        if (rc == S2_OK && fix_S > 1) rc = dev_reserve(ctx, ctx->fixpart, (size_t)fix_S * fix_kcap * (ctx->order == 6 ? 10 : 7) * sizeof(double));
         if (rc != S2_OK) return rc;
         a.wq = (float *)ctx->wq.p;
-        CU(cudaMemsetAsync(ctx->fix.p, 0, sizeof(int), ctx->stream));
+        a.fix_count = (int *)ctx->fix.p;   // zeroed by the sweep itself
+        f32.wq = (const float *)ctx->wq.p;
+        f32.nst = nst;
+        f32.v2 = explicit_i ? (const double2 *)ctx->iplanes.p + (size_t)2 * ni : plane(ctx, 2);
+        f32.v3 = explicit_i ? (const double2 *)ctx->iplanes.p + (size_t)3 * ni : plane(ctx, 3);
+        f32.thresh = ctx->tune[9] == 5 ? 0.0 : kF32FlagThreshold;   // 5: flag every i-particle (tests of the fix-up itself)
+        f32.count = (int *)ctx->fix.p;
+        f32.pos_list = (int *)((char *)ctx->fix.p + 16);
     }
     if (atomic) CU(cudaMemsetAsync(ctx->result.p, 0, (size_t)ni * REC * sizeof(double), ctx->stream));
 
@@ -1030,6 +1062,7 @@ int run_force(s2_ctx *ctx, int ni, const int *d_i_addr, const double *d_h2, bool
     ctx->launches++;
     ctx->ran_force = true;
     ctx->ran_reduce = false;
+    bool flagged_inline = false;
     if (!final_direct && !fused && !atomic) {
         ReduceArgs r{};
         r.part = (const double *)ctx->part.p;
@@ -1044,6 +1077,11 @@ int run_force(s2_ctx *ctx, int ni, const int *d_i_addr, const double *d_h2, bool
         r.order = ctx->order;
         r.flags = flags;
         r.overflow_flag = (int *)ctx->flags.p;
+        if (fixup && reduce_by_warp_kernel(r)) {   // reduce_kernel flags while it has the final sums at hand: no flag launch
+            r.f32 = f32;
+            r.f32.i_addr = a.i_addr;
+            flagged_inline = true;
+        }
         if (ctx->timing) CU(cudaEventRecord(ctx->ev_t[4], ctx->stream));
         CU(launch_reduce(r, ctx->stream));
         if (ctx->timing) CU(cudaEventRecord(ctx->ev_t[5], ctx->stream));
@@ -1053,23 +1091,26 @@ int run_force(s2_ctx *ctx, int ni, const int *d_i_addr, const double *d_h2, bool
     if (fixup) {
         if (!ctx->ran_reduce && ctx->timing) CU(cudaEventRecord(ctx->ev_t[4], ctx->stream));
         const int np64 = nplanes(ctx->order);
-        int *cnt = (int *)ctx->fix.p, *pos = (int *)((char *)ctx->fix.p + 16);
-        const double2 *iv2 = explicit_i ? (const double2 *)ctx->iplanes.p + (size_t)2 * ni : plane(ctx, 2);
-        const double2 *iv3 = explicit_i ? (const double2 *)ctx->iplanes.p + (size_t)3 * ni : plane(ctx, 3);
-        CU(launch_fp32_flag(resp, (const float *)ctx->wq.p, nst, ni, iv2, iv3, a.i_addr, kF32FlagThreshold, pos, cnt, ctx->stream));
-        ForceArgs b = a;   // the flagged particles through the fp64 sweep: one warp per i, all j, final sums overwritten
+        f32.i_addr = a.i_addr;
+        if (!flagged_inline) {
+            CU(launch_fp32_flag(resp, f32, ni, ctx->stream));
+            ctx->launches++;
+        }
+        // the flagged particles through the fp64 fix-up sweep (fp32_fix_sweep_kernel, s2_force_fp64.cu)
+        ForceArgs b = a;
         for (int k = 0; k < kMaxPlanes; ++k) b.jp[k] = b.ip[k] = nullptr;
         for (int k = 0; k < np64; ++k) {
             b.jp[k] = plane(ctx, k);
             b.ip[k] = explicit_i ? (const void *)((double2 *)ctx->iplanes.p + (size_t)k * ni) : b.jp[k];
         }
-        b.h2 = nullptr; b.S = 1; b.slice_len = nj_eff; b.Wj = 1; b.tile = 256; b.stages = 4; b.nslices_total = 1; b.is_final = 1;
-        b.rec = resp; b.seg = nullptr; b.segcap = 0; b.fused = 0; b.cluster = 1; b.atomic = 0; b.wq = nullptr;
-        b.pos_list = pos; b.ni_dev = cnt;
-        const size_t smem64 = force_smem_bytes(np64, b.tile, b.stages);
-        CU(dispatch_force_fp64(ctx->order, 0, 32, dim3((ni + kWarps - 1) / kWarps, 1), smem64, b, ctx->stream, false, nullptr));
+        b.S = fix_S; b.slice_len = fix_slice;
+        b.h2 = nullptr; b.rec = resp; b.wq = nullptr; b.pos_list = f32.pos_list; b.ni_dev = f32.count;
+        b.fix_part = (double *)ctx->fixpart.p;
+        b.fix_kcap = fix_kcap;
+        b.fix_arrive = (unsigned *)ctx->fixarr.p;
+        CU(launch_fp32_fix(b, ctx->sm_count, ctx->stream));
         if (ctx->timing) CU(cudaEventRecord(ctx->ev_t[5], ctx->stream));
-        ctx->launches += 2;
+        ctx->launches++;
         ctx->ran_reduce = true;
         ctx->fix_last = -1;
     }

@@ -34,6 +34,8 @@ struct s2_ctx {
     Buf base, planes, qplanes, stage_dev, iplanes, iqplanes, i_addr, i_h2, part, result, seg, list, flags, counters;
     // device-side CSR of the neighbour lists of the last force call (built on first request, s2_ngb.cu)
     Buf csr_len, csr_bsum, csr_off, csr_list;
+    Buf fixarr;                       // fp32 fix-up: arrival counters of the groups (zero between calls)
+    Buf fixpart;                      // fp32 fix-up: partial rows [S][ni][7|10] of the flagged particles' j-slices
     Buf wq, fix;                       // fp32 fix-up (R-F32): sum of q^2 per (slice, i); {count, flagged positions}
     int fix_last = -1;                // flagged i-particles of the last fp32 call once read back (-1: not read)
     bool csr_valid = false;

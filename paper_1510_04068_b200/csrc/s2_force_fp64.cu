@@ -8,6 +8,8 @@
 // FP64-pipe instruction budget per pair: 32 for 4th order (33 with the
 // decision distance kept separate), 54 for 6th order; the reciprocal square root is one
 // MUFU.RSQ64H seed (rsqrt.approx.ftz.f64, ~2^-22) plus one third-order Newton step (5 FP64 ops).
+#include <algorithm>
+
 #include "s2_force_sweep.cuh"
 
 namespace s2 {
@@ -96,9 +98,8 @@ struct PolicyF64 {
 
     using Part = Acc;   // fp64 partial sums per tile, added to fp64 totals
 
-    static __device__ __forceinline__ void load_i(const ForceArgs &a, int i_, IState &I)
+    static __device__ __forceinline__ void load_i(const ForceArgs &a, int i, IState &I)
     {
-        const int i = a.pos_list ? a.pos_list[i_] : i_;   // sub-list built on the device (fp32 fix-up): position in the i-list
         const int ia = a.i_addr ? a.i_addr[i] : i;
         const double2 p0 = static_cast<const double2 *>(a.ip[0])[ia];
         const double2 p1 = static_cast<const double2 *>(a.ip[1])[ia];
@@ -239,6 +240,163 @@ cudaError_t dispatch_force_fp64(int order, unsigned flags, int L, dim3 grid, siz
     if (ngb) return launch_L<PolicyF64<6, true, true>>(L, grid, smem, a, st, query, ctas_per_sm);
     if (nn) return launch_L<PolicyF64<6, true, false>>(L, grid, smem, a, st, query, ctas_per_sm);
     return launch_L<PolicyF64<6, false, false>>(L, grid, smem, a, st, query, ctas_per_sm);
+}
+
+// ---- fp32 fix-up (reading R-F32) -----------------------------------------------------------------
+// The fp32 sweep flags the few i-particles whose jerk is a strongly cancelling sum (fp32_flag_kernel, s2_results.cu);
+// they are re-evaluated here with the fp64 pair arithmetic above.  The flagged list is short (0.3-0.8 % of the i-list)
+// and its length is known only on the device, so the work is cut into items (pair of flagged i, j-slice of <= 256
+// particles) that the warps of a fixed grid take in turn: a single flagged particle is spread over N / 256 warps
+// (2.5 us at N = 65536) instead of being swept by one warp alone (300 us).  No shared memory and no barrier: lanes
+// read their own j from the L2-resident planes (coalesced 16-byte loads), each j feeds the two i of the item.
+// Sums: lanes combine by the xor-butterfly; the slices of a group are added by the last warp to finish one of them, in
+// a fixed order (below) -- deterministic.  Launched with programmatic stream serialisation behind the flagging kernel.
+constexpr int kFixG = 2;          // flagged i-particles per item
+template <class P>
+__global__ void __launch_bounds__(128, P::ORDER == 6 ? 3 : 4) fp32_fix_sweep_kernel(const ForceArgs a)
+{
+    asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
+    asm volatile("griddepcontrol.wait;" ::: "memory");
+    constexpr int NC = P::ORDER == 6 ? 10 : 7;
+    __shared__ double s_V[kFixG * NC][128];
+    const int count = *a.ni_dev;
+    // groups below the capacity of the partial-row buffer are cut into a.S j-slices, one item each; the (unexpected)
+    // rest takes one item per group that walks the same slices itself and adds them in the combine's order, so that a
+    // particle gets the same bits whichever way it is handled and however many particles were flagged
+    const int ngroups = (count + kFixG - 1) / kFixG, gcap = a.fix_kcap / kFixG;
+    const int nsliced = a.S > 1 ? min(ngroups, gcap) : 0;
+    const long long items_sliced = (long long)nsliced * a.S, items = items_sliced + (ngroups - nsliced);
+    const int lane = threadIdx.x & 31;
+    const long long nw = ((long long)gridDim.x * blockDim.x) >> 5;
+    Decomp d{};
+    Dec D{};
+    for (long long it = ((long long)blockIdx.x * blockDim.x + threadIdx.x) >> 5; it < items; it += nw) {
+        const bool sliced = it < items_sliced;
+        const int g = sliced ? (int)(it / a.S) : nsliced + (int)(it - items_sliced);   // neighbouring warps: same i, next slice
+        const int s_begin = sliced ? (int)(it % a.S) : 0, s_end = sliced ? s_begin + 1 : a.S;
+        typename P::IState I[kFixG];
+        int pos[kFixG];
+#pragma unroll
+        for (int u = 0; u < kFixG; ++u) {
+            pos[u] = a.pos_list[min(g * kFixG + u, count - 1)];   // an odd tail recomputes the last entry, never written
+            P::load_i(a, pos[u], I[u]);
+        }
+        // unsliced (rare): lane l holds the sum of slices l, l + 32, ... -- in shared memory, so that the common path
+        // does not carry 2 x NC live doubles through the j loop
+        if (!sliced) {
+#pragma unroll
+            for (int c = 0; c < kFixG * NC; ++c) s_V[c][threadIdx.x] = 0.0;
+        }
+        for (int s = s_begin; s < s_end; ++s) {
+            typename P::Acc A[kFixG];
+#pragma unroll
+            for (int u = 0; u < kFixG; ++u) A[u].zero();
+            const int j0 = a.j_first + s * a.slice_len, j1 = min(a.j_first + a.nj, j0 + a.slice_len);
+#pragma unroll 4
+            for (int jb = j0; jb < j1; jb += 32) {
+                const bool valid = jb + lane < j1;
+                const int j = valid ? jb + lane : j1 - 1;
+                typename P::JData J;
+                J.p0 = static_cast<const double2 *>(a.jp[0])[j]; J.p1 = static_cast<const double2 *>(a.jp[1])[j];
+                J.p2 = static_cast<const double2 *>(a.jp[2])[j]; J.p3 = static_cast<const double2 *>(a.jp[3])[j];
+                if (P::ORDER == 6) { J.p4 = static_cast<const double2 *>(a.jp[4])[j]; J.p5 = static_cast<const double2 *>(a.jp[5])[j]; }
+#pragma unroll
+                for (int u = 0; u < kFixG; ++u) P::template interact<1, true>(J, valid, j, I[u], A[u], D, d, nullptr, 0);
+            }
+#pragma unroll
+            for (int m = 1; m < 32; m <<= 1) {
+#pragma unroll
+                for (int u = 0; u < kFixG; ++u) A[u].shfl_add(m);      // every lane ends with the same slice sums
+            }
+#pragma unroll
+            for (int u = 0; u < kFixG; ++u) {
+                double out[10];
+                A[u].to_f64(out);
+                const int k = g * kFixG + u;
+                if (sliced) {
+                    if (lane == 0 && k < count) {
+                        double *r = a.fix_part + ((size_t)s * a.fix_kcap + k) * NC;
+#pragma unroll
+                        for (int c = 0; c < NC; ++c) r[c] = out[c];
+                    }
+                } else if (lane == (s & 31)) {
+#pragma unroll
+                    for (int c = 0; c < NC; ++c) s_V[u * NC + c][threadIdx.x] += out[c];
+                }
+            }
+        }
+        bool add_up = !sliced;
+        double V[kFixG][NC];
+#pragma unroll
+        for (int u = 0; u < kFixG; ++u)
+#pragma unroll
+            for (int c = 0; c < NC; ++c) V[u][c] = sliced ? 0.0 : s_V[u * NC + c][threadIdx.x];
+        if (sliced) {
+            // the last warp to finish a slice of this group adds the group's rows: lane l takes slices l, l + 32, ... in
+            // that order, then the xor-butterfly -- the same sums whoever arrives last.  No floating-point atomics.
+            unsigned prev = 0;
+            if (lane == 0) {
+                __threadfence();
+                prev = atomicAdd(a.fix_arrive + g, 1u);
+            }
+            prev = __shfl_sync(0xffffffffu, prev, 0);
+            add_up = prev == (unsigned)a.S - 1u;
+            if (add_up) {
+                __threadfence();
+#pragma unroll
+                for (int u = 0; u < kFixG; ++u) {
+                    const int k = min(g * kFixG + u, count - 1);
+                    for (int sl = lane; sl < a.S; sl += 32) {
+                        const double *r = a.fix_part + ((size_t)sl * a.fix_kcap + k) * NC;
+#pragma unroll
+                        for (int c = 0; c < NC; ++c) V[u][c] += __ldcg(r + c);
+                    }
+                }
+                if (lane == 0) a.fix_arrive[g] = 0u;     // ready for the next call
+            }
+        }
+        if (add_up) {                                    // warp-uniform
+#pragma unroll
+            for (int m = 1; m < 32; m <<= 1) {
+#pragma unroll
+                for (int u = 0; u < kFixG; ++u)
+#pragma unroll
+                    for (int c = 0; c < NC; ++c) V[u][c] += shfl_xor_d(V[u][c], m);
+            }
+            if (lane == 0) {
+#pragma unroll
+                for (int u = 0; u < kFixG; ++u) {
+                    if (g * kFixG + u >= count) continue;
+                    double *r = a.rec + (size_t)pos[u] * REC;
+#pragma unroll
+                    for (int c = 0; c < 7; ++c) r[c] = V[u][c];
+                    if (P::ORDER == 6) { r[9] = V[u][7]; r[10] = V[u][8]; r[11] = V[u][9]; }
+                }
+            }
+        }
+    }
+}
+
+template <class K>
+static cudaError_t launch_pdl_fix(K kern, int grid, const ForceArgs &a, cudaStream_t st)
+{
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3(grid); cfg.blockDim = dim3(128); cfg.stream = st;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    at[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = at; cfg.numAttrs = 1;
+    return cudaLaunchKernelEx(&cfg, kern, a);
+}
+
+// a.S j-slices of a.slice_len; a.ni = length of the whole i-list (bound of the flagged count); sm_count for the grid
+cudaError_t launch_fp32_fix(const ForceArgs &a, int sm_count, cudaStream_t st)
+{
+    const long long worst = (long long)(a.fix_kcap / kFixG) * a.S + a.ni / kFixG + 1;   // items if every i were flagged
+    const int grid = (int)std::min<long long>((worst + 3) / 4, (long long)4 * sm_count);
+    cudaError_t e = a.order == 6 ? launch_pdl_fix(fp32_fix_sweep_kernel<PolicyF64<6, false, false>>, grid, a, st)
+                                 : launch_pdl_fix(fp32_fix_sweep_kernel<PolicyF64<4, false, false>>, grid, a, st);
+    return e;
 }
 
 #endif   // S2_BANK_ONLY

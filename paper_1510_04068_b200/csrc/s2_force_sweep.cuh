@@ -176,6 +176,26 @@ __device__ __forceinline__ void reduce_rows_warp(const double *part, double *out
     }
 }
 
+// fp32 path, reading R-F32: is the jerk of i-particle i a strongly cancelling sum?  Each fp32 pair term is good to
+// ~4e-7, so the error of the sum is ~4e-7 sqrt(sum_j |t_j|^2), and sqrt(sum_j |t_j|^2) ~ sqrt(sum_j q_j^2) V with
+// V = |v_i| + sqrt(2 |pot_i|) (own speed + local escape speed bound the relative speeds that matter).  Called by a whole
+// warp that has just written the final record of i (lane 0); the rows of sum q^2 are added lane-parallel in a fixed order.
+__device__ __forceinline__ void fp32_flag_warp(const F32Flag &f, const double *rec, int i, int ni, int lane)
+{
+    double w = 0.0;
+    for (int s = lane; s < f.nst; s += 32) w += (double)f.wq[(size_t)s * ni + i];
+#pragma unroll
+    for (int m = 1; m < 32; m <<= 1) w += shfl_xor_d(w, m);
+    if (lane == 0) {
+        const double *r = rec + (size_t)i * REC;
+        const double J = sqrt(r[3] * r[3] + r[4] * r[4] + r[5] * r[5]);
+        const int ia = f.i_addr ? f.i_addr[i] : i;
+        const double2 a = f.v2[ia], b = f.v3[ia];
+        const double V = sqrt(a.x * a.x + a.y * a.y + b.x * b.x) + sqrt(2.0 * fabs(r[6]));
+        if (sqrt(w) * V > f.thresh * J) f.pos_list[atomicAdd(f.count, 1)] = i;
+    }
+}
+
 // Ring of ST shared-memory tile buffers filled by 1-D bulk copies (one per plane) that complete on an mbarrier.
 // Thread 0 issues; everybody waits on the barrier of the tile it is about to read.
 template <int NPL>
@@ -242,12 +262,9 @@ __global__ void __launch_bounds__(kThreads, P::kMinBlocks) force_sweep_kernel(co
 {
     extern __shared__ __align__(128) unsigned char smem_raw[];
     constexpr int NPL = P::NPL;
-    int ni_eff = a.ni;
-    if (a.ni_dev) {   // length of a device-built sub-list: the grid was sized for the worst case, surplus CTAs leave
-        ni_eff = *a.ni_dev;
-        if ((int)blockIdx.x * (kWarps / a.Wj) * (32 / L) >= ni_eff) return;
-    }
-    const Decomp d = decompose<L>(a.Wj, ni_eff);
+    const Decomp d = decompose<L>(a.Wj, a.ni);
+    if constexpr (P::kTrackW)   // fp32: the flagged count of this call starts at zero (it is only raised by later launches)
+        if (a.fix_count && blockIdx.x == 0 && blockIdx.y == 0 && threadIdx.x == 0) *a.fix_count = 0;
     TilePipe<NPL> pipe;
     pipe.init(smem_raw, a);
     unsigned char *tiles = pipe.tiles;
@@ -322,15 +339,6 @@ __global__ void __launch_bounds__(kThreads, P::kMinBlocks) force_sweep_kernel(co
 
     double out[10];
     tot.to_f64(out);
-    if (a.pos_list) {   // fp64 re-evaluation of a flagged i-particle: only the sums of its final record are replaced
-        if (d.jl == 0 && d.i_valid) {
-            double *r = a.rec + (size_t)a.pos_list[d.i] * REC;
-#pragma unroll
-            for (int c = 0; c < 7; ++c) r[c] = out[c];
-            if (a.order == 6) { r[9] = out[7]; r[10] = out[8]; r[11] = out[9]; }
-        }
-        return;
-    }
     int nn = D.nn_j;
     int row = d.slice;                      // partial row this thread's record goes to
     bool writer = d.jl == 0 && d.i_valid;
@@ -476,6 +484,8 @@ __global__ void __launch_bounds__(kThreads, P::kMinBlocksTiled) force_sweep_tile
     static_assert(TL == 1 || (!P::NN && !P::NGB), "lanes per i-slot > 1: plain sums only");
     constexpr int IPC = kThreads / TL;   // i-slots per CTA (each holds IPT i-particles)
     const int jl = (threadIdx.x & 31) % TL;
+    if constexpr (P::kTrackW)
+        if (a.fix_count && blockIdx.x == 0 && blockIdx.y == 0 && threadIdx.x == 0) *a.fix_count = 0;
     extern __shared__ __align__(128) unsigned char smem_raw[];
     constexpr int NPL = P::NPL;
     TilePipe<NPL> pipe;

@@ -98,10 +98,14 @@ struct ForceArgs {
     // fp32 path, reading R-F32 (s2_api.cu fp32_fixup): the sweep leaves sum_j q_j^2 per (slice, i) so that particles whose
     // jerk is a strongly cancelling sum can be found and re-evaluated in fp64
     float *wq;                     // [nslices_total][ni], or nullptr
-    // fp64 re-evaluation of a device-built sub-list: i-particle k of this launch is entry pos_list[k] of the i-list, the
-    // count is read from device memory (CTAs beyond it exit), only the sums of its final record are overwritten
+    int *fix_count;                // number of flagged i-particles: the sweep zeroes it (saves a memset node per call)
+    // fp32 fix-up (fp32_fix_sweep_kernel, s2_force_fp64.cu): the flagged i-particles, as positions in the i-list, their
+    // number (device memory: known only after the flag kernel ran), and the partial rows [S][ni][NC] of their j-slices
     const int *pos_list;
     const int *ni_dev;
+    double *fix_part;              // [S][fix_kcap][NC]
+    int fix_kcap;                  // flagged particles the partial rows have room for (even); the rest is swept unsliced
+    unsigned *fix_arrive;          // [ceil(ni / 2)] arrival counters of the fix-up groups, zero between calls
     int atomic;                    // 1: j-slices add their sums to the zeroed final records with fp64 atomics (opt-in,
                                    // the paper's Sapporo2 combine L88; not bit-reproducible; no NN / neighbour lists)
     // uniform-operand sweep (force_sweep_bank_kernel): the chunk of j now in the constant bank
@@ -121,6 +125,17 @@ struct ForceArgs {
     int bank_threads;              // threads per CTA of the chunk launches (128 or 256; 0: the policy's default)
 };
 
+// fp32 path, reading R-F32: what is needed to decide whether an i-particle's jerk is a strongly cancelling sum
+struct F32Flag {
+    const float *wq;               // [nst][ni] sum of q^2 per (slice, i), or nullptr: no flagging
+    int nst;
+    const double2 *v2, *v3;        // fp64 planes P2 (vx, vy), P3 (vz, id) of the i side
+    const int *i_addr;             // nullptr: i-th i-particle lives at index i of the planes
+    double thresh;
+    int *pos_list;                 // out: positions (in the i-list) of the flagged particles, any order
+    int *count;                    // out: their number
+};
+
 struct ReduceArgs {
     const double *part;            // [nslices_total][ni][REC]
     double *out;                   // [ni][REC]
@@ -134,12 +149,14 @@ struct ReduceArgs {
     int order;
     unsigned flags;
     int *overflow_flag;
+    F32Flag f32;                   // fp32 contexts: flag ill-conditioned jerk sums while the final sums are at hand (wq != nullptr)
 };
 
 // kernels' host-side launchers (each returns the cudaError_t of the launch)
 cudaError_t launch_scatter(const ScatterArgs &a, cudaStream_t st);
 cudaError_t launch_predict(const PredictArgs &a, cudaStream_t st);
 cudaError_t launch_reduce(const ReduceArgs &a, cudaStream_t st);
+bool reduce_by_warp_kernel(const ReduceArgs &a);   // true: launch_reduce takes reduce_kernel (one warp per i), which flags inline
 
 struct ForceShape {                // chosen by the balancer in s2_api.cu
     int L;                         // lanes per i (1..32); 0: register-tiled sweep (several i per thread)

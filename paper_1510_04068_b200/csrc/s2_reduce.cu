@@ -32,6 +32,7 @@ __global__ void __launch_bounds__(256) reduce_kernel(const ReduceArgs a)
             reduce_rows_warp<true>(a.part, a.out, a.jid_plane, i, a.ni, S, a.order, lane);
         else
             reduce_rows_warp<false>(a.part, a.out, a.jid_plane, i, a.ni, S, a.order, lane);
+        if (a.f32.wq) fp32_flag_warp(a.f32, a.out, i, a.ni, lane);   // lane 0 reads back the record it has just written
         return;
     }
 
@@ -106,6 +107,7 @@ __global__ void __launch_bounds__(256) reduce_kernel(const ReduceArgs a)
         o[4] = make_double2(__hiloint2double(cnt_total, nn), v[7]);
         o[5] = make_double2(v[8], v[9]);
     }
+    if (a.f32.wq) fp32_flag_warp(a.f32, a.out, i, a.ni, lane);
 }
 
 // Few partial rows, many i-particles (the full-occupancy sweeps with 2-16 j-slices): one THREAD per i streams its
@@ -175,10 +177,15 @@ static cudaError_t launch_reduce_thread(const ReduceArgs &a, cudaStream_t st)
     return cudaGetLastError();
 }
 
+bool reduce_by_warp_kernel(const ReduceArgs &a)
+{
+    return !(!(a.flags & S2_WANT_NGB) && a.nslices_total >= 2 && a.nslices_total <= 16 && a.ni >= 4096);
+}
+
 cudaError_t launch_reduce(const ReduceArgs &a, cudaStream_t st)
 {
     if (a.ni <= 0) return cudaSuccess;
-    if (!(a.flags & S2_WANT_NGB) && a.nslices_total <= 16 && a.ni >= 4096) {
+    if (!reduce_by_warp_kernel(a)) {
         switch (a.nslices_total) {   // ordinary stream order (no programmatic launch): the rows are read through L1
         case 2: return launch_reduce_thread<2>(a, st);
         case 3: return launch_reduce_thread<3>(a, st);

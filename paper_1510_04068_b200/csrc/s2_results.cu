@@ -2,7 +2,7 @@
 // the caller's device arrays (same layouts as s2_get_results), so that a consumer on the GPU -- the block-step
 // integrator kernels, an NCCL combine of j-sharded partial results (sec 2.2.3) -- never goes through
 // the host.  Pure data movement: one thread per i reads its record (three 32-byte sectors) and writes the fields.
-#include "s2_internal.h"
+#include "s2_force_sweep.cuh"
 
 namespace s2 {
 
@@ -33,32 +33,28 @@ cudaError_t launch_unpack_records(const double *rec, int ni, int order, double *
     return cudaGetLastError();
 }
 
-// fp32 path, reading R-F32: which i-particles have a jerk that is a strongly cancelling sum?  Each fp32 pair term is good
-// to ~4e-7, so the error of the sum is ~4e-7 sqrt(sum_j |t_j|^2) and sqrt(sum_j |t_j|^2) ~ sqrt(sum_j q_j^2) V with
-// V = |v_i| + sqrt(2 |pot_i|) (the particle's own speed plus the local escape speed bounds the relative speeds that
-// matter).  The sweep left sum_j q_j^2 per (slice, i); rows are added here in slice order (deterministic).  An i-particle
-// whose estimate exceeds `thresh` times its jerk goes on the list that the fp64 sweep re-evaluates.
-__global__ void __launch_bounds__(256) fp32_flag_kernel(const double *rec, const float *wq, int nst, int ni, const double2 *v2,
-                                                        const double2 *v3, const int *i_addr, double thresh, int *pos_list, int *count)
+// fp32 path, reading R-F32: flag the i-particles whose jerk is a strongly cancelling sum (fp32_flag_warp,
+// s2_force_sweep.cuh) for the launch shapes whose final records are not written by reduce_kernel (which flags inline):
+// single-slice sweeps, the fused combine, reduce_thread_kernel.  One warp per i.
+__global__ void __launch_bounds__(256) fp32_flag_kernel(const double *rec, F32Flag f, int ni)
 {
-    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    asm volatile("griddepcontrol.launch_dependents;" ::: "memory");   // chained by programmatic dependent launch:
+    asm volatile("griddepcontrol.wait;" ::: "memory");                // sweep (-> reduce) -> flag -> fix-up
+    const int i = (blockIdx.x * blockDim.x + threadIdx.x) >> 5;
     if (i >= ni) return;
-    double w = 0.0;
-    for (int s = 0; s < nst; ++s) w += (double)wq[(size_t)s * ni + i];
-    const double *r = rec + (size_t)i * REC;
-    const double J = sqrt(r[3] * r[3] + r[4] * r[4] + r[5] * r[5]);
-    const int ia = i_addr ? i_addr[i] : i;
-    const double2 a = v2[ia], b = v3[ia];
-    const double V = sqrt(a.x * a.x + a.y * a.y + b.x * b.x) + sqrt(2.0 * fabs(r[6]));
-    if (sqrt(w) * V > thresh * J) pos_list[atomicAdd(count, 1)] = i;   // list order is arbitrary; each entry is evaluated on its own
+    fp32_flag_warp(f, rec, i, ni, threadIdx.x & 31);
 }
 
-cudaError_t launch_fp32_flag(const double *rec, const float *wq, int nst, int ni, const double2 *v2, const double2 *v3,
-                             const int *i_addr, double thresh, int *pos_list, int *count, cudaStream_t st)
+cudaError_t launch_fp32_flag(const double *rec, const F32Flag &f, int ni, cudaStream_t st)
 {
     if (ni <= 0) return cudaSuccess;
-    fp32_flag_kernel<<<(ni + 255) / 256, 256, 0, st>>>(rec, wq, nst, ni, v2, v3, i_addr, thresh, pos_list, count);
-    return cudaGetLastError();
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3((unsigned)(((long long)ni * 32 + 255) / 256)); cfg.blockDim = dim3(256); cfg.stream = st;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    at[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = at; cfg.numAttrs = 1;
+    return cudaLaunchKernelEx(&cfg, fp32_flag_kernel, rec, f, ni);
 }
 
 // Self-test of the uniform-operand sweep (s2_api.cu bank_selftest): do two sets of records hold the same sums?

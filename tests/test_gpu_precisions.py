@@ -388,3 +388,51 @@ def test_fp32_fixup_meets_1e5_on_a_cancelling_sum():
     print("fp32 fix-up: flagged", s2.s2_fp32_fixup_count(ctx), "of", il.size, "worst jerk error with / without:",
           out[(0, ())][2].max(), out[(4, ())][2].max())
     s2.s2_close(ctx)
+
+
+@pytest.mark.parametrize("order", [4, 6])
+def test_fp32_fixup_kernels_give_fp64_sums_when_every_particle_is_flagged(order):
+    """The fix-up re-evaluates flagged i-particles with the fp64 pair arithmetic, cut into j-slices that the last warp
+    to arrive adds up; flagged particles beyond the room of its partial-row buffer are swept unsliced.  Forcing EVERY
+    particle to be flagged (s2_set_tuning key 9 = 5) runs both branches on all i: an fp32 context must then return
+    sums within the FP64 tolerances of the oracle, bit-identically from call to call, for address lists and explicit
+    sinks, with decisions and lists unchanged."""
+    w = make_config(4 if order == 6 else 5, N=3000, order=order)
+    ctx = open_and_load(w, order, precision=s2.S2_FP32, ngb_cap=24)
+    s2.s2_predict(ctx, w.t_pred, w.N)
+    tol = dict(acc=1e-13, pot=1e-13, jerk=1e-12, snap=1e-12)
+    for ni, shape in ((700, {}), (700, {0: 3, 1: 4}), (3000, {}), (37, {0: 5, 1: 32}), (1, {})):
+        il = w.ilist(ni)
+        h2 = w.h2[il] * 0.6
+        ref, (xp, vp, ap) = oracle_on_gpu_prediction(ctx, w, order, il, w.eps2, h2, ngb_cap=24)
+        for k in range(9):
+            s2.s2_set_tuning(ctx, k, shape.get(k, 0))
+        s2.s2_set_tuning(ctx, 9, 5)
+        runs = []
+        for _ in range(2):
+            s2.s2_calc_ilist(ctx, il, h2, w.eps2, NN | NGB)
+            runs.append(s2.s2_get_results(ctx, ni))
+        res = runs[0]
+        assert s2.s2_fp32_fixup_count(ctx) == ni
+        for q in ("acc", "jerk", "pot") + (("snap",) if order == 6 else ()):
+            assert np.array_equal(runs[0][q], runs[1][q]), (ni, q)
+            e = rel_err(res[q], getattr(ref, q)).max()
+            assert e <= tol[q], f"order {order} n_i {ni} {shape}: {q} {e:.2e} with every particle re-evaluated in fp64"
+        check_nn_ld(res, ref, f"all flagged n_i {ni}")
+        assert np.array_equal(res["ngb_count"], ref.ngb_count)
+        check_neighbour_lists(ctx, ref, ni, 24, f"all flagged n_i {ni}", counts=res["ngb_count"])
+    # explicit sinks (the i-state comes from the caller's planes, not from the j-store)
+    rng = np.random.default_rng(3)
+    ni = 90
+    xi, vi, ai = rng.normal(size=(ni, 3)) * 0.5, rng.normal(size=(ni, 3)) * 0.3, rng.normal(size=(ni, 3))
+    ids = np.full(ni, -1, np.int32)
+    for k in range(9):
+        s2.s2_set_tuning(ctx, k, 0)
+    s2.s2_set_tuning(ctx, 9, 5)
+    s2.s2_calc_explicit(ctx, ids, xi, vi, ai if order == 6 else None, None, w.eps2, 0)
+    res = s2.s2_get_results(ctx, ni)
+    xp, vp, ap = s2.s2_get_predicted_j(ctx, 0, w.N)
+    ref = oracle.forces(order, w.mass, w.ident, xp, vp, ap, ids, xi, vi, ai if order == 6 else None, w.eps2)
+    for q in ("acc", "jerk", "pot") + (("snap",) if order == 6 else ()):
+        assert rel_err(res[q], getattr(ref, q)).max() <= tol[q], ("explicit", q)
+    s2.s2_close(ctx)
