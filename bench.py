@@ -57,7 +57,7 @@ def parse_args():
     ap.add_argument("--N", type=int, default=0, help="override N (reduced sizes are for debugging only)")
     ap.add_argument("--precision", default="fp64", choices=["fp64", "ds", "fp32"],
                     help="pair-arithmetic precision of the timed step (the default bench line is fp64)")
-    ap.add_argument("--section", default="all", choices=["all", "hbm", "shapes"],
+    ap.add_argument("--section", default="all", choices=["all", "hbm", "shapes", "fp32fix"],
                     help="hbm: only the streaming-kernel (predictor / scatter) measurement, for ncu captures; shapes: the "
                          "launch-shape space around n_i = 32 and the atomics-versus-reduce A/B (profiles/r02_small_ni.md)")
     ap.add_argument("--shard", default="i", choices=["i", "j"],
@@ -181,6 +181,12 @@ def main():
         if rank == 0:
             run_blockstep(args.blockstep, args.bs_tend, tuple(int(x) for x in args.bs_orders.split(",")),
                           tuple(args.bs_precisions.split(",")))
+        return
+    if args.section == "fp32fix":
+        if rank == 0:
+            import torch
+            import paper_1510_04068_b200 as s2
+            print(json.dumps(fp32_fixup_cost(s2, torch, torch.device("cuda", local))), flush=True)
         return
     if args.section == "shapes":
         if rank == 0:
@@ -480,6 +486,49 @@ def graph_time_us(s2, torch, ctx, fn, calls=20, reps=7):
         ts.append(e0.elapsed_time(e1) / calls * 1e3)
     s2.s2_set_stream(ctx, torch.cuda.current_stream().cuda_stream)
     return statistics.median(ts[1:])
+
+
+def fp32_fixup_cost(s2, torch, dev):
+    """Cost of the fp32 path's fp64 re-evaluation of ill-conditioned jerk sums (reading R-F32): device time per
+    s2_calc_ilist_device call with the fix-up (default) and without it (s2_set_tuning key 9 = 4), and the number of
+    flagged particles; config 3 (graph-timed), the headline particle set and config 5 (CUDA events)."""
+    from workloads import make_config
+    out = {"rows": []}
+    for key, nis, flags in ((3, (1, 32, 256, 2048, 16384, 65536), 0), ("H", (262144,), 0), (5, (1048576,), 3)):
+        w = make_config(key)
+        ctx = s2.s2_open(dev.index, 4, s2.S2_FP32, nj_capacity=w.N, ngb_cap=256 if flags else 0)
+        a = np.arange(w.N, dtype=np.int32)
+        s2.s2_set_j(ctx, a, w.ident, w.t_j, w.mass, w.pos, w.vel, w.acc, w.jerk)
+        s2.s2_commit_j(ctx)
+        s2.s2_predict(ctx, w.t_pred, w.N)
+        for ni in nis:
+            ilh = w.ilist(ni)
+            il = torch.from_numpy(ilh).to(dev)
+            h2 = torch.from_numpy(np.ascontiguousarray(w.h2[ilh])).to(dev) if flags else None
+            row = {"cfg": str(key), "N": w.N, "n_i": ni}
+            for name, key9 in (("with_fixup_us", 0), ("without_fixup_us", 4)):
+                s2.s2_set_tuning(ctx, 9, key9)
+                if ni * w.N < 1e9:
+                    us = graph_time_us(s2, torch, ctx, lambda: s2.s2_calc_ilist_device(ctx, il, h2, w.eps2, flags),
+                                       calls=20 if ni * w.N < 2e8 else 4, reps=5)
+                else:
+                    s2.s2_enable_timing(ctx, True)
+                    ts = []
+                    for r in range(3):
+                        s2.s2_calc_ilist_device(ctx, il, h2, w.eps2, flags)
+                        t = s2.s2_get_timing(ctx)
+                        ts.append(t["force_ms"] + t["reduce_ms"])
+                    s2.s2_enable_timing(ctx, False)
+                    us = min(ts[1:]) * 1e3
+                row[name] = round(us, 1)
+            s2.s2_set_tuning(ctx, 9, 0)
+            s2.s2_calc_ilist_device(ctx, il, h2, w.eps2, flags)
+            row["flagged"] = s2.s2_fp32_fixup_count(ctx)
+            row["ginteractions_per_s_with"] = round(ni * w.N / row["with_fixup_us"] / 1e3, 1)
+            row["ginteractions_per_s_without"] = round(ni * w.N / row["without_fixup_us"] / 1e3, 1)
+            out["rows"].append(row)
+        s2.s2_close(ctx)
+    return out
 
 
 def shape_space(s2, torch, dev):
