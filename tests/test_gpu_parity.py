@@ -390,7 +390,7 @@ def test_cfg4_sixth_order_ni1024():
     s2.s2_close(ctx)
 
 
-@pytest.mark.parametrize("kind", ["plummer", "lattice"])
+@pytest.mark.parametrize("kind", ["plummer", "lattice", "plummer-fp32"])
 def test_j_sharded_partials_combine_to_the_unsharded_result(kind):
     """j-sharding: three "ranks" run one after the other on this GPU, each a context that
     holds the whole store and sums over its own address block (s2_set_j_range).  Their partial results, combined the
@@ -399,16 +399,17 @@ def test_j_sharded_partials_combine_to_the_unsharded_result(kind):
     tolerance, nearest neighbours, counts and lists exactly -- exact ties on the lattice included."""
     import torch
     from paper_1510_04068_b200.sharding import ShardedForces, merge_rank_lists
-    w = make_config(5, N=5000) if kind == "plummer" else lattice_workload(12, 0.25)
+    P = s2.S2_FP32 if kind.endswith("fp32") else s2.S2_FP64     # fp32: every shard flags and re-evaluates on its own partial sums
+    w = make_config(5, N=5000) if kind.startswith("plummer") else lattice_workload(12, 0.25)
     cap = 16
     world = 3
     ni = 700
     il = w.ilist(ni)
-    h2 = w.h2[il] * (2.0 if kind == "plummer" else 1.0)
+    h2 = w.h2[il] * (2.0 if kind.startswith("plummer") else 1.0)
     d_il, d_h2 = torch.from_numpy(il).cuda(), torch.from_numpy(np.ascontiguousarray(h2)).cuda()
     parts = []
     for r in range(world):
-        sf = ShardedForces(w.N, order=4, ngb_cap=cap, rank=r, world=world)
+        sf = ShardedForces(w.N, order=4, precision=P, ngb_cap=cap, rank=r, world=world)
         sf.set_all_j(w.ident, w.t_j, w.mass, w.pos, w.vel, w.acc, w.jerk)
         p = sf.partial(w.t_pred, d_il, d_h2, w.eps2, NN | NGB)
         parts.append({k: (v.clone() if v is not None else None) for k, v in p.items()})
@@ -427,7 +428,7 @@ def test_j_sharded_partials_combine_to_the_unsharded_result(kind):
     off, lst = off.cpu().numpy(), lst.cpu().numpy()
     ref = oracle.forces_ilist(4, w.mass, w.ident, xp, vp, None, il, w.eps2, h2, cap)
     res = dict(acc=acc, jerk=jerk, pot=pot, nn_id=best_id.cpu().numpy(), nn_r2=best_r2.cpu().numpy(), ngb_count=cnt)
-    check_forces(res, ref, s2.S2_FP64, 4, NN | NGB, f"j-sharded {kind}")
+    check_forces(res, ref, P, 4, NN | NGB, f"j-sharded {kind}")
     assert (ref.ngb_count > cap).any() or kind == "lattice"
     for i in range(ni):
         want = ref.ngb_list[i][ref.ngb_list[i] >= 0]

@@ -145,3 +145,22 @@ def test_device_integrator_conserves_energy_and_reaches_t_end():
         assert abs((e1 - e0) / e0) < lim and abs((e2 - e0) / e0) < lim
         assert hist.min() < w.N // 8 and hist.max() == w.N
         d.close()
+
+
+@pytest.mark.gpu
+def test_device_integrator_in_fp32_runs_and_conserves_energy():
+    """fp32 pair arithmetic under the integrator (its force calls go through the fp64 re-evaluation of ill-conditioned
+    sums, DESIGN.md R-F32): reaches t_end with block-aligned power-of-two steps and conserves energy at the fp32 level."""
+    import paper_1510_04068_b200 as s2
+    from paper_1510_04068_b200.hermite import DeviceHermite
+    w = make_config(1, N=1024)
+    d = DeviceHermite(w.mass, w.pos, w.vel, w.eps2, order=4, precision=s2.S2_FP32)
+    e0 = d.energy()
+    d.run_until(0.125)
+    st = d.state()
+    assert (st["t"] == 0.125).all() and np.all(np.fmod(st["t"], st["dt"]) == 0.0)
+    e1 = d.energy()
+    hist = d.history()
+    print(f"fp32 integrator: {d.stats()['block_steps']} block steps, n_i min/max {hist.min()}/{hist.max()}, dE/E {(e1 - e0) / e0:.2e}")
+    assert abs((e1 - e0) / e0) < 2e-5 and hist.min() < w.N // 8 and hist.max() == w.N
+    d.close()
