@@ -1077,6 +1077,12 @@ int run_force(s2_ctx *ctx, int ni, const int *d_i_addr, const double *d_h2, bool
         r.order = ctx->order;
         r.flags = flags;
         r.overflow_flag = (int *)ctx->flags.p;
+        ctx->bts_hook_done = false;
+        if (ctx->bts_hook && !ctx->in_selftest && !fixup && flags == 0 && !host_res && reduce_by_warp_kernel(r)) {
+            r.bts = *ctx->bts_hook;          // the integrator's corrector rides on the combine (fp32: the fix-up must run first)
+            r.has_bts = 1;
+            ctx->bts_hook_done = true;
+        }
         if (fixup && reduce_by_warp_kernel(r)) {   // reduce_kernel flags while it has the final sums at hand: no flag launch
             r.f32 = f32;
             r.f32.i_addr = a.i_addr;

@@ -58,6 +58,8 @@ struct s2_ctx {
     cudaEvent_t ev_il[2] = {nullptr, nullptr};
     int il_turn = 0;
     bool flags_dirty = false;         // a device-side commit may have raised the range flag
+    const BtsArgs *bts_hook = nullptr;   // set by s2_bts_run around run_force: corrector to apply inside reduce_kernel
+    bool bts_hook_done = false;       // run_force took the hook (the force call went through reduce_kernel)
     bool in_selftest = false;         // inside bank_selftest (run_force re-entered with a reduced problem)
     cudaEvent_t ev_stage = nullptr;   // H2D of the staging buffer finished
     cudaEvent_t ev_io = nullptr;      // H2D of the i-list upload finished

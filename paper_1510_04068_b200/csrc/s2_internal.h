@@ -125,6 +125,31 @@ struct ForceArgs {
     int bank_threads;              // threads per CTA of the chunk launches (128 or 256; 0: the policy's default)
 };
 
+// ---- block-time-step integrator (s2_bts.cu): state handed to its kernels ----------------------------------------
+struct BtsCtl {                      // device control block (also mirrored to pinned host memory by the select kernel)
+    double t_next;                   // time of the block step that is about to run
+    int n_next;                      // number of active particles of that step
+    int pad;
+};
+
+struct BtsArgs {
+    double *f[kMaxFields];           // base j-store fields (t, m, x, v, a, jerk [, snap, crackle])
+    double *dt;                      // [n] current step of every particle
+    double *pot;                     // [n] potential at the particle's last force evaluation
+    const double *rec;               // result records of the force call on the active list
+    int *ilist;                      // active list (addresses, ascending)
+    int *stage;                      // [n] per-block compaction staging of the select kernel
+    int *bcnt;                       // [nblocks] active particles found by each block
+    unsigned *arrive;                // arrival counter of the select kernel (zero between launches)
+    int *hist;                       // [kLevels] particles per step level
+    BtsCtl *ctl;                     // device control block
+    BtsCtl *h_ctl;                   // the same, in pinned host memory
+    int n, n_act, order;
+    double eta, eta_start, dt_max, dt_min;
+    double eta4;                     // 6th order, averaged criterion: eta of the 4th-order Aarseth step it is averaged with
+    int averaged;
+};
+
 // fp32 path, reading R-F32: what is needed to decide whether an i-particle's jerk is a strongly cancelling sum
 struct F32Flag {
     const float *wq;               // [nst][ni] sum of q^2 per (slice, i), or nullptr: no flagging
@@ -150,6 +175,8 @@ struct ReduceArgs {
     unsigned flags;
     int *overflow_flag;
     F32Flag f32;                   // fp32 contexts: flag ill-conditioned jerk sums while the final sums are at hand (wq != nullptr)
+    int has_bts;                   // block-step integrator: lane 0 applies the corrector to its particle right after the combine
+    BtsArgs bts;
 };
 
 // kernels' host-side launchers (each returns the cudaError_t of the launch)

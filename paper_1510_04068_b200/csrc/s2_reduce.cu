@@ -13,6 +13,7 @@
 #include <math_constants.h>
 
 #include "s2_force_sweep.cuh"
+#include "s2_bts_correct.cuh"
 
 namespace s2 {
 
@@ -33,6 +34,7 @@ __global__ void __launch_bounds__(256) reduce_kernel(const ReduceArgs a)
         else
             reduce_rows_warp<false>(a.part, a.out, a.jid_plane, i, a.ni, S, a.order, lane);
         if (a.f32.wq) fp32_flag_warp(a.f32, a.out, i, a.ni, lane);   // lane 0 reads back the record it has just written
+        if (a.has_bts && lane == 0) bts_correct_one(a.bts, i, a.out + (size_t)i * REC);   // integrator: corrector in the same launch
         return;
     }
 
