@@ -29,7 +29,10 @@ extern "C" {
  *   key 9: 1 = never use the zero-copy path of small host calls (n_i <= 128 with host arrays: the kernels read the
  *          i-list from, and write the final records to, pinned host memory, so no copy is enqueued),
  *          4 = S2_FP32 contexts: no fp64 re-evaluation of ill-conditioned i-particles (A/B of reading R-F32),
- *          5 = S2_FP32 contexts: re-evaluate EVERY i-particle in fp64 (tests of the fix-up kernels: the sums are then fp64-accurate) */
+ *          5 = S2_FP32 contexts: re-evaluate EVERY i-particle in fp64 (tests of the fix-up kernels: the sums are then fp64-accurate),
+ *          6 = block-step integrator: the small-step kernel is not used (every step through the ordinary force call, one
+ *              synchronisation per step; A/B of s2_bts_run)
+ *   key 10: block-step integrator: largest active set the small-step kernel takes (1 .. 1024; 0 = the default, 512) */
 int s2_set_tuning(s2_ctx *ctx, int key, int value);
 /* Shape of the last force launch: out[0]=S, [1]=lanes per i, [2]=warp columns, [3]=grid size,
  * [4]=threads per CTA, [5]=dynamic shared memory bytes, [6]=0 no combine needed / 1 reduce kernel ran /
@@ -70,6 +73,11 @@ int s2_get_csr_timing(s2_ctx *ctx, float *scan_ms, float *fill_ms);
 /* S2_FP32 contexts: number of i-particles of the last force call whose jerk sum was found ill-conditioned and that were
  * re-evaluated in fp64 (reading R-F32); 0 for other precisions.  SYNC. */
 int s2_fp32_fixup_count(s2_ctx *ctx, int *n);
+
+/* Block-step integrator (s2_bts_*, include/s2b200.h): how much of the run went through the small-step kernel -- its
+ * launches, the block steps they ran, and (runs with time_device != 0) their summed device time in milliseconds. */
+struct s2_bts;
+int s2_bts_small_stats(const struct s2_bts *b, long long *launches, long long *steps, double *device_ms);
 
 #ifdef __cplusplus
 }

@@ -90,6 +90,7 @@ def lib() -> C.CDLL:
         "s2_enable_timing": (C.c_int, [vp, C.c_int]),
         "s2_get_timing": (C.c_int, [vp, C.POINTER(C.c_float), C.POINTER(C.c_float), C.POINTER(C.c_float)]),
         "s2_fp32_fixup_count": (C.c_int, [vp, C.POINTER(C.c_int)]),
+        "s2_bts_small_stats": (C.c_int, [vp, C.POINTER(C.c_longlong), C.POINTER(C.c_longlong), C.POINTER(C.c_double)]),
         "s2_peak_fma": (C.c_int, [vp, C.c_int, C.c_int, C.POINTER(C.c_double)]),
         "s2_time_host_roundtrip": (C.c_int, [vp, C.c_int, C.POINTER(C.c_int), C.c_double, C.c_uint, C.c_int, C.POINTER(C.c_double)]),
         "s2_bts_open": (C.c_int, [C.POINTER(vp), vp, C.c_int] + [C.c_double] * 5 + [C.c_int, C.c_double]),
@@ -502,6 +503,12 @@ def s2_bts_stats(b) -> dict:
                               C.byref(ts)), "s2_bts_stats")
     return dict(time=tm.value, t_next=tn.value, n_next=nn.value, block_steps=bs.value, particle_steps=ps.value,
                 wall_ms=wall.value, device_ms=dev.value, timed_steps=ts.value)
+
+
+def s2_bts_small_stats(b) -> dict:
+    ln, st, ms = C.c_longlong(), C.c_longlong(), C.c_double()
+    _check(lib().s2_bts_small_stats(b.handle, C.byref(ln), C.byref(st), C.byref(ms)), "s2_bts_small_stats")
+    return dict(launches=ln.value, steps=st.value, device_ms=ms.value)
 
 
 def s2_bts_get_history(b, first: int = 0, count: int | None = None) -> np.ndarray:

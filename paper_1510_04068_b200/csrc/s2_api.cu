@@ -1539,7 +1539,7 @@ extern "C" int s2_get_j(s2_ctx *ctx, int first, int n, int *id, double *t, doubl
 
 extern "C" int s2_set_tuning(s2_ctx *ctx, int key, int value)
 {
-    if (!ctx || key < 0 || key > 9 || value < 0) return S2_EINVAL;
+    if (!ctx || key < 0 || key > 10 || value < 0) return S2_EINVAL;
     ctx->tune[key] = value;
     return S2_OK;
 }

@@ -23,9 +23,13 @@
 // against the oracle in lock-step with this one) and repeated at the kernels below.
 #include <math_constants.h>
 
+#include <string.h>
+
+#include <algorithm>
 #include <chrono>
 
 #include "s2_ctx.h"
+#include "../../include/s2b200_test.h"
 #include "s2_predict.cuh"
 #include "s2_bts_correct.cuh"
 
@@ -172,7 +176,13 @@ __global__ void bts_iota_kernel(int *p, int n)
 
 namespace s2 {
 cudaError_t launch_predict(const PredictArgs &a, cudaStream_t st);
+cudaError_t launch_bts_small_steps(const ForceArgs &a, const BtsArgs &b, const PredictArgs &pa, int device, int sm_count, cudaStream_t st);
 }
+
+// Small block steps (fp64 contexts): runs of steps with at most kSmallCap active particles are taken by ONE launch of
+// bts_small_steps_kernel (s2_force_fp64.cu), which sweeps, combines, corrects, selects and predicts step after step behind
+// grid barriers and returns at the first step that does not qualify; the host then runs that step the ordinary way.
+constexpr int kSmallCapDefault = 512;
 
 template <class K, class A, class... R>
 static cudaError_t launch_pdl(K kern, dim3 grid, dim3 block, cudaStream_t st, const A &a, R... rest)
@@ -191,13 +201,16 @@ struct s2_bts {
     int n = 0;
     double eps2 = 0, eta = 0, eta_start = 0, dt_max = 0, dt_min = 0, eta4 = 0;
     int averaged = 0;
-    Buf dt, pot, ilist, stage, bcnt, misc;    // misc: {BtsCtl ctl; unsigned arrive; int hist[64]}
+    Buf dt, pot, ilist, stage, bcnt, misc;    // misc: {BtsCtl ctl (256 B); unsigned arrive (64 B); int hist[64]; unsigned bar[2] (64 B)}
     BtsCtl *h_ctl = nullptr;                  // pinned
+    int *h_log = nullptr;                     // pinned, kBtsLog entries: active counts of the steps of one small-step launch
     bool ready = false;
     double time = 0.0;
     long long block_steps = 0, particle_steps = 0;
     double device_ms = 0.0, wall_ms = 0.0;
     long long timed_steps = 0;
+    long long small_launches = 0, small_steps = 0;   // through bts_small_steps_kernel
+    double small_device_ms = 0.0;
     std::vector<int> hist_ni;
     cudaEvent_t ev[2] = {nullptr, nullptr};
 };
@@ -214,8 +227,11 @@ static BtsArgs bts_args(s2_bts *b)
     a.stage = (int *)b->stage.p;
     a.bcnt = (int *)b->bcnt.p;
     a.ctl = (BtsCtl *)b->misc.p;
-    a.arrive = (unsigned *)((char *)b->misc.p + 32);
-    a.hist = (int *)((char *)b->misc.p + 64);
+    static_assert(sizeof(BtsCtl) <= 256, "control block outgrew its slot");
+    a.arrive = (unsigned *)((char *)b->misc.p + 256);     // misc: {BtsCtl (256 B slot); unsigned arrive (64 B slot); int hist[64]}
+    a.hist = (int *)((char *)b->misc.p + 320);
+    a.bar = (unsigned *)((char *)b->misc.p + 576);
+    a.h_log = b->h_log;
     a.h_ctl = b->h_ctl;
     a.n = b->n;
     a.order = ctx->order;
@@ -258,10 +274,11 @@ static int bts_select_predict(s2_bts *b, double t_now, bool host_time)
 {
     s2_ctx *ctx = b->ctx;
     const int nb = (b->n + kSelPerBlock - 1) / kSelPerBlock;
+    BtsArgs a = bts_args(b);
     if (ctx->order == 6)
-        CU(launch_pdl(bts_select_predict_kernel<6>, dim3(nb), dim3(kSelThreads), ctx->stream, bts_args(b), bts_predict_args(b), t_now, host_time ? 1 : 0));
+        CU(launch_pdl(bts_select_predict_kernel<6>, dim3(nb), dim3(kSelThreads), ctx->stream, a, bts_predict_args(b), t_now, host_time ? 1 : 0));
     else
-        CU(launch_pdl(bts_select_predict_kernel<4>, dim3(nb), dim3(kSelThreads), ctx->stream, bts_args(b), bts_predict_args(b), t_now, host_time ? 1 : 0));
+        CU(launch_pdl(bts_select_predict_kernel<4>, dim3(nb), dim3(kSelThreads), ctx->stream, a, bts_predict_args(b), t_now, host_time ? 1 : 0));
     ctx->launches++;
     ctx->predicted = true;
     ctx->nj_pred = b->n;
@@ -290,10 +307,11 @@ extern "C" int s2_bts_open(s2_bts **out, s2_ctx *ctx, int n, double eps2, double
     if (rc == S2_OK) rc = dev_reserve(ctx, b->pot, (size_t)n * sizeof(double));
     if (rc == S2_OK) rc = dev_reserve(ctx, b->ilist, (size_t)n * sizeof(int));
     if (rc == S2_OK) rc = dev_reserve(ctx, b->stage, (size_t)nb * kSelPerBlock * sizeof(int));
-    if (rc == S2_OK) rc = dev_reserve(ctx, b->bcnt, (size_t)nb * sizeof(int));
-    if (rc == S2_OK) rc = dev_reserve(ctx, b->misc, 64 + kLevels * sizeof(int));
+    if (rc == S2_OK) rc = dev_reserve(ctx, b->bcnt, (size_t)std::max(nb, 1024) * sizeof(int));   // (the small-step kernel: one count per CTA)
+    if (rc == S2_OK) rc = dev_reserve(ctx, b->misc, 576 + 64);
     if (rc == S2_OK) {
         cudaError_t e = cudaHostAlloc((void **)&b->h_ctl, sizeof(BtsCtl), cudaHostAllocDefault);
+        if (e == cudaSuccess) e = cudaHostAlloc((void **)&b->h_log, kBtsLog * sizeof(int), cudaHostAllocDefault);
         if (e == cudaSuccess) e = cudaEventCreate(&b->ev[0]);
         if (e == cudaSuccess) e = cudaEventCreate(&b->ev[1]);
         if (e != cudaSuccess) rc = fail_cuda(ctx, e);
@@ -314,6 +332,7 @@ extern "C" int s2_bts_close(s2_bts *b)
     cudaStreamSynchronize(ctx->stream);
     for (Buf *q : {&b->dt, &b->pot, &b->ilist, &b->stage, &b->bcnt, &b->misc}) dev_release(ctx, *q);
     if (b->h_ctl) cudaFreeHost(b->h_ctl);
+    if (b->h_log) cudaFreeHost(b->h_log);
     for (auto &e : b->ev)
         if (e) cudaEventDestroy(e);
     delete b;
@@ -347,8 +366,11 @@ extern "C" int s2_bts_init(s2_bts *b, const double *mass, const double *pos, con
         CU(cudaGetLastError());
         ctx->launches += 1;
     }
+    memset(b->h_ctl, 0, sizeof(BtsCtl));
     b->time = 0.0;
     b->block_steps = b->particle_steps = 0;
+    b->small_launches = b->small_steps = 0;
+    b->small_device_ms = 0.0;
     b->hist_ni.clear();
     rc = bts_select_predict(b, 0.0, true);
     if (rc != S2_OK) return rc;
@@ -372,11 +394,67 @@ extern "C" int s2_bts_run(s2_bts *b, double t_end, long long max_block_steps, in
     // ordinary calls on the context since the last run (an energy evaluation, say) may have re-predicted the j-store
     // to another time: predict to the pending block time again (one launch per s2_bts_run, not per step)
     if (int rc = bts_predict_dev_time(b); rc != S2_OK) return rc;
+    // the small-step kernel computes in fp64 pair arithmetic: fp64 contexts only (s2_set_tuning key 9 = 6 switches it off)
+    bool small_ok = ctx->precision == S2_FP64 && ctx->tune[9] != 6;
+    ForceArgs small{};
+    double *small_part = nullptr;
+    const int kSmallCap = ctx->tune[10] > 0 ? std::min(ctx->tune[10], 1024) : kSmallCapDefault;
+    if (small_ok) {
+        const int np = nplanes(ctx->order), nc = ctx->order == 6 ? 10 : 7;
+        for (int k = 0; k < np; ++k) small.jp[k] = plane(ctx, k);
+        small.nj = b->n;
+        small.eps2 = b->eps2;
+        small.order = ctx->order;
+        if (int rc = dev_reserve(ctx, ctx->fixpart, (size_t)ctx->sm_count * kSmallCap * nc * sizeof(double)); rc != S2_OK) return rc;
+        small_part = (double *)ctx->fixpart.p;
+    }
     while (done < max_block_steps && b->h_ctl->t_next <= t_end) {
         const double t_new = b->h_ctl->t_next;
         const int n_act = b->h_ctl->n_next;
         if (n_act <= 0 || n_act > b->n) return S2_ESTATE;
-        // the j-particles were already predicted to t_new (enqueued behind the previous select)
+        // the j-particles were already predicted to t_new (by the previous select, or by the small-step kernel)
+        if (small_ok && n_act <= kSmallCap) {
+            const int K = (int)std::min<long long>(kBtsLog, max_block_steps - done);
+            const long long steps0 = b->h_ctl->steps;
+            BtsArgs a = bts_args(b);
+            a.spec_cap = kSmallCap;
+            a.max_steps = K;
+            a.t_end = t_end;
+            a.part = small_part;
+            if (time_device) CU(cudaEventRecord(b->ev[0], ctx->stream));
+            const cudaError_t e = launch_bts_small_steps(small, a, bts_predict_args(b), ctx->device, ctx->sm_count, ctx->stream);
+            if (e == cudaErrorNotSupported) {            // this device cannot run it: every step the ordinary way
+                cudaGetLastError();
+                small_ok = false;
+                continue;
+            }
+            CU(e);
+            ctx->launches++;
+            if (time_device) CU(cudaEventRecord(b->ev[1], ctx->stream));
+            CU(cudaStreamSynchronize(ctx->stream));      // one synchronisation per run of small steps
+            const int ran = (int)(b->h_ctl->steps - steps0);
+            if (b->h_ctl->error || ran < 1 || ran > K) return S2_ESTATE;   // (the first step of a launch always qualifies)
+            if (time_device) {
+                float ms = 0.f;
+                CU(cudaEventElapsedTime(&ms, b->ev[0], b->ev[1]));
+                b->device_ms += ms;
+                b->small_device_ms += ms;
+                b->timed_steps += ran;
+            }
+            for (int k = 0; k < ran; ++k) {
+                b->particle_steps += b->h_log[k];
+                b->hist_ni.push_back(b->h_log[k]);
+            }
+            b->time = b->h_ctl->t_done;
+            b->block_steps += ran;
+            b->small_steps += ran;
+            b->small_launches++;
+            done += ran;
+            ctx->predicted = true;
+            ctx->nj_pred = b->n;
+            ctx->calc_done = false;
+            continue;
+        }
         if (time_device) CU(cudaEventRecord(b->ev[0], ctx->stream));
         BtsArgs a = bts_args(b);
         a.n_act = n_act;
@@ -452,6 +530,15 @@ extern "C" int s2_bts_stats(const s2_bts *b, double *time, double *t_next, int *
     if (wall_ms) *wall_ms = b->wall_ms;
     if (device_ms) *device_ms = b->device_ms;
     if (timed_steps) *timed_steps = b->timed_steps;
+    return S2_OK;
+}
+
+extern "C" int s2_bts_small_stats(const s2_bts *b, long long *launches, long long *steps, double *device_ms)
+{
+    if (!b) return S2_EINVAL;
+    if (launches) *launches = b->small_launches;
+    if (steps) *steps = b->small_steps;
+    if (device_ms) *device_ms = b->small_device_ms;
     return S2_OK;
 }
 

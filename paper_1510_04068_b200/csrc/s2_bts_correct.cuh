@@ -38,12 +38,11 @@ __device__ __forceinline__ double next_step(double raw, double old, double t_new
 //   F5 = (S- - 3 J+ + 3 A-)/16, F4 = (S+ - J-)/16, F3 = (5 J+ - 5 A- - S-)/8
 //   a3 = 6 (F3 + 4 F4 + 10 F5)/h^3 (stored as crackle), a4 = 24 (F4 + 5 F5)/h^4, a5 = 120 F5/h^5
 //   dt' = eta (A1 / A4)^(1/3),  A1 = sqrt(|a1||s1| + |j1|^2),  A4 = sqrt(|a3||a5| + |a4|^2)
-// k: position in the active list; r: the final force record of that particle.  Reads the particle's old state from the
+// k: position in the active list (bts_correct_one); r: the final force record of that particle.  Reads the particle's old state from the
 // base j-store, writes the corrected state, its time and its new step in place, and keeps the step-level histogram.
-__device__ __forceinline__ void bts_correct_one(const BtsArgs &a, int k, const double *r)
+// i: address of the particle; t_new: the block time it is corrected to (bts_correct_one below looks both up)
+__device__ __forceinline__ void bts_correct_particle(const BtsArgs &a, int i, double t_new, const double *r)
 {
-    const int i = a.ilist[k];
-    const double t_new = a.ctl->t_next;
     const double dt = a.dt[i];
     double x0[3], v0[3], a0[3], j0[3], a1[3], j1[3], x1[3], v1[3];
 #pragma unroll
@@ -107,6 +106,11 @@ __device__ __forceinline__ void bts_correct_one(const BtsArgs &a, int k, const d
         atomicSub(&a.hist[level_of(dt)], 1);     // integer atomics: the histogram does not depend on their order
         atomicAdd(&a.hist[level_of(nw)], 1);
     }
+}
+
+__device__ __forceinline__ void bts_correct_one(const BtsArgs &a, int k, const double *r)
+{
+    bts_correct_particle(a, a.ilist[k], a.ctl->t_next, r);
 }
 
 }  // namespace s2

@@ -73,7 +73,7 @@ struct s2_ctx {
     double t_pred = 0.0;
 
     // tuning overrides and last launch
-    int tune[10] = {0, 0, 0, 0, 0, 0, 0, 0, 0, 0};
+    int tune[11] = {0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0};
     int last_info[10] = {0, 0, 0, 0, 0, 0, 0, 0, 1, 1};
     std::map<long long, int> occ_cache;
     std::map<long long, std::pair<ForceShape, int>> shape_cache;

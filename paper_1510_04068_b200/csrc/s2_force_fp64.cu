@@ -11,6 +11,8 @@
 #include <algorithm>
 
 #include "s2_force_sweep.cuh"
+#include "s2_predict.cuh"
+#include "s2_bts_correct.cuh"
 
 namespace s2 {
 
@@ -399,6 +401,271 @@ cudaError_t launch_fp32_fix(const ForceArgs &a, int sm_count, cudaStream_t st)
     return e;
 }
 
+
+// ---- small block steps of the integrator, many per launch (s2_bts.cu; sec 3.7) ---------------
+// In a block-step run most steps move a handful of particles (median 4-10 of 16384): three dependent launches and a host
+// synchronisation per step cost 30 us for 1 us of arithmetic.  This kernel runs such steps back to back WITHOUT leaving
+// the GPU: one CTA per SM (cooperative launch: all co-resident), three grid barriers per step,
+//   phase 1  sweep: CTA c holds the j-particles [c jc, (c+1) jc).  One lane per active particle (32 to a warp, its state
+//            in registers), the CTA's j-range cut into as many splits as there are warps to spare; every lane of a warp
+//            reads the same j (one broadcast load from L2).  The splits are added in order through shared memory and
+//            the CTA writes one partial row per active particle;                                           | barrier
+//   phase 2  combine + corrector: active particle k belongs to CTA k mod G; a warp adds one component of the G rows
+//            (lane l takes rows l, l + 32, ... in that order, then the xor-butterfly), then one thread per particle
+//            applies the Hermite corrector and the time-step rule in place (bts_correct_particle) and keeps the
+//            step-level histogram;                                                                         | barrier
+//   phase 3  next block time from the histogram, prediction of every particle to it, each CTA compacts the active
+//            particles of its own address range (ascending) and publishes their number;                   | barrier
+//            then every CTA scans the G counts, copies its segment to the global list and, if the next step is a small
+//            one as well, gathers the (ascending) list into its shared memory.
+// The loop ends at the first step with more than b.spec_cap active particles or past b.t_end, or after b.max_steps; the
+// control block, the list and the predicted j-store are then exactly what an ordinary step of s2_bts_run expects.
+// Every sum is taken in a fixed order: the run is bit-reproducible.  Pair arithmetic: PolicyF64::interact above.
+constexpr int kSmallThreads = 512, kSmallWarps = kSmallThreads / 32;
+constexpr int kSmallRows = 32 * kSmallWarps;   // (particle, j-split) rows in shared memory per round of the sweep
+constexpr int kSmallCapMax = 1024;    // largest spec_cap (the list in shared memory)
+constexpr int kSmallMaxCtas = 256;    // the count scan takes one CTA per thread; rows per lane in the combine = 256 / 32
+constexpr int kSmallPer = 8;          // particles a CTA combines per round
+
+// Barrier over the whole (co-resident) grid.  Arrival is a release-add (this CTA's writes of the phase are visible
+// before it counts), the wait polls with relaxed loads and ends with one acquire fence (which also drops the SM's L1
+// lines: what other CTAs wrote is then read from L2).  The counter only grows during a launch (target = barriers so
+// far x CTAs).  A wait of more than 2^24 polls (seconds; a phase takes microseconds) gives up and reports it rather
+// than hanging the GPU.
+__device__ __forceinline__ bool grid_barrier(unsigned *bar, unsigned target, int *s_flag)
+{
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        asm volatile("red.release.gpu.global.add.u32 [%0], %1;" ::"l"(bar), "r"(1u) : "memory");
+        unsigned spins = 0, v;
+        int ok = 1;
+        for (;;) {
+            asm volatile("ld.relaxed.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(bar) : "memory");
+            if (v >= target) break;
+            if (++spins > (1u << 24)) { ok = 0; break; }
+        }
+        asm volatile("fence.acq_rel.gpu;" ::: "memory");
+        *s_flag = ok;
+    }
+    __syncthreads();
+    return *s_flag != 0;
+}
+
+template <int ORDER>
+__global__ void __launch_bounds__(kSmallThreads, 1) bts_small_steps_kernel(const ForceArgs a, const BtsArgs b, const PredictArgs pa)
+{
+    using P = PolicyF64<ORDER, false, false>;
+    constexpr int NC = ORDER == 6 ? 10 : 7;
+    __shared__ double s_part[NC][kSmallRows];                     // component-major: lanes write neighbouring words
+    __shared__ int s_list[kSmallCapMax];
+    __shared__ int s_off[kSmallMaxCtas + 1];
+    __shared__ int s_w[kSmallWarps];
+    __shared__ unsigned s_hist[2];
+    __shared__ int s_flag;
+    __shared__ double s_r[kSmallPer][12];
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int cta = blockIdx.x, G = gridDim.x;
+    const int N = b.n, cap = b.spec_cap;
+    const int jc = (N + G - 1) / G;                               // j-particles of this CTA in the sweep
+    const int jbeg = min(N, cta * jc), jend = min(N, jbeg + jc);
+    const int pc = (jc + 31) & ~31;                               // particles of this CTA in select + predict: whole warps
+    const int pbeg = (int)min((long long)N, (long long)cta * pc), pend = min(N, pbeg + pc);
+    Decomp d{};
+    Dec D{};
+
+    double t_cur = b.ctl->t_next, t_done = b.ctl->t_done;
+    int n = b.ctl->n_next, step = 0;
+    unsigned target = 0;
+    bool ok = true;
+    if (n <= cap)
+        for (int k = tid; k < n; k += kSmallThreads) s_list[k] = b.ilist[k];
+    __syncthreads();
+
+    while (n >= 1 && n <= cap && t_cur <= b.t_end && step < b.max_steps) {
+        // ---- phase 1: sweep -------------------------------------------------------------------------------------
+        const int ng = (n + 31) >> 5;                             // groups of 32 active particles
+        for (int g0 = 0; g0 < ng; g0 += kSmallWarps) {            // (one round unless n > 512)
+            const int ngr = min(kSmallWarps, ng - g0);
+            const int js = kSmallWarps / ngr;                     // j-splits of this CTA's range: every warp gets an item
+            if (warp < ngr * js) {
+                const int gl = warp / js, sp = warp - gl * js;    // neighbouring warps: same particles, next split
+                const int i = s_list[min((g0 + gl) * 32 + lane, n - 1)];   // (idle lanes recompute the last particle)
+                typename P::IState I;
+                {
+                    const double2 p0 = __ldcg(static_cast<const double2 *>(a.jp[0]) + i), p1 = __ldcg(static_cast<const double2 *>(a.jp[1]) + i);
+                    const double2 p2 = __ldcg(static_cast<const double2 *>(a.jp[2]) + i), p3 = __ldcg(static_cast<const double2 *>(a.jp[3]) + i);
+                    I.x = p0.x; I.y = p0.y; I.z = p1.x; I.vx = p2.x; I.vy = p2.y; I.vz = p3.x;
+                    I.id = __double2loint(p3.y);
+                    I.ax = I.ay = I.az = 0.0;
+                    if (ORDER == 6) {
+                        const double2 p4 = __ldcg(static_cast<const double2 *>(a.jp[4]) + i), p5 = __ldcg(static_cast<const double2 *>(a.jp[5]) + i);
+                        I.ax = p4.x; I.ay = p4.y; I.az = p5.x;
+                    }
+                    I.h2 = 0.0;
+                    I.eps2 = a.eps2;
+                }
+                typename P::Acc A;
+                A.zero();
+                const int len = (jend - jbeg + js - 1) / js;
+                const int j0 = jbeg + sp * len, j1 = min(jend, j0 + len);
+#pragma unroll 4
+                for (int j = j0; j < j1; ++j) {                   // the same j in every lane: broadcast loads
+                    typename P::JData J;
+                    J.p0 = __ldcg(static_cast<const double2 *>(a.jp[0]) + j); J.p1 = __ldcg(static_cast<const double2 *>(a.jp[1]) + j);
+                    J.p2 = __ldcg(static_cast<const double2 *>(a.jp[2]) + j); J.p3 = __ldcg(static_cast<const double2 *>(a.jp[3]) + j);
+                    if (ORDER == 6) {
+                        J.p4 = __ldcg(static_cast<const double2 *>(a.jp[4]) + j); J.p5 = __ldcg(static_cast<const double2 *>(a.jp[5]) + j);
+                    }
+                    P::template interact<1, false>(J, true, j, I, A, D, d, nullptr, 0);
+                }
+                double out[10];
+                A.to_f64(out);
+                const int row = (sp * ngr + gl) * 32 + lane;
+#pragma unroll
+                for (int c = 0; c < NC; ++c) s_part[c][row] = out[c];
+            }
+            __syncthreads();
+            const int nk = min(ngr * 32, n - g0 * 32);            // particles of this round
+            for (int e = tid; e < nk * NC; e += kSmallThreads) {  // this CTA's row of each: the splits in order
+                const int c = e / nk, kl = e - c * nk;
+                double v = 0.0;
+                for (int sp = 0; sp < js; ++sp) v += s_part[c][sp * ngr * 32 + kl];
+                b.part[((size_t)cta * cap + g0 * 32 + kl) * NC + c] = v;
+            }
+            __syncthreads();
+        }
+        if (!(ok = grid_barrier(b.bar, target += G, &s_flag))) break;
+
+        // ---- phase 2: combine + corrector ----------------------------------------------------------------------
+        const int mine = n > cta ? (n - cta + G - 1) / G : 0;     // this CTA's particles: k = cta + m G
+        for (int m0 = 0; m0 < mine; m0 += kSmallPer) {
+            const int mr = min(kSmallPer, mine - m0);
+            for (int it = warp; it < mr * NC; it += kSmallWarps) {
+                const int m = it / NC, c = it - m * NC, k = cta + (m0 + m) * G;
+                double x[kSmallMaxCtas / 32];
+#pragma unroll
+                for (int u = 0; u < kSmallMaxCtas / 32; ++u) {    // all loads in flight, then added in row order
+                    const int row = lane + 32 * u;
+                    x[u] = row < G ? __ldcg(b.part + ((size_t)row * cap + k) * NC + c) : 0.0;
+                }
+                double v = x[0];
+#pragma unroll
+                for (int u = 1; u < kSmallMaxCtas / 32; ++u) v += x[u];
+#pragma unroll
+                for (int q = 1; q < 32; q <<= 1) v += shfl_xor_d(v, q);
+                if (lane == 0) s_r[m][c < 7 ? c : c + 2] = v;     // record layout: acc, jerk, pot at 0..6, snap at 9..11
+            }
+            __syncthreads();
+            if (tid < mr) bts_correct_particle(b, s_list[cta + (m0 + tid) * G], t_cur, s_r[tid]);
+            __syncthreads();
+        }
+        if (!(ok = grid_barrier(b.bar, target += G, &s_flag))) break;
+
+        // ---- phase 3: next block time, prediction, this CTA's share of the next active list -----------------------
+        if (tid < 64) {
+            const unsigned bal = __ballot_sync(0xffffffffu, __ldcg(b.hist + tid) > 0);
+            if (lane == 0) s_hist[warp] = bal;
+        }
+        __syncthreads();
+        const int lev = s_hist[1] ? 63 - __clz(s_hist[1]) : 31 - __clz(s_hist[0] | 1u);   // highest occupied level = smallest step
+        const double t_next = t_cur + scalbn(1.0, -lev);
+        int cnt = 0;
+        for (int base = pbeg; base < pend; base += kSmallThreads) {
+            const int i = base + tid;
+            bool act = false;
+            if (i < pend) {
+                const double x = t_next / __ldcg(b.dt + i);       // exact: dt is a power of two
+                act = x == floor(x);
+                predict_one<ORDER>(pa, i, t_next);
+            }
+            const unsigned bal = __ballot_sync(0xffffffffu, act);
+            if (lane == 0) s_w[warp] = __popc(bal);
+            __syncthreads();
+            int pos = cnt + __popc(bal & ((1u << lane) - 1u)), total = 0;
+#pragma unroll
+            for (int w = 0; w < kSmallWarps; ++w) {
+                if (w < warp) pos += s_w[w];
+                total += s_w[w];
+            }
+            if (act) b.stage[pbeg + pos] = i;
+            cnt += total;
+            __syncthreads();
+        }
+        if (tid == 0) b.bcnt[cta] = cnt;
+        if (!(ok = grid_barrier(b.bar, target += G, &s_flag))) break;
+
+        // ---- every CTA: scan of the G counts, own segment to the global list, the next list if it is a small one ------
+        {
+            const int c = tid < G ? __ldcg(b.bcnt + tid) : 0;
+            int incl = c;
+#pragma unroll
+            for (int q = 1; q < 32; q <<= 1) {
+                const int o = __shfl_up_sync(0xffffffffu, incl, q);
+                if (lane >= q) incl += o;
+            }
+            if (lane == 31) s_w[warp] = incl;
+            __syncthreads();
+            int wb = 0;
+            for (int w = 0; w < warp; ++w) wb += s_w[w];
+            if (tid < G) s_off[tid] = wb + incl - c;
+            if (tid == G - 1) s_off[G] = wb + incl;
+            __syncthreads();
+        }
+        const int n_next = s_off[G];
+        for (int k = tid; k < cnt; k += kSmallThreads) b.ilist[s_off[cta] + k] = b.stage[pbeg + k];
+        if (n_next <= cap) {
+            for (int k = tid; k < n_next; k += kSmallThreads) {
+                int lo = 0, hi = G - 1;                           // CTA of member k: last c with s_off[c] <= k
+                while (lo < hi) {
+                    const int mid = (lo + hi + 1) >> 1;
+                    if (s_off[mid] <= k) lo = mid; else hi = mid - 1;
+                }
+                s_list[k] = __ldcg(b.stage + (size_t)lo * pc + (k - s_off[lo]));
+            }
+        }
+        if (cta == 0 && tid == 0) b.h_log[step] = n;
+        t_done = t_cur;
+        t_cur = t_next;
+        n = n_next;
+        ++step;
+        __syncthreads();
+    }
+
+    if (cta == 0 && tid == 0) {
+        BtsCtl c = *b.ctl;
+        c.t_next = t_cur; c.n_next = n; c.steps += step; c.t_done = t_done;
+        if (!ok) c.error = 1;
+        *b.ctl = c;
+        *b.h_ctl = c;
+    }
+    if (ok) {                                                     // the last CTA out leaves the counters at zero for the next launch
+        __syncthreads();
+        if (tid == 0 && atomicAdd(b.bar + 1, 1u) == (unsigned)G - 1u) {
+            b.bar[0] = 0u;
+            b.bar[1] = 0u;
+        }
+    }
+}
+
+// Launch of the above on the whole chip; a.jp = the fp64 planes, b.spec_cap <= kSmallCapMax, b.part holds
+// sm_count * spec_cap * (7 | 10) doubles.  Returns cudaErrorNotSupported when the device cannot run it (no cooperative
+// launch, or more SMs than the count scan takes): the caller then steps the ordinary way.
+cudaError_t launch_bts_small_steps(const ForceArgs &a, const BtsArgs &b, const PredictArgs &pa, int device, int sm_count, cudaStream_t st)
+{
+    static int supported[64] = {};                                // per device: 0 unknown, 1 yes, -1 no
+    if (device < 0 || device >= 64 || b.spec_cap < 1 || b.spec_cap > kSmallCapMax || sm_count > kSmallMaxCtas) return cudaErrorNotSupported;
+    const void *kern = a.order == 6 ? (const void *)bts_small_steps_kernel<6> : (const void *)bts_small_steps_kernel<4>;
+    if (supported[device] == 0) {
+        int coop = 0, per_sm = 0;
+        cudaError_t e = cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, device);
+        if (e == cudaSuccess) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, bts_small_steps_kernel<6>, kSmallThreads, 0);
+        if (e != cudaSuccess) return e;
+        supported[device] = (coop && per_sm >= 1) ? 1 : -1;
+    }
+    if (supported[device] < 0) return cudaErrorNotSupported;
+    void *args[3] = {(void *)&a, (void *)&b, (void *)&pa};
+    return cudaLaunchCooperativeKernel(kern, dim3(sm_count), dim3(kSmallThreads), args, 0, st);
+}
 #endif   // S2_BANK_ONLY
 
 // ---- uniform-operand sweep (a4 at the largest n_i) ------------------------------------------------------------

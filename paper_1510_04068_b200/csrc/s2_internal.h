@@ -126,10 +126,13 @@ struct ForceArgs {
 };
 
 // ---- block-time-step integrator (s2_bts.cu): state handed to its kernels ----------------------------------------
-struct BtsCtl {                      // device control block (also mirrored to pinned host memory by the select kernel)
+constexpr int kBtsLog = 1024;        // block steps one launch of the small-step kernel may run (entries of its pinned log)
+struct BtsCtl {                      // device control block (mirrored to pinned host memory by the kernels that change it)
     double t_next;                   // time of the block step that is about to run
     int n_next;                      // number of active particles of that step
-    int pad;
+    int error;                       // != 0: a grid barrier of the small-step kernel timed out (state is then undefined)
+    long long steps;                 // block steps completed since s2_bts_init
+    double t_done;                   // time of the last completed block step
 };
 
 struct BtsArgs {
@@ -148,6 +151,13 @@ struct BtsArgs {
     double eta, eta_start, dt_max, dt_min;
     double eta4;                     // 6th order, averaged criterion: eta of the 4th-order Aarseth step it is averaged with
     int averaged;
+    // small-step kernel (bts_small_steps_kernel, s2_force_fp64.cu): runs block steps of at most spec_cap active particles
+    // that lie at or before t_end, at most max_steps of them, and logs each step's active count to pinned h_log
+    int spec_cap, max_steps;
+    double t_end;
+    int *h_log;                      // pinned, kBtsLog entries
+    double *part;                    // partial sums, [CTA][spec_cap][7 or 10]
+    unsigned *bar;                   // bar[0] grid-barrier counter, bar[1] exit counter; both 0 between launches
 };
 
 // fp32 path, reading R-F32: what is needed to decide whether an i-particle's jerk is a strongly cancelling sum

@@ -254,7 +254,9 @@ class DeviceHermite:
         return self.s2.s2_bts_get_state(self.bts)
 
     def stats(self) -> dict:
-        return self.s2.s2_bts_stats(self.bts)
+        st = self.s2.s2_bts_stats(self.bts)
+        st["small"] = self.s2.s2_bts_small_stats(self.bts)   # the share taken by the small-step kernel
+        return st
 
     def history(self) -> np.ndarray:
         return self.s2.s2_bts_get_history(self.bts)

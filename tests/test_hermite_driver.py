@@ -164,3 +164,42 @@ def test_device_integrator_in_fp32_runs_and_conserves_energy():
     print(f"fp32 integrator: {d.stats()['block_steps']} block steps, n_i min/max {hist.min()}/{hist.max()}, dE/E {(e1 - e0) / e0:.2e}")
     assert abs((e1 - e0) / e0) < 2e-5 and hist.min() < w.N // 8 and hist.max() == w.N
     d.close()
+
+
+@pytest.mark.gpu
+@pytest.mark.parametrize("order", [4, 6])
+def test_small_step_kernel_reproduces_the_step_by_step_run(order):
+    """s2_bts_run hands runs of small block steps (<= 512 active particles) to ONE launch of bts_small_steps_kernel, which
+    sweeps, combines, corrects, selects and predicts step after step behind grid barriers and returns at the first step
+    that does not qualify.  The run must be the same run as with one synchronised force call per step (s2_set_tuning
+    key 9 = 6): same block times and active counts step by step, same final t and dt arrays, positions equal to rounding
+    (the kernel adds the j-ranges of the CTAs in another order than the force call adds its j-slices)."""
+    import paper_1510_04068_b200 as s2
+    from paper_1510_04068_b200.hermite import DeviceHermite
+    w = make_config(3, N=2048)
+    runs = {}
+    for mode in ("small", "small cap 48", "stepwise"):
+        d = DeviceHermite(w.mass, w.pos, w.vel, w.eps2, order=order, averaged=order == 6)
+        if mode == "stepwise":
+            s2.s2_set_tuning(d.ctx, 9, 6)
+        elif mode == "small cap 48":
+            s2.s2_set_tuning(d.ctx, 10, 48)               # shorter runs: more hand-overs between the two kinds of step
+        d.run_until(0.0625)
+        d.run_until(0.125)                               # a second call continues the same run
+        runs[mode] = (d.state(), d.history(), d.stats())
+        d.close()
+    sb, hb, tb = runs["stepwise"]
+    assert tb["small"]["steps"] == 0
+    for mode in ("small", "small cap 48"):
+        sa, ha, ta = runs[mode]
+        cap = 48 if mode.endswith("48") else 512
+        assert np.array_equal(ha, hb), "active counts differ step by step"
+        assert ta["block_steps"] == tb["block_steps"] and ta["particle_steps"] == tb["particle_steps"] == int(ha.sum())
+        assert ta["time"] == tb["time"] == 0.125 and (sa["t"] == 0.125).all()
+        assert np.array_equal(sa["dt"], sb["dt"])
+        assert np.abs(sa["pos"] - sb["pos"]).max() < 1e-11 and np.abs(sa["vel"] - sb["vel"]).max() < 1e-10
+        # every step that qualifies went through the kernel except the first of each s2_bts_run call at most, the rest not
+        small = int((ha <= cap).sum())
+        assert small - 2 <= ta["small"]["steps"] <= small and ha.max() == w.N
+        print(f"order {order} {mode}: {ta['block_steps']} block steps, {ta['small']['steps']} in {ta['small']['launches']} launches; "
+              f"wall per step {ta['wall_ms'] / ta['block_steps'] * 1e3:.1f} us, stepwise {tb['wall_ms'] / tb['block_steps'] * 1e3:.1f} us")
