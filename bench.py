@@ -71,6 +71,8 @@ def parse_args():
     ap.add_argument("--bs-tend", type=float, default=1.0, help="end time of the --blockstep runs (N-body time units)")
     ap.add_argument("--bs-orders", default="4,6")
     ap.add_argument("--bs-precisions", default="fp64,ds")
+    ap.add_argument("--bs-profile-cta", type=int, default=0, help="CTA of the small-step kernel whose per-part cycle sums are reported")
+    ap.add_argument("--bs-no-host", action="store_true", help="skip the host reference driver rows of --blockstep")
     return ap.parse_args()
 
 
@@ -180,7 +182,7 @@ def main():
     if args.blockstep:
         if rank == 0:
             run_blockstep(args.blockstep, args.bs_tend, tuple(int(x) for x in args.bs_orders.split(",")),
-                          tuple(args.bs_precisions.split(",")))
+                          tuple(args.bs_precisions.split(",")), host_reference=not args.bs_no_host, prof_cta=args.bs_profile_cta)
         return
     if args.section == "fp32fix":
         if rank == 0:
@@ -405,7 +407,7 @@ def main():
         dist.destroy_process_group()
 
 
-def run_blockstep(n, t_end=1.0, orders=(4, 6), precisions=("fp64", "ds"), host_reference=True):
+def run_blockstep(n, t_end=1.0, orders=(4, 6), precisions=("fp64", "ds"), host_reference=True, prof_cta=0):
     """PAPER.md sec 3.7 (L152-L168), the second workload: block-time-step Hermite runs of an N-particle Plummer sphere
     for t_end N-body time units with the device-resident integrator (s2_bts_*), 4th order (eta = 0.01) and 6th order
     (eta = 0.1, the paper's scheme), fp64 and double-single.  Reports wall time per block step, the summed device time
@@ -431,14 +433,29 @@ def run_blockstep(n, t_end=1.0, orders=(4, 6), precisions=("fp64", "ds"), host_r
             d.close()
             # the same steps again, event-timed, for the summed device time (first 1/8 time unit)
             d = DeviceHermite(w.mass, w.pos, w.vel, w.eps2, order=order, precision=P[name], averaged=order == 6)
+            if name == "fp64":
+                s2.s2_bts_small_profile(d.bts, 1 + prof_cta)     # SM cycles one CTA spends in each part of a small step
             d.run_until(min(t_end, 0.125), time_device=True)
             sd = d.stats()
+            prof = None
+            if name == "fp64":
+                pr = s2.s2_bts_small_profile(d.bts, 0)
+                prof = {k: round(v / max(pr["steps"], 1)) for k, v in pr.items() if k != "steps"}
+                prof["sum"] = sum(prof.values())
             d.close()
             d = DeviceHermite(w.mass, w.pos, w.vel, w.eps2, order=order, precision=P[name], averaged=order == 6)
             t0 = time.perf_counter()
             d.run_until(min(t_end, 0.125))
             wall8 = time.perf_counter() - t0
             d.close()
+            ab = None
+            if name == "fp64":                       # A/B: the same first 1/8 without the small-step kernel (one force call per step)
+                d = DeviceHermite(w.mass, w.pos, w.vel, w.eps2, order=order, precision=P[name], averaged=order == 6)
+                s2.s2_set_tuning(d.ctx, 9, 6)
+                d.run_until(min(t_end, 0.125), time_device=True)
+                sa = d.stats()
+                d.close()
+                ab = {"device_us_per_block_step": sa["device_ms"] / sa["timed_steps"] * 1e3, "block_steps": sa["block_steps"]}
             row = {"integrator": "device (s2_bts)", "order": order, "criterion": "Aarseth" if order == 4 else "mean of Aarseth(eta4) and generalised(eta6) (L156)", "precision": name, "block_steps": st["block_steps"],
                    "particle_steps": st["particle_steps"], "n_i_min": int(hist.min()), "n_i_median": float(np.median(hist)),
                    "n_i_mean": float(hist.mean()), "n_i_max": int(hist.max()), "wall_s": wall,
@@ -446,9 +463,18 @@ def run_blockstep(n, t_end=1.0, orders=(4, 6), precisions=("fp64", "ds"), host_r
                    "ginteractions_per_s_wall": st["particle_steps"] * n / wall / 1e9, "dE_over_E": (e1 - e0) / e0,
                    "first_eighth": {"block_steps": sd["block_steps"], "wall_us_per_block_step": wall8 / sd["block_steps"] * 1e6,
                                     "device_us_per_block_step": sd["device_ms"] / sd["timed_steps"] * 1e3,
-                                    "wall_over_device": wall8 * 1e3 / sd["device_ms"]}}
+                                    "wall_over_device": wall8 * 1e3 / sd["device_ms"],
+                                    "small_step_kernel": {"steps": sd["small"]["steps"], "launches": sd["small"]["launches"],
+                                                          "device_us_per_step": sd["small"]["device_ms"] / max(sd["small"]["steps"], 1) * 1e3},
+                                    "small_step_cycles": prof, "small_step_cycles_cta": prof_cta, "one_force_call_per_step": ab}}
             out["runs"].append(row)
             print(json.dumps(row), file=sys.stderr, flush=True)
+    # the floor under a small step: SM cycles per round trip (two hops) of a word between SMs through L2
+    ctx = s2.s2_open(0, 4, s2.S2_FP64, nj_capacity=64, ngb_cap=0)
+    import torch
+    sms = torch.cuda.get_device_properties(0).multi_processor_count
+    out["hop_round_trip_cycles"] = {str(c): round(s2.s2_hop_latency(ctx, c, 2000)) for c in (2, 16, sms)}
+    s2.s2_close(ctx)
     if host_reference:
         for order, H in ((4, Hermite4), (6, Hermite6)):
             if order not in orders:

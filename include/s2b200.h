@@ -216,8 +216,11 @@ int s2_noalloc_limits(int *max_ni, long long *scratch_bytes);
  * from step to step.  Everything runs in kernels on the context's stream: the particle state is the context's own
  * j-store (the corrector updates it in place, so nothing is re-sent), the corrector and the time-step criterion
  * (Aarseth, L152: eta_4 = 0.01, eta_6 = 0.1), the choice of the next block time and the compaction of the next
- * active list.  Per block step the host reads back 12 bytes (next time, next active count) after one stream
- * synchronisation -- it needs the count to shape the next force launch.  paper_1510_04068_b200/hermite.py is the host
+ * active list.  Per ordinary block step the host reads back 12 bytes (next time, next active count) after one stream
+ * synchronisation -- it needs the count to shape the next force launch; in S2_FP64 contexts runs of small steps (at most
+ * 512 active particles, no more than 512 particles per SM) are taken by one cooperative launch that stays on the GPU
+ * from step to step, and the host synchronises once per run.  Both ways give the same run: same block times and active
+ * sets, states equal to rounding (the sums are taken in another order).  paper_1510_04068_b200/hermite.py is the host
  * reference driver of the same schemes (textbook formulas, refs [27] and [5]).
  * The integrator takes over the j-store of `ctx` (addresses 0 .. n-1, id == address); between s2_bts_run calls the
  * ordinary calls (s2_predict, s2_calc_*, s2_get_*) may be used on the same context, s2_set_j / s2_commit_j may not. */

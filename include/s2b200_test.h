@@ -60,6 +60,12 @@ int s2_time_host_roundtrip(s2_ctx *ctx, int ni, const int *i_address, double eps
  * Returns achieved lane-instructions per second in *fma_per_s.  SYNC. */
 int s2_peak_fma(s2_ctx *ctx, int kind, int iters, double *fma_per_s);
 
+/* Latency of an exchange between SMs through L2, the floor under the integrator's small-step kernel: CTA 0 stores a
+ * word, each of the other ctas - 1 CTAs (one per SM, 2 <= ctas <= SM count) polls it and answers in a word of its own,
+ * CTA 0 polls all answers; relaxed gpu-scope accesses, no fences.  Returns SM cycles (clock64) per round trip = two
+ * hops, averaged over iters.  SYNC. */
+int s2_hop_latency(s2_ctx *ctx, int ctas, int iters, double *cycles_per_round_trip);
+
 /* Test hook for the double-single arithmetic of the S2_DS path (reading P11): for k < n (host arrays) the operands
  * a[k], b[k] are split into (hi, lo) float pairs on the device and out[8k .. 8k+7] receives, as fp64,
  *   [0] the round trip of a   [1] a + b   [2] a - b (cancellation-safe form)   [3] a b   [4] a^2   [5] -3 a
@@ -78,6 +84,14 @@ int s2_fp32_fixup_count(s2_ctx *ctx, int *n);
  * launches, the block steps they ran, and (runs with time_device != 0) their summed device time in milliseconds. */
 struct s2_bts;
 int s2_bts_small_stats(const struct s2_bts *b, long long *launches, long long *steps, double *device_ms);
+/* Where a step of the small-step kernel spends its time, as seen by one CTA: with on = 1 + the CTA's index (CTA 0 combines
+ * and corrects the first active particle of every step, so it is on the critical path; CTAs beyond the active count only
+ * sweep and wait) the kernel adds up the SM cycles (clock64) between its marks into ten sums that out (may be NULL)
+ * receives -- [0] waiting for and scanning the owners' headers, [1] polling the records, [2] sweep, [3] adding the
+ * j-splits and writing the rows, [4] polling and adding the rows of all owners, [5] corrector, [6] the grid barrier,
+ * [7] histogram, reload, prediction, [8] publishing the next active set, [9] the number of steps.  Turning it on
+ * zeroes the sums; on = 0 turns it off; s2_bts_init leaves it off.  SYNC. */
+int s2_bts_small_profile(struct s2_bts *b, int on, long long out[10]);
 
 #ifdef __cplusplus
 }

@@ -91,7 +91,9 @@ def lib() -> C.CDLL:
         "s2_get_timing": (C.c_int, [vp, C.POINTER(C.c_float), C.POINTER(C.c_float), C.POINTER(C.c_float)]),
         "s2_fp32_fixup_count": (C.c_int, [vp, C.POINTER(C.c_int)]),
         "s2_bts_small_stats": (C.c_int, [vp, C.POINTER(C.c_longlong), C.POINTER(C.c_longlong), C.POINTER(C.c_double)]),
+        "s2_bts_small_profile": (C.c_int, [vp, C.c_int, C.POINTER(C.c_longlong)]),
         "s2_peak_fma": (C.c_int, [vp, C.c_int, C.c_int, C.POINTER(C.c_double)]),
+        "s2_hop_latency": (C.c_int, [vp, C.c_int, C.c_int, C.POINTER(C.c_double)]),
         "s2_time_host_roundtrip": (C.c_int, [vp, C.c_int, C.POINTER(C.c_int), C.c_double, C.c_uint, C.c_int, C.POINTER(C.c_double)]),
         "s2_bts_open": (C.c_int, [C.POINTER(vp), vp, C.c_int] + [C.c_double] * 5 + [C.c_int, C.c_double]),
         "s2_bts_close": (C.c_int, [vp]),
@@ -431,6 +433,12 @@ def s2_fp32_fixup_count(ctx) -> int:
     return n.value
 
 
+def s2_hop_latency(ctx, ctas: int, iters: int = 2000) -> float:
+    v = C.c_double()
+    _check(lib().s2_hop_latency(ctx.handle, int(ctas), int(iters), C.byref(v)), "s2_hop_latency", ctx.handle)
+    return v.value
+
+
 def s2_peak_fma(ctx, kind: int, iters: int = 2000) -> float:
     v = C.c_double()
     _check(lib().s2_peak_fma(ctx.handle, kind, iters, C.byref(v)), "s2_peak_fma", ctx.handle)
@@ -509,6 +517,19 @@ def s2_bts_small_stats(b) -> dict:
     ln, st, ms = C.c_longlong(), C.c_longlong(), C.c_double()
     _check(lib().s2_bts_small_stats(b.handle, C.byref(ln), C.byref(st), C.byref(ms)), "s2_bts_small_stats")
     return dict(launches=ln.value, steps=st.value, device_ms=ms.value)
+
+
+_SMALL_PARTS = ("headers", "records", "sweep", "rows_out", "rows_in", "corrector", "barrier", "predict", "publish")
+
+
+def s2_bts_small_profile(b, on: int = 1) -> dict:
+    """Switches the in-kernel profile of the small-step kernel on (1 + index of the CTA to watch) or off (0); returns the
+    sums so far (SM cycles per part)."""
+    out = (C.c_longlong * 10)()
+    _check(lib().s2_bts_small_profile(b.handle, int(on), out), "s2_bts_small_profile", b.ctx.handle)
+    d = {k: int(out[i]) for i, k in enumerate(_SMALL_PARTS)}
+    d["steps"] = int(out[9])
+    return d
 
 
 def s2_bts_get_history(b, first: int = 0, count: int | None = None) -> np.ndarray:

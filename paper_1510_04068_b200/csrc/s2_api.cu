@@ -1626,6 +1626,26 @@ extern "C" int s2_peak_fma(s2_ctx *ctx, int kind, int iters, double *fma_per_s)
     return S2_OK;
 }
 
+extern "C" int s2_hop_latency(s2_ctx *ctx, int ctas, int iters, double *cycles_per_round_trip)
+{
+    if (!ctx || !cycles_per_round_trip || iters <= 0 || ctas < 2 || ctas > ctx->sm_count) return S2_EINVAL;   // co-resident: one CTA per SM at most
+    CU(cudaSetDevice(ctx->device));
+    Buf tmp;
+    const size_t bytes = (size_t)(ctas + 2) * 128;
+    int rc = dev_reserve(ctx, tmp, bytes);
+    if (rc != S2_OK) return rc;
+    long long h = 0;
+    cudaError_t e = cudaMemsetAsync(tmp.p, 0, bytes, ctx->stream);
+    if (e == cudaSuccess) e = run_hop_latency(ctas, iters, (unsigned long long *)tmp.p + 16, (long long *)tmp.p, ctx->stream);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(&h, tmp.p, sizeof h, cudaMemcpyDeviceToHost, ctx->stream);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(ctx->stream);
+    ctx->launches++;
+    dev_release(ctx, tmp);
+    if (e != cudaSuccess) return fail_cuda(ctx, e);
+    *cycles_per_round_trip = (double)h / iters;
+    return S2_OK;
+}
+
 extern "C" int s2_test_ds_ops(s2_ctx *ctx, int n, const double *a, const double *b, double *out)
 {
     if (!ctx || n < 0 || (n > 0 && (!a || !b || !out))) return S2_EINVAL;

@@ -12,6 +12,12 @@
 //     bts_select_predict_kernel   next block time from the histogram, ordered compaction of the next active list,
 //                          prediction of every j to that time, {t_next, n_next} written to pinned host memory
 // and the host reads 12 bytes after one stream synchronisation (it needs n_next to shape the next sweep).
+// That is the ordinary step.  Most block steps, though, move a handful of particles, and three dependent launches plus a
+// synchronisation cost 30 us for a microsecond of arithmetic: in fp64 contexts, runs of steps with at most 512 active
+// particles are handed to ONE cooperative launch of bts_small_steps_kernel (s2_force_fp64.cu), which keeps every
+// particle's state in the shared memory of the SM that owns it and runs step after step without leaving the GPU; it
+// returns at the first step that does not qualify, with the control block, the list and the j-store as an ordinary step
+// expects them.  The host then synchronises once per run of small steps.
 //
 // Block time steps are powers of two and block-aligned (t_i is a multiple of dt_i), hence
 //     t_next = t_now + min_i dt_i        and        i is active at t_next  <=>  t_next is a multiple of dt_i,
@@ -201,6 +207,10 @@ struct s2_bts {
     int n = 0;
     double eps2 = 0, eta = 0, eta_start = 0, dt_max = 0, dt_min = 0, eta4 = 0;
     int averaged = 0;
+    Buf xrows, xrec, xhdr;                    // exchange buffers of the small-step kernel (BtsArgs), zero before its first launch
+    bool x_clean = false;
+    bool profile = false;                     // s2_bts_small_profile
+    int profile_cta = 0;
     Buf dt, pot, ilist, stage, bcnt, misc;    // misc: {BtsCtl ctl (256 B); unsigned arrive (64 B); int hist[64]; unsigned bar[2] (64 B)}
     BtsCtl *h_ctl = nullptr;                  // pinned
     int *h_log = nullptr;                     // pinned, kBtsLog entries: active counts of the steps of one small-step launch
@@ -232,6 +242,8 @@ static BtsArgs bts_args(s2_bts *b)
     a.hist = (int *)((char *)b->misc.p + 320);
     a.bar = (unsigned *)((char *)b->misc.p + 576);
     a.h_log = b->h_log;
+    a.prof = b->profile ? (long long *)((char *)b->misc.p + 640) : nullptr;
+    a.prof_cta = b->profile_cta;
     a.h_ctl = b->h_ctl;
     a.n = b->n;
     a.order = ctx->order;
@@ -308,7 +320,7 @@ extern "C" int s2_bts_open(s2_bts **out, s2_ctx *ctx, int n, double eps2, double
     if (rc == S2_OK) rc = dev_reserve(ctx, b->ilist, (size_t)n * sizeof(int));
     if (rc == S2_OK) rc = dev_reserve(ctx, b->stage, (size_t)nb * kSelPerBlock * sizeof(int));
     if (rc == S2_OK) rc = dev_reserve(ctx, b->bcnt, (size_t)std::max(nb, 1024) * sizeof(int));   // (the small-step kernel: one count per CTA)
-    if (rc == S2_OK) rc = dev_reserve(ctx, b->misc, 576 + 64);
+    if (rc == S2_OK) rc = dev_reserve(ctx, b->misc, 640 + 128);                  // (+ 10 profile sums at 640)
     if (rc == S2_OK) {
         cudaError_t e = cudaHostAlloc((void **)&b->h_ctl, sizeof(BtsCtl), cudaHostAllocDefault);
         if (e == cudaSuccess) e = cudaHostAlloc((void **)&b->h_log, kBtsLog * sizeof(int), cudaHostAllocDefault);
@@ -330,7 +342,7 @@ extern "C" int s2_bts_close(s2_bts *b)
     s2_ctx *ctx = b->ctx;
     cudaSetDevice(ctx->device);
     cudaStreamSynchronize(ctx->stream);
-    for (Buf *q : {&b->dt, &b->pot, &b->ilist, &b->stage, &b->bcnt, &b->misc}) dev_release(ctx, *q);
+    for (Buf *q : {&b->dt, &b->pot, &b->ilist, &b->stage, &b->bcnt, &b->misc, &b->xrows, &b->xrec, &b->xhdr}) dev_release(ctx, *q);
     if (b->h_ctl) cudaFreeHost(b->h_ctl);
     if (b->h_log) cudaFreeHost(b->h_log);
     for (auto &e : b->ev)
@@ -367,6 +379,8 @@ extern "C" int s2_bts_init(s2_bts *b, const double *mass, const double *pos, con
         ctx->launches += 1;
     }
     memset(b->h_ctl, 0, sizeof(BtsCtl));
+    b->profile = false;
+    b->x_clean = false;                      // the sequence tags start again: stale words must not match them
     b->time = 0.0;
     b->block_steps = b->particle_steps = 0;
     b->small_launches = b->small_steps = 0;
@@ -397,16 +411,29 @@ extern "C" int s2_bts_run(s2_bts *b, double t_end, long long max_block_steps, in
     // the small-step kernel computes in fp64 pair arithmetic: fp64 contexts only (s2_set_tuning key 9 = 6 switches it off)
     bool small_ok = ctx->precision == S2_FP64 && ctx->tune[9] != 6;
     ForceArgs small{};
-    double *small_part = nullptr;
     const int kSmallCap = ctx->tune[10] > 0 ? std::min(ctx->tune[10], 1024) : kSmallCapDefault;
     if (small_ok) {
-        const int np = nplanes(ctx->order), nc = ctx->order == 6 ? 10 : 7;
-        for (int k = 0; k < np; ++k) small.jp[k] = plane(ctx, k);
+        const int nc = ctx->order == 6 ? 10 : 7, rw = ctx->order == 6 ? 20 : 14;
         small.nj = b->n;
         small.eps2 = b->eps2;
         small.order = ctx->order;
-        if (int rc = dev_reserve(ctx, ctx->fixpart, (size_t)ctx->sm_count * kSmallCap * nc * sizeof(double)); rc != S2_OK) return rc;
-        small_part = (double *)ctx->fixpart.p;
+        const size_t was[3] = {b->xrows.bytes, b->xrec.bytes, b->xhdr.bytes};
+        int rc = dev_reserve(ctx, b->xrows, (size_t)ctx->sm_count * kSmallCap * nc * 2 * sizeof(unsigned long long));
+        if (rc == S2_OK) rc = dev_reserve(ctx, b->xrec, (size_t)b->n * rw * sizeof(unsigned long long));
+        if (rc == S2_OK) rc = dev_reserve(ctx, b->xhdr, (size_t)ctx->sm_count * sizeof(unsigned long long));
+        if (rc != S2_OK) return rc;
+        // sequence tags are 32 bits: long before they wrap, start again from clean buffers
+        const bool wrap = b->h_ctl->tag > 0x70000000LL;
+        if (wrap) {
+            CU(cudaMemsetAsync(&((BtsCtl *)b->misc.p)->tag, 0, sizeof(long long), ctx->stream));
+            b->h_ctl->tag = 0;
+        }
+        if (wrap || !b->x_clean || was[0] != b->xrows.bytes || was[1] != b->xrec.bytes || was[2] != b->xhdr.bytes) {
+            CU(cudaMemsetAsync(b->xrows.p, 0, b->xrows.bytes, ctx->stream));
+            CU(cudaMemsetAsync(b->xrec.p, 0, b->xrec.bytes, ctx->stream));
+            CU(cudaMemsetAsync(b->xhdr.p, 0, b->xhdr.bytes, ctx->stream));
+            b->x_clean = true;
+        }
     }
     while (done < max_block_steps && b->h_ctl->t_next <= t_end) {
         const double t_new = b->h_ctl->t_next;
@@ -420,7 +447,9 @@ extern "C" int s2_bts_run(s2_bts *b, double t_end, long long max_block_steps, in
             a.spec_cap = kSmallCap;
             a.max_steps = K;
             a.t_end = t_end;
-            a.part = small_part;
+            a.xrows = (unsigned long long *)b->xrows.p;
+            a.xrec = (unsigned long long *)b->xrec.p;
+            a.xhdr = (unsigned long long *)b->xhdr.p;
             if (time_device) CU(cudaEventRecord(b->ev[0], ctx->stream));
             const cudaError_t e = launch_bts_small_steps(small, a, bts_predict_args(b), ctx->device, ctx->sm_count, ctx->stream);
             if (e == cudaErrorNotSupported) {            // this device cannot run it: every step the ordinary way
@@ -530,6 +559,23 @@ extern "C" int s2_bts_stats(const s2_bts *b, double *time, double *t_next, int *
     if (wall_ms) *wall_ms = b->wall_ms;
     if (device_ms) *device_ms = b->device_ms;
     if (timed_steps) *timed_steps = b->timed_steps;
+    return S2_OK;
+}
+
+extern "C" int s2_bts_small_profile(s2_bts *b, int on, long long out[10])
+{
+    if (!b) return S2_EINVAL;
+    s2_ctx *ctx = b->ctx;
+    CU(cudaSetDevice(ctx->device));
+    long long *dev = (long long *)((char *)b->misc.p + 640);
+    if (out) {
+        CU(cudaMemcpyAsync(out, dev, 10 * sizeof(long long), cudaMemcpyDeviceToHost, ctx->stream));
+        CU(cudaStreamSynchronize(ctx->stream));
+    }
+    if (on < 0 || on > ctx->sm_count) return S2_EINVAL;
+    if (on) CU(cudaMemsetAsync(dev, 0, 10 * sizeof(long long), ctx->stream));
+    b->profile = on != 0;
+    b->profile_cta = on ? on - 1 : 0;
     return S2_OK;
 }
 

@@ -405,33 +405,79 @@ cudaError_t launch_fp32_fix(const ForceArgs &a, int sm_count, cudaStream_t st)
 // ---- small block steps of the integrator, many per launch (s2_bts.cu; sec 3.7) ---------------
 // In a block-step run most steps move a handful of particles (median 4-10 of 16384): three dependent launches and a host
 // synchronisation per step cost 30 us for 1 us of arithmetic.  This kernel runs such steps back to back WITHOUT leaving
-// the GPU: one CTA per SM (cooperative launch: all co-resident), three grid barriers per step,
-//   phase 1  sweep: CTA c holds the j-particles [c jc, (c+1) jc).  One lane per active particle (32 to a warp, its state
-//            in registers), the CTA's j-range cut into as many splits as there are warps to spare; every lane of a warp
-//            reads the same j (one broadcast load from L2).  The splits are added in order through shared memory and
-//            the CTA writes one partial row per active particle;                                           | barrier
-//   phase 2  combine + corrector: active particle k belongs to CTA k mod G; a warp adds one component of the G rows
-//            (lane l takes rows l, l + 32, ... in that order, then the xor-butterfly), then one thread per particle
-//            applies the Hermite corrector and the time-step rule in place (bts_correct_particle) and keeps the
-//            step-level histogram;                                                                         | barrier
-//   phase 3  next block time from the histogram, prediction of every particle to it, each CTA compacts the active
-//            particles of its own address range (ascending) and publishes their number;                   | barrier
-//            then every CTA scans the G counts, copies its segment to the global list and, if the next step is a small
-//            one as well, gathers the (ascending) list into its shared memory.
+// the GPU: one CTA of 512 threads per SM (cooperative launch: all co-resident).  CTA c OWNS the particles
+// [c pc, (c+1) pc), one per thread, and keeps their base state, their step and their predicted j-planes in shared
+// memory for the whole launch; global memory is read only where another CTA has changed it, and the predicted planes
+// go back to it once, on the way out.  One block step:
+//   exchange  every owner has published the active particles of its range for this step: a header {count} and one
+//             record {address, id, predicted state} each.  Every CTA polls the headers, scans them (the active list is
+//             ascending by owner and address) and knows n;
+//   phase 1   sweep: the records are polled into shared memory (one thread each); one lane per active particle (32 to
+//             a warp), the CTA's own j-range read from shared memory, cut into as many splits as there are warps to spare; the
+//             splits are added in order and the CTA writes one partial row per active particle;
+//   phase 2   combine + corrector: active particle k belongs to CTA k mod G, which polls the rows of all owners (a warp
+//             per component: lane l takes rows l, l + 32, ... in that order, then the xor-butterfly) while the particle's
+//             old state is already on its way from L2, then one thread per particle applies the Hermite corrector and
+//             the time-step rule (bts_correct_from), writes the new state and keeps the step-level histogram;
+//   barrier   the one grid barrier of a step: corrections and histogram are complete;
+//   phase 3   next block time from the histogram; an owner whose particle was just corrected reloads it; every owner
+//             predicts its particle to the new time (shared planes + global planes) and the owners publish the next
+//             active set.
+// Rows, records and headers are exchanged as 64-bit words {32 bits of payload, 32-bit sequence tag}: the reader polls
+// until the words carry the tag of the step, so the data is its own flag and neither side needs a fence; the barrier
+// after phase 2 keeps any CTA from running more than one exchange ahead of a reader (buffers are reused every step).
 // The loop ends at the first step with more than b.spec_cap active particles or past b.t_end, or after b.max_steps; the
-// control block, the list and the predicted j-store are then exactly what an ordinary step of s2_bts_run expects.
-// Every sum is taken in a fixed order: the run is bit-reproducible.  Pair arithmetic: PolicyF64::interact above.
+// control block, the global list, the base store and the predicted planes are then exactly what an ordinary step of
+// s2_bts_run expects.  Every sum is taken in a fixed order: the run is bit-reproducible.
+// Pair arithmetic: PolicyF64::interact above.
 constexpr int kSmallThreads = 512, kSmallWarps = kSmallThreads / 32;
-constexpr int kSmallRows = 32 * kSmallWarps;   // (particle, j-split) rows in shared memory per round of the sweep
-constexpr int kSmallCapMax = 1024;    // largest spec_cap (the list in shared memory)
-constexpr int kSmallMaxCtas = 256;    // the count scan takes one CTA per thread; rows per lane in the combine = 256 / 32
+constexpr int kSmallCapMax = 1024;    // largest spec_cap (the address list in shared memory)
+constexpr int kSmallMaxCtas = 256;    // the header scan takes one CTA per thread; rows per lane in the combine = 256 / 32
 constexpr int kSmallPer = 8;          // particles a CTA combines per round
+constexpr unsigned kSmallPolls = 1u << 22;   // a wait gives up after this many polls (seconds; a phase takes microseconds)
+
+template <int ORDER>
+struct SmallLayout {                  // dynamic shared memory of bts_small_steps_kernel
+    static constexpr int NFB = ORDER == 6 ? 20 : 14;              // base fields (+ the step as field NFB)
+    static constexpr int NPL = ORDER == 6 ? 6 : 4;                // predicted planes
+    static constexpr int NC = ORDER == 6 ? 10 : 7;                // sums per particle
+    static constexpr int NS = ORDER == 6 ? 9 : 6;                 // doubles of a predicted i-state
+    static constexpr int RW = 2 + 2 * NS;                         // words of a record: address, id, state
+    static constexpr size_t base_off = 0;
+    static constexpr size_t j_off = base_off + (size_t)(NFB + 1) * kSmallThreads * 8;
+    static constexpr size_t part_off = j_off + (size_t)NPL * kSmallThreads * 16;
+    static constexpr size_t own_off = part_off + (size_t)NC * kSmallThreads * 8;
+    static constexpr size_t list_off = own_off + (size_t)kSmallThreads * 4;
+    static constexpr size_t off_off = list_off + (size_t)kSmallCapMax * 4;
+    static constexpr int kRound = ORDER == 6 ? 256 : 512;         // active particles swept per round (their states in shared memory)
+    static constexpr size_t is_off = (off_off + (size_t)(kSmallMaxCtas + 1) * 4 + 15) & ~(size_t)15;
+    static constexpr size_t iid_off = is_off + (size_t)NS * kRound * 8;
+    static constexpr size_t bytes = iid_off + (size_t)kRound * 4;
+};
+
+__device__ __forceinline__ unsigned long long ll_word(unsigned payload, unsigned tag) { return (unsigned long long)payload | ((unsigned long long)tag << 32); }
+__device__ __forceinline__ void ll_store2(unsigned long long *p, unsigned lo, unsigned hi, unsigned tag)   // 16-byte aligned
+{
+    asm volatile("st.relaxed.gpu.global.v2.u64 [%0], {%1, %2};" ::"l"(p), "l"(ll_word(lo, tag)), "l"(ll_word(hi, tag)) : "memory");
+}
+__device__ __forceinline__ void ll_store_double(unsigned long long *p, double v, unsigned tag)
+{
+    ll_store2(p, (unsigned)__double2loint(v), (unsigned)__double2hiint(v), tag);
+}
+__device__ __forceinline__ void ll_load2(const unsigned long long *p, unsigned long long &x, unsigned long long &y)
+{
+    asm volatile("ld.relaxed.gpu.global.v2.u64 {%0, %1}, [%2];" : "=l"(x), "=l"(y) : "l"(p) : "memory");
+}
+__device__ __forceinline__ bool ll_ok(unsigned long long x, unsigned long long y, unsigned tag)
+{
+    return (unsigned)(x >> 32) == tag && (unsigned)(y >> 32) == tag;
+}
+__device__ __forceinline__ double ll_double(unsigned long long x, unsigned long long y) { return __hiloint2double((int)(unsigned)y, (int)(unsigned)x); }
 
 // Barrier over the whole (co-resident) grid.  Arrival is a release-add (this CTA's writes of the phase are visible
 // before it counts), the wait polls with relaxed loads and ends with one acquire fence (which also drops the SM's L1
 // lines: what other CTAs wrote is then read from L2).  The counter only grows during a launch (target = barriers so
-// far x CTAs).  A wait of more than 2^24 polls (seconds; a phase takes microseconds) gives up and reports it rather
-// than hanging the GPU.
+// far x CTAs).
 __device__ __forceinline__ bool grid_barrier(unsigned *bar, unsigned target, int *s_flag)
 {
     __syncthreads();
@@ -442,7 +488,7 @@ __device__ __forceinline__ bool grid_barrier(unsigned *bar, unsigned target, int
         for (;;) {
             asm volatile("ld.relaxed.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(bar) : "memory");
             if (v >= target) break;
-            if (++spins > (1u << 24)) { ok = 0; break; }
+            if (++spins > kSmallPolls) { ok = 0; break; }
         }
         asm volatile("fence.acq_rel.gpu;" ::: "memory");
         *s_flag = ok;
@@ -455,148 +501,120 @@ template <int ORDER>
 __global__ void __launch_bounds__(kSmallThreads, 1) bts_small_steps_kernel(const ForceArgs a, const BtsArgs b, const PredictArgs pa)
 {
     using P = PolicyF64<ORDER, false, false>;
-    constexpr int NC = ORDER == 6 ? 10 : 7;
-    __shared__ double s_part[NC][kSmallRows];                     // component-major: lanes write neighbouring words
-    __shared__ int s_list[kSmallCapMax];
-    __shared__ int s_off[kSmallMaxCtas + 1];
+    using L = SmallLayout<ORDER>;
+    constexpr int NC = L::NC, NFB = L::NFB, NPL = L::NPL, NS = L::NS, RW = L::RW;
+    extern __shared__ __align__(16) unsigned char s_raw[];
+    double (*s_base)[kSmallThreads] = reinterpret_cast<double (*)[kSmallThreads]>(s_raw + L::base_off);
+    double2 (*s_J)[kSmallThreads] = reinterpret_cast<double2 (*)[kSmallThreads]>(s_raw + L::j_off);
+    double (*s_part)[kSmallThreads] = reinterpret_cast<double (*)[kSmallThreads]>(s_raw + L::part_off);
+    int *s_own = reinterpret_cast<int *>(s_raw + L::own_off);     // own active particles (thread numbers), ascending
+    int *s_list = reinterpret_cast<int *>(s_raw + L::list_off);   // addresses of all active particles of the step
+    int *s_off = reinterpret_cast<int *>(s_raw + L::off_off);     // exclusive scan of the owners' counts
+    double (*s_I)[L::kRound] = reinterpret_cast<double (*)[L::kRound]>(s_raw + L::is_off);   // predicted states of a round's particles
+    int *s_Iid = reinterpret_cast<int *>(s_raw + L::iid_off);
     __shared__ int s_w[kSmallWarps];
     __shared__ unsigned s_hist[2];
-    __shared__ int s_flag;
+    __shared__ int s_flag, s_bad;
     __shared__ double s_r[kSmallPer][12];
+    __shared__ long long s_ph[9];                                 // profile (b.prof): cycles of one CTA per part of a step
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int cta = blockIdx.x, G = gridDim.x;
     const int N = b.n, cap = b.spec_cap;
-    const int jc = (N + G - 1) / G;                               // j-particles of this CTA in the sweep
-    const int jbeg = min(N, cta * jc), jend = min(N, jbeg + jc);
-    const int pc = (jc + 31) & ~31;                               // particles of this CTA in select + predict: whole warps
-    const int pbeg = (int)min((long long)N, (long long)cta * pc), pend = min(N, pbeg + pc);
+    const int pc = (((N + G - 1) / G) + 31) & ~31;                // particles per owner (<= kSmallThreads: the launcher checks)
+    const int Gj = (N + pc - 1) / pc;                             // CTAs that own particles
+    const int pbeg = min(N, cta * pc), np = min(N, pbeg + pc) - pbeg;
+    const int i_own = pbeg + tid;
+    const bool have = tid < np;
     Decomp d{};
     Dec D{};
 
     double t_cur = b.ctl->t_next, t_done = b.ctl->t_done;
-    int n = b.ctl->n_next, step = 0;
+    unsigned seq = (unsigned)b.ctl->tag + 1u;                      // tag of the step about to run
+    int step = 0, n = 0;
     unsigned target = 0;
     bool ok = true;
-    if (n <= cap)
-        for (int k = tid; k < n; k += kSmallThreads) s_list[k] = b.ilist[k];
-    __syncthreads();
+    if (tid == 0) s_bad = 0;
+    const bool prof = b.prof != nullptr && cta == b.prof_cta && tid == 0;
+    long long pc0 = 0;
+    if (prof) {
+        for (int q = 0; q < 9; ++q) s_ph[q] = 0;
+        pc0 = clock64();
+    }
+#define S2_PH(i)                     \
+    if (prof) {                      \
+        const long long c1 = clock64(); \
+        s_ph[i] += c1 - pc0;         \
+        pc0 = c1;                    \
+    }
 
-    while (n >= 1 && n <= cap && t_cur <= b.t_end && step < b.max_steps) {
-        // ---- phase 1: sweep -------------------------------------------------------------------------------------
-        const int ng = (n + 31) >> 5;                             // groups of 32 active particles
-        for (int g0 = 0; g0 < ng; g0 += kSmallWarps) {            // (one round unless n > 512)
-            const int ngr = min(kSmallWarps, ng - g0);
-            const int js = kSmallWarps / ngr;                     // j-splits of this CTA's range: every warp gets an item
-            if (warp < ngr * js) {
-                const int gl = warp / js, sp = warp - gl * js;    // neighbouring warps: same particles, next split
-                const int i = s_list[min((g0 + gl) * 32 + lane, n - 1)];   // (idle lanes recompute the last particle)
-                typename P::IState I;
-                {
-                    const double2 p0 = __ldcg(static_cast<const double2 *>(a.jp[0]) + i), p1 = __ldcg(static_cast<const double2 *>(a.jp[1]) + i);
-                    const double2 p2 = __ldcg(static_cast<const double2 *>(a.jp[2]) + i), p3 = __ldcg(static_cast<const double2 *>(a.jp[3]) + i);
-                    I.x = p0.x; I.y = p0.y; I.z = p1.x; I.vx = p2.x; I.vy = p2.y; I.vz = p3.x;
-                    I.id = __double2loint(p3.y);
-                    I.ax = I.ay = I.az = 0.0;
-                    if (ORDER == 6) {
-                        const double2 p4 = __ldcg(static_cast<const double2 *>(a.jp[4]) + i), p5 = __ldcg(static_cast<const double2 *>(a.jp[5]) + i);
-                        I.ax = p4.x; I.ay = p4.y; I.az = p5.x;
-                    }
-                    I.h2 = 0.0;
-                    I.eps2 = a.eps2;
-                }
-                typename P::Acc A;
-                A.zero();
-                const int len = (jend - jbeg + js - 1) / js;
-                const int j0 = jbeg + sp * len, j1 = min(jend, j0 + len);
-#pragma unroll 4
-                for (int j = j0; j < j1; ++j) {                   // the same j in every lane: broadcast loads
-                    typename P::JData J;
-                    J.p0 = __ldcg(static_cast<const double2 *>(a.jp[0]) + j); J.p1 = __ldcg(static_cast<const double2 *>(a.jp[1]) + j);
-                    J.p2 = __ldcg(static_cast<const double2 *>(a.jp[2]) + j); J.p3 = __ldcg(static_cast<const double2 *>(a.jp[3]) + j);
-                    if (ORDER == 6) {
-                        J.p4 = __ldcg(static_cast<const double2 *>(a.jp[4]) + j); J.p5 = __ldcg(static_cast<const double2 *>(a.jp[5]) + j);
-                    }
-                    P::template interact<1, false>(J, true, j, I, A, D, d, nullptr, 0);
-                }
-                double out[10];
-                A.to_f64(out);
-                const int row = (sp * ngr + gl) * 32 + lane;
+    // compaction of the own active particles (ascending), their records and the header, all tagged `tag`
+    auto publish = [&](bool act, const double *xp, const double *vp, const double *ap, int id, unsigned tag) -> int {
+        const unsigned bal = __ballot_sync(0xffffffffu, act);
+        if (lane == 0) s_w[warp] = __popc(bal);
+        __syncthreads();
+        int pos = __popc(bal & ((1u << lane) - 1u)), total = 0;
 #pragma unroll
-                for (int c = 0; c < NC; ++c) s_part[c][row] = out[c];
-            }
-            __syncthreads();
-            const int nk = min(ngr * 32, n - g0 * 32);            // particles of this round
-            for (int e = tid; e < nk * NC; e += kSmallThreads) {  // this CTA's row of each: the splits in order
-                const int c = e / nk, kl = e - c * nk;
-                double v = 0.0;
-                for (int sp = 0; sp < js; ++sp) v += s_part[c][sp * ngr * 32 + kl];
-                b.part[((size_t)cta * cap + g0 * 32 + kl) * NC + c] = v;
-            }
-            __syncthreads();
+        for (int w = 0; w < kSmallWarps; ++w) {
+            if (w < warp) pos += s_w[w];
+            total += s_w[w];
         }
-        if (!(ok = grid_barrier(b.bar, target += G, &s_flag))) break;
-
-        // ---- phase 2: combine + corrector ----------------------------------------------------------------------
-        const int mine = n > cta ? (n - cta + G - 1) / G : 0;     // this CTA's particles: k = cta + m G
-        for (int m0 = 0; m0 < mine; m0 += kSmallPer) {
-            const int mr = min(kSmallPer, mine - m0);
-            for (int it = warp; it < mr * NC; it += kSmallWarps) {
-                const int m = it / NC, c = it - m * NC, k = cta + (m0 + m) * G;
-                double x[kSmallMaxCtas / 32];
+        if (act) {
+            s_own[pos] = tid;
+            if (total <= cap) {                                   // (more than that here alone: the step is not a small one)
+                unsigned long long *r = b.xrec + (size_t)(pbeg + pos) * RW;
+                ll_store2(r, (unsigned)i_own, (unsigned)id, tag);
 #pragma unroll
-                for (int u = 0; u < kSmallMaxCtas / 32; ++u) {    // all loads in flight, then added in row order
-                    const int row = lane + 32 * u;
-                    x[u] = row < G ? __ldcg(b.part + ((size_t)row * cap + k) * NC + c) : 0.0;
+                for (int c = 0; c < 3; ++c) {
+                    ll_store_double(r + 2 + 2 * c, xp[c], tag);
+                    ll_store_double(r + 8 + 2 * c, vp[c], tag);
+                    if (ORDER == 6) ll_store_double(r + 14 + 2 * c, ap[c], tag);
                 }
-                double v = x[0];
-#pragma unroll
-                for (int u = 1; u < kSmallMaxCtas / 32; ++u) v += x[u];
-#pragma unroll
-                for (int q = 1; q < 32; q <<= 1) v += shfl_xor_d(v, q);
-                if (lane == 0) s_r[m][c < 7 ? c : c + 2] = v;     // record layout: acc, jerk, pot at 0..6, snap at 9..11
             }
-            __syncthreads();
-            if (tid < mr) bts_correct_particle(b, s_list[cta + (m0 + tid) * G], t_cur, s_r[tid]);
-            __syncthreads();
         }
-        if (!(ok = grid_barrier(b.bar, target += G, &s_flag))) break;
-
-        // ---- phase 3: next block time, prediction, this CTA's share of the next active list -----------------------
-        if (tid < 64) {
-            const unsigned bal = __ballot_sync(0xffffffffu, __ldcg(b.hist + tid) > 0);
-            if (lane == 0) s_hist[warp] = bal;
+        if (tid == 0) {
+            const unsigned long long h = ll_word((unsigned)total, tag);
+            asm volatile("st.relaxed.gpu.global.u64 [%0], %1;" ::"l"(b.xhdr + cta), "l"(h) : "memory");
         }
         __syncthreads();
-        const int lev = s_hist[1] ? 63 - __clz(s_hist[1]) : 31 - __clz(s_hist[0] | 1u);   // highest occupied level = smallest step
-        const double t_next = t_cur + scalbn(1.0, -lev);
-        int cnt = 0;
-        for (int base = pbeg; base < pend; base += kSmallThreads) {
-            const int i = base + tid;
-            bool act = false;
-            if (i < pend) {
-                const double x = t_next / __ldcg(b.dt + i);       // exact: dt is a power of two
-                act = x == floor(x);
-                predict_one<ORDER>(pa, i, t_next);
-            }
-            const unsigned bal = __ballot_sync(0xffffffffu, act);
-            if (lane == 0) s_w[warp] = __popc(bal);
-            __syncthreads();
-            int pos = cnt + __popc(bal & ((1u << lane) - 1u)), total = 0;
-#pragma unroll
-            for (int w = 0; w < kSmallWarps; ++w) {
-                if (w < warp) pos += s_w[w];
-                total += s_w[w];
-            }
-            if (act) b.stage[pbeg + pos] = i;
-            cnt += total;
-            __syncthreads();
-        }
-        if (tid == 0) b.bcnt[cta] = cnt;
-        if (!(ok = grid_barrier(b.bar, target += G, &s_flag))) break;
+        return total;
+    };
 
-        // ---- every CTA: scan of the G counts, own segment to the global list, the next list if it is a small one ------
+    // ---- entry: resident copies of the own particle, the own active particles of the first step ---------------------
+    int my_id = 0, cnt = 0;
+    bool act = false;
+    {
+        double xp[3] = {0, 0, 0}, vp[3] = {0, 0, 0}, ap[3] = {0, 0, 0};
+        if (have) {
+#pragma unroll
+            for (int k = 0; k < NFB; ++k) s_base[k][tid] = __ldcg(pa.f[k] + i_own);
+            s_base[NFB][tid] = __ldcg(b.dt + i_own);
+            my_id = __ldcg(pa.id + i_own);
+            double2 q[6];
+#pragma unroll
+            for (int p = 0; p < NPL; ++p) s_J[p][tid] = q[p] = __ldcg(pa.p[p] + i_own);   // (already predicted to t_cur)
+            xp[0] = q[0].x; xp[1] = q[0].y; xp[2] = q[1].x; vp[0] = q[2].x; vp[1] = q[2].y; vp[2] = q[3].x;
+            if (ORDER == 6) { ap[0] = q[4].x; ap[1] = q[4].y; ap[2] = q[5].x; }
+            const double x = t_cur / s_base[NFB][tid];            // exact: the step is a power of two
+            act = x == floor(x);
+        }
+        cnt = publish(act, xp, vp, ap, my_id, seq);
+    }
+
+    if (prof) pc0 = clock64();
+    for (;;) {
+        // ---- exchange: the owners' counts of this step -> scan, n ---------------------------------------------------
         {
-            const int c = tid < G ? __ldcg(b.bcnt + tid) : 0;
+            int c = 0;
+            if (tid < Gj) {
+                unsigned long long h = 0;
+                unsigned spins = 0;
+                for (;;) {
+                    asm volatile("ld.relaxed.gpu.global.u64 %0, [%1];" : "=l"(h) : "l"(b.xhdr + tid) : "memory");
+                    if ((unsigned)(h >> 32) == seq) break;
+                    if (++spins > kSmallPolls) { s_bad = 1; break; }
+                }
+                c = (int)(unsigned)h;
+            }
             int incl = c;
 #pragma unroll
             for (int q = 1; q < 32; q <<= 1) {
@@ -607,33 +625,193 @@ __global__ void __launch_bounds__(kSmallThreads, 1) bts_small_steps_kernel(const
             __syncthreads();
             int wb = 0;
             for (int w = 0; w < warp; ++w) wb += s_w[w];
-            if (tid < G) s_off[tid] = wb + incl - c;
-            if (tid == G - 1) s_off[G] = wb + incl;
+            if (tid < Gj) s_off[tid] = wb + incl - c;
+            if (tid == Gj - 1) s_off[Gj] = wb + incl;
             __syncthreads();
         }
-        const int n_next = s_off[G];
-        for (int k = tid; k < cnt; k += kSmallThreads) b.ilist[s_off[cta] + k] = b.stage[pbeg + k];
-        if (n_next <= cap) {
-            for (int k = tid; k < n_next; k += kSmallThreads) {
-                int lo = 0, hi = G - 1;                           // CTA of member k: last c with s_off[c] <= k
+        n = s_off[Gj];
+        if (s_bad) { ok = false; break; }
+        if (!(n >= 1 && n <= cap && t_cur <= b.t_end && step < b.max_steps)) break;
+        S2_PH(0)
+
+        // ---- phase 1: sweep -------------------------------------------------------------------------------------
+        for (int k0 = 0; k0 < n; k0 += L::kRound) {               // (one round unless n > 512 | 256)
+            const int nk = min(L::kRound, n - k0);                // particles of this round
+            // their records, one thread each (polled until they carry this step's tag) -> shared memory
+            for (int kl = tid; kl < nk; kl += kSmallThreads) {
+                const int k = k0 + kl;
+                int lo = 0, hi = Gj - 1;                          // owner of particle k: last c with s_off[c] <= k
                 while (lo < hi) {
                     const int mid = (lo + hi + 1) >> 1;
                     if (s_off[mid] <= k) lo = mid; else hi = mid - 1;
                 }
-                s_list[k] = __ldcg(b.stage + (size_t)lo * pc + (k - s_off[lo]));
+                const unsigned long long *r = b.xrec + ((size_t)lo * pc + (k - s_off[lo])) * RW;
+                unsigned long long w[RW];
+                for (unsigned spins = 0;; ++spins) {
+                    bool all = true;
+#pragma unroll
+                    for (int u = 0; u < RW / 2; ++u) {
+                        ll_load2(r + 2 * u, w[2 * u], w[2 * u + 1]);
+                        all = all && ll_ok(w[2 * u], w[2 * u + 1], seq);
+                    }
+                    if (all) break;
+                    if (spins > kSmallPolls) { s_bad = 1; break; }
+                }
+                s_list[k] = (int)(unsigned)w[0];
+                s_Iid[kl] = (int)(unsigned)w[1];
+#pragma unroll
+                for (int q = 0; q < NS; ++q) s_I[q][kl] = ll_double(w[2 + 2 * q], w[3 + 2 * q]);
             }
+            __syncthreads();
+            S2_PH(1)
+            const int ngr = (nk + 31) >> 5;                       // groups of 32 particles
+            const int js = kSmallWarps / ngr;                     // splits of the own j-range: every warp gets an item
+            // up to 32 particles: the lanes of a warp split its j as well (P2 lanes take the particles, 32 / P2 lane groups
+            // take interleaved j), so that a handful of particles is a handful of pairs per lane, not per warp
+            const int P2 = ngr > 1 ? 32 : (nk <= 1 ? 1 : 1 << (32 - __clz(nk - 1)));
+            if (warp < ngr * js) {
+                const int gl = warp / js, sp = warp - gl * js;    // neighbouring warps: same particles, next split
+                const int ls = lane / P2, sub = 32 / P2;
+                const int kl = min(gl * 32 + (lane & (P2 - 1)), nk - 1);   // (idle lanes recompute the last particle)
+                typename P::IState I;
+                I.x = s_I[0][kl]; I.y = s_I[1][kl]; I.z = s_I[2][kl]; I.vx = s_I[3][kl]; I.vy = s_I[4][kl]; I.vz = s_I[5][kl];
+                I.ax = I.ay = I.az = 0.0;
+                if (ORDER == 6) { I.ax = s_I[6][kl]; I.ay = s_I[7][kl]; I.az = s_I[8][kl]; }
+                I.id = s_Iid[kl];
+                I.h2 = 0.0;
+                I.eps2 = a.eps2;
+                typename P::Acc A;
+                A.zero();
+                const int len = (np + js - 1) / js;
+                const int j0 = sp * len, j1 = min(np, j0 + len);
+#pragma unroll 2
+                for (int jj = j0 + ls; jj < j1; jj += sub) {      // the same j in the lanes of a group: broadcast reads of shared memory
+                    typename P::JData J;
+                    J.p0 = s_J[0][jj]; J.p1 = s_J[1][jj]; J.p2 = s_J[2][jj]; J.p3 = s_J[3][jj];
+                    if (ORDER == 6) { J.p4 = s_J[4][jj]; J.p5 = s_J[5][jj]; }
+                    P::template interact<1, false>(J, true, pbeg + jj, I, A, D, d, nullptr, 0);
+                }
+                for (int m = P2; m < 32; m <<= 1) A.shfl_add(m);  // the lane groups of a particle, fixed order
+                if (ls == 0) {
+                    double out[10];
+                    A.to_f64(out);
+                    const int row = (sp * ngr + gl) * 32 + lane;
+#pragma unroll
+                    for (int c = 0; c < NC; ++c) s_part[c][row] = out[c];
+                }
+            }
+            __syncthreads();
+            S2_PH(2)
+            if (cta < Gj) {
+                for (int e = tid; e < nk * NC; e += kSmallThreads) {   // this owner's row of each: the splits in order
+                    const int c = e / nk, kl = e - c * nk;
+                    double v = 0.0;
+                    for (int sp = 0; sp < js; ++sp) v += s_part[c][sp * ngr * 32 + kl];
+                    ll_store_double(b.xrows + (((size_t)cta * cap + k0 + kl) * NC + c) * 2, v, seq);
+                }
+            }
+            __syncthreads();
         }
+
+        S2_PH(3)
+        // ---- phase 2: combine + corrector ----------------------------------------------------------------------
+        const int mine = n > cta ? (n - cta + G - 1) / G : 0;     // this CTA's particles: k = cta + m G
+        for (int m0 = 0; m0 < mine; m0 += kSmallPer) {
+            const int mr = min(kSmallPer, mine - m0);
+            BtsOld old;
+            int i_m = 0;
+            if (tid < mr) {                                       // old state: on its way while the rows are polled
+                i_m = s_list[cta + (m0 + tid) * G];
+                bts_load_old(b, i_m, old);
+            }
+            for (int it = warp; it < mr * NC; it += kSmallWarps) {
+                const int m = it / NC, c = it - m * NC, k = cta + (m0 + m) * G;
+                unsigned long long x[kSmallMaxCtas / 32], y[kSmallMaxCtas / 32];
+                for (unsigned spins = 0;; ++spins) {
+                    bool all = true;
+#pragma unroll
+                    for (int u = 0; u < kSmallMaxCtas / 32; ++u) {
+                        const int row = lane + 32 * u;
+                        if (row < Gj) {
+                            ll_load2(b.xrows + (((size_t)row * cap + k) * NC + c) * 2, x[u], y[u]);
+                            all = all && ll_ok(x[u], y[u], seq);
+                        }
+                    }
+                    if (all) break;
+                    if (spins > kSmallPolls) { s_bad = 1; break; }
+                }
+                double v = 0.0;
+#pragma unroll
+                for (int u = 0; u < kSmallMaxCtas / 32; ++u)      // added in row order
+                    if (lane + 32 * u < Gj) v += ll_double(x[u], y[u]);
+#pragma unroll
+                for (int q = 1; q < 32; q <<= 1) v += shfl_xor_d(v, q);
+                if (lane == 0) s_r[m][c < 7 ? c : c + 2] = v;     // record layout: acc, jerk, pot at 0..6, snap at 9..11
+            }
+            __syncthreads();
+            S2_PH(4)
+            if (tid < mr) bts_correct_from(b, i_m, t_cur, old, s_r[tid]);
+            __syncthreads();
+            S2_PH(5)
+        }
+        if (!(ok = grid_barrier(b.bar, target += G, &s_flag)) || s_bad) { ok = false; break; }
+        S2_PH(6)
+
+        // ---- phase 3: next block time, reload of a corrected particle, prediction, the next active set -------------------
+        if (tid < 64) {
+            const unsigned bal = __ballot_sync(0xffffffffu, __ldcg(b.hist + tid) > 0);
+            if (lane == 0) s_hist[warp] = bal;
+        }
+        if (have && act) {                                        // corrected in this step (by CTA k mod G): new state from L2
+#pragma unroll
+            for (int k = 0; k < NFB; ++k) s_base[k][tid] = __ldcg(pa.f[k] + i_own);
+            s_base[NFB][tid] = __ldcg(b.dt + i_own);
+        }
+        __syncthreads();
+        const int lev = s_hist[1] ? 63 - __clz(s_hist[1]) : 31 - __clz(s_hist[0] | 1u);   // highest occupied level = smallest step
+        const double t_next = t_cur + scalbn(1.0, -lev);
+        {
+            double xp[3] = {0, 0, 0}, vp[3] = {0, 0, 0}, ap[3] = {0, 0, 0};
+            act = false;
+            if (have) {
+                const double x = t_next / s_base[NFB][tid];       // exact: the step is a power of two
+                act = x == floor(x);
+                predict_state<ORDER>([&](int k) { return s_base[k][tid]; }, t_next, xp, vp, ap);
+                double2 q[6];
+                q[0] = make_double2(xp[0], xp[1]); q[1] = make_double2(xp[2], s_base[1][tid]);
+                q[2] = make_double2(vp[0], vp[1]); q[3] = make_double2(vp[2], __hiloint2double(0, my_id));
+                q[4] = make_double2(ap[0], ap[1]); q[5] = make_double2(ap[2], 0.0);
+#pragma unroll
+                for (int p = 0; p < NPL; ++p) s_J[p][tid] = q[p];  // (the global planes are written once, on the way out)
+            }
+            S2_PH(7)
+            cnt = publish(act, xp, vp, ap, my_id, seq + 1u);
+        }
+        S2_PH(8)
         if (cta == 0 && tid == 0) b.h_log[step] = n;
         t_done = t_cur;
         t_cur = t_next;
-        n = n_next;
         ++step;
-        __syncthreads();
+        ++seq;
     }
 
+    // what the kernel leaves behind for whoever runs the pending step: the predicted planes of the own particles and the
+    // own segment of the active list (s_off is that step's scan)
+    if (ok) {
+        if (have) {
+#pragma unroll
+            for (int p = 0; p < NPL; ++p) pa.p[p][i_own] = s_J[p][tid];
+        }
+        for (int q = tid; q < cnt; q += kSmallThreads) b.ilist[s_off[cta] + q] = pbeg + s_own[q];
+    }
+    if (prof) {
+        for (int q = 0; q < 9; ++q) b.prof[q] += s_ph[q];
+        b.prof[9] += step;
+    }
+#undef S2_PH
     if (cta == 0 && tid == 0) {
         BtsCtl c = *b.ctl;
-        c.t_next = t_cur; c.n_next = n; c.steps += step; c.t_done = t_done;
+        c.t_next = t_cur; c.n_next = n; c.steps += step; c.t_done = t_done; c.tag = (long long)seq;
         if (!ok) c.error = 1;
         *b.ctl = c;
         *b.h_ctl = c;
@@ -647,25 +825,35 @@ __global__ void __launch_bounds__(kSmallThreads, 1) bts_small_steps_kernel(const
     }
 }
 
-// Launch of the above on the whole chip; a.jp = the fp64 planes, b.spec_cap <= kSmallCapMax, b.part holds
-// sm_count * spec_cap * (7 | 10) doubles.  Returns cudaErrorNotSupported when the device cannot run it (no cooperative
-// launch, or more SMs than the count scan takes): the caller then steps the ordinary way.
+// Launch of the above on the whole chip; b.spec_cap <= kSmallCapMax; b.xrows holds sm_count * spec_cap * (7 | 10) * 2 words,
+// b.xrec n * (14 | 20) words, b.xhdr sm_count words, all zero before the first launch after s2_bts_init.  Returns
+// cudaErrorNotSupported when the device or the problem cannot run it (no cooperative launch, more SMs than the header scan
+// takes, more than 512 particles per SM): the caller then steps the ordinary way.
 cudaError_t launch_bts_small_steps(const ForceArgs &a, const BtsArgs &b, const PredictArgs &pa, int device, int sm_count, cudaStream_t st)
 {
     static int supported[64] = {};                                // per device: 0 unknown, 1 yes, -1 no
     if (device < 0 || device >= 64 || b.spec_cap < 1 || b.spec_cap > kSmallCapMax || sm_count > kSmallMaxCtas) return cudaErrorNotSupported;
+    if ((((b.n + sm_count - 1) / sm_count + 31) & ~31) > kSmallThreads) return cudaErrorNotSupported;
     const void *kern = a.order == 6 ? (const void *)bts_small_steps_kernel<6> : (const void *)bts_small_steps_kernel<4>;
+    const size_t smem = a.order == 6 ? SmallLayout<6>::bytes : SmallLayout<4>::bytes;
     if (supported[device] == 0) {
         int coop = 0, per_sm = 0;
         cudaError_t e = cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, device);
-        if (e == cudaSuccess) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, bts_small_steps_kernel<6>, kSmallThreads, 0);
-        if (e != cudaSuccess) return e;
+        if (e == cudaSuccess) e = cudaFuncSetAttribute(bts_small_steps_kernel<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SmallLayout<4>::bytes);
+        if (e == cudaSuccess) e = cudaFuncSetAttribute(bts_small_steps_kernel<6>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SmallLayout<6>::bytes);
+        if (e == cudaSuccess) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, bts_small_steps_kernel<6>, kSmallThreads, SmallLayout<6>::bytes);
+        if (e != cudaSuccess) {
+            cudaGetLastError();
+            supported[device] = -1;
+            return cudaErrorNotSupported;
+        }
         supported[device] = (coop && per_sm >= 1) ? 1 : -1;
     }
     if (supported[device] < 0) return cudaErrorNotSupported;
     void *args[3] = {(void *)&a, (void *)&b, (void *)&pa};
-    return cudaLaunchCooperativeKernel(kern, dim3(sm_count), dim3(kSmallThreads), args, 0, st);
+    return cudaLaunchCooperativeKernel(kern, dim3(sm_count), dim3(kSmallThreads), args, smem, st);
 }
+
 #endif   // S2_BANK_ONLY
 
 // ---- uniform-operand sweep (a4 at the largest n_i) ------------------------------------------------------------

@@ -130,9 +130,10 @@ constexpr int kBtsLog = 1024;        // block steps one launch of the small-step
 struct BtsCtl {                      // device control block (mirrored to pinned host memory by the kernels that change it)
     double t_next;                   // time of the block step that is about to run
     int n_next;                      // number of active particles of that step
-    int error;                       // != 0: a grid barrier of the small-step kernel timed out (state is then undefined)
-    long long steps;                 // block steps completed since s2_bts_init
-    double t_done;                   // time of the last completed block step
+    int error;                       // != 0: a wait inside the small-step kernel timed out (the state is then undefined)
+    long long steps;                 // block steps the small-step kernel has run since s2_bts_init
+    double t_done;                   // time of the last block step it completed
+    long long tag;                   // last sequence tag the small-step kernel used in its exchange buffers
 };
 
 struct BtsArgs {
@@ -156,8 +157,14 @@ struct BtsArgs {
     int spec_cap, max_steps;
     double t_end;
     int *h_log;                      // pinned, kBtsLog entries
-    double *part;                    // partial sums, [CTA][spec_cap][7 or 10]
+    // exchange buffers of that kernel, 64-bit words {32 bits of payload, 32-bit sequence tag}: a reader polls the words it
+    // needs until they carry the tag of the step, so the data is its own flag (no fence, no counter)
+    unsigned long long *xrows;       // partial sums [CTA][spec_cap][7 | 10][2 words]
+    unsigned long long *xrec;        // the active particles of the coming step, by owner: [address of first own + q][14 | 20 words]
+    unsigned long long *xhdr;        // [CTA] {number of own active particles}
     unsigned *bar;                   // bar[0] grid-barrier counter, bar[1] exit counter; both 0 between launches
+    long long *prof;                 // null, or 10 sums: SM cycles CTA prof_cta spent in each part of a step (s2b200_test.h), steps
+    int prof_cta;
 };
 
 // fp32 path, reading R-F32: what is needed to decide whether an i-particle's jerk is a strongly cancelling sum
@@ -214,5 +221,6 @@ inline size_t force_smem_bytes(int nplanes, int tile, int stages)
 }
 
 cudaError_t run_peak_fma(int kind, int iters, int sm_count, cudaStream_t st, double *fma_per_s);
+cudaError_t run_hop_latency(int ctas, int iters, unsigned long long *buf, long long *d_cycles, cudaStream_t st);
 
 }  // namespace s2

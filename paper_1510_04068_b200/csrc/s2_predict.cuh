@@ -20,29 +20,36 @@ __device__ __forceinline__ float2 split_ds(double x)
     return make_float2(hi, lo);
 }
 
-template <int ORDER>
-__device__ __forceinline__ void predict_one(const PredictArgs &a, int j, double t)
+// the Taylor series alone; f(k) returns base field k of the particle (t, m, x[3], v[3], a[3], jerk[3] [, snap[3], crackle[3]])
+template <int ORDER, class F>
+__device__ __forceinline__ void predict_state(F f, double t, double xp[3], double vp[3], double ap[3])
 {
-    const double dt = t - a.f[0][j];
-    const double m = a.f[1][j];
-    const int id = a.id[j];
+    const double dt = t - f(0);
     const double h2 = 0.5 * dt, h3 = dt * (1.0 / 3.0);
-    double xp[3], vp[3], ap[3];
 #pragma unroll
     for (int c = 0; c < 3; ++c) {
-        const double x = a.f[2 + c][j], v = a.f[5 + c][j], ac = a.f[8 + c][j], jk = a.f[11 + c][j];
+        const double x = f(2 + c), v = f(5 + c), ac = f(8 + c), jk = f(11 + c);
         if (ORDER == 4) {
             xp[c] = fma(dt, fma(h2, fma(h3, jk, ac), v), x);
             vp[c] = fma(dt, fma(h2, jk, ac), v);
             ap[c] = ac;
         } else {
-            const double s = a.f[14 + c][j], cr = a.f[17 + c][j];
+            const double s = f(14 + c), cr = f(17 + c);
             const double h4 = 0.25 * dt, h5 = 0.2 * dt;
             xp[c] = fma(dt, fma(h2, fma(h3, fma(h4, fma(h5, cr, s), jk), ac), v), x);
             vp[c] = fma(dt, fma(h2, fma(h3, fma(h4, cr, s), jk), ac), v);
             ap[c] = fma(dt, fma(h2, fma(h3, cr, s), jk), ac);
         }
     }
+}
+
+template <int ORDER>
+__device__ __forceinline__ void predict_one(const PredictArgs &a, int j, double t)
+{
+    const double m = a.f[1][j];
+    const int id = a.id[j];
+    double xp[3], vp[3], ap[3];
+    predict_state<ORDER>([&](int k) { return a.f[k][j]; }, t, xp, vp, ap);
     const double idbits = __hiloint2double(0, id);
     a.p[0][j] = make_double2(xp[0], xp[1]);
     a.p[1][j] = make_double2(xp[2], m);

@@ -196,4 +196,42 @@ cudaError_t run_peak_fma(int kind, int iters, int sm_count, cudaStream_t st, dou
     return cudaSuccess;
 }
 
+// ---- hop latency between SMs through L2 (s2_hop_latency, s2b200_test.h) --------------------------------------
+// CTA 0 stores a 64-bit word; every other CTA polls that word and answers in a word of its own (128 bytes apart);
+// CTA 0 polls all answers (one thread each): one round trip = one store fanned out to all SMs + one gather = two hops.
+// Relaxed gpu-scope loads and stores, no fences: the floor of any exchange between CTAs that live on different SMs.
+__global__ void __launch_bounds__(256) hop_kernel(unsigned long long *buf, int iters, long long *cycles)
+{
+    const int cta = blockIdx.x, G = gridDim.x, tid = threadIdx.x;
+    unsigned long long *flag = buf, *rep = buf + 16;
+    auto ld = [](const unsigned long long *p) {
+        unsigned long long v;
+        asm volatile("ld.relaxed.gpu.global.u64 %0, [%1];" : "=l"(v) : "l"(p) : "memory");
+        return v;
+    };
+    auto st = [](unsigned long long *p, unsigned long long v) { asm volatile("st.relaxed.gpu.global.u64 [%0], %1;" ::"l"(p), "l"(v) : "memory"); };
+    const long long t0 = clock64();
+    for (int i = 1; i <= iters; ++i) {
+        if (cta == 0) {
+            if (tid == 0) st(flag, (unsigned long long)i);
+            for (int c = 1 + tid; c < G; c += blockDim.x) {
+                unsigned spins = 0;
+                while (ld(rep + (size_t)c * 16) != (unsigned long long)i && ++spins < (1u << 22)) {}
+            }
+            __syncthreads();
+        } else if (tid == 0) {
+            unsigned spins = 0;
+            while (ld(flag) != (unsigned long long)i && ++spins < (1u << 22)) {}
+            st(rep + (size_t)cta * 16, (unsigned long long)i);
+        }
+    }
+    if (cta == 0 && tid == 0) *cycles = clock64() - t0;
+}
+
+cudaError_t run_hop_latency(int ctas, int iters, unsigned long long *buf, long long *d_cycles, cudaStream_t st)
+{
+    void *args[3] = {(void *)&buf, (void *)&iters, (void *)&d_cycles};
+    return cudaLaunchCooperativeKernel((const void *)hop_kernel, dim3(ctas), dim3(256), args, 0, st);
+}
+
 }  // namespace s2

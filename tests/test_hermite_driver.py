@@ -203,3 +203,55 @@ def test_small_step_kernel_reproduces_the_step_by_step_run(order):
         assert small - 2 <= ta["small"]["steps"] <= small and ha.max() == w.N
         print(f"order {order} {mode}: {ta['block_steps']} block steps, {ta['small']['steps']} in {ta['small']['launches']} launches; "
               f"wall per step {ta['wall_ms'] / ta['block_steps'] * 1e3:.1f} us, stepwise {tb['wall_ms'] / tb['block_steps'] * 1e3:.1f} us")
+
+
+@pytest.mark.gpu
+@pytest.mark.parametrize("n,cap,chunk", [(100, 0, 0), (100, 1, 3), (3000, 7, 0), (3000, 1024, 5), (1000, 33, 1)])
+def test_small_step_kernel_edges(n, cap, chunk):
+    """Corners of the small-step kernel's index arithmetic: fewer particles than SMs x 32 (most CTAs own none), a cap of one
+    particle, caps that are no multiple of 32, more than 512 active particles in the kernel (two sweep rounds), and runs cut
+    into launches of 1, 3 or 5 steps by max_block_steps.  Each must be the step-by-step run."""
+    import paper_1510_04068_b200 as s2
+    from paper_1510_04068_b200.hermite import DeviceHermite
+    w = make_config(3, N=n)
+    t_end = 0.0625
+
+    def run(stepwise):
+        d = DeviceHermite(w.mass, w.pos, w.vel, w.eps2, order=4)
+        if stepwise:
+            s2.s2_set_tuning(d.ctx, 9, 6)
+        elif cap:
+            s2.s2_set_tuning(d.ctx, 10, cap)
+        if chunk and not stepwise:
+            while d.stats()["t_next"] <= t_end:
+                assert 1 <= s2.s2_bts_run(d.bts, t_end, chunk) <= chunk
+        else:
+            d.run_until(t_end)
+        out = (d.state(), d.history(), d.stats())
+        d.close()
+        return out
+
+    (sa, ha, ta), (sb, hb, tb) = run(False), run(True)
+    assert np.array_equal(ha, hb) and np.array_equal(sa["dt"], sb["dt"]) and np.array_equal(sa["t"], sb["t"])
+    assert np.abs(sa["pos"] - sb["pos"]).max() < 1e-11 and np.abs(sa["vel"] - sb["vel"]).max() < 1e-10
+    assert ta["time"] == tb["time"] == t_end
+    lim = cap if cap else 512
+    small = int((ha <= lim).sum())
+    assert small > 0 and ta["small"]["steps"] >= small - (len(ha) // max(chunk, 1) + 2 if chunk else 2)
+    assert ta["small"]["steps"] <= small
+
+
+@pytest.mark.gpu
+def test_integrator_steps_the_ordinary_way_when_an_sm_would_own_more_than_512_particles():
+    """More than 512 particles per SM do not fit the small-step kernel's shared memory: s2_bts_run falls back to one force
+    call per step (no error, no CPU path) and still follows the block-step scheme."""
+    import torch
+    from paper_1510_04068_b200.hermite import DeviceHermite
+    sms = torch.cuda.get_device_properties(0).multi_processor_count
+    w = make_config(3, N=512 * sms + 1000)
+    d = DeviceHermite(w.mass, w.pos, w.vel, w.eps2, order=4)
+    for _ in range(12):
+        d.step()
+    st, h = d.stats(), d.history()
+    d.close()
+    assert st["small"]["steps"] == 0 and st["block_steps"] == 12 and h.min() >= 1
