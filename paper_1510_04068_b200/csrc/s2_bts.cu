@@ -452,7 +452,9 @@ extern "C" int s2_bts_run(s2_bts *b, double t_end, long long max_block_steps, in
             a.xhdr = (unsigned long long *)b->xhdr.p;
             if (time_device) CU(cudaEventRecord(b->ev[0], ctx->stream));
             const cudaError_t e = launch_bts_small_steps(small, a, bts_predict_args(b), ctx->device, ctx->sm_count, ctx->stream);
-            if (e == cudaErrorNotSupported) {            // this device cannot run it: every step the ordinary way
+            if (e == cudaErrorNotSupported || e == cudaErrorCooperativeLaunchTooLarge || e == cudaErrorLaunchOutOfResources) {
+                // this device (or the share of it this process has right now) cannot hold one CTA per SM at once:
+                // every step the ordinary way -- nothing was launched, nothing is lost
                 cudaGetLastError();
                 small_ok = false;
                 continue;

@@ -255,3 +255,36 @@ def test_integrator_steps_the_ordinary_way_when_an_sm_would_own_more_than_512_pa
     st, h = d.stats(), d.history()
     d.close()
     assert st["small"]["steps"] == 0 and st["block_steps"] == 12 and h.min() >= 1
+
+
+@pytest.mark.gpu
+def test_small_step_profile_and_hop_latency_report_plausible_cycles():
+    """The two diagnostics behind profiles/r02_blockstep.md: the per-part cycle sums of the small-step kernel count exactly
+    the steps that kernel ran, every part of a step costs something, and the sums stay put once switched off; the hop
+    microbenchmark returns a round trip of a few thousand SM cycles that does not shrink when more SMs answer."""
+    import torch
+    import paper_1510_04068_b200 as s2
+    from paper_1510_04068_b200.hermite import DeviceHermite
+    w = make_config(3, N=4096)
+    d = DeviceHermite(w.mass, w.pos, w.vel, w.eps2, order=4)
+    d.run_until(0.03125)
+    before = d.stats()["small"]["steps"]
+    s2.s2_bts_small_profile(d.bts, 1)
+    d.run_until(0.0625)
+    p = s2.s2_bts_small_profile(d.bts, 0)
+    ran = d.stats()["small"]["steps"] - before
+    assert p["steps"] == ran > 100
+    parts = [k for k in p if k != "steps"]
+    assert len(parts) == 9 and all(p[k] > 0 for k in parts)
+    per_step = sum(p[k] for k in parts) / ran
+    assert 2e3 < per_step < 2e5, per_step                       # microseconds, not nanoseconds and not milliseconds
+    d.run_until(0.09375)
+    assert s2.s2_bts_small_profile(d.bts, 0) == p                # off: nothing added
+    sms = torch.cuda.get_device_properties(0).multi_processor_count
+    with pytest.raises(s2.S2Error):
+        s2.s2_bts_small_profile(d.bts, sms + 1)
+    two, many = s2.s2_hop_latency(d.ctx, 2, 500), s2.s2_hop_latency(d.ctx, sms, 500)
+    assert 300 < two < 20000 and many > 0.8 * two, (two, many)
+    with pytest.raises(s2.S2Error):
+        s2.s2_hop_latency(d.ctx, sms + 1, 10)
+    d.close()
