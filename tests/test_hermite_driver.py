@@ -288,3 +288,28 @@ def test_small_step_profile_and_hop_latency_report_plausible_cycles():
     with pytest.raises(s2.S2Error):
         s2.s2_hop_latency(d.ctx, sms + 1, 10)
     d.close()
+
+
+@pytest.mark.gpu
+def test_sixth_order_run_reaches_the_papers_energy_error_level():
+    """PAPER.md sec 3.7 L164 quotes energy errors of about 1e-12 for its 6th-order double-precision runs (and 1e-10 in
+    double-single) without stating softening, time-step cap or start-up.  With eta6 = 0.1 averaged with eta4 = 0.01 (L152,
+    L156), dt_max = 1/64 and the default start-up factor the device integrator conserves the energy of an N = 4096 Plummer
+    sphere over one time unit to a few 1e-12 -- in fp64 and, because this library's double-single pair arithmetic keeps
+    ~48 bits (reading P11), in double-single as well.  A start-up factor ten times larger loses four orders of
+    magnitude in the very first step: the test pins the default."""
+    import paper_1510_04068_b200 as s2
+    from paper_1510_04068_b200.hermite import DeviceHermite
+    w = make_config(3, N=4096)
+    eps2 = (4.0 / w.N) ** 2
+    errs = {}
+    for name, prec, kw in (("fp64", s2.S2_FP64, {}), ("ds", s2.S2_DS, {}), ("fp64, eta_start 0.01", s2.S2_FP64, {"eta_start": 0.01})):
+        d = DeviceHermite(w.mass, w.pos, w.vel, eps2, order=6, precision=prec, averaged=True, dt_max=2.0 ** -6, **kw)
+        e0 = d.energy()
+        d.run_until(1.0)
+        errs[name] = abs((d.energy() - e0) / e0)
+        assert (d.state()["t"] == 1.0).all()
+        d.close()
+    print({k: f"{v:.2e}" for k, v in errs.items()})
+    assert errs["fp64"] < 2e-11 and errs["ds"] < 2e-11
+    assert errs["fp64, eta_start 0.01"] > 10 * errs["fp64"]
