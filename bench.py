@@ -399,12 +399,39 @@ def main():
                                         "full_cfg3_ginteractions_per_s": by[("3", "fp64", 65536)]["ginteractions_per_s"]})
         line["large_configs"] = neighbour_path(s2, torch, dev, measured_peaks().get("hbm_gbs", 6650.0))
         line["hbm_kernels"] = hbm_kernels(s2, torch, dev, measured_peaks().get("hbm_gbs", 6650.0))
+        line["blockstep"] = blockstep_summary(s2)
         line["cpu_baseline"] = cpu_baseline(w)
     if rank == 0:
         print(json.dumps(line), flush=True)
     s2.s2_close(ctx)
     if world > 1:
         dist.destroy_process_group()
+
+
+def blockstep_summary(s2, n=16384):
+    """The second workload (sec 3.7) in the default line: one N-body time unit of
+    an N = 16384 Plummer sphere with the device-resident block-step integrator, 4th and 6th order, fp64 (about 2 s of GPU
+    time).  `bench.py --blockstep N` is the full table (double-single, device time, A/B, host driver; profiles/)."""
+    from paper_1510_04068_b200.hermite import DeviceHermite
+    from workloads import make_config
+    w = make_config(3, N=n)
+    rows = []
+    for order in (4, 6):
+        d = DeviceHermite(w.mass, w.pos, w.vel, w.eps2, order=order, precision=s2.S2_FP64, averaged=order == 6)
+        e0 = d.energy()
+        t0 = time.perf_counter()
+        d.run_until(1.0)
+        wall = time.perf_counter() - t0
+        e1 = d.energy()
+        st, hist = d.stats(), d.history()
+        d.close()
+        rows.append({"order": order, "precision": "fp64", "criterion": "Aarseth eta4=0.01" if order == 4 else "mean of Aarseth(eta4=0.01) and generalised(eta6=0.1) (L156)",
+                     "block_steps": st["block_steps"], "particle_steps": st["particle_steps"], "n_i_median": float(np.median(hist)),
+                     "n_i_mean": float(hist.mean()), "wall_s": wall, "wall_us_per_block_step": wall / st["block_steps"] * 1e6,
+                     "ginteractions_per_s_wall": st["particle_steps"] * n / wall / 1e9, "dE_over_E": (e1 - e0) / e0,
+                     "steps_in_small_step_kernel": st["small"]["steps"], "small_step_kernel_launches": st["small"]["launches"]})
+    return {"workload": f"block-time-step Hermite, Plummer N={n}, eps={w.notes['eps']:.3g}, t=0..1, dt_max=1/8 (DESIGN.md reading R-BTS)",
+            "paper_context": "energy error ~1e-12 for the paper's 6th-order fp64 runs (L164); parameters not stated", "runs": rows}
 
 
 def run_blockstep(n, t_end=1.0, orders=(4, 6), precisions=("fp64", "ds"), host_reference=True, prof_cta=0):
