@@ -420,7 +420,7 @@ extern "C" int s2_bts_run(s2_bts *b, double t_end, long long max_block_steps, in
         const size_t was[3] = {b->xrows.bytes, b->xrec.bytes, b->xhdr.bytes};
         int rc = dev_reserve(ctx, b->xrows, (size_t)ctx->sm_count * kSmallCap * nc * 2 * sizeof(unsigned long long));
         if (rc == S2_OK) rc = dev_reserve(ctx, b->xrec, (size_t)b->n * rw * sizeof(unsigned long long));
-        if (rc == S2_OK) rc = dev_reserve(ctx, b->xhdr, (size_t)ctx->sm_count * sizeof(unsigned long long));
+        if (rc == S2_OK) rc = dev_reserve(ctx, b->xhdr, (size_t)ctx->sm_count * ctx->sm_count * sizeof(unsigned long long));
         if (rc != S2_OK) return rc;
         // sequence tags are 32 bits: long before they wrap, start again from clean buffers
         const bool wrap = b->h_ctl->tag > 0x70000000LL;

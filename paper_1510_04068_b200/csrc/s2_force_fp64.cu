@@ -571,9 +571,9 @@ __global__ void __launch_bounds__(kSmallThreads, 1) bts_small_steps_kernel(const
                 }
             }
         }
-        if (tid == 0) {
+        if (tid < G) {                                            // one copy per reader: no line is polled by more than one CTA
             const unsigned long long h = ll_word((unsigned)total, tag);
-            asm volatile("st.relaxed.gpu.global.u64 [%0], %1;" ::"l"(b.xhdr + cta), "l"(h) : "memory");
+            asm volatile("st.relaxed.gpu.global.u64 [%0], %1;" ::"l"(b.xhdr + (size_t)tid * G + cta), "l"(h) : "memory");
         }
         __syncthreads();
         return total;
@@ -609,7 +609,7 @@ __global__ void __launch_bounds__(kSmallThreads, 1) bts_small_steps_kernel(const
                 unsigned long long h = 0;
                 unsigned spins = 0;
                 for (;;) {
-                    asm volatile("ld.relaxed.gpu.global.u64 %0, [%1];" : "=l"(h) : "l"(b.xhdr + tid) : "memory");
+                    asm volatile("ld.relaxed.gpu.global.u64 %0, [%1];" : "=l"(h) : "l"(b.xhdr + (size_t)cta * G + tid) : "memory");
                     if ((unsigned)(h >> 32) == seq) break;
                     if (++spins > kSmallPolls) { s_bad = 1; break; }
                 }
@@ -826,7 +826,7 @@ __global__ void __launch_bounds__(kSmallThreads, 1) bts_small_steps_kernel(const
 }
 
 // Launch of the above on the whole chip; b.spec_cap <= kSmallCapMax; b.xrows holds sm_count * spec_cap * (7 | 10) * 2 words,
-// b.xrec n * (14 | 20) words, b.xhdr sm_count words, all zero before the first launch after s2_bts_init.  Returns
+// b.xrec n * (14 | 20) words, b.xhdr sm_count^2 words, all zero before the first launch after s2_bts_init.  Returns
 // cudaErrorNotSupported when the device or the problem cannot run it (no cooperative launch, more SMs than the header scan
 // takes, more than 512 particles per SM): the caller then steps the ordinary way.
 cudaError_t launch_bts_small_steps(const ForceArgs &a, const BtsArgs &b, const PredictArgs &pa, int device, int sm_count, cudaStream_t st)

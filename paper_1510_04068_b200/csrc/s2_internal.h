@@ -161,7 +161,7 @@ struct BtsArgs {
     // needs until they carry the tag of the step, so the data is its own flag (no fence, no counter)
     unsigned long long *xrows;       // partial sums [CTA][spec_cap][7 | 10][2 words]
     unsigned long long *xrec;        // the active particles of the coming step, by owner: [address of first own + q][14 | 20 words]
-    unsigned long long *xhdr;        // [CTA] {number of own active particles}
+    unsigned long long *xhdr;        // [reader CTA][owner CTA] {number of the owner's active particles}: one copy per reader
     unsigned *bar;                   // bar[0] grid-barrier counter, bar[1] exit counter; both 0 between launches
     long long *prof;                 // null, or 10 sums: SM cycles CTA prof_cta spent in each part of a step (s2b200_test.h), steps
     int prof_cta;
